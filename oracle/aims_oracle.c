@@ -1,0 +1,410 @@
+/* oracle/aims_oracle.c -- plain, slow FP64 CPU statement of the real-space grid operations of
+ * arXiv:1912.06636 (Huhn, Lange, Yu, Yoon, Blum).  Citations are /root/reference/PAPER.md line numbers.
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference legs may build, load or call it.  It shares no code, header, table or
+ * constant generator with paper_1912_06636_b200/ (the CUDA path) and neither includes the other.
+ *
+ * What it computes (the method reaches the plain definition exactly -- it only skips exact zeros -- so the
+ * oracle is the definition written out; no blocking, no fusion, no reordering beyond the batch loop the
+ * paper itself states):
+ *   O1  phi_i(r) = R_s(|r-R_a|) * Y_lm((r-R_a)/|r-R_a|), exactly 0 for |r-R_a|^2 >= rcut^2, and its gradient
+ *       (basis functions on grid points: "calculate_phi", Fig. 6 L322/L356; L314; cutoff L202).
+ *   O2  nnz(B) = functions "that are nonzero on at least part of the grid points in this batch" (L235).
+ *   O3  h_ij[B] = sum_{r in B} w(r) phi_i(r) (h phi_j)(r)   (Eq. 24, Eq. 25-27), h = sum_B h[B]
+ *       (Eq. 23), with h_KS -> local potential v(r) plus the GGA term in its integrated-by-parts form
+ *       sum_r w g.(grad phi_i phi_j + phi_i grad phi_j) (L67; Eq. 18; reading P2).
+ *       Overlap s_ij: same with v = 1, g absent (Eq. 5 "exactly analogous").
+ *   O4  n(r) = sum_ij phi_i(r) n_ij phi_j(r) (Eq. 3) restricted to nnz(B) (L235, L314 "reduction of the
+ *       density matrix ... to the dense-but-smaller n_ij"), computed as temp = n_ij phi, n = temp . phi
+ *       (Fig. 6b); grad n = 2 sum_ij grad phi_i n_ij phi_j for symmetric n_ij (L67, L93-95).
+ *
+ * Pins (tests/test_oracle_pins.py): Y_lm vs scipy and orthonormality by exact product quadrature; spline vs
+ * scipy CubicSpline; grad phi vs finite differences; Gaussian overlap closed form; S symmetric PSD;
+ * sum_p w n = Tr(D S), sum_p w v n = Tr(D H_LDA), sum_p w g.grad n = Tr(D H_GGA); batched == brute force;
+ * invariance under re-batching.  The paper prints no numerical value for this path, so no pin is "the paper's
+ * number"; all pins are mathematical.
+ *
+ * Arithmetic: IEEE double, no FMA contraction (built with -ffp-contract=off), sums in the loop order written.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+typedef struct {
+  /* basis */
+  int32_t n_atoms, n_species, n_shells, n_splines, n_knots;
+  const double *atom_xyz;           /* [n_atoms][3] */
+  const int32_t *atom_species;      /* [n_atoms] */
+  const int32_t *species_shell_ptr; /* [n_species+1] */
+  const int32_t *shell_l;           /* [n_shells] */
+  const double *shell_rcut;         /* [n_shells] */
+  const int32_t *shell_spline;      /* [n_shells] */
+  double r0, log_inc;
+  const double *spline_coef;        /* [n_splines][n_knots-1][4] */
+  /* grid */
+  int64_t n_points;
+  int32_t n_batches;
+  const double *xyz;                /* [n_points][3] */
+  const double *w;                  /* [n_points] */
+  const int64_t *batch_ptr;         /* [n_batches+1] */
+  /* atom-pair block pattern, upper blocks */
+  const int64_t *row_ptr;           /* [n_atoms+1] */
+  const int32_t *col_atom;          /* [n_blocks] */
+  const int64_t *blk_off;           /* [n_blocks] */
+  const int32_t *blk_ld;            /* [n_blocks] */
+  int64_t n_values;
+} orc_system;
+
+/* ------------------------------------------------------------------ real spherical harmonics (reading P10)
+ * S_lm: homogeneous polynomial of degree l with S_lm(u) = Y_lm(u) on the unit sphere; orthonormal real harmonics,
+ * m = -l..l, no Condon-Shortley phase.  Y[m+l]; if gS != NULL also gS[m+l][3] = grad S_lm at (x,y,z). */
+void orc_solid_harmonics(int l, const double u[3], double *Y, double (*gS)[3]) {
+  const double pi = 3.14159265358979323846;
+  double x = u[0], y = u[1], z = u[2];
+  if (l == 0) {
+    Y[0] = 0.5 * sqrt(1.0 / pi);
+    if (gS) { gS[0][0] = 0; gS[0][1] = 0; gS[0][2] = 0; }
+  } else if (l == 1) {
+    double c = sqrt(3.0 / (4.0 * pi));
+    Y[0] = c * y; Y[1] = c * z; Y[2] = c * x;
+    if (gS) {
+      gS[0][0] = 0; gS[0][1] = c; gS[0][2] = 0;
+      gS[1][0] = 0; gS[1][1] = 0; gS[1][2] = c;
+      gS[2][0] = c; gS[2][1] = 0; gS[2][2] = 0;
+    }
+  } else if (l == 2) {
+    double a = 0.5 * sqrt(15.0 / pi), b = 0.25 * sqrt(5.0 / pi), c = 0.25 * sqrt(15.0 / pi);
+    Y[0] = a * x * y;
+    Y[1] = a * y * z;
+    Y[2] = b * (2.0 * z * z - x * x - y * y);
+    Y[3] = a * x * z;
+    Y[4] = c * (x * x - y * y);
+    if (gS) {
+      gS[0][0] = a * y;        gS[0][1] = a * x;        gS[0][2] = 0;
+      gS[1][0] = 0;            gS[1][1] = a * z;        gS[1][2] = a * y;
+      gS[2][0] = -2.0 * b * x; gS[2][1] = -2.0 * b * y; gS[2][2] = 4.0 * b * z;
+      gS[3][0] = a * z;        gS[3][1] = 0;            gS[3][2] = a * x;
+      gS[4][0] = 2.0 * c * x;  gS[4][1] = -2.0 * c * y; gS[4][2] = 0;
+    }
+  } else if (l == 3) {
+    double a = 0.25 * sqrt(35.0 / (2.0 * pi)), b = 0.5 * sqrt(105.0 / pi), c = 0.25 * sqrt(21.0 / (2.0 * pi));
+    double d = 0.25 * sqrt(7.0 / pi), e = 0.25 * sqrt(105.0 / pi);
+    double x2 = x * x, y2 = y * y, z2 = z * z;
+    Y[0] = a * y * (3.0 * x2 - y2);
+    Y[1] = b * x * y * z;
+    Y[2] = c * y * (4.0 * z2 - x2 - y2);
+    Y[3] = d * z * (2.0 * z2 - 3.0 * x2 - 3.0 * y2);
+    Y[4] = c * x * (4.0 * z2 - x2 - y2);
+    Y[5] = e * z * (x2 - y2);
+    Y[6] = a * x * (x2 - 3.0 * y2);
+    if (gS) {
+      gS[0][0] = a * 6.0 * x * y;            gS[0][1] = a * (3.0 * x2 - 3.0 * y2);      gS[0][2] = 0;
+      gS[1][0] = b * y * z;                  gS[1][1] = b * x * z;                      gS[1][2] = b * x * y;
+      gS[2][0] = c * (-2.0 * x * y);         gS[2][1] = c * (4.0 * z2 - x2 - 3.0 * y2); gS[2][2] = c * 8.0 * y * z;
+      gS[3][0] = d * (-6.0 * x * z);         gS[3][1] = d * (-6.0 * y * z);             gS[3][2] = d * (6.0 * z2 - 3.0 * x2 - 3.0 * y2);
+      gS[4][0] = c * (4.0 * z2 - 3.0 * x2 - y2); gS[4][1] = c * (-2.0 * x * y);         gS[4][2] = c * 8.0 * x * z;
+      gS[5][0] = e * 2.0 * x * z;            gS[5][1] = e * (-2.0 * y * z);             gS[5][2] = e * (x2 - y2);
+      gS[6][0] = a * (3.0 * x2 - 3.0 * y2);  gS[6][1] = a * (-6.0 * x * y);             gS[6][2] = 0;
+    }
+  }
+}
+
+/* ------------------------------------------------------------------ radial function (readings P8, P11)
+ * R is *defined* as the tabulated cubic spline in the log-index coordinate:
+ *   t = ln(max(d,r0)/r0)/log_inc, k = min(floor(t), n_knots-2), x = t-k, R = a + x(b + x(c + x d)),
+ *   dR/dd = (b + 2 c x + 3 d x^2) / (log_inc * max(d,r0)). */
+void orc_radial(const orc_system *S, int spline, double d, double *R, double *dR) {
+  double dd = d > S->r0 ? d : S->r0;
+  double t = log(dd / S->r0) / S->log_inc;
+  int k = (int)floor(t);
+  if (k > S->n_knots - 2) k = S->n_knots - 2;
+  if (k < 0) k = 0;
+  double x = t - (double)k;
+  const double *c = S->spline_coef + ((size_t)spline * (size_t)(S->n_knots - 1) + (size_t)k) * 4;
+  *R = c[0] + x * (c[1] + x * (c[2] + x * c[3]));
+  *dR = (c[1] + x * (2.0 * c[2] + x * 3.0 * c[3])) / (S->log_inc * dd);
+}
+
+/* squared distance in the pinned operation order of reading P6: ((dx*dx + dy*dy) + dz*dz), separate roundings */
+static double dist2(const double *r, const double *Ra, double dv[3]) {
+  dv[0] = r[0] - Ra[0]; dv[1] = r[1] - Ra[1]; dv[2] = r[2] - Ra[2];
+  double xx = dv[0] * dv[0], yy = dv[1] * dv[1], zz = dv[2] * dv[2];
+  double s = xx + yy;
+  return s + zz;
+}
+
+/* O1: all 2l+1 functions of (atom, shell) at point r: phi[m+l], and if grad != NULL grad[m+l][3].
+ * grad phi = (R' - l R/d) Y u + (R/d) grad S_lm(u)   (phi = R(d) S_lm(dvec)/d^l). */
+void orc_shell_at_point(const orc_system *S, int atom, int shell, const double r[3], double *phi, double (*grad)[3]) {
+  int l = S->shell_l[shell];
+  double rc = S->shell_rcut[shell];
+  double rc2 = rc * rc;
+  double dv[3];
+  double d2 = dist2(r, S->atom_xyz + 3 * atom, dv);
+  if (!(d2 < rc2)) {
+    for (int m = 0; m < 2 * l + 1; m++) {
+      phi[m] = 0.0;
+      if (grad) { grad[m][0] = 0.0; grad[m][1] = 0.0; grad[m][2] = 0.0; }
+    }
+    return;
+  }
+  double d = sqrt(d2);
+  double u[3] = {0.0, 0.0, 1.0};                       /* d == 0: direction undefined, take z (P11) */
+  if (d > 0.0) { u[0] = dv[0] / d; u[1] = dv[1] / d; u[2] = dv[2] / d; }
+  double dd = d > S->r0 ? d : S->r0;
+  double R, dR, Y[7], gS[7][3];
+  orc_radial(S, S->shell_spline[shell], d, &R, &dR);
+  orc_solid_harmonics(l, u, Y, grad ? gS : NULL);
+  for (int m = 0; m < 2 * l + 1; m++) {
+    phi[m] = R * Y[m];
+    if (grad) {
+      double f = (dR - (double)l * R / dd) * Y[m];
+      for (int c = 0; c < 3; c++) grad[m][c] = f * u[c] + (R / dd) * gS[m][c];
+    }
+  }
+}
+
+/* ------------------------------------------------------------------ global basis index (reading P7)
+ * atom-major, then the species' shells in order, then m = -l..l. */
+static int atom_n_fn(const orc_system *S, int a) {
+  int sp = S->atom_species[a], n = 0;
+  for (int s = S->species_shell_ptr[sp]; s < S->species_shell_ptr[sp + 1]; s++) n += 2 * S->shell_l[s] + 1;
+  return n;
+}
+/* atom_fn_ptr[n_atoms+1] */
+void orc_atom_fn_ptr(const orc_system *S, int64_t *ptr) {
+  ptr[0] = 0;
+  for (int a = 0; a < S->n_atoms; a++) ptr[a + 1] = ptr[a] + atom_n_fn(S, a);
+}
+/* offset of block (A,B), A <= B, in the value array and its leading dimension; -1 if the pair is not in the pattern */
+static int64_t find_block(const orc_system *S, int A, int B, int *ld) {
+  for (int64_t q = S->row_ptr[A]; q < S->row_ptr[A + 1]; q++)
+    if (S->col_atom[q] == B) { *ld = S->blk_ld[q]; return S->blk_off[q]; }
+  return -1;
+}
+
+/* ------------------------------------------------------------------ O2: nnz(B) (L235; reading P6)
+ * Function i = (a, s, m) is in nnz(B) iff some point p of B has d2(p,a) < rcut_s^2 (strict); decided per shell.
+ * fn_index (capacity: total number of functions) receives the ascending global indices; fn_atom / fn_shell / fn_m
+ * (optional, same capacity) the decomposition of each listed function.  Returns |nnz(B)|. */
+int orc_batch_nnz(const orc_system *S, int b, int32_t *fn_index, int32_t *fn_atom, int32_t *fn_shell, int32_t *fn_m) {
+  int n = 0;
+  int64_t g = 0; /* global index of the first function of the current shell */
+  for (int a = 0; a < S->n_atoms; a++) {
+    int sp = S->atom_species[a];
+    for (int s = S->species_shell_ptr[sp]; s < S->species_shell_ptr[sp + 1]; s++) {
+      int l = S->shell_l[s];
+      double rc2 = S->shell_rcut[s] * S->shell_rcut[s];
+      int touches = 0;
+      for (int64_t p = S->batch_ptr[b]; p < S->batch_ptr[b + 1] && !touches; p++) {
+        double dv[3];
+        if (dist2(S->xyz + 3 * p, S->atom_xyz + 3 * a, dv) < rc2) touches = 1;
+      }
+      if (touches)
+        for (int m = -l; m <= l; m++) {
+          fn_index[n] = (int32_t)(g + m + l);
+          if (fn_atom) fn_atom[n] = a;
+          if (fn_shell) fn_shell[n] = s;
+          if (fn_m) fn_m[n] = m;
+          n++;
+        }
+      g += 2 * l + 1;
+    }
+  }
+  return n;
+}
+
+/* ------------------------------------------------------------------ O1 on a batch ("calculate_phi", L322/L356)
+ * phi[i][p] for i in nnz(B) (row-major, n_p = batch size), dphi[c][i][p] if want_grad.  nnz lists as returned by
+ * orc_batch_nnz. */
+void orc_eval_basis(const orc_system *S, int b, int want_grad, int nnz, const int32_t *fn_atom, const int32_t *fn_shell,
+                    const int32_t *fn_m, double *phi, double *dphi) {
+  int64_t p0 = S->batch_ptr[b];
+  int np = (int)(S->batch_ptr[b + 1] - p0);
+  for (int i = 0; i < nnz;) {                         /* the list holds whole shells: rows i .. i+2l of one (atom, shell) */
+    int l = S->shell_l[fn_shell[i]];
+    for (int p = 0; p < np; p++) {
+      double val[7], gr[7][3];
+      orc_shell_at_point(S, fn_atom[i], fn_shell[i], S->xyz + 3 * (p0 + p), val, want_grad ? gr : NULL);
+      for (int m = 0; m < 2 * l + 1; m++) {
+        phi[(size_t)(i + m) * np + p] = val[m];
+        if (want_grad)
+          for (int c = 0; c < 3; c++) dphi[((size_t)c * nnz + i + m) * np + p] = gr[m][c];
+      }
+    }
+    i += 2 * l + 1;
+  }
+  (void)fn_m;
+}
+
+/* ------------------------------------------------------------------ O3: Hamiltonian / overlap integration
+ * For every listed batch B: h_ij[B] = sum_{p in B} w_p phi_i v_p phi_j                     (Eq. 24-27)
+ *                                   + sum_{p in B} w_p [ (g_p.grad phi_i) phi_j + phi_i (g_p.grad phi_j) ]   (P2)
+ * for i, j in nnz(B); added into H_values (Eq. 23; "insert_into_h", L327) for atom pairs in the upper pattern
+ * (diagonal atom blocks hold the full square).  g == NULL: LDA.  H_values is accumulated into (caller zeroes). */
+void orc_integrate_hamiltonian(const orc_system *S, int n_sel, const int32_t *batches, const double *v, const double *g,
+                               double *H_values) {
+  int64_t *afp = (int64_t *)malloc(sizeof(int64_t) * (S->n_atoms + 1));
+  orc_atom_fn_ptr(S, afp);
+  int nf_tot = (int)afp[S->n_atoms];
+  int32_t *idx = (int32_t *)malloc(sizeof(int32_t) * 4 * (size_t)nf_tot);
+  int32_t *fa = idx + nf_tot, *fs = fa + nf_tot, *fm = fs + nf_tot;
+  for (int q = 0; q < n_sel; q++) {
+    int b = batches[q];
+    int64_t p0 = S->batch_ptr[b];
+    int np = (int)(S->batch_ptr[b + 1] - p0);
+    int nnz = orc_batch_nnz(S, b, idx, fa, fs, fm);
+    if (nnz == 0 || np == 0) continue;
+    double *phi = (double *)malloc(sizeof(double) * (size_t)nnz * np * (g ? 4 : 1));
+    double *dphi = g ? phi + (size_t)nnz * np : NULL;
+    orc_eval_basis(S, b, g != NULL, nnz, fa, fs, fm, phi, dphi);
+    /* G_ip = g_p . grad phi_i(r_p) */
+    double *G = NULL;
+    if (g) {
+      G = (double *)malloc(sizeof(double) * (size_t)nnz * np);
+      for (int i = 0; i < nnz; i++)
+        for (int p = 0; p < np; p++) {
+          double s = 0.0;
+          for (int c = 0; c < 3; c++) s += g[(size_t)c * S->n_points + p0 + p] * dphi[((size_t)c * nnz + i) * np + p];
+          G[(size_t)i * np + p] = s;
+        }
+    }
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int i = 0; i < nnz; i++) {
+      int A = fa[i];
+      int ai = (int)(idx[i] - afp[A]);
+      for (int j = 0; j < nnz; j++) {
+        int B = fa[j];
+        if (B < A) continue;                         /* lower atom blocks are not stored */
+        int ld;
+        int64_t off = find_block(S, A, B, &ld);
+        if (off < 0) continue;                       /* pair outside the pattern: the product is identically zero */
+        int bj = (int)(idx[j] - afp[B]);
+        double h = 0.0;
+        for (int p = 0; p < np; p++) {
+          double wp = S->w[p0 + p];
+          double pi_ = phi[(size_t)i * np + p], pj = phi[(size_t)j * np + p];
+          double term = wp * pi_ * v[p0 + p] * pj;
+          if (g) term += wp * (G[(size_t)i * np + p] * pj + pi_ * G[(size_t)j * np + p]);
+          h += term;
+        }
+        H_values[off + (int64_t)ai * ld + bj] += h;
+      }
+    }
+    free(G);
+    free(phi);
+  }
+  free(idx);
+  free(afp);
+}
+
+/* ------------------------------------------------------------------ O4: density update
+ * For every listed batch B and p in B: n_p = sum_i phi_ip temp_ip, temp_ip = sum_j n_ij[B] phi_jp  (Fig. 6b),
+ * n_ij[B] = D restricted to nnz(B) ("calculate_density_mat", L314/L357; zero outside the pattern);
+ * grad_n[c][p] = 2 sum_i dphi[c]_ip temp_ip (D symmetric).  Only points of the listed batches are written. */
+void orc_update_density(const orc_system *S, int n_sel, const int32_t *batches, const double *D_values, double *n,
+                        double *grad_n) {
+  int64_t *afp = (int64_t *)malloc(sizeof(int64_t) * (S->n_atoms + 1));
+  orc_atom_fn_ptr(S, afp);
+  int nf_tot = (int)afp[S->n_atoms];
+  int32_t *idx = (int32_t *)malloc(sizeof(int32_t) * 4 * (size_t)nf_tot);
+  int32_t *fa = idx + nf_tot, *fs = fa + nf_tot, *fm = fs + nf_tot;
+  for (int q = 0; q < n_sel; q++) {
+    int b = batches[q];
+    int64_t p0 = S->batch_ptr[b];
+    int np = (int)(S->batch_ptr[b + 1] - p0);
+    int nnz = orc_batch_nnz(S, b, idx, fa, fs, fm);
+    if (np == 0) continue;
+    double *phi = (double *)malloc(sizeof(double) * ((size_t)nnz * np * (grad_n ? 4 : 1) + 1));
+    double *dphi = grad_n ? phi + (size_t)nnz * np : NULL;
+    orc_eval_basis(S, b, grad_n != NULL, nnz, fa, fs, fm, phi, dphi);
+    /* calculate_density_mat: dense D_b[i][j] */
+    double *Db = (double *)malloc(sizeof(double) * ((size_t)nnz * nnz + 1));
+    for (int i = 0; i < nnz; i++)
+      for (int j = 0; j < nnz; j++) {
+        int A = fa[i], B = fa[j];
+        int ai = (int)(idx[i] - afp[A]), bj = (int)(idx[j] - afp[B]);
+        int ld;
+        double val = 0.0;
+        if (A <= B) { int64_t off = find_block(S, A, B, &ld); if (off >= 0) val = D_values[off + (int64_t)ai * ld + bj]; }
+        else        { int64_t off = find_block(S, B, A, &ld); if (off >= 0) val = D_values[off + (int64_t)bj * ld + ai]; }
+        Db[(size_t)i * nnz + j] = val;
+      }
+#pragma omp parallel for schedule(static)
+    for (int p = 0; p < np; p++) {
+      double acc = 0.0, gacc[3] = {0.0, 0.0, 0.0};
+      for (int i = 0; i < nnz; i++) {
+        double t = 0.0;
+        for (int j = 0; j < nnz; j++) t += Db[(size_t)i * nnz + j] * phi[(size_t)j * np + p];
+        acc += phi[(size_t)i * np + p] * t;
+        if (grad_n)
+          for (int c = 0; c < 3; c++) gacc[c] += dphi[((size_t)c * nnz + i) * np + p] * t;
+      }
+      n[p0 + p] = acc;
+      if (grad_n)
+        for (int c = 0; c < 3; c++) grad_n[(size_t)c * S->n_points + p0 + p] = 2.0 * gacc[c];
+    }
+    free(Db);
+    free(phi);
+  }
+  free(idx);
+  free(afp);
+}
+
+/* ------------------------------------------------------------------ brute force (tiny inputs only)
+ * No batches, no culling, no block pattern: every function against every function at every point.
+ *   Hd[i][j] = sum_p w_p phi_i v_p phi_j + sum_p w_p [(g.grad phi_i) phi_j + phi_i (g.grad phi_j)]   (Eq. 21)
+ *   n_p = sum_ij phi_i Dd[i][j] phi_j ,  grad n_p = sum_ij (grad phi_i phi_j + phi_i grad phi_j) Dd[i][j] (Eq. 3)
+ * Hd, Dd: dense [n_basis][n_basis].  grad n is written from the product rule, not from the "2 x" shortcut. */
+void orc_brute(const orc_system *S, const double *v, const double *g, double *Hd, const double *Dd, double *n,
+               double *grad_n) {
+  int64_t *afp = (int64_t *)malloc(sizeof(int64_t) * (S->n_atoms + 1));
+  orc_atom_fn_ptr(S, afp);
+  int nb = (int)afp[S->n_atoms];
+  double *phi = (double *)malloc(sizeof(double) * (size_t)nb * 4);
+  double *dph = phi + nb;                              /* dph[c*nb + i] */
+  if (Hd) memset(Hd, 0, sizeof(double) * (size_t)nb * nb);
+  for (int64_t p = 0; p < S->n_points; p++) {
+    int i = 0;
+    for (int a = 0; a < S->n_atoms; a++) {
+      int sp = S->atom_species[a];
+      for (int s = S->species_shell_ptr[sp]; s < S->species_shell_ptr[sp + 1]; s++) {
+        int l = S->shell_l[s];
+        double val[7], gr[7][3];
+        orc_shell_at_point(S, a, s, S->xyz + 3 * p, val, gr);
+        for (int m = 0; m < 2 * l + 1; m++, i++) {
+          phi[i] = val[m];
+          for (int c = 0; c < 3; c++) dph[c * nb + i] = gr[m][c];
+        }
+      }
+    }
+    if (Hd) {
+      double wp = S->w[p];
+      for (int a = 0; a < nb; a++)
+        for (int b = 0; b < nb; b++) {
+          double t = wp * phi[a] * v[p] * phi[b];
+          if (g)
+            for (int c = 0; c < 3; c++)
+              t += wp * g[(size_t)c * S->n_points + p] * (dph[c * nb + a] * phi[b] + phi[a] * dph[c * nb + b]);
+          Hd[(size_t)a * nb + b] += t;
+        }
+    }
+    if (Dd && n) {
+      double acc = 0.0, ga[3] = {0, 0, 0};
+      for (int a = 0; a < nb; a++)
+        for (int b = 0; b < nb; b++) {
+          double dab = Dd[(size_t)a * nb + b];
+          acc += phi[a] * dab * phi[b];
+          if (grad_n)
+            for (int c = 0; c < 3; c++) ga[c] += (dph[c * nb + a] * phi[b] + phi[a] * dph[c * nb + b]) * dab;
+        }
+      n[p] = acc;
+      if (grad_n)
+        for (int c = 0; c < 3; c++) grad_n[(size_t)c * S->n_points + p] = ga[c];
+    }
+  }
+  free(phi);
+  free(afp);
+}
