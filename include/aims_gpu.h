@@ -1,0 +1,148 @@
+/* aims_gpu.h -- C ABI of the B200-native real-space grid operations of arXiv:1912.06636
+ * (Huhn, Lange, Yu, Yoon, Blum: "GPGPU acceleration of all-electron electronic structure theory using localized
+ * numeric atom-centered basis functions").  Citations: PAPER.md L<line> = /root/reference/PAPER.md.
+ *
+ * The three hot calls follow the paper's statement of the problem (Fig. 6):
+ *   aims_gpu_eval_basis             "calculate_phi" on the reduced subspace nnz(B) of every batch   (L235, L314, L322)
+ *   aims_gpu_integrate_hamiltonian  h_ij = sum_B sum_{r in B} w(r) phi_i(r) (h phi_j)(r)             (Eq. 23-27)
+ *   aims_gpu_update_density         n(r) = sum_ij phi_i(r) n_ij phi_j(r) and grad n                  (Eq. 3)
+ * Every step runs in hand-written sm_100a kernels; there is no CPU fallback and no other backend.
+ *
+ * Conventions
+ *  - All functions return AIMS_OK (0) or a negative aims_status; they never throw, exit or print.
+ *  - HOST pointers are read during the call that receives them and may be freed afterwards.
+ *    DEVICE pointers must be valid on the context's device, 16-byte aligned, and are owned by the caller.
+ *  - Work is enqueued on the stream given at creation.  Outputs are valid once the caller has synchronised that
+ *    stream.  Errors detectable at enqueue time are returned; an asynchronous CUDA fault surfaces at the next
+ *    call or at destroy (AIMS_ERR_CUDA, text in aims_gpu_last_error).
+ *  - Global basis index: atom-major, then the species' shells in order, then m = -l..l.
+ *  - Lengths are in Angstrom; nothing converts units.
+ *  - One context per host thread; a context is not thread-safe.
+ */
+#ifndef AIMS_GPU_H
+#define AIMS_GPU_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  AIMS_OK = 0,
+  AIMS_ERR_INVALID_ARG = -1, /* NULL where not allowed, inconsistent sizes, batch range outside [0, n_batches] */
+  AIMS_ERR_CUDA = -2,        /* a CUDA runtime call failed; see aims_gpu_last_error */
+  AIMS_ERR_NOMEM = -3,       /* device workspace could not be allocated */
+  AIMS_ERR_UNSUPPORTED = -4  /* l > 3, > 32 shells per species, > AIMS_MAX_ACTIVE_ATOMS atoms touching one batch, ... */
+} aims_status;
+
+#define AIMS_MAX_L 3
+#define AIMS_MAX_SHELLS_PER_SPECIES 32
+#define AIMS_MAX_ACTIVE_ATOMS 96 /* atoms whose cutoff sphere reaches one batch */
+
+/* Basis: numeric atom-centred functions phi = R_s(d) Y_lm(u) (readings P8-P11).
+ * R_s is DEFINED by the spline table: t = ln(max(d,r0)/r0)/log_inc, k = min(floor t, n_knots-2), x = t-k,
+ * R = a + x(b + x(c + x d)); phi is exactly 0 where |r-R_a|^2 >= rcut^2.  HOST pointers. */
+typedef struct {
+  int32_t n_atoms, n_species, n_shells, n_splines, n_knots;
+  const double *atom_xyz;           /* [n_atoms][3] */
+  const int32_t *atom_species;      /* [n_atoms], 0..n_species-1 */
+  const int32_t *species_shell_ptr; /* [n_species+1]: shells species_shell_ptr[s] .. species_shell_ptr[s+1]-1 */
+  const int32_t *shell_l;           /* [n_shells], 0..AIMS_MAX_L */
+  const double *shell_rcut;         /* [n_shells] */
+  const int32_t *shell_spline;      /* [n_shells], index into spline_coef */
+  double r0, log_inc;               /* knots r_k = r0 exp(log_inc k), k = 0..n_knots-1 */
+  const double *spline_coef;        /* [n_splines][n_knots-1][4] = (a,b,c,d) per interval */
+} aims_basis_desc;
+
+/* Integration grid cut into spatially compact batches.  The points of batch b are
+ * xyz[batch_ptr[b] .. batch_ptr[b+1]); the library never re-batches.  HOST pointers. */
+typedef struct {
+  int64_t n_points;
+  int32_t n_batches;
+  int32_t max_batch_points;         /* >= every batch size */
+  const double *xyz;                /* [n_points][3] */
+  const double *w;                  /* [n_points] integration weight w(r) of Eq. 21 */
+  const int64_t *batch_ptr;         /* [n_batches+1], ascending, batch_ptr[0] = 0 */
+} aims_grid_desc;
+
+/* Atom-pair block-sparse layout of H, S and D (replaces the paper's "locally-indexed dense" storage, L291-297;
+ * SURVEY.md reading P13).  Only blocks with col_atom >= row atom are stored; block q of row A is row-major
+ * [n_fn(A)][blk_ld[q]] at values[blk_off[q]]; diagonal blocks (A,A) hold the full square.  Pairs absent from
+ * the pattern are treated as exactly zero.  blk_off and blk_ld must be even (16-byte rows).  HOST pointers. */
+typedef struct {
+  int32_t n_block_rows;             /* == n_atoms */
+  const int64_t *row_ptr;           /* [n_atoms+1] */
+  const int32_t *col_atom;          /* [n_blocks], ascending within a row */
+  const int64_t *blk_off;           /* [n_blocks] */
+  const int32_t *blk_ld;            /* [n_blocks], >= n_fn(col_atom) */
+  int64_t n_values;
+} aims_bsr_desc;
+
+typedef struct aims_gpu_ctx aims_gpu_ctx;
+
+/* Create a context on `device` (cudaSetDevice ordinal) that enqueues on `cuda_stream` (a cudaStream_t, e.g.
+ * torch.cuda.current_stream().cuda_stream; NULL = legacy default stream).  Copies the three descriptions to the
+ * device, runs the culling once to size every per-batch list, and allocates workspaces (at most
+ * workspace_bytes for the per-chunk Phi planes; 0 = default 24 GiB, clamped to free memory).
+ * Synchronises the stream before returning. */
+int aims_gpu_create(aims_gpu_ctx **out, const aims_basis_desc *basis, const aims_grid_desc *grid,
+                    const aims_bsr_desc *bsr, int device, void *cuda_stream, int64_t workspace_bytes);
+int aims_gpu_destroy(aims_gpu_ctx *ctx);
+/* Text of the last error on this context (ctx-owned, valid until the next call); "" if none. ctx may be NULL. */
+const char *aims_gpu_last_error(const aims_gpu_ctx *ctx);
+
+/* Sizes of the outputs of aims_gpu_eval_basis for batches [b0,b1): n_index = sum nnz(B), n_phi = sum nnz(B)*|B|.
+ * HOST outputs. */
+int aims_gpu_basis_sizes(aims_gpu_ctx *ctx, int32_t b0, int32_t b1, int64_t *n_index, int64_t *n_phi);
+
+/* Step 1 (S1a+S1b).  For each batch b in [b0,b1): the ascending list of global indices of nnz(B_b) (
+ * i in nnz(B) iff some point p of B has ((dx*dx+dy*dy)+dz*dz) < rcut*rcut, decided per shell in separately rounded
+ * IEEE operations, reading P6), and phi (and grad phi if dphi != NULL) of those functions at the batch's points.
+ * DEVICE outputs, caller-sized with aims_gpu_basis_sizes:
+ *   fn_ptr  [b1-b0+1]  fn_index[fn_ptr[k] .. fn_ptr[k+1]) belongs to batch b0+k
+ *   fn_index[n_index]
+ *   phi_ptr [b1-b0+1]  phi[phi_ptr[k] + i*n_p + p], i < nnz, p < n_p = |B| (point index fastest)
+ *   phi     [n_phi]
+ *   dphi    NULL or [3*n_phi]: d phi/d x_c at dphi[3*phi_ptr[k] + (c*nnz + i)*n_p + p] */
+int aims_gpu_eval_basis(aims_gpu_ctx *ctx, int32_t b0, int32_t b1, int64_t *fn_ptr, int32_t *fn_index,
+                        int64_t *phi_ptr, double *phi, double *dphi);
+
+/* Step 2 (S2a-S2d).  H_values (+)= sum over batches [b0,b1) of
+ *     sum_p w_p phi_i(r_p) v_p phi_j(r_p)  +  [g != NULL]  sum_p w_p g_p . (grad phi_i phi_j + phi_i grad phi_j)(r_p)
+ * for i,j in nnz(B), scattered into the block pattern (Eq. 23-27; GGA term in the integrated-by-parts form, L67 and
+ * Eq. 18, reading P2).  Overlap matrix: pass v = 1.  DEVICE pointers:
+ *   v [n_points], g NULL or [3][n_points] (component-major), H_values [n_values].
+ * accumulate == 0: H_values is zeroed first; != 0: added to (Eq. 28-29 partial sums). */
+int aims_gpu_integrate_hamiltonian(aims_gpu_ctx *ctx, int32_t b0, int32_t b1, const double *v, const double *g,
+                                   double *H_values, int accumulate);
+
+/* Step 3 (S3a-S3d).  For every point p of batches [b0,b1):  n[p] = sum_ij phi_i D_ij phi_j,
+ * grad_n[c][p] = 2 sum_ij d_c phi_i D_ij phi_j (D symmetric), i,j in nnz(B) (Eq. 3; Fig. 6b).
+ * DEVICE pointers: D_values [n_values] in the pattern of aims_bsr_desc (upper blocks; the symmetric full matrix is
+ * implied), n [n_points], grad_n NULL or [3][n_points].  Points of other batches are not touched. */
+int aims_gpu_update_density(aims_gpu_ctx *ctx, int32_t b0, int32_t b1, const double *D_values, double *n,
+                            double *grad_n);
+
+/* Synchronise the context stream and report anything the device flagged since the last check: an asynchronous CUDA
+ * fault (AIMS_ERR_CUDA) or a failed device-side capacity / consistency check (AIMS_ERR_UNSUPPORTED). */
+int aims_gpu_synchronize(aims_gpu_ctx *ctx);
+
+/* Static structure found at creation (HOST outputs, any may be NULL): sum and max over all batches of |nnz(B)|,
+ * max number of active atoms, algorithmic flops of one full H pass (GGA: 2*sum n_p nnz^2; LDA: sum n_p nnz (nnz+1))
+ * and of one density pass (2*sum n_p nnz^2). */
+int aims_gpu_stats(aims_gpu_ctx *ctx, int64_t *sum_nnz, int32_t *max_nnz, int32_t *max_active_atoms,
+                   double *flops_h_lda, double *flops_h_gga, double *flops_density);
+
+/* Number of kernels this context has launched since creation (for bench.py's gpu_launches). */
+int64_t aims_gpu_launch_count(const aims_gpu_ctx *ctx);
+
+/* FP64 tensor-pipe (DMMA.8x8x4) peak probe: runs a dependency-free mma.sync.m8n8k4.f64 chain on every SM for about
+ * `ms_target` milliseconds on the context stream and returns the achieved TFLOP/s in *tflops (HOST output).
+ * Used by bench.py as the measured FP64 roofline denominator. */
+int aims_gpu_fp64_peak(aims_gpu_ctx *ctx, double ms_target, double *tflops);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AIMS_GPU_H */

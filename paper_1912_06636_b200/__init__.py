@@ -1,0 +1,7 @@
+"""paper_1912_06636_b200 -- B200-native (sm_100a) real-space grid operations of arXiv:1912.06636.
+
+The product is the C-ABI library libaims_gpu.so (include/aims_gpu.h, csrc/); this package is the thin Python
+binding over it (argument marshalling only).  There is no CPU fallback: a missing library raises.
+"""
+from .binding import (AimsError, Context, aims_gpu_create, aims_gpu_destroy, aims_gpu_eval_basis,  # noqa: F401
+                      aims_gpu_integrate_hamiltonian, aims_gpu_update_density, exported_symbols, load_library)

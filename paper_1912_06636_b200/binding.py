@@ -1,0 +1,285 @@
+"""ctypes binding of libaims_gpu.so (include/aims_gpu.h).  Argument marshalling only: torch supplies device memory
+and the stream; every step of the path runs in the library's CUDA kernels.  No CPU fallback, no other backend.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import re
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libaims_gpu.so")
+HEADER_PATH = os.path.join(os.path.dirname(_HERE), "include", "aims_gpu.h")
+
+_dp = ctypes.POINTER(ctypes.c_double)
+_ip = ctypes.POINTER(ctypes.c_int32)
+_lp = ctypes.POINTER(ctypes.c_int64)
+_vp = ctypes.c_void_p
+
+
+class AimsError(RuntimeError):
+    pass
+
+
+class _BasisDesc(ctypes.Structure):
+    _fields_ = [("n_atoms", ctypes.c_int32), ("n_species", ctypes.c_int32), ("n_shells", ctypes.c_int32),
+                ("n_splines", ctypes.c_int32), ("n_knots", ctypes.c_int32),
+                ("atom_xyz", _dp), ("atom_species", _ip), ("species_shell_ptr", _ip), ("shell_l", _ip),
+                ("shell_rcut", _dp), ("shell_spline", _ip), ("r0", ctypes.c_double), ("log_inc", ctypes.c_double),
+                ("spline_coef", _dp)]
+
+
+class _GridDesc(ctypes.Structure):
+    _fields_ = [("n_points", ctypes.c_int64), ("n_batches", ctypes.c_int32), ("max_batch_points", ctypes.c_int32),
+                ("xyz", _dp), ("w", _dp), ("batch_ptr", _lp)]
+
+
+class _BsrDesc(ctypes.Structure):
+    _fields_ = [("n_block_rows", ctypes.c_int32), ("row_ptr", _lp), ("col_atom", _ip), ("blk_off", _lp),
+                ("blk_ld", _ip), ("n_values", ctypes.c_int64)]
+
+
+_lib = None
+
+
+def exported_symbols():
+    """Names declared in include/aims_gpu.h (every `int|const char*|int64_t aims_gpu_*(`)."""
+    with open(HEADER_PATH) as f:
+        text = f.read()
+    return sorted(set(re.findall(r"\b(aims_gpu_[a-z0-9_]+)\s*\(", text)))
+
+
+def load_library():
+    """dlopen libaims_gpu.so; raises (never falls back) if it is missing or lacks a declared symbol."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise AimsError("libaims_gpu.so is not built: run `python -m paper_1912_06636_b200.build` "
+                        "(nvcc, sm_100a). There is no CPU fallback.")
+    L = ctypes.CDLL(LIB_PATH)
+    for name in exported_symbols():
+        if not hasattr(L, name):
+            raise AimsError("libaims_gpu.so does not export %s" % name)
+    cp = _vp
+    L.aims_gpu_create.restype = ctypes.c_int
+    L.aims_gpu_create.argtypes = [ctypes.POINTER(cp), ctypes.POINTER(_BasisDesc), ctypes.POINTER(_GridDesc),
+                                  ctypes.POINTER(_BsrDesc), ctypes.c_int, _vp, ctypes.c_int64]
+    L.aims_gpu_destroy.restype = ctypes.c_int
+    L.aims_gpu_destroy.argtypes = [cp]
+    L.aims_gpu_last_error.restype = ctypes.c_char_p
+    L.aims_gpu_last_error.argtypes = [cp]
+    L.aims_gpu_basis_sizes.restype = ctypes.c_int
+    L.aims_gpu_basis_sizes.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _lp, _lp]
+    L.aims_gpu_eval_basis.restype = ctypes.c_int
+    L.aims_gpu_eval_basis.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp, _vp, _vp, _vp]
+    L.aims_gpu_integrate_hamiltonian.restype = ctypes.c_int
+    L.aims_gpu_integrate_hamiltonian.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp, _vp, ctypes.c_int]
+    L.aims_gpu_update_density.restype = ctypes.c_int
+    L.aims_gpu_update_density.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp, _vp]
+    L.aims_gpu_synchronize.restype = ctypes.c_int
+    L.aims_gpu_synchronize.argtypes = [cp]
+    L.aims_gpu_stats.restype = ctypes.c_int
+    L.aims_gpu_stats.argtypes = [cp, _lp, _ip, _ip, _dp, _dp, _dp]
+    L.aims_gpu_launch_count.restype = ctypes.c_int64
+    L.aims_gpu_launch_count.argtypes = [cp]
+    L.aims_gpu_fp64_peak.restype = ctypes.c_int
+    L.aims_gpu_fp64_peak.argtypes = [cp, ctypes.c_double, _dp]
+    _lib = L
+    return L
+
+
+def _ptr(t):
+    return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+class Context:
+    """One aims_gpu_ctx.  `bun` is any object with the attribute names of aims_synth.Bundle (numpy arrays)."""
+
+    def __init__(self, bun, device=0, stream=None, workspace_bytes=0):
+        import torch
+        self.torch = torch
+        self.L = load_library()
+        if not torch.cuda.is_available():
+            raise AimsError("no CUDA device: this path has no CPU fallback")
+        self.device = torch.device("cuda", device)
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        f64 = lambda a: np.ascontiguousarray(a, dtype=np.float64)  # noqa: E731
+        i32 = lambda a: np.ascontiguousarray(a, dtype=np.int32)    # noqa: E731
+        i64 = lambda a: np.ascontiguousarray(a, dtype=np.int64)    # noqa: E731
+        k = dict(atom_xyz=f64(bun.atom_xyz), atom_species=i32(bun.atom_species),
+                 species_shell_ptr=i32(bun.species_shell_ptr), shell_l=i32(bun.shell_l), shell_rcut=f64(bun.shell_rcut),
+                 shell_spline=i32(bun.shell_spline), spline_coef=f64(bun.spline_coef), xyz=f64(bun.xyz), w=f64(bun.w),
+                 batch_ptr=i64(bun.batch_ptr), row_ptr=i64(bun.row_ptr), col_atom=i32(bun.col_atom),
+                 blk_off=i64(bun.blk_off), blk_ld=i32(bun.blk_ld))
+        d = lambda a: a.ctypes.data_as(_dp)   # noqa: E731
+        i = lambda a: a.ctypes.data_as(_ip)   # noqa: E731
+        l = lambda a: a.ctypes.data_as(_lp)   # noqa: E731
+        self.n_points = int(k["xyz"].shape[0])
+        self.n_batches = int(k["batch_ptr"].shape[0] - 1)
+        self.n_values = int(bun.n_values)
+        self.batch_ptr = k["batch_ptr"]
+        bd = _BasisDesc(int(k["atom_xyz"].shape[0]), int(k["species_shell_ptr"].shape[0] - 1), int(k["shell_l"].shape[0]),
+                        int(k["spline_coef"].shape[0]), int(bun.n_knots), d(k["atom_xyz"]), i(k["atom_species"]),
+                        i(k["species_shell_ptr"]), i(k["shell_l"]), d(k["shell_rcut"]), i(k["shell_spline"]),
+                        float(bun.r0), float(bun.log_inc), d(k["spline_coef"]))
+        max_bp = int(np.diff(k["batch_ptr"]).max(initial=0))
+        gd = _GridDesc(self.n_points, self.n_batches, max_bp, d(k["xyz"]), d(k["w"]), l(k["batch_ptr"]))
+        pd = _BsrDesc(int(k["atom_xyz"].shape[0]), l(k["row_ptr"]), i(k["col_atom"]), l(k["blk_off"]), i(k["blk_ld"]),
+                      self.n_values)
+        self.h = ctypes.c_void_p()
+        rc = self.L.aims_gpu_create(ctypes.byref(self.h), ctypes.byref(bd), ctypes.byref(gd), ctypes.byref(pd),
+                                    int(device), ctypes.c_void_p(self.stream.cuda_stream), int(workspace_bytes))
+        if rc != 0:
+            msg = self.L.aims_gpu_last_error(self.h).decode() if self.h else ""
+            if self.h:
+                self.L.aims_gpu_destroy(self.h)
+                self.h = None
+            raise AimsError("aims_gpu_create failed (%d): %s" % (rc, msg))
+
+    # ---- plumbing
+    def _check(self, rc, what):
+        if rc != 0:
+            raise AimsError("%s failed (%d): %s" % (what, rc, self.L.aims_gpu_last_error(self.h).decode()))
+
+    def _range(self, b0, b1):
+        return int(b0), int(self.n_batches if b1 is None else b1)
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.L.aims_gpu_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def synchronize(self):
+        self._check(self.L.aims_gpu_synchronize(self.h), "aims_gpu_synchronize")
+
+    def launch_count(self):
+        return int(self.L.aims_gpu_launch_count(self.h))
+
+    def stats(self):
+        s, m, a = ctypes.c_int64(), ctypes.c_int32(), ctypes.c_int32()
+        f1, f2, f3 = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+        self._check(self.L.aims_gpu_stats(self.h, ctypes.byref(s), ctypes.byref(m), ctypes.byref(a), ctypes.byref(f1),
+                                          ctypes.byref(f2), ctypes.byref(f3)), "aims_gpu_stats")
+        return dict(sum_nnz=s.value, max_nnz=m.value, max_active_atoms=a.value, flops_h_lda=f1.value,
+                    flops_h_gga=f2.value, flops_density=f3.value)
+
+    def fp64_peak(self, ms_target=200.0):
+        t = ctypes.c_double()
+        self._check(self.L.aims_gpu_fp64_peak(self.h, float(ms_target), ctypes.byref(t)), "aims_gpu_fp64_peak")
+        return t.value
+
+    def _dev(self, a, dtype=None):
+        torch = self.torch
+        if isinstance(a, torch.Tensor):
+            t = a.to(self.device)
+            return t.contiguous() if dtype is None else t.to(dtype).contiguous()
+        return torch.as_tensor(np.ascontiguousarray(a), dtype=dtype).to(self.device)
+
+    # ---- the three hot calls (device tensors in, device tensors out)
+    def basis_sizes(self, b0=0, b1=None):
+        b0, b1 = self._range(b0, b1)
+        ni, nph = ctypes.c_int64(), ctypes.c_int64()
+        self._check(self.L.aims_gpu_basis_sizes(self.h, b0, b1, ctypes.byref(ni), ctypes.byref(nph)), "aims_gpu_basis_sizes")
+        return ni.value, nph.value
+
+    def eval_basis(self, b0=0, b1=None, want_grad=False):
+        """(fn_ptr, fn_index, phi_ptr, phi, dphi|None) as device tensors (layout: include/aims_gpu.h)."""
+        torch = self.torch
+        b0, b1 = self._range(b0, b1)
+        ni, nph = self.basis_sizes(b0, b1)
+        with torch.cuda.stream(self.stream):
+            fn_ptr = torch.empty(b1 - b0 + 1, dtype=torch.int64, device=self.device)
+            phi_ptr = torch.empty(b1 - b0 + 1, dtype=torch.int64, device=self.device)
+            fn_index = torch.empty(max(ni, 1), dtype=torch.int32, device=self.device)
+            phi = torch.empty(max(nph, 1), dtype=torch.float64, device=self.device)
+            dphi = torch.empty(max(3 * nph, 1), dtype=torch.float64, device=self.device) if want_grad else None
+        self._check(self.L.aims_gpu_eval_basis(self.h, b0, b1, _ptr(fn_ptr), _ptr(fn_index), _ptr(phi_ptr), _ptr(phi),
+                                               _ptr(dphi)), "aims_gpu_eval_basis")
+        return fn_ptr, fn_index[:ni], phi_ptr, phi[:nph], (dphi[:3 * nph] if want_grad else None)
+
+    def integrate_hamiltonian(self, v, g=None, H=None, b0=0, b1=None, accumulate=False):
+        torch = self.torch
+        b0, b1 = self._range(b0, b1)
+        v = self._dev(v, torch.float64)
+        g = None if g is None else self._dev(g, torch.float64)
+        if v.numel() != self.n_points or (g is not None and g.numel() != 3 * self.n_points):
+            raise AimsError("v must have n_points entries and g 3*n_points")
+        if H is None:
+            with torch.cuda.stream(self.stream):
+                H = torch.empty(self.n_values, dtype=torch.float64, device=self.device)
+            accumulate = False
+        self._check(self.L.aims_gpu_integrate_hamiltonian(self.h, b0, b1, _ptr(v), _ptr(g), _ptr(H), int(bool(accumulate))),
+                    "aims_gpu_integrate_hamiltonian")
+        return H
+
+    def update_density(self, D, want_grad=False, n=None, grad_n=None, b0=0, b1=None):
+        torch = self.torch
+        b0, b1 = self._range(b0, b1)
+        D = self._dev(D, torch.float64)
+        if D.numel() != self.n_values:
+            raise AimsError("D must have n_values entries")
+        with torch.cuda.stream(self.stream):
+            if n is None:
+                n = torch.zeros(self.n_points, dtype=torch.float64, device=self.device)
+            if want_grad and grad_n is None:
+                grad_n = torch.zeros((3, self.n_points), dtype=torch.float64, device=self.device)
+        self._check(self.L.aims_gpu_update_density(self.h, b0, b1, _ptr(D), _ptr(n), _ptr(grad_n) if want_grad else None),
+                    "aims_gpu_update_density")
+        return n, (grad_n if want_grad else None)
+
+    # ---- end-to-end with HOST buffers (pinned): H2D of v, g, D; the two calls; D2H of H, n, grad n
+    def make_host_buffers(self, want_grad):
+        torch = self.torch
+        pin = dict(pin_memory=True, dtype=torch.float64)
+        hb = dict(v=torch.empty(self.n_points, **pin), D=torch.empty(self.n_values, **pin),
+                  H=torch.empty(self.n_values, **pin), n=torch.empty(self.n_points, **pin))
+        if want_grad:
+            hb["g"] = torch.empty((3, self.n_points), **pin)
+            hb["grad_n"] = torch.empty((3, self.n_points), **pin)
+        dv = {k: torch.empty_like(t, device=self.device) for k, t in hb.items()}
+        return hb, dv
+
+    def step_host(self, hb, dv, want_grad):
+        """One pass of the whole hot path from pinned host inputs to pinned host outputs, on the context stream."""
+        torch = self.torch
+        with torch.cuda.stream(self.stream):
+            dv["v"].copy_(hb["v"], non_blocking=True)
+            dv["D"].copy_(hb["D"], non_blocking=True)
+            if want_grad:
+                dv["g"].copy_(hb["g"], non_blocking=True)
+            self.integrate_hamiltonian(dv["v"], dv["g"] if want_grad else None, H=dv["H"], accumulate=False)
+            self.update_density(dv["D"], want_grad=want_grad, n=dv["n"], grad_n=dv.get("grad_n"))
+            hb["H"].copy_(dv["H"], non_blocking=True)
+            hb["n"].copy_(dv["n"], non_blocking=True)
+            if want_grad:
+                hb["grad_n"].copy_(dv["grad_n"], non_blocking=True)
+
+
+# ---- module-level functions with the names of the C ABI
+def aims_gpu_create(bun, device=0, stream=None, workspace_bytes=0):
+    return Context(bun, device, stream, workspace_bytes)
+
+
+def aims_gpu_destroy(ctx):
+    ctx.close()
+
+
+def aims_gpu_eval_basis(ctx, b0=0, b1=None, want_grad=False):
+    return ctx.eval_basis(b0, b1, want_grad)
+
+
+def aims_gpu_integrate_hamiltonian(ctx, v, g=None, H=None, b0=0, b1=None, accumulate=False):
+    return ctx.integrate_hamiltonian(v, g, H, b0, b1, accumulate)
+
+
+def aims_gpu_update_density(ctx, D, want_grad=False, n=None, grad_n=None, b0=0, b1=None):
+    return ctx.update_density(D, want_grad, n, grad_n, b0, b1)

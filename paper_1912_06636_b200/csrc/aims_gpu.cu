@@ -1,0 +1,499 @@
+// aims_gpu.cu -- C ABI (include/aims_gpu.h) and host-side orchestration of the sm_100a kernels.
+// No CPU fallback: every step of the path runs in the kernels of basis.cuh / hamiltonian.cuh / density.cuh.
+#include "../../include/aims_gpu.h"
+
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "basis.cuh"
+#include "common.cuh"
+#include "density.cuh"
+#include "hamiltonian.cuh"
+
+using namespace aims;
+
+static_assert(kMaxActive == AIMS_MAX_ACTIVE_ATOMS, "header and kernels disagree");
+
+struct aims_gpu_ctx {
+  int device = 0;
+  cudaStream_t stream = nullptr;
+  std::string err;
+  int64_t launches = 0;
+  std::vector<void *> owned;  // device allocations to free
+
+  DevSys S{};
+  BatchLists L{};
+  int n_batches = 0;
+  int64_t n_points = 0, n_values = 0;
+
+  // host copies of the static structure (dry run)
+  std::vector<long long> batch_ptr, fn_off, act_off, ptab_off, pad_off, api_off, tile_off, item_off;
+  std::vector<int> nnz, n_act;
+  int max_nnz = 0, max_act = 0, max_np = 0;
+  long long *d_pad_off = nullptr, *d_api_off = nullptr;
+  HTile *d_tiles = nullptr;
+  DItem *d_items = nullptr;
+  double flops_h_lda = 0, flops_h_gga = 0, flops_den = 0;
+
+  double *ws = nullptr;      // Phi-plane workspace
+  long long ws_doubles = 0;
+};
+
+namespace {
+
+#define CU_TRY(ctx, call)                                                                          \
+  do {                                                                                             \
+    cudaError_t e_ = (call);                                                                       \
+    if (e_ != cudaSuccess) {                                                                       \
+      (ctx)->err = std::string(#call) + ": " + cudaGetErrorString(e_);                             \
+      return (e_ == cudaErrorMemoryAllocation) ? AIMS_ERR_NOMEM : AIMS_ERR_CUDA;                   \
+    }                                                                                              \
+  } while (0)
+
+template <class T>
+int dev_alloc(aims_gpu_ctx *c, T **p, size_t n) {
+  void *q = nullptr;
+  CU_TRY(c, cudaMalloc(&q, std::max<size_t>(n, 1) * sizeof(T)));
+  c->owned.push_back(q);
+  *p = static_cast<T *>(q);
+  return AIMS_OK;
+}
+template <class T>
+int dev_upload(aims_gpu_ctx *c, T **p, const T *h, size_t n) {
+  int rc = dev_alloc(c, p, n);
+  if (rc) return rc;
+  if (n) CU_TRY(c, cudaMemcpyAsync(*p, h, n * sizeof(T), cudaMemcpyHostToDevice, c->stream));
+  return AIMS_OK;
+}
+
+int fail(aims_gpu_ctx *c, int code, const char *msg) {
+  if (c) c->err = msg;
+  return code;
+}
+
+// asynchronous faults and capacity overflows reported by the kernels
+int check_async(aims_gpu_ctx *c) {
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) { c->err = std::string("kernel launch: ") + cudaGetErrorString(e); return AIMS_ERR_CUDA; }
+  return AIMS_OK;
+}
+
+__global__ void k_fp64_peak(double *out, int iters, double a, double b) {
+  double c0[16], c1[16];
+#pragma unroll
+  for (int i = 0; i < 16; i++) { c0[i] = threadIdx.x * 1e-9 + i; c1[i] = i; }
+  for (int it = 0; it < iters; it++) {
+#pragma unroll
+    for (int i = 0; i < 16; i++) dmma8x8x4(c0[i], c1[i], a, b);
+  }
+  double s = 0;
+#pragma unroll
+  for (int i = 0; i < 16; i++) s += c0[i] + c1[i];
+  if (s == 12345.678) out[0] = s;
+}
+
+bool range_ok(const aims_gpu_ctx *c, int b0, int b1) { return c && b0 >= 0 && b1 >= b0 && b1 <= c->n_batches; }
+
+}  // namespace
+
+extern "C" {
+
+const char *aims_gpu_last_error(const aims_gpu_ctx *ctx) { return ctx ? ctx->err.c_str() : ""; }
+int64_t aims_gpu_launch_count(const aims_gpu_ctx *ctx) { return ctx ? ctx->launches : 0; }
+
+int aims_gpu_destroy(aims_gpu_ctx *ctx) {
+  if (!ctx) return AIMS_ERR_INVALID_ARG;
+  cudaSetDevice(ctx->device);
+  cudaError_t e = cudaStreamSynchronize(ctx->stream);
+  for (void *p : ctx->owned) cudaFree(p);
+  delete ctx;
+  return e == cudaSuccess ? AIMS_OK : AIMS_ERR_CUDA;
+}
+
+int aims_gpu_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_grid_desc *G, const aims_bsr_desc *P,
+                    int device, void *cuda_stream, int64_t workspace_bytes) {
+  if (!out) return AIMS_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (!B || !G || !P) return AIMS_ERR_INVALID_ARG;
+  if (B->n_atoms < 0 || B->n_species <= 0 || B->n_shells <= 0 || B->n_knots < 2 || G->n_points < 0 || G->n_batches < 0 ||
+      P->n_block_rows != B->n_atoms || !B->atom_xyz || !B->atom_species || !B->species_shell_ptr || !B->shell_l ||
+      !B->shell_rcut || !B->shell_spline || !B->spline_coef || !G->batch_ptr || (G->n_points && (!G->xyz || !G->w)) ||
+      !P->row_ptr || !P->col_atom || !P->blk_off || !P->blk_ld || !(B->r0 > 0) || !(B->log_inc > 0))
+    return AIMS_ERR_INVALID_ARG;
+  aims_gpu_ctx *c = new (std::nothrow) aims_gpu_ctx;
+  if (!c) return AIMS_ERR_NOMEM;
+  *out = c;  // returned even on failure so that the caller can read last_error, then destroy
+  c->device = device;
+  c->stream = static_cast<cudaStream_t>(cuda_stream);
+  CU_TRY(c, cudaSetDevice(device));
+  cudaDeviceProp prop;
+  CU_TRY(c, cudaGetDeviceProperties(&prop, device));
+  if (prop.major != 10) return fail(c, AIMS_ERR_UNSUPPORTED, "this library is built for sm_100a (B200) only");
+
+  // ---- validate and derive host-side tables
+  const int na = B->n_atoms, nsp = B->n_species, nsh = B->n_shells;
+  for (int s = 0; s < nsh; s++) {
+    if (B->shell_l[s] < 0 || B->shell_l[s] > AIMS_MAX_L) return fail(c, AIMS_ERR_UNSUPPORTED, "shell_l outside 0..3");
+    if (B->shell_spline[s] < 0 || B->shell_spline[s] >= B->n_splines) return fail(c, AIMS_ERR_INVALID_ARG, "shell_spline out of range");
+  }
+  std::vector<int> sp_nfn(nsp, 0);
+  std::vector<double> sp_rcmax2(nsp, 0.0), shell_rc2(nsh);
+  for (int s = 0; s < nsh; s++) shell_rc2[s] = B->shell_rcut[s] * B->shell_rcut[s];
+  for (int sp = 0; sp < nsp; sp++) {
+    const int s0 = B->species_shell_ptr[sp], s1 = B->species_shell_ptr[sp + 1];
+    if (s0 < 0 || s1 < s0 || s1 > nsh) return fail(c, AIMS_ERR_INVALID_ARG, "species_shell_ptr not ascending");
+    if (s1 - s0 > AIMS_MAX_SHELLS_PER_SPECIES) return fail(c, AIMS_ERR_UNSUPPORTED, "more than 32 shells per species");
+    for (int s = s0; s < s1; s++) { sp_nfn[sp] += 2 * B->shell_l[s] + 1; sp_rcmax2[sp] = std::max(sp_rcmax2[sp], shell_rc2[s]); }
+  }
+  std::vector<int> atom_fn_ptr(na + 1, 0);
+  for (int a = 0; a < na; a++) {
+    const int sp = B->atom_species[a];
+    if (sp < 0 || sp >= nsp) return fail(c, AIMS_ERR_INVALID_ARG, "atom_species out of range");
+    atom_fn_ptr[a + 1] = atom_fn_ptr[a] + sp_nfn[sp];
+  }
+  const long long n_blocks = P->row_ptr[na];
+  for (int a = 0; a < na; a++) {
+    if (P->row_ptr[a + 1] <= P->row_ptr[a] || P->col_atom[P->row_ptr[a]] != a)
+      return fail(c, AIMS_ERR_INVALID_ARG, "every block row must start with its diagonal block");
+    for (long long q = P->row_ptr[a]; q < P->row_ptr[a + 1]; q++) {
+      const int cb = P->col_atom[q];
+      if (cb < a || cb >= na || (q > P->row_ptr[a] && cb <= P->col_atom[q - 1]))
+        return fail(c, AIMS_ERR_INVALID_ARG, "col_atom must be ascending and >= row");
+      if ((P->blk_off[q] & 1) || (P->blk_ld[q] & 1) || P->blk_ld[q] < sp_nfn[B->atom_species[cb]] ||
+          P->blk_ld[q] != P->blk_ld[P->row_ptr[cb]] ||
+          P->blk_off[q] + (long long)sp_nfn[B->atom_species[a]] * P->blk_ld[q] > P->n_values)
+        return fail(c, AIMS_ERR_INVALID_ARG, "blk_off/blk_ld must be even, consistent per column atom and inside n_values");
+    }
+  }
+  c->n_batches = G->n_batches;
+  c->n_points = G->n_points;
+  c->n_values = P->n_values;
+  c->batch_ptr.assign(G->batch_ptr, G->batch_ptr + G->n_batches + 1);
+  if (c->batch_ptr[0] != 0 || c->batch_ptr[G->n_batches] != G->n_points) return fail(c, AIMS_ERR_INVALID_ARG, "batch_ptr must span [0, n_points]");
+  for (int b = 0; b < G->n_batches; b++) {
+    const long long n = c->batch_ptr[b + 1] - c->batch_ptr[b];
+    if (n < 0 || n > G->max_batch_points) return fail(c, AIMS_ERR_INVALID_ARG, "batch_ptr not ascending or batch larger than max_batch_points");
+    c->max_np = std::max<int>(c->max_np, (int)n);
+  }
+
+  // ---- upload (points as structure-of-arrays)
+  DevSys &S = c->S;
+  S.n_atoms = na; S.n_species = nsp; S.n_shells = nsh; S.n_knots = B->n_knots;
+  S.r0 = B->r0; S.log_inc = B->log_inc;
+  int rc;
+#define UP(field, T, hostptr, n)                                           \
+  { T *d_; rc = dev_upload<T>(c, &d_, hostptr, (size_t)(n)); if (rc) return rc; field = d_; }
+  UP(S.atom_xyz, double, B->atom_xyz, 3 * (size_t)na)
+  UP(S.atom_species, int, B->atom_species, na)
+  UP(S.atom_fn_ptr, int, atom_fn_ptr.data(), na + 1)
+  UP(S.sp_shell_ptr, int, B->species_shell_ptr, nsp + 1)
+  UP(S.sp_rcmax2, double, sp_rcmax2.data(), nsp)
+  UP(S.shell_l, int, B->shell_l, nsh)
+  UP(S.shell_rc2, double, shell_rc2.data(), nsh)
+  UP(S.shell_spline, int, B->shell_spline, nsh)
+  UP(S.spline_coef, double, B->spline_coef, (size_t)B->n_splines * (B->n_knots - 1) * 4)
+  {
+    const size_t n = (size_t)G->n_points;
+    std::vector<double> soa(3 * n);
+    for (size_t p = 0; p < n; p++) { soa[p] = G->xyz[3 * p]; soa[n + p] = G->xyz[3 * p + 1]; soa[2 * n + p] = G->xyz[3 * p + 2]; }
+    double *d;
+    rc = dev_upload<double>(c, &d, soa.data(), 3 * n);
+    if (rc) return rc;
+    CU_TRY(c, cudaStreamSynchronize(c->stream));  // soa goes out of scope
+    S.px = d; S.py = d + n; S.pz = d + 2 * n;
+  }
+  UP(S.w, double, G->w, G->n_points)
+  UP(S.batch_ptr, long long, c->batch_ptr.data(), G->n_batches + 1)
+  {
+    std::vector<long long> rp(P->row_ptr, P->row_ptr + na + 1), bo(P->blk_off, P->blk_off + n_blocks);
+    UP(S.row_ptr, long long, rp.data(), na + 1)
+    UP(S.blk_off, long long, bo.data(), n_blocks)
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+  }
+  UP(S.col_atom, int, P->col_atom, n_blocks)
+  UP(S.blk_ld, int, P->blk_ld, n_blocks)
+#undef UP
+
+  // ---- dry run of the culling: sizes of every per-batch list
+  const int nb = c->n_batches;
+  BatchLists &L = c->L;
+  if ((rc = dev_alloc(c, &L.nnz, nb))) return rc;
+  if ((rc = dev_alloc(c, &L.n_act, nb))) return rc;
+  if ((rc = dev_alloc(c, &L.error_flag, 1))) return rc;
+  CU_TRY(c, cudaMemsetAsync(L.error_flag, 0, sizeof(int), c->stream));
+  if (nb) {
+    k_cull<<<nb, 256, 0, c->stream>>>(S, L, 0, 1);
+    c->launches++;
+    if ((rc = check_async(c))) return rc;
+  }
+  c->nnz.resize(nb); c->n_act.resize(nb);
+  int flag = 0;
+  CU_TRY(c, cudaMemcpyAsync(c->nnz.data(), L.nnz, nb * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+  CU_TRY(c, cudaMemcpyAsync(c->n_act.data(), L.n_act, nb * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+  CU_TRY(c, cudaMemcpyAsync(&flag, L.error_flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+  CU_TRY(c, cudaStreamSynchronize(c->stream));
+  if (flag == 1) return fail(c, AIMS_ERR_UNSUPPORTED, "more than 1024 atoms pass the bounding-box test of one batch");
+  if (flag == 2) return fail(c, AIMS_ERR_UNSUPPORTED, "more than AIMS_MAX_ACTIVE_ATOMS atoms touch one batch");
+
+  c->fn_off.assign(nb + 1, 0); c->act_off.assign(nb + 1, 0); c->ptab_off.assign(nb + 1, 0);
+  c->pad_off.assign(nb + 1, 0); c->api_off.assign(nb + 1, 0); c->tile_off.assign(nb + 1, 0); c->item_off.assign(nb + 1, 0);
+  std::vector<HTile> tiles;
+  std::vector<DItem> items;
+  for (int b = 0; b < nb; b++) {
+    const int nz = c->nnz[b], nact = c->n_act[b];
+    const int np = (int)(c->batch_ptr[b + 1] - c->batch_ptr[b]);
+    const int ld = round_up(np, kPadPts);
+    c->max_nnz = std::max(c->max_nnz, nz);
+    c->max_act = std::max(c->max_act, nact);
+    c->fn_off[b + 1] = c->fn_off[b] + nz;
+    c->act_off[b + 1] = c->act_off[b] + nact;
+    c->ptab_off[b + 1] = c->ptab_off[b] + (long long)nact * nact;
+    c->pad_off[b + 1] = c->pad_off[b] + (long long)nz * ld;
+    c->api_off[b + 1] = c->api_off[b] + (long long)nz * np;
+    // Hamiltonian tiles: balanced edge T <= 128, multiple of 8; upper triangle
+    if (nz > 0 && np > 0) {
+      const int nt = (nz + kHT - 1) / kHT;
+      const int T = round_up((nz + nt - 1) / nt, 8);
+      for (int ti = 0; ti < nt; ti++)
+        for (int tj = ti; tj < nt; tj++) tiles.push_back(HTile{b, ti, tj, T});
+    }
+    c->tile_off[b + 1] = (long long)tiles.size();
+    // density items: balanced point tiles <= 208, multiple of 8, covering the padded leading dimension
+    if (np > 0) {
+      const int npt = (ld + kDTN - 1) / kDTN;
+      const int tp = round_up((ld + npt - 1) / npt, 8);
+      for (int q = 0; q < npt; q++) {
+        const int p0 = q * tp;
+        if (p0 < ld) items.push_back(DItem{b, p0, std::min(tp, ld - p0), 0});
+      }
+    }
+    c->item_off[b + 1] = (long long)items.size();
+    c->flops_h_lda += (double)np * nz * (nz + 1.0);
+    c->flops_h_gga += 2.0 * np * (double)nz * nz;
+    c->flops_den += 2.0 * np * (double)nz * nz;
+  }
+  if (c->max_nnz >= 65536) return fail(c, AIMS_ERR_UNSUPPORTED, "nnz(B) >= 65536");
+  {
+    long long *d;
+#define UPL(vec, field) if ((rc = dev_upload<long long>(c, &d, vec.data(), vec.size()))) return rc; field = d;
+    UPL(c->fn_off, L.fn_off) UPL(c->act_off, L.act_off) UPL(c->ptab_off, L.ptab_off)
+    UPL(c->pad_off, c->d_pad_off) UPL(c->api_off, c->d_api_off)
+#undef UPL
+  }
+  if ((rc = dev_upload<HTile>(c, &c->d_tiles, tiles.data(), tiles.size()))) return rc;
+  if ((rc = dev_upload<DItem>(c, &c->d_items, items.data(), items.size()))) return rc;
+  CU_TRY(c, cudaStreamSynchronize(c->stream));
+  if ((rc = dev_alloc(c, &L.fn_index, (size_t)c->fn_off[nb]))) return rc;
+  if ((rc = dev_alloc(c, &L.fn_info, (size_t)c->fn_off[nb]))) return rc;
+  if ((rc = dev_alloc(c, &L.act_atom, (size_t)c->act_off[nb]))) return rc;
+  if ((rc = dev_alloc(c, &L.act_mask, (size_t)c->act_off[nb]))) return rc;
+  if ((rc = dev_alloc(c, &L.act_row0, (size_t)c->act_off[nb]))) return rc;
+  if ((rc = dev_alloc(c, &L.act_ld, (size_t)c->act_off[nb]))) return rc;
+  if ((rc = dev_alloc(c, &L.ptab, (size_t)c->ptab_off[nb]))) return rc;
+
+  // ---- Phi-plane workspace: enough for the largest single batch with 4 planes, at most the requested budget
+  long long want = workspace_bytes > 0 ? workspace_bytes : (24ll << 30);
+  size_t free_b = 0, total_b = 0;
+  CU_TRY(c, cudaMemGetInfo(&free_b, &total_b));
+  want = std::min<long long>(want, (long long)(free_b * 0.8));
+  long long max_batch_d = 0;
+  for (int b = 0; b < nb; b++) max_batch_d = std::max(max_batch_d, c->pad_off[b + 1] - c->pad_off[b]);
+  long long need_all = 4 * c->pad_off[nb], need_min = 4 * max_batch_d;
+  long long wsd = std::min(need_all, std::max(want / 8, need_min));
+  if (wsd * 8 > (long long)free_b) return fail(c, AIMS_ERR_NOMEM, "not enough device memory for one batch of Phi planes");
+  if ((rc = dev_alloc(c, &c->ws, (size_t)wsd))) return rc;
+  c->ws_doubles = wsd;
+
+  // opt in to large dynamic shared memory
+  CU_TRY(c, cudaFuncSetAttribute(k_hamiltonian<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h_smem_bytes<false>()));
+  CU_TRY(c, cudaFuncSetAttribute(k_hamiltonian<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h_smem_bytes<true>()));
+  const size_t dsm = d_smem_bytes(c->max_nnz, std::max(c->max_act, 1));
+  if (dsm > (size_t)prop.sharedMemPerBlockOptin) return fail(c, AIMS_ERR_UNSUPPORTED, "nnz(B) / active atoms too large for the density kernel's shared memory");
+  CU_TRY(c, cudaFuncSetAttribute(k_density<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dsm));
+  CU_TRY(c, cudaFuncSetAttribute(k_density<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dsm));
+  CU_TRY(c, cudaStreamSynchronize(c->stream));
+  return AIMS_OK;
+}
+
+int aims_gpu_stats(aims_gpu_ctx *c, int64_t *sum_nnz, int32_t *max_nnz, int32_t *max_active_atoms, double *flops_h_lda,
+                   double *flops_h_gga, double *flops_density) {
+  if (!c) return AIMS_ERR_INVALID_ARG;
+  if (sum_nnz) *sum_nnz = c->fn_off.empty() ? 0 : c->fn_off.back();
+  if (max_nnz) *max_nnz = c->max_nnz;
+  if (max_active_atoms) *max_active_atoms = c->max_act;
+  if (flops_h_lda) *flops_h_lda = c->flops_h_lda;
+  if (flops_h_gga) *flops_h_gga = c->flops_h_gga;
+  if (flops_density) *flops_density = c->flops_den;
+  return AIMS_OK;
+}
+
+int aims_gpu_basis_sizes(aims_gpu_ctx *c, int32_t b0, int32_t b1, int64_t *n_index, int64_t *n_phi) {
+  if (!range_ok(c, b0, b1)) return fail(c, AIMS_ERR_INVALID_ARG, "batch range outside [0, n_batches]");
+  if (n_index) *n_index = c->fn_off[b1] - c->fn_off[b0];
+  if (n_phi) *n_phi = c->api_off[b1] - c->api_off[b0];
+  return AIMS_OK;
+}
+
+}  // extern "C"
+
+namespace {
+
+// S1a for batches [b0,b1): rebuilds every per-batch list on the device (part of each hot call)
+int run_cull(aims_gpu_ctx *c, int b0, int b1) {
+  if (b1 > b0) {
+    k_cull<<<b1 - b0, 256, 0, c->stream>>>(c->S, c->L, b0, 0);
+    c->launches++;
+  }
+  return check_async(c);
+}
+
+// last batch (exclusive) of the chunk starting at bs such that nplanes planes fit the workspace
+int chunk_end(const aims_gpu_ctx *c, int bs, int b1, int nplanes) {
+  const long long cap = c->ws_doubles / nplanes;
+  int lo = bs + 1, hi = b1;  // at least one batch (create guaranteed it fits)
+  while (lo < hi) {
+    int mid = (lo + hi + 1) >> 1;
+    if (c->pad_off[mid] - c->pad_off[bs] <= cap) lo = mid; else hi = mid - 1;
+  }
+  return lo;
+}
+
+template <int MODE>
+void launch_eval(aims_gpu_ctx *c, const EvalArgs &E, int bs, int be) {
+  k_eval<MODE><<<be - bs, 256, 0, c->stream>>>(c->S, c->L, E, bs);
+  c->launches++;
+}
+
+}  // namespace
+
+extern "C" {
+
+int aims_gpu_eval_basis(aims_gpu_ctx *c, int32_t b0, int32_t b1, int64_t *fn_ptr, int32_t *fn_index, int64_t *phi_ptr,
+                        double *phi, double *dphi) {
+  if (!range_ok(c, b0, b1)) return fail(c, AIMS_ERR_INVALID_ARG, "batch range outside [0, n_batches]");
+  if (!fn_ptr || !fn_index || !phi_ptr || !phi) return fail(c, AIMS_ERR_INVALID_ARG, "NULL output");
+  CU_TRY(c, cudaSetDevice(c->device));
+  int rc = run_cull(c, b0, b1);
+  if (rc) return rc;
+  k_export_lists<<<b1 - b0 + 1, 128, 0, c->stream>>>(c->L, c->S, b0, b1, (long long *)fn_ptr, fn_index, (long long *)phi_ptr, c->d_api_off);
+  c->launches++;
+  if (b1 > b0) {
+    EvalArgs E{};
+    E.plane[0] = phi; E.plane[1] = dphi;
+    E.api = 1; E.api_off = c->d_api_off; E.api_base = c->api_off[b0];
+    E.n_points = c->n_points;
+    if (dphi) launch_eval<kEvalPhiGrad>(c, E, b0, b1); else launch_eval<kEvalPhi>(c, E, b0, b1);
+  }
+  return check_async(c);
+}
+
+int aims_gpu_integrate_hamiltonian(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, const double *g,
+                                   double *H_values, int accumulate) {
+  if (!range_ok(c, b0, b1)) return fail(c, AIMS_ERR_INVALID_ARG, "batch range outside [0, n_batches]");
+  if (!v || !H_values) return fail(c, AIMS_ERR_INVALID_ARG, "NULL v or H_values");
+  CU_TRY(c, cudaSetDevice(c->device));
+  if (!accumulate) CU_TRY(c, cudaMemsetAsync(H_values, 0, (size_t)c->n_values * sizeof(double), c->stream));
+  int rc = run_cull(c, b0, b1);
+  if (rc) return rc;
+  for (int bs = b0; bs < b1;) {
+    const int be = chunk_end(c, bs, b1, 2);
+    const long long plane = c->ws_doubles / 2;
+    EvalArgs E{};
+    E.plane[0] = c->ws; E.plane[1] = c->ws + plane;
+    E.pad_off = c->d_pad_off; E.pad_base = c->pad_off[bs];
+    E.v = v; E.g = g; E.n_points = c->n_points;
+    if (g) launch_eval<kEvalHGga>(c, E, bs, be); else launch_eval<kEvalHLda>(c, E, bs, be);
+    const long long nt = c->tile_off[be] - c->tile_off[bs];
+    if (nt > 0) {
+      HArgs A{c->d_tiles + c->tile_off[bs], E.plane[0], E.plane[1], c->d_pad_off, c->pad_off[bs], H_values};
+      if (g) k_hamiltonian<true><<<(unsigned)nt, kHThreads, h_smem_bytes<true>(), c->stream>>>(c->S, c->L, A);
+      else k_hamiltonian<false><<<(unsigned)nt, kHThreads, h_smem_bytes<false>(), c->stream>>>(c->S, c->L, A);
+      c->launches++;
+    }
+    if ((rc = check_async(c))) return rc;
+    bs = be;
+  }
+  return AIMS_OK;
+}
+
+int aims_gpu_update_density(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *D_values, double *n, double *grad_n) {
+  if (!range_ok(c, b0, b1)) return fail(c, AIMS_ERR_INVALID_ARG, "batch range outside [0, n_batches]");
+  if (!D_values || !n) return fail(c, AIMS_ERR_INVALID_ARG, "NULL D_values or n");
+  CU_TRY(c, cudaSetDevice(c->device));
+  int rc = run_cull(c, b0, b1);
+  if (rc) return rc;
+  const int npl = grad_n ? 4 : 1;
+  const size_t dsm = d_smem_bytes(c->max_nnz, std::max(c->max_act, 1));
+  for (int bs = b0; bs < b1;) {
+    const int be = chunk_end(c, bs, b1, npl);
+    const long long plane = c->ws_doubles / npl;
+    EvalArgs E{};
+    for (int q = 0; q < npl; q++) E.plane[q] = c->ws + q * plane;
+    if (!grad_n) E.plane[1] = c->ws;  // unused
+    E.pad_off = c->d_pad_off; E.pad_base = c->pad_off[bs];
+    E.n_points = c->n_points;
+    if (grad_n) launch_eval<kEvalPhiGrad>(c, E, bs, be); else launch_eval<kEvalPhi>(c, E, bs, be);
+    const long long ni = c->item_off[be] - c->item_off[bs];
+    if (ni > 0) {
+      DArgs A{};
+      A.items = c->d_items + c->item_off[bs];
+      A.P = E.plane[0];
+      for (int q = 0; q < 3; q++) A.G[q] = grad_n ? E.plane[q + 1] : nullptr;
+      A.pad_off = c->d_pad_off; A.pad_base = c->pad_off[bs];
+      A.D = D_values; A.n = n; A.gn = grad_n; A.n_points = c->n_points; A.max_nnz_pad = c->max_nnz;
+      if (grad_n) k_density<true><<<(unsigned)ni, kDThreads, dsm, c->stream>>>(c->S, c->L, A, std::max(c->max_act, 1));
+      else k_density<false><<<(unsigned)ni, kDThreads, dsm, c->stream>>>(c->S, c->L, A, std::max(c->max_act, 1));
+      c->launches++;
+    }
+    if ((rc = check_async(c))) return rc;
+    bs = be;
+  }
+  return AIMS_OK;
+}
+
+int aims_gpu_synchronize(aims_gpu_ctx *c) {
+  if (!c) return AIMS_ERR_INVALID_ARG;
+  CU_TRY(c, cudaSetDevice(c->device));
+  int flag = 0;
+  CU_TRY(c, cudaMemcpyAsync(&flag, c->L.error_flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+  CU_TRY(c, cudaStreamSynchronize(c->stream));
+  if (flag) {
+    c->err = "device-side capacity or consistency check failed (flag " + std::to_string(flag) + ")";
+    return AIMS_ERR_UNSUPPORTED;
+  }
+  return AIMS_OK;
+}
+
+int aims_gpu_fp64_peak(aims_gpu_ctx *c, double ms_target, double *tflops) {
+  if (!c || !tflops) return AIMS_ERR_INVALID_ARG;
+  CU_TRY(c, cudaSetDevice(c->device));
+  cudaDeviceProp prop;
+  CU_TRY(c, cudaGetDeviceProperties(&prop, c->device));
+  double *out;
+  int rc = dev_alloc(c, &out, 16);
+  if (rc) return rc;
+  const int iters = 20000;
+  const dim3 grid(prop.multiProcessorCount), block(256);
+  cudaEvent_t e0, e1;
+  CU_TRY(c, cudaEventCreate(&e0));
+  CU_TRY(c, cudaEventCreate(&e1));
+  k_fp64_peak<<<grid, block, 0, c->stream>>>(out, iters, 1.0000001, 1e-9);  // warm-up, ~5 ms
+  c->launches++;
+  const int reps = std::max(1, (int)(ms_target / 5.3));
+  CU_TRY(c, cudaEventRecord(e0, c->stream));
+  for (int r = 0; r < reps; r++) k_fp64_peak<<<grid, block, 0, c->stream>>>(out, iters, 1.0000001, 1e-9);
+  c->launches += reps;
+  CU_TRY(c, cudaEventRecord(e1, c->stream));
+  CU_TRY(c, cudaEventSynchronize(e1));
+  float ms = 0;
+  CU_TRY(c, cudaEventElapsedTime(&ms, e0, e1));
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  *tflops = 2.0 * 256 * 16 * (double)iters * grid.x * (block.x / 32) * reps / (ms * 1e-3) * 1e-12;
+  return AIMS_OK;
+}
+
+}  // extern "C"

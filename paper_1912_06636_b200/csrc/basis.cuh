@@ -1,0 +1,388 @@
+// basis.cuh -- S1a (active-function culling, nnz(B): PAPER.md L235) and S1b (basis evaluation, "calculate_phi":
+// PAPER.md L314/L322/L356) on the GPU.  The paper keeps this stage on the CPU (L381); here it is two kernels.
+#pragma once
+#include "common.cuh"
+
+namespace aims {
+
+// ---------------------------------------------------------------------------------------------------------------
+// k_cull: one CTA per batch.
+//   1. bounding box of the batch's points
+//   2. atoms whose largest cutoff sphere may reach the box (conservative)            -> candidate list (smem)
+//   3. exact test per candidate: min_p d2(p, atom) in separately rounded IEEE ops (reading P6), one warp per atom;
+//      shell s touches the batch iff min d2 < rcut_s^2 (strict)                       -> shell bit mask
+//   4. active atoms in ascending order (rank sort), rows per slot, nnz(B)
+//   5. (not in the dry run) function lists, slot tables and the atom-pair offset table of the batch
+// dry != 0: only nnz[b], n_act[b] are written (used once at context creation to size every list).
+// ---------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_cull(DevSys S, BatchLists L, int b_first, int dry) {
+  const int b = b_first + blockIdx.x;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const long long p0 = S.batch_ptr[b];
+  const int np = (int)(S.batch_ptr[b + 1] - p0);
+
+  __shared__ double s_red[8][6];
+  __shared__ double s_box[6];
+  __shared__ int s_ncand, s_nact, s_nnz;
+  __shared__ int s_cand[kMaxCand];
+  __shared__ unsigned s_cmask[kMaxCand];
+  __shared__ int s_act_atom[kMaxActive];
+  __shared__ unsigned s_act_mask[kMaxActive];
+  __shared__ int s_act_row0[kMaxActive];
+
+  if (tid == 0) { s_ncand = 0; s_nact = 0; s_nnz = 0; }
+
+  // 1. bounding box
+  double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
+  for (int p = tid; p < np; p += 256) {
+    double x = S.px[p0 + p], y = S.py[p0 + p], z = S.pz[p0 + p];
+    lo[0] = fmin(lo[0], x); hi[0] = fmax(hi[0], x);
+    lo[1] = fmin(lo[1], y); hi[1] = fmax(hi[1], y);
+    lo[2] = fmin(lo[2], z); hi[2] = fmax(hi[2], z);
+  }
+#pragma unroll
+  for (int c = 0; c < 3; c++)
+    for (int o = 16; o > 0; o >>= 1) {
+      lo[c] = fmin(lo[c], __shfl_xor_sync(0xffffffffu, lo[c], o));
+      hi[c] = fmax(hi[c], __shfl_xor_sync(0xffffffffu, hi[c], o));
+    }
+  if (lane == 0)
+    for (int c = 0; c < 3; c++) { s_red[warp][c] = lo[c]; s_red[warp][3 + c] = hi[c]; }
+  __syncthreads();
+  if (tid < 6) {
+    double v = s_red[0][tid];
+    for (int w2 = 1; w2 < 8; w2++) v = (tid < 3) ? fmin(v, s_red[w2][tid]) : fmax(v, s_red[w2][tid]);
+    s_box[tid] = v;
+  }
+  __syncthreads();
+
+  // 2. candidates: distance from the atom to the box, against the species' largest cutoff (with slack)
+  if (np > 0)
+    for (int a = tid; a < S.n_atoms; a += 256) {
+      double q = 0.0;
+#pragma unroll
+      for (int c = 0; c < 3; c++) {
+        double x = S.atom_xyz[3 * a + c];
+        double e = fmax(fmax(s_box[c] - x, x - s_box[3 + c]), 0.0);
+        q += e * e;
+      }
+      if (q <= S.sp_rcmax2[S.atom_species[a]] * (1.0 + 1e-9)) {
+        int k = atomicAdd(&s_ncand, 1);
+        if (k < kMaxCand) s_cand[k] = a;
+      }
+    }
+  __syncthreads();
+  int ncand = s_ncand;
+  if (ncand > kMaxCand) { if (tid == 0) atomicExch(L.error_flag, 1); ncand = kMaxCand; }
+
+  // 3. exact test, one warp per candidate
+  for (int c = warp; c < ncand; c += 8) {
+    const int a = s_cand[c];
+    const double X = S.atom_xyz[3 * a], Y = S.atom_xyz[3 * a + 1], Z = S.atom_xyz[3 * a + 2];
+    double dmin = 1e300;
+    for (int p = lane; p < np; p += 32) {
+      double dx = S.px[p0 + p] - X, dy = S.py[p0 + p] - Y, dz = S.pz[p0 + p] - Z;
+      double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+      dmin = fmin(dmin, d2);
+    }
+    for (int o = 16; o > 0; o >>= 1) dmin = fmin(dmin, __shfl_xor_sync(0xffffffffu, dmin, o));
+    if (lane == 0) {
+      const int sp = S.atom_species[a];
+      const int s0 = S.sp_shell_ptr[sp], s1 = S.sp_shell_ptr[sp + 1];
+      unsigned m = 0;
+      for (int s = s0; s < s1; s++)
+        if (dmin < S.shell_rc2[s]) m |= 1u << (s - s0);
+      s_cmask[c] = m;
+      if (m) atomicAdd(&s_nact, 1);
+    }
+  }
+  __syncthreads();
+  const int nact = s_nact;
+  if (nact > kMaxActive) {
+    if (tid == 0) { atomicExch(L.error_flag, 2); L.nnz[b] = 0; L.n_act[b] = nact; }
+    return;
+  }
+
+  // 4. ascending order of the active atoms (rank sort over the small candidate list)
+  for (int c = tid; c < ncand; c += 256)
+    if (s_cmask[c]) {
+      const int a = s_cand[c];
+      int rank = 0;
+      for (int c2 = 0; c2 < ncand; c2++) rank += (s_cmask[c2] != 0 && s_cand[c2] < a);
+      s_act_atom[rank] = a;
+      s_act_mask[rank] = s_cmask[c];
+    }
+  __syncthreads();
+  if (tid == 0) {
+    int row = 0;
+    for (int s = 0; s < nact; s++) {
+      s_act_row0[s] = row;
+      const int sp = S.atom_species[s_act_atom[s]];
+      const int s0 = S.sp_shell_ptr[sp], s1 = S.sp_shell_ptr[sp + 1];
+      for (int sh = s0; sh < s1; sh++)
+        if (s_act_mask[s] >> (sh - s0) & 1u) row += 2 * S.shell_l[sh] + 1;
+    }
+    s_nnz = row;
+    if (dry) { L.nnz[b] = row; L.n_act[b] = nact; }
+  }
+  __syncthreads();
+  if (dry) return;
+
+  // 5. lists.  Offsets were fixed by the dry run; the counts must agree.
+  const long long fo = L.fn_off[b], ao = L.act_off[b], po = L.ptab_off[b];
+  if ((long long)s_nnz != L.fn_off[b + 1] - fo || (long long)nact != L.act_off[b + 1] - ao) {
+    if (tid == 0) atomicExch(L.error_flag, 3);
+    return;
+  }
+  if (tid == 0) { L.nnz[b] = s_nnz; L.n_act[b] = nact; }
+  for (int s = tid; s < nact; s += 256) {
+    const int a = s_act_atom[s];
+    L.act_atom[ao + s] = a;
+    L.act_mask[ao + s] = s_act_mask[s];
+    L.act_row0[ao + s] = s_act_row0[s];
+    L.act_ld[ao + s] = S.blk_ld[S.row_ptr[a]];   // diagonal block (a,a) is the first block of row a
+    const int sp = S.atom_species[a];
+    const int s0 = S.sp_shell_ptr[sp], s1 = S.sp_shell_ptr[sp + 1];
+    int row = s_act_row0[s], local = 0;
+    for (int sh = s0; sh < s1; sh++) {
+      const int nm = 2 * S.shell_l[sh] + 1;
+      if (s_act_mask[s] >> (sh - s0) & 1u)
+        for (int m = 0; m < nm; m++, row++) {
+          L.fn_index[fo + row] = S.atom_fn_ptr[a] + local + m;
+          L.fn_info[fo + row] = (s << 16) | (local + m);
+        }
+      local += nm;
+    }
+  }
+  for (int q = tid; q < nact * nact; q += 256) {
+    const int sa = q / nact, sb = q - sa * nact;
+    const int A = s_act_atom[min(sa, sb)], B = s_act_atom[max(sa, sb)];
+    long long lo2 = S.row_ptr[A], hi2 = S.row_ptr[A + 1] - 1, found = -1;
+    while (lo2 <= hi2) {
+      long long mid = (lo2 + hi2) >> 1;
+      int cb = S.col_atom[mid];
+      if (cb == B) { found = S.blk_off[mid]; break; }
+      if (cb < B) lo2 = mid + 1; else hi2 = mid - 1;
+    }
+    L.ptab[po + q] = found;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Real solid harmonics S_lm (orthonormal real Y_lm on the unit sphere, m = -l..l, no Condon-Shortley phase)
+// and their Cartesian gradients, l <= 3, as explicit polynomials with literal constants.
+// ---------------------------------------------------------------------------------------------------------------
+template <bool GRAD>
+__device__ __forceinline__ void solid_harmonics(int l, double x, double y, double z, double *Y, double *gx, double *gy,
+                                                double *gz) {
+  if (l == 0) {
+    Y[0] = 0.28209479177387814;
+    if (GRAD) { gx[0] = 0.0; gy[0] = 0.0; gz[0] = 0.0; }
+  } else if (l == 1) {
+    const double c = 0.4886025119029199;
+    Y[0] = c * y; Y[1] = c * z; Y[2] = c * x;
+    if (GRAD) {
+      gx[0] = 0.0; gy[0] = c;   gz[0] = 0.0;
+      gx[1] = 0.0; gy[1] = 0.0; gz[1] = c;
+      gx[2] = c;   gy[2] = 0.0; gz[2] = 0.0;
+    }
+  } else if (l == 2) {
+    const double a = 1.0925484305920792, bq = 0.31539156525252005, c = 0.5462742152960396;
+    const double xx = x * x, yy = y * y, zz = z * z;
+    Y[0] = a * (x * y);
+    Y[1] = a * (y * z);
+    Y[2] = bq * (2.0 * zz - xx - yy);
+    Y[3] = a * (x * z);
+    Y[4] = c * (xx - yy);
+    if (GRAD) {
+      gx[0] = a * y;          gy[0] = a * x;          gz[0] = 0.0;
+      gx[1] = 0.0;            gy[1] = a * z;          gz[1] = a * y;
+      gx[2] = -2.0 * bq * x;  gy[2] = -2.0 * bq * y;  gz[2] = 4.0 * bq * z;
+      gx[3] = a * z;          gy[3] = 0.0;            gz[3] = a * x;
+      gx[4] = 2.0 * c * x;    gy[4] = -2.0 * c * y;   gz[4] = 0.0;
+    }
+  } else {
+    const double a = 0.5900435899266435, bq = 2.890611442640554, c = 0.4570457994644658, d = 0.3731763325901154,
+                 e = 1.445305721320277;
+    const double xx = x * x, yy = y * y, zz = z * z;
+    const double q = 4.0 * zz - xx - yy;
+    Y[0] = a * y * (3.0 * xx - yy);
+    Y[1] = bq * x * y * z;
+    Y[2] = c * y * q;
+    Y[3] = d * z * (2.0 * zz - 3.0 * xx - 3.0 * yy);
+    Y[4] = c * x * q;
+    Y[5] = e * z * (xx - yy);
+    Y[6] = a * x * (xx - 3.0 * yy);
+    if (GRAD) {
+      gx[0] = 6.0 * a * x * y;          gy[0] = 3.0 * a * (xx - yy);      gz[0] = 0.0;
+      gx[1] = bq * y * z;               gy[1] = bq * x * z;               gz[1] = bq * x * y;
+      gx[2] = -2.0 * c * x * y;         gy[2] = c * (q - 2.0 * yy);       gz[2] = 8.0 * c * y * z;
+      gx[3] = -6.0 * d * x * z;         gy[3] = -6.0 * d * y * z;         gz[3] = 3.0 * d * (2.0 * zz - xx - yy);
+      gx[4] = c * (q - 2.0 * xx);       gy[4] = -2.0 * c * x * y;         gz[4] = 8.0 * c * x * z;
+      gx[5] = 2.0 * e * x * z;          gy[5] = -2.0 * e * y * z;         gz[5] = e * (xx - yy);
+      gx[6] = 3.0 * a * (xx - yy);      gy[6] = -6.0 * a * x * y;         gz[6] = 0.0;
+    }
+  }
+}
+
+// Output modes of k_eval
+enum EvalMode {
+  kEvalPhi = 0,      // plane0 = Phi                                   (density, LDA; API without gradient)
+  kEvalPhiGrad = 1,  // plane0 = Phi, planes 1..3 = d/dx, d/dy, d/dz   (density with grad n; API with gradient)
+  kEvalHLda = 2,     // plane0 = Phi, plane1 = w v Phi                 (S2a fused: Eq. 25 "K = w phi" times v)
+  kEvalHGga = 3      // plane0 = Phi, plane1 = w (v/2 Phi + g . grad Phi)
+};
+
+struct EvalArgs {
+  double *plane[4];
+  // internal layout: element (row, p) of batch b at plane[q] + (pad_off[b] - pad_base) + row*ld + p, ld = round_up(np, kPadPts)
+  const long long *pad_off;
+  long long pad_base;
+  // API layout (api != 0): phi at plane[0] + (api_off[b]-api_base) + row*np + p,
+  //                        dphi component c at plane[1] + 3*(api_off[b]-api_base) + (c*nnz + row)*np + p
+  const long long *api_off;
+  long long api_base;
+  int api;
+  const double *v, *g;   // [n_points], [3][n_points]
+  long long n_points;
+};
+
+// ---------------------------------------------------------------------------------------------------------------
+// k_eval: one CTA per batch, one thread per point (columns beyond n_p up to the padded leading dimension get zeros).
+// For each active atom: geometry and log once per point, solid harmonics once per l, one spline Horner per shell.
+// Stores are coalesced along the point index.
+// ---------------------------------------------------------------------------------------------------------------
+template <int MODE>
+__global__ void __launch_bounds__(256) k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first) {
+  constexpr bool GRAD = (MODE == kEvalPhiGrad || MODE == kEvalHGga);
+  const int b = b_first + blockIdx.x;
+  const int tid = threadIdx.x;
+  const long long p0 = S.batch_ptr[b];
+  const int np = (int)(S.batch_ptr[b + 1] - p0);
+  const int nnz = L.nnz[b], nact = L.n_act[b];
+  if (nnz == 0 || np == 0) return;
+  const long long ao = L.act_off[b];
+
+  __shared__ double s_ax[kMaxActive], s_ay[kMaxActive], s_az[kMaxActive];
+  __shared__ int s_s0[kMaxActive], s_s1[kMaxActive], s_row0[kMaxActive];
+  __shared__ unsigned s_mask[kMaxActive];
+  for (int s = tid; s < nact; s += 256) {
+    const int a = L.act_atom[ao + s];
+    s_ax[s] = S.atom_xyz[3 * a]; s_ay[s] = S.atom_xyz[3 * a + 1]; s_az[s] = S.atom_xyz[3 * a + 2];
+    const int sp = S.atom_species[a];
+    s_s0[s] = S.sp_shell_ptr[sp]; s_s1[s] = S.sp_shell_ptr[sp + 1];
+    s_row0[s] = L.act_row0[ao + s];
+    s_mask[s] = L.act_mask[ao + s];
+  }
+  __syncthreads();
+
+  const int ld = E.api ? np : round_up(np, kPadPts);
+  double *o0, *o1, *o2 = nullptr, *o3 = nullptr;
+  long long cstride = 0;  // distance between gradient components (API layout) -- internal layout uses separate planes
+  if (E.api) {
+    const long long off = E.api_off[b] - E.api_base;
+    o0 = E.plane[0] + off;
+    o1 = E.plane[1] ? E.plane[1] + 3 * off : nullptr;
+    cstride = (long long)nnz * np;
+    if (GRAD) { o2 = o1 + cstride; o3 = o2 + cstride; }
+  } else {
+    const long long off = E.pad_off[b] - E.pad_base;
+    o0 = E.plane[0] + off;
+    o1 = E.plane[1] + off;
+    if (MODE == kEvalPhiGrad) { o2 = E.plane[2] + off; o3 = E.plane[3] + off; }
+  }
+  const int nk1 = S.n_knots - 1;
+
+  for (int p = tid; p < ld; p += 256) {
+    if (p >= np) {  // zero padding columns (internal layout only)
+      for (int r = 0; r < nnz; r++) {
+        o0[(long long)r * ld + p] = 0.0;
+        if (MODE != kEvalPhi) o1[(long long)r * ld + p] = 0.0;
+        if (MODE == kEvalPhiGrad) { o2[(long long)r * ld + p] = 0.0; o3[(long long)r * ld + p] = 0.0; }
+      }
+      continue;
+    }
+    const double x = S.px[p0 + p], y = S.py[p0 + p], z = S.pz[p0 + p];
+    double wv = 0.0, wgx = 0.0, wgy = 0.0, wgz = 0.0;
+    if (MODE == kEvalHLda) wv = S.w[p0 + p] * E.v[p0 + p];
+    if (MODE == kEvalHGga) {
+      const double w = S.w[p0 + p];
+      wv = 0.5 * w * E.v[p0 + p];
+      wgx = w * E.g[p0 + p]; wgy = w * E.g[E.n_points + p0 + p]; wgz = w * E.g[2 * E.n_points + p0 + p];
+    }
+    for (int s = 0; s < nact; s++) {
+      const double dx = x - s_ax[s], dy = y - s_ay[s], dz = z - s_az[s];
+      const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+      const double d = sqrt(d2);
+      double ux = 0.0, uy = 0.0, uz = 1.0;
+      if (d > 0.0) { const double inv = 1.0 / d; ux = dx * inv; uy = dy * inv; uz = dz * inv; }
+      const double dd = fmax(d, S.r0);
+      const double t = log(dd / S.r0) / S.log_inc;
+      int k = (int)floor(t);
+      k = max(0, min(k, S.n_knots - 2));
+      const double xs = t - (double)k;
+      const double inv_dd = 1.0 / dd;
+      const unsigned mask = s_mask[s];
+      long long row = s_row0[s];
+      int lcur = -1;
+      double Y[7], gx[7], gy[7], gz[7];
+      for (int sh = s_s0[s]; sh < s_s1[s]; sh++) {
+        if (!(mask >> (sh - s_s0[s]) & 1u)) continue;
+        const int l = S.shell_l[sh];
+        const int nm = 2 * l + 1;
+        if (d2 < S.shell_rc2[sh]) {
+          if (l != lcur) { solid_harmonics<GRAD>(l, ux, uy, uz, Y, gx, gy, gz); lcur = l; }
+          const double2 *cf = reinterpret_cast<const double2 *>(S.spline_coef + ((long long)S.shell_spline[sh] * nk1 + k) * 4);
+          const double2 c01 = __ldg(cf), c23 = __ldg(cf + 1);
+          const double R = c01.x + xs * (c01.y + xs * (c23.x + xs * c23.y));
+          double f = 0.0, Rd = 0.0;
+          if (GRAD) {
+            const double dR = (c01.y + xs * (2.0 * c23.x + xs * 3.0 * c23.y)) / (S.log_inc * dd);
+            Rd = R * inv_dd;
+            f = dR - (double)l * Rd;
+          }
+#pragma unroll
+          for (int m = 0; m < 7; m++) {
+            if (m < nm) {
+              const double phi = R * Y[m];
+              const long long o = (row + m) * ld + p;
+              o0[o] = phi;
+              if (MODE == kEvalHLda) o1[o] = wv * phi;
+              if (GRAD) {
+                const double fy = f * Y[m];
+                const double ex = fy * ux + Rd * gx[m], ey = fy * uy + Rd * gy[m], ez = fy * uz + Rd * gz[m];
+                if (MODE == kEvalPhiGrad) { o1[o] = ex; o2[o] = ey; o3[o] = ez; }
+                else o1[o] = wv * phi + (wgx * ex + wgy * ey + wgz * ez);
+              }
+            }
+          }
+        } else {
+          for (int m = 0; m < nm; m++) {
+            const long long o = (row + m) * ld + p;
+            o0[o] = 0.0;
+            if (MODE != kEvalPhi) o1[o] = 0.0;
+            if (MODE == kEvalPhiGrad) { o2[o] = 0.0; o3[o] = 0.0; }
+          }
+        }
+        row += nm;
+      }
+    }
+  }
+}
+
+// copy the per-batch lists of [b0,b1) into caller arrays (aims_gpu_eval_basis outputs)
+__global__ void k_export_lists(BatchLists L, DevSys S, int b0, int b1, long long *fn_ptr, int *fn_index, long long *phi_ptr,
+                               const long long *api_off) {
+  const int k = blockIdx.x;        // batch b0+k; block b1-b0 writes the final pointers
+  const int b = b0 + k;
+  if (b == b1) {
+    if (threadIdx.x == 0) { fn_ptr[k] = L.fn_off[b1] - L.fn_off[b0]; phi_ptr[k] = api_off[b1] - api_off[b0]; }
+    return;
+  }
+  const long long fo = L.fn_off[b], base = L.fn_off[b0];
+  if (threadIdx.x == 0) { fn_ptr[k] = fo - base; phi_ptr[k] = api_off[b] - api_off[b0]; }
+  const int nnz = L.nnz[b];
+  for (int i = threadIdx.x; i < nnz; i += blockDim.x) fn_index[fo - base + i] = L.fn_index[fo + i];
+}
+
+}  // namespace aims
