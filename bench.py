@@ -1,0 +1,360 @@
+#!/usr/bin/env python
+"""bench.py -- grid points/s for H integration + density update (FP64) on the 375-atom Bi2Se3-shaped slab.
+
+One "step" = one pass of the whole hot path over the whole grid: aims_gpu_integrate_hamiltonian (GGA) followed by
+aims_gpu_update_density (with grad n), each including its own culling and basis evaluation.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1..5]
+
+N > 1 (torchrun): contiguous batch ranges balanced by n_p*nnz^2 are sharded over the ranks; each rank adds its
+partial H (Eq. 28) and the partial sums are combined by ONE NCCL all-reduce (Eq. 29, "the only communication
+step"); the density needs none (L312).  Total work is fixed -> "scaling": "strong".
+
+--impl reference times the CPU oracle (oracle/) on a bounded seeded sample of the same workload (rank 0 only).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "grid points/s for H integration + density update (FP64); % of FP64 peak"
+UNIT = "points/s"
+# FP64 peak of the B200 tensor pipe from unit counts and clocks: 148 SMs x 64 FMA/clk x 2 x
+# 1.965 GHz; the DMMA-chain probe (aims_gpu_fp64_peak) measures 37.2 TFLOP/s on this pool, i.e. exactly this number.
+FP64_PEAK_NOMINAL_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+
+WORKLOADS = {
+    1: "config1: 3-atom molecule, 13,200 points, batches <=128, GGA",
+    2: "config2: 64-atom Si-like cluster, 1,159,680 points, batches <=200, LDA",
+    3: "config3: 64-atom Si-like cluster, 1,159,680 points, batches <=200, GGA",
+    4: "config4: 200-atom two-species slab, 3,624,000 points, batches <=200, GGA",
+    5: "config5: 375-atom Bi2Se3-shaped slab (3 QL x 5x5), 7,927,500 points, batches <=200, GGA",
+}
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=5)
+    ap.add_argument("--max-batch", type=int, default=None)
+    ap.add_argument("--n-rad", type=int, default=None, help="debug: coarser grid (not the benchmark workload)")
+    ap.add_argument("--n-ang", type=int, default=None)
+    ap.add_argument("--cpu-sample-batches", type=int, default=96)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def partition_batches(cost, n_parts):
+    """Contiguous ranges [lo, hi) of (almost) equal total cost; cost[b] >= 0.  Pure host logic (tested on CPU)."""
+    nb = len(cost)
+    csum = np.concatenate([[0.0], np.cumsum(np.asarray(cost, dtype=np.float64))])
+    bounds = [0]
+    for r in range(1, n_parts):
+        target = csum[-1] * r / n_parts
+        bounds.append(int(np.clip(np.searchsorted(csum, target, side="left"), bounds[-1], nb)))
+    bounds.append(nb)
+    return [(bounds[r], bounds[r + 1]) for r in range(n_parts)]
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.rows = []
+        self.proc = None
+        self.idx = gpu_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.idx), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), [x.strip() for x in line.split(",")]))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        rows = [r for (t, r) in self.rows if t0 <= t <= t1 + 0.3] or [r for (_, r) in self.rows]
+        sm, smax, reasons = [], [], set()
+        for r in rows:
+            try:
+                sm.append(float(r[1]))
+                smax.append(float(r[2]))
+            except Exception:
+                continue
+            for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(smax)), "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def sample_batches(n_batches, k, seed=20191206):
+    rng = np.random.default_rng(seed)
+    return np.sort(rng.choice(n_batches, size=min(k, n_batches), replace=False)).astype(np.int32)
+
+
+def time_oracle(bun, batches, gga, repeats=1):
+    """Oracle as it stands on the host cores: H integration + density update on the listed batches."""
+    from oracle import oracle as orc
+    o = orc.Oracle(bun)
+    pts = int(sum(bun.batch_ptr[b + 1] - bun.batch_ptr[b] for b in batches))
+    best = None
+    for _ in range(repeats):
+        t0 = time.perf_counter()
+        o.integrate_hamiltonian(bun.v, bun.g if gga else None, batches=batches)
+        o.update_density(bun.D_values, want_grad=gga, batches=batches)
+        dt = time.perf_counter() - t0
+        best = dt if best is None else min(best, dt)
+    return pts, best, orc.num_threads()
+
+
+def run_reference(args, bun, gga, workload):
+    """--impl reference: the CPU oracle, rank 0 only, a bounded sample per step."""
+    per_step = max(4, args.cpu_sample_batches // 4)
+    times, pts_step = [], 0
+    for s in range(args.warmup + args.steps):
+        sel = sample_batches(bun.n_batches, per_step, seed=1000 + s)
+        pts, dt, cores = time_oracle(bun, sel, gga)
+        if s >= args.warmup:
+            times.append(dt)
+            pts_step += pts
+    total = sum(times)
+    val = pts_step / total
+    sample = "%d seeded batches per step (about %d points) of %s" % (per_step, pts_step // max(args.steps, 1), workload)
+    out = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": 1e3 * total / max(args.steps, 1), "higher_is_better": True,
+           "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": workload, "sample": sample},
+           "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+           "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out))
+
+
+def main():
+    args = parse()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    gga = args.config != 2
+    workload = WORKLOADS[args.config]
+    if args.max_batch:
+        workload += " (max batch %d)" % args.max_batch
+    if args.n_rad or args.n_ang:
+        workload += " [DEBUG GRID n_rad=%s n_ang=%s: not the benchmark workload]" % (args.n_rad, args.n_ang)
+
+    import aims_synth
+    if args.impl == "reference":
+        if rank != 0:
+            return 0
+        bun = aims_synth.make_config(args.config, n_rad=args.n_rad, n_ang=args.n_ang, max_batch=args.max_batch)
+        run_reference(args, bun, gga, workload)
+        return 0
+
+    import torch
+    import torch.distributed as dist
+    import paper_1912_06636_b200 as aims
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    t_gen = time.time()
+    bun = aims_synth.make_config(args.config, n_rad=args.n_rad, n_ang=args.n_ang, max_batch=args.max_batch)
+    t_gen = time.time() - t_gen
+    stream = torch.cuda.Stream(device=local_rank)
+    t_create = time.time()
+    ctx = aims.aims_gpu_create(bun, device=local_rank, stream=stream)
+    t_create = time.time() - t_create
+    st = ctx.stats()
+    nnz = ctx.batch_nnz().astype(np.float64)
+    npb = np.diff(bun.batch_ptr).astype(np.float64)
+    cost = npb * nnz * nnz
+    b0, b1 = partition_batches(cost, world)[rank]
+    my_points = int(bun.batch_ptr[b1] - bun.batch_ptr[b0])
+    flops_h = float(((2.0 if gga else 1.0) * npb * nnz * (nnz + (0.0 if gga else 1.0)))[b0:b1].sum())
+    flops_n = float((2.0 * npb * nnz * nnz)[b0:b1].sum())
+
+    with torch.cuda.stream(stream):
+        v = torch.as_tensor(bun.v).to("cuda", non_blocking=False)
+        g = torch.as_tensor(bun.g).to("cuda") if gga else None
+        D = torch.as_tensor(bun.D_values).to("cuda")
+        H = torch.empty(bun.n_values, dtype=torch.float64, device="cuda")
+        n = torch.zeros(bun.n_points, dtype=torch.float64, device="cuda")
+        gn = torch.zeros((3, bun.n_points), dtype=torch.float64, device="cuda") if gga else None
+    stream.synchronize()
+
+    def step():
+        with torch.cuda.stream(stream):
+            ctx.integrate_hamiltonian(v, g, H=H, b0=b0, b1=b1, accumulate=False)
+            if world > 1:
+                dist.all_reduce(H)                        # Eq. 29: the only communication step
+            ctx.update_density(D, want_grad=gga, n=n, grad_n=gn, b0=b0, b1=b1)
+
+    def barrier():
+        stream.synchronize()
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+
+    peak_measured = ctx.fp64_peak(200.0)
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    ctx.synchronize()
+
+    # ---- timed region: exactly K steps, CUDA events on the launching stream, clocks sampled meanwhile
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    time.sleep(0.3)
+    ctx.timing_enable(True)
+    launches0 = ctx.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    tw0 = time.time()
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    barrier()
+    tw1 = time.time()
+    ms_total = e0.elapsed_time(e1)
+    kern = ctx.timing_read()
+    ctx.timing_enable(False)
+    launches = ctx.launch_count() - launches0
+    clocks = sampler.stop(tw0, tw1)
+    if world > 1:
+        t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+        lt = torch.tensor([launches], dtype=torch.int64, device="cuda")
+        dist.all_reduce(lt)
+        launches = int(lt.item())
+    ms_step = ms_total / args.steps
+    value = bun.n_points / (ms_step * 1e-3)
+
+    # ---- e2e: same step through the binding with pinned HOST buffers, copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        hb, dv = ctx.make_host_buffers(gga)
+        hb["v"].copy_(torch.as_tensor(bun.v))
+        hb["D"].copy_(torch.as_tensor(bun.D_values))
+        if gga:
+            hb["g"].copy_(torch.as_tensor(bun.g))
+
+        def step_e2e():
+            with torch.cuda.stream(stream):
+                dv["v"].copy_(hb["v"], non_blocking=True)
+                dv["D"].copy_(hb["D"], non_blocking=True)
+                if gga:
+                    dv["g"].copy_(hb["g"], non_blocking=True)
+                ctx.integrate_hamiltonian(dv["v"], dv["g"] if gga else None, H=dv["H"], b0=b0, b1=b1, accumulate=False)
+                if world > 1:
+                    dist.all_reduce(dv["H"])
+                ctx.update_density(dv["D"], want_grad=gga, n=dv["n"], grad_n=dv.get("grad_n"), b0=b0, b1=b1)
+                hb["H"].copy_(dv["H"], non_blocking=True)
+                lo, hi = int(bun.batch_ptr[b0]), int(bun.batch_ptr[b1])
+                hb["n"][lo:hi].copy_(dv["n"][lo:hi], non_blocking=True)
+                if gga:
+                    hb["grad_n"][:, lo:hi].copy_(dv["grad_n"][:, lo:hi], non_blocking=True)
+        step_e2e()
+        barrier()
+        k2 = max(2, min(args.steps, 3))
+        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        f0.record(stream)
+        for _ in range(k2):
+            step_e2e()
+        f1.record(stream)
+        barrier()
+        ms_e = f0.elapsed_time(f1) / k2
+        if world > 1:
+            t = torch.tensor([ms_e], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms_e = float(t.item())
+        h2d = 8 * (bun.n_points + bun.n_values + (3 * bun.n_points if gga else 0))
+        d2h = 8 * (bun.n_values + my_points * (4 if gga else 1))
+        e2e = {"value": bun.n_points / (ms_e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+               "d2h_bytes_per_step": int(d2h), "ms_per_step": ms_e}
+        # the end-to-end outputs are the same numbers as the device-resident ones
+        assert torch.equal(hb["n"][int(bun.batch_ptr[b0]):int(bun.batch_ptr[b1])],
+                           n[int(bun.batch_ptr[b0]):int(bun.batch_ptr[b1])].cpu())
+
+    # ---- roofline of the dominant kernel (FP64 tensor pipe), live CUDA-event durations from the timed region
+    kflops = {"k_hamiltonian": flops_h, "k_density": flops_n}
+    dom = max(kflops, key=lambda k: kern[k][0])
+    kd = {}
+    for k in ("k_cull", "k_eval", "k_hamiltonian", "k_density"):
+        ms, ln = kern[k]
+        kd[k] = {"ms_per_step": ms / args.steps, "launches_per_step": ln / args.steps}
+        if k in kflops and ms > 0:
+            kd[k]["tflops"] = kflops[k] * args.steps / (ms * 1e-3) / 1e12
+    dom_ms, dom_ln = kern[dom]
+    achieved = kflops[dom] * args.steps / (dom_ms * 1e-3) / 1e12
+    roofline = {"bound": "tensor", "kernel": dom, "achieved": achieved, "peak": FP64_PEAK_NOMINAL_TFLOPS,
+                "unit": "TFLOP/s", "frac": achieved / FP64_PEAK_NOMINAL_TFLOPS, "traffic": None,
+                "peak_source": "FP64 DMMA pipe: 148 SM x 64 FMA/clk x 2 x 1.965 GHz (unit counts x max clock); the "
+                               "in-run DMMA-chain probe measured %.2f TFLOP/s" % peak_measured,
+                "peak_measured_probe": peak_measured, "frac_of_measured_probe": achieved / peak_measured,
+                "avg_launch_ms": dom_ms / max(dom_ln, 1), "algorithmic_flops_per_step": kflops[dom],
+                "share_of_step": dom_ms / ms_total}
+    total_tflops = (flops_h + flops_n) / (ms_step * 1e-3) / 1e12
+
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+           "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
+           "data": "synthetic",
+           "config": {"workload": workload, "n_points": bun.n_points, "n_batches": bun.n_batches, "n_basis": bun.n_basis,
+                      "mean_nnz": float(nnz.mean()) if len(nnz) else 0.0, "max_nnz": st["max_nnz"],
+                      "max_active_atoms": st["max_active_atoms"], "parallelism": "batch-range x%d" % world,
+                      "l2": "inputs larger than L2: each step streams %.1f GB of Phi planes plus a %.2f GB H and D"
+                            % (8e-9 * 6 * st["sum_nnz"] * 208, 8e-9 * bun.n_values)},
+           "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
+           "fp64_tflops_step": total_tflops, "fp64_frac_of_peak_step": total_tflops / FP64_PEAK_NOMINAL_TFLOPS,
+           "kernels": kd, "setup_s": {"generate_inputs": t_gen, "create_ctx": t_create}}
+
+    # ---- CPU baseline: the oracle on a bounded seeded sample, rank 0 at N=1 only
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        sel = sample_batches(bun.n_batches, args.cpu_sample_batches)
+        pts, dt, cores = time_oracle(bun, sel, gga)
+        out["cpu_baseline"] = {"value": pts / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+                               "sample": "%d seeded batches (%d points) of the same workload, %.1f s" % (len(sel), pts, dt)}
+    else:
+        out["cpu_baseline"] = None
+    if rank == 0:
+        print(json.dumps(out))
+    ctx.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

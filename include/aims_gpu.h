@@ -134,6 +134,17 @@ int aims_gpu_synchronize(aims_gpu_ctx *ctx);
 int aims_gpu_stats(aims_gpu_ctx *ctx, int64_t *sum_nnz, int32_t *max_nnz, int32_t *max_active_atoms,
                    double *flops_h_lda, double *flops_h_gga, double *flops_density);
 
+/* |nnz(B)| of every batch as found at creation (HOST output, [n_batches]); used to balance batch ranges over GPUs. */
+int aims_gpu_batch_nnz(aims_gpu_ctx *ctx, int32_t *nnz);
+
+/* Per-kernel device timing for bench.py's roofline: when enabled, every kernel launch of this context is bracketed by
+ * CUDA events on the context stream.  aims_gpu_timing_enable synchronises, clears what was recorded and switches
+ * recording on (enable != 0) or off.  aims_gpu_timing_read synchronises and returns, since the last enable/read, the
+ * summed device milliseconds ms[5] and launch counts launches[5] (HOST outputs) of
+ *   [0] k_cull  [1] k_eval  [2] k_hamiltonian  [3] k_density  [4] other. */
+int aims_gpu_timing_enable(aims_gpu_ctx *ctx, int enable);
+int aims_gpu_timing_read(aims_gpu_ctx *ctx, double *ms, int64_t *launches);
+
 /* Number of kernels this context has launched since creation (for bench.py's gpu_launches). */
 int64_t aims_gpu_launch_count(const aims_gpu_ctx *ctx);
 

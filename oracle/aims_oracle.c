@@ -57,6 +57,14 @@ typedef struct {
   int64_t n_values;
 } orc_system;
 
+/* number of OpenMP threads the batch loops use (reported by bench.py's cpu_baseline; no arithmetic) */
+#ifdef _OPENMP
+#include <omp.h>
+int orc_num_threads(void) { return omp_get_max_threads(); }
+#else
+int orc_num_threads(void) { return 1; }
+#endif
+
 /* ------------------------------------------------------------------ real spherical harmonics (reading P10)
  * S_lm: homogeneous polynomial of degree l with S_lm(u) = Y_lm(u) on the unit sphere; orthonormal real harmonics,
  * m = -l..l, no Condon-Shortley phase.  Y[m+l]; if gS != NULL also gS[m+l][3] = grad S_lm at (x,y,z). */

@@ -72,6 +72,12 @@ def _l(a):
     return a.ctypes.data_as(_lp)
 
 
+def num_threads():
+    L = _load()
+    L.orc_num_threads.restype = ctypes.c_int
+    return int(L.orc_num_threads())
+
+
 def solid_harmonics(l, u, want_grad=False):
     """Y[2l+1] (and grad S_lm [2l+1][3]) at the 3-vector u (O1, reading P10)."""
     u = np.ascontiguousarray(u, dtype=np.float64)

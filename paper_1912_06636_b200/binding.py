@@ -81,6 +81,12 @@ def load_library():
     L.aims_gpu_update_density.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp, _vp]
     L.aims_gpu_synchronize.restype = ctypes.c_int
     L.aims_gpu_synchronize.argtypes = [cp]
+    L.aims_gpu_batch_nnz.restype = ctypes.c_int
+    L.aims_gpu_batch_nnz.argtypes = [cp, _ip]
+    L.aims_gpu_timing_enable.restype = ctypes.c_int
+    L.aims_gpu_timing_enable.argtypes = [cp, ctypes.c_int]
+    L.aims_gpu_timing_read.restype = ctypes.c_int
+    L.aims_gpu_timing_read.argtypes = [cp, _dp, _lp]
     L.aims_gpu_stats.restype = ctypes.c_int
     L.aims_gpu_stats.argtypes = [cp, _lp, _ip, _ip, _dp, _dp, _dp]
     L.aims_gpu_launch_count.restype = ctypes.c_int64
@@ -160,6 +166,22 @@ class Context:
 
     def synchronize(self):
         self._check(self.L.aims_gpu_synchronize(self.h), "aims_gpu_synchronize")
+
+    def batch_nnz(self):
+        out = np.zeros(max(self.n_batches, 1), dtype=np.int32)
+        self._check(self.L.aims_gpu_batch_nnz(self.h, out.ctypes.data_as(_ip)), "aims_gpu_batch_nnz")
+        return out[:self.n_batches]
+
+    def timing_enable(self, enable=True):
+        self._check(self.L.aims_gpu_timing_enable(self.h, int(bool(enable))), "aims_gpu_timing_enable")
+
+    def timing_read(self):
+        """{kernel: (device ms, launches)} since the last enable/read."""
+        ms = (ctypes.c_double * 5)()
+        ln = (ctypes.c_int64 * 5)()
+        self._check(self.L.aims_gpu_timing_read(self.h, ms, ln), "aims_gpu_timing_read")
+        names = ("k_cull", "k_eval", "k_hamiltonian", "k_density", "other")
+        return {k: (ms[i], int(ln[i])) for i, k in enumerate(names)}
 
     def launch_count(self):
         return int(self.L.aims_gpu_launch_count(self.h))

@@ -41,7 +41,15 @@ struct aims_gpu_ctx {
 
   double *ws = nullptr;      // Phi-plane workspace
   long long ws_doubles = 0;
+
+  // optional per-kernel timing (CUDA events on the context stream around every launch)
+  bool timing = false;
+  struct Span { cudaEvent_t e0, e1; int kind; };
+  std::vector<Span> spans;       // recorded since the last read
+  std::vector<Span> pool;        // reusable events
 };
+
+enum { kKindCull = 0, kKindEval = 1, kKindHam = 2, kKindDen = 3, kKindOther = 4, kNumKinds = 5 };
 
 namespace {
 
@@ -82,6 +90,26 @@ int check_async(aims_gpu_ctx *c) {
   return AIMS_OK;
 }
 
+// Brackets one kernel launch with events when timing is on; always counts the launch.
+struct TimedLaunch {
+  aims_gpu_ctx *c;
+  aims_gpu_ctx::Span sp{};
+  bool on;
+  TimedLaunch(aims_gpu_ctx *ctx, int kind) : c(ctx), on(ctx->timing) {
+    c->launches++;
+    if (!on) return;
+    if (!c->pool.empty()) { sp = c->pool.back(); c->pool.pop_back(); }
+    else if (cudaEventCreate(&sp.e0) != cudaSuccess || cudaEventCreate(&sp.e1) != cudaSuccess) { on = false; return; }
+    sp.kind = kind;
+    cudaEventRecord(sp.e0, c->stream);
+  }
+  ~TimedLaunch() {
+    if (!on) return;
+    cudaEventRecord(sp.e1, c->stream);
+    c->spans.push_back(sp);
+  }
+};
+
 __global__ void k_fp64_peak(double *out, int iters, double a, double b) {
   double c0[16], c1[16];
 #pragma unroll
@@ -110,6 +138,8 @@ int aims_gpu_destroy(aims_gpu_ctx *ctx) {
   cudaSetDevice(ctx->device);
   cudaError_t e = cudaStreamSynchronize(ctx->stream);
   for (void *p : ctx->owned) cudaFree(p);
+  for (auto &sp : ctx->spans) { cudaEventDestroy(sp.e0); cudaEventDestroy(sp.e1); }
+  for (auto &sp : ctx->pool) { cudaEventDestroy(sp.e0); cudaEventDestroy(sp.e1); }
   delete ctx;
   return e == cudaSuccess ? AIMS_OK : AIMS_ERR_CUDA;
 }
@@ -226,8 +256,7 @@ int aims_gpu_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_gri
   if ((rc = dev_alloc(c, &L.error_flag, 1))) return rc;
   CU_TRY(c, cudaMemsetAsync(L.error_flag, 0, sizeof(int), c->stream));
   if (nb) {
-    k_cull<<<nb, 256, 0, c->stream>>>(S, L, 0, 1);
-    c->launches++;
+    { TimedLaunch t(c, kKindCull); k_cull<<<nb, 256, 0, c->stream>>>(S, L, 0, 1); }
     if ((rc = check_async(c))) return rc;
   }
   c->nnz.resize(nb); c->n_act.resize(nb);
@@ -331,6 +360,12 @@ int aims_gpu_stats(aims_gpu_ctx *c, int64_t *sum_nnz, int32_t *max_nnz, int32_t 
   return AIMS_OK;
 }
 
+int aims_gpu_batch_nnz(aims_gpu_ctx *c, int32_t *nnz) {
+  if (!c || !nnz) return AIMS_ERR_INVALID_ARG;
+  std::copy(c->nnz.begin(), c->nnz.end(), nnz);
+  return AIMS_OK;
+}
+
 int aims_gpu_basis_sizes(aims_gpu_ctx *c, int32_t b0, int32_t b1, int64_t *n_index, int64_t *n_phi) {
   if (!range_ok(c, b0, b1)) return fail(c, AIMS_ERR_INVALID_ARG, "batch range outside [0, n_batches]");
   if (n_index) *n_index = c->fn_off[b1] - c->fn_off[b0];
@@ -345,8 +380,8 @@ namespace {
 // S1a for batches [b0,b1): rebuilds every per-batch list on the device (part of each hot call)
 int run_cull(aims_gpu_ctx *c, int b0, int b1) {
   if (b1 > b0) {
+    TimedLaunch t(c, kKindCull);
     k_cull<<<b1 - b0, 256, 0, c->stream>>>(c->S, c->L, b0, 0);
-    c->launches++;
   }
   return check_async(c);
 }
@@ -364,8 +399,8 @@ int chunk_end(const aims_gpu_ctx *c, int bs, int b1, int nplanes) {
 
 template <int MODE>
 void launch_eval(aims_gpu_ctx *c, const EvalArgs &E, int bs, int be) {
+  TimedLaunch t(c, kKindEval);
   k_eval<MODE><<<be - bs, 256, 0, c->stream>>>(c->S, c->L, E, bs);
-  c->launches++;
 }
 
 }  // namespace
@@ -379,8 +414,8 @@ int aims_gpu_eval_basis(aims_gpu_ctx *c, int32_t b0, int32_t b1, int64_t *fn_ptr
   CU_TRY(c, cudaSetDevice(c->device));
   int rc = run_cull(c, b0, b1);
   if (rc) return rc;
-  k_export_lists<<<b1 - b0 + 1, 128, 0, c->stream>>>(c->L, c->S, b0, b1, (long long *)fn_ptr, fn_index, (long long *)phi_ptr, c->d_api_off);
-  c->launches++;
+  { TimedLaunch t(c, kKindOther);
+    k_export_lists<<<b1 - b0 + 1, 128, 0, c->stream>>>(c->L, c->S, b0, b1, (long long *)fn_ptr, fn_index, (long long *)phi_ptr, c->d_api_off); }
   if (b1 > b0) {
     EvalArgs E{};
     E.plane[0] = phi; E.plane[1] = dphi;
@@ -410,9 +445,9 @@ int aims_gpu_integrate_hamiltonian(aims_gpu_ctx *c, int32_t b0, int32_t b1, cons
     const long long nt = c->tile_off[be] - c->tile_off[bs];
     if (nt > 0) {
       HArgs A{c->d_tiles + c->tile_off[bs], E.plane[0], E.plane[1], c->d_pad_off, c->pad_off[bs], H_values};
+      TimedLaunch t(c, kKindHam);
       if (g) k_hamiltonian<true><<<(unsigned)nt, kHThreads, h_smem_bytes<true>(), c->stream>>>(c->S, c->L, A);
       else k_hamiltonian<false><<<(unsigned)nt, kHThreads, h_smem_bytes<false>(), c->stream>>>(c->S, c->L, A);
-      c->launches++;
     }
     if ((rc = check_async(c))) return rc;
     bs = be;
@@ -445,13 +480,39 @@ int aims_gpu_update_density(aims_gpu_ctx *c, int32_t b0, int32_t b1, const doubl
       for (int q = 0; q < 3; q++) A.G[q] = grad_n ? E.plane[q + 1] : nullptr;
       A.pad_off = c->d_pad_off; A.pad_base = c->pad_off[bs];
       A.D = D_values; A.n = n; A.gn = grad_n; A.n_points = c->n_points; A.max_nnz_pad = c->max_nnz;
+      TimedLaunch t(c, kKindDen);
       if (grad_n) k_density<true><<<(unsigned)ni, kDThreads, dsm, c->stream>>>(c->S, c->L, A, std::max(c->max_act, 1));
       else k_density<false><<<(unsigned)ni, kDThreads, dsm, c->stream>>>(c->S, c->L, A, std::max(c->max_act, 1));
-      c->launches++;
     }
     if ((rc = check_async(c))) return rc;
     bs = be;
   }
+  return AIMS_OK;
+}
+
+int aims_gpu_timing_enable(aims_gpu_ctx *c, int enable) {
+  if (!c) return AIMS_ERR_INVALID_ARG;
+  CU_TRY(c, cudaSetDevice(c->device));
+  CU_TRY(c, cudaStreamSynchronize(c->stream));
+  for (auto &sp : c->spans) c->pool.push_back(sp);
+  c->spans.clear();
+  c->timing = enable != 0;
+  return AIMS_OK;
+}
+
+int aims_gpu_timing_read(aims_gpu_ctx *c, double *ms, int64_t *launches) {
+  if (!c || !ms || !launches) return AIMS_ERR_INVALID_ARG;
+  CU_TRY(c, cudaSetDevice(c->device));
+  CU_TRY(c, cudaStreamSynchronize(c->stream));
+  for (int k = 0; k < kNumKinds; k++) { ms[k] = 0.0; launches[k] = 0; }
+  for (auto &sp : c->spans) {
+    float t = 0.f;
+    CU_TRY(c, cudaEventElapsedTime(&t, sp.e0, sp.e1));
+    ms[sp.kind] += t;
+    launches[sp.kind]++;
+    c->pool.push_back(sp);
+  }
+  c->spans.clear();
   return AIMS_OK;
 }
 
