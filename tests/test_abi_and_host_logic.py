@@ -1,0 +1,162 @@
+"""CPU-side checks (-m "not gpu"): the C-ABI library builds, loads and exports every symbol include/aims_gpu.h
+declares (no compute calls without a GPU); the product path fails loudly without a CUDA device; the host logic that
+shards batches over ranks (bench.py partition_batches) is correct; and the N > 1 data path
+(per-rank partial H, Eq. 28, summed by ONE all-reduce, Eq. 29; density needs none, L312) is
+exercised with world_size 2 over gloo, with the CPU oracle standing in for the per-rank kernels.
+"""
+import ctypes
+import os
+import re
+import socket
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib_path():
+    from paper_1912_06636_b200 import build as gpu_build
+    return gpu_build.build()
+
+
+def test_library_exports_every_declared_symbol(lib_path):
+    with open(os.path.join(ROOT, "include", "aims_gpu.h")) as f:
+        text = f.read()
+    declared = sorted(set(re.findall(r"\b(aims_gpu_[a-z0-9_]+)\s*\(", text)))
+    assert {"aims_gpu_create", "aims_gpu_destroy", "aims_gpu_eval_basis", "aims_gpu_integrate_hamiltonian",
+            "aims_gpu_update_density"} <= set(declared)
+    lib = ctypes.CDLL(lib_path)
+    for name in declared:
+        assert hasattr(lib, name), "libaims_gpu.so does not export %s" % name
+    # the binding checks the same list when it loads
+    import paper_1912_06636_b200 as aims
+    assert aims.exported_symbols() == declared
+    aims.load_library()
+
+
+def test_boundary_has_no_torch_or_cxx_types(lib_path):
+    """extern "C", plain pointers and sizes: the exported names are unmangled and the header compiles as C."""
+    out = subprocess.run(["nm", "-D", "--defined-only", lib_path], capture_output=True, text=True, check=True).stdout
+    names = [ln.split()[-1] for ln in out.splitlines() if " T " in ln]
+    assert any(n == "aims_gpu_create" for n in names)
+    src = "#include \"aims_gpu.h\"\nint main(void){aims_basis_desc b; aims_grid_desc g; aims_bsr_desc p; (void)b;(void)g;(void)p; return AIMS_OK;}\n"
+    r = subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"), "-x", "c", "-", "-o",
+                        "/dev/null"], input=src, text=True, capture_output=True)
+    assert r.returncode == 0, r.stderr
+
+
+def test_library_contains_sm100a_fp64_tensor_code(lib_path):
+    """The contraction kernels are DMMA (FP64 tensor pipe) SASS for sm_100a -- evidence that no other arch is built."""
+    r = subprocess.run(["cuobjdump", "-lelf", lib_path], capture_output=True, text=True)
+    if r.returncode != 0:
+        pytest.skip("cuobjdump unavailable")
+    assert "sm_100a" in r.stdout and "sm_90" not in r.stdout and "sm_80" not in r.stdout
+
+
+def test_product_path_fails_loudly_without_gpu():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    import aims_synth
+    import paper_1912_06636_b200 as aims
+    bun = aims_synth.make_config(1, n_rad=4, n_ang=6)
+    with pytest.raises(aims.AimsError):
+        aims.aims_gpu_create(bun)
+
+
+def test_product_does_not_import_oracle():
+    """The product package and the input generators never import, read or run anything under oracle/."""
+    for pkg in ("paper_1912_06636_b200", "aims_synth"):
+        for dirpath, _, files in os.walk(os.path.join(ROOT, pkg)):
+            for fn in files:
+                if fn.endswith((".py", ".cu", ".cuh", ".c", ".h")):
+                    with open(os.path.join(dirpath, fn)) as f:
+                        text = f.read()
+                    assert not re.search(r"^\s*(from|import)\s+oracle\b", text, re.M), fn
+                    assert "aims_oracle" not in text, fn
+    with open(os.path.join(ROOT, "oracle", "aims_oracle.c")) as f:
+        text = f.read()
+    assert "#include \"aims_gpu.h\"" not in text and "common.cuh" not in text
+
+
+# ------------------------------------------------------------------------------------------- sharding host logic
+def _partition():
+    sys.path.insert(0, ROOT)
+    import bench
+    return bench.partition_batches
+
+
+def test_partition_batches_is_a_contiguous_cover_and_balanced():
+    part = _partition()
+    rng = np.random.default_rng(3)
+    for nb, n_parts in [(1, 1), (5, 2), (7, 8), (1000, 2), (1000, 4), (39638, 8), (0, 2)]:
+        cost = rng.uniform(0.0, 1.0, nb) ** 3
+        rs = part(cost, n_parts)
+        assert len(rs) == n_parts and rs[0][0] == 0 and rs[-1][1] == nb
+        for (a0, a1), (b0, b1) in zip(rs[:-1], rs[1:]):
+            assert a1 == b0 and a0 <= a1
+        if nb >= 1000:
+            loads = np.array([cost[a:b].sum() for a, b in rs])
+            assert loads.max() <= loads.mean() + cost.max() + 1e-12     # off by at most one batch
+    assert part(np.zeros(4), 2)[-1][1] == 4
+
+
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    p = s.getsockname()[1]
+    s.close()
+    return p
+
+
+_WORKER = r"""
+import os, sys
+import numpy as np
+import torch, torch.distributed as dist
+sys.path.insert(0, %(root)r)
+import aims_synth, bench
+from oracle.oracle import Oracle
+rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+dist.init_process_group("gloo", rank=rank, world_size=world)
+bun = aims_synth.make_config(1, n_rad=12, n_ang=26, max_batch=40)
+orc = Oracle(bun)
+nnz = np.array([len(orc.batch_nnz(b)[0]) for b in range(bun.n_batches)], dtype=np.float64)
+cost = np.diff(bun.batch_ptr) * nnz * nnz
+b0, b1 = bench.partition_batches(cost, world)[rank]
+mine = np.arange(b0, b1)
+H = torch.from_numpy(orc.integrate_hamiltonian(bun.v, bun.g, batches=mine))     # Eq. 28: this rank's partial sum
+dist.all_reduce(H)                                                               # Eq. 29: the only communication step
+n, gn = orc.update_density(bun.D_values, want_grad=True, batches=mine)           # L312: no synchronisation needed
+lo, hi = int(bun.batch_ptr[b0]), int(bun.batch_ptr[b1])
+assert np.all(n[:lo] == 0) and np.all(n[hi:] == 0)
+parts = [torch.zeros(bun.n_points, dtype=torch.float64) for _ in range(world)]
+dist.all_gather(parts, torch.from_numpy(n))
+n_all = sum(parts).numpy()
+if rank == 0:
+    H_ref = orc.integrate_hamiltonian(bun.v, bun.g)
+    n_ref, _ = orc.update_density(bun.D_values, want_grad=True)
+    eH = np.linalg.norm(H.numpy() - H_ref) / np.linalg.norm(H_ref)
+    assert eH < 1e-13, eH
+    assert np.array_equal(n_all, n_ref)           # disjoint point ranges: bitwise the single-rank result
+    print("OK", b0, b1, eH)
+dist.destroy_process_group()
+"""
+
+
+def test_two_rank_gloo_partial_sums_equal_single_rank(tmp_path):
+    script = tmp_path / "worker.py"
+    script.write_text(_WORKER % {"root": ROOT})
+    port = _free_port()
+    procs = []
+    for r in range(2):
+        env = dict(os.environ, RANK=str(r), WORLD_SIZE="2", MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port),
+                   OMP_NUM_THREADS="2")
+        procs.append(subprocess.Popen([sys.executable, str(script)], env=env, stdout=subprocess.PIPE,
+                                      stderr=subprocess.STDOUT, text=True))
+    outs = [p.communicate(timeout=300)[0] for p in procs]
+    assert all(p.returncode == 0 for p in procs), "\n".join(outs)
+    assert "OK" in outs[0]
