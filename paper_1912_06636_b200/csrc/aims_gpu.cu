@@ -31,13 +31,14 @@ struct aims_gpu_ctx {
   int64_t n_points = 0, n_values = 0;
 
   // host copies of the static structure (dry run)
-  std::vector<long long> batch_ptr, fn_off, act_off, ptab_off, pad_off, api_off, tile_off, item_off;
+  std::vector<long long> batch_ptr, fn_off, act_off, ptab_off, pad_off, dpad_off, api_off, tile_off, item_off;
   std::vector<int> nnz, n_act;
   int max_nnz = 0, max_act = 0, max_np = 0;
-  long long *d_pad_off = nullptr, *d_api_off = nullptr;
+  long long *d_pad_off = nullptr, *d_dpad_off = nullptr, *d_api_off = nullptr;
   HTile *d_tiles = nullptr;
   DItem *d_items = nullptr;
   double flops_h_lda = 0, flops_h_gga = 0, flops_den = 0;
+  bool ptab_in_smem = true;
 
   double *ws = nullptr;      // Phi-plane workspace
   long long ws_doubles = 0;
@@ -269,35 +270,35 @@ int aims_gpu_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_gri
   if (flag == 2) return fail(c, AIMS_ERR_UNSUPPORTED, "more than AIMS_MAX_ACTIVE_ATOMS atoms touch one batch");
 
   c->fn_off.assign(nb + 1, 0); c->act_off.assign(nb + 1, 0); c->ptab_off.assign(nb + 1, 0);
-  c->pad_off.assign(nb + 1, 0); c->api_off.assign(nb + 1, 0); c->tile_off.assign(nb + 1, 0); c->item_off.assign(nb + 1, 0);
+  c->pad_off.assign(nb + 1, 0); c->dpad_off.assign(nb + 1, 0); c->api_off.assign(nb + 1, 0); c->tile_off.assign(nb + 1, 0); c->item_off.assign(nb + 1, 0);
   std::vector<HTile> tiles;
   std::vector<DItem> items;
   for (int b = 0; b < nb; b++) {
     const int nz = c->nnz[b], nact = c->n_act[b];
     const int np = (int)(c->batch_ptr[b + 1] - c->batch_ptr[b]);
-    const int ld = round_up(np, kPadPts);
+    const int nz8 = pad8(nz), np8 = pad8(np);
     c->max_nnz = std::max(c->max_nnz, nz);
     c->max_act = std::max(c->max_act, nact);
     c->fn_off[b + 1] = c->fn_off[b] + nz;
     c->act_off[b + 1] = c->act_off[b] + nact;
     c->ptab_off[b + 1] = c->ptab_off[b] + (long long)nact * nact;
-    c->pad_off[b + 1] = c->pad_off[b] + (long long)nz * ld;
+    c->pad_off[b + 1] = c->pad_off[b] + (long long)nz8 * np8;                 // H layout
+    c->dpad_off[b + 1] = c->dpad_off[b] + (long long)round_up(nz, 16) * np8;   // density layout
     c->api_off[b + 1] = c->api_off[b] + (long long)nz * np;
-    // Hamiltonian tiles: balanced edge T <= 128, multiple of 8; upper triangle
+    // Hamiltonian tiles: I panels of kHIB blocks x J panels of kHJB blocks that contain a block (bi, bj >= bi)
     if (nz > 0 && np > 0) {
-      const int nt = (nz + kHT - 1) / kHT;
-      const int T = round_up((nz + nt - 1) / nt, 8);
-      for (int ti = 0; ti < nt; ti++)
-        for (int tj = ti; tj < nt; tj++) tiles.push_back(HTile{b, ti, tj, T});
+      const int nblk = blk_count(nz8 >> 3);
+      for (int ti = 0; ti * kHIB < nblk; ti++)
+        for (int tj = 0; tj * kHJB < nblk; tj++)
+          if (std::min(tj * kHJB + kHJB, nblk) - 1 >= ti * kHIB) tiles.push_back(HTile{b, (short)ti, (short)tj});
     }
     c->tile_off[b + 1] = (long long)tiles.size();
-    // density items: balanced point tiles <= 208, multiple of 8, covering the padded leading dimension
-    if (np > 0) {
-      const int npt = (ld + kDTN - 1) / kDTN;
-      const int tp = round_up((ld + npt - 1) / npt, 8);
-      for (int q = 0; q < npt; q++) {
-        const int p0 = q * tp;
-        if (p0 < ld) items.push_back(DItem{b, p0, std::min(tp, ld - p0), 0});
+    // density items: balanced ranges of <= kDNP points, multiples of 8
+    if (nz > 0 && np > 0) {
+      const int nsub = np8 >> 3, nit = (np8 + kDNP - 1) / kDNP;
+      for (int q = 0; q < nit; q++) {
+        const int s0 = (int)((long long)q * nsub / nit), s1 = (int)((long long)(q + 1) * nsub / nit);
+        if (s1 > s0) items.push_back(DItem{b, s0 * 8, (s1 - s0) * 8, 0});
       }
     }
     c->item_off[b + 1] = (long long)items.size();
@@ -310,7 +311,7 @@ int aims_gpu_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_gri
     long long *d;
 #define UPL(vec, field) if ((rc = dev_upload<long long>(c, &d, vec.data(), vec.size()))) return rc; field = d;
     UPL(c->fn_off, L.fn_off) UPL(c->act_off, L.act_off) UPL(c->ptab_off, L.ptab_off)
-    UPL(c->pad_off, c->d_pad_off) UPL(c->api_off, c->d_api_off)
+    UPL(c->pad_off, c->d_pad_off) UPL(c->dpad_off, c->d_dpad_off) UPL(c->api_off, c->d_api_off)
 #undef UPL
   }
   if ((rc = dev_upload<HTile>(c, &c->d_tiles, tiles.data(), tiles.size()))) return rc;
@@ -330,9 +331,9 @@ int aims_gpu_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_gri
   CU_TRY(c, cudaMemGetInfo(&free_b, &total_b));
   want = std::min<long long>(want, (long long)(free_b * 0.8));
   long long max_batch_d = 0;
-  for (int b = 0; b < nb; b++) max_batch_d = std::max(max_batch_d, c->pad_off[b + 1] - c->pad_off[b]);
-  long long need_all = 4 * c->pad_off[nb], need_min = 4 * max_batch_d;
-  long long wsd = std::min(need_all, std::max(want / 8, need_min));
+  for (int b = 0; b < nb; b++) max_batch_d = std::max(max_batch_d, c->dpad_off[b + 1] - c->dpad_off[b]);
+  long long need_all = 4 * c->dpad_off[nb], need_min = 4 * max_batch_d;
+  long long wsd = std::min(need_all, std::max(want / 8, need_min)) + 4 * 64;
   if (wsd * 8 > (long long)free_b) return fail(c, AIMS_ERR_NOMEM, "not enough device memory for one batch of Phi planes");
   if ((rc = dev_alloc(c, &c->ws, (size_t)wsd))) return rc;
   c->ws_doubles = wsd;
@@ -340,8 +341,9 @@ int aims_gpu_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_gri
   // opt in to large dynamic shared memory
   CU_TRY(c, cudaFuncSetAttribute(k_hamiltonian<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h_smem_bytes<false>()));
   CU_TRY(c, cudaFuncSetAttribute(k_hamiltonian<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h_smem_bytes<true>()));
-  const size_t dsm = d_smem_bytes(c->max_nnz, std::max(c->max_act, 1));
-  if (dsm > (size_t)prop.sharedMemPerBlockOptin) return fail(c, AIMS_ERR_UNSUPPORTED, "nnz(B) / active atoms too large for the density kernel's shared memory");
+  c->ptab_in_smem = d_smem_bytes(c->max_nnz, std::max(c->max_act, 1), true) <= (size_t)prop.sharedMemPerBlockOptin;
+  const size_t dsm = d_smem_bytes(c->max_nnz, std::max(c->max_act, 1), c->ptab_in_smem);
+  if (dsm > (size_t)prop.sharedMemPerBlockOptin) return fail(c, AIMS_ERR_UNSUPPORTED, "nnz(B) too large for the density kernel's shared memory");
   CU_TRY(c, cudaFuncSetAttribute(k_density<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dsm));
   CU_TRY(c, cudaFuncSetAttribute(k_density<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dsm));
   CU_TRY(c, cudaStreamSynchronize(c->stream));
@@ -387,12 +389,12 @@ int run_cull(aims_gpu_ctx *c, int b0, int b1) {
 }
 
 // last batch (exclusive) of the chunk starting at bs such that nplanes planes fit the workspace
-int chunk_end(const aims_gpu_ctx *c, int bs, int b1, int nplanes) {
-  const long long cap = c->ws_doubles / nplanes;
+int chunk_end(const aims_gpu_ctx *c, const std::vector<long long> &off, int bs, int b1, int nplanes) {
+  const long long cap = (c->ws_doubles / nplanes) & ~63ll;   // plane stride: 512-byte aligned
   int lo = bs + 1, hi = b1;  // at least one batch (create guaranteed it fits)
   while (lo < hi) {
     int mid = (lo + hi + 1) >> 1;
-    if (c->pad_off[mid] - c->pad_off[bs] <= cap) lo = mid; else hi = mid - 1;
+    if (off[mid] - off[bs] <= cap) lo = mid; else hi = mid - 1;
   }
   return lo;
 }
@@ -435,8 +437,8 @@ int aims_gpu_integrate_hamiltonian(aims_gpu_ctx *c, int32_t b0, int32_t b1, cons
   int rc = run_cull(c, b0, b1);
   if (rc) return rc;
   for (int bs = b0; bs < b1;) {
-    const int be = chunk_end(c, bs, b1, 2);
-    const long long plane = c->ws_doubles / 2;
+    const int be = chunk_end(c, c->pad_off, bs, b1, 2);
+    const long long plane = (c->ws_doubles / 2) & ~63ll;
     EvalArgs E{};
     E.plane[0] = c->ws; E.plane[1] = c->ws + plane;
     E.pad_off = c->d_pad_off; E.pad_base = c->pad_off[bs];
@@ -462,14 +464,14 @@ int aims_gpu_update_density(aims_gpu_ctx *c, int32_t b0, int32_t b1, const doubl
   int rc = run_cull(c, b0, b1);
   if (rc) return rc;
   const int npl = grad_n ? 4 : 1;
-  const size_t dsm = d_smem_bytes(c->max_nnz, std::max(c->max_act, 1));
+  const size_t dsm = d_smem_bytes(c->max_nnz, std::max(c->max_act, 1), c->ptab_in_smem);
   for (int bs = b0; bs < b1;) {
-    const int be = chunk_end(c, bs, b1, npl);
-    const long long plane = c->ws_doubles / npl;
+    const int be = chunk_end(c, c->dpad_off, bs, b1, npl);
+    const long long plane = (c->ws_doubles / npl) & ~63ll;
     EvalArgs E{};
     for (int q = 0; q < npl; q++) E.plane[q] = c->ws + q * plane;
     if (!grad_n) E.plane[1] = c->ws;  // unused
-    E.pad_off = c->d_pad_off; E.pad_base = c->pad_off[bs];
+    E.pad_off = c->d_dpad_off; E.pad_base = c->dpad_off[bs]; E.dlayout = 1;
     E.n_points = c->n_points;
     if (grad_n) launch_eval<kEvalPhiGrad>(c, E, bs, be); else launch_eval<kEvalPhi>(c, E, bs, be);
     const long long ni = c->item_off[be] - c->item_off[bs];
@@ -478,8 +480,9 @@ int aims_gpu_update_density(aims_gpu_ctx *c, int32_t b0, int32_t b1, const doubl
       A.items = c->d_items + c->item_off[bs];
       A.P = E.plane[0];
       for (int q = 0; q < 3; q++) A.G[q] = grad_n ? E.plane[q + 1] : nullptr;
-      A.pad_off = c->d_pad_off; A.pad_base = c->pad_off[bs];
+      A.pad_off = c->d_dpad_off; A.pad_base = c->dpad_off[bs];
       A.D = D_values; A.n = n; A.gn = grad_n; A.n_points = c->n_points; A.max_nnz_pad = c->max_nnz;
+      A.ptab_in_smem = c->ptab_in_smem ? 1 : 0;
       TimedLaunch t(c, kKindDen);
       if (grad_n) k_density<true><<<(unsigned)ni, kDThreads, dsm, c->stream>>>(c->S, c->L, A, std::max(c->max_act, 1));
       else k_density<false><<<(unsigned)ni, kDThreads, dsm, c->stream>>>(c->S, c->L, A, std::max(c->max_act, 1));

@@ -235,7 +235,11 @@ enum EvalMode {
 
 struct EvalArgs {
   double *plane[4];
-  // internal layout: element (row, p) of batch b at plane[q] + (pad_off[b] - pad_base) + row*ld + p, ld = round_up(np, kPadPts)
+  // internal k4 layout (common.cuh): element (row, p) of batch b at
+  //   plane[q] + (pad_off[b] - pad_base) + ((p >> 2) * pad8(nnz) + row) * 4 + (p & 3); rows in [nnz, pad8(nnz)) and
+  //   points in [n_p, pad8(n_p)) are written as zeros; a batch occupies pad8(nnz) * pad8(n_p) doubles per plane.
+  // dlayout != 0: the density layout, chunks of 16 rows: (((row >> 4) * (np8 >> 2) + (p >> 2)) * 16 + (row & 15)) * 4 + (p & 3),
+  //   rows padded with zeros to a multiple of 16; a batch occupies round_up(nnz,16) * pad8(n_p) doubles per plane
   const long long *pad_off;
   long long pad_base;
   // API layout (api != 0): phi at plane[0] + (api_off[b]-api_base) + row*np + p,
@@ -243,14 +247,15 @@ struct EvalArgs {
   const long long *api_off;
   long long api_base;
   int api;
+  int dlayout;           // internal planes in the density layout (common.cuh "k4 layout, chunked") instead of the H layout
   const double *v, *g;   // [n_points], [3][n_points]
   long long n_points;
 };
 
 // ---------------------------------------------------------------------------------------------------------------
-// k_eval: one CTA per batch, one thread per point (columns beyond n_p up to the padded leading dimension get zeros).
-// For each active atom: geometry and log once per point, solid harmonics once per l, one spline Horner per shell.
-// Stores are coalesced along the point index.
+// k_eval: one CTA per batch, one thread per point.  For each active atom: geometry and log once per point, solid
+// harmonics once per l, one spline Horner per shell.  In the k4 layout the four threads of a 4-point group write one
+// full 32-byte sector per row; in the API layout stores are coalesced along the point index.
 // ---------------------------------------------------------------------------------------------------------------
 template <int MODE>
 __global__ void __launch_bounds__(256) k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first) {
@@ -276,14 +281,15 @@ __global__ void __launch_bounds__(256) k_eval(DevSys S, BatchLists L, EvalArgs E
   }
   __syncthreads();
 
-  const int ld = E.api ? np : round_up(np, kPadPts);
+  const int nnz8 = pad8(nnz), np8 = pad8(np);
+  const int npx = E.api ? np : np8;             // points this CTA writes (API: exactly n_p; k4: zero columns up to pad8)
+  const int nrows = E.api ? nnz : (E.dlayout ? round_up(nnz, 16) : nnz8);   // rows this CTA writes
   double *o0, *o1, *o2 = nullptr, *o3 = nullptr;
-  long long cstride = 0;  // distance between gradient components (API layout) -- internal layout uses separate planes
   if (E.api) {
     const long long off = E.api_off[b] - E.api_base;
     o0 = E.plane[0] + off;
     o1 = E.plane[1] ? E.plane[1] + 3 * off : nullptr;
-    cstride = (long long)nnz * np;
+    const long long cstride = (long long)nnz * np;
     if (GRAD) { o2 = o1 + cstride; o3 = o2 + cstride; }
   } else {
     const long long off = E.pad_off[b] - E.pad_base;
@@ -293,14 +299,26 @@ __global__ void __launch_bounds__(256) k_eval(DevSys S, BatchLists L, EvalArgs E
   }
   const int nk1 = S.n_knots - 1;
 
-  for (int p = tid; p < ld; p += 256) {
-    if (p >= np) {  // zero padding columns (internal layout only)
-      for (int r = 0; r < nnz; r++) {
-        o0[(long long)r * ld + p] = 0.0;
-        if (MODE != kEvalPhi) o1[(long long)r * ld + p] = 0.0;
-        if (MODE == kEvalPhiGrad) { o2[(long long)r * ld + p] = 0.0; o3[(long long)r * ld + p] = 0.0; }
+  for (int p = tid; p < npx; p += 256) {
+    // element (row, p) at pb + (row >> 4) * cs + (row & 15) * rs  [D layout]   or   pb + row * rs  [API, H layout]
+    const long long pb = E.api ? (long long)p : (E.dlayout ? (long long)(p >> 2) * 64 + (p & 3) : ((long long)(p >> 2) * nnz8) * 4 + (p & 3));
+    const long long rs = E.api ? (long long)np : 4;
+    const long long cs = E.dlayout ? (long long)np8 * 16 - 64 : 0;   // extra jump at every 16-row chunk boundary
+#define AIMS_EIDX(row) (pb + (long long)(row) * rs + (long long)((row) >> 4) * cs)
+    if (p >= np) {  // zero padding columns (k4 layout only)
+      for (int r = 0; r < nrows; r++) {
+        const long long o = AIMS_EIDX(r);
+        o0[o] = 0.0;
+        if (MODE != kEvalPhi) o1[o] = 0.0;
+        if (MODE == kEvalPhiGrad) { o2[o] = 0.0; o3[o] = 0.0; }
       }
       continue;
+    }
+    for (int r = nnz; r < nrows; r++) {   // zero padding rows (k4 layout only)
+      const long long o = AIMS_EIDX(r);
+      o0[o] = 0.0;
+      if (MODE != kEvalPhi) o1[o] = 0.0;
+      if (MODE == kEvalPhiGrad) { o2[o] = 0.0; o3[o] = 0.0; }
     }
     const double x = S.px[p0 + p], y = S.py[p0 + p], z = S.pz[p0 + p];
     double wv = 0.0, wgx = 0.0, wgy = 0.0, wgz = 0.0;
@@ -345,7 +363,7 @@ __global__ void __launch_bounds__(256) k_eval(DevSys S, BatchLists L, EvalArgs E
           for (int m = 0; m < 7; m++) {
             if (m < nm) {
               const double phi = R * Y[m];
-              const long long o = (row + m) * ld + p;
+              const long long o = AIMS_EIDX(row + m);
               o0[o] = phi;
               if (MODE == kEvalHLda) o1[o] = wv * phi;
               if (GRAD) {
@@ -358,7 +376,7 @@ __global__ void __launch_bounds__(256) k_eval(DevSys S, BatchLists L, EvalArgs E
           }
         } else {
           for (int m = 0; m < nm; m++) {
-            const long long o = (row + m) * ld + p;
+            const long long o = AIMS_EIDX(row + m);
             o0[o] = 0.0;
             if (MODE != kEvalPhi) o1[o] = 0.0;
             if (MODE == kEvalPhiGrad) { o2[o] = 0.0; o3[o] = 0.0; }
@@ -368,6 +386,7 @@ __global__ void __launch_bounds__(256) k_eval(DevSys S, BatchLists L, EvalArgs E
       }
     }
   }
+#undef AIMS_EIDX
 }
 
 // copy the per-batch lists of [b0,b1) into caller arrays (aims_gpu_eval_basis outputs)

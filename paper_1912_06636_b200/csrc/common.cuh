@@ -49,7 +49,17 @@ struct BatchLists {
 
 constexpr int kMaxActive = 96;        // AIMS_MAX_ACTIVE_ATOMS
 constexpr int kMaxCand = 1024;        // atoms passing the bounding-box test for one batch
-constexpr int kPadPts = 16;           // internal Phi planes: leading dimension = n_p rounded up to this
+
+// Internal Phi planes ("k4 layout"): rows (functions) padded with zero rows to a multiple of 8, points padded with zero
+// columns to a multiple of 8; element (row, p) of a batch sits at
+//     plane_offset(b) + ((p >> 2) * nnz8 + row) * 4 + (p & 3)
+// so that the 8-row x 4-point operand fragment of DMMA.8x8x4 (lane = 4*row + point) is 32 consecutive doubles: one
+// conflict-free LDS.64 per fragment, and any row range of one 4-point group is one contiguous segment (bulk-copyable).
+// The density kernel uses the same 4-point interleave but in chunks of 16 rows ("density layout"):
+//     plane_offset(b) + (((row >> 4) * (np8 >> 2) + (p >> 2)) * 16 + (row & 15)) * 4 + (p & 3),   rows padded to 16,
+// so that the 16 functions of one K stage for ALL points of the batch are one contiguous segment (one bulk copy).
+__host__ __device__ inline int pad8(int x) { return (x + 7) & ~7; }
+__host__ __device__ inline int pad4(int x) { return (x + 3) & ~3; }
 
 __host__ __device__ inline int round_up(int x, int m) { return (x + m - 1) / m * m; }
 
@@ -72,6 +82,38 @@ __device__ __forceinline__ void cp_async8(unsigned dst, const void *src, int src
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
+// ---- mbarrier + 1-D bulk async copy (TMA unit; SASS UBLKCP) ---------------------------------------------------
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+// global -> shared bulk copy of `bytes` (multiple of 16; both addresses 16-byte aligned), completion counted on `bar`
+__device__ __forceinline__ void bulk_g2s(unsigned dst, const void *src, unsigned bytes, unsigned bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(dst),
+               "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+// the executing thread's prior cp.async operations arrive on `bar` when they complete (count not incremented)
+__device__ __forceinline__ void cp_async_mbar_arrive_noinc(unsigned bar) {
+  asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];\n" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory"); }
 __device__ __forceinline__ void red_add_f64(double *addr, double v) {
   asm volatile("red.global.add.f64 [%0], %1;\n" ::"l"(addr), "d"(v) : "memory");
 }

@@ -4,209 +4,286 @@
 // on the FP64 tensor pipe (DMMA.8x8x4).  D_b ("calculate_density_mat", L314/L357) is never materialised: its tiles are
 // gathered straight from the block-sparse D into shared memory with 8-byte cp.async.
 //
-// One CTA (16 warps) per (batch, point tile of <= 208 points).  It walks the rows of temp in tiles of 64; for each row
-// tile the K loop runs over all nnz functions in chunks of 16.  After a row tile its 64 x np accumulators are
-// multiplied with Phi (and grad Phi) and reduced over rows with warp shuffles into per-warp-row partial sums in
-// shared memory; the final sums are stored once, without atomics (deterministic).
+// One CTA (16 warps, one per SM) per (batch, range of <= 224 points).  Warp-specialised:
+//   warps 0..13  MMA warps.  The points are cut into PB <= 7 blocks of 3-4 sub-tiles of 8 points and the rows of temp
+//                are walked in M-tiles of IB blocks of 3-4 sub-tiles of 8 rows (IB = 2 for PB = 7); warp (pb, ib)
+//                owns one 32x32-ish block, K runs over all nnz functions in stages of 16.  After an M-tile its block of
+//                temp is multiplied with Phi (and grad Phi), reduced over rows with warp shuffles and added to a
+//                per-(ib) partial sum in shared memory -- no atomics, deterministic.
+//   warps 14,15  producers.  Per stage: the D tile (M-tile rows x 16 functions) by 8-byte cp.async gathers, and the Phi
+//                rows of the stage for all points by ONE bulk async copy (contiguous in the density layout).
+// Stages are handed over with mbarriers (full: producer -> MMA, empty: MMA -> producer); there is no CTA-wide barrier
+// in the main loop, and every DMMA is unpredicated straight-line code (see hamiltonian.cuh for the measurements).
 #pragma once
 #include "common.cuh"
+#include "hamiltonian.cuh"   // blk_start / blk_count
 
 namespace aims {
 
-constexpr int kDTM = 64;            // rows of temp per row tile
-constexpr int kDTN = 208;           // max points per point tile (26 sub-tiles of 8)
-constexpr int kDKC = 16;            // K chunk (functions j) per stage
-constexpr int kDAld = kDKC + 4;     // smem stride of the D tile rows
-constexpr int kDBld = kDTN + 4;     // smem stride of the Phi tile rows ((k*212 + p) mod 16 distinct over a fragment)
+constexpr int kDKC = 16;            // K (functions j) per stage
+constexpr int kDTM = 128;           // max rows of an M-tile (4 blocks)
+constexpr int kDNP = 224;           // max points per CTA (7 blocks of 32)
 constexpr int kDStages = 3;
 constexpr int kDThreads = 512;
-constexpr int kDNsub = 7;           // n sub-tiles per warp: ceil(26 / 4)
+constexpr int kDMmaWarps = 14;
+constexpr int kDProdLanes = 64;
+constexpr int kDAStage = kDTM * kDKC;      // doubles
+constexpr int kDBStage = kDNP * kDKC;      // doubles
 
-struct DItem { int b, p0, npt, pad; };
+struct DItem { int b, p0, npt, pad; };     // points [p0, p0+npt) of batch b; p0 and npt multiples of 8
 
 struct DArgs {
   const DItem *items;
   const double *P;                  // Phi plane
   const double *G[3];               // gradient planes (GRAD only)
-  const long long *pad_off;
+  const long long *pad_off;         // [n_batches+1] prefix of round_up(nnz,16)*pad8(np) (density layout)
   long long pad_base;
   const double *D;                  // block-sparse density matrix
   double *n, *gn;                   // outputs [n_points], [3][n_points]
   long long n_points;
   int max_nnz_pad;                  // capacity of the fn_info smem array
+  int ptab_in_smem;                 // the batch's atom-pair offset table is staged in shared memory
 };
 
-inline size_t d_smem_bytes(int max_nnz, int max_act) {
-  size_t s = (size_t)kDStages * (kDTM * kDAld + kDKC * kDBld) * sizeof(double);
-  s += (size_t)4 * 4 * kDTN * sizeof(double);                 // part[wm][q][col]
-  s += (size_t)max_act * max_act * sizeof(long long);         // ptab
-  s += (size_t)round_up(max_nnz, 4) * sizeof(int) + (size_t)kMaxActive * sizeof(int);
+inline size_t d_smem_bytes(int max_nnz, int max_act, bool ptab_in_smem) {
+  size_t s = (size_t)kDStages * (kDAStage + kDBStage) * sizeof(double);
+  s += (size_t)4 * 4 * kDNP * sizeof(double);                 // part[ib][q][col]
+  s += 2 * kDStages * sizeof(unsigned long long);             // full / empty barriers
+  if (ptab_in_smem) s += (size_t)max_act * max_act * sizeof(long long);
+  s += (size_t)pad8(max_nnz) * sizeof(int) + (size_t)kMaxActive * sizeof(int);
   return s;
+}
+
+// one K step of 4 functions for a warp block of (8 WA rows) x (8 WB points)
+template <int WA, int WB>
+__device__ __forceinline__ void d_mma_k4(double (&acc)[4][4][2], const double *tA, const double *tB) {
+  double fa[WA], fb[WB];
+#pragma unroll
+  for (int a = 0; a < WA; a++) fa[a] = tA[a * 32];
+#pragma unroll
+  for (int c = 0; c < WB; c++) fb[c] = tB[c * (2 * kDKC * 4)];
+#pragma unroll
+  for (int a = 0; a < WA; a++)
+#pragma unroll
+    for (int c = 0; c < WB; c++) dmma8x8x4(acc[a][c][0], acc[a][c][1], fa[a], fb[c]);
+}
+
+__device__ __forceinline__ void d_mma_stage(int variant, double (&acc)[4][4][2], const double *tA, const double *tB, int tm,
+                                            int nk4) {
+#define AIMS_D_CASE(WA, WB)                                                                                  \
+  case WA * 4 + WB:                                                                                          \
+    _Pragma("unroll 1") for (int t = 0; t < nk4; t++) d_mma_k4<WA, WB>(acc, tA + t * tm * 4, tB + t * 16);   \
+    break;
+  switch (variant) {
+    AIMS_D_CASE(4, 4) AIMS_D_CASE(4, 3) AIMS_D_CASE(3, 4) AIMS_D_CASE(3, 3)
+    AIMS_D_CASE(4, 2) AIMS_D_CASE(4, 1) AIMS_D_CASE(3, 2) AIMS_D_CASE(3, 1)
+    AIMS_D_CASE(2, 4) AIMS_D_CASE(2, 3) AIMS_D_CASE(2, 2) AIMS_D_CASE(2, 1)
+    AIMS_D_CASE(1, 4) AIMS_D_CASE(1, 3) AIMS_D_CASE(1, 2) AIMS_D_CASE(1, 1)
+    default: break;
+  }
+#undef AIMS_D_CASE
 }
 
 template <bool GRAD>
 __global__ void __launch_bounds__(kDThreads, 1) k_density(DevSys S, BatchLists L, DArgs A, int max_act) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  double *sA = reinterpret_cast<double *>(smem_raw);                     // [stage][64][20]
-  double *sB = sA + (size_t)kDStages * kDTM * kDAld;                     // [stage][16][212]
-  double *sPart = sB + (size_t)kDStages * kDKC * kDBld;                  // [4][4][208]
-  long long *sPtab = reinterpret_cast<long long *>(sPart + 4 * 4 * kDTN);
-  int *sInfo = reinterpret_cast<int *>(sPtab + (size_t)max_act * max_act);
-  int *sLd = sInfo + round_up(A.max_nnz_pad, 4);
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  double *sA = reinterpret_cast<double *>(smem_raw);                     // [stage][k4][tm][4]
+  double *sB = sA + (size_t)kDStages * kDAStage;                         // [stage][point group][16][4]
+  double *sPart = sB + (size_t)kDStages * kDBStage;                      // [ib][q][col]
+  unsigned long long *s_bar = reinterpret_cast<unsigned long long *>(sPart + 4 * 4 * kDNP);
+  int *sInfo = reinterpret_cast<int *>(s_bar + 2 * kDStages);           // 16-byte aligned; [pad8(max nnz)]
+  int *sLd = sInfo + pad8(A.max_nnz_pad);
+  long long *sPtab = reinterpret_cast<long long *>(sLd + kMaxActive);
 
   const DItem it = A.items[blockIdx.x];
   const int b = it.b;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int wn = warp >> 2, wm = (warp + wn) & 3;
   const int nnz = L.nnz[b], nact = L.n_act[b];
+  const int nnz8 = pad8(nnz), nsub = nnz8 >> 3, nblk = blk_count(nsub);
   const long long pbase = S.batch_ptr[b];
   const int np = (int)(S.batch_ptr[b + 1] - pbase);
-  const int ld = round_up(np, kPadPts);
   const long long boff = A.pad_off[b] - A.pad_base;
-  const int p0 = it.p0, npt = it.npt;                    // this CTA's points [p0, p0+npt) of the batch
-  const int nsn = (npt + 7) >> 3;                        // live n sub-tiles
+  const int p0 = it.p0, npt = it.npt;                    // this CTA's points [p0, p0+npt) of the batch (multiples of 8)
+  const int psub = npt >> 3, PB = blk_count(psub);       // point sub-tiles and blocks
+  const int IB = min(4, kDMmaWarps / PB);                // row blocks per M-tile
+  const int n_mt = (nblk + IB - 1) / IB;                 // M-tiles
+  const int nkc = (nnz8 + kDKC - 1) / kDKC;              // K stages per M-tile
+  const int nsteps = n_mt * nkc;
   const long long fo = L.fn_off[b], ao = L.act_off[b];
+  const long long *gptab = L.ptab + L.ptab_off[b];
 
-  for (int i = tid; i < nnz; i += kDThreads) sInfo[i] = L.fn_info[fo + i];
+  for (int i = tid; i < nnz8; i += kDThreads) sInfo[i] = i < nnz ? L.fn_info[fo + i] : -1;
   for (int i = tid; i < nact; i += kDThreads) sLd[i] = L.act_ld[ao + i];
-  for (int i = tid; i < nact * nact; i += kDThreads) sPtab[i] = L.ptab[L.ptab_off[b] + i];
-  for (int i = tid; i < 4 * 4 * kDTN; i += kDThreads) sPart[i] = 0.0;
-  __syncthreads();
-
-  const double *gP = A.P + boff;
-  const int nk = (nnz + kDKC - 1) / kDKC;                // K chunks per row tile
-  const int nrt = (nnz + kDTM - 1) / kDTM;               // row tiles
-  const int nsteps = nk * nrt;
-
-  // ---- producer
-  auto load_step = [&](int stage, int step) {
-    const int rt = step / nk, kc = step - rt * nk;
-    const int k0 = kc * kDKC;
-    // A: D_b[rt*64 + r][k0 + k], two elements per thread, gathered from the block pattern
-    double *dA = sA + (size_t)stage * kDTM * kDAld;
+  if (A.ptab_in_smem)
+    for (int i = tid; i < nact * nact; i += kDThreads) sPtab[i] = gptab[i];
+  for (int i = tid; i < 4 * 4 * kDNP; i += kDThreads) sPart[i] = 0.0;
+  const unsigned bar_full = smem_u32(s_bar), bar_empty = bar_full + 8 * kDStages;
+  if (tid == 0) {
 #pragma unroll
-    for (int h = 0; h < (kDTM * kDKC) / kDThreads; h++) {
-      const int e = tid + h * kDThreads;
-      const int r = e >> 4, k = e & 15;
-      const int i = rt * kDTM + r, j = k0 + k;
-      const double *src = A.D;
-      int bytes = 0;
-      if (i < nnz && j < nnz) {
-        const int fi = sInfo[i], fj = sInfo[j];
-        const int si = fi >> 16, sj = fj >> 16, ai = fi & 0xFFFF, bj = fj & 0xFFFF;
-        const long long base = sPtab[si * nact + sj];
-        if (base >= 0) {
-          src = (si <= sj) ? A.D + base + (long long)ai * sLd[sj] + bj     // stored block (si,sj): row ai, col bj
-                           : A.D + base + (long long)bj * sLd[si] + ai;    // stored block (sj,si): transposed read
-          bytes = 8;
+    for (int s = 0; s < kDStages; s++) {
+      mbar_init(bar_full + 8 * s, kDProdLanes + 1);      // 64 cp.async completions + the expect_tx arrival
+      mbar_init(bar_empty + 8 * s, kDMmaWarps);
+    }
+    mbar_fence_init();
+  }
+  __syncthreads();
+  const long long *ptab = A.ptab_in_smem ? sPtab : gptab;
+  const double *gP = A.P + boff;
+
+  if (warp >= kDMmaWarps) {
+    // =========================================================================== producers
+    const int pl = tid - kDMmaWarps * 32;                // 0..63
+    const int np8 = pad8(np);
+#pragma unroll 1
+    for (int step = 0; step < nsteps; step++) {
+      const int s = step % kDStages;
+      if (step >= kDStages) mbar_wait(bar_empty + 8 * s, (unsigned)(step / kDStages - 1) & 1u);
+      const int mt = step / nkc, kc = step - mt * nkc;
+      const int k0 = kc * kDKC;
+      const int bi0 = mt * IB, bi1 = min(bi0 + IB, nblk);
+      const int i0 = blk_start(bi0, nsub, nblk), tm = blk_start(bi1, nsub, nblk) - i0;
+      if (pl == kDProdLanes - 1) {
+        // Phi rows [k0, k0+16) of every point of the CTA: ONE contiguous segment in the density layout
+        mbar_expect_tx(bar_full + 8 * s, (unsigned)npt * 128u);
+        bulk_g2s(smem_u32(sB + (size_t)s * kDBStage), gP + ((long long)kc * (np8 >> 2) + (p0 >> 2)) * 64, (unsigned)npt * 128u,
+                 bar_full + 8 * s);
+      }
+      // D_b[i0 + r][k0 + 4t .. +3]: one (row, 4-function group) per lane and pass; gathered from the block pattern
+      // (stored block (si,sj) for si <= sj, transposed read of block (sj,si) below the diagonal)
+      double *dA = sA + (size_t)s * kDAStage;
+      const int ng = min(kDKC, nnz8 - k0) >> 2;          // 4-function groups with at least one real function
+      for (int e = pl; e < tm * ng; e += kDProdLanes) {
+        const int t = e / tm, r = e - t * tm;            // consecutive lanes -> consecutive rows (transposed reads coalesce)
+        const int i = i0 + r, j = k0 + 4 * t;
+        const unsigned dst = smem_u32(dA + (t * tm + r) * 4);
+        if (i >= nnz) {
+#pragma unroll
+          for (int q = 0; q < 4; q++) cp_async8(dst + 8u * q, A.D, 0);
+          continue;
+        }
+        const int fi = sInfo[i];
+        const int si = fi >> 16, ri = fi & 0xFFFF;
+        const int4 fj4 = *reinterpret_cast<const int4 *>(sInfo + j);   // sInfo is padded with -1 up to nnz8
+        const int fjq[4] = {fj4.x, fj4.y, fj4.z, fj4.w};
+        if (fj4.w >= 0 && (fj4.x >> 16) == (fj4.w >> 16) && (fj4.w - fj4.x) == 3) {
+          // fast path: four consecutive functions of one atom
+          const int sj = fj4.x >> 16, cj = fj4.x & 0xFFFF;
+          const long long base = ptab[si * nact + sj];
+          const double *src = A.D;
+          long long stride = 0;
+          int bytes = 0;
+          if (base >= 0) {
+            bytes = 8;
+            if (si <= sj) { src = A.D + base + (long long)ri * sLd[sj] + cj; stride = 1; }
+            else { src = A.D + base + (long long)cj * sLd[si] + ri; stride = sLd[si]; }
+          }
+#pragma unroll
+          for (int q = 0; q < 4; q++) cp_async8(dst + 8u * q, src + q * stride, bytes);
+        } else {
+#pragma unroll
+          for (int q = 0; q < 4; q++) {
+            const double *src = A.D;
+            int bytes = 0;
+            if (fjq[q] >= 0) {
+              const int sj = fjq[q] >> 16, cj = fjq[q] & 0xFFFF;
+              const long long base = ptab[si * nact + sj];
+              if (base >= 0) {
+                src = (si <= sj) ? A.D + base + (long long)ri * sLd[sj] + cj : A.D + base + (long long)cj * sLd[si] + ri;
+                bytes = 8;
+              }
+            }
+            cp_async8(dst + 8u * q, src, bytes);
+          }
         }
       }
-      cp_async8(smem_u32(dA + r * kDAld + k), src, bytes);
+      cp_async_mbar_arrive_noinc(bar_full + 8 * s);
     }
-    // B: Phi[k0 + k][p0 .. p0+npt), 16-byte chunks
-    double *dB = sB + (size_t)stage * kDKC * kDBld;
-    const int nch = (npt + 1) >> 1;                      // chunks per row (npt even except possibly never: ld is even)
-    for (int c = tid; c < kDKC * nch; c += kDThreads) {
-      const int k = c / nch, ch = c - k * nch;
-      const int j = k0 + k;
-      const bool ok = j < nnz;
-      const double *src = gP + (long long)(ok ? j : 0) * ld + p0 + ch * 2;
-      cp_async16(smem_u32(dB + k * kDBld + ch * 2), src, ok ? 16 : 0);
-    }
-  };
+  } else {
+    // =========================================================================== MMA warps
+    const int pb = warp % PB, ib = warp / PB;
+    const bool wlive = warp < PB * IB;
+    const int ps0 = wlive ? blk_start(pb, psub, PB) : 0;                       // first point (within the CTA) of my block
+    const int wb = wlive ? (blk_start(pb + 1, psub, PB) - ps0) >> 3 : 0;
+    const int fr = lane >> 2, fk = lane & 3;
+    const int np8 = pad8(np);
+    const int boffl = (ps0 >> 2) * (kDKC * 4) + (fr >> 2) * (kDKC * 4) + fk * 4 + (fr & 3);
+    double acc[4][4][2];
+#pragma unroll
+    for (int a = 0; a < 4; a++)
+#pragma unroll
+      for (int c = 0; c < 4; c++) { acc[a][c][0] = 0.0; acc[a][c][1] = 0.0; }
 
-  double acc[2][kDNsub][2];
-#pragma unroll
-  for (int a = 0; a < 2; a++)
-#pragma unroll
-    for (int c = 0; c < kDNsub; c++) { acc[a][c][0] = 0.0; acc[a][c][1] = 0.0; }
+#pragma unroll 1
+    for (int step = 0; step < nsteps; step++) {
+      const int s = step % kDStages;
+      const int mt = step / nkc, kc = step - mt * nkc;
+      const int bi0 = mt * IB, bi1 = min(bi0 + IB, nblk);
+      const int i0 = blk_start(bi0, nsub, nblk), tm = blk_start(bi1, nsub, nblk) - i0;
+      const int bi = bi0 + ib;
+      const bool blive = wlive && bi < bi1;
+      int wa = 0, ri0 = 0;
+      if (blive) { ri0 = blk_start(bi, nsub, nblk); wa = (blk_start(bi + 1, nsub, nblk) - ri0) >> 3; }
+      mbar_wait(bar_full + 8 * s, (unsigned)(step / kDStages) & 1u);
+      if (blive)
+        d_mma_stage(wa * 4 + wb, acc, sA + (size_t)s * kDAStage + (ri0 - i0) * 4 + lane, sB + (size_t)s * kDBStage + boffl, tm,
+                    min(kDKC, nnz8 - kc * kDKC) >> 2);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar_empty + 8 * s);
 
+      if (kc == nkc - 1 && blive) {
+        // ---- M-tile epilogue: n_p += sum_i Phi_ip temp_ip (and gradient), rows reduced by shuffles
 #pragma unroll
-  for (int s = 0; s < kDStages - 1; s++) {
-    if (s < nsteps) load_step(s, s);
-    cp_async_commit();
-  }
-
-  const int fr = lane >> 2, fk = lane & 3;
-  for (int step = 0; step < nsteps; step++) {
-    cp_async_wait<kDStages - 2>();
-    __syncthreads();
-    {
-      const int nx = step + kDStages - 1;
-      if (nx < nsteps) load_step(nx % kDStages, nx);
-      cp_async_commit();
-    }
-    const int rt = step / nk, kc = step - rt * nk;
-    const double *tA = sA + (size_t)(step % kDStages) * kDTM * kDAld;
-    const double *tB = sB + (size_t)(step % kDStages) * kDKC * kDBld;
-    const int rows_left = nnz - rt * kDTM;               // live rows in this row tile
+        for (int c = 0; c < 4; c++) {
+          if (c < wb) {
+            const int col = ps0 + c * 8 + 2 * fk;            // within the CTA's point range (even)
+            const int p = p0 + col;                          // within the batch
+            double sn[2] = {0.0, 0.0}, sg[3][2] = {{0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}};
 #pragma unroll
-    for (int ks = 0; ks < kDKC / 4; ks++) {
-      double fa[2], fb[kDNsub];
+            for (int a = 0; a < 4; a++) {
+              if (a < wa) {
+                const int i = ri0 + a * 8 + fr;              // < nnz8: padding rows are zero in the planes
+                const long long o = (((long long)(i >> 4) * (np8 >> 2) + (p >> 2)) * 16 + (i & 15)) * 4 + (p & 3);
+                const double2 ph = *reinterpret_cast<const double2 *>(gP + o);
+                sn[0] += ph.x * acc[a][c][0];
+                sn[1] += ph.y * acc[a][c][1];
+                if (GRAD)
 #pragma unroll
-      for (int a = 0; a < 2; a++) fa[a] = tA[((wm + 4 * a) * 8 + fr) * kDAld + ks * 4 + fk];
+                  for (int q = 0; q < 3; q++) {
+                    const double2 gq = *reinterpret_cast<const double2 *>(A.G[q] + boff + o);
+                    sg[q][0] += gq.x * acc[a][c][0];
+                    sg[q][1] += gq.y * acc[a][c][1];
+                  }
+              }
+            }
 #pragma unroll
-      for (int c = 0; c < kDNsub; c++)
-        if (wn + 4 * c < nsn) fb[c] = tB[(ks * 4 + fk) * kDBld + (wn + 4 * c) * 8 + fr];
-#pragma unroll
-      for (int a = 0; a < 2; a++)
-        if ((wm + 4 * a) * 8 < rows_left)
-#pragma unroll
-          for (int c = 0; c < kDNsub; c++)
-            if (wn + 4 * c < nsn) dmma8x8x4(acc[a][c][0], acc[a][c][1], fa[a], fb[c]);
-    }
-
-    if (kc == nk - 1) {
-      // ---- row-tile epilogue: n_p += sum_i Phi_ip temp_ip (and gradient), rows reduced by shuffles
-#pragma unroll
-      for (int c = 0; c < kDNsub; c++) {
-        if (wn + 4 * c < nsn) {
-          const int col = (wn + 4 * c) * 8 + 2 * fk;       // within the point tile
-          double sn[2] = {0.0, 0.0}, sg[3][2] = {{0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}};
-#pragma unroll
-          for (int a = 0; a < 2; a++) {
-            const int i = rt * kDTM + (wm + 4 * a) * 8 + fr;
-            if (i < nnz) {
-              const long long o = (long long)i * ld + p0 + col;
-              const double2 ph = *reinterpret_cast<const double2 *>(gP + o);
-              sn[0] += ph.x * acc[a][c][0];
-              sn[1] += ph.y * acc[a][c][1];
+            for (int e = 0; e < 2; e++) {
+              double v = sn[e];
+              v += __shfl_xor_sync(0xffffffffu, v, 4); v += __shfl_xor_sync(0xffffffffu, v, 8); v += __shfl_xor_sync(0xffffffffu, v, 16);
+              sn[e] = v;
               if (GRAD)
 #pragma unroll
                 for (int q = 0; q < 3; q++) {
-                  const double2 gq = *reinterpret_cast<const double2 *>(A.G[q] + boff + o);
-                  sg[q][0] += gq.x * acc[a][c][0];
-                  sg[q][1] += gq.y * acc[a][c][1];
+                  double u = sg[q][e];
+                  u += __shfl_xor_sync(0xffffffffu, u, 4); u += __shfl_xor_sync(0xffffffffu, u, 8); u += __shfl_xor_sync(0xffffffffu, u, 16);
+                  sg[q][e] = u;
                 }
             }
-          }
+            if (fr == 0) {   // lanes 0..3 own columns 2*fk, 2*fk+1; (ib, column) has exactly one owner warp -> no race
+              double *pp = sPart + (size_t)(ib * 4) * kDNP + col;
+              pp[0] += sn[0]; pp[1] += sn[1];
+              if (GRAD)
 #pragma unroll
-          for (int e = 0; e < 2; e++) {
-            double v = sn[e];
-            v += __shfl_xor_sync(0xffffffffu, v, 4); v += __shfl_xor_sync(0xffffffffu, v, 8); v += __shfl_xor_sync(0xffffffffu, v, 16);
-            sn[e] = v;
-            if (GRAD)
-#pragma unroll
-              for (int q = 0; q < 3; q++) {
-                double u = sg[q][e];
-                u += __shfl_xor_sync(0xffffffffu, u, 4); u += __shfl_xor_sync(0xffffffffu, u, 8); u += __shfl_xor_sync(0xffffffffu, u, 16);
-                sg[q][e] = u;
-              }
-          }
-          if (fr == 0) {   // lanes 0..3 own columns 2*fk, 2*fk+1; (wm, column) has exactly one owner warp -> no race
-            double *pp = sPart + (size_t)(wm * 4) * kDTN + col;
-            pp[0] += sn[0]; pp[1] += sn[1];
-            if (GRAD)
-#pragma unroll
-              for (int q = 0; q < 3; q++) { pp[(q + 1) * kDTN] += sg[q][0]; pp[(q + 1) * kDTN + 1] += sg[q][1]; }
+                for (int q = 0; q < 3; q++) { pp[(q + 1) * kDNP] += sg[q][0]; pp[(q + 1) * kDNP + 1] += sg[q][1]; }
+            }
           }
         }
 #pragma unroll
-        for (int a = 0; a < 2; a++) { acc[a][c][0] = 0.0; acc[a][c][1] = 0.0; }
+        for (int a = 0; a < 4; a++)
+#pragma unroll
+          for (int c = 0; c < 4; c++) { acc[a][c][0] = 0.0; acc[a][c][1] = 0.0; }
       }
     }
   }
-  cp_async_wait<0>();
   __syncthreads();
 
   // ---- S3d: store (mapping to the global point array is the identity on the batch's contiguous range)
@@ -215,14 +292,14 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density(DevSys S, BatchLists L
     if (p >= np) continue;
     double v = 0.0;
 #pragma unroll
-    for (int m = 0; m < 4; m++) v += sPart[(size_t)(m * 4) * kDTN + col];
+    for (int m = 0; m < 4; m++) v += sPart[(size_t)(m * 4) * kDNP + col];
     A.n[pbase + p] = v;
     if (GRAD)
 #pragma unroll
       for (int q = 0; q < 3; q++) {
         double u = 0.0;
 #pragma unroll
-        for (int m = 0; m < 4; m++) u += sPart[(size_t)(m * 4 + q + 1) * kDTN + col];
+        for (int m = 0; m < 4; m++) u += sPart[(size_t)(m * 4 + q + 1) * kDNP + col];
         A.gn[(long long)q * A.n_points + pbase + p] = 2.0 * u;
       }
   }

@@ -1,92 +1,177 @@
 // hamiltonian.cuh -- S2b/S2c/S2d: batch contraction h[B] = K . L (Eq. 25-27) on the FP64 tensor pipe
 // (DMMA.8x8x4), fused with the scatter into the atom-pair block-sparse H ("insert_into_h", L327/L342, L385-388).
 //
-// Operands come from the planes written by k_eval: P = Phi and Q = w v Phi (LDA) or w (v/2 Phi + g.grad Phi) (GGA).
+// Operands come from the planes written by k_eval (k4 layout, common.cuh): P = Phi and Q = w v Phi (LDA) or
+// w (v/2 Phi + g.grad Phi) (GGA).
 //   LDA : h[B] = P Q^T                 (symmetric; SYRK-shaped, paper: dgmm + syr2k with h phi = v phi)
 //   GGA : h[B] = P Q^T + Q P^T         (SYR2K-shaped, as in Fig. 6a)
-// Only upper tiles (tj >= ti) of the nnz x nnz batch matrix are computed; on diagonal tiles only 8x8 sub-tiles on or
-// above the diagonal.  One CTA (16 warps) per tile of T x T (T <= 128, multiple of 8, balanced per batch); warp
-// (wm, wn) owns the 8x8 sub-tiles (mi, ni) with mi = wm mod 4, ni = wn mod 4, so ragged tiles and diagonal tiles stay
-// balanced over the four SM sub-partitions.
+//
+// Decomposition.  The nnz8 = pad8(nnz) rows of a batch are cut into nblk = ceil(nnz8/32) blocks of 3 or 4 sub-tiles of 8
+// rows (no padding beyond the multiple of 8).  Only blocks (bi, bj >= bi) are computed, one warp per block, and on a
+// diagonal block only the sub-tiles on or above the diagonal.  A CTA (8 warps) owns an I panel of up to 4 blocks and a
+// J panel of up to 2 blocks; two CTAs are resident per SM so that one CTA's scatter epilogue overlaps the other's main
+// loop.  B200 measurements behind this shape: a predicated-off DMMA still occupies the pipe
+// for its full 16 cycles, so every DMMA here sits in straight-line code selected by warp-uniform branches (one
+// template instance per block shape); and one warp per SM sub-partition already sustains 95 % of the DMMA peak, so
+// idle warps of ragged or diagonal tiles cost nothing while the co-resident CTA has work.
+//
+// Pipeline: 4 stages of 8 points; thread 0 issues one bulk async copy (UBLKCP) per panel and 4-point group -- in the
+// k4 layout a panel's rows of one group are one contiguous segment -- completing on the stage's mbarrier.
 #pragma once
 #include "common.cuh"
 
 namespace aims {
 
-constexpr int kHT = 128;          // max tile edge
-constexpr int kHKC = 16;          // points per pipeline stage
-constexpr int kHLds = kHKC + 4;   // smem row stride in doubles: (row*20 + k) mod 16 distinct over an 8x4 fragment
-constexpr int kHPanel = kHT * kHLds;           // doubles per panel per stage
-constexpr int kHCld = kHT + 8;    // row stride of the C staging tile (conflict-free 16-byte fragment stores)
-constexpr int kHThreads = 512;
+constexpr int kHI = 128;          // max rows of the I panel (4 blocks)
+constexpr int kHJ = 64;           // max rows of the J panel (2 blocks)
+constexpr int kHIB = 4, kHJB = 2; // blocks per panel
+constexpr int kHStages = 4;
+constexpr int kHThreads = 256;
+constexpr int kHStripLd = 40;     // row stride of a warp's 8-row staging strip (conflict-free 16-byte stores)
 
-struct HTile { int b, ti, tj, t; };
+struct HTile { int b; short ti, tj; };
 
 struct HArgs {
   const HTile *tiles;       // tile list of this launch (already offset)
   const double *P, *Q;      // planes
-  const long long *pad_off; // [n_batches+1] prefix of nnz*ld (doubles)
+  const long long *pad_off; // [n_batches+1] prefix of pad8(nnz)*pad8(np) (doubles)
   long long pad_base;
   double *H;                // block-sparse values
 };
 
+// first row of block k when nsub sub-tiles of 8 rows are cut into nblk blocks (sizes differ by at most one sub-tile)
+__host__ __device__ inline int blk_start(int k, int nsub, int nblk) { return (int)(((long long)k * nsub) / nblk) * 8; }
+__host__ __device__ inline int blk_count(int nsub) { return (nsub + 3) >> 2; }
+
 template <bool GGA>
-__host__ __device__ constexpr int h_stages() { return GGA ? 2 : 3; }
+__host__ __device__ constexpr int h_group_doubles() { return (kHI + kHJ) * 4 * (GGA ? 2 : 1); }
+template <bool GGA>
+__host__ __device__ constexpr int h_stage_doubles() { return 2 * h_group_doubles<GGA>(); }
 template <bool GGA>
 constexpr size_t h_smem_bytes() {
-  size_t pipe = (size_t)h_stages<GGA>() * (GGA ? 4 : 2) * kHPanel * sizeof(double);
-  size_t cst = (size_t)kHT * kHCld * sizeof(double);
-  return (pipe > cst ? pipe : cst) + 2 * kHT * sizeof(int) + kMaxActive * sizeof(int);
+  return (size_t)kHStages * h_stage_doubles<GGA>() * sizeof(double) + kHStages * sizeof(unsigned long long) +
+         (kHI + kHJ + kMaxActive) * sizeof(int);
+}
+
+// one 4-point group of one warp block: (8 WA) x (8 WB) outputs, straight-line unpredicated DMMAs
+template <int WA, int WB, bool DIAG, bool GGA>
+__device__ __forceinline__ void h_mma_group(double (&acc)[4][4][2], const double *gb, int aoff, int boff) {
+  double fa[WA], fb[WB];
+#pragma unroll
+  for (int a = 0; a < WA; a++) fa[a] = gb[aoff + a * 32];                       // P_I
+#pragma unroll
+  for (int c = 0; c < WB; c++) fb[c] = gb[kHI * 4 + boff + c * 32];             // Q_J
+#pragma unroll
+  for (int a = 0; a < WA; a++)
+#pragma unroll
+    for (int c = 0; c < WB; c++)
+      if (!DIAG || c >= a) dmma8x8x4(acc[a][c][0], acc[a][c][1], fa[a], fb[c]);
+  if (GGA) {
+#pragma unroll
+    for (int a = 0; a < WA; a++) fa[a] = gb[(kHI + kHJ) * 4 + aoff + a * 32];   // Q_I
+#pragma unroll
+    for (int c = 0; c < WB; c++) fb[c] = gb[(2 * kHI + kHJ) * 4 + boff + c * 32];  // P_J
+#pragma unroll
+    for (int a = 0; a < WA; a++)
+#pragma unroll
+      for (int c = 0; c < WB; c++)
+        if (!DIAG || c >= a) dmma8x8x4(acc[a][c][0], acc[a][c][1], fa[a], fb[c]);
+  }
 }
 
 template <bool GGA>
-__global__ void __launch_bounds__(kHThreads, 1) k_hamiltonian(DevSys S, BatchLists L, HArgs A) {
-  constexpr int NST = h_stages<GGA>();
-  constexpr int NPAN = GGA ? 4 : 2;   // panels per stage: P_I, Q_J [, Q_I, P_J]
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+__device__ __forceinline__ void h_mma_stage(int variant, double (&acc)[4][4][2], const double *st, int aoff, int boff) {
+  constexpr int GW = h_group_doubles<GGA>();
+#define AIMS_H_CASE(WA, WB, DG)                                                          \
+  case (WA * 4 + WB) * 2 + DG:                                                           \
+    h_mma_group<WA, WB, DG != 0, GGA>(acc, st, aoff, boff);                              \
+    h_mma_group<WA, WB, DG != 0, GGA>(acc, st + GW, aoff, boff);                         \
+    break;
+  switch (variant) {
+    AIMS_H_CASE(4, 4, 0) AIMS_H_CASE(4, 3, 0) AIMS_H_CASE(3, 4, 0) AIMS_H_CASE(3, 3, 0)
+    AIMS_H_CASE(4, 4, 1) AIMS_H_CASE(3, 3, 1)
+    AIMS_H_CASE(4, 2, 0) AIMS_H_CASE(4, 1, 0) AIMS_H_CASE(3, 2, 0) AIMS_H_CASE(3, 1, 0)
+    AIMS_H_CASE(2, 4, 0) AIMS_H_CASE(2, 3, 0) AIMS_H_CASE(2, 2, 0) AIMS_H_CASE(2, 1, 0)
+    AIMS_H_CASE(1, 4, 0) AIMS_H_CASE(1, 3, 0) AIMS_H_CASE(1, 2, 0) AIMS_H_CASE(1, 1, 0)
+    AIMS_H_CASE(2, 2, 1) AIMS_H_CASE(1, 1, 1)
+    default: break;
+  }
+#undef AIMS_H_CASE
+}
+
+template <bool GGA>
+__global__ void __launch_bounds__(kHThreads, 2) k_hamiltonian(DevSys S, BatchLists L, HArgs A) {
+  constexpr int NST = kHStages;
+  constexpr int GW = h_group_doubles<GGA>(), SW = h_stage_doubles<GGA>();
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   double *sm = reinterpret_cast<double *>(smem_raw);
-  constexpr size_t pipe_d = (size_t)NST * NPAN * kHPanel, cst_d = (size_t)kHT * kHCld;
-  int *s_rowinfo = reinterpret_cast<int *>(sm + (pipe_d > cst_d ? pipe_d : cst_d));
-  int *s_colinfo = s_rowinfo + kHT;
-  int *s_ld = s_colinfo + kHT;
+  unsigned long long *s_bar = reinterpret_cast<unsigned long long *>(sm + (size_t)NST * SW);
+  int *s_rowinfo = reinterpret_cast<int *>(s_bar + NST);
+  int *s_colinfo = s_rowinfo + kHI;
+  int *s_ld = s_colinfo + kHJ;
 
   const HTile tile = A.tiles[blockIdx.x];
-  const int b = tile.b, T = tile.t;
+  const int b = tile.b;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int wn = warp >> 2, wm = (warp + wn) & 3;   // each SM sub-partition (warp & 3) sees every wm and every wn
   const int nnz = L.nnz[b], nact = L.n_act[b];
-  const int np = (int)(S.batch_ptr[b + 1] - S.batch_ptr[b]);
-  const int ld = round_up(np, kPadPts);
-  const long long boff = A.pad_off[b] - A.pad_base;
-  const int i0 = tile.ti * T, j0 = tile.tj * T;
-  const int vi = min(T, nnz - i0), vj = min(T, nnz - j0);   // valid rows / cols of this tile
-  const bool diag = (tile.ti == tile.tj);
+  const int nnz8 = pad8(nnz), nsub = nnz8 >> 3, nblk = blk_count(nsub);
+  const int np8 = pad8((int)(S.batch_ptr[b + 1] - S.batch_ptr[b]));
+  const int nchunk = np8 >> 3;                                    // 8 points (two 4-point groups) per stage
+  const long long boff_plane = A.pad_off[b] - A.pad_base;
   const long long fo = L.fn_off[b], ao = L.act_off[b];
 
-  // row / column bookkeeping for the scatter
-  for (int r = tid; r < kHT; r += kHThreads) {
-    s_rowinfo[r] = (r < vi) ? L.fn_info[fo + i0 + r] : 0;
-    s_colinfo[r] = (r < vj) ? L.fn_info[fo + j0 + r] : 0;
+  const int bI0 = tile.ti * kHIB, bI1 = min(bI0 + kHIB, nblk);
+  const int bJ0 = tile.tj * kHJB, bJ1 = min(bJ0 + kHJB, nblk);
+  const int rI0 = blk_start(bI0, nsub, nblk), rI1 = blk_start(bI1, nsub, nblk);
+  const int rJ0 = blk_start(bJ0, nsub, nblk), rJ1 = blk_start(bJ1, nsub, nblk);
+
+  // this warp's block
+  const int bi = bI0 + (warp & 3), bj = bJ0 + (warp >> 2);
+  const bool live = bi < bI1 && bj < bJ1 && bj >= bi;
+  int wa = 0, wb = 0, ri0 = 0, cj0 = 0;
+  if (live) {
+    ri0 = blk_start(bi, nsub, nblk); cj0 = blk_start(bj, nsub, nblk);
+    wa = (blk_start(bi + 1, nsub, nblk) - ri0) >> 3;
+    wb = (blk_start(bj + 1, nsub, nblk) - cj0) >> 3;
   }
+  const bool diag = live && bi == bj;
+  const int variant = live ? (wa * 4 + wb) * 2 + (diag ? 1 : 0) : -1;
+  const int aoff = (ri0 - rI0) * 4 + lane, boff = (cj0 - rJ0) * 4 + lane;
+
+  // row / column bookkeeping for the scatter
+  for (int r = tid; r < kHI; r += kHThreads) s_rowinfo[r] = (rI0 + r < min(rI1, nnz)) ? L.fn_info[fo + rI0 + r] : -1;
+  for (int r = tid; r < kHJ; r += kHThreads) s_colinfo[r] = (rJ0 + r < min(rJ1, nnz)) ? L.fn_info[fo + rJ0 + r] : -1;
   for (int s = tid; s < nact; s += kHThreads) s_ld[s] = L.act_ld[ao + s];
 
-  // which of my 4x4 sub-tiles exist
-  const int nsi = (vi + 7) >> 3, nsj = (vj + 7) >> 3;
-  unsigned amask = 0;
+  const unsigned bar0 = smem_u32(s_bar);
+  if (tid == 0) {
 #pragma unroll
-  for (int a = 0; a < 4; a++)
+    for (int s = 0; s < NST; s++) mbar_init(bar0 + 8 * s, 1);
+    mbar_fence_init();
+  }
+  __syncthreads();
+
+  // ---- producer (thread 0): chunk q -> stage s; per 4-point group one contiguous segment per panel
+  const double *gP = A.P + boff_plane, *gQ = A.Q + boff_plane;
+  const unsigned bytesI = (unsigned)(rI1 - rI0) * 32u, bytesJ = (unsigned)(rJ1 - rJ0) * 32u;
+  auto issue = [&](int q, int s) {
+    const unsigned bar = bar0 + 8 * s;
+    mbar_expect_tx(bar, 2u * (GGA ? 2u : 1u) * (bytesI + bytesJ));
+    const unsigned dst = smem_u32(sm + (size_t)s * SW);
 #pragma unroll
-    for (int c = 0; c < 4; c++) {
-      const int mi = wm + 4 * a, ni = wn + 4 * c;
-      if (mi < nsi && ni < nsj && (!diag || ni >= mi)) amask |= 1u << (a * 4 + c);
+    for (int g = 0; g < 2; g++) {
+      const long long gI = ((long long)(2 * q + g) * nnz8 + rI0) * 4, gJ = ((long long)(2 * q + g) * nnz8 + rJ0) * 4;
+      const unsigned d = dst + (unsigned)(g * GW) * 8u;
+      bulk_g2s(d, gP + gI, bytesI, bar);
+      bulk_g2s(d + kHI * 32u, gQ + gJ, bytesJ, bar);
+      if (GGA) {
+        bulk_g2s(d + (kHI + kHJ) * 32u, gQ + gI, bytesI, bar);
+        bulk_g2s(d + (2 * kHI + kHJ) * 32u, gP + gJ, bytesJ, bar);
+      }
     }
-  unsigned rmask = 0, cmask = 0;   // rows a / cols c with any live sub-tile
-#pragma unroll
-  for (int a = 0; a < 4; a++)
-    if (amask >> (a * 4) & 0xFu) rmask |= 1u << a;
-#pragma unroll
-  for (int c = 0; c < 4; c++)
-    if (amask & (0x1111u << c)) cmask |= 1u << c;
+  };
+  if (tid == 0)
+    for (int q = 0; q < min(NST, nchunk); q++) issue(q, q);
 
   double acc[4][4][2];
 #pragma unroll
@@ -94,95 +179,48 @@ __global__ void __launch_bounds__(kHThreads, 1) k_hamiltonian(DevSys S, BatchLis
 #pragma unroll
     for (int c = 0; c < 4; c++) { acc[a][c][0] = 0.0; acc[a][c][1] = 0.0; }
 
-  // ---- producer: 16-byte cp.async of one K-chunk (kHKC points) of every panel
-  const double *gP = A.P + boff, *gQ = A.Q + boff;
-  const int nk = ld / kHKC;
-  auto load_stage = [&](int stage, int kc) {
-    double *base = sm + (size_t)stage * NPAN * kHPanel;
-    const int pcol = kc * kHKC;
-    // chunk id: 8 chunks of 16 B per row, kHT rows, NPAN panels
-    for (int c = tid; c < NPAN * kHT * 8; c += kHThreads) {
-      const int pan = c / (kHT * 8), rem = c - pan * (kHT * 8);
-      const int r = rem >> 3, ch = rem & 7;
-      const bool isI = (pan == 0 || pan == 2);
-      const int row = (isI ? i0 : j0) + r;
-      const bool ok = r < (isI ? vi : vj);
-      const double *plane = (pan == 0 || pan == 3) ? gP : gQ;
-      const double *src = plane + (long long)(ok ? row : 0) * ld + pcol + ch * 2;
-      cp_async16(smem_u32(base + (size_t)pan * kHPanel + r * kHLds + ch * 2), src, ok ? 16 : 0);
-    }
-  };
-
-#pragma unroll
-  for (int s = 0; s < NST - 1; s++) {
-    if (s < nk) load_stage(s, s);
-    cp_async_commit();
+#pragma unroll 1
+  for (int q = 0; q < nchunk; q++) {
+    const int s = q % NST;
+    mbar_wait(bar0 + 8 * s, (unsigned)(q / NST) & 1u);
+    h_mma_stage<GGA>(variant, acc, sm + (size_t)s * SW, aoff, boff);
+    __syncthreads();                                  // every warp is done reading stage s
+    if (tid == 0 && q + NST < nchunk) issue(q + NST, s);
   }
 
+  // ---- epilogue (S2d): per warp, 8-row strips through shared memory, then coalesced REDs along the block row
+  if (!live) return;
+  double *strip = sm + warp * (8 * kHStripLd);
   const int fr = lane >> 2, fk = lane & 3;
-  for (int kc = 0; kc < nk; kc++) {
-    cp_async_wait<NST - 2>();
-    __syncthreads();
-    {  // prefetch chunk kc+NST-1 into the stage freed by the previous iteration
-      const int nx = kc + NST - 1;
-      if (nx < nk) load_stage(nx % NST, nx);
-      cp_async_commit();
-    }
-    const double *st = sm + (size_t)(kc % NST) * NPAN * kHPanel;
-    const double *sPI = st, *sQJ = st + kHPanel, *sQI = st + 2 * kHPanel, *sPJ = st + 3 * kHPanel;
-#pragma unroll
-    for (int ks = 0; ks < kHKC / 4; ks++) {
-      double fa[4], fb[4], ga[4], gb[4];
-#pragma unroll
-      for (int a = 0; a < 4; a++) {
-        const int o = ((wm + 4 * a) * 8 + fr) * kHLds + ks * 4 + fk;
-        if (rmask >> a & 1u) { fa[a] = sPI[o]; if (GGA) ga[a] = sQI[o]; }
-      }
-#pragma unroll
-      for (int c = 0; c < 4; c++) {
-        const int o = ((wn + 4 * c) * 8 + fr) * kHLds + ks * 4 + fk;
-        if (cmask >> c & 1u) { fb[c] = sQJ[o]; if (GGA) gb[c] = sPJ[o]; }
-      }
-#pragma unroll
-      for (int a = 0; a < 4; a++)
-#pragma unroll
-        for (int c = 0; c < 4; c++)
-          if (amask >> (a * 4 + c) & 1u) {
-            dmma8x8x4(acc[a][c][0], acc[a][c][1], fa[a], fb[c]);
-            if (GGA) dmma8x8x4(acc[a][c][0], acc[a][c][1], ga[a], gb[c]);
-          }
-    }
-  }
-  cp_async_wait<0>();
-  __syncthreads();
-
-  // ---- epilogue: stage the tile in smem, then add row segments into the block-sparse H (S2d)
-  double *sC = sm;
-#pragma unroll
-  for (int a = 0; a < 4; a++)
-#pragma unroll
-    for (int c = 0; c < 4; c++)
-      if (amask >> (a * 4 + c) & 1u) {
-        const int r = (wm + 4 * a) * 8 + fr, cc = (wn + 4 * c) * 8 + 2 * fk;
-        *reinterpret_cast<double2 *>(sC + r * kHCld + cc) = make_double2(acc[a][c][0], acc[a][c][1]);
-      }
-  __syncthreads();
   const long long *ptab = L.ptab + L.ptab_off[b];
-  for (int r = warp; r < vi; r += kHThreads / 32) {
-    const int ri = s_rowinfo[r];
-    const int si = ri >> 16, ai = ri & 0xFFFF;
-    for (int c = lane; c < vj; c += 32) {
-      if (diag && (c >> 3) < (r >> 3)) continue;            // sub-tile below the diagonal: not computed
-      const int ci = s_colinfo[c];
-      const int sj = ci >> 16, bj = ci & 0xFFFF;
-      if (si > sj) continue;                                // lower atom block (only inside diagonal sub-tiles)
-      const long long base = __ldg(ptab + si * nact + sj);
-      if (base < 0) continue;                               // atom pair outside the pattern: exact zero
-      const double val = sC[r * kHCld + c];
-      const int ldb = s_ld[sj];
-      red_add_f64(A.H + base + (long long)ai * ldb + bj, val);
-      // diagonal atom block holds the full square: mirror unless (c,r) is itself computed in this tile
-      if (si == sj && !(diag && (c >> 3) == (r >> 3))) red_add_f64(A.H + base + (long long)bj * ldb + ai, val);
+  const int ci = (lane < wb * 8) ? s_colinfo[cj0 - rJ0 + lane] : -1;
+  const int sj = ci >> 16, cb = ci & 0xFFFF;
+  const int ldj = (ci >= 0) ? s_ld[sj] : 0;
+  const int csub = lane >> 3;
+#pragma unroll
+  for (int a = 0; a < 4; a++) {
+    if (a < wa) {
+      __syncwarp();
+#pragma unroll
+      for (int c = 0; c < 4; c++)
+        if (c < wb && (!diag || c >= a))
+          *reinterpret_cast<double2 *>(strip + fr * kHStripLd + c * 8 + 2 * fk) = make_double2(acc[a][c][0], acc[a][c][1]);
+      __syncwarp();
+      if (ci >= 0 && !(diag && csub < a)) {
+#pragma unroll 2
+        for (int r = 0; r < 8; r++) {
+          const int ri = s_rowinfo[ri0 - rI0 + a * 8 + r];
+          if (ri < 0) break;                                  // rows beyond nnz (zero padding) end the batch matrix
+          const int si = ri >> 16, ra = ri & 0xFFFF;
+          if (si > sj) continue;                              // lower atom block (only inside diagonal sub-tiles)
+          const long long base = __ldg(ptab + si * nact + sj);
+          if (base < 0) continue;                             // atom pair outside the pattern: exact zero
+          const double val = strip[r * kHStripLd + lane];
+          red_add_f64(A.H + base + (long long)ra * ldj + cb, val);
+          // diagonal atom block holds the full square: mirror unless (col,row) is itself computed (same diagonal sub-tile)
+          if (si == sj && !(diag && csub == a)) red_add_f64(A.H + base + (long long)cb * ldj + ra, val);
+        }
+      }
     }
   }
 }
