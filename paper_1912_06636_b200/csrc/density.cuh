@@ -108,7 +108,6 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density(DevSys S, BatchLists L
   const int IB = min(4, kDMmaWarps / PB);                // row blocks per M-tile
   const int n_mt = (nblk + IB - 1) / IB;                 // M-tiles
   const int nkc = (nnz8 + kDKC - 1) / kDKC;              // K stages per M-tile
-  const int nsteps = n_mt * nkc;
   const long long fo = L.fn_off[b], ao = L.act_off[b];
   const long long *gptab = L.ptab + L.ptab_off[b];
 
@@ -134,14 +133,16 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density(DevSys S, BatchLists L
     // =========================================================================== producers
     const int pl = tid - kDMmaWarps * 32;                // 0..63
     const int np8 = pad8(np);
+    int step = 0;
 #pragma unroll 1
-    for (int step = 0; step < nsteps; step++) {
-      const int s = step % kDStages;
-      if (step >= kDStages) mbar_wait(bar_empty + 8 * s, (unsigned)(step / kDStages - 1) & 1u);
-      const int mt = step / nkc, kc = step - mt * nkc;
-      const int k0 = kc * kDKC;
+    for (int mt = 0; mt < n_mt; mt++) {
       const int bi0 = mt * IB, bi1 = min(bi0 + IB, nblk);
       const int i0 = blk_start(bi0, nsub, nblk), tm = blk_start(bi1, nsub, nblk) - i0;
+#pragma unroll 1
+      for (int kc = 0; kc < nkc; kc++, step++) {
+      const int s = step % kDStages;
+      if (step >= kDStages) mbar_wait(bar_empty + 8 * s, (unsigned)(step / kDStages - 1) & 1u);
+      const int k0 = kc * kDKC;
       if (pl == kDProdLanes - 1) {
         // Phi rows [k0, k0+16) of every point of the CTA: ONE contiguous segment in the density layout
         mbar_expect_tx(bar_full + 8 * s, (unsigned)npt * 128u);
@@ -152,8 +153,8 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density(DevSys S, BatchLists L
       // (stored block (si,sj) for si <= sj, transposed read of block (sj,si) below the diagonal)
       double *dA = sA + (size_t)s * kDAStage;
       const int ng = min(kDKC, nnz8 - k0) >> 2;          // 4-function groups with at least one real function
-      for (int e = pl; e < tm * ng; e += kDProdLanes) {
-        const int t = e / tm, r = e - t * tm;            // consecutive lanes -> consecutive rows (transposed reads coalesce)
+      for (int t = 0; t < ng; t++)
+      for (int r = pl; r < tm; r += kDProdLanes) {       // consecutive lanes -> consecutive rows (transposed reads coalesce)
         const int i = i0 + r, j = k0 + 4 * t;
         const unsigned dst = smem_u32(dA + (t * tm + r) * 4);
         if (i >= nnz) {
@@ -197,6 +198,7 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density(DevSys S, BatchLists L
         }
       }
       cp_async_mbar_arrive_noinc(bar_full + 8 * s);
+      }
     }
   } else {
     // =========================================================================== MMA warps
@@ -213,19 +215,23 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density(DevSys S, BatchLists L
 #pragma unroll
       for (int c = 0; c < 4; c++) { acc[a][c][0] = 0.0; acc[a][c][1] = 0.0; }
 
+    int step = 0;
 #pragma unroll 1
-    for (int step = 0; step < nsteps; step++) {
-      const int s = step % kDStages;
-      const int mt = step / nkc, kc = step - mt * nkc;
+    for (int mt = 0; mt < n_mt; mt++) {
       const int bi0 = mt * IB, bi1 = min(bi0 + IB, nblk);
       const int i0 = blk_start(bi0, nsub, nblk), tm = blk_start(bi1, nsub, nblk) - i0;
       const int bi = bi0 + ib;
       const bool blive = wlive && bi < bi1;
       int wa = 0, ri0 = 0;
       if (blive) { ri0 = blk_start(bi, nsub, nblk); wa = (blk_start(bi + 1, nsub, nblk) - ri0) >> 3; }
+      const int variant = wa * 4 + wb;
+      const int aoffl = (ri0 - i0) * 4 + lane;
+#pragma unroll 1
+      for (int kc = 0; kc < nkc; kc++, step++) {
+      const int s = step % kDStages;
       mbar_wait(bar_full + 8 * s, (unsigned)(step / kDStages) & 1u);
       if (blive)
-        d_mma_stage(wa * 4 + wb, acc, sA + (size_t)s * kDAStage + (ri0 - i0) * 4 + lane, sB + (size_t)s * kDBStage + boffl, tm,
+        d_mma_stage(variant, acc, sA + (size_t)s * kDAStage + aoffl, sB + (size_t)s * kDBStage + boffl, tm,
                     min(kDKC, nnz8 - kc * kDKC) >> 2);
       __syncwarp();
       if (lane == 0) mbar_arrive(bar_empty + 8 * s);
@@ -281,6 +287,7 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density(DevSys S, BatchLists L
         for (int a = 0; a < 4; a++)
 #pragma unroll
           for (int c = 0; c < 4; c++) { acc[a][c][0] = 0.0; acc[a][c][1] = 0.0; }
+      }
       }
     }
   }

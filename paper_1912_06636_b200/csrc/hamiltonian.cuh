@@ -15,8 +15,10 @@
 // template instance per block shape); and one warp per SM sub-partition already sustains 95 % of the DMMA peak, so
 // idle warps of ragged or diagonal tiles cost nothing while the co-resident CTA has work.
 //
-// Pipeline: 4 stages of 8 points; thread 0 issues one bulk async copy (UBLKCP) per panel and 4-point group -- in the
-// k4 layout a panel's rows of one group are one contiguous segment -- completing on the stage's mbarrier.
+// Pipeline: 3 stages of 8 points; one elected lane issues one bulk async copy (UBLKCP) per panel and 4-point group -- in
+// the k4 layout a panel's rows of one group are one contiguous segment -- completing on the stage's "full" mbarrier;
+// warps release a stage on its "empty" mbarrier.  There is no CTA-wide barrier after the set-up, so warps of different
+// block shapes drift freely and each starts its scatter epilogue (private staging strip) as soon as its block is done.
 #pragma once
 #include "common.cuh"
 
@@ -25,7 +27,7 @@ namespace aims {
 constexpr int kHI = 128;          // max rows of the I panel (4 blocks)
 constexpr int kHJ = 64;           // max rows of the J panel (2 blocks)
 constexpr int kHIB = 4, kHJB = 2; // blocks per panel
-constexpr int kHStages = 4;
+constexpr int kHStages = 3;
 constexpr int kHThreads = 256;
 constexpr int kHStripLd = 40;     // row stride of a warp's 8-row staging strip (conflict-free 16-byte stores)
 
@@ -40,7 +42,7 @@ struct HArgs {
 };
 
 // first row of block k when nsub sub-tiles of 8 rows are cut into nblk blocks (sizes differ by at most one sub-tile)
-__host__ __device__ inline int blk_start(int k, int nsub, int nblk) { return (int)(((long long)k * nsub) / nblk) * 8; }
+__host__ __device__ inline int blk_start(int k, int nsub, int nblk) { return (int)((unsigned)(k * nsub) / (unsigned)nblk) * 8; }
 __host__ __device__ inline int blk_count(int nsub) { return (nsub + 3) >> 2; }
 
 template <bool GGA>
@@ -49,8 +51,8 @@ template <bool GGA>
 __host__ __device__ constexpr int h_stage_doubles() { return 2 * h_group_doubles<GGA>(); }
 template <bool GGA>
 constexpr size_t h_smem_bytes() {
-  return (size_t)kHStages * h_stage_doubles<GGA>() * sizeof(double) + kHStages * sizeof(unsigned long long) +
-         (kHI + kHJ + kMaxActive) * sizeof(int);
+  return (size_t)kHStages * h_stage_doubles<GGA>() * sizeof(double) + (size_t)8 * 8 * kHStripLd * sizeof(double) +
+         2 * kHStages * sizeof(unsigned long long) + (kHI + kHJ + kMaxActive) * sizeof(int);
 }
 
 // one 4-point group of one warp block: (8 WA) x (8 WB) outputs, straight-line unpredicated DMMAs
@@ -105,8 +107,9 @@ __global__ void __launch_bounds__(kHThreads, 2) k_hamiltonian(DevSys S, BatchLis
   constexpr int GW = h_group_doubles<GGA>(), SW = h_stage_doubles<GGA>();
   extern __shared__ __align__(128) unsigned char smem_raw[];
   double *sm = reinterpret_cast<double *>(smem_raw);
-  unsigned long long *s_bar = reinterpret_cast<unsigned long long *>(sm + (size_t)NST * SW);
-  int *s_rowinfo = reinterpret_cast<int *>(s_bar + NST);
+  double *s_strip = sm + (size_t)NST * SW;                                  // [8 warps][8][kHStripLd]
+  unsigned long long *s_bar = reinterpret_cast<unsigned long long *>(s_strip + 8 * 8 * kHStripLd);   // full[NST], empty[NST]
+  int *s_rowinfo = reinterpret_cast<int *>(s_bar + 2 * NST);
   int *s_colinfo = s_rowinfo + kHI;
   int *s_ld = s_colinfo + kHJ;
 
@@ -125,9 +128,20 @@ __global__ void __launch_bounds__(kHThreads, 2) k_hamiltonian(DevSys S, BatchLis
   const int rI0 = blk_start(bI0, nsub, nblk), rI1 = blk_start(bI1, nsub, nblk);
   const int rJ0 = blk_start(bJ0, nsub, nblk), rJ1 = blk_start(bJ1, nsub, nblk);
 
-  // this warp's block
-  const int bi = bI0 + (warp & 3), bj = bJ0 + (warp >> 2);
-  const bool live = bi < bI1 && bj < bJ1 && bj >= bi;
+  // Live blocks (bi, bj >= bi) of this tile, enumerated column by column, are dealt to the warps in order, rotated by
+  // the tile index so that the partly filled tiles along the diagonal load the four SM sub-partitions evenly.
+  const int nI = bI1 - bI0, nJ = bJ1 - bJ0;
+  int nlive = 0, my_bi = -1, my_bj = -1;
+  const int slot = (warp + (int)(blockIdx.x & 7)) & 7;
+  for (int cj = 0; cj < nJ; cj++) {
+    const int cnt = min(nI, bJ0 + cj - bI0 + 1);                  // blocks bi = bI0 .. bI0+cnt-1 are on or above the diagonal
+    if (cnt > 0) {
+      if (slot >= nlive && slot < nlive + cnt) { my_bi = bI0 + slot - nlive; my_bj = bJ0 + cj; }
+      nlive += cnt;
+    }
+  }
+  const bool live = my_bi >= 0;
+  const int bi = my_bi, bj = my_bj;
   int wa = 0, wb = 0, ri0 = 0, cj0 = 0;
   if (live) {
     ri0 = blk_start(bi, nsub, nblk); cj0 = blk_start(bj, nsub, nblk);
@@ -143,19 +157,21 @@ __global__ void __launch_bounds__(kHThreads, 2) k_hamiltonian(DevSys S, BatchLis
   for (int r = tid; r < kHJ; r += kHThreads) s_colinfo[r] = (rJ0 + r < min(rJ1, nnz)) ? L.fn_info[fo + rJ0 + r] : -1;
   for (int s = tid; s < nact; s += kHThreads) s_ld[s] = L.act_ld[ao + s];
 
-  const unsigned bar0 = smem_u32(s_bar);
+  const unsigned bar_full = smem_u32(s_bar), bar_empty = bar_full + 8 * NST;
   if (tid == 0) {
 #pragma unroll
-    for (int s = 0; s < NST; s++) mbar_init(bar0 + 8 * s, 1);
+    for (int s = 0; s < NST; s++) { mbar_init(bar_full + 8 * s, 1); mbar_init(bar_empty + 8 * s, (unsigned)nlive); }
     mbar_fence_init();
   }
   __syncthreads();
+  if (!live) return;                                              // no CTA-wide barrier below this line
 
-  // ---- producer (thread 0): chunk q -> stage s; per 4-point group one contiguous segment per panel
+  // ---- producer: chunk q -> stage q % NST; per 4-point group one contiguous segment per panel
   const double *gP = A.P + boff_plane, *gQ = A.Q + boff_plane;
   const unsigned bytesI = (unsigned)(rI1 - rI0) * 32u, bytesJ = (unsigned)(rJ1 - rJ0) * 32u;
-  auto issue = [&](int q, int s) {
-    const unsigned bar = bar0 + 8 * s;
+  auto issue = [&](int q) {
+    const int s = q % NST;
+    const unsigned bar = bar_full + 8 * s;
     mbar_expect_tx(bar, 2u * (GGA ? 2u : 1u) * (bytesI + bytesJ));
     const unsigned dst = smem_u32(sm + (size_t)s * SW);
 #pragma unroll
@@ -170,8 +186,9 @@ __global__ void __launch_bounds__(kHThreads, 2) k_hamiltonian(DevSys S, BatchLis
       }
     }
   };
-  if (tid == 0)
-    for (int q = 0; q < min(NST, nchunk); q++) issue(q, q);
+  // the live warp in slot 0 fills the pipeline; afterwards the refill duty rotates over the live warps
+  if (slot == 0 && lane == 0)
+    for (int q = 0; q < min(NST, nchunk); q++) issue(q);
 
   double acc[4][4][2];
 #pragma unroll
@@ -182,15 +199,23 @@ __global__ void __launch_bounds__(kHThreads, 2) k_hamiltonian(DevSys S, BatchLis
 #pragma unroll 1
   for (int q = 0; q < nchunk; q++) {
     const int s = q % NST;
-    mbar_wait(bar0 + 8 * s, (unsigned)(q / NST) & 1u);
+    mbar_wait(bar_full + 8 * s, (unsigned)(q / NST) & 1u);
     h_mma_stage<GGA>(variant, acc, sm + (size_t)s * SW, aoff, boff);
-    __syncthreads();                                  // every warp is done reading stage s
-    if (tid == 0 && q + NST < nchunk) issue(q + NST, s);
+    __syncwarp();
+    if (lane == 0) {
+      mbar_arrive(bar_empty + 8 * s);                     // this warp is done reading stage s
+      // refill the stage released one chunk ago (lagged by one so that the wait below is normally already satisfied)
+      const int qq = q - 1;
+      if (qq >= 0 && qq + NST < nchunk && slot == qq % nlive) {
+        mbar_wait(bar_empty + 8 * (qq % NST), (unsigned)(qq / NST) & 1u);
+        issue(qq + NST);
+      }
+    }
+    __syncwarp();
   }
 
   // ---- epilogue (S2d): per warp, 8-row strips through shared memory, then coalesced REDs along the block row
-  if (!live) return;
-  double *strip = sm + warp * (8 * kHStripLd);
+  double *strip = s_strip + warp * (8 * kHStripLd);
   const int fr = lane >> 2, fk = lane & 3;
   const long long *ptab = L.ptab + L.ptab_off[b];
   const int ci = (lane < wb * 8) ? s_colinfo[cj0 - rJ0 + lane] : -1;
