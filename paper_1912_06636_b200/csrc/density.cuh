@@ -117,6 +117,7 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density(DevSys S, BatchLists L
     for (int i = tid; i < nact * nact; i += kDThreads) sPtab[i] = gptab[i];
   for (int i = tid; i < 4 * 4 * kDNP; i += kDThreads) sPart[i] = 0.0;
   const unsigned bar_full = smem_u32(s_bar), bar_empty = bar_full + 8 * kDStages;
+  __shared__ int s_map[kDMmaWarps];                      // MMA warp -> (pb | ib << 8), -1 = idle
   if (tid == 0) {
 #pragma unroll
     for (int s = 0; s < kDStages; s++) {
@@ -124,6 +125,27 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density(DevSys S, BatchLists L
       mbar_init(bar_empty + 8 * s, kDMmaWarps);
     }
     mbar_fence_init();
+    // Deal the PB*IB blocks (work ~ point sub-tiles wb) to the MMA warps so that the four SM sub-partitions carry equal
+    // DMMA load: sub-partition q hosts MMA warps q, q+4, q+8(, q+12) -- 2 and 3 have only three because the producers
+    // sit there.  Blocks in descending size go to the sub-partition whose remaining slots need the largest average.
+    const int nb = PB * IB;
+    int cnt[4], load[4] = {0, 0, 0, 0}, used[4] = {0, 0, 0, 0}, total = 0;
+    for (int q = 0; q < 4; q++) cnt[q] = nb / 4 + (q < (nb & 3) ? 1 : 0);
+    for (int w = 0; w < kDMmaWarps; w++) s_map[w] = -1;
+    for (int pb2 = 0; pb2 < PB; pb2++) total += IB * ((blk_start(pb2 + 1, psub, PB) - blk_start(pb2, psub, PB)) >> 3);
+    for (int sz = 4; sz >= 1; sz--)
+      for (int pb2 = 0; pb2 < PB; pb2++) {
+        if (((blk_start(pb2 + 1, psub, PB) - blk_start(pb2, psub, PB)) >> 3) != sz) continue;
+        for (int ib2 = 0; ib2 < IB; ib2++) {
+          int best = -1;
+          for (int q = 0; q < 4; q++) {
+            if (used[q] >= cnt[q]) continue;
+            if (best < 0 || (total - 4 * load[q]) * (cnt[best] - used[best]) > (total - 4 * load[best]) * (cnt[q] - used[q])) best = q;
+          }
+          s_map[best + 4 * used[best]] = pb2 | (ib2 << 8);
+          used[best]++; load[best] += sz;
+        }
+      }
   }
   __syncthreads();
   const long long *ptab = A.ptab_in_smem ? sPtab : gptab;
@@ -202,8 +224,9 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density(DevSys S, BatchLists L
     }
   } else {
     // =========================================================================== MMA warps
-    const int pb = warp % PB, ib = warp / PB;
-    const bool wlive = warp < PB * IB;
+    const int wmap = s_map[warp];
+    const bool wlive = wmap >= 0;
+    const int pb = wmap & 0xFF, ib = wlive ? (wmap >> 8) : 0;
     const int ps0 = wlive ? blk_start(pb, psub, PB) : 0;                       // first point (within the CTA) of my block
     const int wb = wlive ? (blk_start(pb + 1, psub, PB) - ps0) >> 3 : 0;
     const int fr = lane >> 2, fk = lane & 3;
