@@ -5,6 +5,7 @@
 #include <algorithm>
 #include <cstdio>
 #include <cstring>
+#include <map>
 #include <new>
 #include <string>
 #include <vector>
@@ -39,6 +40,8 @@ struct aims_gpu_ctx {
   DItem *d_items = nullptr;
   double flops_h_lda = 0, flops_h_gga = 0, flops_den = 0;
   bool ptab_in_smem = true;
+  std::vector<DItem> h_items;                                  // host copy of the density work items
+  std::map<std::pair<int, int>, int *> item_order;             // (bs, be) -> device permutation, heaviest item first
 
   double *ws = nullptr;      // Phi-plane workspace
   long long ws_doubles = 0;
@@ -316,6 +319,7 @@ int aims_gpu_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_gri
   }
   if ((rc = dev_upload<HTile>(c, &c->d_tiles, tiles.data(), tiles.size()))) return rc;
   if ((rc = dev_upload<DItem>(c, &c->d_items, items.data(), items.size()))) return rc;
+  c->h_items = items;
   CU_TRY(c, cudaStreamSynchronize(c->stream));
   if ((rc = dev_alloc(c, &L.fn_index, (size_t)c->fn_off[nb]))) return rc;
   if ((rc = dev_alloc(c, &L.fn_info, (size_t)c->fn_off[nb]))) return rc;
@@ -399,6 +403,29 @@ int chunk_end(const aims_gpu_ctx *c, const std::vector<long long> &off, int bs, 
   return lo;
 }
 
+// Launch order of the density items of batches [bs, be): heaviest (largest nnz) first, so that the last CTAs of a launch
+// are the cheapest ones (a CTA's cost varies by 50x over a slab).  Built once per distinct range and kept on the device.
+int density_order(aims_gpu_ctx *c, int bs, int be, const int **out) {
+  auto key = std::make_pair(bs, be);
+  auto it = c->item_order.find(key);
+  if (it != c->item_order.end()) { *out = it->second; return AIMS_OK; }
+  const long long i0 = c->item_off[bs], i1 = c->item_off[be];
+  std::vector<int> ord((size_t)(i1 - i0));
+  for (long long i = i0; i < i1; i++) ord[(size_t)(i - i0)] = (int)(i - i0);
+  std::stable_sort(ord.begin(), ord.end(), [&](int a, int b) {
+    const DItem &x = c->h_items[(size_t)(i0 + a)], &y = c->h_items[(size_t)(i0 + b)];
+    const long long cx = (long long)c->nnz[x.b] * c->nnz[x.b] * x.npt, cy = (long long)c->nnz[y.b] * c->nnz[y.b] * y.npt;
+    return cx > cy;
+  });
+  int *d = nullptr;
+  int rc = dev_upload<int>(c, &d, ord.data(), ord.size());
+  if (rc) return rc;
+  CU_TRY(c, cudaStreamSynchronize(c->stream));   // ord is a temporary
+  c->item_order[key] = d;
+  *out = d;
+  return AIMS_OK;
+}
+
 template <int MODE>
 void launch_eval(aims_gpu_ctx *c, const EvalArgs &E, int bs, int be) {
   TimedLaunch t(c, kKindEval);
@@ -477,6 +504,7 @@ int aims_gpu_update_density(aims_gpu_ctx *c, int32_t b0, int32_t b1, const doubl
     const long long ni = c->item_off[be] - c->item_off[bs];
     if (ni > 0) {
       DArgs A{};
+      if ((rc = density_order(c, bs, be, &A.order))) return rc;
       A.items = c->d_items + c->item_off[bs];
       A.P = E.plane[0];
       for (int q = 0; q < 3; q++) A.G[q] = grad_n ? E.plane[q + 1] : nullptr;

@@ -258,7 +258,7 @@ struct EvalArgs {
 // full 32-byte sector per row; in the API layout stores are coalesced along the point index.
 // ---------------------------------------------------------------------------------------------------------------
 template <int MODE>
-__global__ void __launch_bounds__(256) k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first) {
+__global__ void __launch_bounds__(256, 2) k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first) {
   constexpr bool GRAD = (MODE == kEvalPhiGrad || MODE == kEvalHGga);
   const int b = b_first + blockIdx.x;
   const int tid = threadIdx.x;
