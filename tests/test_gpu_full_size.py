@@ -1,0 +1,134 @@
+"""Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (whole-grid calls, default
+workspace, chunked launches).  The oracle cannot finish a full config in seconds, so the checks are:
+  * nnz(B) lists of a seeded sample of batches (plus the largest and smallest) bit-exact against the oracle;
+  * n, grad n of the whole-grid call compared element by element with the oracle on the sampled batches (a batch's
+    density depends on nothing outside the batch, so these are outputs "the oracle can compute one by one");
+  * H restricted to the sampled batches (accumulated batch by batch through [b, b+1)) against the oracle on the same list;
+  * properties that hold at any size, on the whole-grid outputs: the whole-grid H equals the sum of two half-range
+    calls; padding entries stay zero; diagonal atom blocks are symmetric; and the three trace identities
+    sum_p w n = Tr(D S), sum_p w v n = Tr(D H_LDA), sum_p w g.grad n = Tr(D (H_GGA - H_LDA)).
+Tolerances as in test_gpu_parity.py (north_star): 1e-11 relative Frobenius (H), 1e-11 max-norm relative (n, grad n).
+"""
+import numpy as np
+import pytest
+
+import aims_synth
+from aims_synth import bsr_pad_mask
+from oracle.oracle import Oracle
+
+pytestmark = pytest.mark.gpu
+
+TOL_H = 1e-11
+TOL_N = 1e-11
+
+FULL = {
+    "cfg2_full_lda": (2, {}, False, 24),
+    "cfg3_full_gga": (3, {}, True, 24),
+    "cfg4_full_b64": (4, dict(max_batch=64), True, 48),
+    "cfg4_full_b500": (4, dict(max_batch=500), True, 10),
+    "cfg5_full_gga": (5, {}, True, 24),
+}
+
+
+def _rel_fro(a, b):
+    return np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300)
+
+
+def _rel_max(a, b):
+    return np.abs(a - b).max() / max(np.abs(b).max(), 1e-300)
+
+
+@pytest.fixture(scope="module", params=list(FULL))
+def full(request):
+    import paper_1912_06636_b200 as aims
+    cfg, kw, gga, k = FULL[request.param]
+    bun = aims_synth.make_config(cfg, **kw)
+    ctx = aims.aims_gpu_create(bun, device=0)
+    nnz = ctx.batch_nnz()
+    rng = np.random.default_rng(7 + cfg)
+    sel = np.unique(np.concatenate([[0, bun.n_batches - 1, int(np.argmax(nnz)), int(np.argmin(nnz))],
+                                    rng.integers(0, bun.n_batches, k)])).astype(np.int32)
+    yield request.param, bun, Oracle(bun), ctx, gga, sel
+    ctx.close()
+
+
+def test_full_size_lists_bit_exact_on_sample(full):
+    name, bun, orc, ctx, gga, sel = full
+    nnz = ctx.batch_nnz()
+    for b in sel:
+        fn_ptr, fn_index, phi_ptr, phi, dphi = ctx.eval_basis(int(b), int(b) + 1, want_grad=False)
+        ctx.synchronize()
+        ref = orc.batch_nnz(int(b))[0]
+        assert np.array_equal(fn_index.cpu().numpy(), ref)
+        assert nnz[b] == len(ref)
+
+
+def test_full_size_density_on_sampled_batches(full):
+    name, bun, orc, ctx, gga, sel = full
+    n, gn = ctx.update_density(bun.D_values, want_grad=gga)          # whole grid, as bench.py launches it
+    ctx.synchronize()
+    n = n.cpu().numpy()
+    gn = gn.cpu().numpy() if gga else None
+    n_ref, gn_ref = orc.update_density(bun.D_values, want_grad=gga, batches=sel)
+    idx = np.concatenate([np.arange(bun.batch_ptr[b], bun.batch_ptr[b + 1]) for b in sel])
+    assert _rel_max(n[idx], n_ref[idx]) <= TOL_N
+    if gga:
+        assert _rel_max(gn[:, idx], gn_ref[:, idx]) <= TOL_N
+    assert np.isfinite(n).all()
+
+
+def test_full_size_hamiltonian_on_sampled_batches(full):
+    import torch
+    name, bun, orc, ctx, gga, sel = full
+    g = bun.g if gga else None
+    H = torch.zeros(bun.n_values, dtype=torch.float64, device="cuda")
+    vd = torch.as_tensor(bun.v).cuda()
+    gd = torch.as_tensor(bun.g).cuda() if gga else None
+    for b in sel:
+        ctx.integrate_hamiltonian(vd, gd, H=H, b0=int(b), b1=int(b) + 1, accumulate=True)
+    ctx.synchronize()
+    ref = orc.integrate_hamiltonian(bun.v, g, batches=sel)
+    assert _rel_fro(H.cpu().numpy(), ref) <= TOL_H
+
+
+def test_full_size_properties_of_whole_grid_outputs(full):
+    import torch
+    name, bun, orc, ctx, gga, sel = full
+    vd = torch.as_tensor(bun.v).cuda()
+    gd = torch.as_tensor(bun.g).cuda() if gga else None
+    one = torch.ones(bun.n_points, dtype=torch.float64, device="cuda")
+    Hfull = ctx.integrate_hamiltonian(vd, gd).cpu().numpy()           # whole grid, as bench.py launches it
+    mid = bun.n_batches // 2
+    Hsum = torch.zeros(bun.n_values, dtype=torch.float64, device="cuda")
+    ctx.integrate_hamiltonian(vd, gd, H=Hsum, b0=0, b1=mid, accumulate=True)
+    ctx.integrate_hamiltonian(vd, gd, H=Hsum, b0=mid, b1=bun.n_batches, accumulate=True)
+    S = ctx.integrate_hamiltonian(one).cpu().numpy()
+    Hl = ctx.integrate_hamiltonian(vd).cpu().numpy() if gga else Hfull
+    n, gn = ctx.update_density(bun.D_values, want_grad=gga)
+    ctx.synchronize()
+    assert _rel_fro(Hsum.cpu().numpy(), Hfull) <= 1e-13              # Eq. 28-29: partial sums over batch ranges
+    assert np.all(Hfull[bsr_pad_mask(bun)] == 0.0)
+    # diagonal atom blocks hold the full square and must be symmetric (same sums, mirrored)
+    worst = 0.0
+    for a in range(0, bun.n_atoms, max(1, bun.n_atoms // 40)):
+        q = bun.row_ptr[a]
+        nf = bun.atom_fn_ptr[a + 1] - bun.atom_fn_ptr[a]
+        blk = Hfull[bun.blk_off[q]: bun.blk_off[q] + nf * bun.blk_ld[q]].reshape(nf, bun.blk_ld[q])[:, :nf]
+        worst = max(worst, np.abs(blk - blk.T).max() / max(np.abs(blk).max(), 1e-300))
+    assert worst <= 1e-12
+    # trace identities on the GPU outputs alone
+    n = n.cpu().numpy()
+    wgt = np.full(bun.n_values, 2.0)
+    for a in range(bun.n_atoms):
+        q = bun.row_ptr[a]
+        nfa = bun.atom_fn_ptr[a + 1] - bun.atom_fn_ptr[a]
+        wgt[bun.blk_off[q]: bun.blk_off[q] + nfa * bun.blk_ld[q]] = 1.0
+    tr = lambda M: float((wgt * bun.D_values * M).sum())  # noqa: E731
+    # scale: the identities are sums of many terms of both signs; compare against the sum of magnitudes
+    mag = float((np.abs(wgt * bun.D_values * S)).sum())
+    assert abs((bun.w * n).sum() - tr(S)) <= 1e-11 * mag
+    assert abs((bun.w * bun.v * n).sum() - tr(Hl)) <= 1e-11 * max(mag, float(np.abs(wgt * bun.D_values * Hl).sum()))
+    if gga:
+        gn = gn.cpu().numpy()
+        magg = float(np.abs(wgt * bun.D_values * (Hfull - Hl)).sum())
+        assert abs((bun.w * (bun.g * gn).sum(0)).sum() - tr(Hfull - Hl)) <= 1e-11 * max(magg, 1e-300)
