@@ -299,9 +299,20 @@ int aims_gpu_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_gri
     // density items: balanced ranges of <= kDNP points, multiples of 8
     if (nz > 0 && np > 0) {
       const int nsub = np8 >> 3, nit = (np8 + kDNP - 1) / kDNP;
-      for (int q = 0; q < nit; q++) {
-        const int s0 = (int)((long long)q * nsub / nit), s1 = (int)((long long)(q + 1) * nsub / nit);
-        if (s1 > s0) items.push_back(DItem{b, s0 * 8, (s1 - s0) * 8, 0});
+      const int bal = (nsub + nit - 1) / nit;                      // sub-tiles of the largest item of a balanced split
+      if (nit > 1 && bal > 16 && bal <= 20 && nsub - (nit - 1) * (kDNP >> 3) >= 6) {
+        // a balanced split would give items of 5 point blocks, which occupy only 10 of the 14 MMA warps: take full
+        // 224-point items and one remainder item instead
+        for (int q = 0, s0 = 0; q < nit; q++) {
+          const int s1 = std::min(nsub, s0 + (kDNP >> 3));
+          items.push_back(DItem{b, s0 * 8, (s1 - s0) * 8, 0});
+          s0 = s1;
+        }
+      } else {
+        for (int q = 0; q < nit; q++) {
+          const int s0 = (int)((long long)q * nsub / nit), s1 = (int)((long long)(q + 1) * nsub / nit);
+          if (s1 > s0) items.push_back(DItem{b, s0 * 8, (s1 - s0) * 8, 0});
+        }
       }
     }
     c->item_off[b + 1] = (long long)items.size();

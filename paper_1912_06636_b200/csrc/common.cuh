@@ -109,6 +109,10 @@ __device__ __forceinline__ void bulk_g2s(unsigned dst, const void *src, unsigned
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(dst),
                "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
+// bulk prefetch of `bytes` (multiple of 16, 16-byte aligned) of global memory into L2; no completion tracking
+__device__ __forceinline__ void bulk_prefetch_l2(const void *src, unsigned bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;\n" ::"l"(src), "r"(bytes) : "memory");
+}
 // the executing thread's prior cp.async operations arrive on `bar` when they complete (count not incremented)
 __device__ __forceinline__ void cp_async_mbar_arrive_noinc(unsigned bar) {
   asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];\n" ::"r"(bar) : "memory");

@@ -6,7 +6,7 @@
 //
 // One CTA (16 warps, one per SM) per (batch, range of <= 224 points).  Warp-specialised:
 //   warps 0..13  MMA warps.  The points are cut into PB <= 7 blocks of 3-4 sub-tiles of 8 points and the rows of temp
-//                are walked in M-tiles of IB blocks of 3-4 sub-tiles of 8 rows (IB = 2 for PB = 7); warp (pb, ib)
+//                are walked in M-tiles of IB = min(8, 14 / PB) blocks of 3-4 sub-tiles of 8 rows; warp (pb, ib)
 //                owns one 32x32-ish block, K runs over all nnz functions in stages of 16.  After an M-tile its block of
 //                temp is multiplied with Phi (and grad Phi), reduced over rows with warp shuffles and added to a
 //                per-(ib) partial sum in shared memory -- no atomics, deterministic.
@@ -21,14 +21,17 @@
 namespace aims {
 
 constexpr int kDKC = 16;            // K (functions j) per stage
-constexpr int kDTM = 128;           // max rows of an M-tile (4 blocks)
 constexpr int kDNP = 224;           // max points per CTA (7 blocks of 32)
-constexpr int kDStages = 3;
+constexpr int kDStages = 4;
 constexpr int kDThreads = 512;
 constexpr int kDMmaWarps = 14;
 constexpr int kDProdLanes = 64;
-constexpr int kDAStage = kDTM * kDKC;      // doubles
-constexpr int kDBStage = kDNP * kDKC;      // doubles
+// One pipeline stage holds the D tile (M-tile rows x 16) followed by the Phi tile (CTA points x 16).  With PB point
+// blocks and IB = min(4, 14 / PB) row blocks per M-tile, rows + points never exceed 64 + 224 (PB = 7, IB = 2).
+constexpr int kDStageRows = 64 + kDNP;             // rows of D plus points of Phi per stage
+constexpr int kDStage = kDStageRows * kDKC;        // doubles per stage
+constexpr int kDPartCols = 448;                    // max of (row blocks per M-tile) x (points of the CTA): 7 x 64
+constexpr int kDPrefetchLead = 6;                  // stages before the M-tile epilogue at which its operands are prefetched to L2
 
 struct DItem { int b, p0, npt, pad; };     // points [p0, p0+npt) of batch b; p0 and npt multiples of 8
 
@@ -47,8 +50,8 @@ struct DArgs {
 };
 
 inline size_t d_smem_bytes(int max_nnz, int max_act, bool ptab_in_smem) {
-  size_t s = (size_t)kDStages * (kDAStage + kDBStage) * sizeof(double);
-  s += (size_t)4 * 4 * kDNP * sizeof(double);                 // part[ib][q][col]
+  size_t s = (size_t)kDStages * kDStage * sizeof(double);
+  s += (size_t)4 * kDPartCols * sizeof(double);               // part[ib][q][col of the CTA], IB * npt <= kDPartCols
   s += 2 * kDStages * sizeof(unsigned long long);             // full / empty barriers
   if (ptab_in_smem) s += (size_t)max_act * max_act * sizeof(long long);
   s += (size_t)pad8(max_nnz) * sizeof(int) + (size_t)kMaxActive * sizeof(int);
@@ -88,10 +91,9 @@ __device__ __forceinline__ void d_mma_stage(int variant, double (&acc)[4][4][2],
 template <bool GRAD>
 __global__ void __launch_bounds__(kDThreads, 1) k_density(DevSys S, BatchLists L, DArgs A, int max_act) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  double *sA = reinterpret_cast<double *>(smem_raw);                     // [stage][k4][tm][4]
-  double *sB = sA + (size_t)kDStages * kDAStage;                         // [stage][point group][16][4]
-  double *sPart = sB + (size_t)kDStages * kDBStage;                      // [ib][q][col]
-  unsigned long long *s_bar = reinterpret_cast<unsigned long long *>(sPart + 4 * 4 * kDNP);
+  double *sA = reinterpret_cast<double *>(smem_raw);                     // stage s: [k4][tm][4] at sA + s * kDStage
+  double *sPart = sA + (size_t)kDStages * kDStage;                       // [ib][q][col]
+  unsigned long long *s_bar = reinterpret_cast<unsigned long long *>(sPart + 4 * kDPartCols);
   int *sInfo = reinterpret_cast<int *>(s_bar + 2 * kDStages);           // 16-byte aligned; [pad8(max nnz)]
   int *sLd = sInfo + pad8(A.max_nnz_pad);
   long long *sPtab = reinterpret_cast<long long *>(sLd + kMaxActive);
@@ -106,8 +108,9 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density(DevSys S, BatchLists L
   const long long boff = A.pad_off[b] - A.pad_base;
   const int p0 = it.p0, npt = it.npt;                    // this CTA's points [p0, p0+npt) of the batch (multiples of 8)
   const int psub = npt >> 3, PB = blk_count(psub);       // point sub-tiles and blocks
-  const int IB = min(4, kDMmaWarps / PB);                // row blocks per M-tile
+  const int IB = min(8, kDMmaWarps / PB);                // row blocks per M-tile: 2,2,2,3,4,7,8 for PB = 7..1
   const int n_mt = (nblk + IB - 1) / IB;                 // M-tiles
+  const double *sB = sA + IB * 32 * kDKC;                // stage s: [point group][16][4] at sB + s * kDStage
   const int nkc = (nnz8 + kDKC - 1) / kDKC;              // K stages per M-tile
   const long long fo = L.fn_off[b], ao = L.act_off[b];
   const long long *gptab = L.ptab + L.ptab_off[b];
@@ -116,7 +119,7 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density(DevSys S, BatchLists L
   for (int i = tid; i < nact; i += kDThreads) sLd[i] = L.act_ld[ao + i];
   if (A.ptab_in_smem)
     for (int i = tid; i < nact * nact; i += kDThreads) sPtab[i] = gptab[i];
-  for (int i = tid; i < 4 * 4 * kDNP; i += kDThreads) sPart[i] = 0.0;
+  for (int i = tid; i < 4 * kDPartCols; i += kDThreads) sPart[i] = 0.0;
   const unsigned bar_full = smem_u32(s_bar), bar_empty = bar_full + 8 * kDStages;
   __shared__ int s_map[kDMmaWarps];                      // MMA warp -> (pb | ib << 8), -1 = idle
   if (tid == 0) {
@@ -166,15 +169,25 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density(DevSys S, BatchLists L
       const int s = step % kDStages;
       if (step >= kDStages) mbar_wait(bar_empty + 8 * s, (unsigned)(step / kDStages - 1) & 1u);
       const int k0 = kc * kDKC;
+      if (kc == max(nkc - kDPrefetchLead, 0)) {
+        // operands of this M-tile's epilogue (rows [i0, i0+tm) of Phi and grad Phi at the CTA's points): whole 16-row
+        // chunks are contiguous in the density layout -> one bulk L2 prefetch per chunk and plane
+        const int c0 = i0 >> 4, nch = ((i0 + tm - 1) >> 4) - c0 + 1;
+        for (int idx = pl; idx < nch * (GRAD ? 4 : 1); idx += kDProdLanes) {
+          const int c = c0 + (GRAD ? (idx >> 2) : idx), q = GRAD ? (idx & 3) : 0;
+          const double *base = (q == 0) ? gP : A.G[q - 1] + boff;
+          bulk_prefetch_l2(base + ((long long)c * (np8 >> 2) + (p0 >> 2)) * 64, (unsigned)npt * 128u);
+        }
+      }
       if (pl == kDProdLanes - 1) {
         // Phi rows [k0, k0+16) of every point of the CTA: ONE contiguous segment in the density layout
         mbar_expect_tx(bar_full + 8 * s, (unsigned)npt * 128u);
-        bulk_g2s(smem_u32(sB + (size_t)s * kDBStage), gP + ((long long)kc * (np8 >> 2) + (p0 >> 2)) * 64, (unsigned)npt * 128u,
+        bulk_g2s(smem_u32(sB + (size_t)s * kDStage), gP + ((long long)kc * (np8 >> 2) + (p0 >> 2)) * 64, (unsigned)npt * 128u,
                  bar_full + 8 * s);
       }
       // D_b[i0 + r][k0 + 4t .. +3]: one (row, 4-function group) per lane and pass; gathered from the block pattern
       // (stored block (si,sj) for si <= sj, transposed read of block (sj,si) below the diagonal)
-      double *dA = sA + (size_t)s * kDAStage;
+      double *dA = sA + (size_t)s * kDStage;
       const int ng = min(kDKC, nnz8 - k0) >> 2;          // 4-function groups with at least one real function
       for (int t = 0; t < ng; t++)
       for (int r = pl; r < tm; r += kDProdLanes) {       // consecutive lanes -> consecutive rows (transposed reads coalesce)
@@ -255,7 +268,7 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density(DevSys S, BatchLists L
       const int s = step % kDStages;
       mbar_wait(bar_full + 8 * s, (unsigned)(step / kDStages) & 1u);
       if (blive)
-        d_mma_stage(variant, acc, sA + (size_t)s * kDAStage + aoffl, sB + (size_t)s * kDBStage + boffl, tm,
+        d_mma_stage(variant, acc, sA + (size_t)s * kDStage + aoffl, sB + (size_t)s * kDStage + boffl, tm,
                     min(kDKC, nnz8 - kc * kDKC) >> 2);
       __syncwarp();
       if (lane == 0) mbar_arrive(bar_empty + 8 * s);
@@ -299,11 +312,11 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density(DevSys S, BatchLists L
                 }
             }
             if (fr == 0) {   // lanes 0..3 own columns 2*fk, 2*fk+1; (ib, column) has exactly one owner warp -> no race
-              double *pp = sPart + (size_t)(ib * 4) * kDNP + col;
+              double *pp = sPart + (ib * 4) * npt + col;
               pp[0] += sn[0]; pp[1] += sn[1];
               if (GRAD)
 #pragma unroll
-                for (int q = 0; q < 3; q++) { pp[(q + 1) * kDNP] += sg[q][0]; pp[(q + 1) * kDNP + 1] += sg[q][1]; }
+                for (int q = 0; q < 3; q++) { pp[(q + 1) * npt] += sg[q][0]; pp[(q + 1) * npt + 1] += sg[q][1]; }
             }
           }
         }
@@ -322,15 +335,13 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density(DevSys S, BatchLists L
     const int p = p0 + col;
     if (p >= np) continue;
     double v = 0.0;
-#pragma unroll
-    for (int m = 0; m < 4; m++) v += sPart[(size_t)(m * 4) * kDNP + col];
+    for (int m = 0; m < IB; m++) v += sPart[(m * 4) * npt + col];
     A.n[pbase + p] = v;
     if (GRAD)
 #pragma unroll
       for (int q = 0; q < 3; q++) {
         double u = 0.0;
-#pragma unroll
-        for (int m = 0; m < 4; m++) u += sPart[(size_t)(m * 4 + q + 1) * kDNP + col];
+        for (int m = 0; m < IB; m++) u += sPart[(m * 4 + q + 1) * npt + col];
         A.gn[(long long)q * A.n_points + pbase + p] = 2.0 * u;
       }
   }
