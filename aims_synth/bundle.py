@@ -193,3 +193,23 @@ def make_config(cfg, n_rad=None, n_ang=None, max_batch=None, seed=None, gaussian
             blk[:, :n] = 0.5 * (blk[:, :n] + blk[:, :n].T)
         bun.D_values = vals
     return bun
+
+
+def make_q_values(bun, seed_offset=1000):
+    """Stand-in for the energy-weighted density matrix q_ij of PAPER.md Eq. 17 (needs eigenvectors, which this build does not
+    have): symmetric uniform[-1,1] * exp(-R_AB / 4 A) on the block pattern, drawn block by block from its own seeded
+    stream (bun.seed + seed_offset) exactly like D of configs 2-5 (P21)."""
+    rng = np.random.default_rng(bun.seed + seed_offset)
+    na = bun.n_atoms
+    atom_nfn = np.diff(bun.atom_fn_ptr).astype(np.int64)
+    vals = rng.uniform(-1.0, 1.0, bun.n_values)
+    rows = np.repeat(np.arange(na), np.diff(bun.row_ptr))
+    Rab = np.linalg.norm(bun.atom_xyz[rows] - bun.atom_xyz[bun.col_atom], axis=1)
+    vals *= np.repeat(np.exp(-Rab / 4.0), atom_nfn[rows] * bun.blk_ld)
+    vals[bsr_pad_mask(bun)] = 0.0
+    for a in range(na):
+        q = bun.row_ptr[a]
+        n, ld = int(atom_nfn[a]), int(bun.blk_ld[q])
+        blk = vals[bun.blk_off[q]: bun.blk_off[q] + n * ld].reshape(n, ld)
+        blk[:, :n] = 0.5 * (blk[:, :n] + blk[:, :n].T)
+    return vals

@@ -18,11 +18,13 @@
  *   O4  n(r) = sum_ij phi_i(r) n_ij phi_j(r) (Eq. 3) restricted to nnz(B) (L235, L314 "reduction of the
  *       density matrix ... to the dense-but-smaller n_ij"), computed as temp = n_ij phi, n = temp . phi
  *       (Fig. 6b); grad n = 2 sum_ij grad phi_i n_ij phi_j for symmetric n_ij (L67, L93-95).
+ *   O5  Pulay forces F_at (Eq. 16 and Eq. 18) for the reduced h_KS; see the block at the end of this file.
  *
  * Pins (tests/test_oracle_pins.py): Y_lm vs scipy and orthonormality by exact product quadrature; spline vs
  * scipy CubicSpline; grad phi vs finite differences; Gaussian overlap closed form; S symmetric PSD;
  * sum_p w n = Tr(D S), sum_p w v n = Tr(D H_LDA), sum_p w g.grad n = Tr(D H_GGA); batched == brute force;
- * invariance under re-batching.  The paper prints no numerical value for this path, so no pin is "the paper's
+ * invariance under re-batching; Hessian of phi vs finite differences of grad phi; Pulay forces vs central differences
+ * of Tr(D H(R)) - Tr(Q S(R)) under atom displacement and vs the term-by-term brute force.  The paper prints no numerical value for this path, so no pin is "the paper's
  * number"; all pins are mathematical.
  *
  * Arithmetic: IEEE double, no FMA contraction (built with -ffp-contract=off), sums in the loop order written.
@@ -413,6 +415,256 @@ void orc_brute(const orc_system *S, const double *v, const double *g, double *Hd
         for (int c = 0; c < 3; c++) grad_n[(size_t)c * S->n_points + p] = ga[c];
     }
   }
+  free(phi);
+  free(afp);
+}
+
+/* ====================================================================================================================
+ * Pulay forces (Eq. 14-18; evaluated "alongside the density update"
+ * on the same batches, L301-308, L405).  With the reduced h_KS of this build (local potential v plus the GGA term of
+ * reading P2, g = 2 df/d|grad n|^2 grad n supplied as a field) and nabla_at phi_i = -grad phi_i for i centred on atom
+ * `at`, 0 otherwise, Eq. 16 and Eq. 18 read on the grid
+ *   F_at = 2 sum_p w_p sum_{i on at} sum_j { grad phi_i [ n_ij (v_p phi_j + g_p.grad phi_j) - q_ij phi_j ]
+ *                                            + (Hess phi_i g_p) n_ij phi_j }                                  (all at r_p)
+ * i.e. F_at = -d/dR_at [ Tr(n h(R)) - Tr(q s(R)) ] at fixed n_ij, q_ij, v, g, w and grid -- the pin used in
+ * tests/test_oracle_pins.py (central differences of the already pinned H and S).  The atomic-ZORA term (Eq. 19) and
+ * the Hellmann-Feynman force (L403, not on this path in the paper either) are outside the reduced h_KS.
+ * ==================================================================================================================== */
+
+/* second derivatives of the solid harmonics S_lm at (x,y,z): hS[m+l][6] = (xx, yy, zz, xy, xz, yz) */
+void orc_solid_harmonics_hess(int l, const double u[3], double (*hS)[6]) {
+  const double pi = 3.14159265358979323846;
+  double x = u[0], y = u[1], z = u[2];
+  for (int m = 0; m < 2 * l + 1; m++)
+    for (int k = 0; k < 6; k++) hS[m][k] = 0.0;
+  if (l == 2) {
+    double a = 0.5 * sqrt(15.0 / pi), b = 0.25 * sqrt(5.0 / pi), c = 0.25 * sqrt(15.0 / pi);
+    hS[0][3] = a;                                             /* a x y */
+    hS[1][5] = a;                                             /* a y z */
+    hS[2][0] = -2.0 * b; hS[2][1] = -2.0 * b; hS[2][2] = 4.0 * b;   /* b (2 z^2 - x^2 - y^2) */
+    hS[3][4] = a;                                             /* a x z */
+    hS[4][0] = 2.0 * c; hS[4][1] = -2.0 * c;                  /* c (x^2 - y^2) */
+  } else if (l == 3) {
+    double a = 0.25 * sqrt(35.0 / (2.0 * pi)), b = 0.5 * sqrt(105.0 / pi), c = 0.25 * sqrt(21.0 / (2.0 * pi));
+    double d = 0.25 * sqrt(7.0 / pi), e = 0.25 * sqrt(105.0 / pi);
+    /* a (3 x^2 y - y^3) */
+    hS[0][0] = 6.0 * a * y; hS[0][1] = -6.0 * a * y; hS[0][3] = 6.0 * a * x;
+    /* b x y z */
+    hS[1][3] = b * z; hS[1][4] = b * y; hS[1][5] = b * x;
+    /* c (4 y z^2 - x^2 y - y^3) */
+    hS[2][0] = -2.0 * c * y; hS[2][1] = -6.0 * c * y; hS[2][2] = 8.0 * c * y; hS[2][3] = -2.0 * c * x; hS[2][5] = 8.0 * c * z;
+    /* d (2 z^3 - 3 x^2 z - 3 y^2 z) */
+    hS[3][0] = -6.0 * d * z; hS[3][1] = -6.0 * d * z; hS[3][2] = 12.0 * d * z; hS[3][4] = -6.0 * d * x; hS[3][5] = -6.0 * d * y;
+    /* c (4 x z^2 - x^3 - x y^2) */
+    hS[4][0] = -6.0 * c * x; hS[4][1] = -2.0 * c * x; hS[4][2] = 8.0 * c * x; hS[4][3] = -2.0 * c * y; hS[4][4] = 8.0 * c * z;
+    /* e (x^2 z - y^2 z) */
+    hS[5][0] = 2.0 * e * z; hS[5][1] = -2.0 * e * z; hS[5][4] = 2.0 * e * x; hS[5][5] = -2.0 * e * y;
+    /* a (x^3 - 3 x y^2) */
+    hS[6][0] = 6.0 * a * x; hS[6][1] = -6.0 * a * x; hS[6][3] = -6.0 * a * y;
+  }
+}
+
+/* radial spline with second derivative: with s = log_inc * max(d,r0),
+ *   R' = R_t / s,  R'' = R_tt / s^2 - R_t / (s * max(d,r0)),  R_t = b + 2cx + 3dx^2,  R_tt = 2c + 6dx. */
+void orc_radial2(const orc_system *S, int spline, double d, double *R, double *dR, double *d2R) {
+  double dd = d > S->r0 ? d : S->r0;
+  double t = log(dd / S->r0) / S->log_inc;
+  int k = (int)floor(t);
+  if (k > S->n_knots - 2) k = S->n_knots - 2;
+  if (k < 0) k = 0;
+  double x = t - (double)k;
+  const double *c = S->spline_coef + ((size_t)spline * (size_t)(S->n_knots - 1) + (size_t)k) * 4;
+  double Rt = c[1] + x * (2.0 * c[2] + x * 3.0 * c[3]);
+  double Rtt = 2.0 * c[2] + 6.0 * c[3] * x;
+  double s = S->log_inc * dd;
+  *R = c[0] + x * (c[1] + x * (c[2] + x * c[3]));
+  *dR = Rt / s;
+  *d2R = Rtt / (s * s) - Rt / (s * dd);
+}
+
+/* phi, grad phi and the Hessian hess[m+l][6] = (xx, yy, zz, xy, xz, yz) of the 2l+1 functions of (atom, shell) at r.
+ * With phi = F(d) S_lm(dvec), F = R d^-l:
+ *   d_c d_e phi = A u_c u_e Y + B (delta_ce - u_c u_e) Y + B (u_c gS_e + u_e gS_c) + (R/d^2) hS_ce,
+ *   A = R'' - 2 l R'/d + l(l+1) R/d^2,   B = (R' - l R/d)/d,   Y, gS, hS = S_lm and its derivatives at the unit vector u. */
+void orc_shell_hess_at_point(const orc_system *S, int atom, int shell, const double r[3], double *phi, double (*grad)[3],
+                             double (*hess)[6]) {
+  static const int ic[6] = {0, 1, 2, 0, 0, 1}, ie[6] = {0, 1, 2, 1, 2, 2};
+  int l = S->shell_l[shell];
+  double rc = S->shell_rcut[shell];
+  double rc2 = rc * rc;
+  double dv[3];
+  double d2 = dist2(r, S->atom_xyz + 3 * atom, dv);
+  if (!(d2 < rc2)) {
+    for (int m = 0; m < 2 * l + 1; m++) {
+      phi[m] = 0.0;
+      for (int c = 0; c < 3; c++) grad[m][c] = 0.0;
+      for (int k = 0; k < 6; k++) hess[m][k] = 0.0;
+    }
+    return;
+  }
+  double d = sqrt(d2);
+  double u[3] = {0.0, 0.0, 1.0};
+  if (d > 0.0) { u[0] = dv[0] / d; u[1] = dv[1] / d; u[2] = dv[2] / d; }
+  double dd = d > S->r0 ? d : S->r0;
+  double R, dR, d2R, Y[7], gS[7][3], hS[7][6];
+  orc_radial2(S, S->shell_spline[shell], d, &R, &dR, &d2R);
+  orc_solid_harmonics(l, u, Y, gS);
+  orc_solid_harmonics_hess(l, u, hS);
+  double A = d2R - 2.0 * l * dR / dd + (double)(l * (l + 1)) * R / (dd * dd);
+  double B = (dR - (double)l * R / dd) / dd;
+  for (int m = 0; m < 2 * l + 1; m++) {
+    phi[m] = R * Y[m];
+    for (int c = 0; c < 3; c++) grad[m][c] = (dR - (double)l * R / dd) * Y[m] * u[c] + (R / dd) * gS[m][c];
+    for (int k = 0; k < 6; k++) {
+      int c = ic[k], e = ie[k];
+      double delta = (c == e) ? 1.0 : 0.0;
+      hess[m][k] = A * u[c] * u[e] * Y[m] + B * (delta - u[c] * u[e]) * Y[m] + B * (u[c] * gS[m][e] + u[e] * gS[m][c]) +
+                   (R / (dd * dd)) * hS[m][k];
+    }
+  }
+}
+
+/* dense restriction of a block-sparse symmetric matrix to nnz(B) ("calculate_density_mat", L314/L357) */
+static void restrict_matrix(const orc_system *S, const int64_t *afp, int nnz, const int32_t *idx, const int32_t *fa,
+                            const double *values, double *Mb) {
+  for (int i = 0; i < nnz; i++)
+    for (int j = 0; j < nnz; j++) {
+      int A = fa[i], B = fa[j];
+      int ai = (int)(idx[i] - afp[A]), bj = (int)(idx[j] - afp[B]);
+      int ld;
+      double val = 0.0;
+      if (A <= B) { int64_t off = find_block(S, A, B, &ld); if (off >= 0) val = values[off + (int64_t)ai * ld + bj]; }
+      else        { int64_t off = find_block(S, B, A, &ld); if (off >= 0) val = values[off + (int64_t)bj * ld + ai]; }
+      Mb[(size_t)i * nnz + j] = val;
+    }
+}
+
+/* Pulay forces on the listed batches, added into F[n_atoms][3] (caller zeroes).  g == NULL: no GGA term;
+ * Q_values == NULL: no energy-weighted term.  Per batch: temp matrices  Tn = n_ij phi,  Tg = n_ij (g.grad phi),
+ * Tq = q_ij phi  (the DSYMM-shaped products of Fig. 6b), then the point sums of the header formula. */
+void orc_pulay_forces(const orc_system *S, int n_sel, const int32_t *batches, const double *v, const double *g,
+                      const double *D_values, const double *Q_values, double *F) {
+  int64_t *afp = (int64_t *)malloc(sizeof(int64_t) * (S->n_atoms + 1));
+  orc_atom_fn_ptr(S, afp);
+  int nf_tot = (int)afp[S->n_atoms];
+  int32_t *idx = (int32_t *)malloc(sizeof(int32_t) * 4 * (size_t)nf_tot);
+  int32_t *fa = idx + nf_tot, *fs = fa + nf_tot, *fm = fs + nf_tot;
+  for (int q = 0; q < n_sel; q++) {
+    int b = batches[q];
+    int64_t p0 = S->batch_ptr[b];
+    int np = (int)(S->batch_ptr[b + 1] - p0);
+    int nnz = orc_batch_nnz(S, b, idx, fa, fs, fm);
+    if (nnz == 0 || np == 0) continue;
+    size_t sz = (size_t)nnz * np;
+    double *phi = (double *)malloc(sizeof(double) * sz * 10);     /* phi, dphi[3], hess[6] */
+    double *dphi = phi + sz, *hes = phi + 4 * sz;
+    for (int i = 0; i < nnz;) {
+      int l = S->shell_l[fs[i]];
+      for (int p = 0; p < np; p++) {
+        double val[7], gr[7][3], hh[7][6];
+        orc_shell_hess_at_point(S, fa[i], fs[i], S->xyz + 3 * (p0 + p), val, gr, hh);
+        for (int m = 0; m < 2 * l + 1; m++) {
+          phi[(size_t)(i + m) * np + p] = val[m];
+          for (int c = 0; c < 3; c++) dphi[((size_t)c * nnz + i + m) * np + p] = gr[m][c];
+          for (int k = 0; k < 6; k++) hes[((size_t)k * nnz + i + m) * np + p] = hh[m][k];
+        }
+      }
+      i += 2 * l + 1;
+    }
+    double *Db = (double *)malloc(sizeof(double) * (size_t)nnz * nnz);
+    double *Qb = Q_values ? (double *)malloc(sizeof(double) * (size_t)nnz * nnz) : NULL;
+    restrict_matrix(S, afp, nnz, idx, fa, D_values, Db);
+    if (Qb) restrict_matrix(S, afp, nnz, idx, fa, Q_values, Qb);
+    double *Frow = (double *)calloc((size_t)nnz * 3, sizeof(double));     /* per-function contribution, summed per atom below */
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int i = 0; i < nnz; i++) {
+      double f[3] = {0.0, 0.0, 0.0};
+      for (int p = 0; p < np; p++) {
+        double gp[3] = {0.0, 0.0, 0.0};
+        if (g) for (int c = 0; c < 3; c++) gp[c] = g[(size_t)c * S->n_points + p0 + p];
+        double tn = 0.0, tg = 0.0, tq = 0.0;
+        for (int j = 0; j < nnz; j++) {
+          double dij = Db[(size_t)i * nnz + j];
+          tn += dij * phi[(size_t)j * np + p];
+          if (g) {
+            double Gj = 0.0;
+            for (int c = 0; c < 3; c++) Gj += gp[c] * dphi[((size_t)c * nnz + j) * np + p];
+            tg += dij * Gj;
+          }
+          if (Qb) tq += Qb[(size_t)i * nnz + j] * phi[(size_t)j * np + p];
+        }
+        double wp = S->w[p0 + p];
+        double x = v[p0 + p] * tn + tg - tq;
+        static const int hx[3][3] = {{0, 3, 4}, {3, 1, 5}, {4, 5, 2}};   /* index of (c,e) in (xx,yy,zz,xy,xz,yz) */
+        for (int c = 0; c < 3; c++) {
+          double t = dphi[((size_t)c * nnz + i) * np + p] * x;
+          if (g) {
+            double hg = 0.0;
+            for (int e = 0; e < 3; e++) hg += hes[((size_t)hx[c][e] * nnz + i) * np + p] * gp[e];
+            t += hg * tn;
+          }
+          f[c] += 2.0 * wp * t;
+        }
+      }
+      for (int c = 0; c < 3; c++) Frow[(size_t)i * 3 + c] = f[c];
+    }
+    for (int i = 0; i < nnz; i++)
+      for (int c = 0; c < 3; c++) F[(size_t)fa[i] * 3 + c] += Frow[(size_t)i * 3 + c];
+    free(Frow);
+    free(Qb);
+    free(Db);
+    free(phi);
+  }
+  free(idx);
+  free(afp);
+}
+
+/* brute-force Pulay forces (tiny inputs only): no batches, no culling, dense Dd, Qd [n_basis][n_basis] (Qd may be NULL),
+ * written from Eq. 16 and Eq. 18 term by term with nabla_at phi_i = -grad phi_i:
+ *   F_at = -2 sum_ij int [nabla_at phi_i] n_ij v phi_j + 2 sum_ij int [nabla_at phi_i] q_ij phi_j
+ *          -2 sum_ij int [nabla_at phi_i] n_ij (g.grad phi_j) - 2 sum_ij int phi_i n_ij (g.nabla_at grad phi_j). */
+void orc_brute_forces(const orc_system *S, const double *v, const double *g, const double *Dd, const double *Qd, double *F) {
+  int64_t *afp = (int64_t *)malloc(sizeof(int64_t) * (S->n_atoms + 1));
+  orc_atom_fn_ptr(S, afp);
+  int nb = (int)afp[S->n_atoms];
+  double *phi = (double *)malloc(sizeof(double) * (size_t)nb * 10);
+  double *dph = phi + nb, *hes = phi + 4 * (size_t)nb;        /* dph[c*nb+i], hes[k*nb+i] */
+  int *at_of = (int *)malloc(sizeof(int) * (size_t)nb);
+  static const int hx[3][3] = {{0, 3, 4}, {3, 1, 5}, {4, 5, 2}};
+  for (int64_t p = 0; p < S->n_points; p++) {
+    int i = 0;
+    for (int a = 0; a < S->n_atoms; a++) {
+      int sp = S->atom_species[a];
+      for (int s = S->species_shell_ptr[sp]; s < S->species_shell_ptr[sp + 1]; s++) {
+        int l = S->shell_l[s];
+        double val[7], gr[7][3], hh[7][6];
+        orc_shell_hess_at_point(S, a, s, S->xyz + 3 * p, val, gr, hh);
+        for (int m = 0; m < 2 * l + 1; m++, i++) {
+          phi[i] = val[m]; at_of[i] = a;
+          for (int c = 0; c < 3; c++) dph[c * nb + i] = gr[m][c];
+          for (int k = 0; k < 6; k++) hes[k * nb + i] = hh[m][k];
+        }
+      }
+    }
+    double wp = S->w[p];
+    for (int a = 0; a < nb; a++)
+      for (int b = 0; b < nb; b++) {
+        double nab = Dd[(size_t)a * nb + b], qab = Qd ? Qd[(size_t)a * nb + b] : 0.0;
+        double Gb = 0.0;
+        if (g) for (int c = 0; c < 3; c++) Gb += g[(size_t)c * S->n_points + p] * dph[c * nb + b];
+        for (int c = 0; c < 3; c++) {
+          double nat_phi_a = -dph[c * nb + a];                       /* [nabla_at phi_a]_c for at = atom of a */
+          F[at_of[a] * 3 + c] += wp * (-2.0 * nat_phi_a * nab * v[p] * phi[b] + 2.0 * nat_phi_a * qab * phi[b]);
+          if (g) {
+            F[at_of[a] * 3 + c] += wp * (-2.0 * nat_phi_a * nab * Gb);
+            double nat_gb = 0.0;                                     /* g . nabla_at grad phi_b, component c, at = atom of b */
+            for (int e = 0; e < 3; e++) nat_gb += -hes[hx[c][e] * nb + b] * g[(size_t)e * S->n_points + p];
+            F[at_of[b] * 3 + c] += wp * (-2.0 * phi[a] * nab * nat_gb);
+          }
+        }
+      }
+  }
+  free(at_of);
   free(phi);
   free(afp);
 }

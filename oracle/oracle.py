@@ -56,6 +56,11 @@ def _load():
         L.orc_integrate_hamiltonian.argtypes = [sp, ctypes.c_int, _ip, _dp, _dp, _dp]
         L.orc_update_density.argtypes = [sp, ctypes.c_int, _ip, _dp, _dp, _dp]
         L.orc_brute.argtypes = [sp, _dp, _dp, _dp, _dp, _dp, _dp]
+        L.orc_solid_harmonics_hess.argtypes = [ctypes.c_int, _dp, _dp]
+        L.orc_radial2.argtypes = [sp, ctypes.c_int, ctypes.c_double, _dp, _dp, _dp]
+        L.orc_shell_hess_at_point.argtypes = [sp, ctypes.c_int, ctypes.c_int, _dp, _dp, _dp, _dp]
+        L.orc_pulay_forces.argtypes = [sp, ctypes.c_int, _ip, _dp, _dp, _dp, _dp, _dp]
+        L.orc_brute_forces.argtypes = [sp, _dp, _dp, _dp, _dp, _dp]
         _lib = L
     return _lib
 
@@ -85,6 +90,14 @@ def solid_harmonics(l, u, want_grad=False):
     G = np.zeros((2 * l + 1, 3)) if want_grad else None
     _load().orc_solid_harmonics(int(l), _d(u), _d(Y), _d(G))
     return (Y, G) if want_grad else Y
+
+
+def solid_harmonics_hess(l, u):
+    """Second derivatives of S_lm at u: [2l+1][6] = (xx, yy, zz, xy, xz, yz)."""
+    u = np.ascontiguousarray(u, dtype=np.float64)
+    H = np.zeros((2 * l + 1, 6))
+    _load().orc_solid_harmonics_hess(int(l), _d(u), _d(H))
+    return H
 
 
 class Oracle:
@@ -189,3 +202,37 @@ class Oracle:
         Dd = None if D_dense is None else np.ascontiguousarray(D_dense, dtype=np.float64)
         self.L.orc_brute(ctypes.byref(self.sys), _d(v), _d(g), _d(Hd), _d(Dd), _d(n), _d(gn))
         return Hd, n, gn
+
+    # ---- Pulay forces (Eq. 16, 18)
+    def radial2(self, spline, d):
+        R, dR, d2R = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+        self.L.orc_radial2(ctypes.byref(self.sys), int(spline), float(d), ctypes.byref(R), ctypes.byref(dR), ctypes.byref(d2R))
+        return R.value, dR.value, d2R.value
+
+    def shell_hess_at_point(self, atom, shell, r):
+        """(phi[2l+1], grad[2l+1][3], hess[2l+1][6] = xx, yy, zz, xy, xz, yz)"""
+        l = int(self.keep["shell_l"][shell])
+        r = np.ascontiguousarray(r, dtype=np.float64)
+        phi, gr, he = np.zeros(2 * l + 1), np.zeros((2 * l + 1, 3)), np.zeros((2 * l + 1, 6))
+        self.L.orc_shell_hess_at_point(ctypes.byref(self.sys), int(atom), int(shell), _d(r), _d(phi), _d(gr), _d(he))
+        return phi, gr, he
+
+    def pulay_forces(self, v, D_values, g=None, Q_values=None, batches=None):
+        """F[n_atoms][3] summed over the listed batches."""
+        sel = self._sel(batches)
+        v = np.ascontiguousarray(v, dtype=np.float64)
+        g = None if g is None else np.ascontiguousarray(g, dtype=np.float64)
+        D = np.ascontiguousarray(D_values, dtype=np.float64)
+        Q = None if Q_values is None else np.ascontiguousarray(Q_values, dtype=np.float64)
+        F = np.zeros((self.sys.n_atoms, 3))
+        self.L.orc_pulay_forces(ctypes.byref(self.sys), len(sel), _i(sel), _d(v), _d(g), _d(D), _d(Q), _d(F))
+        return F
+
+    def brute_forces(self, v, D_dense, g=None, Q_dense=None):
+        v = np.ascontiguousarray(v, dtype=np.float64)
+        g = None if g is None else np.ascontiguousarray(g, dtype=np.float64)
+        Dd = np.ascontiguousarray(D_dense, dtype=np.float64)
+        Qd = None if Q_dense is None else np.ascontiguousarray(Q_dense, dtype=np.float64)
+        F = np.zeros((self.sys.n_atoms, 3))
+        self.L.orc_brute_forces(ctypes.byref(self.sys), _d(v), _d(g), _d(Dd), _d(Qd), _d(F))
+        return F

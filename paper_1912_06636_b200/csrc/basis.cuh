@@ -257,8 +257,11 @@ struct EvalArgs {
 // harmonics once per l, one spline Horner per shell.  In the k4 layout the four threads of a 4-point group write one
 // full 32-byte sector per row; in the API layout stores are coalesced along the point index.
 // ---------------------------------------------------------------------------------------------------------------
+#ifndef AIMS_EVAL_CTAS_PER_SM
+#define AIMS_EVAL_CTAS_PER_SM 2
+#endif
 template <int MODE>
-__global__ void __launch_bounds__(256, 2) k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first) {
+__global__ void __launch_bounds__(256, AIMS_EVAL_CTAS_PER_SM) k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first) {
   constexpr bool GRAD = (MODE == kEvalPhiGrad || MODE == kEvalHGga);
   const int b = b_first + blockIdx.x;
   const int tid = threadIdx.x;
