@@ -4,7 +4,10 @@
 One "step" = one pass of the whole hot path over the whole grid: aims_gpu_integrate_hamiltonian (GGA) followed by
 aims_gpu_update_density (with grad n), each including its own culling and basis evaluation.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1..5]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1..5] [--path scf|forces]
+
+--path forces times the widened row f1 instead: one step = one aims_gpu_pulay_forces (GGA term and the
+energy-weighted density matrix) over the whole grid; it is a separate line, not the headline metric.
 
 N > 1 (torchrun): contiguous batch ranges balanced by n_p*nnz^2 are sharded over the ranks; each rank adds its
 partial H (Eq. 28) and the partial sums are combined by ONE NCCL all-reduce (Eq. 29, "the only communication
@@ -54,6 +57,7 @@ def parse():
     ap.add_argument("--cpu-sample-batches", type=int, default=96)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--path", default="scf", choices=["scf", "forces"])
     return ap.parse_args()
 
 
@@ -121,35 +125,39 @@ def sample_batches(n_batches, k, seed=20191206):
     return np.sort(rng.choice(n_batches, size=min(k, n_batches), replace=False)).astype(np.int32)
 
 
-def time_oracle(bun, batches, gga, repeats=1):
-    """Oracle as it stands on the host cores: H integration + density update on the listed batches."""
+def time_oracle(bun, batches, gga, repeats=1, forces_q=None):
+    """Oracle as it stands on the host cores: H integration + density update (or, with forces_q, the Pulay forces) on
+    the listed batches."""
     from oracle import oracle as orc
     o = orc.Oracle(bun)
     pts = int(sum(bun.batch_ptr[b + 1] - bun.batch_ptr[b] for b in batches))
     best = None
     for _ in range(repeats):
         t0 = time.perf_counter()
-        o.integrate_hamiltonian(bun.v, bun.g if gga else None, batches=batches)
-        o.update_density(bun.D_values, want_grad=gga, batches=batches)
+        if forces_q is not None:
+            o.pulay_forces(bun.v, bun.D_values, g=bun.g if gga else None, Q_values=forces_q, batches=batches)
+        else:
+            o.integrate_hamiltonian(bun.v, bun.g if gga else None, batches=batches)
+            o.update_density(bun.D_values, want_grad=gga, batches=batches)
         dt = time.perf_counter() - t0
         best = dt if best is None else min(best, dt)
     return pts, best, orc.num_threads()
 
 
-def run_reference(args, bun, gga, workload):
+def run_reference(args, bun, gga, workload, metric, forces_q=None):
     """--impl reference: the CPU oracle, rank 0 only, a bounded sample per step."""
     per_step = max(4, args.cpu_sample_batches // 4)
     times, pts_step = [], 0
     for s in range(args.warmup + args.steps):
         sel = sample_batches(bun.n_batches, per_step, seed=1000 + s)
-        pts, dt, cores = time_oracle(bun, sel, gga)
+        pts, dt, cores = time_oracle(bun, sel, gga, forces_q=forces_q)
         if s >= args.warmup:
             times.append(dt)
             pts_step += pts
     total = sum(times)
     val = pts_step / total
     sample = "%d seeded batches per step (about %d points) of %s" % (per_step, pts_step // max(args.steps, 1), workload)
-    out = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+    out = {"impl": "reference", "metric": metric, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": 1e3 * total / max(args.steps, 1), "higher_is_better": True,
            "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
            "config": {"workload": workload, "sample": sample},
@@ -171,12 +179,15 @@ def main():
     if args.n_rad or args.n_ang:
         workload += " [DEBUG GRID n_rad=%s n_ang=%s: not the benchmark workload]" % (args.n_rad, args.n_ang)
 
+    forces = args.path == "forces"
+    metric = METRIC if not forces else "grid points/s for the Pulay-force pass (FP64); % of FP64 peak"
+
     import aims_synth
     if args.impl == "reference":
         if rank != 0:
             return 0
         bun = aims_synth.make_config(args.config, n_rad=args.n_rad, n_ang=args.n_ang, max_batch=args.max_batch)
-        run_reference(args, bun, gga, workload)
+        run_reference(args, bun, gga, workload, metric, forces_q=aims_synth.make_q_values(bun) if forces else None)
         return 0
 
     import torch
@@ -203,6 +214,9 @@ def main():
     my_points = int(bun.batch_ptr[b1] - bun.batch_ptr[b0])
     flops_h = float(((2.0 if gga else 1.0) * npb * nnz * (nnz + (0.0 if gga else 1.0)))[b0:b1].sum())
     flops_n = float((2.0 * npb * nnz * nnz)[b0:b1].sum())
+    # Pulay forces: the DSYMM-shaped products q_b Phi, n_b L and (GGA) n_b Phi, 2 n_p nnz^2 each
+    flops_f = (3.0 if gga else 2.0) * flops_n
+    Qh = aims_synth.make_q_values(bun) if forces else None
 
     with torch.cuda.stream(stream):
         v = torch.as_tensor(bun.v).to("cuda", non_blocking=False)
@@ -211,10 +225,17 @@ def main():
         H = torch.empty(bun.n_values, dtype=torch.float64, device="cuda")
         n = torch.zeros(bun.n_points, dtype=torch.float64, device="cuda")
         gn = torch.zeros((3, bun.n_points), dtype=torch.float64, device="cuda") if gga else None
+        Q = torch.as_tensor(Qh).to("cuda") if forces else None
+        F = torch.zeros((bun.n_atoms, 3), dtype=torch.float64, device="cuda")
     stream.synchronize()
 
     def step():
         with torch.cuda.stream(stream):
+            if forces:
+                ctx.pulay_forces(v, D, g=g, Q=Q, F=F, b0=b0, b1=b1, accumulate=False)
+                if world > 1:
+                    dist.all_reduce(F)
+                return
             ctx.integrate_hamiltonian(v, g, H=H, b0=b0, b1=b1, accumulate=False)
             if world > 1:
                 dist.all_reduce(H)                        # Eq. 29: the only communication step
@@ -270,6 +291,11 @@ def main():
         hb["D"].copy_(torch.as_tensor(bun.D_values))
         if gga:
             hb["g"].copy_(torch.as_tensor(bun.g))
+        if forces:
+            hb["Q"] = torch.empty(bun.n_values, dtype=torch.float64, pin_memory=True)
+            hb["Q"].copy_(torch.as_tensor(Qh))
+            hb["F"] = torch.empty((bun.n_atoms, 3), dtype=torch.float64, pin_memory=True)
+            dv["Q"], dv["F"] = torch.empty_like(Q), torch.empty_like(F)
 
         def step_e2e():
             with torch.cuda.stream(stream):
@@ -277,6 +303,13 @@ def main():
                 dv["D"].copy_(hb["D"], non_blocking=True)
                 if gga:
                     dv["g"].copy_(hb["g"], non_blocking=True)
+                if forces:
+                    dv["Q"].copy_(hb["Q"], non_blocking=True)
+                    ctx.pulay_forces(dv["v"], dv["D"], g=dv["g"] if gga else None, Q=dv["Q"], F=dv["F"], b0=b0, b1=b1)
+                    if world > 1:
+                        dist.all_reduce(dv["F"])
+                    hb["F"].copy_(dv["F"], non_blocking=True)
+                    return
                 ctx.integrate_hamiltonian(dv["v"], dv["g"] if gga else None, H=dv["H"], b0=b0, b1=b1, accumulate=False)
                 if world > 1:
                     dist.all_reduce(dv["H"])
@@ -302,17 +335,22 @@ def main():
             ms_e = float(t.item())
         h2d = 8 * (bun.n_points + bun.n_values + (3 * bun.n_points if gga else 0))
         d2h = 8 * (bun.n_values + my_points * (4 if gga else 1))
+        if forces:
+            h2d, d2h = h2d + 8 * bun.n_values, 8 * 3 * bun.n_atoms
         e2e = {"value": bun.n_points / (ms_e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                "d2h_bytes_per_step": int(d2h), "ms_per_step": ms_e}
         # the end-to-end outputs are the same numbers as the device-resident ones
-        assert torch.equal(hb["n"][int(bun.batch_ptr[b0]):int(bun.batch_ptr[b1])],
-                           n[int(bun.batch_ptr[b0]):int(bun.batch_ptr[b1])].cpu())
+        if forces:
+            assert torch.allclose(hb["F"], F.cpu(), rtol=0, atol=1e-10 * float(F.abs().max()))   # atomics: rounding only
+        else:
+            assert torch.equal(hb["n"][int(bun.batch_ptr[b0]):int(bun.batch_ptr[b1])],
+                               n[int(bun.batch_ptr[b0]):int(bun.batch_ptr[b1])].cpu())
 
     # ---- roofline of the dominant kernel (FP64 tensor pipe), live CUDA-event durations from the timed region
-    kflops = {"k_hamiltonian": flops_h, "k_density": flops_n}
+    kflops = {"k_forces": flops_f} if forces else {"k_hamiltonian": flops_h, "k_density": flops_n}
     dom = max(kflops, key=lambda k: kern[k][0])
     kd = {}
-    for k in ("k_cull", "k_eval", "k_hamiltonian", "k_density"):
+    for k in ("k_cull", "k_eval", "k_forces") if forces else ("k_cull", "k_eval", "k_hamiltonian", "k_density"):
         ms, ln = kern[k]
         kd[k] = {"ms_per_step": ms / args.steps, "launches_per_step": ln / args.steps}
         if k in kflops and ms > 0:
@@ -326,16 +364,16 @@ def main():
                 "peak_measured_probe": peak_measured, "frac_of_measured_probe": achieved / peak_measured,
                 "avg_launch_ms": dom_ms / max(dom_ln, 1), "algorithmic_flops_per_step": kflops[dom],
                 "share_of_step": dom_ms / ms_total}
-    total_tflops = (flops_h + flops_n) / (ms_step * 1e-3) / 1e12
+    total_tflops = (flops_f if forces else flops_h + flops_n) / (ms_step * 1e-3) / 1e12
 
-    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+    out = {"metric": metric, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
            "data": "synthetic",
            "config": {"workload": workload, "n_points": bun.n_points, "n_batches": bun.n_batches, "n_basis": bun.n_basis,
                       "mean_nnz": float(nnz.mean()) if len(nnz) else 0.0, "max_nnz": st["max_nnz"],
                       "max_active_atoms": st["max_active_atoms"], "parallelism": "batch-range x%d" % world,
                       "l2": "inputs larger than L2: each step streams %.1f GB of Phi planes plus a %.2f GB H and D"
-                            % (8e-9 * 6 * st["sum_nnz"] * 208, 8e-9 * bun.n_values)},
+                            % (8e-9 * ((8 if gga else 5) if forces else 6) * st["sum_nnz"] * 208, 8e-9 * bun.n_values)},
            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
            "fp64_tflops_step": total_tflops, "fp64_frac_of_peak_step": total_tflops / FP64_PEAK_NOMINAL_TFLOPS,
            "kernels": kd, "setup_s": {"generate_inputs": t_gen, "create_ctx": t_create}}
@@ -343,7 +381,7 @@ def main():
     # ---- CPU baseline: the oracle on a bounded seeded sample, rank 0 at N=1 only
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         sel = sample_batches(bun.n_batches, args.cpu_sample_batches)
-        pts, dt, cores = time_oracle(bun, sel, gga)
+        pts, dt, cores = time_oracle(bun, sel, gga, forces_q=Qh)
         out["cpu_baseline"] = {"value": pts / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
                                "sample": "%d seeded batches (%d points) of the same workload, %.1f s" % (len(sel), pts, dt)}
     else:

@@ -124,6 +124,20 @@ int aims_gpu_integrate_hamiltonian(aims_gpu_ctx *ctx, int32_t b0, int32_t b1, co
 int aims_gpu_update_density(aims_gpu_ctx *ctx, int32_t b0, int32_t b1, const double *D_values, double *n,
                             double *grad_n);
 
+/* Row f1 of SURVEY.md 8(f): Pulay forces, evaluated on the same batches as the density update (Eq. 14-18
+ * L129-150; L301-308; L405).  For the reduced h_KS of this library (local potential v plus the GGA term above) and
+ * nabla_at phi_i = -grad phi_i for the functions i centred on atom `at`, Eq. 16 and Eq. 18 on the grid:
+ *   F[at][c] (+)= 2 sum_{p in batches [b0,b1)} w_p sum_{i on at} sum_j
+ *        { d_c phi_i [ n_ij (v_p phi_j + g_p . grad phi_j) - q_ij phi_j ]  +  (Hess phi_i g_p)_c n_ij phi_j }   (at r_p)
+ * = -d/dR_at [ Tr(n h(R)) - Tr(q s(R)) ] at fixed n_ij, q_ij, v, g, weights and grid.  The Hellmann-Feynman, multipole and
+ * atomic-ZORA terms (L403, Eq. 19) are not on this path.  DEVICE pointers:
+ *   v [n_points]; g NULL (no GGA term) or [3][n_points]; D_values [n_values] = n_ij and Q_values NULL or [n_values] =
+ *   the energy-weighted density matrix q_ij of Eq. 17, both in the pattern of aims_bsr_desc (symmetric, upper blocks);
+ *   F [n_atoms][3].  accumulate == 0: F is zeroed first.  F is accumulated with floating-point atomics: two runs agree
+ *   to rounding, not bitwise. */
+int aims_gpu_pulay_forces(aims_gpu_ctx *ctx, int32_t b0, int32_t b1, const double *v, const double *g,
+                          const double *D_values, const double *Q_values, double *F, int accumulate);
+
 /* Synchronise the context stream and report anything the device flagged since the last check: an asynchronous CUDA
  * fault (AIMS_ERR_CUDA) or a failed device-side capacity / consistency check (AIMS_ERR_UNSUPPORTED). */
 int aims_gpu_synchronize(aims_gpu_ctx *ctx);
@@ -140,8 +154,8 @@ int aims_gpu_batch_nnz(aims_gpu_ctx *ctx, int32_t *nnz);
 /* Per-kernel device timing for bench.py's roofline: when enabled, every kernel launch of this context is bracketed by
  * CUDA events on the context stream.  aims_gpu_timing_enable synchronises, clears what was recorded and switches
  * recording on (enable != 0) or off.  aims_gpu_timing_read synchronises and returns, since the last enable/read, the
- * summed device milliseconds ms[5] and launch counts launches[5] (HOST outputs) of
- *   [0] k_cull  [1] k_eval  [2] k_hamiltonian  [3] k_density  [4] other. */
+ * summed device milliseconds ms[6] and launch counts launches[6] (HOST outputs) of
+ *   [0] k_cull  [1] k_eval  [2] k_hamiltonian  [3] k_density  [4] other  [5] k_forces. */
 int aims_gpu_timing_enable(aims_gpu_ctx *ctx, int enable);
 int aims_gpu_timing_read(aims_gpu_ctx *ctx, double *ms, int64_t *launches);
 

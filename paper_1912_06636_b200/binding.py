@@ -79,6 +79,8 @@ def load_library():
     L.aims_gpu_integrate_hamiltonian.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp, _vp, ctypes.c_int]
     L.aims_gpu_update_density.restype = ctypes.c_int
     L.aims_gpu_update_density.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp, _vp]
+    L.aims_gpu_pulay_forces.restype = ctypes.c_int
+    L.aims_gpu_pulay_forces.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp, _vp, _vp, _vp, ctypes.c_int]
     L.aims_gpu_synchronize.restype = ctypes.c_int
     L.aims_gpu_synchronize.argtypes = [cp]
     L.aims_gpu_batch_nnz.restype = ctypes.c_int
@@ -126,6 +128,7 @@ class Context:
         self.n_points = int(k["xyz"].shape[0])
         self.n_batches = int(k["batch_ptr"].shape[0] - 1)
         self.n_values = int(bun.n_values)
+        self.n_atoms = int(k["atom_xyz"].shape[0])
         self.batch_ptr = k["batch_ptr"]
         bd = _BasisDesc(int(k["atom_xyz"].shape[0]), int(k["species_shell_ptr"].shape[0] - 1), int(k["shell_l"].shape[0]),
                         int(k["spline_coef"].shape[0]), int(bun.n_knots), d(k["atom_xyz"]), i(k["atom_species"]),
@@ -177,10 +180,10 @@ class Context:
 
     def timing_read(self):
         """{kernel: (device ms, launches)} since the last enable/read."""
-        ms = (ctypes.c_double * 5)()
-        ln = (ctypes.c_int64 * 5)()
+        ms = (ctypes.c_double * 6)()
+        ln = (ctypes.c_int64 * 6)()
         self._check(self.L.aims_gpu_timing_read(self.h, ms, ln), "aims_gpu_timing_read")
-        names = ("k_cull", "k_eval", "k_hamiltonian", "k_density", "other")
+        names = ("k_cull", "k_eval", "k_hamiltonian", "k_density", "other", "k_forces")
         return {k: (ms[i], int(ln[i])) for i, k in enumerate(names)}
 
     def launch_count(self):
@@ -258,6 +261,26 @@ class Context:
                     "aims_gpu_update_density")
         return n, (grad_n if want_grad else None)
 
+    def pulay_forces(self, v, D, g=None, Q=None, F=None, b0=0, b1=None, accumulate=False):
+        """F[n_atoms][3] (device tensor): Pulay forces of batches [b0,b1) (include/aims_gpu.h: aims_gpu_pulay_forces)."""
+        torch = self.torch
+        b0, b1 = self._range(b0, b1)
+        v = self._dev(v, torch.float64)
+        D = self._dev(D, torch.float64)
+        g = None if g is None else self._dev(g, torch.float64)
+        Q = None if Q is None else self._dev(Q, torch.float64)
+        if v.numel() != self.n_points or (g is not None and g.numel() != 3 * self.n_points):
+            raise AimsError("v must have n_points entries and g 3*n_points")
+        if D.numel() != self.n_values or (Q is not None and Q.numel() != self.n_values):
+            raise AimsError("D and Q must have n_values entries")
+        if F is None:
+            with torch.cuda.stream(self.stream):
+                F = torch.empty((self.n_atoms, 3), dtype=torch.float64, device=self.device)
+            accumulate = False
+        self._check(self.L.aims_gpu_pulay_forces(self.h, b0, b1, _ptr(v), _ptr(g), _ptr(D), _ptr(Q), _ptr(F),
+                                                 int(bool(accumulate))), "aims_gpu_pulay_forces")
+        return F
+
     # ---- end-to-end with HOST buffers (pinned): H2D of v, g, D; the two calls; D2H of H, n, grad n
     def make_host_buffers(self, want_grad):
         torch = self.torch
@@ -305,3 +328,7 @@ def aims_gpu_integrate_hamiltonian(ctx, v, g=None, H=None, b0=0, b1=None, accumu
 
 def aims_gpu_update_density(ctx, D, want_grad=False, n=None, grad_n=None, b0=0, b1=None):
     return ctx.update_density(D, want_grad, n, grad_n, b0, b1)
+
+
+def aims_gpu_pulay_forces(ctx, v, D, g=None, Q=None, F=None, b0=0, b1=None, accumulate=False):
+    return ctx.pulay_forces(v, D, g, Q, F, b0, b1, accumulate)

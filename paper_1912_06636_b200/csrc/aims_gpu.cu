@@ -13,6 +13,7 @@
 #include "basis.cuh"
 #include "common.cuh"
 #include "density.cuh"
+#include "forces.cuh"
 #include "hamiltonian.cuh"
 
 using namespace aims;
@@ -39,7 +40,7 @@ struct aims_gpu_ctx {
   HTile *d_tiles = nullptr;
   DItem *d_items = nullptr;
   double flops_h_lda = 0, flops_h_gga = 0, flops_den = 0;
-  bool ptab_in_smem = true;
+  bool ptab_in_smem = true, f_ptab_in_smem = true;
   std::vector<DItem> h_items;                                  // host copy of the density work items
   std::map<std::pair<int, int>, int *> item_order;             // (bs, be) -> device permutation, heaviest item first
 
@@ -53,7 +54,7 @@ struct aims_gpu_ctx {
   std::vector<Span> pool;        // reusable events
 };
 
-enum { kKindCull = 0, kKindEval = 1, kKindHam = 2, kKindDen = 3, kKindOther = 4, kNumKinds = 5 };
+enum { kKindCull = 0, kKindEval = 1, kKindHam = 2, kKindDen = 3, kKindOther = 4, kKindForce = 5, kNumKinds = 6 };
 
 namespace {
 
@@ -340,15 +341,15 @@ int aims_gpu_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_gri
   if ((rc = dev_alloc(c, &L.act_ld, (size_t)c->act_off[nb]))) return rc;
   if ((rc = dev_alloc(c, &L.ptab, (size_t)c->ptab_off[nb]))) return rc;
 
-  // ---- Phi-plane workspace: enough for the largest single batch with 4 planes, at most the requested budget
+  // ---- Phi-plane workspace: enough for the largest single batch with 8 planes (forces), at most the requested budget
   long long want = workspace_bytes > 0 ? workspace_bytes : (24ll << 30);
   size_t free_b = 0, total_b = 0;
   CU_TRY(c, cudaMemGetInfo(&free_b, &total_b));
   want = std::min<long long>(want, (long long)(free_b * 0.8));
   long long max_batch_d = 0;
   for (int b = 0; b < nb; b++) max_batch_d = std::max(max_batch_d, c->dpad_off[b + 1] - c->dpad_off[b]);
-  long long need_all = 4 * c->dpad_off[nb], need_min = 4 * max_batch_d;
-  long long wsd = std::min(need_all, std::max(want / 8, need_min)) + 4 * 64;
+  long long need_all = 8 * c->dpad_off[nb], need_min = 8 * max_batch_d;
+  long long wsd = std::min(need_all, std::max(want / 8, need_min)) + 8 * 64;
   if (wsd * 8 > (long long)free_b) return fail(c, AIMS_ERR_NOMEM, "not enough device memory for one batch of Phi planes");
   if ((rc = dev_alloc(c, &c->ws, (size_t)wsd))) return rc;
   c->ws_doubles = wsd;
@@ -361,6 +362,10 @@ int aims_gpu_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_gri
   if (dsm > (size_t)prop.sharedMemPerBlockOptin) return fail(c, AIMS_ERR_UNSUPPORTED, "nnz(B) too large for the density kernel's shared memory");
   CU_TRY(c, cudaFuncSetAttribute(k_density<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dsm));
   CU_TRY(c, cudaFuncSetAttribute(k_density<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dsm));
+  c->f_ptab_in_smem = f_smem_bytes(c->max_nnz, std::max(c->max_act, 1), true) <= (size_t)prop.sharedMemPerBlockOptin;
+  const size_t fsm = f_smem_bytes(c->max_nnz, std::max(c->max_act, 1), c->f_ptab_in_smem);
+  CU_TRY(c, cudaFuncSetAttribute(k_forces<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsm));
+  CU_TRY(c, cudaFuncSetAttribute(k_forces<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsm));
   CU_TRY(c, cudaStreamSynchronize(c->stream));
   return AIMS_OK;
 }
@@ -525,6 +530,44 @@ int aims_gpu_update_density(aims_gpu_ctx *c, int32_t b0, int32_t b1, const doubl
       TimedLaunch t(c, kKindDen);
       if (grad_n) k_density<true><<<(unsigned)ni, kDThreads, dsm, c->stream>>>(c->S, c->L, A, std::max(c->max_act, 1));
       else k_density<false><<<(unsigned)ni, kDThreads, dsm, c->stream>>>(c->S, c->L, A, std::max(c->max_act, 1));
+    }
+    if ((rc = check_async(c))) return rc;
+    bs = be;
+  }
+  return AIMS_OK;
+}
+
+int aims_gpu_pulay_forces(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, const double *g, const double *D_values,
+                          const double *Q_values, double *F, int accumulate) {
+  if (!range_ok(c, b0, b1)) return fail(c, AIMS_ERR_INVALID_ARG, "batch range outside [0, n_batches]");
+  if (!v || !D_values || !F) return fail(c, AIMS_ERR_INVALID_ARG, "NULL v, D_values or F");
+  CU_TRY(c, cudaSetDevice(c->device));
+  if (!accumulate) CU_TRY(c, cudaMemsetAsync(F, 0, (size_t)c->S.n_atoms * 3 * sizeof(double), c->stream));
+  int rc = run_cull(c, b0, b1);
+  if (rc) return rc;
+  const int npl = g ? 8 : 5;
+  const size_t fsm = f_smem_bytes(c->max_nnz, std::max(c->max_act, 1), c->f_ptab_in_smem);
+  for (int bs = b0; bs < b1;) {
+    const int be = chunk_end(c, c->dpad_off, bs, b1, npl);
+    const long long plane = (c->ws_doubles / npl) & ~63ll;
+    EvalArgs E{};
+    for (int q = 0; q < npl; q++) E.plane[q] = c->ws + q * plane;
+    E.pad_off = c->d_dpad_off; E.pad_base = c->dpad_off[bs]; E.dlayout = 1;
+    E.v = v; E.g = g; E.n_points = c->n_points;
+    if (g) launch_eval<kEvalForceGga>(c, E, bs, be); else launch_eval<kEvalForceLda>(c, E, bs, be);
+    const long long ni = c->item_off[be] - c->item_off[bs];
+    if (ni > 0) {
+      FArgs A{};
+      if ((rc = density_order(c, bs, be, &A.order))) return rc;
+      A.items = c->d_items + c->item_off[bs];
+      A.P = E.plane[0]; A.Lp = E.plane[1];
+      for (int q = 0; q < 6; q++) A.E[q] = (q < npl - 2) ? E.plane[q + 2] : nullptr;
+      A.pad_off = c->d_dpad_off; A.pad_base = c->dpad_off[bs];
+      A.D = D_values; A.Q = Q_values; A.F = F; A.max_nnz_pad = c->max_nnz;
+      A.ptab_in_smem = c->f_ptab_in_smem ? 1 : 0;
+      TimedLaunch t(c, kKindForce);
+      if (g) k_forces<true><<<(unsigned)ni, kDThreads, fsm, c->stream>>>(c->S, c->L, A, std::max(c->max_act, 1));
+      else k_forces<false><<<(unsigned)ni, kDThreads, fsm, c->stream>>>(c->S, c->L, A, std::max(c->max_act, 1));
     }
     if ((rc = check_async(c))) return rc;
     bs = be;

@@ -230,11 +230,18 @@ enum EvalMode {
   kEvalPhi = 0,      // plane0 = Phi                                   (density, LDA; API without gradient)
   kEvalPhiGrad = 1,  // plane0 = Phi, planes 1..3 = d/dx, d/dy, d/dz   (density with grad n; API with gradient)
   kEvalHLda = 2,     // plane0 = Phi, plane1 = w v Phi                 (S2a fused: Eq. 25 "K = w phi" times v)
-  kEvalHGga = 3      // plane0 = Phi, plane1 = w (v/2 Phi + g . grad Phi)
+  kEvalHGga = 3,     // plane0 = Phi, plane1 = w (v/2 Phi + g . grad Phi)
+  // Pulay forces (forces.cuh; Eq. 16, 18 L137-150): plane0 = Phi, plane1 = L = v Phi (+ g . grad Phi),
+  // planes 2..4 = w d/dx_c Phi, and with the GGA term planes 5..7 = w (Hess Phi g)_c
+  kEvalForceLda = 4,
+  kEvalForceGga = 5
 };
+__host__ __device__ constexpr int eval_planes(int mode) {
+  return mode == kEvalPhi ? 1 : mode == kEvalPhiGrad ? 4 : mode == kEvalForceLda ? 5 : mode == kEvalForceGga ? 8 : 2;
+}
 
 struct EvalArgs {
-  double *plane[4];
+  double *plane[8];
   // internal k4 layout (common.cuh): element (row, p) of batch b at
   //   plane[q] + (pad_off[b] - pad_base) + ((p >> 2) * pad8(nnz) + row) * 4 + (p & 3); rows in [nnz, pad8(nnz)) and
   //   points in [n_p, pad8(n_p)) are written as zeros; a batch occupies pad8(nnz) * pad8(n_p) doubles per plane.
@@ -253,6 +260,37 @@ struct EvalArgs {
 };
 
 // ---------------------------------------------------------------------------------------------------------------
+// (Hess S_lm) g for the solid harmonics above (second derivatives of the same polynomials), l <= 3: hx,hy,hz[m].
+// Used by the Pulay-force planes (Eq. 18: the GGA term needs nabla_at grad phi).
+// ---------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void solid_hessian_dot(int l, double x, double y, double z, double px, double py, double pz,
+                                                  double *hx, double *hy, double *hz) {
+  if (l < 2) {
+#pragma unroll
+    for (int m = 0; m < 3; m++) { hx[m] = 0.0; hy[m] = 0.0; hz[m] = 0.0; }
+  } else if (l == 2) {
+    const double a = 1.0925484305920792, bq = 0.31539156525252005, c = 0.5462742152960396;
+    hx[0] = a * py;            hy[0] = a * px;            hz[0] = 0.0;
+    hx[1] = 0.0;               hy[1] = a * pz;            hz[1] = a * py;
+    hx[2] = -2.0 * bq * px;    hy[2] = -2.0 * bq * py;    hz[2] = 4.0 * bq * pz;
+    hx[3] = a * pz;            hy[3] = 0.0;               hz[3] = a * px;
+    hx[4] = 2.0 * c * px;      hy[4] = -2.0 * c * py;     hz[4] = 0.0;
+  } else {
+    const double a = 0.5900435899266435, bq = 2.890611442640554, c = 0.4570457994644658, d = 0.3731763325901154,
+                 e = 1.445305721320277;
+    const double xy = y * px + x * py, xz = z * px + x * pz, yz = z * py + y * pz;   // symmetric pair products
+    const double dxy = x * px - y * py;
+    hx[0] = 6.0 * a * xy;                                    hy[0] = 6.0 * a * dxy;                                   hz[0] = 0.0;
+    hx[1] = bq * yz;                                         hy[1] = bq * xz;                                         hz[1] = bq * xy;
+    hx[2] = -2.0 * c * xy;                                   hy[2] = c * (-2.0 * x * px - 6.0 * y * py + 8.0 * z * pz); hz[2] = 8.0 * c * yz;
+    hx[3] = -6.0 * d * xz;                                   hy[3] = -6.0 * d * yz;                                   hz[3] = d * (-6.0 * x * px - 6.0 * y * py + 12.0 * z * pz);
+    hx[4] = c * (-6.0 * x * px - 2.0 * y * py + 8.0 * z * pz); hy[4] = -2.0 * c * xy;                                 hz[4] = 8.0 * c * xz;
+    hx[5] = 2.0 * e * xz;                                    hy[5] = -2.0 * e * yz;                                   hz[5] = 2.0 * e * dxy;
+    hx[6] = 6.0 * a * dxy;                                   hy[6] = -6.0 * a * xy;                                   hz[6] = 0.0;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------------
 // k_eval: one CTA per batch, one thread per point.  For each active atom: geometry and log once per point, solid
 // harmonics once per l, one spline Horner per shell.  In the k4 layout the four threads of a 4-point group write one
 // full 32-byte sector per row; in the API layout stores are coalesced along the point index.
@@ -261,8 +299,12 @@ struct EvalArgs {
 #define AIMS_EVAL_CTAS_PER_SM 2
 #endif
 template <int MODE>
-__global__ void __launch_bounds__(256, AIMS_EVAL_CTAS_PER_SM) k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first) {
-  constexpr bool GRAD = (MODE == kEvalPhiGrad || MODE == kEvalHGga);
+__global__ void __launch_bounds__(256, (MODE >= kEvalForceLda) ? 1 : AIMS_EVAL_CTAS_PER_SM)
+k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first) {
+  constexpr bool FORCE = (MODE == kEvalForceLda || MODE == kEvalForceGga);
+  constexpr bool HESS = (MODE == kEvalForceGga);
+  constexpr bool GRAD = (MODE == kEvalPhiGrad || MODE == kEvalHGga || FORCE);
+  constexpr int NPL = eval_planes(MODE);
   const int b = b_first + blockIdx.x;
   const int tid = threadIdx.x;
   const long long p0 = S.batch_ptr[b];
@@ -287,18 +329,19 @@ __global__ void __launch_bounds__(256, AIMS_EVAL_CTAS_PER_SM) k_eval(DevSys S, B
   const int nnz8 = pad8(nnz), np8 = pad8(np);
   const int npx = E.api ? np : np8;             // points this CTA writes (API: exactly n_p; k4: zero columns up to pad8)
   const int nrows = E.api ? nnz : (E.dlayout ? round_up(nnz, 16) : nnz8);   // rows this CTA writes
-  double *o0, *o1, *o2 = nullptr, *o3 = nullptr;
+  double *o[NPL];
   if (E.api) {
     const long long off = E.api_off[b] - E.api_base;
-    o0 = E.plane[0] + off;
-    o1 = E.plane[1] ? E.plane[1] + 3 * off : nullptr;
-    const long long cstride = (long long)nnz * np;
-    if (GRAD) { o2 = o1 + cstride; o3 = o2 + cstride; }
+    o[0] = E.plane[0] + off;
+    if (NPL > 1) {
+      const long long cstride = (long long)nnz * np;
+#pragma unroll
+      for (int q = 1; q < NPL; q++) o[q] = E.plane[1] ? E.plane[1] + 3 * off + (q - 1) * cstride : nullptr;
+    }
   } else {
     const long long off = E.pad_off[b] - E.pad_base;
-    o0 = E.plane[0] + off;
-    o1 = E.plane[1] + off;
-    if (MODE == kEvalPhiGrad) { o2 = E.plane[2] + off; o3 = E.plane[3] + off; }
+#pragma unroll
+    for (int q = 0; q < NPL; q++) o[q] = E.plane[q] + off;
   }
   const int nk1 = S.n_knots - 1;
 
@@ -308,28 +351,28 @@ __global__ void __launch_bounds__(256, AIMS_EVAL_CTAS_PER_SM) k_eval(DevSys S, B
     const long long rs = E.api ? (long long)np : 4;
     const long long cs = E.dlayout ? (long long)np8 * 16 - 64 : 0;   // extra jump at every 16-row chunk boundary
 #define AIMS_EIDX(row) (pb + (long long)(row) * rs + (long long)((row) >> 4) * cs)
+#define AIMS_EZERO(idx)                                   \
+  {                                                       \
+    const long long o_ = (idx);                           \
+    _Pragma("unroll") for (int q_ = 0; q_ < NPL; q_++) o[q_][o_] = 0.0; \
+  }
     if (p >= np) {  // zero padding columns (k4 layout only)
-      for (int r = 0; r < nrows; r++) {
-        const long long o = AIMS_EIDX(r);
-        o0[o] = 0.0;
-        if (MODE != kEvalPhi) o1[o] = 0.0;
-        if (MODE == kEvalPhiGrad) { o2[o] = 0.0; o3[o] = 0.0; }
-      }
+      for (int r = 0; r < nrows; r++) AIMS_EZERO(AIMS_EIDX(r))
       continue;
     }
-    for (int r = nnz; r < nrows; r++) {   // zero padding rows (k4 layout only)
-      const long long o = AIMS_EIDX(r);
-      o0[o] = 0.0;
-      if (MODE != kEvalPhi) o1[o] = 0.0;
-      if (MODE == kEvalPhiGrad) { o2[o] = 0.0; o3[o] = 0.0; }
-    }
+    for (int r = nnz; r < nrows; r++) AIMS_EZERO(AIMS_EIDX(r))   // zero padding rows (k4 layout only)
     const double x = S.px[p0 + p], y = S.py[p0 + p], z = S.pz[p0 + p];
-    double wv = 0.0, wgx = 0.0, wgy = 0.0, wgz = 0.0;
+    double wv = 0.0, wgx = 0.0, wgy = 0.0, wgz = 0.0, w = 0.0;
     if (MODE == kEvalHLda) wv = S.w[p0 + p] * E.v[p0 + p];
     if (MODE == kEvalHGga) {
-      const double w = S.w[p0 + p];
+      w = S.w[p0 + p];
       wv = 0.5 * w * E.v[p0 + p];
       wgx = w * E.g[p0 + p]; wgy = w * E.g[E.n_points + p0 + p]; wgz = w * E.g[2 * E.n_points + p0 + p];
+    }
+    if (FORCE) {   // here wv = v and (wgx, wgy, wgz) = g, unweighted; the weight multiplies the epilogue planes
+      w = S.w[p0 + p];
+      wv = E.v[p0 + p];
+      if (HESS) { wgx = E.g[p0 + p]; wgy = E.g[E.n_points + p0 + p]; wgz = E.g[2 * E.n_points + p0 + p]; }
     }
     for (int s = 0; s < nact; s++) {
       const double dx = x - s_ax[s], dy = y - s_ay[s], dz = z - s_az[s];
@@ -343,52 +386,76 @@ __global__ void __launch_bounds__(256, AIMS_EVAL_CTAS_PER_SM) k_eval(DevSys S, B
       k = max(0, min(k, S.n_knots - 2));
       const double xs = t - (double)k;
       const double inv_dd = 1.0 / dd;
+      const double ug = HESS ? (ux * wgx + uy * wgy + uz * wgz) : 0.0;
       const unsigned mask = s_mask[s];
       long long row = s_row0[s];
       int lcur = -1;
       double Y[7], gx[7], gy[7], gz[7];
+      double hx[HESS ? 7 : 1], hy[HESS ? 7 : 1], hz[HESS ? 7 : 1];
       for (int sh = s_s0[s]; sh < s_s1[s]; sh++) {
         if (!(mask >> (sh - s_s0[s]) & 1u)) continue;
         const int l = S.shell_l[sh];
         const int nm = 2 * l + 1;
         if (d2 < S.shell_rc2[sh]) {
-          if (l != lcur) { solid_harmonics<GRAD>(l, ux, uy, uz, Y, gx, gy, gz); lcur = l; }
+          if (l != lcur) {
+            solid_harmonics<GRAD>(l, ux, uy, uz, Y, gx, gy, gz);
+            if constexpr (HESS) solid_hessian_dot(l, ux, uy, uz, wgx, wgy, wgz, hx, hy, hz);
+            lcur = l;
+          }
           const double2 *cf = reinterpret_cast<const double2 *>(S.spline_coef + ((long long)S.shell_spline[sh] * nk1 + k) * 4);
           const double2 c01 = __ldg(cf), c23 = __ldg(cf + 1);
           const double R = c01.x + xs * (c01.y + xs * (c23.x + xs * c23.y));
-          double f = 0.0, Rd = 0.0;
+          double f = 0.0, Rd = 0.0, hA = 0.0, hB = 0.0, hC = 0.0;
           if (GRAD) {
-            const double dR = (c01.y + xs * (2.0 * c23.x + xs * 3.0 * c23.y)) / (S.log_inc * dd);
+            const double Rt = c01.y + xs * (2.0 * c23.x + xs * 3.0 * c23.y);
+            const double sc = S.log_inc * dd;
+            const double dR = Rt / sc;
             Rd = R * inv_dd;
             f = dR - (double)l * Rd;
+            if (HESS) {
+              // Hess phi = A u u^T Y + B (1 - u u^T) Y + B (u gS^T + gS u^T) + C Hess S, phi = (R / d^l) S_lm(dvec)
+              const double Rtt = 2.0 * c23.x + 6.0 * c23.y * xs;
+              const double d2R = Rtt / (sc * sc) - Rt / (sc * dd);
+              hA = d2R - 2.0 * (double)l * dR * inv_dd + (double)(l * (l + 1)) * Rd * inv_dd;
+              hB = f * inv_dd;
+              hC = Rd * inv_dd;
+            }
           }
 #pragma unroll
           for (int m = 0; m < 7; m++) {
             if (m < nm) {
               const double phi = R * Y[m];
-              const long long o = AIMS_EIDX(row + m);
-              o0[o] = phi;
-              if (MODE == kEvalHLda) o1[o] = wv * phi;
+              const long long oi = AIMS_EIDX(row + m);
+              o[0][oi] = phi;
+              if (MODE == kEvalHLda) o[1][oi] = wv * phi;
               if (GRAD) {
                 const double fy = f * Y[m];
                 const double ex = fy * ux + Rd * gx[m], ey = fy * uy + Rd * gy[m], ez = fy * uz + Rd * gz[m];
-                if (MODE == kEvalPhiGrad) { o1[o] = ex; o2[o] = ey; o3[o] = ez; }
-                else o1[o] = wv * phi + (wgx * ex + wgy * ey + wgz * ez);
+                if (MODE == kEvalPhiGrad) { o[1][oi] = ex; o[2][oi] = ey; o[3][oi] = ez; }
+                if (MODE == kEvalHGga) o[1][oi] = wv * phi + (wgx * ex + wgy * ey + wgz * ez);
+                if (FORCE) {
+                  o[1][oi] = HESS ? wv * phi + (wgx * ex + wgy * ey + wgz * ez) : wv * phi;
+                  o[2 % NPL][oi] = w * ex; o[3 % NPL][oi] = w * ey; o[4 % NPL][oi] = w * ez;
+                  if (HESS) {
+                    const double gsg = gx[m] * wgx + gy[m] * wgy + gz[m] * wgz;
+                    const double along = (hA - hB) * ug * Y[m] + hB * gsg;      // coefficient of u
+                    const double by = hB * Y[m], bug = hB * ug;
+                    o[5 % NPL][oi] = w * (along * ux + by * wgx + bug * gx[m] + hC * hx[m]);
+                    o[6 % NPL][oi] = w * (along * uy + by * wgy + bug * gy[m] + hC * hy[m]);
+                    o[7 % NPL][oi] = w * (along * uz + by * wgz + bug * gz[m] + hC * hz[m]);
+                  }
+                }
               }
             }
           }
         } else {
-          for (int m = 0; m < nm; m++) {
-            const long long o = AIMS_EIDX(row + m);
-            o0[o] = 0.0;
-            if (MODE != kEvalPhi) o1[o] = 0.0;
-            if (MODE == kEvalPhiGrad) { o2[o] = 0.0; o3[o] = 0.0; }
-          }
+          for (int m = 0; m < nm; m++) AIMS_EZERO(AIMS_EIDX(row + m))
         }
         row += nm;
       }
     }
   }
+#undef AIMS_EZERO
 #undef AIMS_EIDX
 }
 

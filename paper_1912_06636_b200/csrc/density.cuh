@@ -88,6 +88,84 @@ __device__ __forceinline__ void d_mma_stage(int variant, double (&acc)[4][4][2],
 #undef AIMS_D_CASE
 }
 
+// Producer side of one K stage: the tile D_b[i0 + r][k0 .. k0+15], r < tm, of the symmetric block-sparse matrix M restricted
+// to nnz(B) ("calculate_density_mat"), written as [4-function group][row][4] into dA.  pl = 0..63.
+__device__ __forceinline__ void d_gather_tile(double *dA, const double *M, int i0, int tm, int k0, int nnz, int nnz8, int nact,
+                                              const int *sInfo, const int *sLd, const long long *ptab, int pl) {
+  // D_b[i0 + r][k0 + 4t .. +3]: one (row, 4-function group) per lane and pass; gathered from the block pattern
+  // (stored block (si,sj) for si <= sj, transposed read of block (sj,si) below the diagonal)
+  const int ng = min(kDKC, nnz8 - k0) >> 2;          // 4-function groups with at least one real function
+  for (int t = 0; t < ng; t++)
+  for (int r = pl; r < tm; r += kDProdLanes) {       // consecutive lanes -> consecutive rows (transposed reads coalesce)
+    const int i = i0 + r, j = k0 + 4 * t;
+    const unsigned dst = smem_u32(dA + (t * tm + r) * 4);
+    if (i >= nnz) {
+#pragma unroll
+      for (int q = 0; q < 4; q++) cp_async8(dst + 8u * q, M, 0);
+      continue;
+    }
+    const int fi = sInfo[i];
+    const int si = fi >> 16, ri = fi & 0xFFFF;
+    const int4 fj4 = *reinterpret_cast<const int4 *>(sInfo + j);   // sInfo is padded with -1 up to nnz8
+    const int fjq[4] = {fj4.x, fj4.y, fj4.z, fj4.w};
+    if (fj4.w >= 0 && (fj4.x >> 16) == (fj4.w >> 16) && (fj4.w - fj4.x) == 3) {
+      // fast path: four consecutive functions of one atom
+      const int sj = fj4.x >> 16, cj = fj4.x & 0xFFFF;
+      const long long base = ptab[si * nact + sj];
+      const double *src = M;
+      long long stride = 0;
+      int bytes = 0;
+      if (base >= 0) {
+        bytes = 8;
+        if (si <= sj) { src = M + base + (long long)ri * sLd[sj] + cj; stride = 1; }
+        else { src = M + base + (long long)cj * sLd[si] + ri; stride = sLd[si]; }
+      }
+#pragma unroll
+      for (int q = 0; q < 4; q++) cp_async8(dst + 8u * q, src + q * stride, bytes);
+    } else {
+#pragma unroll
+      for (int q = 0; q < 4; q++) {
+        const double *src = M;
+        int bytes = 0;
+        if (fjq[q] >= 0) {
+          const int sj = fjq[q] >> 16, cj = fjq[q] & 0xFFFF;
+          const long long base = ptab[si * nact + sj];
+          if (base >= 0) {
+            src = (si <= sj) ? M + base + (long long)ri * sLd[sj] + cj : M + base + (long long)cj * sLd[si] + ri;
+            bytes = 8;
+          }
+        }
+        cp_async8(dst + 8u * q, src, bytes);
+      }
+    }
+  }
+}
+
+// Deal the PB*IB blocks (work ~ point sub-tiles wb) to the MMA warps so that the four SM sub-partitions carry equal
+// DMMA load: sub-partition q hosts MMA warps q, q+4, q+8(, q+12) -- 2 and 3 have only three because the producers
+// sit there.  Blocks in descending size go to the sub-partition whose remaining slots need the largest average.
+// s_map[warp] = pb | ib << 8, -1 = idle.  One thread.
+__device__ __forceinline__ void d_deal_blocks(int *s_map, int PB, int IB, int psub) {
+  const int nb = PB * IB;
+  int cnt[4], load[4] = {0, 0, 0, 0}, used[4] = {0, 0, 0, 0}, total = 0;
+  for (int q = 0; q < 4; q++) cnt[q] = nb / 4 + (q < (nb & 3) ? 1 : 0);
+  for (int w = 0; w < kDMmaWarps; w++) s_map[w] = -1;
+  for (int pb2 = 0; pb2 < PB; pb2++) total += IB * ((blk_start(pb2 + 1, psub, PB) - blk_start(pb2, psub, PB)) >> 3);
+  for (int sz = 4; sz >= 1; sz--)
+    for (int pb2 = 0; pb2 < PB; pb2++) {
+      if (((blk_start(pb2 + 1, psub, PB) - blk_start(pb2, psub, PB)) >> 3) != sz) continue;
+      for (int ib2 = 0; ib2 < IB; ib2++) {
+        int best = -1;
+        for (int q = 0; q < 4; q++) {
+          if (used[q] >= cnt[q]) continue;
+          if (best < 0 || (total - 4 * load[q]) * (cnt[best] - used[best]) > (total - 4 * load[best]) * (cnt[q] - used[q])) best = q;
+        }
+        s_map[best + 4 * used[best]] = pb2 | (ib2 << 8);
+        used[best]++; load[best] += sz;
+      }
+    }
+}
+
 template <bool GRAD>
 __global__ void __launch_bounds__(kDThreads, 1) k_density(DevSys S, BatchLists L, DArgs A, int max_act) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -129,27 +207,7 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density(DevSys S, BatchLists L
       mbar_init(bar_empty + 8 * s, kDMmaWarps);
     }
     mbar_fence_init();
-    // Deal the PB*IB blocks (work ~ point sub-tiles wb) to the MMA warps so that the four SM sub-partitions carry equal
-    // DMMA load: sub-partition q hosts MMA warps q, q+4, q+8(, q+12) -- 2 and 3 have only three because the producers
-    // sit there.  Blocks in descending size go to the sub-partition whose remaining slots need the largest average.
-    const int nb = PB * IB;
-    int cnt[4], load[4] = {0, 0, 0, 0}, used[4] = {0, 0, 0, 0}, total = 0;
-    for (int q = 0; q < 4; q++) cnt[q] = nb / 4 + (q < (nb & 3) ? 1 : 0);
-    for (int w = 0; w < kDMmaWarps; w++) s_map[w] = -1;
-    for (int pb2 = 0; pb2 < PB; pb2++) total += IB * ((blk_start(pb2 + 1, psub, PB) - blk_start(pb2, psub, PB)) >> 3);
-    for (int sz = 4; sz >= 1; sz--)
-      for (int pb2 = 0; pb2 < PB; pb2++) {
-        if (((blk_start(pb2 + 1, psub, PB) - blk_start(pb2, psub, PB)) >> 3) != sz) continue;
-        for (int ib2 = 0; ib2 < IB; ib2++) {
-          int best = -1;
-          for (int q = 0; q < 4; q++) {
-            if (used[q] >= cnt[q]) continue;
-            if (best < 0 || (total - 4 * load[q]) * (cnt[best] - used[best]) > (total - 4 * load[best]) * (cnt[q] - used[q])) best = q;
-          }
-          s_map[best + 4 * used[best]] = pb2 | (ib2 << 8);
-          used[best]++; load[best] += sz;
-        }
-      }
+    d_deal_blocks(s_map, PB, IB, psub);
   }
   __syncthreads();
   const long long *ptab = A.ptab_in_smem ? sPtab : gptab;
@@ -185,54 +243,7 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density(DevSys S, BatchLists L
         bulk_g2s(smem_u32(sB + (size_t)s * kDStage), gP + ((long long)kc * (np8 >> 2) + (p0 >> 2)) * 64, (unsigned)npt * 128u,
                  bar_full + 8 * s);
       }
-      // D_b[i0 + r][k0 + 4t .. +3]: one (row, 4-function group) per lane and pass; gathered from the block pattern
-      // (stored block (si,sj) for si <= sj, transposed read of block (sj,si) below the diagonal)
-      double *dA = sA + (size_t)s * kDStage;
-      const int ng = min(kDKC, nnz8 - k0) >> 2;          // 4-function groups with at least one real function
-      for (int t = 0; t < ng; t++)
-      for (int r = pl; r < tm; r += kDProdLanes) {       // consecutive lanes -> consecutive rows (transposed reads coalesce)
-        const int i = i0 + r, j = k0 + 4 * t;
-        const unsigned dst = smem_u32(dA + (t * tm + r) * 4);
-        if (i >= nnz) {
-#pragma unroll
-          for (int q = 0; q < 4; q++) cp_async8(dst + 8u * q, A.D, 0);
-          continue;
-        }
-        const int fi = sInfo[i];
-        const int si = fi >> 16, ri = fi & 0xFFFF;
-        const int4 fj4 = *reinterpret_cast<const int4 *>(sInfo + j);   // sInfo is padded with -1 up to nnz8
-        const int fjq[4] = {fj4.x, fj4.y, fj4.z, fj4.w};
-        if (fj4.w >= 0 && (fj4.x >> 16) == (fj4.w >> 16) && (fj4.w - fj4.x) == 3) {
-          // fast path: four consecutive functions of one atom
-          const int sj = fj4.x >> 16, cj = fj4.x & 0xFFFF;
-          const long long base = ptab[si * nact + sj];
-          const double *src = A.D;
-          long long stride = 0;
-          int bytes = 0;
-          if (base >= 0) {
-            bytes = 8;
-            if (si <= sj) { src = A.D + base + (long long)ri * sLd[sj] + cj; stride = 1; }
-            else { src = A.D + base + (long long)cj * sLd[si] + ri; stride = sLd[si]; }
-          }
-#pragma unroll
-          for (int q = 0; q < 4; q++) cp_async8(dst + 8u * q, src + q * stride, bytes);
-        } else {
-#pragma unroll
-          for (int q = 0; q < 4; q++) {
-            const double *src = A.D;
-            int bytes = 0;
-            if (fjq[q] >= 0) {
-              const int sj = fjq[q] >> 16, cj = fjq[q] & 0xFFFF;
-              const long long base = ptab[si * nact + sj];
-              if (base >= 0) {
-                src = (si <= sj) ? A.D + base + (long long)ri * sLd[sj] + cj : A.D + base + (long long)cj * sLd[si] + ri;
-                bytes = 8;
-              }
-            }
-            cp_async8(dst + 8u * q, src, bytes);
-          }
-        }
-      }
+      d_gather_tile(sA + (size_t)s * kDStage, A.D, i0, tm, k0, nnz, nnz8, nact, sInfo, sLd, ptab, pl);
       cp_async_mbar_arrive_noinc(bar_full + 8 * s);
       }
     }
