@@ -161,16 +161,7 @@ __global__ void __launch_bounds__(kDThreads, 1) k_forces(DevSys S, BatchLists L,
         const int nseg = pass == 0 ? nseg0 : 1;
 #pragma unroll 1
         for (int seg = 0; seg < nseg; seg++) {
-#pragma unroll 1
-          for (int kc = 0; kc < nkc; kc++, step++) {
-            const int s = step % kDStages;
-            mbar_wait(bar_full + 8 * s, (unsigned)(step / kDStages) & 1u);
-            if (blive)
-              d_mma_stage(variant, acc, sA + (size_t)s * kDStage + aoffl, sB + (size_t)s * kDStage + boffl, tm,
-                          min(kDKC, nnz8 - kc * kDKC) >> 2);
-            __syncwarp();
-            if (lane == 0) mbar_arrive(bar_empty + 8 * s);
-          }
+          d_mma_kloop(blive ? variant : 0, acc, sA + aoffl, sB + boffl, tm, nkc, nnz8, step, bar_full, bar_empty, lane);
           if (seg < nseg - 1) {
             // end of the q_b Phi segment: flip the sign, n_b L is added on top in the next segment (X = n_b L - q_b Phi)
 #pragma unroll
