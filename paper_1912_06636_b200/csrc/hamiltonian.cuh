@@ -55,39 +55,91 @@ constexpr size_t h_smem_bytes() {
          2 * kHStages * sizeof(unsigned long long) + (kHI + kHJ + kMaxActive) * sizeof(int);
 }
 
-// one 4-point group of one warp block: (8 WA) x (8 WB) outputs, straight-line unpredicated DMMAs
-template <int WA, int WB, bool DIAG, bool GGA>
-__device__ __forceinline__ void h_mma_group(double (&acc)[4][4][2], const double *gb, int aoff, int boff) {
+// The whole point loop of one warp block of (8 WA) x (8 WB) outputs as ONE instruction stream of straight-line,
+// unpredicated DMMAs.  A stage holds two 4-point groups; per group LDA has one product step (P_I Q_J^T), GGA two
+// (P_I Q_J^T, then Q_I P_J^T).  Operand fragments are reloaded in place while the DMMAs of the current step are issued
+// (an A fragment is dead after its row, a B fragment after the last row that uses it; on a diagonal block row a uses
+// only columns c >= a, so B fragment a dies with row a), and the reloads of a stage's last step already fetch the first
+// step of the NEXT stage, whose "full" barrier is waited for after the first row of DMMAs is in the pipe (see
+// density.cuh: d_mma_kloop_t for the measurements behind this).
+// refill(q): called by lane 0 after chunk q was released -- the kernel's rotating refill duty.
+template <int WA, int WB, bool DIAG, bool GGA, class Refill>
+__device__ __forceinline__ void h_mma_loop_t(double (&acc)[4][4][2], const double *sm, int aoff, int boff, int nchunk,
+                                             unsigned bar_full, unsigned bar_empty, int lane, Refill &&refill) {
+  constexpr int NST = kHStages;
+  constexpr int GW = h_group_doubles<GGA>(), SW = h_stage_doubles<GGA>();
+  constexpr int NU = GGA ? 4 : 2;                                       // product steps per stage
+  // fragment bases of step u inside a stage
+  auto a_base = [&](const double *st, int u) {
+    return st + (GGA ? (u >> 1) : u) * GW + ((GGA && (u & 1)) ? (kHI + kHJ) * 4 : 0) + aoff;
+  };
+  auto b_base = [&](const double *st, int u) {
+    return st + (GGA ? (u >> 1) : u) * GW + ((GGA && (u & 1)) ? (2 * kHI + kHJ) * 4 : kHI * 4) + boff;
+  };
+  mbar_wait(bar_full, 0u);
+  const double *st = sm;
   double fa[WA], fb[WB];
+  {
+    const double *a0 = a_base(st, 0), *b0 = b_base(st, 0);
 #pragma unroll
-  for (int a = 0; a < WA; a++) fa[a] = gb[aoff + a * 32];                       // P_I
+    for (int a = 0; a < WA; a++) fa[a] = a0[a * 32];
 #pragma unroll
-  for (int c = 0; c < WB; c++) fb[c] = gb[kHI * 4 + boff + c * 32];             // Q_J
+    for (int c = 0; c < WB; c++) fb[c] = b0[c * 32];
+  }
+#pragma unroll 1
+  for (int q = 0; q < nchunk; q++) {
+    const int s = q % NST;
+    const double *st1 = st;
 #pragma unroll
-  for (int a = 0; a < WA; a++)
+    for (int u = 0; u < NU; u++) {
+      const double *a1, *b1;
+      // row 0 first, then (last step of the stage) make sure the next stage has landed before reloading from it
 #pragma unroll
-    for (int c = 0; c < WB; c++)
-      if (!DIAG || c >= a) dmma8x8x4(acc[a][c][0], acc[a][c][1], fa[a], fb[c]);
-  if (GGA) {
+      for (int c = 0; c < WB; c++) dmma8x8x4(acc[0][c][0], acc[0][c][1], fa[0], fb[c]);
+      if (u + 1 < NU) {
+        a1 = a_base(st, u + 1); b1 = b_base(st, u + 1);
+      } else {
+        if (q + 1 < nchunk) {
+          const int s1 = (q + 1) % NST;
+          mbar_wait(bar_full + 8 * s1, (unsigned)((q + 1) / NST) & 1u);
+          st1 = sm + (size_t)s1 * SW;
+        }
+        a1 = a_base(st1, 0); b1 = b_base(st1, 0);                       // no next chunk: harmless reload of this stage
+      }
+      fa[0] = a1[0];
+      if (DIAG || WA == 1) fb[0] = b1[0];
 #pragma unroll
-    for (int a = 0; a < WA; a++) fa[a] = gb[(kHI + kHJ) * 4 + aoff + a * 32];   // Q_I
+      for (int a = 1; a < WA; a++) {
 #pragma unroll
-    for (int c = 0; c < WB; c++) fb[c] = gb[(2 * kHI + kHJ) * 4 + boff + c * 32];  // P_J
+        for (int c = 0; c < WB; c++)
+          if (!DIAG || c >= a) {
+            dmma8x8x4(acc[a][c][0], acc[a][c][1], fa[a], fb[c]);
+            if (!DIAG && a == WA - 1) fb[c] = b1[c * 32];
+          }
+        fa[a] = a1[a * 32];
+        if (DIAG) fb[a] = b1[a * 32];
+      }
+      if (!DIAG && WA == 1) {
 #pragma unroll
-    for (int a = 0; a < WA; a++)
-#pragma unroll
-      for (int c = 0; c < WB; c++)
-        if (!DIAG || c >= a) dmma8x8x4(acc[a][c][0], acc[a][c][1], fa[a], fb[c]);
+        for (int c = 1; c < WB; c++) fb[c] = b1[c * 32];
+      }
+    }
+    st = st1;
+    __syncwarp();
+    if (lane == 0) {
+      mbar_arrive(bar_empty + 8 * s);                     // every fragment of stage s is in registers
+      refill(q);
+    }
+    __syncwarp();
   }
 }
 
-template <bool GGA>
-__device__ __forceinline__ void h_mma_stage(int variant, double (&acc)[4][4][2], const double *st, int aoff, int boff) {
-  constexpr int GW = h_group_doubles<GGA>();
-#define AIMS_H_CASE(WA, WB, DG)                                                          \
-  case (WA * 4 + WB) * 2 + DG:                                                           \
-    h_mma_group<WA, WB, DG != 0, GGA>(acc, st, aoff, boff);                              \
-    h_mma_group<WA, WB, DG != 0, GGA>(acc, st + GW, aoff, boff);                         \
+template <bool GGA, class Refill>
+__device__ __forceinline__ void h_mma_loop(int variant, double (&acc)[4][4][2], const double *sm, int aoff, int boff,
+                                           int nchunk, unsigned bar_full, unsigned bar_empty, int lane, Refill &&refill) {
+#define AIMS_H_CASE(WA, WB, DG)                                                                              \
+  case (WA * 4 + WB) * 2 + DG:                                                                               \
+    h_mma_loop_t<WA, WB, DG != 0, GGA>(acc, sm, aoff, boff, nchunk, bar_full, bar_empty, lane, refill);     \
     break;
   switch (variant) {
     AIMS_H_CASE(4, 4, 0) AIMS_H_CASE(4, 3, 0) AIMS_H_CASE(3, 4, 0) AIMS_H_CASE(3, 3, 0)
@@ -196,23 +248,14 @@ __global__ void __launch_bounds__(kHThreads, 2) k_hamiltonian(DevSys S, BatchLis
 #pragma unroll
     for (int c = 0; c < 4; c++) { acc[a][c][0] = 0.0; acc[a][c][1] = 0.0; }
 
-#pragma unroll 1
-  for (int q = 0; q < nchunk; q++) {
-    const int s = q % NST;
-    mbar_wait(bar_full + 8 * s, (unsigned)(q / NST) & 1u);
-    h_mma_stage<GGA>(variant, acc, sm + (size_t)s * SW, aoff, boff);
-    __syncwarp();
-    if (lane == 0) {
-      mbar_arrive(bar_empty + 8 * s);                     // this warp is done reading stage s
-      // refill the stage released one chunk ago (lagged by one so that the wait below is normally already satisfied)
-      const int qq = q - 1;
-      if (qq >= 0 && qq + NST < nchunk && slot == qq % nlive) {
-        mbar_wait(bar_empty + 8 * (qq % NST), (unsigned)(qq / NST) & 1u);
-        issue(qq + NST);
-      }
+  h_mma_loop<GGA>(variant, acc, sm, aoff, boff, nchunk, bar_full, bar_empty, lane, [&](int q) {
+    // refill the stage released one chunk ago (lagged by one so that the wait below is normally already satisfied)
+    const int qq = q - 1;
+    if (qq >= 0 && qq + NST < nchunk && slot == qq % nlive) {
+      mbar_wait(bar_empty + 8 * (qq % NST), (unsigned)(qq / NST) & 1u);
+      issue(qq + NST);
     }
-    __syncwarp();
-  }
+  });
 
   // ---- epilogue (S2d): per warp, 8-row strips through shared memory, then coalesced REDs along the block row
   double *strip = s_strip + warp * (8 * kHStripLd);
