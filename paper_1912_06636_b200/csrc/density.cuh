@@ -352,21 +352,35 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density(DevSys S, BatchLists L
             const int col = ps0 + c * 8 + 2 * fk;            // within the CTA's point range (even)
             const int p = p0 + col;                          // within the batch
             double sn[2] = {0.0, 0.0}, sg[3][2] = {{0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}};
+            // two row sub-tiles at a time: all their loads (L2-prefetched by the producers) are issued before the first
+            // FMA, so that an epilogue costs 2 x wb load round trips instead of 4 x wb
+            constexpr int NQ = GRAD ? 4 : 1;
 #pragma unroll
-            for (int a = 0; a < 4; a++) {
-              if (a < wa) {
-                const int i = ri0 + a * 8 + fr;              // < nnz8: padding rows are zero in the planes
-                const long long o = (((long long)(i >> 4) * (np8 >> 2) + (p >> 2)) * 16 + (i & 15)) * 4 + (p & 3);
-                const double2 ph = *reinterpret_cast<const double2 *>(gP + o);
-                sn[0] += ph.x * acc[a][c][0];
-                sn[1] += ph.y * acc[a][c][1];
-                if (GRAD)
+            for (int a0 = 0; a0 < 4; a0 += 2) {
+              if (a0 < wa) {
+                double2 ev[2][NQ];
 #pragma unroll
-                  for (int q = 0; q < 3; q++) {
-                    const double2 gq = *reinterpret_cast<const double2 *>(A.G[q] + boff + o);
-                    sg[q][0] += gq.x * acc[a][c][0];
-                    sg[q][1] += gq.y * acc[a][c][1];
+                for (int da = 0; da < 2; da++) {
+                  const int i = ri0 + min(a0 + da, wa - 1) * 8 + fr;   // < nnz8: padding rows are zero in the planes
+                  const long long o = (((long long)(i >> 4) * (np8 >> 2) + (p >> 2)) * 16 + (i & 15)) * 4 + (p & 3);
+                  ev[da][0] = __ldg(reinterpret_cast<const double2 *>(gP + o));
+                  if (GRAD)
+#pragma unroll
+                    for (int q = 0; q < 3; q++) ev[da][q + 1] = __ldg(reinterpret_cast<const double2 *>(A.G[q] + boff + o));
+                }
+#pragma unroll
+                for (int da = 0; da < 2; da++) {
+                  if (a0 + da < wa) {
+                    sn[0] += ev[da][0].x * acc[a0 + da][c][0];
+                    sn[1] += ev[da][0].y * acc[a0 + da][c][1];
+                    if (GRAD)
+#pragma unroll
+                      for (int q = 0; q < 3; q++) {
+                        sg[q][0] += ev[da][q + 1].x * acc[a0 + da][c][0];
+                        sg[q][1] += ev[da][q + 1].y * acc[a0 + da][c][1];
+                      }
                   }
+                }
               }
             }
 #pragma unroll

@@ -172,37 +172,42 @@ __global__ void __launch_bounds__(kDThreads, 1) k_forces(DevSys S, BatchLists L,
         }
         if (blive) {
           // ---- epilogue of this pass: row sums over the block's points of acc * (weighted derivative plane)
-          double f[4][3];
+          // two row sub-tiles at a time; per point sub-tile their six loads (L2-prefetched by the producers) are issued
+          // before the first FMA
 #pragma unroll
-          for (int a = 0; a < 4; a++) { f[a][0] = 0.0; f[a][1] = 0.0; f[a][2] = 0.0; }
+          for (int a0 = 0; a0 < 4; a0 += 2) {
+            if (a0 < wa) {
+              double f[2][3] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}};
+              const int i_[2] = {ri0 + a0 * 8 + fr, ri0 + min(a0 + 1, wa - 1) * 8 + fr};   // < nnz8: padding rows are zero in the planes
 #pragma unroll
-          for (int c = 0; c < 4; c++) {
-            if (c < wb) {
-              const int p = p0 + ps0 + c * 8 + 2 * fk;           // within the batch (even)
+              for (int c = 0; c < 4; c++) {
+                if (c < wb) {
+                  const int p = p0 + ps0 + c * 8 + 2 * fk;           // within the batch (even)
+                  double2 ev[2][3];
 #pragma unroll
-              for (int a = 0; a < 4; a++) {
-                if (a < wa) {
-                  const int i = ri0 + a * 8 + fr;                // < nnz8 <= round_up(nnz,16): padding rows are zero in the planes
-                  const long long o = boff + (((long long)(i >> 4) * (np8 >> 2) + (p >> 2)) * 16 + (i & 15)) * 4 + (p & 3);
+                  for (int da = 0; da < 2; da++) {
+                    const int i = i_[da];
+                    const long long o = boff + (((long long)(i >> 4) * (np8 >> 2) + (p >> 2)) * 16 + (i & 15)) * 4 + (p & 3);
 #pragma unroll
-                  for (int q = 0; q < 3; q++) {
-                    const double2 e = *reinterpret_cast<const double2 *>(A.E[3 * pass + q] + o);
-                    f[a][q] += e.x * acc[a][c][0] + e.y * acc[a][c][1];
+                    for (int q = 0; q < 3; q++) ev[da][q] = __ldg(reinterpret_cast<const double2 *>(A.E[3 * pass + q] + o));
                   }
+#pragma unroll
+                  for (int da = 0; da < 2; da++)
+#pragma unroll
+                    for (int q = 0; q < 3; q++)
+                      f[da][q] += ev[da][q].x * acc[min(a0 + da, 3)][c][0] + ev[da][q].y * acc[min(a0 + da, 3)][c][1];
                 }
               }
-            }
-          }
 #pragma unroll
-          for (int a = 0; a < 4; a++) {
-            if (a < wa) {
-              const int fi = sInfo[ri0 + a * 8 + fr];
+              for (int da = 0; da < 2; da++) {
+                const int fi = sInfo[i_[da]];
 #pragma unroll
-              for (int q = 0; q < 3; q++) {
-                double v = f[a][q];
-                v += __shfl_xor_sync(0xffffffffu, v, 1);
-                v += __shfl_xor_sync(0xffffffffu, v, 2);
-                if (fk == 0 && fi >= 0) atomicAdd(sF + (fi >> 16) * 3 + q, v);
+                for (int q = 0; q < 3; q++) {
+                  double v = f[da][q];
+                  v += __shfl_xor_sync(0xffffffffu, v, 1);
+                  v += __shfl_xor_sync(0xffffffffu, v, 2);
+                  if (fk == 0 && fi >= 0 && a0 + da < wa) atomicAdd(sF + (fi >> 16) * 3 + q, v);
+                }
               }
             }
           }
