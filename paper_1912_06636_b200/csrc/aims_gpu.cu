@@ -366,6 +366,14 @@ int aims_gpu_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_gri
   const size_t fsm = f_smem_bytes(c->max_nnz, std::max(c->max_act, 1), c->f_ptab_in_smem);
   CU_TRY(c, cudaFuncSetAttribute(k_forces<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsm));
   CU_TRY(c, cudaFuncSetAttribute(k_forces<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsm));
+  {
+    const int esm = (int)eval_smem_bytes(c->max_nnz);
+    if ((size_t)esm + 4096 > (size_t)prop.sharedMemPerBlockOptin) return fail(c, AIMS_ERR_UNSUPPORTED, "nnz(B) too large for the evaluation kernel's shared memory");
+#define EV_ATTR(M, LY) CU_TRY(c, cudaFuncSetAttribute(k_eval<M, LY>, cudaFuncAttributeMaxDynamicSharedMemorySize, esm));
+    EV_ATTR(kEvalPhi, kLayApi) EV_ATTR(kEvalPhiGrad, kLayApi) EV_ATTR(kEvalHLda, kLayH) EV_ATTR(kEvalHGga, kLayH)
+    EV_ATTR(kEvalPhi, kLayD) EV_ATTR(kEvalPhiGrad, kLayD) EV_ATTR(kEvalForceLda, kLayD) EV_ATTR(kEvalForceGga, kLayD)
+#undef EV_ATTR
+  }
   CU_TRY(c, cudaStreamSynchronize(c->stream));
   return AIMS_OK;
 }
@@ -442,10 +450,10 @@ int density_order(aims_gpu_ctx *c, int bs, int be, const int **out) {
   return AIMS_OK;
 }
 
-template <int MODE>
+template <int MODE, int LAYOUT>
 void launch_eval(aims_gpu_ctx *c, const EvalArgs &E, int bs, int be) {
   TimedLaunch t(c, kKindEval);
-  k_eval<MODE><<<be - bs, 256, 0, c->stream>>>(c->S, c->L, E, bs);
+  k_eval<MODE, LAYOUT><<<be - bs, 256, eval_smem_bytes(c->max_nnz), c->stream>>>(c->S, c->L, E, bs, std::max(c->max_nnz, 1));
 }
 
 }  // namespace
@@ -464,9 +472,9 @@ int aims_gpu_eval_basis(aims_gpu_ctx *c, int32_t b0, int32_t b1, int64_t *fn_ptr
   if (b1 > b0) {
     EvalArgs E{};
     E.plane[0] = phi; E.plane[1] = dphi;
-    E.api = 1; E.api_off = c->d_api_off; E.api_base = c->api_off[b0];
+    E.api_off = c->d_api_off; E.api_base = c->api_off[b0];
     E.n_points = c->n_points;
-    if (dphi) launch_eval<kEvalPhiGrad>(c, E, b0, b1); else launch_eval<kEvalPhi>(c, E, b0, b1);
+    if (dphi) launch_eval<kEvalPhiGrad, kLayApi>(c, E, b0, b1); else launch_eval<kEvalPhi, kLayApi>(c, E, b0, b1);
   }
   return check_async(c);
 }
@@ -486,7 +494,7 @@ int aims_gpu_integrate_hamiltonian(aims_gpu_ctx *c, int32_t b0, int32_t b1, cons
     E.plane[0] = c->ws; E.plane[1] = c->ws + plane;
     E.pad_off = c->d_pad_off; E.pad_base = c->pad_off[bs];
     E.v = v; E.g = g; E.n_points = c->n_points;
-    if (g) launch_eval<kEvalHGga>(c, E, bs, be); else launch_eval<kEvalHLda>(c, E, bs, be);
+    if (g) launch_eval<kEvalHGga, kLayH>(c, E, bs, be); else launch_eval<kEvalHLda, kLayH>(c, E, bs, be);
     const long long nt = c->tile_off[be] - c->tile_off[bs];
     if (nt > 0) {
       HArgs A{c->d_tiles + c->tile_off[bs], E.plane[0], E.plane[1], c->d_pad_off, c->pad_off[bs], H_values};
@@ -514,9 +522,9 @@ int aims_gpu_update_density(aims_gpu_ctx *c, int32_t b0, int32_t b1, const doubl
     EvalArgs E{};
     for (int q = 0; q < npl; q++) E.plane[q] = c->ws + q * plane;
     if (!grad_n) E.plane[1] = c->ws;  // unused
-    E.pad_off = c->d_dpad_off; E.pad_base = c->dpad_off[bs]; E.dlayout = 1;
+    E.pad_off = c->d_dpad_off; E.pad_base = c->dpad_off[bs];
     E.n_points = c->n_points;
-    if (grad_n) launch_eval<kEvalPhiGrad>(c, E, bs, be); else launch_eval<kEvalPhi>(c, E, bs, be);
+    if (grad_n) launch_eval<kEvalPhiGrad, kLayD>(c, E, bs, be); else launch_eval<kEvalPhi, kLayD>(c, E, bs, be);
     const long long ni = c->item_off[be] - c->item_off[bs];
     if (ni > 0) {
       DArgs A{};
@@ -552,9 +560,9 @@ int aims_gpu_pulay_forces(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double 
     const long long plane = (c->ws_doubles / npl) & ~63ll;
     EvalArgs E{};
     for (int q = 0; q < npl; q++) E.plane[q] = c->ws + q * plane;
-    E.pad_off = c->d_dpad_off; E.pad_base = c->dpad_off[bs]; E.dlayout = 1;
+    E.pad_off = c->d_dpad_off; E.pad_base = c->dpad_off[bs];
     E.v = v; E.g = g; E.n_points = c->n_points;
-    if (g) launch_eval<kEvalForceGga>(c, E, bs, be); else launch_eval<kEvalForceLda>(c, E, bs, be);
+    if (g) launch_eval<kEvalForceGga, kLayD>(c, E, bs, be); else launch_eval<kEvalForceLda, kLayD>(c, E, bs, be);
     const long long ni = c->item_off[be] - c->item_off[bs];
     if (ni > 0) {
       FArgs A{};

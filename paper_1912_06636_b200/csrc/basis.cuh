@@ -1,6 +1,8 @@
 // basis.cuh -- S1a (active-function culling, nnz(B): PAPER.md L235) and S1b (basis evaluation, "calculate_phi":
 // PAPER.md L314/L322/L356) on the GPU.  The paper keeps this stage on the CPU (L381); here it is two kernels.
 #pragma once
+#include <algorithm>
+
 #include "common.cuh"
 
 namespace aims {
@@ -242,19 +244,17 @@ __host__ __device__ constexpr int eval_planes(int mode) {
 
 struct EvalArgs {
   double *plane[8];
-  // internal k4 layout (common.cuh): element (row, p) of batch b at
+  // kLayH, the k4 layout of common.cuh: element (row, p) of batch b at
   //   plane[q] + (pad_off[b] - pad_base) + ((p >> 2) * pad8(nnz) + row) * 4 + (p & 3); rows in [nnz, pad8(nnz)) and
   //   points in [n_p, pad8(n_p)) are written as zeros; a batch occupies pad8(nnz) * pad8(n_p) doubles per plane.
-  // dlayout != 0: the density layout, chunks of 16 rows: (((row >> 4) * (np8 >> 2) + (p >> 2)) * 16 + (row & 15)) * 4 + (p & 3),
+  // kLayD, chunks of 16 rows: (((row >> 4) * (np8 >> 2) + (p >> 2)) * 16 + (row & 15)) * 4 + (p & 3),
   //   rows padded with zeros to a multiple of 16; a batch occupies round_up(nnz,16) * pad8(n_p) doubles per plane
   const long long *pad_off;
   long long pad_base;
-  // API layout (api != 0): phi at plane[0] + (api_off[b]-api_base) + row*np + p,
-  //                        dphi component c at plane[1] + 3*(api_off[b]-api_base) + (c*nnz + row)*np + p
+  // kLayApi: phi at plane[0] + (api_off[b]-api_base) + row*np + p,
+  //          dphi component c at plane[1] + 3*(api_off[b]-api_base) + (c*nnz + row)*np + p
   const long long *api_off;
   long long api_base;
-  int api;
-  int dlayout;           // internal planes in the density layout (common.cuh "k4 layout, chunked") instead of the H layout
   const double *v, *g;   // [n_points], [3][n_points]
   long long n_points;
 };
@@ -291,16 +291,34 @@ __device__ __forceinline__ void solid_hessian_dot(int l, double x, double y, dou
 }
 
 // ---------------------------------------------------------------------------------------------------------------
-// k_eval: one CTA per batch, one thread per point.  For each active atom: geometry and log once per point, solid
-// harmonics once per l, one spline Horner per shell.  In the k4 layout the four threads of a 4-point group write one
-// full 32-byte sector per row; in the API layout stores are coalesced along the point index.
+// k_eval: one CTA per batch, one thread per point.
+//   set-up   the batch's active shells become a flat list in shared memory: (slot, l, first row, spline row, rcut^2)
+//   per point walk the list: geometry and ONE log per (point, atom) when the slot changes, solid harmonics once per l,
+//            one spline Horner per shell, then 2l+1 values per output plane.
+// The output layout is a template parameter, so that an element address is one 32-bit multiply-add on a per-plane base
+// pointer: kLayApi (aims_gpu_eval_basis: [row][point]), kLayH (k4 layout of hamiltonian.cuh), kLayD (k4 layout in chunks
+// of 16 rows of density.cuh / forces.cuh).  In the k4 layouts the four threads of a 4-point group write one full 32-byte
+// sector per row; in the API layout stores are coalesced along the point index.
 // ---------------------------------------------------------------------------------------------------------------
+enum EvalLayout { kLayApi = 0, kLayH = 1, kLayD = 2 };
+
 #ifndef AIMS_EVAL_CTAS_PER_SM
 #define AIMS_EVAL_CTAS_PER_SM 2
 #endif
-template <int MODE>
+// dynamic shared memory of k_eval: one entry per active shell of the batch (<= nnz(B) of them)
+inline size_t eval_smem_bytes(int max_nnz) { return (size_t)std::max(max_nnz, 1) * (sizeof(int2) + sizeof(double)); }
+
+template <int LAYOUT>
+__device__ __forceinline__ int eval_row_off(int row, int np, int np8) {
+  // offset of (row, point 0-of-thread) relative to the thread's point base
+  if (LAYOUT == kLayApi) return row * np;
+  if (LAYOUT == kLayH) return row * 4;
+  return row * 4 + (row >> 4) * (np8 * 16 - 64);
+}
+
+template <int MODE, int LAYOUT>
 __global__ void __launch_bounds__(256, (MODE >= kEvalForceLda) ? 1 : AIMS_EVAL_CTAS_PER_SM)
-k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first) {
+k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
   constexpr bool FORCE = (MODE == kEvalForceLda || MODE == kEvalForceGga);
   constexpr bool HESS = (MODE == kEvalForceGga);
   constexpr bool GRAD = (MODE == kEvalPhiGrad || MODE == kEvalHGga || FORCE);
@@ -313,54 +331,76 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first) {
   if (nnz == 0 || np == 0) return;
   const long long ao = L.act_off[b];
 
+  extern __shared__ __align__(16) unsigned char eval_smem[];
+  double *s_rc2 = reinterpret_cast<double *>(eval_smem);                 // [n_ent]
+  int2 *s_ent = reinterpret_cast<int2 *>(s_rc2 + max_ent);                // [n_ent] x = slot | l << 8 | row << 12, y = spline row
   __shared__ double s_ax[kMaxActive], s_ay[kMaxActive], s_az[kMaxActive];
-  __shared__ int s_s0[kMaxActive], s_s1[kMaxActive], s_row0[kMaxActive];
-  __shared__ unsigned s_mask[kMaxActive];
+  __shared__ int s_e0[kMaxActive + 1];
+  const int nk1 = S.n_knots - 1;
   for (int s = tid; s < nact; s += 256) {
     const int a = L.act_atom[ao + s];
     s_ax[s] = S.atom_xyz[3 * a]; s_ay[s] = S.atom_xyz[3 * a + 1]; s_az[s] = S.atom_xyz[3 * a + 2];
+    s_e0[s + 1] = __popc(L.act_mask[ao + s]);
+  }
+  __syncthreads();
+  if (tid == 0) {
+    int e = 0;
+    s_e0[0] = 0;
+    for (int s = 0; s < nact; s++) { const int c = s_e0[s + 1]; s_e0[s] = e; e += c; }
+    s_e0[nact] = e;
+  }
+  __syncthreads();
+  const int n_ent = s_e0[nact];
+  if (n_ent > max_ent) { if (tid == 0) atomicExch(L.error_flag, 4); return; }
+  for (int s = tid; s < nact; s += 256) {
+    const int a = L.act_atom[ao + s];
     const int sp = S.atom_species[a];
-    s_s0[s] = S.sp_shell_ptr[sp]; s_s1[s] = S.sp_shell_ptr[sp + 1];
-    s_row0[s] = L.act_row0[ao + s];
-    s_mask[s] = L.act_mask[ao + s];
+    const int s0 = S.sp_shell_ptr[sp], s1 = S.sp_shell_ptr[sp + 1];
+    const unsigned mask = L.act_mask[ao + s];
+    int row = L.act_row0[ao + s], e = s_e0[s];
+    for (int sh = s0; sh < s1; sh++) {
+      if (!(mask >> (sh - s0) & 1u)) continue;
+      const int l = S.shell_l[sh];
+      s_ent[e] = make_int2(s | (l << 8) | (row << 12), S.shell_spline[sh] * nk1);
+      s_rc2[e] = S.shell_rc2[sh];
+      row += 2 * l + 1;
+      e++;
+    }
   }
   __syncthreads();
 
   const int nnz8 = pad8(nnz), np8 = pad8(np);
-  const int npx = E.api ? np : np8;             // points this CTA writes (API: exactly n_p; k4: zero columns up to pad8)
-  const int nrows = E.api ? nnz : (E.dlayout ? round_up(nnz, 16) : nnz8);   // rows this CTA writes
+  const int npx = LAYOUT == kLayApi ? np : np8;             // points this CTA writes (k4: zero columns up to pad8)
+  const int nrows = LAYOUT == kLayApi ? nnz : (LAYOUT == kLayD ? round_up(nnz, 16) : nnz8);   // rows this CTA writes
   double *o[NPL];
-  if (E.api) {
+  if (LAYOUT == kLayApi) {
     const long long off = E.api_off[b] - E.api_base;
     o[0] = E.plane[0] + off;
-    if (NPL > 1) {
-      const long long cstride = (long long)nnz * np;
+    const long long cstride = (long long)nnz * np;
 #pragma unroll
-      for (int q = 1; q < NPL; q++) o[q] = E.plane[1] ? E.plane[1] + 3 * off + (q - 1) * cstride : nullptr;
-    }
+    for (int q = 1; q < NPL; q++) o[q] = E.plane[1] + 3 * off + (q - 1) * cstride;
   } else {
     const long long off = E.pad_off[b] - E.pad_base;
 #pragma unroll
     for (int q = 0; q < NPL; q++) o[q] = E.plane[q] + off;
   }
-  const int nk1 = S.n_knots - 1;
 
   for (int p = tid; p < npx; p += 256) {
-    // element (row, p) at pb + (row >> 4) * cs + (row & 15) * rs  [D layout]   or   pb + row * rs  [API, H layout]
-    const long long pb = E.api ? (long long)p : (E.dlayout ? (long long)(p >> 2) * 64 + (p & 3) : ((long long)(p >> 2) * nnz8) * 4 + (p & 3));
-    const long long rs = E.api ? (long long)np : 4;
-    const long long cs = E.dlayout ? (long long)np8 * 16 - 64 : 0;   // extra jump at every 16-row chunk boundary
-#define AIMS_EIDX(row) (pb + (long long)(row) * rs + (long long)((row) >> 4) * cs)
-#define AIMS_EZERO(idx)                                   \
-  {                                                       \
-    const long long o_ = (idx);                           \
-    _Pragma("unroll") for (int q_ = 0; q_ < NPL; q_++) o[q_][o_] = 0.0; \
+    // the thread's point base inside the batch's plane; element (row, p) at pbase + eval_row_off(row)
+    const int pbase = LAYOUT == kLayApi ? p : (LAYOUT == kLayH ? (p >> 2) * nnz8 * 4 + (p & 3) : (p >> 2) * 64 + (p & 3));
+    double *op[NPL];
+#pragma unroll
+    for (int q = 0; q < NPL; q++) op[q] = o[q] + pbase;
+#define AIMS_EZERO(idx)                                                  \
+  {                                                                      \
+    const int o_ = (idx);                                                \
+    _Pragma("unroll") for (int q_ = 0; q_ < NPL; q_++) op[q_][o_] = 0.0; \
   }
-    if (p >= np) {  // zero padding columns (k4 layout only)
-      for (int r = 0; r < nrows; r++) AIMS_EZERO(AIMS_EIDX(r))
+    if (p >= np) {  // zero padding columns (k4 layouts only)
+      for (int r = 0; r < nrows; r++) AIMS_EZERO(eval_row_off<LAYOUT>(r, np, np8))
       continue;
     }
-    for (int r = nnz; r < nrows; r++) AIMS_EZERO(AIMS_EIDX(r))   // zero padding rows (k4 layout only)
+    for (int r = nnz; r < nrows; r++) AIMS_EZERO(eval_row_off<LAYOUT>(r, np, np8))   // zero padding rows
     const double x = S.px[p0 + p], y = S.py[p0 + p], z = S.pz[p0 + p];
     double wv = 0.0, wgx = 0.0, wgy = 0.0, wgz = 0.0, w = 0.0;
     if (MODE == kEvalHLda) wv = S.w[p0 + p] * E.v[p0 + p];
@@ -374,89 +414,93 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first) {
       wv = E.v[p0 + p];
       if (HESS) { wgx = E.g[p0 + p]; wgy = E.g[E.n_points + p0 + p]; wgz = E.g[2 * E.n_points + p0 + p]; }
     }
-    for (int s = 0; s < nact; s++) {
-      const double dx = x - s_ax[s], dy = y - s_ay[s], dz = z - s_az[s];
-      const double d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
-      const double d = sqrt(d2);
-      double ux = 0.0, uy = 0.0, uz = 1.0;
-      if (d > 0.0) { const double inv = 1.0 / d; ux = dx * inv; uy = dy * inv; uz = dz * inv; }
-      const double dd = fmax(d, S.r0);
-      const double t = log(dd / S.r0) / S.log_inc;
-      int k = (int)floor(t);
-      k = max(0, min(k, S.n_knots - 2));
-      const double xs = t - (double)k;
-      const double inv_dd = 1.0 / dd;
-      const double ug = HESS ? (ux * wgx + uy * wgy + uz * wgz) : 0.0;
-      const unsigned mask = s_mask[s];
-      long long row = s_row0[s];
-      int lcur = -1;
-      double Y[7], gx[7], gy[7], gz[7];
-      double hx[HESS ? 7 : 1], hy[HESS ? 7 : 1], hz[HESS ? 7 : 1];
-      for (int sh = s_s0[s]; sh < s_s1[s]; sh++) {
-        if (!(mask >> (sh - s_s0[s]) & 1u)) continue;
-        const int l = S.shell_l[sh];
-        const int nm = 2 * l + 1;
-        if (d2 < S.shell_rc2[sh]) {
-          if (l != lcur) {
-            solid_harmonics<GRAD>(l, ux, uy, uz, Y, gx, gy, gz);
-            if constexpr (HESS) solid_hessian_dot(l, ux, uy, uz, wgx, wgy, wgz, hx, hy, hz);
-            lcur = l;
+    int cur = -1, lcur = -1, k = 0;
+    double d2 = 0.0, ux = 0.0, uy = 0.0, uz = 1.0, dd = 1.0, inv_dd = 1.0, xs = 0.0, ug = 0.0;
+    double Y[7], gx[7], gy[7], gz[7];
+    double hx[HESS ? 7 : 1], hy[HESS ? 7 : 1], hz[HESS ? 7 : 1];
+#pragma unroll 1
+    for (int e = 0; e < n_ent; e++) {
+      const int2 en = s_ent[e];
+      const int slot = en.x & 0xFF, l = (en.x >> 8) & 3, row = en.x >> 12;
+      if (slot != cur) {
+        cur = slot; lcur = -1;
+        const double dx = x - s_ax[slot], dy = y - s_ay[slot], dz = z - s_az[slot];
+        d2 = __dadd_rn(__dadd_rn(__dmul_rn(dx, dx), __dmul_rn(dy, dy)), __dmul_rn(dz, dz));
+        const double d = sqrt(d2);
+        ux = 0.0; uy = 0.0; uz = 1.0;
+        if (d > 0.0) { const double inv = 1.0 / d; ux = dx * inv; uy = dy * inv; uz = dz * inv; }
+        dd = fmax(d, S.r0);
+        const double t = log(dd / S.r0) / S.log_inc;
+        k = (int)floor(t);
+        k = max(0, min(k, S.n_knots - 2));
+        xs = t - (double)k;
+        inv_dd = 1.0 / dd;
+        if (HESS) ug = ux * wgx + uy * wgy + uz * wgz;
+      }
+      const int nm = 2 * l + 1;
+      const int ro = eval_row_off<LAYOUT>(row, np, np8);
+      // offset of row + m: rows of one shell may straddle a 16-row chunk boundary in the D layout
+      const int mstep = LAYOUT == kLayApi ? np : 4;
+      const int wrap = LAYOUT == kLayD ? 16 - (row & 15) : 8;          // first m that lies in the next chunk
+      const int jump = LAYOUT == kLayD ? np8 * 16 - 64 : 0;
+      if (d2 < s_rc2[e]) {
+        if (l != lcur) {
+          solid_harmonics<GRAD>(l, ux, uy, uz, Y, gx, gy, gz);
+          if constexpr (HESS) solid_hessian_dot(l, ux, uy, uz, wgx, wgy, wgz, hx, hy, hz);
+          lcur = l;
+        }
+        const double2 *cf = reinterpret_cast<const double2 *>(S.spline_coef + (long long)(en.y + k) * 4);
+        const double2 c01 = __ldg(cf), c23 = __ldg(cf + 1);
+        const double R = c01.x + xs * (c01.y + xs * (c23.x + xs * c23.y));
+        double f = 0.0, Rd = 0.0, hA = 0.0, hB = 0.0, hC = 0.0;
+        if (GRAD) {
+          const double Rt = c01.y + xs * (2.0 * c23.x + xs * 3.0 * c23.y);
+          const double sc = S.log_inc * dd;
+          const double dR = Rt / sc;
+          Rd = R * inv_dd;
+          f = dR - (double)l * Rd;
+          if (HESS) {
+            // Hess phi = A u u^T Y + B (1 - u u^T) Y + B (u gS^T + gS u^T) + C Hess S, phi = (R / d^l) S_lm(dvec)
+            const double Rtt = 2.0 * c23.x + 6.0 * c23.y * xs;
+            const double d2R = Rtt / (sc * sc) - Rt / (sc * dd);
+            hA = d2R - 2.0 * (double)l * dR * inv_dd + (double)(l * (l + 1)) * Rd * inv_dd;
+            hB = f * inv_dd;
+            hC = Rd * inv_dd;
           }
-          const double2 *cf = reinterpret_cast<const double2 *>(S.spline_coef + ((long long)S.shell_spline[sh] * nk1 + k) * 4);
-          const double2 c01 = __ldg(cf), c23 = __ldg(cf + 1);
-          const double R = c01.x + xs * (c01.y + xs * (c23.x + xs * c23.y));
-          double f = 0.0, Rd = 0.0, hA = 0.0, hB = 0.0, hC = 0.0;
-          if (GRAD) {
-            const double Rt = c01.y + xs * (2.0 * c23.x + xs * 3.0 * c23.y);
-            const double sc = S.log_inc * dd;
-            const double dR = Rt / sc;
-            Rd = R * inv_dd;
-            f = dR - (double)l * Rd;
-            if (HESS) {
-              // Hess phi = A u u^T Y + B (1 - u u^T) Y + B (u gS^T + gS u^T) + C Hess S, phi = (R / d^l) S_lm(dvec)
-              const double Rtt = 2.0 * c23.x + 6.0 * c23.y * xs;
-              const double d2R = Rtt / (sc * sc) - Rt / (sc * dd);
-              hA = d2R - 2.0 * (double)l * dR * inv_dd + (double)(l * (l + 1)) * Rd * inv_dd;
-              hB = f * inv_dd;
-              hC = Rd * inv_dd;
-            }
-          }
+        }
 #pragma unroll
-          for (int m = 0; m < 7; m++) {
-            if (m < nm) {
-              const double phi = R * Y[m];
-              const long long oi = AIMS_EIDX(row + m);
-              o[0][oi] = phi;
-              if (MODE == kEvalHLda) o[1][oi] = wv * phi;
-              if (GRAD) {
-                const double fy = f * Y[m];
-                const double ex = fy * ux + Rd * gx[m], ey = fy * uy + Rd * gy[m], ez = fy * uz + Rd * gz[m];
-                if (MODE == kEvalPhiGrad) { o[1][oi] = ex; o[2][oi] = ey; o[3][oi] = ez; }
-                if (MODE == kEvalHGga) o[1][oi] = wv * phi + (wgx * ex + wgy * ey + wgz * ez);
-                if (FORCE) {
-                  o[1][oi] = HESS ? wv * phi + (wgx * ex + wgy * ey + wgz * ez) : wv * phi;
-                  o[2 % NPL][oi] = w * ex; o[3 % NPL][oi] = w * ey; o[4 % NPL][oi] = w * ez;
-                  if (HESS) {
-                    const double gsg = gx[m] * wgx + gy[m] * wgy + gz[m] * wgz;
-                    const double along = (hA - hB) * ug * Y[m] + hB * gsg;      // coefficient of u
-                    const double by = hB * Y[m], bug = hB * ug;
-                    o[5 % NPL][oi] = w * (along * ux + by * wgx + bug * gx[m] + hC * hx[m]);
-                    o[6 % NPL][oi] = w * (along * uy + by * wgy + bug * gy[m] + hC * hy[m]);
-                    o[7 % NPL][oi] = w * (along * uz + by * wgz + bug * gz[m] + hC * hz[m]);
-                  }
+        for (int m = 0; m < 7; m++) {
+          if (m < nm) {
+            const double phi = R * Y[m];
+            const int oi = ro + m * mstep + (m >= wrap ? jump : 0);
+            op[0][oi] = phi;
+            if (MODE == kEvalHLda) op[1 % NPL][oi] = wv * phi;
+            if (GRAD) {
+              const double fy = f * Y[m];
+              const double ex = fy * ux + Rd * gx[m], ey = fy * uy + Rd * gy[m], ez = fy * uz + Rd * gz[m];
+              if (MODE == kEvalPhiGrad) { op[1 % NPL][oi] = ex; op[2 % NPL][oi] = ey; op[3 % NPL][oi] = ez; }
+              if (MODE == kEvalHGga) op[1 % NPL][oi] = wv * phi + (wgx * ex + wgy * ey + wgz * ez);
+              if (FORCE) {
+                op[1 % NPL][oi] = HESS ? wv * phi + (wgx * ex + wgy * ey + wgz * ez) : wv * phi;
+                op[2 % NPL][oi] = w * ex; op[3 % NPL][oi] = w * ey; op[4 % NPL][oi] = w * ez;
+                if (HESS) {
+                  const double gsg = gx[m] * wgx + gy[m] * wgy + gz[m] * wgz;
+                  const double along = (hA - hB) * ug * Y[m] + hB * gsg;      // coefficient of u
+                  const double by = hB * Y[m], bug = hB * ug;
+                  op[5 % NPL][oi] = w * (along * ux + by * wgx + bug * gx[m] + hC * hx[m]);
+                  op[6 % NPL][oi] = w * (along * uy + by * wgy + bug * gy[m] + hC * hy[m]);
+                  op[7 % NPL][oi] = w * (along * uz + by * wgz + bug * gz[m] + hC * hz[m]);
                 }
               }
             }
           }
-        } else {
-          for (int m = 0; m < nm; m++) AIMS_EZERO(AIMS_EIDX(row + m))
         }
-        row += nm;
+      } else {
+        for (int m = 0; m < nm; m++) AIMS_EZERO(ro + m * mstep + (m >= wrap ? jump : 0))
       }
     }
   }
 #undef AIMS_EZERO
-#undef AIMS_EIDX
 }
 
 // copy the per-batch lists of [b0,b1) into caller arrays (aims_gpu_eval_basis outputs)
