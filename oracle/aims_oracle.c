@@ -668,3 +668,118 @@ void orc_brute_forces(const orc_system *S, const double *v, const double *g, con
   free(phi);
   free(afp);
 }
+
+/* ====================================================================================================================
+ * Kinetic term of h_KS (Eq. 4 L73 h_ij = <phi_i|h_KS|phi_j>, Eq. 24-27
+ * L228-260, Fig. 6a "h_times_phi" then DSYR2K).  With (h phi_j)(r) = -1/2 lap phi_j(r) + v(r) phi_j(r) the batch
+ * product K.L of Eq. 27 is not symmetric on the grid; Fig. 6a symmetrises it with DSYR2K, read here with alpha = 1/2
+ * (reading P1b):
+ *   h_ij[B] = 1/2 sum_{r in B} w(r) [ phi_i (h phi_j) + (h phi_i) phi_j ](r)   [+ the GGA term of O3, already symmetric].
+ * lap phi is the trace of the Hessian of orc_shell_hess_at_point (pinned by finite differences in
+ * tests/test_oracle_force_pins.py); the brute-force version below uses the radial form
+ *   lap (R(d) Y_lm) = (R'' + 2 R'/d - l(l+1) R/d^2) Y_lm   instead, so that the two pin each other.
+ * Further pins (tests/test_oracle_kinetic_pins.py): closed-form kinetic integrals of Gaussians; T symmetric positive
+ * semidefinite; reduces to O3 for kinetic == 0.
+ * ==================================================================================================================== */
+void orc_integrate_hamiltonian_ks(const orc_system *S, int n_sel, const int32_t *batches, const double *v, const double *g,
+                                  int kinetic, double *H_values) {
+  int64_t *afp = (int64_t *)malloc(sizeof(int64_t) * (S->n_atoms + 1));
+  orc_atom_fn_ptr(S, afp);
+  int nf_tot = (int)afp[S->n_atoms];
+  int32_t *idx = (int32_t *)malloc(sizeof(int32_t) * 4 * (size_t)nf_tot);
+  int32_t *fa = idx + nf_tot, *fs = fa + nf_tot, *fm = fs + nf_tot;
+  for (int q = 0; q < n_sel; q++) {
+    int b = batches[q];
+    int64_t p0 = S->batch_ptr[b];
+    int np = (int)(S->batch_ptr[b + 1] - p0);
+    int nnz = orc_batch_nnz(S, b, idx, fa, fs, fm);
+    if (nnz == 0 || np == 0) continue;
+    size_t sz = (size_t)nnz * np;
+    double *phi = (double *)malloc(sizeof(double) * sz * 3);   /* phi, L = h phi, G = g . grad phi */
+    double *Lp = phi + sz, *G = phi + 2 * sz;
+    for (int i = 0; i < nnz;) {
+      int l = S->shell_l[fs[i]];
+      for (int p = 0; p < np; p++) {
+        double val[7], gr[7][3], hh[7][6];
+        orc_shell_hess_at_point(S, fa[i], fs[i], S->xyz + 3 * (p0 + p), val, gr, hh);
+        for (int m = 0; m < 2 * l + 1; m++) {
+          size_t o = (size_t)(i + m) * np + p;
+          double lap = (hh[m][0] + hh[m][1]) + hh[m][2];
+          phi[o] = val[m];
+          Lp[o] = v[p0 + p] * val[m];
+          if (kinetic) Lp[o] += -0.5 * lap;
+          double s = 0.0;
+          if (g) for (int c = 0; c < 3; c++) s += g[(size_t)c * S->n_points + p0 + p] * gr[m][c];
+          G[o] = s;
+        }
+      }
+      i += 2 * l + 1;
+    }
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int i = 0; i < nnz; i++) {
+      int A = fa[i];
+      int ai = (int)(idx[i] - afp[A]);
+      for (int j = 0; j < nnz; j++) {
+        int B = fa[j];
+        if (B < A) continue;
+        int ld;
+        int64_t off = find_block(S, A, B, &ld);
+        if (off < 0) continue;
+        int bj = (int)(idx[j] - afp[B]);
+        double h = 0.0;
+        for (int p = 0; p < np; p++) {
+          double wp = S->w[p0 + p];
+          double pi_ = phi[(size_t)i * np + p], pj = phi[(size_t)j * np + p];
+          double term = 0.5 * wp * (pi_ * Lp[(size_t)j * np + p] + Lp[(size_t)i * np + p] * pj);
+          if (g) term += wp * (G[(size_t)i * np + p] * pj + pi_ * G[(size_t)j * np + p]);
+          h += term;
+        }
+        H_values[off + (int64_t)ai * ld + bj] += h;
+      }
+    }
+    free(phi);
+  }
+  free(idx);
+  free(afp);
+}
+
+/* brute force (tiny inputs only): dense Hd[n_basis][n_basis] = 1/2 sum_p w [phi_i (h phi_j) + (h phi_i) phi_j],
+ * h phi = -1/2 (R'' + 2 R'/d - l(l+1) R/d^2) Y_lm + v phi, all functions x all points, no batches, no culling. */
+void orc_brute_kinetic(const orc_system *S, const double *v, double *Hd) {
+  int64_t *afp = (int64_t *)malloc(sizeof(int64_t) * (S->n_atoms + 1));
+  orc_atom_fn_ptr(S, afp);
+  int nb = (int)afp[S->n_atoms];
+  double *phi = (double *)malloc(sizeof(double) * (size_t)nb * 2);
+  double *Lp = phi + nb;
+  for (int64_t p = 0; p < S->n_points; p++) {
+    int i = 0;
+    for (int a = 0; a < S->n_atoms; a++) {
+      int sp = S->atom_species[a];
+      for (int s = S->species_shell_ptr[sp]; s < S->species_shell_ptr[sp + 1]; s++) {
+        int l = S->shell_l[s];
+        double rc = S->shell_rcut[s], dv[3];
+        double d2 = dist2(S->xyz + 3 * p, S->atom_xyz + 3 * a, dv);
+        double Y[7];
+        double R = 0.0, dR = 0.0, d2R = 0.0, dd = 1.0;
+        int inside = d2 < rc * rc;
+        if (inside) {
+          double d = sqrt(d2);
+          double u[3] = {0.0, 0.0, 1.0};
+          if (d > 0.0) { u[0] = dv[0] / d; u[1] = dv[1] / d; u[2] = dv[2] / d; }
+          dd = d > S->r0 ? d : S->r0;
+          orc_radial2(S, S->shell_spline[s], d, &R, &dR, &d2R);
+          orc_solid_harmonics(l, u, Y, NULL);
+        }
+        for (int m = 0; m < 2 * l + 1; m++, i++) {
+          phi[i] = inside ? R * Y[m] : 0.0;
+          Lp[i] = inside ? -0.5 * (d2R + 2.0 * dR / dd - (double)(l * (l + 1)) * R / (dd * dd)) * Y[m] + v[p] * phi[i] : 0.0;
+        }
+      }
+    }
+    double wp = S->w[p];
+    for (int a = 0; a < nb; a++)
+      for (int c = 0; c < nb; c++) Hd[(size_t)a * nb + c] += 0.5 * wp * (phi[a] * Lp[c] + Lp[a] * phi[c]);
+  }
+  free(phi);
+  free(afp);
+}

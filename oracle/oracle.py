@@ -61,6 +61,8 @@ def _load():
         L.orc_shell_hess_at_point.argtypes = [sp, ctypes.c_int, ctypes.c_int, _dp, _dp, _dp, _dp]
         L.orc_pulay_forces.argtypes = [sp, ctypes.c_int, _ip, _dp, _dp, _dp, _dp, _dp]
         L.orc_brute_forces.argtypes = [sp, _dp, _dp, _dp, _dp, _dp]
+        L.orc_integrate_hamiltonian_ks.argtypes = [sp, ctypes.c_int, _ip, _dp, _dp, ctypes.c_int, _dp]
+        L.orc_brute_kinetic.argtypes = [sp, _dp, _dp]
         _lib = L
     return _lib
 
@@ -179,6 +181,21 @@ class Oracle:
         H = np.zeros(self.n_values) if H_values is None else H_values
         self.L.orc_integrate_hamiltonian(ctypes.byref(self.sys), len(sel), _i(sel), _d(v), _d(g), _d(H))
         return H
+
+    def integrate_hamiltonian_ks(self, v, g=None, kinetic=True, batches=None):
+        """H with (h phi) = -1/2 lap phi + v phi symmetrised as in Fig. 6a (DSYR2K, alpha = 1/2) plus the GGA term."""
+        sel = self._sel(batches)
+        v = np.ascontiguousarray(v, dtype=np.float64)
+        g = None if g is None else np.ascontiguousarray(g, dtype=np.float64)
+        H = np.zeros(self.n_values)
+        self.L.orc_integrate_hamiltonian_ks(ctypes.byref(self.sys), len(sel), _i(sel), _d(v), _d(g), int(bool(kinetic)), _d(H))
+        return H
+
+    def brute_kinetic(self, v):
+        nb = self.n_basis
+        Hd = np.zeros((nb, nb))
+        self.L.orc_brute_kinetic(ctypes.byref(self.sys), _d(np.ascontiguousarray(v, dtype=np.float64)), _d(Hd))
+        return Hd
 
     # ---- O4
     def update_density(self, D_values, want_grad=False, batches=None):
