@@ -58,6 +58,8 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--path", default="scf", choices=["scf", "forces"])
+    ap.add_argument("--kinetic", action="store_true",
+                    help="scf path with the full h_KS phi (kinetic term, row f2): a separate line, not the headline metric")
     return ap.parse_args()
 
 
@@ -125,7 +127,7 @@ def sample_batches(n_batches, k, seed=20191206):
     return np.sort(rng.choice(n_batches, size=min(k, n_batches), replace=False)).astype(np.int32)
 
 
-def time_oracle(bun, batches, gga, repeats=1, forces_q=None):
+def time_oracle(bun, batches, gga, repeats=1, forces_q=None, kinetic=False):
     """Oracle as it stands on the host cores: H integration + density update (or, with forces_q, the Pulay forces) on
     the listed batches."""
     from oracle import oracle as orc
@@ -137,7 +139,10 @@ def time_oracle(bun, batches, gga, repeats=1, forces_q=None):
         if forces_q is not None:
             o.pulay_forces(bun.v, bun.D_values, g=bun.g if gga else None, Q_values=forces_q, batches=batches)
         else:
-            o.integrate_hamiltonian(bun.v, bun.g if gga else None, batches=batches)
+            if kinetic:
+                o.integrate_hamiltonian_ks(bun.v, bun.g if gga else None, kinetic=True, batches=batches)
+            else:
+                o.integrate_hamiltonian(bun.v, bun.g if gga else None, batches=batches)
             o.update_density(bun.D_values, want_grad=gga, batches=batches)
         dt = time.perf_counter() - t0
         best = dt if best is None else min(best, dt)
@@ -150,7 +155,7 @@ def run_reference(args, bun, gga, workload, metric, forces_q=None):
     times, pts_step = [], 0
     for s in range(args.warmup + args.steps):
         sel = sample_batches(bun.n_batches, per_step, seed=1000 + s)
-        pts, dt, cores = time_oracle(bun, sel, gga, forces_q=forces_q)
+        pts, dt, cores = time_oracle(bun, sel, gga, forces_q=forces_q, kinetic=args.kinetic and forces_q is None)
         if s >= args.warmup:
             times.append(dt)
             pts_step += pts
@@ -181,6 +186,9 @@ def main():
 
     forces = args.path == "forces"
     metric = METRIC if not forces else "grid points/s for the Pulay-force pass (FP64); % of FP64 peak"
+    if args.kinetic and not forces:
+        metric = "grid points/s for H integration with the kinetic term + density update (FP64); % of FP64 peak"
+    kin = bool(args.kinetic)
 
     import aims_synth
     if args.impl == "reference":
@@ -212,7 +220,8 @@ def main():
     cost = npb * nnz * nnz
     b0, b1 = partition_batches(cost, world)[rank]
     my_points = int(bun.batch_ptr[b1] - bun.batch_ptr[b0])
-    flops_h = float(((2.0 if gga else 1.0) * npb * nnz * (nnz + (0.0 if gga else 1.0)))[b0:b1].sum())
+    syr2k = gga or bool(args.kinetic)            # Q not proportional to P: one full product, symmetrised
+    flops_h = float(((2.0 if syr2k else 1.0) * npb * nnz * (nnz + (0.0 if syr2k else 1.0)))[b0:b1].sum())
     flops_n = float((2.0 * npb * nnz * nnz)[b0:b1].sum())
     # Pulay forces: the DSYMM-shaped products q_b Phi, n_b L and (GGA) n_b Phi, 2 n_p nnz^2 each
     flops_f = (3.0 if gga else 2.0) * flops_n
@@ -236,7 +245,7 @@ def main():
                 if world > 1:
                     dist.all_reduce(F)
                 return
-            ctx.integrate_hamiltonian(v, g, H=H, b0=b0, b1=b1, accumulate=False)
+            ctx.integrate_hamiltonian(v, g, H=H, b0=b0, b1=b1, accumulate=False, kinetic=kin)
             if world > 1:
                 dist.all_reduce(H)                        # Eq. 29: the only communication step
             ctx.update_density(D, want_grad=gga, n=n, grad_n=gn, b0=b0, b1=b1)
@@ -310,7 +319,8 @@ def main():
                         dist.all_reduce(dv["F"])
                     hb["F"].copy_(dv["F"], non_blocking=True)
                     return
-                ctx.integrate_hamiltonian(dv["v"], dv["g"] if gga else None, H=dv["H"], b0=b0, b1=b1, accumulate=False)
+                ctx.integrate_hamiltonian(dv["v"], dv["g"] if gga else None, H=dv["H"], b0=b0, b1=b1, accumulate=False,
+                                          kinetic=kin)
                 if world > 1:
                     dist.all_reduce(dv["H"])
                 ctx.update_density(dv["D"], want_grad=gga, n=dv["n"], grad_n=dv.get("grad_n"), b0=b0, b1=b1)
@@ -381,7 +391,7 @@ def main():
     # ---- CPU baseline: the oracle on a bounded seeded sample, rank 0 at N=1 only
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         sel = sample_batches(bun.n_batches, args.cpu_sample_batches)
-        pts, dt, cores = time_oracle(bun, sel, gga, forces_q=Qh)
+        pts, dt, cores = time_oracle(bun, sel, gga, forces_q=Qh, kinetic=kin and not forces)
         out["cpu_baseline"] = {"value": pts / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
                                "sample": "%d seeded batches (%d points) of the same workload, %.1f s" % (len(sel), pts, dt)}
     else:

@@ -117,6 +117,15 @@ int aims_gpu_eval_basis(aims_gpu_ctx *ctx, int32_t b0, int32_t b1, int64_t *fn_p
 int aims_gpu_integrate_hamiltonian(aims_gpu_ctx *ctx, int32_t b0, int32_t b1, const double *v, const double *g,
                                    double *H_values, int accumulate);
 
+/* Row f2 of SURVEY.md 8(f): the full h_KS phi of Eq. 26 with the kinetic operator, "h_times_phi" of
+ * Fig. 6a (L323).  kinetic != 0:  (h phi_j)(r) = -1/2 lap phi_j(r) + v(r) phi_j(r); the batch product K.L of Eq. 27 is then
+ * not symmetric on the grid and is symmetrised as Fig. 6a does with DSYR2K (alpha = 1/2, reading P1b):
+ *   H_values (+)= sum_p w_p { 1/2 [phi_i (h phi_j) + (h phi_i) phi_j] + [g != NULL] g_p . grad(phi_i phi_j) }(r_p).
+ * lap (R(d) Y_lm) = (R'' + 2 R'/d - l(l+1) R/d^2) Y_lm with R'' from the same spline table.  kinetic == 0: identical to
+ * aims_gpu_integrate_hamiltonian.  Arguments as there. */
+int aims_gpu_integrate_hamiltonian_ks(aims_gpu_ctx *ctx, int32_t b0, int32_t b1, const double *v, const double *g,
+                                      int kinetic, double *H_values, int accumulate);
+
 /* Step 3 (S3a-S3d).  For every point p of batches [b0,b1):  n[p] = sum_ij phi_i D_ij phi_j,
  * grad_n[c][p] = 2 sum_ij d_c phi_i D_ij phi_j (D symmetric), i,j in nnz(B) (Eq. 3; Fig. 6b).
  * DEVICE pointers: D_values [n_values] in the pattern of aims_bsr_desc (upper blocks; the symmetric full matrix is

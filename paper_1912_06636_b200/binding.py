@@ -77,6 +77,8 @@ def load_library():
     L.aims_gpu_eval_basis.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp, _vp, _vp, _vp]
     L.aims_gpu_integrate_hamiltonian.restype = ctypes.c_int
     L.aims_gpu_integrate_hamiltonian.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp, _vp, ctypes.c_int]
+    L.aims_gpu_integrate_hamiltonian_ks.restype = ctypes.c_int
+    L.aims_gpu_integrate_hamiltonian_ks.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp, ctypes.c_int, _vp, ctypes.c_int]
     L.aims_gpu_update_density.restype = ctypes.c_int
     L.aims_gpu_update_density.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp, _vp]
     L.aims_gpu_pulay_forces.restype = ctypes.c_int
@@ -231,7 +233,7 @@ class Context:
                                                _ptr(dphi)), "aims_gpu_eval_basis")
         return fn_ptr, fn_index[:ni], phi_ptr, phi[:nph], (dphi[:3 * nph] if want_grad else None)
 
-    def integrate_hamiltonian(self, v, g=None, H=None, b0=0, b1=None, accumulate=False):
+    def integrate_hamiltonian(self, v, g=None, H=None, b0=0, b1=None, accumulate=False, kinetic=False):
         torch = self.torch
         b0, b1 = self._range(b0, b1)
         v = self._dev(v, torch.float64)
@@ -242,6 +244,10 @@ class Context:
             with torch.cuda.stream(self.stream):
                 H = torch.empty(self.n_values, dtype=torch.float64, device=self.device)
             accumulate = False
+        if kinetic:
+            self._check(self.L.aims_gpu_integrate_hamiltonian_ks(self.h, b0, b1, _ptr(v), _ptr(g), 1, _ptr(H),
+                                                                 int(bool(accumulate))), "aims_gpu_integrate_hamiltonian_ks")
+            return H
         self._check(self.L.aims_gpu_integrate_hamiltonian(self.h, b0, b1, _ptr(v), _ptr(g), _ptr(H), int(bool(accumulate))),
                     "aims_gpu_integrate_hamiltonian")
         return H
@@ -324,6 +330,10 @@ def aims_gpu_eval_basis(ctx, b0=0, b1=None, want_grad=False):
 
 def aims_gpu_integrate_hamiltonian(ctx, v, g=None, H=None, b0=0, b1=None, accumulate=False):
     return ctx.integrate_hamiltonian(v, g, H, b0, b1, accumulate)
+
+
+def aims_gpu_integrate_hamiltonian_ks(ctx, v, g=None, kinetic=True, H=None, b0=0, b1=None, accumulate=False):
+    return ctx.integrate_hamiltonian(v, g, H, b0, b1, accumulate, kinetic=kinetic)
 
 
 def aims_gpu_update_density(ctx, D, want_grad=False, n=None, grad_n=None, b0=0, b1=None):

@@ -371,6 +371,7 @@ int aims_gpu_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_gri
     if ((size_t)esm + 4096 > (size_t)prop.sharedMemPerBlockOptin) return fail(c, AIMS_ERR_UNSUPPORTED, "nnz(B) too large for the evaluation kernel's shared memory");
 #define EV_ATTR(M, LY) CU_TRY(c, cudaFuncSetAttribute(k_eval<M, LY>, cudaFuncAttributeMaxDynamicSharedMemorySize, esm));
     EV_ATTR(kEvalPhi, kLayApi) EV_ATTR(kEvalPhiGrad, kLayApi) EV_ATTR(kEvalHLda, kLayH) EV_ATTR(kEvalHGga, kLayH)
+    EV_ATTR(kEvalHKinLda, kLayH) EV_ATTR(kEvalHKinGga, kLayH)
     EV_ATTR(kEvalPhi, kLayD) EV_ATTR(kEvalPhiGrad, kLayD) EV_ATTR(kEvalForceLda, kLayD) EV_ATTR(kEvalForceGga, kLayD)
 #undef EV_ATTR
   }
@@ -479,14 +480,15 @@ int aims_gpu_eval_basis(aims_gpu_ctx *c, int32_t b0, int32_t b1, int64_t *fn_ptr
   return check_async(c);
 }
 
-int aims_gpu_integrate_hamiltonian(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, const double *g,
-                                   double *H_values, int accumulate) {
+static int run_hamiltonian(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, const double *g, int kinetic,
+                           double *H_values, int accumulate) {
   if (!range_ok(c, b0, b1)) return fail(c, AIMS_ERR_INVALID_ARG, "batch range outside [0, n_batches]");
   if (!v || !H_values) return fail(c, AIMS_ERR_INVALID_ARG, "NULL v or H_values");
   CU_TRY(c, cudaSetDevice(c->device));
   if (!accumulate) CU_TRY(c, cudaMemsetAsync(H_values, 0, (size_t)c->n_values * sizeof(double), c->stream));
   int rc = run_cull(c, b0, b1);
   if (rc) return rc;
+  const bool syr2k = g || kinetic;     // Q is not proportional to P: P Q^T + Q P^T
   for (int bs = b0; bs < b1;) {
     const int be = chunk_end(c, c->pad_off, bs, b1, 2);
     const long long plane = (c->ws_doubles / 2) & ~63ll;
@@ -494,18 +496,30 @@ int aims_gpu_integrate_hamiltonian(aims_gpu_ctx *c, int32_t b0, int32_t b1, cons
     E.plane[0] = c->ws; E.plane[1] = c->ws + plane;
     E.pad_off = c->d_pad_off; E.pad_base = c->pad_off[bs];
     E.v = v; E.g = g; E.n_points = c->n_points;
-    if (g) launch_eval<kEvalHGga, kLayH>(c, E, bs, be); else launch_eval<kEvalHLda, kLayH>(c, E, bs, be);
+    if (kinetic) { if (g) launch_eval<kEvalHKinGga, kLayH>(c, E, bs, be); else launch_eval<kEvalHKinLda, kLayH>(c, E, bs, be); }
+    else if (g) launch_eval<kEvalHGga, kLayH>(c, E, bs, be);
+    else launch_eval<kEvalHLda, kLayH>(c, E, bs, be);
     const long long nt = c->tile_off[be] - c->tile_off[bs];
     if (nt > 0) {
       HArgs A{c->d_tiles + c->tile_off[bs], E.plane[0], E.plane[1], c->d_pad_off, c->pad_off[bs], H_values};
       TimedLaunch t(c, kKindHam);
-      if (g) k_hamiltonian<true><<<(unsigned)nt, kHThreads, h_smem_bytes<true>(), c->stream>>>(c->S, c->L, A);
+      if (syr2k) k_hamiltonian<true><<<(unsigned)nt, kHThreads, h_smem_bytes<true>(), c->stream>>>(c->S, c->L, A);
       else k_hamiltonian<false><<<(unsigned)nt, kHThreads, h_smem_bytes<false>(), c->stream>>>(c->S, c->L, A);
     }
     if ((rc = check_async(c))) return rc;
     bs = be;
   }
   return AIMS_OK;
+}
+
+int aims_gpu_integrate_hamiltonian(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, const double *g,
+                                   double *H_values, int accumulate) {
+  return run_hamiltonian(c, b0, b1, v, g, 0, H_values, accumulate);
+}
+
+int aims_gpu_integrate_hamiltonian_ks(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, const double *g, int kinetic,
+                                      double *H_values, int accumulate) {
+  return run_hamiltonian(c, b0, b1, v, g, kinetic, H_values, accumulate);
 }
 
 int aims_gpu_update_density(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *D_values, double *n, double *grad_n) {

@@ -236,7 +236,12 @@ enum EvalMode {
   // Pulay forces (forces.cuh; Eq. 16, 18 L137-150): plane0 = Phi, plane1 = L = v Phi (+ g . grad Phi),
   // planes 2..4 = w d/dx_c Phi, and with the GGA term planes 5..7 = w (Hess Phi g)_c
   kEvalForceLda = 4,
-  kEvalForceGga = 5
+  kEvalForceGga = 5,
+  // full h_KS phi with the kinetic operator (Eq. 26, Fig. 6a "h_times_phi"):
+  // plane0 = Phi, plane1 = w ((v Phi - 1/2 lap Phi) / 2 [+ g . grad Phi]) -- the SYR2K form P Q^T + Q P^T then gives
+  // 1/2 [phi_i (h phi_j) + (h phi_i) phi_j], Fig. 6a's DSYR2K with alpha = 1/2
+  kEvalHKinLda = 6,
+  kEvalHKinGga = 7
 };
 __host__ __device__ constexpr int eval_planes(int mode) {
   return mode == kEvalPhi ? 1 : mode == kEvalPhiGrad ? 4 : mode == kEvalForceLda ? 5 : mode == kEvalForceGga ? 8 : 2;
@@ -321,7 +326,8 @@ __global__ void __launch_bounds__(256, (MODE >= kEvalForceLda) ? 1 : AIMS_EVAL_C
 k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
   constexpr bool FORCE = (MODE == kEvalForceLda || MODE == kEvalForceGga);
   constexpr bool HESS = (MODE == kEvalForceGga);
-  constexpr bool GRAD = (MODE == kEvalPhiGrad || MODE == kEvalHGga || FORCE);
+  constexpr bool KIN = (MODE == kEvalHKinLda || MODE == kEvalHKinGga);
+  constexpr bool GRAD = (MODE == kEvalPhiGrad || MODE == kEvalHGga || MODE == kEvalHKinGga || FORCE);
   constexpr int NPL = eval_planes(MODE);
   const int b = b_first + blockIdx.x;
   const int tid = threadIdx.x;
@@ -404,7 +410,8 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
     const double x = S.px[p0 + p], y = S.py[p0 + p], z = S.pz[p0 + p];
     double wv = 0.0, wgx = 0.0, wgy = 0.0, wgz = 0.0, w = 0.0;
     if (MODE == kEvalHLda) wv = S.w[p0 + p] * E.v[p0 + p];
-    if (MODE == kEvalHGga) {
+    if (MODE == kEvalHKinLda) { w = S.w[p0 + p]; wv = 0.5 * w * E.v[p0 + p]; }
+    if (MODE == kEvalHGga || MODE == kEvalHKinGga) {
       w = S.w[p0 + p];
       wv = 0.5 * w * E.v[p0 + p];
       wgx = w * E.g[p0 + p]; wgy = w * E.g[E.n_points + p0 + p]; wgz = w * E.g[2 * E.n_points + p0 + p];
@@ -452,13 +459,19 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
         const double2 *cf = reinterpret_cast<const double2 *>(S.spline_coef + (long long)(en.y + k) * 4);
         const double2 c01 = __ldg(cf), c23 = __ldg(cf + 1);
         const double R = c01.x + xs * (c01.y + xs * (c23.x + xs * c23.y));
-        double f = 0.0, Rd = 0.0, hA = 0.0, hB = 0.0, hC = 0.0;
-        if (GRAD) {
+        double f = 0.0, Rd = 0.0, hA = 0.0, hB = 0.0, hC = 0.0, qlap = 0.0;
+        if (GRAD || KIN) {
           const double Rt = c01.y + xs * (2.0 * c23.x + xs * 3.0 * c23.y);
           const double sc = S.log_inc * dd;
           const double dR = Rt / sc;
           Rd = R * inv_dd;
           f = dR - (double)l * Rd;
+          if (KIN) {
+            // lap (R(d) Y_lm) = (R'' + 2 R'/d - l(l+1) R/d^2) Y_lm;  qlap = -w/4 times the radial factor
+            const double Rtt = 2.0 * c23.x + 6.0 * c23.y * xs;
+            const double d2R = Rtt / (sc * sc) - Rt / (sc * dd);
+            qlap = -0.25 * w * (d2R + 2.0 * dR * inv_dd - (double)(l * (l + 1)) * Rd * inv_dd);
+          }
           if (HESS) {
             // Hess phi = A u u^T Y + B (1 - u u^T) Y + B (u gS^T + gS u^T) + C Hess S, phi = (R / d^l) S_lm(dvec)
             const double Rtt = 2.0 * c23.x + 6.0 * c23.y * xs;
@@ -475,11 +488,13 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
             const int oi = ro + m * mstep + (m >= wrap ? jump : 0);
             op[0][oi] = phi;
             if (MODE == kEvalHLda) op[1 % NPL][oi] = wv * phi;
+            if (MODE == kEvalHKinLda) op[1 % NPL][oi] = wv * phi + qlap * Y[m];
             if (GRAD) {
               const double fy = f * Y[m];
               const double ex = fy * ux + Rd * gx[m], ey = fy * uy + Rd * gy[m], ez = fy * uz + Rd * gz[m];
               if (MODE == kEvalPhiGrad) { op[1 % NPL][oi] = ex; op[2 % NPL][oi] = ey; op[3 % NPL][oi] = ez; }
               if (MODE == kEvalHGga) op[1 % NPL][oi] = wv * phi + (wgx * ex + wgy * ey + wgz * ez);
+              if (MODE == kEvalHKinGga) op[1 % NPL][oi] = wv * phi + (wgx * ex + wgy * ey + wgz * ez) + qlap * Y[m];
               if (FORCE) {
                 op[1 % NPL][oi] = HESS ? wv * phi + (wgx * ex + wgy * ey + wgz * ez) : wv * phi;
                 op[2 % NPL][oi] = w * ex; op[3 % NPL][oi] = w * ey; op[4 % NPL][oi] = w * ez;

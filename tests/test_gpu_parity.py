@@ -114,6 +114,22 @@ def test_hamiltonian_matches_oracle(case, mode):
     assert np.all(H[bsr_pad_mask(bun)] == 0.0)                      # padding columns are never written
 
 
+@pytest.mark.parametrize("mode", ["kin_lda", "kin_gga", "kin_only", "off"])
+def test_hamiltonian_with_kinetic_term_matches_oracle(case, mode):
+    """Row f2: (h phi) = -1/2 lap phi + v phi, symmetrised as Fig. 6a's DSYR2K (aims_gpu_integrate_hamiltonian_ks)."""
+    name, bun, orc, ctx = case
+    v = np.zeros(bun.n_points) if mode == "kin_only" else bun.v
+    g = bun.g if mode == "kin_gga" else None
+    kin = mode != "off"
+    H = ctx.integrate_hamiltonian(v, g, kinetic=kin).cpu().numpy()
+    ctx.synchronize()
+    ref = orc.integrate_hamiltonian_ks(v, g, kinetic=kin)
+    assert _rel_fro(H, ref) <= TOL_H
+    assert np.all(H[bsr_pad_mask(bun)] == 0.0)
+    if mode == "off":
+        assert np.array_equal(H, ctx.integrate_hamiltonian(v, g).cpu().numpy()) or _rel_fro(H, ctx.integrate_hamiltonian(v, g).cpu().numpy()) <= 1e-13
+
+
 def test_hamiltonian_accumulate_and_subranges(case):
     name, bun, orc, ctx = case
     import torch
