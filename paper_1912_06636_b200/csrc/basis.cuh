@@ -322,7 +322,7 @@ __device__ __forceinline__ int eval_row_off(int row, int np, int np8) {
 }
 
 template <int MODE, int LAYOUT>
-__global__ void __launch_bounds__(256, (MODE >= kEvalForceLda) ? 1 : AIMS_EVAL_CTAS_PER_SM)
+__global__ void __launch_bounds__(256, (MODE == kEvalForceLda || MODE == kEvalForceGga) ? 1 : AIMS_EVAL_CTAS_PER_SM)
 k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
   constexpr bool FORCE = (MODE == kEvalForceLda || MODE == kEvalForceGga);
   constexpr bool HESS = (MODE == kEvalForceGga);
