@@ -112,7 +112,7 @@ int aims_gpu_eval_basis(aims_gpu_ctx *ctx, int32_t b0, int32_t b1, int64_t *fn_p
  *     sum_p w_p phi_i(r_p) v_p phi_j(r_p)  +  [g != NULL]  sum_p w_p g_p . (grad phi_i phi_j + phi_i grad phi_j)(r_p)
  * for i,j in nnz(B), scattered into the block pattern (Eq. 23-27; GGA term in the integrated-by-parts form, L67 and
  * Eq. 18, reading P2).  Overlap matrix: pass v = 1.  DEVICE pointers:
- *   v [n_points], g NULL or [3][n_points] (component-major), H_values [n_values].
+ *   v [n_points] (may be NULL only if n_points == 0), g NULL or [3][n_points] (component-major), H_values [n_values].
  * accumulate == 0: H_values is zeroed first; != 0: added to (Eq. 28-29 partial sums). */
 int aims_gpu_integrate_hamiltonian(aims_gpu_ctx *ctx, int32_t b0, int32_t b1, const double *v, const double *g,
                                    double *H_values, int accumulate);

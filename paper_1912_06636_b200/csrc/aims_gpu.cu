@@ -483,7 +483,7 @@ int aims_gpu_eval_basis(aims_gpu_ctx *c, int32_t b0, int32_t b1, int64_t *fn_ptr
 static int run_hamiltonian(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, const double *g, int kinetic,
                            double *H_values, int accumulate) {
   if (!range_ok(c, b0, b1)) return fail(c, AIMS_ERR_INVALID_ARG, "batch range outside [0, n_batches]");
-  if (!v || !H_values) return fail(c, AIMS_ERR_INVALID_ARG, "NULL v or H_values");
+  if ((!v && c->n_points) || !H_values) return fail(c, AIMS_ERR_INVALID_ARG, "NULL v or H_values");
   CU_TRY(c, cudaSetDevice(c->device));
   if (!accumulate) CU_TRY(c, cudaMemsetAsync(H_values, 0, (size_t)c->n_values * sizeof(double), c->stream));
   int rc = run_cull(c, b0, b1);
@@ -524,7 +524,7 @@ int aims_gpu_integrate_hamiltonian_ks(aims_gpu_ctx *c, int32_t b0, int32_t b1, c
 
 int aims_gpu_update_density(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *D_values, double *n, double *grad_n) {
   if (!range_ok(c, b0, b1)) return fail(c, AIMS_ERR_INVALID_ARG, "batch range outside [0, n_batches]");
-  if (!D_values || !n) return fail(c, AIMS_ERR_INVALID_ARG, "NULL D_values or n");
+  if (!D_values || (!n && c->n_points)) return fail(c, AIMS_ERR_INVALID_ARG, "NULL D_values or n");
   CU_TRY(c, cudaSetDevice(c->device));
   int rc = run_cull(c, b0, b1);
   if (rc) return rc;
@@ -562,7 +562,7 @@ int aims_gpu_update_density(aims_gpu_ctx *c, int32_t b0, int32_t b1, const doubl
 int aims_gpu_pulay_forces(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, const double *g, const double *D_values,
                           const double *Q_values, double *F, int accumulate) {
   if (!range_ok(c, b0, b1)) return fail(c, AIMS_ERR_INVALID_ARG, "batch range outside [0, n_batches]");
-  if (!v || !D_values || !F) return fail(c, AIMS_ERR_INVALID_ARG, "NULL v, D_values or F");
+  if ((!v && c->n_points) || !D_values || !F) return fail(c, AIMS_ERR_INVALID_ARG, "NULL v, D_values or F");
   CU_TRY(c, cudaSetDevice(c->device));
   if (!accumulate) CU_TRY(c, cudaMemsetAsync(F, 0, (size_t)c->S.n_atoms * 3 * sizeof(double), c->stream));
   int rc = run_cull(c, b0, b1);
