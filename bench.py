@@ -375,6 +375,30 @@ def main():
                 "avg_launch_ms": dom_ms / max(dom_ln, 1), "algorithmic_flops_per_step": kflops[dom],
                 "share_of_step": dom_ms / ms_total}
     total_tflops = (flops_f if forces else flops_h + flops_n) / (ms_step * 1e-3) / 1e12
+    # DRAM traffic per launch of the dominant kernel from the committed `ncu --set full` capture (config 5 only)
+    if args.config == 5 and not (args.max_batch or args.n_rad or args.n_ang) and world == 1:
+        roofline["traffic"] = {"k_density": 125.75e9, "k_hamiltonian": 28.46e9, "k_forces": 152.29e9}[dom]
+        roofline["traffic_note"] = ("dram__bytes_read.sum + dram__bytes_write.sum of one launch (bytes), "
+                                    "profiles/r01_ncu_full_config5.md; Phi-plane bytes consumed per launch: 25.8e9")
+    # second roofline: the HBM-bound evaluation kernel (algorithmic bytes = 8 B x planes x padded rows x padded points)
+    pad = lambda a, m: np.ceil(a / m) * m                                   # noqa: E731
+    pl_h, pl_d = 2.0, (4.0 if gga else 1.0)
+    if forces:
+        eval_bytes = 8.0 * float(((8.0 if gga else 5.0) * pad(nnz, 16) * pad(npb, 8))[b0:b1].sum())
+    else:
+        eval_bytes = 8.0 * float((pl_h * pad(nnz, 8) * pad(npb, 8) + pl_d * pad(nnz, 16) * pad(npb, 8))[b0:b1].sum())
+    hbm_peak, hbm_src = 6561.9, "fallback: this pool's measured copy bandwidth recorded in DESIGN.md"
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            hbm_peak, hbm_src = float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (burst copy bandwidth)"
+    except Exception:
+        pass
+    ev_ms, ev_ln = kern["k_eval"]
+    ev_gbs = eval_bytes * args.steps / (ev_ms * 1e-3) / 1e9 if ev_ms > 0 else 0.0
+    roofline_eval = {"bound": "hbm", "kernel": "k_eval", "achieved": ev_gbs, "peak": hbm_peak, "unit": "GB/s",
+                     "frac": ev_gbs / hbm_peak, "peak_source": hbm_src, "algorithmic_bytes_per_step": eval_bytes,
+                     "avg_launch_ms": ev_ms / max(ev_ln, 1), "share_of_step": ev_ms / ms_total,
+                     "traffic": None}
 
     out = {"metric": metric, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
@@ -383,9 +407,9 @@ def main():
                       "mean_nnz": float(nnz.mean()) if len(nnz) else 0.0, "max_nnz": st["max_nnz"],
                       "max_active_atoms": st["max_active_atoms"], "parallelism": "batch-range x%d" % world,
                       "l2": "inputs larger than L2: each step streams %.1f GB of Phi planes plus a %.2f GB H and D"
-                            % (8e-9 * ((8 if gga else 5) if forces else 6) * st["sum_nnz"] * 208, 8e-9 * bun.n_values)},
+                            % (1e-9 * eval_bytes, 8e-9 * bun.n_values)},
            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
-           "fp64_tflops_step": total_tflops, "fp64_frac_of_peak_step": total_tflops / FP64_PEAK_NOMINAL_TFLOPS,
+           "roofline_eval": roofline_eval, "fp64_tflops_step": total_tflops, "fp64_frac_of_peak_step": total_tflops / FP64_PEAK_NOMINAL_TFLOPS,
            "kernels": kd, "setup_s": {"generate_inputs": t_gen, "create_ctx": t_create}}
 
     # ---- CPU baseline: the oracle on a bounded seeded sample, rank 0 at N=1 only
