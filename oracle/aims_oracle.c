@@ -429,6 +429,9 @@ void orc_brute(const orc_system *S, const double *v, const double *g, double *Hd
  * i.e. F_at = -d/dR_at [ Tr(n h(R)) - Tr(q s(R)) ] at fixed n_ij, q_ij, v, g, w and grid -- the pin used in
  * tests/test_oracle_pins.py (central differences of the already pinned H and S).  The atomic-ZORA term (Eq. 19) and
  * the Hellmann-Feynman force (L403, not on this path in the paper either) are outside the reduced h_KS.
+ * kinetic != 0: h_KS phi_j in the first term of Eq. 16 also carries -1/2 lap phi_j (row f2), i.e. v_p phi_j -> v_p phi_j - 1/2 lap phi_j.
+ * Eq. 16 uses the Hermiticity of h_KS, which holds on the grid only to quadrature accuracy for the kinetic operator, so that
+ * part equals -d/dR_at Tr(n t(R)) to grid accuracy only (pinned so), while batched == brute force stays exact.
  * ==================================================================================================================== */
 
 /* second derivatives of the solid harmonics S_lm at (x,y,z): hS[m+l][6] = (xx, yy, zz, xy, xz, yz) */
@@ -543,7 +546,7 @@ static void restrict_matrix(const orc_system *S, const int64_t *afp, int nnz, co
  * Q_values == NULL: no energy-weighted term.  Per batch: temp matrices  Tn = n_ij phi,  Tg = n_ij (g.grad phi),
  * Tq = q_ij phi  (the DSYMM-shaped products of Fig. 6b), then the point sums of the header formula. */
 void orc_pulay_forces(const orc_system *S, int n_sel, const int32_t *batches, const double *v, const double *g,
-                      const double *D_values, const double *Q_values, double *F) {
+                      const double *D_values, const double *Q_values, int kinetic, double *F) {
   int64_t *afp = (int64_t *)malloc(sizeof(int64_t) * (S->n_atoms + 1));
   orc_atom_fn_ptr(S, afp);
   int nf_tot = (int)afp[S->n_atoms];
@@ -582,10 +585,14 @@ void orc_pulay_forces(const orc_system *S, int n_sel, const int32_t *batches, co
       for (int p = 0; p < np; p++) {
         double gp[3] = {0.0, 0.0, 0.0};
         if (g) for (int c = 0; c < 3; c++) gp[c] = g[(size_t)c * S->n_points + p0 + p];
-        double tn = 0.0, tg = 0.0, tq = 0.0;
+        double tn = 0.0, tg = 0.0, tq = 0.0, tk = 0.0;
         for (int j = 0; j < nnz; j++) {
           double dij = Db[(size_t)i * nnz + j];
           tn += dij * phi[(size_t)j * np + p];
+          if (kinetic) {                               /* h_KS phi_j of Eq. 16 with the kinetic operator: -1/2 lap phi_j */
+            double lap = (hes[((size_t)0 * nnz + j) * np + p] + hes[((size_t)1 * nnz + j) * np + p]) + hes[((size_t)2 * nnz + j) * np + p];
+            tk += dij * (-0.5 * lap);
+          }
           if (g) {
             double Gj = 0.0;
             for (int c = 0; c < 3; c++) Gj += gp[c] * dphi[((size_t)c * nnz + j) * np + p];
@@ -594,7 +601,7 @@ void orc_pulay_forces(const orc_system *S, int n_sel, const int32_t *batches, co
           if (Qb) tq += Qb[(size_t)i * nnz + j] * phi[(size_t)j * np + p];
         }
         double wp = S->w[p0 + p];
-        double x = v[p0 + p] * tn + tg - tq;
+        double x = v[p0 + p] * tn + tg - tq + tk;
         static const int hx[3][3] = {{0, 3, 4}, {3, 1, 5}, {4, 5, 2}};   /* index of (c,e) in (xx,yy,zz,xy,xz,yz) */
         for (int c = 0; c < 3; c++) {
           double t = dphi[((size_t)c * nnz + i) * np + p] * x;
@@ -623,7 +630,8 @@ void orc_pulay_forces(const orc_system *S, int n_sel, const int32_t *batches, co
  * written from Eq. 16 and Eq. 18 term by term with nabla_at phi_i = -grad phi_i:
  *   F_at = -2 sum_ij int [nabla_at phi_i] n_ij v phi_j + 2 sum_ij int [nabla_at phi_i] q_ij phi_j
  *          -2 sum_ij int [nabla_at phi_i] n_ij (g.grad phi_j) - 2 sum_ij int phi_i n_ij (g.nabla_at grad phi_j). */
-void orc_brute_forces(const orc_system *S, const double *v, const double *g, const double *Dd, const double *Qd, double *F) {
+void orc_brute_forces(const orc_system *S, const double *v, const double *g, const double *Dd, const double *Qd, int kinetic,
+                      double *F) {
   int64_t *afp = (int64_t *)malloc(sizeof(int64_t) * (S->n_atoms + 1));
   orc_atom_fn_ptr(S, afp);
   int nb = (int)afp[S->n_atoms];
@@ -655,6 +663,7 @@ void orc_brute_forces(const orc_system *S, const double *v, const double *g, con
         for (int c = 0; c < 3; c++) {
           double nat_phi_a = -dph[c * nb + a];                       /* [nabla_at phi_a]_c for at = atom of a */
           F[at_of[a] * 3 + c] += wp * (-2.0 * nat_phi_a * nab * v[p] * phi[b] + 2.0 * nat_phi_a * qab * phi[b]);
+          if (kinetic) F[at_of[a] * 3 + c] += wp * (-2.0 * nat_phi_a * nab * (-0.5 * ((hes[0 * nb + b] + hes[1 * nb + b]) + hes[2 * nb + b])));
           if (g) {
             F[at_of[a] * 3 + c] += wp * (-2.0 * nat_phi_a * nab * Gb);
             double nat_gb = 0.0;                                     /* g . nabla_at grad phi_b, component c, at = atom of b */

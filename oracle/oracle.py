@@ -59,8 +59,8 @@ def _load():
         L.orc_solid_harmonics_hess.argtypes = [ctypes.c_int, _dp, _dp]
         L.orc_radial2.argtypes = [sp, ctypes.c_int, ctypes.c_double, _dp, _dp, _dp]
         L.orc_shell_hess_at_point.argtypes = [sp, ctypes.c_int, ctypes.c_int, _dp, _dp, _dp, _dp]
-        L.orc_pulay_forces.argtypes = [sp, ctypes.c_int, _ip, _dp, _dp, _dp, _dp, _dp]
-        L.orc_brute_forces.argtypes = [sp, _dp, _dp, _dp, _dp, _dp]
+        L.orc_pulay_forces.argtypes = [sp, ctypes.c_int, _ip, _dp, _dp, _dp, _dp, ctypes.c_int, _dp]
+        L.orc_brute_forces.argtypes = [sp, _dp, _dp, _dp, _dp, ctypes.c_int, _dp]
         L.orc_integrate_hamiltonian_ks.argtypes = [sp, ctypes.c_int, _ip, _dp, _dp, ctypes.c_int, _dp]
         L.orc_brute_kinetic.argtypes = [sp, _dp, _dp]
         _lib = L
@@ -234,7 +234,7 @@ class Oracle:
         self.L.orc_shell_hess_at_point(ctypes.byref(self.sys), int(atom), int(shell), _d(r), _d(phi), _d(gr), _d(he))
         return phi, gr, he
 
-    def pulay_forces(self, v, D_values, g=None, Q_values=None, batches=None):
+    def pulay_forces(self, v, D_values, g=None, Q_values=None, batches=None, kinetic=False):
         """F[n_atoms][3] summed over the listed batches."""
         sel = self._sel(batches)
         v = np.ascontiguousarray(v, dtype=np.float64)
@@ -242,14 +242,14 @@ class Oracle:
         D = np.ascontiguousarray(D_values, dtype=np.float64)
         Q = None if Q_values is None else np.ascontiguousarray(Q_values, dtype=np.float64)
         F = np.zeros((self.sys.n_atoms, 3))
-        self.L.orc_pulay_forces(ctypes.byref(self.sys), len(sel), _i(sel), _d(v), _d(g), _d(D), _d(Q), _d(F))
+        self.L.orc_pulay_forces(ctypes.byref(self.sys), len(sel), _i(sel), _d(v), _d(g), _d(D), _d(Q), int(bool(kinetic)), _d(F))
         return F
 
-    def brute_forces(self, v, D_dense, g=None, Q_dense=None):
+    def brute_forces(self, v, D_dense, g=None, Q_dense=None, kinetic=False):
         v = np.ascontiguousarray(v, dtype=np.float64)
         g = None if g is None else np.ascontiguousarray(g, dtype=np.float64)
         Dd = np.ascontiguousarray(D_dense, dtype=np.float64)
         Qd = None if Q_dense is None else np.ascontiguousarray(Q_dense, dtype=np.float64)
         F = np.zeros((self.sys.n_atoms, 3))
-        self.L.orc_brute_forces(ctypes.byref(self.sys), _d(v), _d(g), _d(Dd), _d(Qd), _d(F))
+        self.L.orc_brute_forces(ctypes.byref(self.sys), _d(v), _d(g), _d(Dd), _d(Qd), int(bool(kinetic)), _d(F))
         return F

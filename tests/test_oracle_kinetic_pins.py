@@ -83,3 +83,42 @@ def test_kinetic_invariant_under_rebatching():
     Ha = bsr_to_dense(a, Oracle(a).integrate_hamiltonian_ks(a.v, a.g, kinetic=True))
     Hc = bsr_to_dense(c, Oracle(c).integrate_hamiltonian_ks(c.v, c.g, kinetic=True))
     assert np.abs(Ha - Hc).max() <= 1e-12 * np.abs(Ha).max()
+
+
+# --------------------------------------------------------------------------- forces with the kinetic operator (Eq. 16)
+def test_kinetic_forces_batched_equal_brute_force_and_off_switch(toy5, cfg1):
+    for b in (cfg1, toy5[0]):
+        o = Oracle(b)
+        Dd = bsr_to_dense(b, b.D_values)
+        F = o.pulay_forces(b.v, b.D_values, g=b.g, kinetic=True)
+        Fb = o.brute_forces(b.v, Dd, g=b.g, kinetic=True)
+        assert np.abs(F - Fb).max() <= 1e-12 * np.abs(Fb).max()
+        F0 = o.pulay_forces(b.v, b.D_values, g=b.g, kinetic=False)
+        Fk = o.pulay_forces(np.zeros(b.n_points), b.D_values, kinetic=True)
+        assert np.abs(F - (F0 + Fk)).max() <= 1e-12 * np.abs(F).max()       # the kinetic part is additive
+        assert np.abs(Fk).max() > 1e-3
+
+
+def test_kinetic_forces_are_minus_gradient_of_kinetic_energy_to_grid_accuracy():
+    # Eq. 16 relies on the Hermiticity of h_KS; on the grid that holds to quadrature accuracy for -1/2 lap, so the pin is
+    # loose in value but catches a wrong sign or factor
+    import copy
+    b = aims_synth.make_config(1, n_rad=60, n_ang=302)
+    o = Oracle(b)
+    zero = np.zeros(b.n_points)
+    Dd = bsr_to_dense(b, b.D_values)
+    F = o.pulay_forces(zero, b.D_values, kinetic=True)
+
+    def energy(xyz):
+        b2 = copy.copy(b)
+        b2.atom_xyz = np.ascontiguousarray(xyz)
+        return float((Dd * bsr_to_dense(b2, Oracle(b2).integrate_hamiltonian_ks(zero, kinetic=True))).sum())
+
+    h = 2e-4
+    scale = np.abs(F).max()
+    for a, c in ((0, 0), (1, 0), (2, 1)):
+        xp, xm = b.atom_xyz.copy(), b.atom_xyz.copy()
+        xp[a, c] += h
+        xm[a, c] -= h
+        fd = -(energy(xp) - energy(xm)) / (2 * h)
+        assert abs(fd - F[a, c]) <= 2e-2 * scale, (a, c, fd, F[a, c])
