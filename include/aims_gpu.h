@@ -147,6 +147,13 @@ int aims_gpu_update_density(aims_gpu_ctx *ctx, int32_t b0, int32_t b1, const dou
 int aims_gpu_pulay_forces(aims_gpu_ctx *ctx, int32_t b0, int32_t b1, const double *v, const double *g,
                           const double *D_values, const double *Q_values, double *F, int accumulate);
 
+/* aims_gpu_pulay_forces with the h_KS phi_j of Eq. 16 carrying the kinetic operator when kinetic != 0:
+ * v_p phi_j -> v_p phi_j - 1/2 lap phi_j(r_p) in the formula above (rows f1 + f2).  Eq. 16 uses the Hermiticity of h_KS,
+ * which the grid quadrature reproduces only to its own accuracy for -1/2 lap: that part is the gradient of Tr(n t(R)) to
+ * grid accuracy.  kinetic == 0: identical to aims_gpu_pulay_forces. */
+int aims_gpu_pulay_forces_ks(aims_gpu_ctx *ctx, int32_t b0, int32_t b1, const double *v, const double *g, int kinetic,
+                             const double *D_values, const double *Q_values, double *F, int accumulate);
+
 /* Synchronise the context stream and report anything the device flagged since the last check: an asynchronous CUDA
  * fault (AIMS_ERR_CUDA) or a failed device-side capacity / consistency check (AIMS_ERR_UNSUPPORTED). */
 int aims_gpu_synchronize(aims_gpu_ctx *ctx);

@@ -83,6 +83,8 @@ def load_library():
     L.aims_gpu_update_density.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp, _vp]
     L.aims_gpu_pulay_forces.restype = ctypes.c_int
     L.aims_gpu_pulay_forces.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp, _vp, _vp, _vp, ctypes.c_int]
+    L.aims_gpu_pulay_forces_ks.restype = ctypes.c_int
+    L.aims_gpu_pulay_forces_ks.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp, ctypes.c_int, _vp, _vp, _vp, ctypes.c_int]
     L.aims_gpu_synchronize.restype = ctypes.c_int
     L.aims_gpu_synchronize.argtypes = [cp]
     L.aims_gpu_batch_nnz.restype = ctypes.c_int
@@ -267,7 +269,7 @@ class Context:
                     "aims_gpu_update_density")
         return n, (grad_n if want_grad else None)
 
-    def pulay_forces(self, v, D, g=None, Q=None, F=None, b0=0, b1=None, accumulate=False):
+    def pulay_forces(self, v, D, g=None, Q=None, F=None, b0=0, b1=None, accumulate=False, kinetic=False):
         """F[n_atoms][3] (device tensor): Pulay forces of batches [b0,b1) (include/aims_gpu.h: aims_gpu_pulay_forces)."""
         torch = self.torch
         b0, b1 = self._range(b0, b1)
@@ -283,6 +285,10 @@ class Context:
             with torch.cuda.stream(self.stream):
                 F = torch.empty((self.n_atoms, 3), dtype=torch.float64, device=self.device)
             accumulate = False
+        if kinetic:
+            self._check(self.L.aims_gpu_pulay_forces_ks(self.h, b0, b1, _ptr(v), _ptr(g), 1, _ptr(D), _ptr(Q), _ptr(F),
+                                                        int(bool(accumulate))), "aims_gpu_pulay_forces_ks")
+            return F
         self._check(self.L.aims_gpu_pulay_forces(self.h, b0, b1, _ptr(v), _ptr(g), _ptr(D), _ptr(Q), _ptr(F),
                                                  int(bool(accumulate))), "aims_gpu_pulay_forces")
         return F
@@ -342,3 +348,7 @@ def aims_gpu_update_density(ctx, D, want_grad=False, n=None, grad_n=None, b0=0, 
 
 def aims_gpu_pulay_forces(ctx, v, D, g=None, Q=None, F=None, b0=0, b1=None, accumulate=False):
     return ctx.pulay_forces(v, D, g, Q, F, b0, b1, accumulate)
+
+
+def aims_gpu_pulay_forces_ks(ctx, v, D, g=None, kinetic=True, Q=None, F=None, b0=0, b1=None, accumulate=False):
+    return ctx.pulay_forces(v, D, g, Q, F, b0, b1, accumulate, kinetic=kinetic)

@@ -559,8 +559,8 @@ int aims_gpu_update_density(aims_gpu_ctx *c, int32_t b0, int32_t b1, const doubl
   return AIMS_OK;
 }
 
-int aims_gpu_pulay_forces(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, const double *g, const double *D_values,
-                          const double *Q_values, double *F, int accumulate) {
+static int run_forces(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, const double *g, int kinetic,
+                      const double *D_values, const double *Q_values, double *F, int accumulate) {
   if (!range_ok(c, b0, b1)) return fail(c, AIMS_ERR_INVALID_ARG, "batch range outside [0, n_batches]");
   if ((!v && c->n_points) || !D_values || !F) return fail(c, AIMS_ERR_INVALID_ARG, "NULL v, D_values or F");
   CU_TRY(c, cudaSetDevice(c->device));
@@ -575,7 +575,7 @@ int aims_gpu_pulay_forces(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double 
     EvalArgs E{};
     for (int q = 0; q < npl; q++) E.plane[q] = c->ws + q * plane;
     E.pad_off = c->d_dpad_off; E.pad_base = c->dpad_off[bs];
-    E.v = v; E.g = g; E.n_points = c->n_points;
+    E.v = v; E.g = g; E.n_points = c->n_points; E.kinetic = kinetic ? 1 : 0;
     if (g) launch_eval<kEvalForceGga, kLayD>(c, E, bs, be); else launch_eval<kEvalForceLda, kLayD>(c, E, bs, be);
     const long long ni = c->item_off[be] - c->item_off[bs];
     if (ni > 0) {
@@ -595,6 +595,16 @@ int aims_gpu_pulay_forces(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double 
     bs = be;
   }
   return AIMS_OK;
+}
+
+int aims_gpu_pulay_forces(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, const double *g, const double *D_values,
+                          const double *Q_values, double *F, int accumulate) {
+  return run_forces(c, b0, b1, v, g, 0, D_values, Q_values, F, accumulate);
+}
+
+int aims_gpu_pulay_forces_ks(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, const double *g, int kinetic,
+                             const double *D_values, const double *Q_values, double *F, int accumulate) {
+  return run_forces(c, b0, b1, v, g, kinetic, D_values, Q_values, F, accumulate);
 }
 
 int aims_gpu_timing_enable(aims_gpu_ctx *c, int enable) {

@@ -262,6 +262,7 @@ struct EvalArgs {
   long long api_base;
   const double *v, *g;   // [n_points], [3][n_points]
   long long n_points;
+  int kinetic;           // force modes only: L also carries -1/2 lap Phi (h_KS phi of Eq. 16 with the kinetic operator)
 };
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -466,11 +467,12 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
           const double dR = Rt / sc;
           Rd = R * inv_dd;
           f = dR - (double)l * Rd;
-          if (KIN) {
-            // lap (R(d) Y_lm) = (R'' + 2 R'/d - l(l+1) R/d^2) Y_lm;  qlap = -w/4 times the radial factor
+          if (KIN || (FORCE && E.kinetic)) {
+            // lap (R(d) Y_lm) = (R'' + 2 R'/d - l(l+1) R/d^2) Y_lm;  qlap = -w/4 (H planes) or -1/2 (force planes) times
+            // the radial factor
             const double Rtt = 2.0 * c23.x + 6.0 * c23.y * xs;
             const double d2R = Rtt / (sc * sc) - Rt / (sc * dd);
-            qlap = -0.25 * w * (d2R + 2.0 * dR * inv_dd - (double)(l * (l + 1)) * Rd * inv_dd);
+            qlap = (FORCE ? -0.5 : -0.25 * w) * (d2R + 2.0 * dR * inv_dd - (double)(l * (l + 1)) * Rd * inv_dd);
           }
           if (HESS) {
             // Hess phi = A u u^T Y + B (1 - u u^T) Y + B (u gS^T + gS u^T) + C Hess S, phi = (R / d^l) S_lm(dvec)
@@ -496,7 +498,7 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
               if (MODE == kEvalHGga) op[1 % NPL][oi] = wv * phi + (wgx * ex + wgy * ey + wgz * ez);
               if (MODE == kEvalHKinGga) op[1 % NPL][oi] = wv * phi + (wgx * ex + wgy * ey + wgz * ez) + qlap * Y[m];
               if (FORCE) {
-                op[1 % NPL][oi] = HESS ? wv * phi + (wgx * ex + wgy * ey + wgz * ez) : wv * phi;
+                op[1 % NPL][oi] = (HESS ? wv * phi + (wgx * ex + wgy * ey + wgz * ez) : wv * phi) + qlap * Y[m];
                 op[2 % NPL][oi] = w * ex; op[3 % NPL][oi] = w * ey; op[4 % NPL][oi] = w * ez;
                 if (HESS) {
                   const double gsg = gx[m] * wgx + gy[m] * wgy + gz[m] * wgz;

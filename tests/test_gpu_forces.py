@@ -54,6 +54,18 @@ def test_forces_match_oracle(case, mode):
     assert _rel_max(F, ref) <= TOL_F
 
 
+@pytest.mark.parametrize("mode", ["lda", "gga_q"])
+def test_forces_with_kinetic_operator_match_oracle(case, mode):
+    """Rows f1 + f2: h_KS phi_j of Eq. 16 with -1/2 lap phi_j (aims_gpu_pulay_forces_ks)."""
+    name, bun, orc, ctx, Q = case
+    g = bun.g if mode.startswith("gga") else None
+    q = Q if mode.endswith("_q") else None
+    F = ctx.pulay_forces(bun.v, bun.D_values, g=g, Q=q, kinetic=True).cpu().numpy()
+    ctx.synchronize()
+    ref = orc.pulay_forces(bun.v, bun.D_values, g=g, Q_values=q, kinetic=True)
+    assert _rel_max(F, ref) <= TOL_F
+
+
 def test_forces_accumulate_and_subranges(case):
     name, bun, orc, ctx, Q = case
     import torch
