@@ -792,3 +792,63 @@ void orc_brute_kinetic(const orc_system *S, const double *v, double *Hd) {
   free(phi);
   free(afp);
 }
+
+/* ====================================================================================================================
+ * Hessian of the density ("the Hessian matrix of the density,
+ * d_xi d_xj n(r) (i, j = 1,...,3), is needed at least for total energy gradient calculations (forces and stresses) ...
+ * straightforward extensions of Eq. (3) ... six components, and each component has the same cost as n(r) itself").
+ * Differentiating Eq. 3 twice, for symmetric n_ij restricted to nnz(B):
+ *   d_c d_e n(r) = 2 sum_ij n_ij [ (d_c d_e phi_i) phi_j + (d_c phi_i)(d_e phi_j) ](r),
+ * components in the order (xx, yy, zz, xy, xz, yz).  Written as the double sum, no intermediate products.
+ * Pins (tests/test_oracle_hessian_pins.py): central differences of the pinned grad n on displaced points; closed form for one
+ * Gaussian; brute force over all functions in numpy; trace = Laplacian of n from the same pieces.
+ * ==================================================================================================================== */
+void orc_density_hessian(const orc_system *S, int n_sel, const int32_t *batches, const double *D_values, double *hess_n) {
+  static const int ic[6] = {0, 1, 2, 0, 0, 1}, ie[6] = {0, 1, 2, 1, 2, 2};
+  int64_t *afp = (int64_t *)malloc(sizeof(int64_t) * (S->n_atoms + 1));
+  orc_atom_fn_ptr(S, afp);
+  int nf_tot = (int)afp[S->n_atoms];
+  int32_t *idx = (int32_t *)malloc(sizeof(int32_t) * 4 * (size_t)nf_tot);
+  int32_t *fa = idx + nf_tot, *fs = fa + nf_tot, *fm = fs + nf_tot;
+  for (int q = 0; q < n_sel; q++) {
+    int b = batches[q];
+    int64_t p0 = S->batch_ptr[b];
+    int np = (int)(S->batch_ptr[b + 1] - p0);
+    int nnz = orc_batch_nnz(S, b, idx, fa, fs, fm);
+    if (np == 0) continue;
+    size_t sz = (size_t)nnz * np;
+    double *phi = (double *)malloc(sizeof(double) * (sz * 10 + 1));     /* phi, dphi[3], hess[6] */
+    double *dphi = phi + sz, *hes = phi + 4 * sz;
+    for (int i = 0; i < nnz;) {
+      int l = S->shell_l[fs[i]];
+      for (int p = 0; p < np; p++) {
+        double val[7], gr[7][3], hh[7][6];
+        orc_shell_hess_at_point(S, fa[i], fs[i], S->xyz + 3 * (p0 + p), val, gr, hh);
+        for (int m = 0; m < 2 * l + 1; m++) {
+          phi[(size_t)(i + m) * np + p] = val[m];
+          for (int c = 0; c < 3; c++) dphi[((size_t)c * nnz + i + m) * np + p] = gr[m][c];
+          for (int k = 0; k < 6; k++) hes[((size_t)k * nnz + i + m) * np + p] = hh[m][k];
+        }
+      }
+      i += 2 * l + 1;
+    }
+    double *Db = (double *)malloc(sizeof(double) * ((size_t)nnz * nnz + 1));
+    restrict_matrix(S, afp, nnz, idx, fa, D_values, Db);
+#pragma omp parallel for schedule(static)
+    for (int p = 0; p < np; p++) {
+      for (int k = 0; k < 6; k++) {
+        int c = ic[k], e = ie[k];
+        double acc = 0.0;
+        for (int i = 0; i < nnz; i++)
+          for (int j = 0; j < nnz; j++)
+            acc += Db[(size_t)i * nnz + j] * (hes[((size_t)k * nnz + i) * np + p] * phi[(size_t)j * np + p] +
+                                              dphi[((size_t)c * nnz + i) * np + p] * dphi[((size_t)e * nnz + j) * np + p]);
+        hess_n[(size_t)k * S->n_points + p0 + p] = 2.0 * acc;
+      }
+    }
+    free(Db);
+    free(phi);
+  }
+  free(idx);
+  free(afp);
+}

@@ -63,6 +63,7 @@ def _load():
         L.orc_brute_forces.argtypes = [sp, _dp, _dp, _dp, _dp, ctypes.c_int, _dp]
         L.orc_integrate_hamiltonian_ks.argtypes = [sp, ctypes.c_int, _ip, _dp, _dp, ctypes.c_int, _dp]
         L.orc_brute_kinetic.argtypes = [sp, _dp, _dp]
+        L.orc_density_hessian.argtypes = [sp, ctypes.c_int, _ip, _dp, _dp]
         _lib = L
     return _lib
 
@@ -206,6 +207,14 @@ class Oracle:
         gn = np.zeros((3, self.n_points)) if want_grad else None
         self.L.orc_update_density(ctypes.byref(self.sys), len(sel), _i(sel), _d(D), _d(n), _d(gn))
         return n, gn
+
+    def density_hessian(self, D_values, batches=None):
+        """hess_n[6][n_points] in the order (xx, yy, zz, xy, xz, yz); entries of batches not listed stay 0."""
+        sel = self._sel(batches)
+        D = np.ascontiguousarray(D_values, dtype=np.float64)
+        H = np.zeros((6, self.n_points))
+        self.L.orc_density_hessian(ctypes.byref(self.sys), len(sel), _i(sel), _d(D), _d(H))
+        return H
 
     # ---- brute force, tiny inputs
     def brute(self, v=None, g=None, D_dense=None, want_grad=False):
