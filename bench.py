@@ -57,7 +57,7 @@ def parse():
     ap.add_argument("--cpu-sample-batches", type=int, default=96)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--path", default="scf", choices=["scf", "forces"])
+    ap.add_argument("--path", default="scf", choices=["scf", "forces", "hessian"])
     ap.add_argument("--kinetic", action="store_true",
                     help="scf path with the full h_KS phi (kinetic term, row f2): a separate line, not the headline metric")
     return ap.parse_args()
@@ -127,7 +127,7 @@ def sample_batches(n_batches, k, seed=20191206):
     return np.sort(rng.choice(n_batches, size=min(k, n_batches), replace=False)).astype(np.int32)
 
 
-def time_oracle(bun, batches, gga, repeats=1, forces_q=None, kinetic=False):
+def time_oracle(bun, batches, gga, repeats=1, forces_q=None, kinetic=False, hessian=False):
     """Oracle as it stands on the host cores: H integration + density update (or, with forces_q, the Pulay forces) on
     the listed batches."""
     from oracle import oracle as orc
@@ -136,7 +136,9 @@ def time_oracle(bun, batches, gga, repeats=1, forces_q=None, kinetic=False):
     best = None
     for _ in range(repeats):
         t0 = time.perf_counter()
-        if forces_q is not None:
+        if hessian:
+            o.density_hessian(bun.D_values, batches=batches)
+        elif forces_q is not None:
             o.pulay_forces(bun.v, bun.D_values, g=bun.g if gga else None, Q_values=forces_q, batches=batches)
         else:
             if kinetic:
@@ -149,13 +151,13 @@ def time_oracle(bun, batches, gga, repeats=1, forces_q=None, kinetic=False):
     return pts, best, orc.num_threads()
 
 
-def run_reference(args, bun, gga, workload, metric, forces_q=None):
+def run_reference(args, bun, gga, workload, metric, forces_q=None, hessian=False):
     """--impl reference: the CPU oracle, rank 0 only, a bounded sample per step."""
     per_step = max(4, args.cpu_sample_batches // 4)
     times, pts_step = [], 0
     for s in range(args.warmup + args.steps):
         sel = sample_batches(bun.n_batches, per_step, seed=1000 + s)
-        pts, dt, cores = time_oracle(bun, sel, gga, forces_q=forces_q, kinetic=args.kinetic and forces_q is None)
+        pts, dt, cores = time_oracle(bun, sel, gga, forces_q=forces_q, kinetic=args.kinetic and forces_q is None, hessian=hessian)
         if s >= args.warmup:
             times.append(dt)
             pts_step += pts
@@ -185,8 +187,11 @@ def main():
         workload += " [DEBUG GRID n_rad=%s n_ang=%s: not the benchmark workload]" % (args.n_rad, args.n_ang)
 
     forces = args.path == "forces"
+    hessian = args.path == "hessian"
     metric = METRIC if not forces else "grid points/s for the Pulay-force pass (FP64); % of FP64 peak"
-    if args.kinetic and not forces:
+    if hessian:
+        metric = "grid points/s for the density-Hessian pass (FP64); % of FP64 peak"
+    if args.kinetic and not forces and not hessian:
         metric = "grid points/s for H integration with the kinetic term + density update (FP64); % of FP64 peak"
     kin = bool(args.kinetic)
 
@@ -195,7 +200,10 @@ def main():
         if rank != 0:
             return 0
         bun = aims_synth.make_config(args.config, n_rad=args.n_rad, n_ang=args.n_ang, max_batch=args.max_batch)
-        run_reference(args, bun, gga, workload, metric, forces_q=aims_synth.make_q_values(bun) if forces else None)
+        if hessian:
+            args.cpu_sample_batches = min(args.cpu_sample_batches, 32)
+        run_reference(args, bun, gga, workload, metric, forces_q=aims_synth.make_q_values(bun) if forces else None,
+                      hessian=hessian)
         return 0
 
     import torch
@@ -225,6 +233,7 @@ def main():
     flops_n = float((2.0 * npb * nnz * nnz)[b0:b1].sum())
     # Pulay forces: the DSYMM-shaped products q_b Phi, n_b L and (GGA) n_b Phi, 2 n_p nnz^2 each
     flops_f = (3.0 if gga else 2.0) * flops_n
+    flops_x = 4.0 * flops_n                      # density Hessian: n_b Phi and n_b d_e Phi, e = x, y, z
     Qh = aims_synth.make_q_values(bun) if forces else None
 
     with torch.cuda.stream(stream):
@@ -236,10 +245,14 @@ def main():
         gn = torch.zeros((3, bun.n_points), dtype=torch.float64, device="cuda") if gga else None
         Q = torch.as_tensor(Qh).to("cuda") if forces else None
         F = torch.zeros((bun.n_atoms, 3), dtype=torch.float64, device="cuda")
+        Hn = torch.zeros((6, bun.n_points), dtype=torch.float64, device="cuda") if hessian else None
     stream.synchronize()
 
     def step():
         with torch.cuda.stream(stream):
+            if hessian:
+                ctx.density_hessian(D, hess_n=Hn, b0=b0, b1=b1)
+                return
             if forces:
                 ctx.pulay_forces(v, D, g=g, Q=Q, F=F, b0=b0, b1=b1, accumulate=False)
                 if world > 1:
@@ -306,8 +319,18 @@ def main():
             hb["F"] = torch.empty((bun.n_atoms, 3), dtype=torch.float64, pin_memory=True)
             dv["Q"], dv["F"] = torch.empty_like(Q), torch.empty_like(F)
 
+        if hessian:
+            hb["Hn"] = torch.empty((6, bun.n_points), dtype=torch.float64, pin_memory=True)
+            dv["Hn"] = torch.empty_like(Hn)
+
         def step_e2e():
             with torch.cuda.stream(stream):
+                if hessian:
+                    dv["D"].copy_(hb["D"], non_blocking=True)
+                    ctx.density_hessian(dv["D"], hess_n=dv["Hn"], b0=b0, b1=b1)
+                    lo, hi = int(bun.batch_ptr[b0]), int(bun.batch_ptr[b1])
+                    hb["Hn"][:, lo:hi].copy_(dv["Hn"][:, lo:hi], non_blocking=True)
+                    return
                 dv["v"].copy_(hb["v"], non_blocking=True)
                 dv["D"].copy_(hb["D"], non_blocking=True)
                 if gga:
@@ -347,20 +370,30 @@ def main():
         d2h = 8 * (bun.n_values + my_points * (4 if gga else 1))
         if forces:
             h2d, d2h = h2d + 8 * bun.n_values, 8 * 3 * bun.n_atoms
+        if hessian:
+            h2d, d2h = 8 * bun.n_values, 8 * 6 * my_points
         e2e = {"value": bun.n_points / (ms_e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                "d2h_bytes_per_step": int(d2h), "ms_per_step": ms_e}
         # the end-to-end outputs are the same numbers as the device-resident ones
-        if forces:
+        if hessian:
+            assert torch.equal(hb["Hn"][:, int(bun.batch_ptr[b0]):int(bun.batch_ptr[b1])],
+                               Hn[:, int(bun.batch_ptr[b0]):int(bun.batch_ptr[b1])].cpu())
+        elif forces:
             assert torch.allclose(hb["F"], F.cpu(), rtol=0, atol=1e-10 * float(F.abs().max()))   # atomics: rounding only
         else:
             assert torch.equal(hb["n"][int(bun.batch_ptr[b0]):int(bun.batch_ptr[b1])],
                                n[int(bun.batch_ptr[b0]):int(bun.batch_ptr[b1])].cpu())
 
     # ---- roofline of the dominant kernel (FP64 tensor pipe), live CUDA-event durations from the timed region
-    kflops = {"k_forces": flops_f} if forces else {"k_hamiltonian": flops_h, "k_density": flops_n}
+    if hessian:                                  # the library times k_density_hessian in the k_forces slot
+        kern = dict(kern)
+        kern["k_density_hessian"] = kern["k_forces"]
+    kflops = ({"k_density_hessian": flops_x} if hessian else {"k_forces": flops_f} if forces
+              else {"k_hamiltonian": flops_h, "k_density": flops_n})
     dom = max(kflops, key=lambda k: kern[k][0])
     kd = {}
-    for k in ("k_cull", "k_eval", "k_forces") if forces else ("k_cull", "k_eval", "k_hamiltonian", "k_density"):
+    for k in (("k_cull", "k_eval", "k_density_hessian") if hessian else ("k_cull", "k_eval", "k_forces") if forces
+              else ("k_cull", "k_eval", "k_hamiltonian", "k_density")):
         ms, ln = kern[k]
         kd[k] = {"ms_per_step": ms / args.steps, "launches_per_step": ln / args.steps}
         if k in kflops and ms > 0:
@@ -374,16 +407,18 @@ def main():
                 "peak_measured_probe": peak_measured, "frac_of_measured_probe": achieved / peak_measured,
                 "avg_launch_ms": dom_ms / max(dom_ln, 1), "algorithmic_flops_per_step": kflops[dom],
                 "share_of_step": dom_ms / ms_total}
-    total_tflops = (flops_f if forces else flops_h + flops_n) / (ms_step * 1e-3) / 1e12
+    total_tflops = (flops_x if hessian else flops_f if forces else flops_h + flops_n) / (ms_step * 1e-3) / 1e12
     # DRAM traffic per launch of the dominant kernel from the committed `ncu --set full` capture (config 5 only)
     if args.config == 5 and not (args.max_batch or args.n_rad or args.n_ang) and world == 1:
-        roofline["traffic"] = {"k_density": 125.75e9, "k_hamiltonian": 28.46e9, "k_forces": 152.29e9}[dom]
+        roofline["traffic"] = {"k_density": 125.75e9, "k_hamiltonian": 28.46e9, "k_forces": 152.29e9}.get(dom)
         roofline["traffic_note"] = ("dram__bytes_read.sum + dram__bytes_write.sum of one launch (bytes), "
                                     "profiles/r01_ncu_full_config5.md; Phi-plane bytes consumed per launch: 25.8e9")
     # second roofline: the HBM-bound evaluation kernel (algorithmic bytes = 8 B x planes x padded rows x padded points)
     pad = lambda a, m: np.ceil(a / m) * m                                   # noqa: E731
     pl_h, pl_d = 2.0, (4.0 if gga else 1.0)
-    if forces:
+    if hessian:
+        eval_bytes = 8.0 * float((10.0 * pad(nnz, 16) * pad(npb, 8))[b0:b1].sum())
+    elif forces:
         eval_bytes = 8.0 * float(((8.0 if gga else 5.0) * pad(nnz, 16) * pad(npb, 8))[b0:b1].sum())
     else:
         eval_bytes = 8.0 * float((pl_h * pad(nnz, 8) * pad(npb, 8) + pl_d * pad(nnz, 16) * pad(npb, 8))[b0:b1].sum())
@@ -415,7 +450,9 @@ def main():
     # ---- CPU baseline: the oracle on a bounded seeded sample, rank 0 at N=1 only
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         sel = sample_batches(bun.n_batches, args.cpu_sample_batches)
-        pts, dt, cores = time_oracle(bun, sel, gga, forces_q=Qh, kinetic=kin and not forces)
+        if hessian:
+            sel = sel[:32]
+        pts, dt, cores = time_oracle(bun, sel, gga, forces_q=Qh, kinetic=kin and not forces and not hessian, hessian=hessian)
         out["cpu_baseline"] = {"value": pts / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
                                "sample": "%d seeded batches (%d points) of the same workload, %.1f s" % (len(sel), pts, dt)}
     else:

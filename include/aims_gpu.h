@@ -133,6 +133,13 @@ int aims_gpu_integrate_hamiltonian_ks(aims_gpu_ctx *ctx, int32_t b0, int32_t b1,
 int aims_gpu_update_density(aims_gpu_ctx *ctx, int32_t b0, int32_t b1, const double *D_values, double *n,
                             double *grad_n);
 
+/* Row f1 of SURVEY.md 8(f): Hessian of the density, needed for total-energy gradients.  For every point
+ * p of batches [b0,b1), with symmetric n_ij restricted to nnz(B):
+ *   hess_n[k][p] = 2 sum_ij n_ij [ (d_c d_e phi_i) phi_j + (d_c phi_i)(d_e phi_j) ](r_p),  k = (c,e) in (xx, yy, zz, xy, xz, yz).
+ * DEVICE pointers: D_values [n_values] (pattern of aims_bsr_desc), hess_n [6][n_points] (component-major).  Points of other
+ * batches are not touched.  Reduced without atomics: bitwise reproducible.  Timed under slot [5] of aims_gpu_timing_read. */
+int aims_gpu_density_hessian(aims_gpu_ctx *ctx, int32_t b0, int32_t b1, const double *D_values, double *hess_n);
+
 /* Row f1 of SURVEY.md 8(f): Pulay forces, evaluated on the same batches as the density update (Eq. 14-18
  * L129-150; L301-308; L405).  For the reduced h_KS of this library (local potential v plus the GGA term above) and
  * nabla_at phi_i = -grad phi_i for the functions i centred on atom `at`, Eq. 16 and Eq. 18 on the grid:
@@ -171,7 +178,7 @@ int aims_gpu_batch_nnz(aims_gpu_ctx *ctx, int32_t *nnz);
  * CUDA events on the context stream.  aims_gpu_timing_enable synchronises, clears what was recorded and switches
  * recording on (enable != 0) or off.  aims_gpu_timing_read synchronises and returns, since the last enable/read, the
  * summed device milliseconds ms[6] and launch counts launches[6] (HOST outputs) of
- *   [0] k_cull  [1] k_eval  [2] k_hamiltonian  [3] k_density  [4] other  [5] k_forces. */
+ *   [0] k_cull  [1] k_eval  [2] k_hamiltonian  [3] k_density  [4] other  [5] k_forces / k_density_hessian. */
 int aims_gpu_timing_enable(aims_gpu_ctx *ctx, int enable);
 int aims_gpu_timing_read(aims_gpu_ctx *ctx, double *ms, int64_t *launches);
 

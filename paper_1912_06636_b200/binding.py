@@ -81,6 +81,8 @@ def load_library():
     L.aims_gpu_integrate_hamiltonian_ks.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp, ctypes.c_int, _vp, ctypes.c_int]
     L.aims_gpu_update_density.restype = ctypes.c_int
     L.aims_gpu_update_density.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp, _vp]
+    L.aims_gpu_density_hessian.restype = ctypes.c_int
+    L.aims_gpu_density_hessian.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp]
     L.aims_gpu_pulay_forces.restype = ctypes.c_int
     L.aims_gpu_pulay_forces.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp, _vp, _vp, _vp, ctypes.c_int]
     L.aims_gpu_pulay_forces_ks.restype = ctypes.c_int
@@ -269,6 +271,19 @@ class Context:
                     "aims_gpu_update_density")
         return n, (grad_n if want_grad else None)
 
+    def density_hessian(self, D, hess_n=None, b0=0, b1=None):
+        """hess_n[6][n_points] (xx, yy, zz, xy, xz, yz), device tensor (include/aims_gpu.h: aims_gpu_density_hessian)."""
+        torch = self.torch
+        b0, b1 = self._range(b0, b1)
+        D = self._dev(D, torch.float64)
+        if D.numel() != self.n_values:
+            raise AimsError("D must have n_values entries")
+        if hess_n is None:
+            with torch.cuda.stream(self.stream):
+                hess_n = torch.zeros((6, self.n_points), dtype=torch.float64, device=self.device)
+        self._check(self.L.aims_gpu_density_hessian(self.h, b0, b1, _ptr(D), _ptr(hess_n)), "aims_gpu_density_hessian")
+        return hess_n
+
     def pulay_forces(self, v, D, g=None, Q=None, F=None, b0=0, b1=None, accumulate=False, kinetic=False):
         """F[n_atoms][3] (device tensor): Pulay forces of batches [b0,b1) (include/aims_gpu.h: aims_gpu_pulay_forces)."""
         torch = self.torch
@@ -344,6 +359,10 @@ def aims_gpu_integrate_hamiltonian_ks(ctx, v, g=None, kinetic=True, H=None, b0=0
 
 def aims_gpu_update_density(ctx, D, want_grad=False, n=None, grad_n=None, b0=0, b1=None):
     return ctx.update_density(D, want_grad, n, grad_n, b0, b1)
+
+
+def aims_gpu_density_hessian(ctx, D, hess_n=None, b0=0, b1=None):
+    return ctx.density_hessian(D, hess_n, b0, b1)
 
 
 def aims_gpu_pulay_forces(ctx, v, D, g=None, Q=None, F=None, b0=0, b1=None, accumulate=False):

@@ -14,6 +14,7 @@
 #include "common.cuh"
 #include "density.cuh"
 #include "forces.cuh"
+#include "hessian.cuh"
 #include "hamiltonian.cuh"
 
 using namespace aims;
@@ -40,7 +41,7 @@ struct aims_gpu_ctx {
   HTile *d_tiles = nullptr;
   DItem *d_items = nullptr;
   double flops_h_lda = 0, flops_h_gga = 0, flops_den = 0;
-  bool ptab_in_smem = true, f_ptab_in_smem = true;
+  bool ptab_in_smem = true, f_ptab_in_smem = true, x_ptab_in_smem = true;
   std::vector<DItem> h_items;                                  // host copy of the density work items
   std::map<std::pair<int, int>, int *> item_order;             // (bs, be) -> device permutation, heaviest item first
 
@@ -341,15 +342,15 @@ int aims_gpu_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_gri
   if ((rc = dev_alloc(c, &L.act_ld, (size_t)c->act_off[nb]))) return rc;
   if ((rc = dev_alloc(c, &L.ptab, (size_t)c->ptab_off[nb]))) return rc;
 
-  // ---- Phi-plane workspace: enough for the largest single batch with 8 planes (forces), at most the requested budget
+  // ---- Phi-plane workspace: enough for the largest single batch with 10 planes (density Hessian), at most the requested budget
   long long want = workspace_bytes > 0 ? workspace_bytes : (24ll << 30);
   size_t free_b = 0, total_b = 0;
   CU_TRY(c, cudaMemGetInfo(&free_b, &total_b));
   want = std::min<long long>(want, (long long)(free_b * 0.8));
   long long max_batch_d = 0;
   for (int b = 0; b < nb; b++) max_batch_d = std::max(max_batch_d, c->dpad_off[b + 1] - c->dpad_off[b]);
-  long long need_all = 8 * c->dpad_off[nb], need_min = 8 * max_batch_d;
-  long long wsd = std::min(need_all, std::max(want / 8, need_min)) + 8 * 64;
+  long long need_all = 10 * c->dpad_off[nb], need_min = 10 * max_batch_d;
+  long long wsd = std::min(need_all, std::max(want / 8, need_min)) + 10 * 64;
   if (wsd * 8 > (long long)free_b) return fail(c, AIMS_ERR_NOMEM, "not enough device memory for one batch of Phi planes");
   if ((rc = dev_alloc(c, &c->ws, (size_t)wsd))) return rc;
   c->ws_doubles = wsd;
@@ -362,6 +363,10 @@ int aims_gpu_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_gri
   if (dsm > (size_t)prop.sharedMemPerBlockOptin) return fail(c, AIMS_ERR_UNSUPPORTED, "nnz(B) too large for the density kernel's shared memory");
   CU_TRY(c, cudaFuncSetAttribute(k_density<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dsm));
   CU_TRY(c, cudaFuncSetAttribute(k_density<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dsm));
+  c->x_ptab_in_smem = x_smem_bytes(c->max_nnz, std::max(c->max_act, 1), true) <= (size_t)prop.sharedMemPerBlockOptin;
+  if (x_smem_bytes(c->max_nnz, std::max(c->max_act, 1), c->x_ptab_in_smem) <= (size_t)prop.sharedMemPerBlockOptin)
+    CU_TRY(c, cudaFuncSetAttribute(k_density_hessian, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                   (int)x_smem_bytes(c->max_nnz, std::max(c->max_act, 1), c->x_ptab_in_smem)));
   c->f_ptab_in_smem = f_smem_bytes(c->max_nnz, std::max(c->max_act, 1), true) <= (size_t)prop.sharedMemPerBlockOptin;
   const size_t fsm = f_smem_bytes(c->max_nnz, std::max(c->max_act, 1), c->f_ptab_in_smem);
   CU_TRY(c, cudaFuncSetAttribute(k_forces<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsm));
@@ -372,6 +377,7 @@ int aims_gpu_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_gri
 #define EV_ATTR(M, LY) CU_TRY(c, cudaFuncSetAttribute(k_eval<M, LY>, cudaFuncAttributeMaxDynamicSharedMemorySize, esm));
     EV_ATTR(kEvalPhi, kLayApi) EV_ATTR(kEvalPhiGrad, kLayApi) EV_ATTR(kEvalHLda, kLayH) EV_ATTR(kEvalHGga, kLayH)
     EV_ATTR(kEvalHKinLda, kLayH) EV_ATTR(kEvalHKinGga, kLayH)
+    EV_ATTR(kEvalHess, kLayD)
     EV_ATTR(kEvalPhi, kLayD) EV_ATTR(kEvalPhiGrad, kLayD) EV_ATTR(kEvalForceLda, kLayD) EV_ATTR(kEvalForceGga, kLayD)
 #undef EV_ATTR
   }
@@ -590,6 +596,43 @@ static int run_forces(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, 
       TimedLaunch t(c, kKindForce);
       if (g) k_forces<true><<<(unsigned)ni, kDThreads, fsm, c->stream>>>(c->S, c->L, A, std::max(c->max_act, 1));
       else k_forces<false><<<(unsigned)ni, kDThreads, fsm, c->stream>>>(c->S, c->L, A, std::max(c->max_act, 1));
+    }
+    if ((rc = check_async(c))) return rc;
+    bs = be;
+  }
+  return AIMS_OK;
+}
+
+int aims_gpu_density_hessian(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *D_values, double *hess_n) {
+  if (!range_ok(c, b0, b1)) return fail(c, AIMS_ERR_INVALID_ARG, "batch range outside [0, n_batches]");
+  if (!D_values || (!hess_n && c->n_points)) return fail(c, AIMS_ERR_INVALID_ARG, "NULL D_values or hess_n");
+  CU_TRY(c, cudaSetDevice(c->device));
+  const size_t xsm = x_smem_bytes(c->max_nnz, std::max(c->max_act, 1), c->x_ptab_in_smem);
+  cudaDeviceProp prop;
+  CU_TRY(c, cudaGetDeviceProperties(&prop, c->device));
+  if (xsm > (size_t)prop.sharedMemPerBlockOptin) return fail(c, AIMS_ERR_UNSUPPORTED, "nnz(B) too large for the Hessian kernel's shared memory");
+  int rc = run_cull(c, b0, b1);
+  if (rc) return rc;
+  const int npl = 10;
+  for (int bs = b0; bs < b1;) {
+    const int be = chunk_end(c, c->dpad_off, bs, b1, npl);
+    const long long plane = (c->ws_doubles / npl) & ~63ll;
+    EvalArgs E{};
+    for (int q = 0; q < npl; q++) E.plane[q] = c->ws + q * plane;
+    E.pad_off = c->d_dpad_off; E.pad_base = c->dpad_off[bs];
+    E.n_points = c->n_points;
+    launch_eval<kEvalHess, kLayD>(c, E, bs, be);
+    const long long ni = c->item_off[be] - c->item_off[bs];
+    if (ni > 0) {
+      XArgs A{};
+      if ((rc = density_order(c, bs, be, &A.order))) return rc;
+      A.items = c->d_items + c->item_off[bs];
+      for (int q = 0; q < npl; q++) A.PL[q] = E.plane[q];
+      A.pad_off = c->d_dpad_off; A.pad_base = c->dpad_off[bs];
+      A.D = D_values; A.hn = hess_n; A.n_points = c->n_points; A.max_nnz_pad = c->max_nnz;
+      A.ptab_in_smem = c->x_ptab_in_smem ? 1 : 0;
+      TimedLaunch t(c, kKindForce);
+      k_density_hessian<<<(unsigned)ni, kDThreads, xsm, c->stream>>>(c->S, c->L, A, std::max(c->max_act, 1));
     }
     if ((rc = check_async(c))) return rc;
     bs = be;

@@ -241,14 +241,17 @@ enum EvalMode {
   // plane0 = Phi, plane1 = w ((v Phi - 1/2 lap Phi) / 2 [+ g . grad Phi]) -- the SYR2K form P Q^T + Q P^T then gives
   // 1/2 [phi_i (h phi_j) + (h phi_i) phi_j], Fig. 6a's DSYR2K with alpha = 1/2
   kEvalHKinLda = 6,
-  kEvalHKinGga = 7
+  kEvalHKinGga = 7,
+  // Hessian of the density (hessian.cuh): plane0 = Phi, planes 1..3 = d/dx_c Phi,
+  // planes 4..9 = d_c d_e Phi in the order (xx, yy, zz, xy, xz, yz)
+  kEvalHess = 8
 };
 __host__ __device__ constexpr int eval_planes(int mode) {
-  return mode == kEvalPhi ? 1 : mode == kEvalPhiGrad ? 4 : mode == kEvalForceLda ? 5 : mode == kEvalForceGga ? 8 : 2;
+  return mode == kEvalPhi ? 1 : mode == kEvalPhiGrad ? 4 : mode == kEvalForceLda ? 5 : mode == kEvalForceGga ? 8 : mode == kEvalHess ? 10 : 2;
 }
 
 struct EvalArgs {
-  double *plane[8];
+  double *plane[10];
   // kLayH, the k4 layout of common.cuh: element (row, p) of batch b at
   //   plane[q] + (pad_off[b] - pad_base) + ((p >> 2) * pad8(nnz) + row) * 4 + (p & 3); rows in [nnz, pad8(nnz)) and
   //   points in [n_p, pad8(n_p)) are written as zeros; a batch occupies pad8(nnz) * pad8(n_p) doubles per plane.
@@ -323,12 +326,13 @@ __device__ __forceinline__ int eval_row_off(int row, int np, int np8) {
 }
 
 template <int MODE, int LAYOUT>
-__global__ void __launch_bounds__(256, (MODE == kEvalForceLda || MODE == kEvalForceGga) ? 1 : AIMS_EVAL_CTAS_PER_SM)
+__global__ void __launch_bounds__(256, (MODE == kEvalForceLda || MODE == kEvalForceGga || MODE == kEvalHess) ? 1 : AIMS_EVAL_CTAS_PER_SM)
 k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
   constexpr bool FORCE = (MODE == kEvalForceLda || MODE == kEvalForceGga);
   constexpr bool HESS = (MODE == kEvalForceGga);
   constexpr bool KIN = (MODE == kEvalHKinLda || MODE == kEvalHKinGga);
-  constexpr bool GRAD = (MODE == kEvalPhiGrad || MODE == kEvalHGga || MODE == kEvalHKinGga || FORCE);
+  constexpr bool FULLH = (MODE == kEvalHess);        // all six second derivatives of every function
+  constexpr bool GRAD = (MODE == kEvalPhiGrad || MODE == kEvalHGga || MODE == kEvalHKinGga || FORCE || FULLH);
   constexpr int NPL = eval_planes(MODE);
   const int b = b_first + blockIdx.x;
   const int tid = threadIdx.x;
@@ -426,6 +430,7 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
     double d2 = 0.0, ux = 0.0, uy = 0.0, uz = 1.0, dd = 1.0, inv_dd = 1.0, xs = 0.0, ug = 0.0;
     double Y[7], gx[7], gy[7], gz[7];
     double hx[HESS ? 7 : 1], hy[HESS ? 7 : 1], hz[HESS ? 7 : 1];
+    double s2[FULLH ? 6 : 1][FULLH ? 7 : 1];        // Hess S_lm at the unit vector: (xx, yy, zz, xy, xz, yz)
 #pragma unroll 1
     for (int e = 0; e < n_ent; e++) {
       const int2 en = s_ent[e];
@@ -455,6 +460,14 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
         if (l != lcur) {
           solid_harmonics<GRAD>(l, ux, uy, uz, Y, gx, gy, gz);
           if constexpr (HESS) solid_hessian_dot(l, ux, uy, uz, wgx, wgy, wgz, hx, hy, hz);
+          if constexpr (FULLH) {
+            // columns of Hess S_lm = (Hess S_lm) e_c for the three unit vectors e_c
+            double t0[7], t1[7], t2[7];
+            solid_hessian_dot(l, ux, uy, uz, 1.0, 0.0, 0.0, s2[0], t1, t2);       // xx, (yx), (zx)
+            solid_hessian_dot(l, ux, uy, uz, 0.0, 1.0, 0.0, s2[3], s2[1], t2);    // xy, yy, (zy)
+            solid_hessian_dot(l, ux, uy, uz, 0.0, 0.0, 1.0, s2[4], s2[5], s2[2]); // xz, yz, zz
+            (void)t0;
+          }
           lcur = l;
         }
         const double2 *cf = reinterpret_cast<const double2 *>(S.spline_coef + (long long)(en.y + k) * 4);
@@ -474,7 +487,7 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
             const double d2R = Rtt / (sc * sc) - Rt / (sc * dd);
             qlap = (FORCE ? -0.5 : -0.25 * w) * (d2R + 2.0 * dR * inv_dd - (double)(l * (l + 1)) * Rd * inv_dd);
           }
-          if (HESS) {
+          if (HESS || FULLH) {
             // Hess phi = A u u^T Y + B (1 - u u^T) Y + B (u gS^T + gS u^T) + C Hess S, phi = (R / d^l) S_lm(dvec)
             const double Rtt = 2.0 * c23.x + 6.0 * c23.y * xs;
             const double d2R = Rtt / (sc * sc) - Rt / (sc * dd);
@@ -494,7 +507,17 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
             if (GRAD) {
               const double fy = f * Y[m];
               const double ex = fy * ux + Rd * gx[m], ey = fy * uy + Rd * gy[m], ez = fy * uz + Rd * gz[m];
-              if (MODE == kEvalPhiGrad) { op[1 % NPL][oi] = ex; op[2 % NPL][oi] = ey; op[3 % NPL][oi] = ez; }
+              if (MODE == kEvalPhiGrad || FULLH) { op[1 % NPL][oi] = ex; op[2 % NPL][oi] = ey; op[3 % NPL][oi] = ez; }
+              if (FULLH) {
+                const double ab = (hA - hB) * Y[m], by = hB * Y[m];
+                const double ax = ab * ux + hB * gx[m], ay = ab * uy + hB * gy[m], az = ab * uz + hB * gz[m];   // u_e coefficient
+                op[4 % NPL][oi] = ax * ux + hB * ux * gx[m] + by + hC * s2[0][FULLH ? m : 0];
+                op[5 % NPL][oi] = ay * uy + hB * uy * gy[m] + by + hC * s2[FULLH ? 1 : 0][FULLH ? m : 0];
+                op[6 % NPL][oi] = az * uz + hB * uz * gz[m] + by + hC * s2[FULLH ? 2 : 0][FULLH ? m : 0];
+                op[7 % NPL][oi] = ax * uy + hB * ux * gy[m] + hC * s2[FULLH ? 3 : 0][FULLH ? m : 0];
+                op[8 % NPL][oi] = ax * uz + hB * ux * gz[m] + hC * s2[FULLH ? 4 : 0][FULLH ? m : 0];
+                op[9 % NPL][oi] = ay * uz + hB * uy * gz[m] + hC * s2[FULLH ? 5 : 0][FULLH ? m : 0];
+              }
               if (MODE == kEvalHGga) op[1 % NPL][oi] = wv * phi + (wgx * ex + wgy * ey + wgz * ez);
               if (MODE == kEvalHKinGga) op[1 % NPL][oi] = wv * phi + (wgx * ex + wgy * ey + wgz * ez) + qlap * Y[m];
               if (FORCE) {
