@@ -852,3 +852,46 @@ void orc_density_hessian(const orc_system *S, int n_sel, const int32_t *batches,
   free(idx);
   free(afp);
 }
+
+/* ====================================================================================================================
+ * Periodic boundary conditions: Bloch sums (Eq. 6-8, Eq. 11-12,
+ * L113-115).  The real-space matrix h^uc_IJ (Eq. 12) runs over the N_rs functions -- the cell's functions and their
+ * periodic images that are non-zero inside the cell at T = 0 -- and is integrated by O3 unchanged ("the exact same
+ * real-space integration code", the points having been mapped back into the cell by the input generator).  Inserting
+ * Eq. 7, chi_ik = sum_T e^{ik.T} phi_i(r - T), into Eq. 11 gives
+ *   h_ij(k) = sum_{I image of i} sum_{J image of j} e^{ik.(T_J - T_I)} h^uc_IJ        (L115, "Bloch phase factors"),
+ * and s_ij(k) analogously.  atom_home[A] < n_home is the cell atom that atom A is an image of (the cell's own atoms are
+ * atoms 0..n_home-1 with T = 0), atom_T[A] its lattice translation.  Output: dense [n_hb][n_hb] real and imaginary parts,
+ * n_hb = functions of the cell atoms.  Accumulated into (caller zeroes).
+ * Pins (tests/test_oracle_periodic_pins.py): closed-form lattice sums of Gaussian overlaps; direct quadrature of Eq. 8 with
+ * explicitly built Bloch functions; Hermitian, real at k = 0, positive definite; sum of weights = cell volume.
+ * ==================================================================================================================== */
+void orc_bloch_fold(const orc_system *S, const double *H_values, const int32_t *atom_home, const double *atom_T, int n_home,
+                    const double *kpt, double *out_re, double *out_im) {
+  int64_t *afp = (int64_t *)malloc(sizeof(int64_t) * (S->n_atoms + 1));
+  orc_atom_fn_ptr(S, afp);
+  int64_t nhb = afp[n_home];
+  for (int A = 0; A < S->n_atoms; A++) {
+    int nA = (int)(afp[A + 1] - afp[A]);
+    for (int64_t q = S->row_ptr[A]; q < S->row_ptr[A + 1]; q++) {
+      int B = S->col_atom[q];
+      int nB = (int)(afp[B + 1] - afp[B]);
+      int ld = S->blk_ld[q];
+      double th = 0.0;
+      for (int c = 0; c < 3; c++) th += kpt[c] * (atom_T[3 * B + c] - atom_T[3 * A + c]);
+      double cs = cos(th), sn = sin(th);
+      int64_t i0 = afp[atom_home[A]], j0 = afp[atom_home[B]];
+      for (int a = 0; a < nA; a++)
+        for (int b = 0; b < nB; b++) {
+          double h = H_values[S->blk_off[q] + (int64_t)a * ld + b];
+          out_re[(i0 + a) * nhb + (j0 + b)] += h * cs;
+          out_im[(i0 + a) * nhb + (j0 + b)] += h * sn;
+          if (A != B) {                         /* the stored block also stands for h^uc_JI = h^uc_IJ, phase conjugated */
+            out_re[(j0 + b) * nhb + (i0 + a)] += h * cs;
+            out_im[(j0 + b) * nhb + (i0 + a)] -= h * sn;
+          }
+        }
+    }
+  }
+  free(afp);
+}

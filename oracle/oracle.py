@@ -64,6 +64,7 @@ def _load():
         L.orc_integrate_hamiltonian_ks.argtypes = [sp, ctypes.c_int, _ip, _dp, _dp, ctypes.c_int, _dp]
         L.orc_brute_kinetic.argtypes = [sp, _dp, _dp]
         L.orc_density_hessian.argtypes = [sp, ctypes.c_int, _ip, _dp, _dp]
+        L.orc_bloch_fold.argtypes = [sp, _dp, _ip, _dp, ctypes.c_int, _dp, _dp, _dp]
         _lib = L
     return _lib
 
@@ -215,6 +216,19 @@ class Oracle:
         H = np.zeros((6, self.n_points))
         self.L.orc_density_hessian(ctypes.byref(self.sys), len(sel), _i(sel), _d(D), _d(H))
         return H
+
+    def bloch_fold(self, H_values, atom_home, atom_T, n_home, kpt):
+        """Complex dense [n_hb][n_hb] matrix h_ij(k) = sum_IJ e^{ik.(T_J - T_I)} h^uc_IJ (Eq. 7, 11, 12)."""
+        H = np.ascontiguousarray(H_values, dtype=np.float64)
+        home = np.ascontiguousarray(atom_home, dtype=np.int32)
+        T = np.ascontiguousarray(atom_T, dtype=np.float64)
+        k = np.ascontiguousarray(kpt, dtype=np.float64)
+        afp = np.zeros(self.sys.n_atoms + 1, dtype=np.int64)
+        self.L.orc_atom_fn_ptr(ctypes.byref(self.sys), _l(afp))
+        nhb = int(afp[n_home])
+        re, im = np.zeros((nhb, nhb)), np.zeros((nhb, nhb))
+        self.L.orc_bloch_fold(ctypes.byref(self.sys), _d(H), _i(home), _d(T), int(n_home), _d(k), _d(re), _d(im))
+        return re + 1j * im
 
     # ---- brute force, tiny inputs
     def brute(self, v=None, g=None, D_dense=None, want_grad=False):
