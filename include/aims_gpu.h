@@ -161,6 +161,19 @@ int aims_gpu_pulay_forces(aims_gpu_ctx *ctx, int32_t b0, int32_t b1, const doubl
 int aims_gpu_pulay_forces_ks(aims_gpu_ctx *ctx, int32_t b0, int32_t b1, const double *v, const double *g, int kinetic,
                              const double *D_values, const double *Q_values, double *F, int accumulate);
 
+/* Row f3 of SURVEY.md 8(f): periodic boundary conditions.  The real-space matrix h^uc of Eq. 12 runs over
+ * the N_rs functions of the cell atoms AND their periodic images that reach into the cell; the caller passes all of them as
+ * atoms (the cell's own atoms first) with the grid points mapped back into the cell at T = 0 (L113-115), and
+ * aims_gpu_integrate_hamiltonian / aims_gpu_update_density run unchanged ("the exact same real-space integration code").
+ * This call forms the Bloch sums of Eq. 7 inserted into Eq. 11 (L115):
+ *   out[i][j] (+)= sum_{I image of i} sum_{J image of j} e^{i k.(T_J - T_I)} H[I][J],   i, j = functions of the cell atoms.
+ * H_values: DEVICE [n_values] (h^uc or s^uc, upper blocks, symmetric).  HOST inputs: atom_home [n_atoms] (index < n_home of the
+ * cell atom an atom is an image of; atoms 0..n_home-1 are the cell's own, with atom_T = 0), atom_T [n_atoms][3] lattice
+ * translations, kpt [3] (rad / Angstrom).  DEVICE outputs out_re, out_im: dense row-major [n_hb][n_hb], n_hb = functions of
+ * the cell atoms.  accumulate == 0: zeroed first.  Synchronises the context stream before returning. */
+int aims_gpu_bloch_fold(aims_gpu_ctx *ctx, const double *H_values, const int32_t *atom_home, const double *atom_T,
+                        int32_t n_home, const double *kpt, double *out_re, double *out_im, int accumulate);
+
 /* Synchronise the context stream and report anything the device flagged since the last check: an asynchronous CUDA
  * fault (AIMS_ERR_CUDA) or a failed device-side capacity / consistency check (AIMS_ERR_UNSUPPORTED). */
 int aims_gpu_synchronize(aims_gpu_ctx *ctx);

@@ -81,6 +81,8 @@ def load_library():
     L.aims_gpu_integrate_hamiltonian_ks.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp, ctypes.c_int, _vp, ctypes.c_int]
     L.aims_gpu_update_density.restype = ctypes.c_int
     L.aims_gpu_update_density.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp, _vp]
+    L.aims_gpu_bloch_fold.restype = ctypes.c_int
+    L.aims_gpu_bloch_fold.argtypes = [cp, _vp, _ip, _dp, ctypes.c_int32, _dp, _vp, _vp, ctypes.c_int]
     L.aims_gpu_density_hessian.restype = ctypes.c_int
     L.aims_gpu_density_hessian.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp]
     L.aims_gpu_pulay_forces.restype = ctypes.c_int
@@ -271,6 +273,24 @@ class Context:
                     "aims_gpu_update_density")
         return n, (grad_n if want_grad else None)
 
+    def bloch_fold(self, H, atom_home, atom_T, n_home, kpt, n_home_basis):
+        """Complex device tensor [n_hb][n_hb]: Bloch sums of a real-space matrix (include/aims_gpu.h: aims_gpu_bloch_fold)."""
+        torch = self.torch
+        H = self._dev(H, torch.float64)
+        if H.numel() != self.n_values:
+            raise AimsError("H must have n_values entries")
+        home = np.ascontiguousarray(atom_home, dtype=np.int32)
+        T = np.ascontiguousarray(atom_T, dtype=np.float64)
+        k = np.ascontiguousarray(kpt, dtype=np.float64)
+        if home.shape[0] != self.n_atoms or T.shape != (self.n_atoms, 3) or k.shape != (3,):
+            raise AimsError("atom_home [n_atoms], atom_T [n_atoms][3], kpt [3]")
+        with torch.cuda.stream(self.stream):
+            re = torch.empty((n_home_basis, n_home_basis), dtype=torch.float64, device=self.device)
+            im = torch.empty_like(re)
+        self._check(self.L.aims_gpu_bloch_fold(self.h, _ptr(H), home.ctypes.data_as(_ip), T.ctypes.data_as(_dp), int(n_home),
+                                               k.ctypes.data_as(_dp), _ptr(re), _ptr(im), 0), "aims_gpu_bloch_fold")
+        return torch.complex(re, im)
+
     def density_hessian(self, D, hess_n=None, b0=0, b1=None):
         """hess_n[6][n_points] (xx, yy, zz, xy, xz, yz), device tensor (include/aims_gpu.h: aims_gpu_density_hessian)."""
         torch = self.torch
@@ -359,6 +379,10 @@ def aims_gpu_integrate_hamiltonian_ks(ctx, v, g=None, kinetic=True, H=None, b0=0
 
 def aims_gpu_update_density(ctx, D, want_grad=False, n=None, grad_n=None, b0=0, b1=None):
     return ctx.update_density(D, want_grad, n, grad_n, b0, b1)
+
+
+def aims_gpu_bloch_fold(ctx, H, atom_home, atom_T, n_home, kpt, n_home_basis):
+    return ctx.bloch_fold(H, atom_home, atom_T, n_home, kpt, n_home_basis)
 
 
 def aims_gpu_density_hessian(ctx, D, hess_n=None, b0=0, b1=None):

@@ -3,6 +3,7 @@
 #include "../../include/aims_gpu.h"
 
 #include <algorithm>
+#include <cmath>
 #include <cstdio>
 #include <cstring>
 #include <map>
@@ -11,6 +12,7 @@
 #include <vector>
 
 #include "basis.cuh"
+#include "bloch.cuh"
 #include "common.cuh"
 #include "density.cuh"
 #include "forces.cuh"
@@ -36,6 +38,8 @@ struct aims_gpu_ctx {
   // host copies of the static structure (dry run)
   std::vector<long long> batch_ptr, fn_off, act_off, ptab_off, pad_off, dpad_off, api_off, tile_off, item_off;
   std::vector<int> nnz, n_act;
+  std::vector<int> h_atom_fn_ptr, h_col_atom, h_blk_ld;          // host copies of the pattern (Bloch sums)
+  std::vector<long long> h_row_ptr, h_blk_off;
   int max_nnz = 0, max_act = 0, max_np = 0;
   long long *d_pad_off = nullptr, *d_dpad_off = nullptr, *d_api_off = nullptr;
   HTile *d_tiles = nullptr;
@@ -205,6 +209,11 @@ int aims_gpu_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_gri
         return fail(c, AIMS_ERR_INVALID_ARG, "blk_off/blk_ld must be even, consistent per column atom and inside n_values");
     }
   }
+  c->h_atom_fn_ptr = atom_fn_ptr;
+  c->h_row_ptr.assign(P->row_ptr, P->row_ptr + na + 1);
+  c->h_col_atom.assign(P->col_atom, P->col_atom + n_blocks);
+  c->h_blk_off.assign(P->blk_off, P->blk_off + n_blocks);
+  c->h_blk_ld.assign(P->blk_ld, P->blk_ld + n_blocks);
   c->n_batches = G->n_batches;
   c->n_points = G->n_points;
   c->n_values = P->n_values;
@@ -601,6 +610,51 @@ static int run_forces(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, 
     bs = be;
   }
   return AIMS_OK;
+}
+
+int aims_gpu_bloch_fold(aims_gpu_ctx *c, const double *H_values, const int32_t *atom_home, const double *atom_T,
+                        int32_t n_home, const double *kpt, double *out_re, double *out_im, int accumulate) {
+  if (!c || !H_values || !atom_home || !atom_T || !kpt || !out_re || !out_im) return fail(c, AIMS_ERR_INVALID_ARG, "NULL argument");
+  const int na = c->S.n_atoms;
+  if (n_home <= 0 || n_home > na) return fail(c, AIMS_ERR_INVALID_ARG, "n_home outside [1, n_atoms]");
+  for (int a = 0; a < na; a++) {
+    const int h = atom_home[a];
+    if (h < 0 || h >= n_home || c->h_atom_fn_ptr[h + 1] - c->h_atom_fn_ptr[h] != c->h_atom_fn_ptr[a + 1] - c->h_atom_fn_ptr[a])
+      return fail(c, AIMS_ERR_INVALID_ARG, "atom_home must map every atom to a cell atom (< n_home) with the same functions");
+  }
+  CU_TRY(c, cudaSetDevice(c->device));
+  const int nhb = c->h_atom_fn_ptr[n_home];
+  if (!accumulate) {
+    CU_TRY(c, cudaMemsetAsync(out_re, 0, (size_t)nhb * nhb * sizeof(double), c->stream));
+    CU_TRY(c, cudaMemsetAsync(out_im, 0, (size_t)nhb * nhb * sizeof(double), c->stream));
+  }
+  std::vector<BlochBlock> blocks;
+  blocks.reserve(c->h_col_atom.size());
+  for (int A = 0; A < na; A++)
+    for (long long q = c->h_row_ptr[A]; q < c->h_row_ptr[A + 1]; q++) {
+      const int B = c->h_col_atom[(size_t)q];
+      double th = 0.0;
+      for (int d = 0; d < 3; d++) th += kpt[d] * (atom_T[3 * B + d] - atom_T[3 * A + d]);
+      BlochBlock bb;
+      bb.off = c->h_blk_off[(size_t)q]; bb.ld = c->h_blk_ld[(size_t)q];
+      bb.nA = c->h_atom_fn_ptr[A + 1] - c->h_atom_fn_ptr[A]; bb.nB = c->h_atom_fn_ptr[B + 1] - c->h_atom_fn_ptr[B];
+      bb.i0 = c->h_atom_fn_ptr[atom_home[A]]; bb.j0 = c->h_atom_fn_ptr[atom_home[B]];
+      bb.diag = (A == B) ? 1 : 0;
+      bb.cs = cos(th); bb.sn = sin(th);
+      blocks.push_back(bb);
+    }
+  if (blocks.empty()) return AIMS_OK;
+  BlochBlock *d_blocks = nullptr;
+  CU_TRY(c, cudaMalloc(&d_blocks, blocks.size() * sizeof(BlochBlock)));
+  cudaError_t e = cudaMemcpyAsync(d_blocks, blocks.data(), blocks.size() * sizeof(BlochBlock), cudaMemcpyHostToDevice, c->stream);
+  if (e == cudaSuccess) {
+    TimedLaunch t(c, kKindOther);
+    k_bloch_fold<<<(unsigned)blocks.size(), 128, 0, c->stream>>>(d_blocks, H_values, nhb, out_re, out_im);
+  }
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);   // blocks is a host temporary; the table is freed below
+  cudaFree(d_blocks);
+  if (e != cudaSuccess) { c->err = std::string("aims_gpu_bloch_fold: ") + cudaGetErrorString(e); return AIMS_ERR_CUDA; }
+  return check_async(c);
 }
 
 int aims_gpu_density_hessian(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *D_values, double *hess_n) {
