@@ -265,6 +265,8 @@ __global__ void __launch_bounds__(kHThreads, 2) k_hamiltonian(DevSys S, BatchLis
   const int sj = ci >> 16, cb = ci & 0xFFFF;
   const int ldj = (ci >= 0) ? s_ld[sj] : 0;
   const int csub = lane >> 3;
+  int cur_si = -1;                                            // atom slot of the row whose block offset is cached in `base`
+  long long base = -1;
 #pragma unroll
   for (int a = 0; a < 4; a++) {
     if (a < wa) {
@@ -275,13 +277,13 @@ __global__ void __launch_bounds__(kHThreads, 2) k_hamiltonian(DevSys S, BatchLis
           *reinterpret_cast<double2 *>(strip + fr * kHStripLd + c * 8 + 2 * fk) = make_double2(acc[a][c][0], acc[a][c][1]);
       __syncwarp();
       if (ci >= 0 && !(diag && csub < a)) {
-#pragma unroll 2
+#pragma unroll
         for (int r = 0; r < 8; r++) {
           const int ri = s_rowinfo[ri0 - rI0 + a * 8 + r];
           if (ri < 0) break;                                  // rows beyond nnz (zero padding) end the batch matrix
           const int si = ri >> 16, ra = ri & 0xFFFF;
           if (si > sj) continue;                              // lower atom block (only inside diagonal sub-tiles)
-          const long long base = __ldg(ptab + si * nact + sj);
+          if (si != cur_si) { cur_si = si; base = __ldg(ptab + si * nact + sj); }   // rows of one atom share the block
           if (base < 0) continue;                             // atom pair outside the pattern: exact zero
           const double val = strip[r * kHStripLd + lane];
           red_add_f64(A.H + base + (long long)ra * ldj + cb, val);
