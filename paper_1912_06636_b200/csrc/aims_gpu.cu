@@ -36,12 +36,12 @@ struct aims_gpu_ctx {
   int64_t n_points = 0, n_values = 0;
 
   // host copies of the static structure (dry run)
-  std::vector<long long> batch_ptr, fn_off, act_off, ptab_off, pad_off, dpad_off, api_off, tile_off, item_off;
+  std::vector<long long> batch_ptr, fn_off, act_off, ptab_off, pad_off, pad16_off, dpad_off, api_off, tile_off, item_off;
   std::vector<int> nnz, n_act;
   std::vector<int> h_atom_fn_ptr, h_col_atom, h_blk_ld;          // host copies of the pattern (Bloch sums)
   std::vector<long long> h_row_ptr, h_blk_off;
   int max_nnz = 0, max_act = 0, max_np = 0;
-  long long *d_pad_off = nullptr, *d_dpad_off = nullptr, *d_api_off = nullptr;
+  long long *d_pad_off = nullptr, *d_pad16_off = nullptr, *d_dpad_off = nullptr, *d_api_off = nullptr;
   HTile *d_tiles = nullptr;
   DItem *d_items = nullptr;
   double flops_h_lda = 0, flops_h_gga = 0, flops_den = 0;
@@ -284,7 +284,7 @@ int aims_gpu_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_gri
   if (flag == 2) return fail(c, AIMS_ERR_UNSUPPORTED, "more than AIMS_MAX_ACTIVE_ATOMS atoms touch one batch");
 
   c->fn_off.assign(nb + 1, 0); c->act_off.assign(nb + 1, 0); c->ptab_off.assign(nb + 1, 0);
-  c->pad_off.assign(nb + 1, 0); c->dpad_off.assign(nb + 1, 0); c->api_off.assign(nb + 1, 0); c->tile_off.assign(nb + 1, 0); c->item_off.assign(nb + 1, 0);
+  c->pad_off.assign(nb + 1, 0); c->pad16_off.assign(nb + 1, 0); c->dpad_off.assign(nb + 1, 0); c->api_off.assign(nb + 1, 0); c->tile_off.assign(nb + 1, 0); c->item_off.assign(nb + 1, 0);
   std::vector<HTile> tiles;
   std::vector<DItem> items;
   for (int b = 0; b < nb; b++) {
@@ -297,6 +297,7 @@ int aims_gpu_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_gri
     c->act_off[b + 1] = c->act_off[b] + nact;
     c->ptab_off[b + 1] = c->ptab_off[b] + (long long)nact * nact;
     c->pad_off[b + 1] = c->pad_off[b] + (long long)nz8 * np8;                 // H layout
+    c->pad16_off[b + 1] = c->pad16_off[b] + (long long)nz8 * round_up(np, 16);   // H layout of the LDA planes (16-point stages)
     c->dpad_off[b + 1] = c->dpad_off[b] + (long long)round_up(nz, 16) * np8;   // density layout
     c->api_off[b + 1] = c->api_off[b] + (long long)nz * np;
     // Hamiltonian tiles: I panels of kHIB blocks x J panels of kHJB blocks that contain a block (bi, bj >= bi)
@@ -336,7 +337,7 @@ int aims_gpu_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_gri
     long long *d;
 #define UPL(vec, field) if ((rc = dev_upload<long long>(c, &d, vec.data(), vec.size()))) return rc; field = d;
     UPL(c->fn_off, L.fn_off) UPL(c->act_off, L.act_off) UPL(c->ptab_off, L.ptab_off)
-    UPL(c->pad_off, c->d_pad_off) UPL(c->dpad_off, c->d_dpad_off) UPL(c->api_off, c->d_api_off)
+    UPL(c->pad_off, c->d_pad_off) UPL(c->pad16_off, c->d_pad16_off) UPL(c->dpad_off, c->d_dpad_off) UPL(c->api_off, c->d_api_off)
 #undef UPL
   }
   if ((rc = dev_upload<HTile>(c, &c->d_tiles, tiles.data(), tiles.size()))) return rc;
@@ -504,19 +505,22 @@ static int run_hamiltonian(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double
   int rc = run_cull(c, b0, b1);
   if (rc) return rc;
   const bool syr2k = g || kinetic;     // Q is not proportional to P: P Q^T + Q P^T
+  // the LDA kernel runs 16-point stages on planes padded to a multiple of 16 points
+  const std::vector<long long> &poff = syr2k ? c->pad_off : c->pad16_off;
+  const long long *d_poff = syr2k ? c->d_pad_off : c->d_pad16_off;
   for (int bs = b0; bs < b1;) {
-    const int be = chunk_end(c, c->pad_off, bs, b1, 2);
+    const int be = chunk_end(c, poff, bs, b1, 2);
     const long long plane = (c->ws_doubles / 2) & ~63ll;
     EvalArgs E{};
     E.plane[0] = c->ws; E.plane[1] = c->ws + plane;
-    E.pad_off = c->d_pad_off; E.pad_base = c->pad_off[bs];
+    E.pad_off = d_poff; E.pad_base = poff[bs]; E.point_pad = syr2k ? 8 : 16;
     E.v = v; E.g = g; E.n_points = c->n_points;
     if (kinetic) { if (g) launch_eval<kEvalHKinGga, kLayH>(c, E, bs, be); else launch_eval<kEvalHKinLda, kLayH>(c, E, bs, be); }
     else if (g) launch_eval<kEvalHGga, kLayH>(c, E, bs, be);
     else launch_eval<kEvalHLda, kLayH>(c, E, bs, be);
     const long long nt = c->tile_off[be] - c->tile_off[bs];
     if (nt > 0) {
-      HArgs A{c->d_tiles + c->tile_off[bs], E.plane[0], E.plane[1], c->d_pad_off, c->pad_off[bs], H_values};
+      HArgs A{c->d_tiles + c->tile_off[bs], E.plane[0], E.plane[1], d_poff, poff[bs], H_values};
       TimedLaunch t(c, kKindHam);
       if (syr2k) k_hamiltonian<true><<<(unsigned)nt, kHThreads, h_smem_bytes<true>(), c->stream>>>(c->S, c->L, A);
       else k_hamiltonian<false><<<(unsigned)nt, kHThreads, h_smem_bytes<false>(), c->stream>>>(c->S, c->L, A);

@@ -265,6 +265,7 @@ struct EvalArgs {
   long long api_base;
   const double *v, *g;   // [n_points], [3][n_points]
   long long n_points;
+  int point_pad;         // kLayH only: zero columns up to this multiple of points (0 = 8; 16 for the LDA Hamiltonian planes)
   int kinetic;           // force modes only: L also carries -1/2 lap Phi (h_KS phi of Eq. 16 with the kinetic operator)
 };
 
@@ -381,7 +382,8 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
   __syncthreads();
 
   const int nnz8 = pad8(nnz), np8 = pad8(np);
-  const int npx = LAYOUT == kLayApi ? np : np8;             // points this CTA writes (k4: zero columns up to pad8)
+  // points this CTA writes (k4 layouts: zero columns up to the padded point count)
+  const int npx = LAYOUT == kLayApi ? np : (LAYOUT == kLayH && E.point_pad > 8 ? round_up(np, E.point_pad) : np8);
   const int nrows = LAYOUT == kLayApi ? nnz : (LAYOUT == kLayD ? round_up(nnz, 16) : nnz8);   // rows this CTA writes
   double *o[NPL];
   if (LAYOUT == kLayApi) {

@@ -36,7 +36,7 @@ struct HTile { int b; short ti, tj; };
 struct HArgs {
   const HTile *tiles;       // tile list of this launch (already offset)
   const double *P, *Q;      // planes
-  const long long *pad_off; // [n_batches+1] prefix of pad8(nnz)*pad8(np) (doubles)
+  const long long *pad_off; // [n_batches+1] prefix of pad8(nnz)*round_up(np, GGA ? 8 : 16) (doubles)
   long long pad_base;
   double *H;                // block-sparse values
 };
@@ -48,7 +48,9 @@ __host__ __device__ inline int blk_count(int nsub) { return (nsub + 3) >> 2; }
 template <bool GGA>
 __host__ __device__ constexpr int h_group_doubles() { return (kHI + kHJ) * 4 * (GGA ? 2 : 1); }
 template <bool GGA>
-__host__ __device__ constexpr int h_stage_doubles() { return 2 * h_group_doubles<GGA>(); }
+__host__ __device__ constexpr int h_stage_groups() { return GGA ? 2 : 4; }   // 4-point groups per stage: 8 / 16 points
+template <bool GGA>
+__host__ __device__ constexpr int h_stage_doubles() { return h_stage_groups<GGA>() * h_group_doubles<GGA>(); }
 template <bool GGA>
 constexpr size_t h_smem_bytes() {
   return (size_t)kHStages * h_stage_doubles<GGA>() * sizeof(double) + (size_t)8 * 8 * kHStripLd * sizeof(double) +
@@ -68,7 +70,7 @@ __device__ __forceinline__ void h_mma_loop_t(double (&acc)[4][4][2], const doubl
                                              unsigned bar_full, unsigned bar_empty, int lane, Refill &&refill) {
   constexpr int NST = kHStages;
   constexpr int GW = h_group_doubles<GGA>(), SW = h_stage_doubles<GGA>();
-  constexpr int NU = GGA ? 4 : 2;                                       // product steps per stage
+  constexpr int NU = 4;                                                 // product steps per stage (LDA: 4 groups x 1, GGA: 2 x 2)
   // fragment bases of step u inside a stage
   auto a_base = [&](const double *st, int u) {
     return st + (GGA ? (u >> 1) : u) * GW + ((GGA && (u & 1)) ? (kHI + kHJ) * 4 : 0) + aoff;
@@ -170,8 +172,11 @@ __global__ void __launch_bounds__(kHThreads, 2) k_hamiltonian(DevSys S, BatchLis
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int nnz = L.nnz[b], nact = L.n_act[b];
   const int nnz8 = pad8(nnz), nsub = nnz8 >> 3, nblk = blk_count(nsub);
-  const int np8 = pad8((int)(S.batch_ptr[b + 1] - S.batch_ptr[b]));
-  const int nchunk = np8 >> 3;                                    // 8 points (two 4-point groups) per stage
+  // a stage holds 8 points (GGA: two groups, two products each) or 16 points (LDA: four groups); the LDA planes are padded
+  // with zero columns to a multiple of 16 points, so that both run four product steps per barrier round trip
+  constexpr int NG = h_stage_groups<GGA>();
+  const int npp = round_up((int)(S.batch_ptr[b + 1] - S.batch_ptr[b]), 4 * NG);
+  const int nchunk = npp / (4 * NG);
   const long long boff_plane = A.pad_off[b] - A.pad_base;
   const long long fo = L.fn_off[b], ao = L.act_off[b];
 
@@ -224,11 +229,11 @@ __global__ void __launch_bounds__(kHThreads, 2) k_hamiltonian(DevSys S, BatchLis
   auto issue = [&](int q) {
     const int s = q % NST;
     const unsigned bar = bar_full + 8 * s;
-    mbar_expect_tx(bar, 2u * (GGA ? 2u : 1u) * (bytesI + bytesJ));
+    mbar_expect_tx(bar, (unsigned)NG * (GGA ? 2u : 1u) * (bytesI + bytesJ));
     const unsigned dst = smem_u32(sm + (size_t)s * SW);
 #pragma unroll
-    for (int g = 0; g < 2; g++) {
-      const long long gI = ((long long)(2 * q + g) * nnz8 + rI0) * 4, gJ = ((long long)(2 * q + g) * nnz8 + rJ0) * 4;
+    for (int g = 0; g < NG; g++) {
+      const long long gI = ((long long)(NG * q + g) * nnz8 + rI0) * 4, gJ = ((long long)(NG * q + g) * nnz8 + rJ0) * 4;
       const unsigned d = dst + (unsigned)(g * GW) * 8u;
       bulk_g2s(d, gP + gI, bytesI, bar);
       bulk_g2s(d + kHI * 32u, gQ + gJ, bytesJ, bar);
