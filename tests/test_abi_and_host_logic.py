@@ -136,7 +136,18 @@ assert np.all(n[:lo] == 0) and np.all(n[hi:] == 0)
 parts = [torch.zeros(bun.n_points, dtype=torch.float64) for _ in range(world)]
 dist.all_gather(parts, torch.from_numpy(n))
 n_all = sum(parts).numpy()
+# widened rows: forces are partial sums like H (one all-reduce of 3 n_atoms numbers); the density Hessian shards like n
+Q = aims_synth.make_q_values(bun)
+F = torch.from_numpy(orc.pulay_forces(bun.v, bun.D_values, g=bun.g, Q_values=Q, batches=mine, kinetic=True))
+dist.all_reduce(F)
+hn = orc.density_hessian(bun.D_values, batches=mine)
+assert np.all(hn[:, :lo] == 0) and np.all(hn[:, hi:] == 0)
+hparts = [torch.zeros((6, bun.n_points), dtype=torch.float64) for _ in range(world)]
+dist.all_gather(hparts, torch.from_numpy(hn))
 if rank == 0:
+    F_ref = orc.pulay_forces(bun.v, bun.D_values, g=bun.g, Q_values=Q, kinetic=True)
+    assert np.abs(F.numpy() - F_ref).max() <= 1e-13 * np.abs(F_ref).max()
+    assert np.array_equal(sum(hparts).numpy(), orc.density_hessian(bun.D_values))
     H_ref = orc.integrate_hamiltonian(bun.v, bun.g)
     n_ref, _ = orc.update_density(bun.D_values, want_grad=True)
     eH = np.linalg.norm(H.numpy() - H_ref) / np.linalg.norm(H_ref)
