@@ -213,3 +213,9 @@ def make_q_values(bun, seed_offset=1000):
         blk = vals[bun.blk_off[q]: bun.blk_off[q] + n * ld].reshape(n, ld)
         blk[:, :n] = 0.5 * (blk[:, :n] + blk[:, :n].T)
     return vals
+
+
+def make_xi(bun):
+    """Stand-in for xi = d f_xc / d tau of a meta-GGA: a smooth positive field derived from the bundle's
+    seeded potential, xi_p = 0.3 + v_p^2 (no new random draws, so every bundle variant has one)."""
+    return 0.3 + np.asarray(bun.v) ** 2

@@ -895,3 +895,54 @@ void orc_bloch_fold(const orc_system *S, const double *H_values, const int32_t *
   }
   free(afp);
 }
+
+/* ====================================================================================================================
+ * tau matrix of meta-GGA functionals ("The evaluation of the tau matrix for
+ * meta-GGAs has been omitted in (a) for brevity.  It is calculated via a single DGEMM ... and added to the h^uc_ij matrix
+ * at the end of each batch").  The paper gives no formula; reading P1c takes the standard one: with the kinetic
+ * energy density tau(r) = 1/2 sum_ij n_ij grad phi_i . grad phi_j and xi(r) = d f_xc / d tau supplied as a field,
+ *   h_ij[B] += 1/2 sum_{r in B} w(r) xi(r) grad phi_i(r) . grad phi_j(r)          (= d/d n_ij of sum_r w f_xc(tau(r))).
+ * Added into H_values (upper atom-pair blocks, diagonal blocks full), like O3.
+ * Pins (tests/test_oracle_kinetic_pins.py): xi = 1 gives the kinetic matrix of the Laplacian form to grid accuracy
+ * (integration by parts) and the numpy grad-grad matrix exactly; Tr(n M) = sum_r w xi tau; symmetric, PSD for xi > 0.
+ * ==================================================================================================================== */
+void orc_tau_matrix(const orc_system *S, int n_sel, const int32_t *batches, const double *xi, double *H_values) {
+  int64_t *afp = (int64_t *)malloc(sizeof(int64_t) * (S->n_atoms + 1));
+  orc_atom_fn_ptr(S, afp);
+  int nf_tot = (int)afp[S->n_atoms];
+  int32_t *idx = (int32_t *)malloc(sizeof(int32_t) * 4 * (size_t)nf_tot);
+  int32_t *fa = idx + nf_tot, *fs = fa + nf_tot, *fm = fs + nf_tot;
+  for (int q = 0; q < n_sel; q++) {
+    int b = batches[q];
+    int64_t p0 = S->batch_ptr[b];
+    int np = (int)(S->batch_ptr[b + 1] - p0);
+    int nnz = orc_batch_nnz(S, b, idx, fa, fs, fm);
+    if (nnz == 0 || np == 0) continue;
+    double *phi = (double *)malloc(sizeof(double) * (size_t)nnz * np * 4);
+    double *dphi = phi + (size_t)nnz * np;
+    orc_eval_basis(S, b, 1, nnz, fa, fs, fm, phi, dphi);
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int i = 0; i < nnz; i++) {
+      int A = fa[i];
+      int ai = (int)(idx[i] - afp[A]);
+      for (int j = 0; j < nnz; j++) {
+        int B = fa[j];
+        if (B < A) continue;
+        int ld;
+        int64_t off = find_block(S, A, B, &ld);
+        if (off < 0) continue;
+        int bj = (int)(idx[j] - afp[B]);
+        double h = 0.0;
+        for (int p = 0; p < np; p++) {
+          double gg = 0.0;
+          for (int c = 0; c < 3; c++) gg += dphi[((size_t)c * nnz + i) * np + p] * dphi[((size_t)c * nnz + j) * np + p];
+          h += 0.5 * S->w[p0 + p] * xi[p0 + p] * gg;
+        }
+        H_values[off + (int64_t)ai * ld + bj] += h;
+      }
+    }
+    free(phi);
+  }
+  free(idx);
+  free(afp);
+}

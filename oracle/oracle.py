@@ -64,6 +64,7 @@ def _load():
         L.orc_integrate_hamiltonian_ks.argtypes = [sp, ctypes.c_int, _ip, _dp, _dp, ctypes.c_int, _dp]
         L.orc_brute_kinetic.argtypes = [sp, _dp, _dp]
         L.orc_density_hessian.argtypes = [sp, ctypes.c_int, _ip, _dp, _dp]
+        L.orc_tau_matrix.argtypes = [sp, ctypes.c_int, _ip, _dp, _dp]
         L.orc_bloch_fold.argtypes = [sp, _dp, _ip, _dp, ctypes.c_int, _dp, _dp, _dp]
         _lib = L
     return _lib
@@ -191,6 +192,14 @@ class Oracle:
         g = None if g is None else np.ascontiguousarray(g, dtype=np.float64)
         H = np.zeros(self.n_values)
         self.L.orc_integrate_hamiltonian_ks(ctypes.byref(self.sys), len(sel), _i(sel), _d(v), _d(g), int(bool(kinetic)), _d(H))
+        return H
+
+    def tau_matrix(self, xi, batches=None, H_values=None):
+        """H_values += 1/2 sum_p w xi grad phi_i . grad phi_j (meta-GGA tau matrix, reading P1c)."""
+        sel = self._sel(batches)
+        xi = np.ascontiguousarray(xi, dtype=np.float64)
+        H = np.zeros(self.n_values) if H_values is None else H_values
+        self.L.orc_tau_matrix(ctypes.byref(self.sys), len(sel), _i(sel), _d(xi), _d(H))
         return H
 
     def brute_kinetic(self, v):

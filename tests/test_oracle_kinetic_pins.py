@@ -122,3 +122,43 @@ def test_kinetic_forces_are_minus_gradient_of_kinetic_energy_to_grid_accuracy():
         xm[a, c] -= h
         fd = -(energy(xp) - energy(xm)) / (2 * h)
         assert abs(fd - F[a, c]) <= 2e-2 * scale, (a, c, fd, F[a, c])
+
+
+# --------------------------------------------------------------------------- meta-GGA tau matrix (L377, reading P1c)
+def test_tau_matrix_with_unit_xi_is_the_kinetic_matrix():
+    b = aims_synth.make_config(1, n_rad=60, n_ang=302)
+    o = Oracle(b)
+    M = bsr_to_dense(b, o.tau_matrix(np.ones(b.n_points)))
+    T = bsr_to_dense(b, o.integrate_hamiltonian_ks(np.zeros(b.n_points), kinetic=True))
+    scale = np.abs(M).max()
+    assert np.abs(M - T).max() <= 5e-3 * scale                  # integration by parts: grid accuracy
+    assert np.abs(M - M.T).max() <= 1e-14 * scale
+    GG = np.zeros_like(M)
+    for bi in range(b.n_batches):
+        idx, _, dphi = o.eval_basis(bi, want_grad=True)
+        w = b.w[b.batch_ptr[bi]:b.batch_ptr[bi + 1]]
+        for c in range(3):
+            GG[np.ix_(idx, idx)] += 0.5 * (dphi[c] * w) @ dphi[c].T
+    assert np.abs(M - GG).max() <= 1e-12 * scale                # the same sum in another order
+
+
+def test_tau_matrix_trace_identity_psd_and_additivity(toy5):
+    b, o = toy5
+    xi = aims_synth.make_xi(b)
+    assert xi.min() > 0
+    Mv = o.tau_matrix(xi)
+    M = bsr_to_dense(b, Mv)
+    Dd = bsr_to_dense(b, b.D_values)
+    tau = np.zeros(b.n_points)                                  # tau_p = 1/2 sum_ij n_ij grad phi_i . grad phi_j
+    for bi in range(b.n_batches):
+        idx, _, dphi = o.eval_basis(bi, want_grad=True)
+        Db = Dd[np.ix_(idx, idx)]
+        tau[b.batch_ptr[bi]:b.batch_ptr[bi + 1]] = 0.5 * sum(((Db @ dphi[c]) * dphi[c]).sum(0) for c in range(3))
+    lhs, rhs = float((Dd * M).sum()), float((b.w * xi * tau).sum())
+    assert abs(lhs - rhs) <= 1e-11 * max(abs(lhs), abs(rhs), 1.0)
+    assert np.linalg.eigvalsh(0.5 * (M + M.T)).min() >= -1e-12 * np.abs(M).max()
+    H = o.integrate_hamiltonian(b.v, b.g)
+    H2 = o.tau_matrix(xi, H_values=H.copy())
+    assert np.abs(H2 - (H + Mv)).max() <= 1e-13 * np.abs(H2).max()     # "added to h^uc_ij"
+    half = o.tau_matrix(xi, batches=np.arange(b.n_batches // 2)) + o.tau_matrix(xi, batches=np.arange(b.n_batches // 2, b.n_batches))
+    assert np.abs(half - Mv).max() <= 1e-13 * np.abs(Mv).max()
