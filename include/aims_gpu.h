@@ -126,6 +126,12 @@ int aims_gpu_integrate_hamiltonian(aims_gpu_ctx *ctx, int32_t b0, int32_t b1, co
 int aims_gpu_integrate_hamiltonian_ks(aims_gpu_ctx *ctx, int32_t b0, int32_t b1, const double *v, const double *g,
                                       int kinetic, double *H_values, int accumulate);
 
+/* Row f2, meta-GGA: the "tau matrix" of PAPER.md L377 ("calculated via a single DGEMM ... and added to the h^uc_ij matrix at
+ * the end of each batch"; the paper gives no formula, reading P1c):
+ *   H_values += sum over batches [b0,b1) of  1/2 sum_p w_p xi_p grad phi_i(r_p) . grad phi_j(r_p),   xi = d f_xc / d tau.
+ * Always accumulates.  DEVICE pointers: xi [n_points], H_values [n_values]. */
+int aims_gpu_add_tau_matrix(aims_gpu_ctx *ctx, int32_t b0, int32_t b1, const double *xi, double *H_values);
+
 /* Step 3 (S3a-S3d).  For every point p of batches [b0,b1):  n[p] = sum_ij phi_i D_ij phi_j,
  * grad_n[c][p] = 2 sum_ij d_c phi_i D_ij phi_j (D symmetric), i,j in nnz(B) (Eq. 3; Fig. 6b).
  * DEVICE pointers: D_values [n_values] in the pattern of aims_bsr_desc (upper blocks; the symmetric full matrix is

@@ -79,6 +79,8 @@ def load_library():
     L.aims_gpu_integrate_hamiltonian.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp, _vp, ctypes.c_int]
     L.aims_gpu_integrate_hamiltonian_ks.restype = ctypes.c_int
     L.aims_gpu_integrate_hamiltonian_ks.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp, ctypes.c_int, _vp, ctypes.c_int]
+    L.aims_gpu_add_tau_matrix.restype = ctypes.c_int
+    L.aims_gpu_add_tau_matrix.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp]
     L.aims_gpu_update_density.restype = ctypes.c_int
     L.aims_gpu_update_density.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp, _vp]
     L.aims_gpu_bloch_fold.restype = ctypes.c_int
@@ -258,6 +260,19 @@ class Context:
                     "aims_gpu_integrate_hamiltonian")
         return H
 
+    def add_tau_matrix(self, xi, H=None, b0=0, b1=None):
+        """H += 1/2 sum_p w xi grad phi_i . grad phi_j (include/aims_gpu.h: aims_gpu_add_tau_matrix); H = None starts from zero."""
+        torch = self.torch
+        b0, b1 = self._range(b0, b1)
+        xi = self._dev(xi, torch.float64)
+        if xi.numel() != self.n_points:
+            raise AimsError("xi must have n_points entries")
+        if H is None:
+            with torch.cuda.stream(self.stream):
+                H = torch.zeros(self.n_values, dtype=torch.float64, device=self.device)
+        self._check(self.L.aims_gpu_add_tau_matrix(self.h, b0, b1, _ptr(xi), _ptr(H)), "aims_gpu_add_tau_matrix")
+        return H
+
     def update_density(self, D, want_grad=False, n=None, grad_n=None, b0=0, b1=None):
         torch = self.torch
         b0, b1 = self._range(b0, b1)
@@ -375,6 +390,10 @@ def aims_gpu_integrate_hamiltonian(ctx, v, g=None, H=None, b0=0, b1=None, accumu
 
 def aims_gpu_integrate_hamiltonian_ks(ctx, v, g=None, kinetic=True, H=None, b0=0, b1=None, accumulate=False):
     return ctx.integrate_hamiltonian(v, g, H, b0, b1, accumulate, kinetic=kinetic)
+
+
+def aims_gpu_add_tau_matrix(ctx, xi, H=None, b0=0, b1=None):
+    return ctx.add_tau_matrix(xi, H, b0, b1)
 
 
 def aims_gpu_update_density(ctx, D, want_grad=False, n=None, grad_n=None, b0=0, b1=None):

@@ -386,7 +386,7 @@ int aims_gpu_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_gri
     if ((size_t)esm + 4096 > (size_t)prop.sharedMemPerBlockOptin) return fail(c, AIMS_ERR_UNSUPPORTED, "nnz(B) too large for the evaluation kernel's shared memory");
 #define EV_ATTR(M, LY) CU_TRY(c, cudaFuncSetAttribute(k_eval<M, LY>, cudaFuncAttributeMaxDynamicSharedMemorySize, esm));
     EV_ATTR(kEvalPhi, kLayApi) EV_ATTR(kEvalPhiGrad, kLayApi) EV_ATTR(kEvalHLda, kLayH) EV_ATTR(kEvalHGga, kLayH)
-    EV_ATTR(kEvalHKinLda, kLayH) EV_ATTR(kEvalHKinGga, kLayH)
+    EV_ATTR(kEvalHKinLda, kLayH) EV_ATTR(kEvalHKinGga, kLayH) EV_ATTR(kEvalTau, kLayH)
     EV_ATTR(kEvalHess, kLayD)
     EV_ATTR(kEvalPhi, kLayD) EV_ATTR(kEvalPhiGrad, kLayD) EV_ATTR(kEvalForceLda, kLayD) EV_ATTR(kEvalForceGga, kLayD)
 #undef EV_ATTR
@@ -520,10 +520,37 @@ static int run_hamiltonian(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double
     else launch_eval<kEvalHLda, kLayH>(c, E, bs, be);
     const long long nt = c->tile_off[be] - c->tile_off[bs];
     if (nt > 0) {
-      HArgs A{c->d_tiles + c->tile_off[bs], E.plane[0], E.plane[1], d_poff, poff[bs], H_values};
+      HArgs A{c->d_tiles + c->tile_off[bs], E.plane[0], E.plane[1], d_poff, poff[bs], H_values, 1};
       TimedLaunch t(c, kKindHam);
       if (syr2k) k_hamiltonian<true><<<(unsigned)nt, kHThreads, h_smem_bytes<true>(), c->stream>>>(c->S, c->L, A);
       else k_hamiltonian<false><<<(unsigned)nt, kHThreads, h_smem_bytes<false>(), c->stream>>>(c->S, c->L, A);
+    }
+    if ((rc = check_async(c))) return rc;
+    bs = be;
+  }
+  return AIMS_OK;
+}
+
+int aims_gpu_add_tau_matrix(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *xi, double *H_values) {
+  if (!range_ok(c, b0, b1)) return fail(c, AIMS_ERR_INVALID_ARG, "batch range outside [0, n_batches]");
+  if ((!xi && c->n_points) || !H_values) return fail(c, AIMS_ERR_INVALID_ARG, "NULL xi or H_values");
+  CU_TRY(c, cudaSetDevice(c->device));
+  int rc = run_cull(c, b0, b1);
+  if (rc) return rc;
+  for (int bs = b0; bs < b1;) {
+    // two planes of 3 x the 16-padded points each: [d_x Phi | d_y Phi | d_z Phi] and w xi / 2 times it
+    const int be = chunk_end(c, c->pad16_off, bs, b1, 6);
+    const long long third = (c->ws_doubles / 6) & ~63ll;
+    EvalArgs E{};
+    E.plane[0] = c->ws; E.plane[1] = c->ws + 3 * third;
+    E.pad_off = c->d_pad16_off; E.pad_base = c->pad16_off[bs]; E.point_pad = 16;
+    E.v = xi; E.n_points = c->n_points;
+    launch_eval<kEvalTau, kLayH>(c, E, bs, be);
+    const long long nt = c->tile_off[be] - c->tile_off[bs];
+    if (nt > 0) {
+      HArgs A{c->d_tiles + c->tile_off[bs], E.plane[0], E.plane[1], c->d_pad16_off, c->pad16_off[bs], H_values, 3};
+      TimedLaunch t(c, kKindHam);
+      k_hamiltonian<false><<<(unsigned)nt, kHThreads, h_smem_bytes<false>(), c->stream>>>(c->S, c->L, A);
     }
     if ((rc = check_async(c))) return rc;
     bs = be;

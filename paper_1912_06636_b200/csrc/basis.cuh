@@ -244,7 +244,10 @@ enum EvalMode {
   kEvalHKinGga = 7,
   // Hessian of the density (hessian.cuh): plane0 = Phi, planes 1..3 = d/dx_c Phi,
   // planes 4..9 = d_c d_e Phi in the order (xx, yy, zz, xy, xz, yz)
-  kEvalHess = 8
+  kEvalHess = 8,
+  // meta-GGA tau matrix (reading P1c): plane0 = [d_x Phi | d_y Phi | d_z Phi] stacked along the
+  // points (kLayH with 3 x the padded points), plane1 = w xi / 2 times plane0; E.v carries xi
+  kEvalTau = 9
 };
 __host__ __device__ constexpr int eval_planes(int mode) {
   return mode == kEvalPhi ? 1 : mode == kEvalPhiGrad ? 4 : mode == kEvalForceLda ? 5 : mode == kEvalForceGga ? 8 : mode == kEvalHess ? 10 : 2;
@@ -333,7 +336,8 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
   constexpr bool HESS = (MODE == kEvalForceGga);
   constexpr bool KIN = (MODE == kEvalHKinLda || MODE == kEvalHKinGga);
   constexpr bool FULLH = (MODE == kEvalHess);        // all six second derivatives of every function
-  constexpr bool GRAD = (MODE == kEvalPhiGrad || MODE == kEvalHGga || MODE == kEvalHKinGga || FORCE || FULLH);
+  constexpr bool TAU = (MODE == kEvalTau);
+  constexpr bool GRAD = (MODE == kEvalPhiGrad || MODE == kEvalHGga || MODE == kEvalHKinGga || FORCE || FULLH || TAU);
   constexpr int NPL = eval_planes(MODE);
   const int b = b_first + blockIdx.x;
   const int tid = threadIdx.x;
@@ -393,10 +397,11 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
 #pragma unroll
     for (int q = 1; q < NPL; q++) o[q] = E.plane[1] + 3 * off + (q - 1) * cstride;
   } else {
-    const long long off = E.pad_off[b] - E.pad_base;
+    const long long off = (E.pad_off[b] - E.pad_base) * (TAU ? 3 : 1);
 #pragma unroll
     for (int q = 0; q < NPL; q++) o[q] = E.plane[q] + off;
   }
+  const int cstr = TAU ? npx * nnz8 : 0;          // kEvalTau: distance between the d_x, d_y, d_z parts of a plane
 
   for (int p = tid; p < npx; p += 256) {
     // the thread's point base inside the batch's plane; element (row, p) at pbase + eval_row_off(row)
@@ -407,7 +412,10 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
 #define AIMS_EZERO(idx)                                                  \
   {                                                                      \
     const int o_ = (idx);                                                \
-    _Pragma("unroll") for (int q_ = 0; q_ < NPL; q_++) op[q_][o_] = 0.0; \
+    _Pragma("unroll") for (int q_ = 0; q_ < NPL; q_++) {                 \
+      op[q_][o_] = 0.0;                                                  \
+      if (TAU) { op[q_][o_ + cstr] = 0.0; op[q_][o_ + 2 * cstr] = 0.0; } \
+    }                                                                    \
   }
     if (p >= np) {  // zero padding columns (k4 layouts only)
       for (int r = 0; r < nrows; r++) AIMS_EZERO(eval_row_off<LAYOUT>(r, np, np8))
@@ -417,6 +425,7 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
     const double x = S.px[p0 + p], y = S.py[p0 + p], z = S.pz[p0 + p];
     double wv = 0.0, wgx = 0.0, wgy = 0.0, wgz = 0.0, w = 0.0;
     if (MODE == kEvalHLda) wv = S.w[p0 + p] * E.v[p0 + p];
+    if (TAU) wv = 0.5 * S.w[p0 + p] * E.v[p0 + p];             // w xi / 2
     if (MODE == kEvalHKinLda) { w = S.w[p0 + p]; wv = 0.5 * w * E.v[p0 + p]; }
     if (MODE == kEvalHGga || MODE == kEvalHKinGga) {
       w = S.w[p0 + p];
@@ -503,7 +512,7 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
           if (m < nm) {
             const double phi = R * Y[m];
             const int oi = ro + m * mstep + (m >= wrap ? jump : 0);
-            op[0][oi] = phi;
+            if (!TAU) op[0][oi] = phi;
             if (MODE == kEvalHLda) op[1 % NPL][oi] = wv * phi;
             if (MODE == kEvalHKinLda) op[1 % NPL][oi] = wv * phi + qlap * Y[m];
             if (GRAD) {
@@ -519,6 +528,10 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
                 op[7 % NPL][oi] = ax * uy + hB * ux * gy[m] + hC * s2[FULLH ? 3 : 0][FULLH ? m : 0];
                 op[8 % NPL][oi] = ax * uz + hB * ux * gz[m] + hC * s2[FULLH ? 4 : 0][FULLH ? m : 0];
                 op[9 % NPL][oi] = ay * uz + hB * uy * gz[m] + hC * s2[FULLH ? 5 : 0][FULLH ? m : 0];
+              }
+              if (TAU) {
+                op[0][oi] = ex; op[0][oi + cstr] = ey; op[0][oi + 2 * cstr] = ez;
+                op[1 % NPL][oi] = wv * ex; op[1 % NPL][oi + cstr] = wv * ey; op[1 % NPL][oi + 2 * cstr] = wv * ez;
               }
               if (MODE == kEvalHGga) op[1 % NPL][oi] = wv * phi + (wgx * ex + wgy * ey + wgz * ez);
               if (MODE == kEvalHKinGga) op[1 % NPL][oi] = wv * phi + (wgx * ex + wgy * ey + wgz * ez) + qlap * Y[m];

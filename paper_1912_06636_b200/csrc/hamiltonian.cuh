@@ -39,6 +39,7 @@ struct HArgs {
   const long long *pad_off; // [n_batches+1] prefix of pad8(nnz)*round_up(np, GGA ? 8 : 16) (doubles)
   long long pad_base;
   double *H;                // block-sparse values
+  int pmul;                 // planes hold pmul x the (padded) points of a batch: 1, or 3 for the stacked gradient planes of the tau matrix
 };
 
 // first row of block k when nsub sub-tiles of 8 rows are cut into nblk blocks (sizes differ by at most one sub-tile)
@@ -176,8 +177,8 @@ __global__ void __launch_bounds__(kHThreads, 2) k_hamiltonian(DevSys S, BatchLis
   // with zero columns to a multiple of 16 points, so that both run four product steps per barrier round trip
   constexpr int NG = h_stage_groups<GGA>();
   const int npp = round_up((int)(S.batch_ptr[b + 1] - S.batch_ptr[b]), 4 * NG);
-  const int nchunk = npp / (4 * NG);
-  const long long boff_plane = A.pad_off[b] - A.pad_base;
+  const int nchunk = A.pmul * (npp / (4 * NG));
+  const long long boff_plane = (A.pad_off[b] - A.pad_base) * A.pmul;
   const long long fo = L.fn_off[b], ao = L.act_off[b];
 
   const int bI0 = tile.ti * kHIB, bI1 = min(bI0 + kHIB, nblk);

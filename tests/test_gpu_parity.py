@@ -130,6 +130,24 @@ def test_hamiltonian_with_kinetic_term_matches_oracle(case, mode):
         assert np.array_equal(H, ctx.integrate_hamiltonian(v, g).cpu().numpy()) or _rel_fro(H, ctx.integrate_hamiltonian(v, g).cpu().numpy()) <= 1e-13
 
 
+def test_tau_matrix_matches_oracle_and_is_added_to_H(case):
+    """Row f2, meta-GGA tau matrix (reading P1c): aims_gpu_add_tau_matrix."""
+    name, bun, orc, ctx = case
+    xi = aims_synth.make_xi(bun)
+    M = ctx.add_tau_matrix(xi).cpu().numpy()
+    ctx.synchronize()
+    ref = orc.tau_matrix(xi)
+    assert _rel_fro(M, ref) <= TOL_H
+    assert np.all(M[bsr_pad_mask(bun)] == 0.0)
+    H = ctx.integrate_hamiltonian(bun.v, bun.g, kinetic=True)
+    mid = bun.n_batches // 2
+    ctx.add_tau_matrix(xi, H=H, b0=0, b1=mid)
+    ctx.add_tau_matrix(xi, H=H, b0=mid)
+    ctx.synchronize()
+    full = orc.tau_matrix(xi, H_values=orc.integrate_hamiltonian_ks(bun.v, bun.g, kinetic=True))
+    assert _rel_fro(H.cpu().numpy(), full) <= TOL_H
+
+
 def test_hamiltonian_accumulate_and_subranges(case):
     name, bun, orc, ctx = case
     import torch
