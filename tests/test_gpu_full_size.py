@@ -132,3 +132,33 @@ def test_full_size_properties_of_whole_grid_outputs(full):
         gn = gn.cpu().numpy()
         magg = float(np.abs(wgt * bun.D_values * (Hfull - Hl)).sum())
         assert abs((bun.w * (bun.g * gn).sum(0)).sum() - tr(Hfull - Hl)) <= 1e-11 * max(magg, 1e-300)
+
+
+def test_full_size_widened_rows_on_sampled_batches(full):
+    """Kinetic term + tau matrix, Pulay forces and the density Hessian at full size: sampled batches against the oracle
+    (through [b, b+1) for the sums H and F, whole-grid call for the per-point Hessian).  Config 5 and config 3 only, and a
+    subset of the sample, to bound the oracle's time."""
+    import torch
+    from aims_synth import make_q_values, make_xi
+    name, bun, orc, ctx, gga, sel = full
+    if name not in ("cfg5_full_gga", "cfg3_full_gga"):
+        pytest.skip("widened rows are sampled on configs 3 and 5")
+    sub = sel[:: max(1, len(sel) // 8)][:8]
+    vd, gd = torch.as_tensor(bun.v).cuda(), torch.as_tensor(bun.g).cuda()
+    xi = make_xi(bun)
+    Q = make_q_values(bun)
+    H = torch.zeros(bun.n_values, dtype=torch.float64, device="cuda")
+    F = torch.zeros((bun.n_atoms, 3), dtype=torch.float64, device="cuda")
+    for b in sub:
+        ctx.integrate_hamiltonian(vd, gd, H=H, b0=int(b), b1=int(b) + 1, accumulate=True, kinetic=True)
+        ctx.add_tau_matrix(xi, H=H, b0=int(b), b1=int(b) + 1)
+        ctx.pulay_forces(vd, bun.D_values, g=gd, Q=Q, F=F, b0=int(b), b1=int(b) + 1, accumulate=True, kinetic=True)
+    Hn = ctx.density_hessian(bun.D_values)                          # whole grid, as bench.py --path hessian launches it
+    ctx.synchronize()
+    ref = orc.tau_matrix(xi, batches=sub, H_values=orc.integrate_hamiltonian_ks(bun.v, bun.g, kinetic=True, batches=sub))
+    assert _rel_fro(H.cpu().numpy(), ref) <= TOL_H
+    F_ref = orc.pulay_forces(bun.v, bun.D_values, g=bun.g, Q_values=Q, batches=sub, kinetic=True)
+    assert _rel_max(F.cpu().numpy(), F_ref) <= TOL_N
+    Hn_ref = orc.density_hessian(bun.D_values, batches=sub[:3])
+    idx = np.concatenate([np.arange(bun.batch_ptr[b], bun.batch_ptr[b + 1]) for b in sub[:3]])
+    assert _rel_max(Hn.cpu().numpy()[:, idx], Hn_ref[:, idx]) <= TOL_N
