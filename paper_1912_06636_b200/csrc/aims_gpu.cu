@@ -25,6 +25,8 @@ static_assert(kMaxActive == AIMS_MAX_ACTIVE_ATOMS, "header and kernels disagree"
 
 struct aims_gpu_ctx {
   int device = 0;
+  int sm_count = 148;
+  size_t smem_optin = 0;       // largest opt-in dynamic shared memory per CTA
   cudaStream_t stream = nullptr;
   std::string err;
   int64_t launches = 0;
@@ -173,6 +175,8 @@ int aims_gpu_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_gri
   cudaDeviceProp prop;
   CU_TRY(c, cudaGetDeviceProperties(&prop, device));
   if (prop.major != 10) return fail(c, AIMS_ERR_UNSUPPORTED, "this library is built for sm_100a (B200) only");
+  c->sm_count = prop.multiProcessorCount;
+  c->smem_optin = (size_t)prop.sharedMemPerBlockOptin;
 
   // ---- validate and derive host-side tables
   const int na = B->n_atoms, nsp = B->n_species, nsh = B->n_shells;
@@ -447,10 +451,20 @@ int chunk_end(const aims_gpu_ctx *c, const std::vector<long long> &off, int bs, 
 // Launch order of the density items of batches [bs, be): heaviest (largest nnz) first, so that the last CTAs of a launch
 // are the cheapest ones (a CTA's cost varies by 50x over a slab).  Built once per distinct range and kept on the device.
 int density_order(aims_gpu_ctx *c, int bs, int be, const int **out) {
+  const long long i0 = c->item_off[bs], i1 = c->item_off[be];
+  if (i1 - i0 <= 2ll * c->sm_count) { *out = nullptr; return AIMS_OK; }   // fewer items than two waves: any order
   auto key = std::make_pair(bs, be);
   auto it = c->item_order.find(key);
   if (it != c->item_order.end()) { *out = it->second; return AIMS_OK; }
-  const long long i0 = c->item_off[bs], i1 = c->item_off[be];
+  if (c->item_order.size() >= 64) {
+    // a caller walking over many distinct ranges: do not let the cache grow without bound
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    for (auto &kv : c->item_order) {
+      c->owned.erase(std::remove(c->owned.begin(), c->owned.end(), (void *)kv.second), c->owned.end());
+      cudaFree(kv.second);
+    }
+    c->item_order.clear();
+  }
   std::vector<int> ord((size_t)(i1 - i0));
   for (long long i = i0; i < i1; i++) ord[(size_t)(i - i0)] = (int)(i - i0);
   std::stable_sort(ord.begin(), ord.end(), [&](int a, int b) {
@@ -693,9 +707,7 @@ int aims_gpu_density_hessian(aims_gpu_ctx *c, int32_t b0, int32_t b1, const doub
   if (!D_values || (!hess_n && c->n_points)) return fail(c, AIMS_ERR_INVALID_ARG, "NULL D_values or hess_n");
   CU_TRY(c, cudaSetDevice(c->device));
   const size_t xsm = x_smem_bytes(c->max_nnz, std::max(c->max_act, 1), c->x_ptab_in_smem);
-  cudaDeviceProp prop;
-  CU_TRY(c, cudaGetDeviceProperties(&prop, c->device));
-  if (xsm > (size_t)prop.sharedMemPerBlockOptin) return fail(c, AIMS_ERR_UNSUPPORTED, "nnz(B) too large for the Hessian kernel's shared memory");
+  if (xsm > c->smem_optin) return fail(c, AIMS_ERR_UNSUPPORTED, "nnz(B) too large for the Hessian kernel's shared memory");
   int rc = run_cull(c, b0, b1);
   if (rc) return rc;
   const int npl = 10;
@@ -777,13 +789,11 @@ int aims_gpu_synchronize(aims_gpu_ctx *c) {
 int aims_gpu_fp64_peak(aims_gpu_ctx *c, double ms_target, double *tflops) {
   if (!c || !tflops) return AIMS_ERR_INVALID_ARG;
   CU_TRY(c, cudaSetDevice(c->device));
-  cudaDeviceProp prop;
-  CU_TRY(c, cudaGetDeviceProperties(&prop, c->device));
   double *out;
   int rc = dev_alloc(c, &out, 16);
   if (rc) return rc;
   const int iters = 20000;
-  const dim3 grid(prop.multiProcessorCount), block(256);
+  const dim3 grid(c->sm_count), block(256);
   cudaEvent_t e0, e1;
   CU_TRY(c, cudaEventCreate(&e0));
   CU_TRY(c, cudaEventCreate(&e1));

@@ -37,7 +37,7 @@ struct DItem { int b, p0, npt, pad; };     // points [p0, p0+npt) of batch b; p0
 
 struct DArgs {
   const DItem *items;
-  const int *order;                 // launch order: CTA x works on items[order[x]]
+  const int *order;                 // launch order: CTA x works on items[order[x]] (NULL: items[x])
   const double *P;                  // Phi plane
   const double *G[3];               // gradient planes (GRAD only)
   const long long *pad_off;         // [n_batches+1] prefix of round_up(nnz,16)*pad8(np) (density layout)
@@ -244,7 +244,7 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density(DevSys S, BatchLists L
   int *sLd = sInfo + pad8(A.max_nnz_pad);
   long long *sPtab = reinterpret_cast<long long *>(sLd + kMaxActive);
 
-  const DItem it = A.items[A.order[blockIdx.x]];
+  const DItem it = A.items[A.order ? A.order[blockIdx.x] : blockIdx.x];
   const int b = it.b;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int nnz = L.nnz[b], nact = L.n_act[b];

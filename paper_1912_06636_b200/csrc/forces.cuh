@@ -21,7 +21,7 @@ namespace aims {
 
 struct FArgs {
   const DItem *items;
-  const int *order;                 // launch order: CTA x works on items[order[x]]
+  const int *order;                 // launch order: CTA x works on items[order[x]] (NULL: items[x])
   const double *P, *Lp;             // planes Phi and L = v Phi (+ g.grad Phi), density layout
   const double *E[6];               // w d_c Phi (c = x,y,z) and, GGA only, w (Hess Phi g)_c
   const long long *pad_off;         // [n_batches+1] prefix of round_up(nnz,16)*pad8(np)
@@ -51,7 +51,7 @@ __global__ void __launch_bounds__(kDThreads, 1) k_forces(DevSys S, BatchLists L,
   int *sLd = sInfo + pad8(A.max_nnz_pad);
   long long *sPtab = reinterpret_cast<long long *>(sLd + kMaxActive);
 
-  const DItem it = A.items[A.order[blockIdx.x]];
+  const DItem it = A.items[A.order ? A.order[blockIdx.x] : blockIdx.x];
   const int b = it.b;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int nnz = L.nnz[b], nact = L.n_act[b];

@@ -20,7 +20,7 @@ namespace aims {
 
 struct XArgs {
   const DItem *items;
-  const int *order;                 // launch order: CTA x works on items[order[x]]
+  const int *order;                 // launch order: CTA x works on items[order[x]] (NULL: items[x])
   const double *PL[10];             // planes Phi, d_x, d_y, d_z Phi, then d_c d_e Phi (xx, yy, zz, xy, xz, yz); density layout
   const long long *pad_off;         // [n_batches+1] prefix of round_up(nnz,16)*pad8(np)
   long long pad_base;
@@ -93,7 +93,7 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density_hessian(DevSys S, Batc
   int *sLd = sInfo + pad8(A.max_nnz_pad);
   long long *sPtab = reinterpret_cast<long long *>(sLd + kMaxActive);
 
-  const DItem it = A.items[A.order[blockIdx.x]];
+  const DItem it = A.items[A.order ? A.order[blockIdx.x] : blockIdx.x];
   const int b = it.b;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int nnz = L.nnz[b], nact = L.n_act[b];
