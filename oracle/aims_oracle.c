@@ -946,3 +946,50 @@ void orc_tau_matrix(const orc_system *S, int n_sel, const int32_t *batches, cons
   free(idx);
   free(afp);
 }
+
+/* ====================================================================================================================
+ * Partition of unity (Eq. 21-22: the integration weight w(r) of a grid point
+ * contains the atom-centred partition function, "a modified version of the partition function proposed by Stratmann et al."
+ * cited at L190/L200 but not written out; reading P5 takes the textbook Stratmann-Scuseria-Frisch cell function):
+ *   mu_AB = (d_A - d_B) / R_AB,  x = clamp(mu / 0.64, -1, 1),  z = (35 x - 35 x^3 + 21 x^5 - 5 x^7) / 16,  s = (1 - z) / 2,
+ *   P_A(r) = prod_{B in cand(r), B != A} s(mu_AB),   w_A(r) = P_A(r) / sum_{B in cand(r)} P_B(r),
+ * cand(r) = atoms within r_part of r (the O(N) neighbour restriction of L200).  out[p] = w_{owner[p]}(xyz[p]); 0 if the owner
+ * is not a candidate.  Plain scans over all atoms, products in ascending atom order.
+ * Pins (tests/test_oracle_partition_pins.py): sum over owners = 1 at arbitrary points; 1/2 on the bisecting plane of two atoms
+ * and exactly 1 / 0 beyond mu = -+0.64; the polynomial's end values and symmetry s(mu) + s(-mu) = 1; rigid motions.
+ * ==================================================================================================================== */
+static double orc_stratmann_s(double mu) {
+  double x = mu / 0.64;
+  if (x <= -1.0) return 1.0;
+  if (x >= 1.0) return 0.0;
+  double z = (35.0 * x - 35.0 * x * x * x + 21.0 * x * x * x * x * x - 5.0 * x * x * x * x * x * x * x) / 16.0;
+  double s = 0.5 * (1.0 - z);
+  if (s < 0.0) s = 0.0;
+  if (s > 1.0) s = 1.0;
+  return s;
+}
+
+void orc_partition_weights(const orc_system *S, int64_t n, const double *xyz, const int32_t *owner, double r_part, double *out) {
+#pragma omp parallel for schedule(dynamic, 256)
+  for (int64_t p = 0; p < n; p++) {
+    const double *r = xyz + 3 * p;
+    double sum = 0.0, pown = 0.0;
+    for (int A = 0; A < S->n_atoms; A++) {
+      const double *Ra = S->atom_xyz + 3 * A;
+      double dA = sqrt((r[0] - Ra[0]) * (r[0] - Ra[0]) + (r[1] - Ra[1]) * (r[1] - Ra[1]) + (r[2] - Ra[2]) * (r[2] - Ra[2]));
+      if (dA > r_part) continue;
+      double P = 1.0;
+      for (int B = 0; B < S->n_atoms; B++) {
+        if (B == A) continue;
+        const double *Rb = S->atom_xyz + 3 * B;
+        double dB = sqrt((r[0] - Rb[0]) * (r[0] - Rb[0]) + (r[1] - Rb[1]) * (r[1] - Rb[1]) + (r[2] - Rb[2]) * (r[2] - Rb[2]));
+        if (dB > r_part) continue;
+        double Rab = sqrt((Ra[0] - Rb[0]) * (Ra[0] - Rb[0]) + (Ra[1] - Rb[1]) * (Ra[1] - Rb[1]) + (Ra[2] - Rb[2]) * (Ra[2] - Rb[2]));
+        P *= orc_stratmann_s((dA - dB) / Rab);
+      }
+      sum += P;
+      if (A == owner[p]) pown = P;
+    }
+    out[p] = sum > 0.0 ? pown / sum : 0.0;
+  }
+}

@@ -64,6 +64,7 @@ def _load():
         L.orc_integrate_hamiltonian_ks.argtypes = [sp, ctypes.c_int, _ip, _dp, _dp, ctypes.c_int, _dp]
         L.orc_brute_kinetic.argtypes = [sp, _dp, _dp]
         L.orc_density_hessian.argtypes = [sp, ctypes.c_int, _ip, _dp, _dp]
+        L.orc_partition_weights.argtypes = [sp, ctypes.c_int64, _dp, _ip, ctypes.c_double, _dp]
         L.orc_tau_matrix.argtypes = [sp, ctypes.c_int, _ip, _dp, _dp]
         L.orc_bloch_fold.argtypes = [sp, _dp, _ip, _dp, ctypes.c_int, _dp, _dp, _dp]
         _lib = L
@@ -225,6 +226,14 @@ class Oracle:
         H = np.zeros((6, self.n_points))
         self.L.orc_density_hessian(ctypes.byref(self.sys), len(sel), _i(sel), _d(D), _d(H))
         return H
+
+    def partition_weights(self, xyz, owner, r_part):
+        """w_owner(xyz) of the neighbour-restricted Stratmann partition (reading P5) over this system's atoms."""
+        xyz = np.ascontiguousarray(xyz, dtype=np.float64)
+        owner = np.ascontiguousarray(owner, dtype=np.int32)
+        out = np.zeros(len(xyz))
+        self.L.orc_partition_weights(ctypes.byref(self.sys), len(xyz), _d(xyz), _i(owner), float(r_part), _d(out))
+        return out
 
     def bloch_fold(self, H_values, atom_home, atom_T, n_home, kpt):
         """Complex dense [n_hb][n_hb] matrix h_ij(k) = sum_IJ e^{ik.(T_J - T_I)} h^uc_IJ (Eq. 7, 11, 12)."""
