@@ -167,6 +167,17 @@ int aims_gpu_pulay_forces(aims_gpu_ctx *ctx, int32_t b0, int32_t b1, const doubl
 int aims_gpu_pulay_forces_ks(aims_gpu_ctx *ctx, int32_t b0, int32_t b1, const double *v, const double *g, int kinetic,
                              const double *D_values, const double *Q_values, double *F, int accumulate);
 
+/* Row f4 of SURVEY.md 8(f): the partition-of-unity factor of the integration weights w(r) (Eq. 21-22; the
+ * paper cites "a modified version of the partition function proposed by Stratmann et al." without writing it out; DESIGN.md
+ * reading P5 takes the textbook Stratmann-Scuseria-Frisch cell function with a = 0.64, restricted to the atoms within r_part
+ * of the point):  w_part[p] = P_owner(r_p) / sum_{A in cand(r_p)} P_A(r_p),  P_A = prod_{B in cand, B != A} s(mu_AB),
+ * mu_AB = (|r-R_A| - |r-R_B|) / |R_A-R_B|, cand(r) = atoms with sqrt((dx*dx + dy*dy) + dz*dz) <= r_part in separately rounded IEEE
+ * operations (a discrete decision, as in reading P6); 0 if the owner is not a candidate.  The atoms are
+ * the context's.  DEVICE pointers: xyz [n][3], owner [n] (atom index of the point's grid), w_part [n] (output).  The caller
+ * multiplies with the radial and angular quadrature weights to obtain aims_grid_desc.w. */
+int aims_gpu_partition_weights(aims_gpu_ctx *ctx, int64_t n, const double *xyz, const int32_t *owner, double r_part,
+                               double *w_part);
+
 /* Row f3 of SURVEY.md 8(f): periodic boundary conditions.  The real-space matrix h^uc of Eq. 12 runs over
  * the N_rs functions of the cell atoms AND their periodic images that reach into the cell; the caller passes all of them as
  * atoms (the cell's own atoms first) with the grid points mapped back into the cell at T = 0 (L113-115), and

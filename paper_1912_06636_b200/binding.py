@@ -83,6 +83,8 @@ def load_library():
     L.aims_gpu_add_tau_matrix.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp]
     L.aims_gpu_update_density.restype = ctypes.c_int
     L.aims_gpu_update_density.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp, _vp]
+    L.aims_gpu_partition_weights.restype = ctypes.c_int
+    L.aims_gpu_partition_weights.argtypes = [cp, ctypes.c_int64, _vp, _vp, ctypes.c_double, _vp]
     L.aims_gpu_bloch_fold.restype = ctypes.c_int
     L.aims_gpu_bloch_fold.argtypes = [cp, _vp, _ip, _dp, ctypes.c_int32, _dp, _vp, _vp, ctypes.c_int]
     L.aims_gpu_density_hessian.restype = ctypes.c_int
@@ -288,6 +290,19 @@ class Context:
                     "aims_gpu_update_density")
         return n, (grad_n if want_grad else None)
 
+    def partition_weights(self, xyz, owner, r_part):
+        """w_owner(xyz) of the Stratmann partition over the context's atoms (include/aims_gpu.h: aims_gpu_partition_weights)."""
+        torch = self.torch
+        xyz = self._dev(xyz, torch.float64).reshape(-1, 3).contiguous()
+        owner = self._dev(owner, torch.int32)
+        if owner.numel() != xyz.shape[0]:
+            raise AimsError("owner must have one entry per point")
+        with torch.cuda.stream(self.stream):
+            out = torch.empty(xyz.shape[0], dtype=torch.float64, device=self.device)
+        self._check(self.L.aims_gpu_partition_weights(self.h, int(xyz.shape[0]), _ptr(xyz), _ptr(owner), float(r_part), _ptr(out)),
+                    "aims_gpu_partition_weights")
+        return out
+
     def bloch_fold(self, H, atom_home, atom_T, n_home, kpt, n_home_basis):
         """Complex device tensor [n_hb][n_hb]: Bloch sums of a real-space matrix (include/aims_gpu.h: aims_gpu_bloch_fold)."""
         torch = self.torch
@@ -398,6 +413,10 @@ def aims_gpu_add_tau_matrix(ctx, xi, H=None, b0=0, b1=None):
 
 def aims_gpu_update_density(ctx, D, want_grad=False, n=None, grad_n=None, b0=0, b1=None):
     return ctx.update_density(D, want_grad, n, grad_n, b0, b1)
+
+
+def aims_gpu_partition_weights(ctx, xyz, owner, r_part):
+    return ctx.partition_weights(xyz, owner, r_part)
 
 
 def aims_gpu_bloch_fold(ctx, H, atom_home, atom_T, n_home, kpt, n_home_basis):

@@ -6,7 +6,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "csrc", "aims_gpu.cu")
 LIB = os.path.join(HERE, "libaims_gpu.so")
-DEPS = [os.path.join(HERE, "csrc", f) for f in ("aims_gpu.cu", "common.cuh", "basis.cuh", "hamiltonian.cuh", "density.cuh", "forces.cuh", "hessian.cuh", "bloch.cuh")]
+DEPS = [os.path.join(HERE, "csrc", f) for f in ("aims_gpu.cu", "common.cuh", "basis.cuh", "hamiltonian.cuh", "density.cuh", "forces.cuh", "hessian.cuh", "bloch.cuh", "partition.cuh")]
 DEPS.append(os.path.join(os.path.dirname(HERE), "include", "aims_gpu.h"))
 
 

@@ -17,6 +17,7 @@
 #include "density.cuh"
 #include "forces.cuh"
 #include "hessian.cuh"
+#include "partition.cuh"
 #include "hamiltonian.cuh"
 
 using namespace aims;
@@ -655,6 +656,18 @@ static int run_forces(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, 
     bs = be;
   }
   return AIMS_OK;
+}
+
+int aims_gpu_partition_weights(aims_gpu_ctx *c, int64_t n, const double *xyz, const int32_t *owner, double r_part,
+                               double *w_part) {
+  if (!c || n < 0 || (n && (!xyz || !owner || !w_part)) || !(r_part > 0)) return fail(c, AIMS_ERR_INVALID_ARG, "NULL array, n < 0 or r_part <= 0");
+  CU_TRY(c, cudaSetDevice(c->device));
+  if (n) {
+    TimedLaunch t(c, kKindOther);
+    k_partition_weights<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(c->S.n_atoms, c->S.atom_xyz, (long long)n, xyz, owner,
+                                                                          r_part, w_part);
+  }
+  return check_async(c);
 }
 
 int aims_gpu_bloch_fold(aims_gpu_ctx *c, const double *H_values, const int32_t *atom_home, const double *atom_T,
