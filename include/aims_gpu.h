@@ -220,6 +220,13 @@ int64_t aims_gpu_launch_count(const aims_gpu_ctx *ctx);
  * Used by bench.py as the measured FP64 roofline denominator. */
 int aims_gpu_fp64_peak(aims_gpu_ctx *ctx, double ms_target, double *tflops);
 
+/* DMMA operand-pattern probe behind the K-loop design of the contraction kernels: warps_per_sm warps
+ * per SM (1..16) each run 16 DMMA.8x8x4 per step on a 32x32 accumulator block with
+ *   variant 1: operands in registers;  2: the step's 8 fragments loaded from shared memory, then its DMMAs;
+ *   variant 3: the loads of the next step issued before the DMMAs of the current one.
+ * Returns the achieved TFLOP/s in *tflops (HOST output).  Diagnostic only. */
+int aims_gpu_dmma_probe(aims_gpu_ctx *ctx, int variant, int warps_per_sm, double *tflops);
+
 #ifdef __cplusplus
 }
 #endif

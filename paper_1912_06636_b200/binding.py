@@ -105,6 +105,8 @@ def load_library():
     L.aims_gpu_stats.argtypes = [cp, _lp, _ip, _ip, _dp, _dp, _dp]
     L.aims_gpu_launch_count.restype = ctypes.c_int64
     L.aims_gpu_launch_count.argtypes = [cp]
+    L.aims_gpu_dmma_probe.restype = ctypes.c_int
+    L.aims_gpu_dmma_probe.argtypes = [cp, ctypes.c_int, ctypes.c_int, _dp]
     L.aims_gpu_fp64_peak.restype = ctypes.c_int
     L.aims_gpu_fp64_peak.argtypes = [cp, ctypes.c_double, _dp]
     _lib = L
@@ -208,6 +210,11 @@ class Context:
                                           ctypes.byref(f2), ctypes.byref(f3)), "aims_gpu_stats")
         return dict(sum_nnz=s.value, max_nnz=m.value, max_active_atoms=a.value, flops_h_lda=f1.value,
                     flops_h_gga=f2.value, flops_density=f3.value)
+
+    def dmma_probe(self, variant, warps_per_sm):
+        t = ctypes.c_double()
+        self._check(self.L.aims_gpu_dmma_probe(self.h, int(variant), int(warps_per_sm), ctypes.byref(t)), "aims_gpu_dmma_probe")
+        return t.value
 
     def fp64_peak(self, ms_target=200.0):
         t = ctypes.c_double()

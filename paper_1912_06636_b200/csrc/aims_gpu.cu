@@ -137,6 +137,73 @@ __global__ void k_fp64_peak(double *out, int iters, double a, double b) {
   if (s == 12345.678) out[0] = s;
 }
 
+// DMMA operand-pattern probe (aims_gpu_dmma_probe): one warp works on a 32x32 accumulator block, 16 DMMAs per step.
+//   V = 1: operands stay in registers (4x4 outer product);  V = 2: the 8 fragments of a step are loaded from shared memory,
+//   then its 16 DMMAs are issued ("load-then-compute");  V = 3: the loads of step t+1 are issued before the DMMAs of step t.
+template <int V>
+__global__ void __launch_bounds__(512, 1) k_dmma_probe(double *out, int iters, double a0, double b0) {
+  __shared__ double sm[4096];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int i = threadIdx.x; i < 4096; i += blockDim.x) sm[i] = 1e-9 * i;
+  __syncthreads();
+  double acc[4][4][2];
+#pragma unroll
+  for (int a = 0; a < 4; a++)
+#pragma unroll
+    for (int c = 0; c < 4; c++) { acc[a][c][0] = a + lane; acc[a][c][1] = c; }
+  double fa[4], fb[4];
+#pragma unroll
+  for (int a = 0; a < 4; a++) { fa[a] = a0 + a * 1e-3; fb[a] = b0 + a * 1e-4; }
+  const double *tA = sm + lane + (warp & 3) * 512, *tB = sm + 2048 + lane + (warp & 3) * 512;
+  if (V == 1) {
+    for (int it = 0; it < iters; it++) {
+#pragma unroll
+      for (int a = 0; a < 4; a++)
+#pragma unroll
+        for (int c = 0; c < 4; c++) dmma8x8x4(acc[a][c][0], acc[a][c][1], fa[a], fb[c]);
+    }
+  } else if (V == 2) {
+#pragma unroll 1
+    for (int it = 0; it < iters; it++) {
+      const int o = (it & 3) * 128;
+#pragma unroll
+      for (int a = 0; a < 4; a++) fa[a] = tA[o + a * 32];
+#pragma unroll
+      for (int c = 0; c < 4; c++) fb[c] = tB[o + c * 32];
+#pragma unroll
+      for (int a = 0; a < 4; a++)
+#pragma unroll
+        for (int c = 0; c < 4; c++) dmma8x8x4(acc[a][c][0], acc[a][c][1], fa[a], fb[c]);
+    }
+  } else {
+    double na[4], nb[4];
+#pragma unroll
+    for (int a = 0; a < 4; a++) { fa[a] = tA[a * 32]; fb[a] = tB[a * 32]; }
+#pragma unroll 1
+    for (int it = 0; it < iters; it += 2) {
+      const int o = ((it + 1) & 3) * 128, o2 = ((it + 2) & 3) * 128;
+#pragma unroll
+      for (int a = 0; a < 4; a++) { na[a] = tA[o + a * 32]; nb[a] = tB[o + a * 32]; }
+#pragma unroll
+      for (int a = 0; a < 4; a++)
+#pragma unroll
+        for (int c = 0; c < 4; c++) dmma8x8x4(acc[a][c][0], acc[a][c][1], fa[a], fb[c]);
+#pragma unroll
+      for (int a = 0; a < 4; a++) { fa[a] = tA[o2 + a * 32]; fb[a] = tB[o2 + a * 32]; }
+#pragma unroll
+      for (int a = 0; a < 4; a++)
+#pragma unroll
+        for (int c = 0; c < 4; c++) dmma8x8x4(acc[a][c][0], acc[a][c][1], na[a], nb[c]);
+    }
+  }
+  double s = 0;
+#pragma unroll
+  for (int a = 0; a < 4; a++)
+#pragma unroll
+    for (int c = 0; c < 4; c++) s += acc[a][c][0] + acc[a][c][1];
+  if (s == 12345.678) out[0] = s;
+}
+
 bool range_ok(const aims_gpu_ctx *c, int b0, int b1) { return c && b0 >= 0 && b1 >= b0 && b1 <= c->n_batches; }
 
 }  // namespace
@@ -797,6 +864,32 @@ int aims_gpu_synchronize(aims_gpu_ctx *c) {
     return AIMS_ERR_UNSUPPORTED;
   }
   return AIMS_OK;
+}
+
+int aims_gpu_dmma_probe(aims_gpu_ctx *c, int variant, int warps_per_sm, double *tflops) {
+  if (!c || !tflops || variant < 1 || variant > 3 || warps_per_sm < 1 || warps_per_sm > 16) return fail(c, AIMS_ERR_INVALID_ARG, "variant 1..3, warps_per_sm 1..16");
+  CU_TRY(c, cudaSetDevice(c->device));
+  double *out;
+  int rc = dev_alloc(c, &out, 16);
+  if (rc) return rc;
+  const int iters = 40000, threads = 32 * warps_per_sm;
+  cudaEvent_t e0, e1;
+  CU_TRY(c, cudaEventCreate(&e0));
+  CU_TRY(c, cudaEventCreate(&e1));
+  for (int rep = 0; rep < 2; rep++) {          // the first launch warms up
+    if (rep == 1) CU_TRY(c, cudaEventRecord(e0, c->stream));
+    if (variant == 1) k_dmma_probe<1><<<c->sm_count, threads, 0, c->stream>>>(out, iters, 1.0000001, 1e-9);
+    else if (variant == 2) k_dmma_probe<2><<<c->sm_count, threads, 0, c->stream>>>(out, iters, 1.0000001, 1e-9);
+    else k_dmma_probe<3><<<c->sm_count, threads, 0, c->stream>>>(out, iters, 1.0000001, 1e-9);
+    c->launches++;
+  }
+  CU_TRY(c, cudaEventRecord(e1, c->stream));
+  CU_TRY(c, cudaEventSynchronize(e1));
+  float ms = 0;
+  CU_TRY(c, cudaEventElapsedTime(&ms, e0, e1));
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  *tflops = 2.0 * 256 * 16 * (double)iters * c->sm_count * warps_per_sm / (ms * 1e-3) * 1e-12;
+  return check_async(c);
 }
 
 int aims_gpu_fp64_peak(aims_gpu_ctx *c, double ms_target, double *tflops) {

@@ -152,3 +152,16 @@ def test_error_codes():
     ctx = _ctx(crowd)                                                     # 64 <= 96: still supported
     assert ctx.stats()["max_active_atoms"] == 64
     ctx.close()
+
+
+def test_diagnostic_probes_report_plausible_fp64_throughput():
+    bun = aims_synth.make_config(1, max_batch=64)
+    ctx = _ctx(bun)
+    peak = ctx.fp64_peak(50.0)
+    assert 30.0 < peak < 40.0                                            # B200 FP64 tensor pipe: 37.2 TFLOP/s
+    t = ctx.dmma_probe(3, 16)
+    assert 0.8 * peak < t <= 1.02 * peak
+    import paper_1912_06636_b200 as aims
+    with pytest.raises(aims.AimsError):
+        ctx.dmma_probe(7, 16)
+    ctx.close()
