@@ -165,3 +165,30 @@ def test_diagnostic_probes_report_plausible_fp64_throughput():
     with pytest.raises(aims.AimsError):
         ctx.dmma_probe(7, 16)
     ctx.close()
+
+
+def test_ninety_active_atoms_per_batch_uses_the_global_pair_table():
+    """90 atoms squeezed into ~1 A: every batch sees all of them (close to AIMS_MAX_ACTIVE_ATOMS = 96), nnz(B) ~ 2,000, and
+    the batch's atom-pair offset table (90^2 entries) no longer fits the contraction kernels' shared memory, so the
+    kernels read it from global memory -- a path the ordinary configurations never take."""
+    base = aims_synth.make_config(4, n_rad=4, n_ang=6, max_batch=100, keep_atoms=90)
+    bun = copy.copy(base)
+    bun.atom_xyz = np.ascontiguousarray(base.atom_xyz * 0.04)
+    bun.xyz = np.ascontiguousarray(base.xyz * 0.04)          # points follow their atoms; weights, fields and D unchanged
+    ctx = _ctx(bun)
+    st = ctx.stats()
+    assert st["max_active_atoms"] == 90 and st["max_nnz"] > 1800
+    orc = Oracle(bun)
+    rel = lambda a, r: np.abs(a - r).max() / max(np.abs(r).max(), 1e-300)    # noqa: E731
+    H = ctx.integrate_hamiltonian(bun.v, bun.g).cpu().numpy()
+    ref = orc.integrate_hamiltonian(bun.v, bun.g)
+    assert np.linalg.norm(H - ref) <= 1e-11 * np.linalg.norm(ref)
+    n, gn = ctx.update_density(bun.D_values, want_grad=True)
+    n_ref, gn_ref = orc.update_density(bun.D_values, want_grad=True)
+    assert rel(n.cpu().numpy(), n_ref) <= 1e-11 and rel(gn.cpu().numpy(), gn_ref) <= 1e-11
+    Q = make_q_values(bun)
+    F = ctx.pulay_forces(bun.v, bun.D_values, g=bun.g, Q=Q).cpu().numpy()
+    assert rel(F, orc.pulay_forces(bun.v, bun.D_values, g=bun.g, Q_values=Q)) <= 1e-11
+    Hn = ctx.density_hessian(bun.D_values).cpu().numpy()
+    assert rel(Hn, orc.density_hessian(bun.D_values)) <= 1e-11
+    ctx.close()
