@@ -53,6 +53,7 @@ struct aims_gpu_ctx {
   std::map<std::pair<int, int>, int *> item_order;             // (bs, be) -> device permutation, heaviest item first
 
   double *ws = nullptr;      // Phi-plane workspace
+  double *probe_out = nullptr;
   long long ws_doubles = 0;
 
   // optional per-kernel timing (CUDA events on the context stream around every launch)
@@ -869,9 +870,8 @@ int aims_gpu_synchronize(aims_gpu_ctx *c) {
 int aims_gpu_dmma_probe(aims_gpu_ctx *c, int variant, int warps_per_sm, double *tflops) {
   if (!c || !tflops || variant < 1 || variant > 3 || warps_per_sm < 1 || warps_per_sm > 16) return fail(c, AIMS_ERR_INVALID_ARG, "variant 1..3, warps_per_sm 1..16");
   CU_TRY(c, cudaSetDevice(c->device));
-  double *out;
-  int rc = dev_alloc(c, &out, 16);
-  if (rc) return rc;
+  if (!c->probe_out) { int rc = dev_alloc(c, &c->probe_out, 16); if (rc) return rc; }   // scratch of the probes, allocated once
+  double *out = c->probe_out;
   const int iters = 40000, threads = 32 * warps_per_sm;
   cudaEvent_t e0, e1;
   CU_TRY(c, cudaEventCreate(&e0));
@@ -895,9 +895,8 @@ int aims_gpu_dmma_probe(aims_gpu_ctx *c, int variant, int warps_per_sm, double *
 int aims_gpu_fp64_peak(aims_gpu_ctx *c, double ms_target, double *tflops) {
   if (!c || !tflops) return AIMS_ERR_INVALID_ARG;
   CU_TRY(c, cudaSetDevice(c->device));
-  double *out;
-  int rc = dev_alloc(c, &out, 16);
-  if (rc) return rc;
+  if (!c->probe_out) { int rc = dev_alloc(c, &c->probe_out, 16); if (rc) return rc; }   // scratch of the probes, allocated once
+  double *out = c->probe_out;
   const int iters = 20000;
   const dim3 grid(c->sm_count), block(256);
   cudaEvent_t e0, e1;
