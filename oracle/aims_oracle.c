@@ -19,6 +19,9 @@
  *       density matrix ... to the dense-but-smaller n_ij"), computed as temp = n_ij phi, n = temp . phi
  *       (Fig. 6b); grad n = 2 sum_ij grad phi_i n_ij phi_j for symmetric n_ij (L67, L93-95).
  *   O5  Pulay forces F_at (Eq. 16 and Eq. 18) for the reduced h_KS; see the block at the end of this file.
+ *   O6+ (blocks further down, each with its own header and pins): kinetic term of h_KS and the meta-GGA tau matrix
+ *       (Eq. 26, Fig. 6a), Hessian of the density (L93-95), Bloch sums for periodic systems (Eq. 7, 11, 12), the
+ *       Stratmann partition of unity (Eq. 21-22, reading P5).
  *
  * Pins (tests/test_oracle_pins.py): Y_lm vs scipy and orthonormality by exact product quadrature; spline vs
  * scipy CubicSpline; grad phi vs finite differences; Gaussian overlap closed form; S symmetric PSD;
