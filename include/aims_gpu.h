@@ -9,15 +9,25 @@
  * Every step runs in hand-written sm_100a kernels; there is no CPU fallback and no other backend.
  *
  * Conventions
- *  - All functions return AIMS_OK (0) or a negative aims_status; they never throw, exit or print.
+ *  - All functions return AIMS_OK (0) or a negative aims_status; they never throw (every entry point catches C++
+ *    exceptions of its host-side bookkeeping: std::bad_alloc -> AIMS_ERR_NOMEM), exit or print.
  *  - HOST pointers are read during the call that receives them and may be freed afterwards.
  *    DEVICE pointers must be valid on the context's device, 16-byte aligned, and are owned by the caller.
  *  - Work is enqueued on the stream given at creation.  Outputs are valid once the caller has synchronised that
  *    stream.  Errors detectable at enqueue time are returned; an asynchronous CUDA fault surfaces at the next
- *    call or at destroy (AIMS_ERR_CUDA, text in aims_gpu_last_error).
+ *    call or at destroy (AIMS_ERR_CUDA, text in aims_gpu_last_error).  Device-side capacity / consistency flags raised
+ *    by a hot call are reported ONLY by aims_gpu_synchronize (once; the flag is then cleared).
  *  - Global basis index: atom-major, then the species' shells in order, then m = -l..l.
  *  - Lengths are in Angstrom; nothing converts units.
- *  - One context per host thread; a context is not thread-safe.
+ *  - One context per host thread; a context is not thread-safe.  Several contexts may be alive at once (also on one device).
+ *
+ * Deviations from the signatures sketched in SURVEY.md 8(b), and why:
+ *  - aims_gpu_create takes `workspace_bytes`: Phi planes of the whole grid do not fit in HBM (config 5: 54 GB per plane), so
+ *    every call streams them through a workspace in chunks of batches; its size is the caller's to bound.
+ *  - aims_gpu_basis_sizes / aims_gpu_eval_basis have no `want_grad`: a NULL `dphi` is the flag, and the sizes do not depend
+ *    on it (dphi is 3 * n_phi).
+ * The diagnostic entry points (timing, launch count, FP64 probes) are grouped at the end of this header; nothing on the
+ * product path needs them.
  */
 #ifndef AIMS_GPU_H
 #define AIMS_GPU_H
@@ -84,8 +94,10 @@ typedef struct aims_gpu_ctx aims_gpu_ctx;
 /* Create a context on `device` (cudaSetDevice ordinal) that enqueues on `cuda_stream` (a cudaStream_t, e.g.
  * torch.cuda.current_stream().cuda_stream; NULL = legacy default stream).  Copies the three descriptions to the
  * device, runs the culling once to size every per-batch list, and allocates workspaces (at most
- * workspace_bytes for the per-chunk Phi planes; 0 = default 24 GiB, clamped to free memory).
- * Synchronises the stream before returning. */
+ * workspace_bytes for the per-chunk Phi planes, never less than one batch in every plane layout; 0 = default 24 GiB,
+ * clamped to free memory).  Synchronises the stream before returning.
+ * On failure *out is NULL (nothing to free) or a half-built context that accepts ONLY aims_gpu_last_error and
+ * aims_gpu_destroy -- the caller must still destroy it. */
 int aims_gpu_create(aims_gpu_ctx **out, const aims_basis_desc *basis, const aims_grid_desc *grid,
                     const aims_bsr_desc *bsr, int device, void *cuda_stream, int64_t workspace_bytes);
 int aims_gpu_destroy(aims_gpu_ctx *ctx);
@@ -191,6 +203,14 @@ int aims_gpu_partition_weights(aims_gpu_ctx *ctx, int64_t n, const double *xyz, 
 int aims_gpu_bloch_fold(aims_gpu_ctx *ctx, const double *H_values, const int32_t *atom_home, const double *atom_T,
                         int32_t n_home, const double *kpt, double *out_re, double *out_im, int accumulate);
 
+/* Bitwise-reproducible H (PAPER.md L231 leaves the order of the batch sums free, it does not forbid a
+ * fixed one).  enable != 0: aims_gpu_integrate_hamiltonian[_ks] and aims_gpu_add_tau_matrix add every batch's contribution
+ * to H in ascending batch order ("ordered scatter": a tile of batch b waits until all tiles of the batches before b have
+ * added), so that two runs with the same inputs, batch range, accumulate history and workspace size give bit-identical
+ * H_values.  Default 0: contributions are added with floating-point reductions in arrival order (reruns agree to rounding).
+ * n, grad n and hess n are reduced without atomics and are bitwise reproducible in either mode; F is not. */
+int aims_gpu_set_deterministic(aims_gpu_ctx *ctx, int enable);
+
 /* Synchronise the context stream and report anything the device flagged since the last check: an asynchronous CUDA
  * fault (AIMS_ERR_CUDA) or a failed device-side capacity / consistency check (AIMS_ERR_UNSUPPORTED). */
 int aims_gpu_synchronize(aims_gpu_ctx *ctx);
@@ -203,6 +223,9 @@ int aims_gpu_stats(aims_gpu_ctx *ctx, int64_t *sum_nnz, int32_t *max_nnz, int32_
 
 /* |nnz(B)| of every batch as found at creation (HOST output, [n_batches]); used to balance batch ranges over GPUs. */
 int aims_gpu_batch_nnz(aims_gpu_ctx *ctx, int32_t *nnz);
+
+/* ===================================================== diagnostics =====================================================
+ * Nothing below is needed to compute anything; bench.py and the profiles use it. */
 
 /* Per-kernel device timing for bench.py's roofline: when enabled, every kernel launch of this context is bracketed by
  * CUDA events on the context stream.  aims_gpu_timing_enable synchronises, clears what was recorded and switches

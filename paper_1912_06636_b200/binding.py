@@ -95,6 +95,8 @@ def load_library():
     L.aims_gpu_pulay_forces_ks.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp, ctypes.c_int, _vp, _vp, _vp, ctypes.c_int]
     L.aims_gpu_synchronize.restype = ctypes.c_int
     L.aims_gpu_synchronize.argtypes = [cp]
+    L.aims_gpu_set_deterministic.restype = ctypes.c_int
+    L.aims_gpu_set_deterministic.argtypes = [cp, ctypes.c_int]
     L.aims_gpu_batch_nnz.restype = ctypes.c_int
     L.aims_gpu_batch_nnz.argtypes = [cp, _ip]
     L.aims_gpu_timing_enable.restype = ctypes.c_int
@@ -144,6 +146,10 @@ class Context:
         self.n_values = int(bun.n_values)
         self.n_atoms = int(k["atom_xyz"].shape[0])
         self.batch_ptr = k["batch_ptr"]
+        nfn_shell = 2 * k["shell_l"].astype(np.int64) + 1
+        sp_nfn = np.array([nfn_shell[k["species_shell_ptr"][q]:k["species_shell_ptr"][q + 1]].sum()
+                           for q in range(len(k["species_shell_ptr"]) - 1)], dtype=np.int64)
+        self.atom_fn_ptr = np.concatenate([[0], np.cumsum(sp_nfn[k["atom_species"]])]).astype(np.int64)  # output sizes only
         bd = _BasisDesc(int(k["atom_xyz"].shape[0]), int(k["species_shell_ptr"].shape[0] - 1), int(k["shell_l"].shape[0]),
                         int(k["spline_coef"].shape[0]), int(bun.n_knots), d(k["atom_xyz"]), i(k["atom_species"]),
                         i(k["species_shell_ptr"]), i(k["shell_l"]), d(k["shell_rcut"]), i(k["shell_spline"]),
@@ -184,6 +190,9 @@ class Context:
     def synchronize(self):
         self._check(self.L.aims_gpu_synchronize(self.h), "aims_gpu_synchronize")
 
+    def set_deterministic(self, enable=True):
+        self._check(self.L.aims_gpu_set_deterministic(self.h, int(bool(enable))), "aims_gpu_set_deterministic")
+
     def batch_nnz(self):
         out = np.zeros(max(self.n_batches, 1), dtype=np.int32)
         self._check(self.L.aims_gpu_batch_nnz(self.h, out.ctypes.data_as(_ip)), "aims_gpu_batch_nnz")
@@ -222,11 +231,16 @@ class Context:
         return t.value
 
     def _dev(self, a, dtype=None):
+        """Device copy of `a` on the CONTEXT stream (the stream the kernels run on): the copy is ordered before the
+        kernels that read it, and the caching allocator ties the temporary to that stream."""
         torch = self.torch
-        if isinstance(a, torch.Tensor):
-            t = a.to(self.device)
-            return t.contiguous() if dtype is None else t.to(dtype).contiguous()
-        return torch.as_tensor(np.ascontiguousarray(a), dtype=dtype).to(self.device)
+        with torch.cuda.stream(self.stream):
+            if isinstance(a, torch.Tensor):
+                if a.device == self.device and a.is_contiguous() and (dtype is None or a.dtype == dtype):
+                    return a
+                t = a.to(self.device)
+                return t.contiguous() if dtype is None else t.to(dtype).contiguous()
+            return torch.as_tensor(np.ascontiguousarray(a), dtype=dtype).to(self.device)
 
     # ---- the three hot calls (device tensors in, device tensors out)
     def basis_sizes(self, b0=0, b1=None):
@@ -310,9 +324,14 @@ class Context:
                     "aims_gpu_partition_weights")
         return out
 
-    def bloch_fold(self, H, atom_home, atom_T, n_home, kpt, n_home_basis):
-        """Complex device tensor [n_hb][n_hb]: Bloch sums of a real-space matrix (include/aims_gpu.h: aims_gpu_bloch_fold)."""
+    def bloch_fold(self, H, atom_home, atom_T, n_home, kpt, n_home_basis=None):
+        """Complex device tensor [n_hb][n_hb]: Bloch sums of a real-space matrix (include/aims_gpu.h: aims_gpu_bloch_fold).
+        n_hb = functions of the first n_home atoms (what the library writes); n_home_basis, if given, must agree."""
         torch = self.torch
+        n_hb = int(self.atom_fn_ptr[int(n_home)])
+        if n_home_basis is not None and int(n_home_basis) != n_hb:
+            raise AimsError("n_home_basis %d != functions of the %d cell atoms (%d)" % (n_home_basis, n_home, n_hb))
+        n_home_basis = n_hb
         H = self._dev(H, torch.float64)
         if H.numel() != self.n_values:
             raise AimsError("H must have n_values entries")
@@ -426,7 +445,11 @@ def aims_gpu_partition_weights(ctx, xyz, owner, r_part):
     return ctx.partition_weights(xyz, owner, r_part)
 
 
-def aims_gpu_bloch_fold(ctx, H, atom_home, atom_T, n_home, kpt, n_home_basis):
+def aims_gpu_set_deterministic(ctx, enable=True):
+    ctx.set_deterministic(enable)
+
+
+def aims_gpu_bloch_fold(ctx, H, atom_home, atom_T, n_home, kpt, n_home_basis=None):
     return ctx.bloch_fold(H, atom_home, atom_T, n_home, kpt, n_home_basis)
 
 

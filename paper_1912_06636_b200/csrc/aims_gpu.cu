@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstring>
 #include <map>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -54,6 +55,9 @@ struct aims_gpu_ctx {
 
   double *ws = nullptr;      // Phi-plane workspace
   double *probe_out = nullptr;
+  bool deterministic = false;                                   // aims_gpu_set_deterministic: ordered scatter into H
+  unsigned *det_counters = nullptr;                             // [2] ticket / done counters of the ordered scatter
+  long long *d_tile_off = nullptr;
   long long ws_doubles = 0;
 
   // optional per-kernel timing (CUDA events on the context stream around every launch)
@@ -207,6 +211,55 @@ __global__ void __launch_bounds__(512, 1) k_dmma_probe(double *out, int iters, d
 
 bool range_ok(const aims_gpu_ctx *c, int b0, int b1) { return c && b0 >= 0 && b1 >= b0 && b1 <= c->n_batches; }
 
+// Every extern "C" entry runs its body through this: no C++ exception (std::bad_alloc of the host-side tables and
+// strings, or anything else) crosses the C boundary -- include/aims_gpu.h promises status codes only.
+template <class F>
+int guarded(aims_gpu_ctx *c, F &&body) noexcept {
+  try {
+    return body();
+  } catch (const std::bad_alloc &) {
+    try { if (c) c->err = "out of host memory"; } catch (...) {}
+    return AIMS_ERR_NOMEM;
+  } catch (...) {
+    try { if (c) c->err = "unexpected C++ exception"; } catch (...) {}
+    return AIMS_ERR_INVALID_ARG;
+  }
+}
+
+// Opt every kernel with dynamic shared memory in to the device maximum, ONCE per device and process.  The attribute is
+// per function and device, not per context: sizing it from one context's max nnz(B) would shrink it under another,
+// larger context that is still alive.
+template <class K>
+cudaError_t smem_optin_max(K kernel, size_t optin) {
+  cudaFuncAttributes fa;
+  cudaError_t e = cudaFuncGetAttributes(&fa, kernel);
+  if (e != cudaSuccess) return e;
+  return cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(optin - fa.sharedSizeBytes));
+}
+constexpr size_t kStaticSmemMargin = 4096;   // >= the static shared memory of any kernel here (k_eval: 2.8 KB)
+
+cudaError_t smem_optin_all(int device, size_t optin) {
+  static std::mutex mu;
+  static bool done[64] = {};
+  std::lock_guard<std::mutex> lock(mu);
+  if (device >= 0 && device < 64 && done[device]) return cudaSuccess;
+  cudaError_t e;
+#define AIMS_OPTIN(k) if ((e = smem_optin_max(k, optin)) != cudaSuccess) return e;
+  AIMS_OPTIN(k_hamiltonian<false>) AIMS_OPTIN(k_hamiltonian<true>)
+  AIMS_OPTIN(k_density<false>) AIMS_OPTIN(k_density<true>)
+  AIMS_OPTIN(k_density_hessian)
+  AIMS_OPTIN(k_forces<false>) AIMS_OPTIN(k_forces<true>)
+#define AIMS_OPTIN_EV(M, LY) AIMS_OPTIN((k_eval<M, LY>))
+  AIMS_OPTIN_EV(kEvalPhi, kLayApi) AIMS_OPTIN_EV(kEvalPhiGrad, kLayApi) AIMS_OPTIN_EV(kEvalHLda, kLayH)
+  AIMS_OPTIN_EV(kEvalHGga, kLayH) AIMS_OPTIN_EV(kEvalHKinLda, kLayH) AIMS_OPTIN_EV(kEvalHKinGga, kLayH)
+  AIMS_OPTIN_EV(kEvalTau, kLayH) AIMS_OPTIN_EV(kEvalHess, kLayD) AIMS_OPTIN_EV(kEvalPhi, kLayD)
+  AIMS_OPTIN_EV(kEvalPhiGrad, kLayD) AIMS_OPTIN_EV(kEvalForceLda, kLayD) AIMS_OPTIN_EV(kEvalForceGga, kLayD)
+#undef AIMS_OPTIN_EV
+#undef AIMS_OPTIN
+  if (device >= 0 && device < 64) done[device] = true;
+  return cudaSuccess;
+}
+
 }  // namespace
 
 extern "C" {
@@ -225,7 +278,7 @@ int aims_gpu_destroy(aims_gpu_ctx *ctx) {
   return e == cudaSuccess ? AIMS_OK : AIMS_ERR_CUDA;
 }
 
-int aims_gpu_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_grid_desc *G, const aims_bsr_desc *P,
+static int impl_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_grid_desc *G, const aims_bsr_desc *P,
                     int device, void *cuda_stream, int64_t workspace_bytes) {
   if (!out) return AIMS_ERR_INVALID_ARG;
   *out = nullptr;
@@ -425,50 +478,43 @@ int aims_gpu_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_gri
   if ((rc = dev_alloc(c, &L.act_ld, (size_t)c->act_off[nb]))) return rc;
   if ((rc = dev_alloc(c, &L.ptab, (size_t)c->ptab_off[nb]))) return rc;
 
-  // ---- Phi-plane workspace: enough for the largest single batch with 10 planes (density Hessian), at most the requested budget
+  // ---- Phi-plane workspace: at least the largest single batch in EVERY plane layout used by a call (10 planes of the
+  // density layout for the Hessian, 6 x the 16-point-padded H layout for the tau matrix), at most the requested budget
   long long want = workspace_bytes > 0 ? workspace_bytes : (24ll << 30);
   size_t free_b = 0, total_b = 0;
   CU_TRY(c, cudaMemGetInfo(&free_b, &total_b));
   want = std::min<long long>(want, (long long)(free_b * 0.8));
-  long long max_batch_d = 0;
-  for (int b = 0; b < nb; b++) max_batch_d = std::max(max_batch_d, c->dpad_off[b + 1] - c->dpad_off[b]);
-  long long need_all = 10 * c->dpad_off[nb], need_min = 10 * max_batch_d;
+  long long need_min = 0;
+  for (int b = 0; b < nb; b++)
+    need_min = std::max({need_min, 10 * (c->dpad_off[b + 1] - c->dpad_off[b]), 6 * (c->pad16_off[b + 1] - c->pad16_off[b]),
+                         2 * (c->pad_off[b + 1] - c->pad_off[b])});
+  const long long need_all = std::max({10 * c->dpad_off[nb], 6 * c->pad16_off[nb], 2 * c->pad_off[nb]});
   long long wsd = std::min(need_all, std::max(want / 8, need_min)) + 10 * 64;
   if (wsd * 8 > (long long)free_b) return fail(c, AIMS_ERR_NOMEM, "not enough device memory for one batch of Phi planes");
   if ((rc = dev_alloc(c, &c->ws, (size_t)wsd))) return rc;
   c->ws_doubles = wsd;
+  if ((rc = dev_alloc(c, &c->det_counters, 2))) return rc;
+  if ((rc = dev_upload<long long>(c, &c->d_tile_off, c->tile_off.data(), c->tile_off.size()))) return rc;
 
-  // opt in to large dynamic shared memory
-  CU_TRY(c, cudaFuncSetAttribute(k_hamiltonian<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h_smem_bytes<false>()));
-  CU_TRY(c, cudaFuncSetAttribute(k_hamiltonian<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h_smem_bytes<true>()));
-  c->ptab_in_smem = d_smem_bytes(c->max_nnz, std::max(c->max_act, 1), true) <= (size_t)prop.sharedMemPerBlockOptin;
-  const size_t dsm = d_smem_bytes(c->max_nnz, std::max(c->max_act, 1), c->ptab_in_smem);
-  if (dsm > (size_t)prop.sharedMemPerBlockOptin) return fail(c, AIMS_ERR_UNSUPPORTED, "nnz(B) too large for the density kernel's shared memory");
-  CU_TRY(c, cudaFuncSetAttribute(k_density<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dsm));
-  CU_TRY(c, cudaFuncSetAttribute(k_density<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dsm));
-  c->x_ptab_in_smem = x_smem_bytes(c->max_nnz, std::max(c->max_act, 1), true) <= (size_t)prop.sharedMemPerBlockOptin;
-  if (x_smem_bytes(c->max_nnz, std::max(c->max_act, 1), c->x_ptab_in_smem) <= (size_t)prop.sharedMemPerBlockOptin)
-    CU_TRY(c, cudaFuncSetAttribute(k_density_hessian, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                   (int)x_smem_bytes(c->max_nnz, std::max(c->max_act, 1), c->x_ptab_in_smem)));
-  c->f_ptab_in_smem = f_smem_bytes(c->max_nnz, std::max(c->max_act, 1), true) <= (size_t)prop.sharedMemPerBlockOptin;
-  const size_t fsm = f_smem_bytes(c->max_nnz, std::max(c->max_act, 1), c->f_ptab_in_smem);
-  CU_TRY(c, cudaFuncSetAttribute(k_forces<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsm));
-  CU_TRY(c, cudaFuncSetAttribute(k_forces<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fsm));
-  {
-    const int esm = (int)eval_smem_bytes(c->max_nnz);
-    if ((size_t)esm + 4096 > (size_t)prop.sharedMemPerBlockOptin) return fail(c, AIMS_ERR_UNSUPPORTED, "nnz(B) too large for the evaluation kernel's shared memory");
-#define EV_ATTR(M, LY) CU_TRY(c, cudaFuncSetAttribute(k_eval<M, LY>, cudaFuncAttributeMaxDynamicSharedMemorySize, esm));
-    EV_ATTR(kEvalPhi, kLayApi) EV_ATTR(kEvalPhiGrad, kLayApi) EV_ATTR(kEvalHLda, kLayH) EV_ATTR(kEvalHGga, kLayH)
-    EV_ATTR(kEvalHKinLda, kLayH) EV_ATTR(kEvalHKinGga, kLayH) EV_ATTR(kEvalTau, kLayH)
-    EV_ATTR(kEvalHess, kLayD)
-    EV_ATTR(kEvalPhi, kLayD) EV_ATTR(kEvalPhiGrad, kLayD) EV_ATTR(kEvalForceLda, kLayD) EV_ATTR(kEvalForceGga, kLayD)
-#undef EV_ATTR
-  }
+  // large dynamic shared memory: every kernel is opted in to the device maximum once per device (see smem_optin_all);
+  // here only this context's own requirements are checked against it
+  CU_TRY(c, smem_optin_all(device, c->smem_optin));
+  const size_t lim = c->smem_optin - kStaticSmemMargin;
+  const int mact = std::max(c->max_act, 1);
+  c->ptab_in_smem = d_smem_bytes(c->max_nnz, mact, true) <= lim;
+  if (d_smem_bytes(c->max_nnz, mact, c->ptab_in_smem) > lim)
+    return fail(c, AIMS_ERR_UNSUPPORTED, "nnz(B) too large for the density kernel's shared memory");
+  c->x_ptab_in_smem = x_smem_bytes(c->max_nnz, mact, true) <= lim;
+  c->f_ptab_in_smem = f_smem_bytes(c->max_nnz, mact, true) <= lim;
+  if (f_smem_bytes(c->max_nnz, mact, c->f_ptab_in_smem) > lim)
+    return fail(c, AIMS_ERR_UNSUPPORTED, "nnz(B) too large for the force kernel's shared memory");
+  if (eval_smem_bytes(c->max_nnz) > lim)
+    return fail(c, AIMS_ERR_UNSUPPORTED, "nnz(B) too large for the evaluation kernel's shared memory");
   CU_TRY(c, cudaStreamSynchronize(c->stream));
   return AIMS_OK;
 }
 
-int aims_gpu_stats(aims_gpu_ctx *c, int64_t *sum_nnz, int32_t *max_nnz, int32_t *max_active_atoms, double *flops_h_lda,
+static int impl_stats(aims_gpu_ctx *c, int64_t *sum_nnz, int32_t *max_nnz, int32_t *max_active_atoms, double *flops_h_lda,
                    double *flops_h_gga, double *flops_density) {
   if (!c) return AIMS_ERR_INVALID_ARG;
   if (sum_nnz) *sum_nnz = c->fn_off.empty() ? 0 : c->fn_off.back();
@@ -480,13 +526,13 @@ int aims_gpu_stats(aims_gpu_ctx *c, int64_t *sum_nnz, int32_t *max_nnz, int32_t 
   return AIMS_OK;
 }
 
-int aims_gpu_batch_nnz(aims_gpu_ctx *c, int32_t *nnz) {
+static int impl_batch_nnz(aims_gpu_ctx *c, int32_t *nnz) {
   if (!c || !nnz) return AIMS_ERR_INVALID_ARG;
   std::copy(c->nnz.begin(), c->nnz.end(), nnz);
   return AIMS_OK;
 }
 
-int aims_gpu_basis_sizes(aims_gpu_ctx *c, int32_t b0, int32_t b1, int64_t *n_index, int64_t *n_phi) {
+static int impl_basis_sizes(aims_gpu_ctx *c, int32_t b0, int32_t b1, int64_t *n_index, int64_t *n_phi) {
   if (!range_ok(c, b0, b1)) return fail(c, AIMS_ERR_INVALID_ARG, "batch range outside [0, n_batches]");
   if (n_index) *n_index = c->fn_off[b1] - c->fn_off[b0];
   if (n_phi) *n_phi = c->api_off[b1] - c->api_off[b0];
@@ -507,9 +553,11 @@ int run_cull(aims_gpu_ctx *c, int b0, int b1) {
 }
 
 // last batch (exclusive) of the chunk starting at bs such that nplanes planes fit the workspace
+// (-1: even one batch does not fit -- cannot happen for the layouts create sized the workspace for)
 int chunk_end(const aims_gpu_ctx *c, const std::vector<long long> &off, int bs, int b1, int nplanes) {
   const long long cap = (c->ws_doubles / nplanes) & ~63ll;   // plane stride: 512-byte aligned
-  int lo = bs + 1, hi = b1;  // at least one batch (create guaranteed it fits)
+  if (off[bs + 1] - off[bs] > cap) return -1;
+  int lo = bs + 1, hi = b1;
   while (lo < hi) {
     int mid = (lo + hi + 1) >> 1;
     if (off[mid] - off[bs] <= cap) lo = mid; else hi = mid - 1;
@@ -550,6 +598,20 @@ int density_order(aims_gpu_ctx *c, int bs, int be, const int **out) {
   return AIMS_OK;
 }
 
+// One k_hamiltonian launch over the tiles of batches [bs, ...).  In deterministic mode (aims_gpu_set_deterministic) the
+// CTAs take their tile from a ticket counter and scatter in batch order (hamiltonian.cuh: "ordered scatter").
+int launch_hamiltonian(aims_gpu_ctx *c, bool syr2k, HArgs A, int bs, long long nt) {
+  if (c->deterministic) {
+    CU_TRY(c, cudaMemsetAsync(c->det_counters, 0, 2 * sizeof(unsigned), c->stream));
+    A.det = 1; A.ticket = c->det_counters; A.done = c->det_counters + 1;
+    A.tile_off = c->d_tile_off; A.tile_base = c->tile_off[bs];
+  }
+  TimedLaunch t(c, kKindHam);
+  if (syr2k) k_hamiltonian<true><<<(unsigned)nt, kHThreads, h_smem_bytes<true>(), c->stream>>>(c->S, c->L, A);
+  else k_hamiltonian<false><<<(unsigned)nt, kHThreads, h_smem_bytes<false>(), c->stream>>>(c->S, c->L, A);
+  return AIMS_OK;
+}
+
 template <int MODE, int LAYOUT>
 void launch_eval(aims_gpu_ctx *c, const EvalArgs &E, int bs, int be) {
   TimedLaunch t(c, kKindEval);
@@ -560,7 +622,7 @@ void launch_eval(aims_gpu_ctx *c, const EvalArgs &E, int bs, int be) {
 
 extern "C" {
 
-int aims_gpu_eval_basis(aims_gpu_ctx *c, int32_t b0, int32_t b1, int64_t *fn_ptr, int32_t *fn_index, int64_t *phi_ptr,
+static int impl_eval_basis(aims_gpu_ctx *c, int32_t b0, int32_t b1, int64_t *fn_ptr, int32_t *fn_index, int64_t *phi_ptr,
                         double *phi, double *dphi) {
   if (!range_ok(c, b0, b1)) return fail(c, AIMS_ERR_INVALID_ARG, "batch range outside [0, n_batches]");
   if (!fn_ptr || !fn_index || !phi_ptr || !phi) return fail(c, AIMS_ERR_INVALID_ARG, "NULL output");
@@ -593,6 +655,7 @@ static int run_hamiltonian(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double
   const long long *d_poff = syr2k ? c->d_pad_off : c->d_pad16_off;
   for (int bs = b0; bs < b1;) {
     const int be = chunk_end(c, poff, bs, b1, 2);
+    if (be < 0) return fail(c, AIMS_ERR_NOMEM, "workspace too small for one batch of Phi planes");
     const long long plane = (c->ws_doubles / 2) & ~63ll;
     EvalArgs E{};
     E.plane[0] = c->ws; E.plane[1] = c->ws + plane;
@@ -604,9 +667,7 @@ static int run_hamiltonian(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double
     const long long nt = c->tile_off[be] - c->tile_off[bs];
     if (nt > 0) {
       HArgs A{c->d_tiles + c->tile_off[bs], E.plane[0], E.plane[1], d_poff, poff[bs], H_values, 1};
-      TimedLaunch t(c, kKindHam);
-      if (syr2k) k_hamiltonian<true><<<(unsigned)nt, kHThreads, h_smem_bytes<true>(), c->stream>>>(c->S, c->L, A);
-      else k_hamiltonian<false><<<(unsigned)nt, kHThreads, h_smem_bytes<false>(), c->stream>>>(c->S, c->L, A);
+      if ((rc = launch_hamiltonian(c, syr2k, A, bs, nt))) return rc;
     }
     if ((rc = check_async(c))) return rc;
     bs = be;
@@ -614,7 +675,7 @@ static int run_hamiltonian(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double
   return AIMS_OK;
 }
 
-int aims_gpu_add_tau_matrix(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *xi, double *H_values) {
+static int impl_add_tau_matrix(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *xi, double *H_values) {
   if (!range_ok(c, b0, b1)) return fail(c, AIMS_ERR_INVALID_ARG, "batch range outside [0, n_batches]");
   if ((!xi && c->n_points) || !H_values) return fail(c, AIMS_ERR_INVALID_ARG, "NULL xi or H_values");
   CU_TRY(c, cudaSetDevice(c->device));
@@ -623,6 +684,7 @@ int aims_gpu_add_tau_matrix(aims_gpu_ctx *c, int32_t b0, int32_t b1, const doubl
   for (int bs = b0; bs < b1;) {
     // two planes of 3 x the 16-padded points each: [d_x Phi | d_y Phi | d_z Phi] and w xi / 2 times it
     const int be = chunk_end(c, c->pad16_off, bs, b1, 6);
+    if (be < 0) return fail(c, AIMS_ERR_NOMEM, "workspace too small for one batch of Phi planes");
     const long long third = (c->ws_doubles / 6) & ~63ll;
     EvalArgs E{};
     E.plane[0] = c->ws; E.plane[1] = c->ws + 3 * third;
@@ -632,8 +694,7 @@ int aims_gpu_add_tau_matrix(aims_gpu_ctx *c, int32_t b0, int32_t b1, const doubl
     const long long nt = c->tile_off[be] - c->tile_off[bs];
     if (nt > 0) {
       HArgs A{c->d_tiles + c->tile_off[bs], E.plane[0], E.plane[1], c->d_pad16_off, c->pad16_off[bs], H_values, 3};
-      TimedLaunch t(c, kKindHam);
-      k_hamiltonian<false><<<(unsigned)nt, kHThreads, h_smem_bytes<false>(), c->stream>>>(c->S, c->L, A);
+      if ((rc = launch_hamiltonian(c, false, A, bs, nt))) return rc;
     }
     if ((rc = check_async(c))) return rc;
     bs = be;
@@ -641,17 +702,17 @@ int aims_gpu_add_tau_matrix(aims_gpu_ctx *c, int32_t b0, int32_t b1, const doubl
   return AIMS_OK;
 }
 
-int aims_gpu_integrate_hamiltonian(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, const double *g,
+static int impl_integrate_hamiltonian(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, const double *g,
                                    double *H_values, int accumulate) {
   return run_hamiltonian(c, b0, b1, v, g, 0, H_values, accumulate);
 }
 
-int aims_gpu_integrate_hamiltonian_ks(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, const double *g, int kinetic,
+static int impl_integrate_hamiltonian_ks(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, const double *g, int kinetic,
                                       double *H_values, int accumulate) {
   return run_hamiltonian(c, b0, b1, v, g, kinetic, H_values, accumulate);
 }
 
-int aims_gpu_update_density(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *D_values, double *n, double *grad_n) {
+static int impl_update_density(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *D_values, double *n, double *grad_n) {
   if (!range_ok(c, b0, b1)) return fail(c, AIMS_ERR_INVALID_ARG, "batch range outside [0, n_batches]");
   if (!D_values || (!n && c->n_points)) return fail(c, AIMS_ERR_INVALID_ARG, "NULL D_values or n");
   CU_TRY(c, cudaSetDevice(c->device));
@@ -661,6 +722,7 @@ int aims_gpu_update_density(aims_gpu_ctx *c, int32_t b0, int32_t b1, const doubl
   const size_t dsm = d_smem_bytes(c->max_nnz, std::max(c->max_act, 1), c->ptab_in_smem);
   for (int bs = b0; bs < b1;) {
     const int be = chunk_end(c, c->dpad_off, bs, b1, npl);
+    if (be < 0) return fail(c, AIMS_ERR_NOMEM, "workspace too small for one batch of Phi planes");
     const long long plane = (c->ws_doubles / npl) & ~63ll;
     EvalArgs E{};
     for (int q = 0; q < npl; q++) E.plane[q] = c->ws + q * plane;
@@ -700,6 +762,7 @@ static int run_forces(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, 
   const size_t fsm = f_smem_bytes(c->max_nnz, std::max(c->max_act, 1), c->f_ptab_in_smem);
   for (int bs = b0; bs < b1;) {
     const int be = chunk_end(c, c->dpad_off, bs, b1, npl);
+    if (be < 0) return fail(c, AIMS_ERR_NOMEM, "workspace too small for one batch of Phi planes");
     const long long plane = (c->ws_doubles / npl) & ~63ll;
     EvalArgs E{};
     for (int q = 0; q < npl; q++) E.plane[q] = c->ws + q * plane;
@@ -726,7 +789,7 @@ static int run_forces(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, 
   return AIMS_OK;
 }
 
-int aims_gpu_partition_weights(aims_gpu_ctx *c, int64_t n, const double *xyz, const int32_t *owner, double r_part,
+static int impl_partition_weights(aims_gpu_ctx *c, int64_t n, const double *xyz, const int32_t *owner, double r_part,
                                double *w_part) {
   if (!c || n < 0 || (n && (!xyz || !owner || !w_part)) || !(r_part > 0)) return fail(c, AIMS_ERR_INVALID_ARG, "NULL array, n < 0 or r_part <= 0");
   CU_TRY(c, cudaSetDevice(c->device));
@@ -738,7 +801,7 @@ int aims_gpu_partition_weights(aims_gpu_ctx *c, int64_t n, const double *xyz, co
   return check_async(c);
 }
 
-int aims_gpu_bloch_fold(aims_gpu_ctx *c, const double *H_values, const int32_t *atom_home, const double *atom_T,
+static int impl_bloch_fold(aims_gpu_ctx *c, const double *H_values, const int32_t *atom_home, const double *atom_T,
                         int32_t n_home, const double *kpt, double *out_re, double *out_im, int accumulate) {
   if (!c || !H_values || !atom_home || !atom_T || !kpt || !out_re || !out_im) return fail(c, AIMS_ERR_INVALID_ARG, "NULL argument");
   const int na = c->S.n_atoms;
@@ -783,17 +846,18 @@ int aims_gpu_bloch_fold(aims_gpu_ctx *c, const double *H_values, const int32_t *
   return check_async(c);
 }
 
-int aims_gpu_density_hessian(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *D_values, double *hess_n) {
+static int impl_density_hessian(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *D_values, double *hess_n) {
   if (!range_ok(c, b0, b1)) return fail(c, AIMS_ERR_INVALID_ARG, "batch range outside [0, n_batches]");
   if (!D_values || (!hess_n && c->n_points)) return fail(c, AIMS_ERR_INVALID_ARG, "NULL D_values or hess_n");
   CU_TRY(c, cudaSetDevice(c->device));
   const size_t xsm = x_smem_bytes(c->max_nnz, std::max(c->max_act, 1), c->x_ptab_in_smem);
-  if (xsm > c->smem_optin) return fail(c, AIMS_ERR_UNSUPPORTED, "nnz(B) too large for the Hessian kernel's shared memory");
+  if (xsm > c->smem_optin - kStaticSmemMargin) return fail(c, AIMS_ERR_UNSUPPORTED, "nnz(B) too large for the Hessian kernel's shared memory");
   int rc = run_cull(c, b0, b1);
   if (rc) return rc;
   const int npl = 10;
   for (int bs = b0; bs < b1;) {
     const int be = chunk_end(c, c->dpad_off, bs, b1, npl);
+    if (be < 0) return fail(c, AIMS_ERR_NOMEM, "workspace too small for one batch of Phi planes");
     const long long plane = (c->ws_doubles / npl) & ~63ll;
     EvalArgs E{};
     for (int q = 0; q < npl; q++) E.plane[q] = c->ws + q * plane;
@@ -818,17 +882,23 @@ int aims_gpu_density_hessian(aims_gpu_ctx *c, int32_t b0, int32_t b1, const doub
   return AIMS_OK;
 }
 
-int aims_gpu_pulay_forces(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, const double *g, const double *D_values,
+static int impl_pulay_forces(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, const double *g, const double *D_values,
                           const double *Q_values, double *F, int accumulate) {
   return run_forces(c, b0, b1, v, g, 0, D_values, Q_values, F, accumulate);
 }
 
-int aims_gpu_pulay_forces_ks(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, const double *g, int kinetic,
+static int impl_pulay_forces_ks(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, const double *g, int kinetic,
                              const double *D_values, const double *Q_values, double *F, int accumulate) {
   return run_forces(c, b0, b1, v, g, kinetic, D_values, Q_values, F, accumulate);
 }
 
-int aims_gpu_timing_enable(aims_gpu_ctx *c, int enable) {
+static int impl_set_deterministic(aims_gpu_ctx *c, int enable) {
+  if (!c) return AIMS_ERR_INVALID_ARG;
+  c->deterministic = enable != 0;
+  return AIMS_OK;
+}
+
+static int impl_timing_enable(aims_gpu_ctx *c, int enable) {
   if (!c) return AIMS_ERR_INVALID_ARG;
   CU_TRY(c, cudaSetDevice(c->device));
   CU_TRY(c, cudaStreamSynchronize(c->stream));
@@ -838,36 +908,41 @@ int aims_gpu_timing_enable(aims_gpu_ctx *c, int enable) {
   return AIMS_OK;
 }
 
-int aims_gpu_timing_read(aims_gpu_ctx *c, double *ms, int64_t *launches) {
+static int impl_timing_read(aims_gpu_ctx *c, double *ms, int64_t *launches) {
   if (!c || !ms || !launches) return AIMS_ERR_INVALID_ARG;
   CU_TRY(c, cudaSetDevice(c->device));
   CU_TRY(c, cudaStreamSynchronize(c->stream));
   for (int k = 0; k < kNumKinds; k++) { ms[k] = 0.0; launches[k] = 0; }
+  cudaError_t bad = cudaSuccess;
   for (auto &sp : c->spans) {
     float t = 0.f;
-    CU_TRY(c, cudaEventElapsedTime(&t, sp.e0, sp.e1));
-    ms[sp.kind] += t;
-    launches[sp.kind]++;
-    c->pool.push_back(sp);
+    const cudaError_t e = cudaEventElapsedTime(&t, sp.e0, sp.e1);
+    if (e != cudaSuccess) bad = e;
+    else { ms[sp.kind] += t; launches[sp.kind]++; }
+    c->pool.push_back(sp);          // every span goes back to the pool exactly once, also on an error
   }
   c->spans.clear();
+  if (bad != cudaSuccess) { c->err = std::string("cudaEventElapsedTime: ") + cudaGetErrorString(bad); return AIMS_ERR_CUDA; }
   return AIMS_OK;
 }
 
-int aims_gpu_synchronize(aims_gpu_ctx *c) {
+static int impl_synchronize(aims_gpu_ctx *c) {
   if (!c) return AIMS_ERR_INVALID_ARG;
   CU_TRY(c, cudaSetDevice(c->device));
   int flag = 0;
   CU_TRY(c, cudaMemcpyAsync(&flag, c->L.error_flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
   CU_TRY(c, cudaStreamSynchronize(c->stream));
   if (flag) {
+    // reported once: the flag is cleared, so that a later synchronize reports only what was flagged since
+    CU_TRY(c, cudaMemsetAsync(c->L.error_flag, 0, sizeof(int), c->stream));
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
     c->err = "device-side capacity or consistency check failed (flag " + std::to_string(flag) + ")";
     return AIMS_ERR_UNSUPPORTED;
   }
   return AIMS_OK;
 }
 
-int aims_gpu_dmma_probe(aims_gpu_ctx *c, int variant, int warps_per_sm, double *tflops) {
+static int impl_dmma_probe(aims_gpu_ctx *c, int variant, int warps_per_sm, double *tflops) {
   if (!c || !tflops || variant < 1 || variant > 3 || warps_per_sm < 1 || warps_per_sm > 16) return fail(c, AIMS_ERR_INVALID_ARG, "variant 1..3, warps_per_sm 1..16");
   CU_TRY(c, cudaSetDevice(c->device));
   if (!c->probe_out) { int rc = dev_alloc(c, &c->probe_out, 16); if (rc) return rc; }   // scratch of the probes, allocated once
@@ -892,7 +967,7 @@ int aims_gpu_dmma_probe(aims_gpu_ctx *c, int variant, int warps_per_sm, double *
   return check_async(c);
 }
 
-int aims_gpu_fp64_peak(aims_gpu_ctx *c, double ms_target, double *tflops) {
+static int impl_fp64_peak(aims_gpu_ctx *c, double ms_target, double *tflops) {
   if (!c || !tflops) return AIMS_ERR_INVALID_ARG;
   CU_TRY(c, cudaSetDevice(c->device));
   if (!c->probe_out) { int rc = dev_alloc(c, &c->probe_out, 16); if (rc) return rc; }   // scratch of the probes, allocated once
@@ -915,6 +990,94 @@ int aims_gpu_fp64_peak(aims_gpu_ctx *c, double ms_target, double *tflops) {
   cudaEventDestroy(e0); cudaEventDestroy(e1);
   *tflops = 2.0 * 256 * 16 * (double)iters * grid.x * (block.x / 32) * reps / (ms * 1e-3) * 1e-12;
   return AIMS_OK;
+}
+
+}  // extern "C"
+
+// ---- the exported entry points: every body runs under `guarded` (no exception leaves the library)
+extern "C" {
+
+int aims_gpu_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_grid_desc *G, const aims_bsr_desc *P, int device, void *cuda_stream, int64_t workspace_bytes) {
+  // on failure *out is either NULL or a context that only aims_gpu_last_error and aims_gpu_destroy accept
+  const int rc = guarded(nullptr, [&] { return impl_create(out, B, G, P, device, cuda_stream, workspace_bytes); });
+  if (rc == AIMS_ERR_NOMEM && out && *out) guarded(nullptr, [&] { if ((*out)->err.empty()) (*out)->err = "out of memory"; return 0; });
+  return rc;
+}
+
+int aims_gpu_stats(aims_gpu_ctx *c, int64_t *sum_nnz, int32_t *max_nnz, int32_t *max_active_atoms, double *flops_h_lda, double *flops_h_gga, double *flops_density) {
+  return guarded(c, [&] { return impl_stats(c, sum_nnz, max_nnz, max_active_atoms, flops_h_lda, flops_h_gga, flops_density); });
+}
+
+int aims_gpu_batch_nnz(aims_gpu_ctx *c, int32_t *nnz) {
+  return guarded(c, [&] { return impl_batch_nnz(c, nnz); });
+}
+
+int aims_gpu_basis_sizes(aims_gpu_ctx *c, int32_t b0, int32_t b1, int64_t *n_index, int64_t *n_phi) {
+  return guarded(c, [&] { return impl_basis_sizes(c, b0, b1, n_index, n_phi); });
+}
+
+int aims_gpu_eval_basis(aims_gpu_ctx *c, int32_t b0, int32_t b1, int64_t *fn_ptr, int32_t *fn_index, int64_t *phi_ptr, double *phi, double *dphi) {
+  return guarded(c, [&] { return impl_eval_basis(c, b0, b1, fn_ptr, fn_index, phi_ptr, phi, dphi); });
+}
+
+int aims_gpu_add_tau_matrix(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *xi, double *H_values) {
+  return guarded(c, [&] { return impl_add_tau_matrix(c, b0, b1, xi, H_values); });
+}
+
+int aims_gpu_integrate_hamiltonian(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, const double *g, double *H_values, int accumulate) {
+  return guarded(c, [&] { return impl_integrate_hamiltonian(c, b0, b1, v, g, H_values, accumulate); });
+}
+
+int aims_gpu_integrate_hamiltonian_ks(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, const double *g, int kinetic, double *H_values, int accumulate) {
+  return guarded(c, [&] { return impl_integrate_hamiltonian_ks(c, b0, b1, v, g, kinetic, H_values, accumulate); });
+}
+
+int aims_gpu_update_density(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *D_values, double *n, double *grad_n) {
+  return guarded(c, [&] { return impl_update_density(c, b0, b1, D_values, n, grad_n); });
+}
+
+int aims_gpu_partition_weights(aims_gpu_ctx *c, int64_t n, const double *xyz, const int32_t *owner, double r_part, double *w_part) {
+  return guarded(c, [&] { return impl_partition_weights(c, n, xyz, owner, r_part, w_part); });
+}
+
+int aims_gpu_bloch_fold(aims_gpu_ctx *c, const double *H_values, const int32_t *atom_home, const double *atom_T, int32_t n_home, const double *kpt, double *out_re, double *out_im, int accumulate) {
+  return guarded(c, [&] { return impl_bloch_fold(c, H_values, atom_home, atom_T, n_home, kpt, out_re, out_im, accumulate); });
+}
+
+int aims_gpu_density_hessian(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *D_values, double *hess_n) {
+  return guarded(c, [&] { return impl_density_hessian(c, b0, b1, D_values, hess_n); });
+}
+
+int aims_gpu_pulay_forces(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, const double *g, const double *D_values, const double *Q_values, double *F, int accumulate) {
+  return guarded(c, [&] { return impl_pulay_forces(c, b0, b1, v, g, D_values, Q_values, F, accumulate); });
+}
+
+int aims_gpu_pulay_forces_ks(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, const double *g, int kinetic, const double *D_values, const double *Q_values, double *F, int accumulate) {
+  return guarded(c, [&] { return impl_pulay_forces_ks(c, b0, b1, v, g, kinetic, D_values, Q_values, F, accumulate); });
+}
+
+int aims_gpu_set_deterministic(aims_gpu_ctx *c, int enable) {
+  return guarded(c, [&] { return impl_set_deterministic(c, enable); });
+}
+
+int aims_gpu_timing_enable(aims_gpu_ctx *c, int enable) {
+  return guarded(c, [&] { return impl_timing_enable(c, enable); });
+}
+
+int aims_gpu_timing_read(aims_gpu_ctx *c, double *ms, int64_t *launches) {
+  return guarded(c, [&] { return impl_timing_read(c, ms, launches); });
+}
+
+int aims_gpu_synchronize(aims_gpu_ctx *c) {
+  return guarded(c, [&] { return impl_synchronize(c); });
+}
+
+int aims_gpu_dmma_probe(aims_gpu_ctx *c, int variant, int warps_per_sm, double *tflops) {
+  return guarded(c, [&] { return impl_dmma_probe(c, variant, warps_per_sm, tflops); });
+}
+
+int aims_gpu_fp64_peak(aims_gpu_ctx *c, double ms_target, double *tflops) {
+  return guarded(c, [&] { return impl_fp64_peak(c, ms_target, tflops); });
 }
 
 }  // extern "C"

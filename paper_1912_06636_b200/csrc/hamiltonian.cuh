@@ -40,6 +40,12 @@ struct HArgs {
   long long pad_base;
   double *H;                // block-sparse values
   int pmul;                 // planes hold pmul x the (padded) points of a batch: 1, or 3 for the stacked gradient planes of the tau matrix
+  // ordered scatter (deterministic mode): CTAs take tiles from `ticket` in list order (sorted by batch)
+  // and a tile of batch b adds to H only after `done` says that every tile of the batches before b has finished adding
+  int det;
+  unsigned *ticket, *done;
+  const long long *tile_off;   // [n_batches+1] first tile of every batch (context-wide numbering)
+  long long tile_base;         // tile_off of the launch's first batch
 };
 
 // first row of block k when nsub sub-tiles of 8 rows are cut into nblk blocks (sizes differ by at most one sub-tile)
@@ -168,9 +174,18 @@ __global__ void __launch_bounds__(kHThreads, 2) k_hamiltonian(DevSys S, BatchLis
   int *s_colinfo = s_rowinfo + kHI;
   int *s_ld = s_colinfo + kHJ;
 
-  const HTile tile = A.tiles[blockIdx.x];
-  const int b = tile.b;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  __shared__ unsigned s_tix, s_warps_done;
+  unsigned tix = blockIdx.x;
+  if (A.det) {
+    // ordered scatter: tiles are taken in list order (ascending batch) by ticket, so that every tile a CTA may have to
+    // wait for below was started before it -- no deadlock whatever order the hardware dispatches CTAs in
+    if (tid == 0) { s_tix = atomicAdd(A.ticket, 1u); s_warps_done = 0; }
+    __syncthreads();
+    tix = s_tix;
+  }
+  const HTile tile = A.tiles[tix];
+  const int b = tile.b;
   const int nnz = L.nnz[b], nact = L.n_act[b];
   const int nnz8 = pad8(nnz), nsub = nnz8 >> 3, nblk = blk_count(nsub);
   // a stage holds 8 points (GGA: two groups, two products each) or 16 points (LDA: four groups); the LDA planes are padded
@@ -264,6 +279,17 @@ __global__ void __launch_bounds__(kHThreads, 2) k_hamiltonian(DevSys S, BatchLis
   });
 
   // ---- epilogue (S2d): per warp, 8-row strips through shared memory, then coalesced REDs along the block row
+  if (A.det) {
+    // Within one batch every H element is added to by exactly one lane of one tile, so only the order ACROSS batches
+    // matters: wait until all tiles of earlier batches are done.  (`done` counts finished tiles; a tile can only finish
+    // after all tiles of earlier batches, so done >= first tile of b  <=>  all earlier tiles finished.)
+    const unsigned need = (unsigned)(A.tile_off[b] - A.tile_base);
+    if (lane == 0) {
+      unsigned seen;
+      do { asm volatile("ld.acquire.gpu.global.u32 %0, [%1];\n" : "=r"(seen) : "l"(A.done) : "memory"); } while (seen < need);
+    }
+    __syncwarp();
+  }
   double *strip = s_strip + warp * (8 * kHStripLd);
   const int fr = lane >> 2, fk = lane & 3;
   const long long *ptab = L.ptab + L.ptab_off[b];
@@ -297,6 +323,14 @@ __global__ void __launch_bounds__(kHThreads, 2) k_hamiltonian(DevSys S, BatchLis
           if (si == sj && !(diag && csub == a)) red_add_f64(A.H + base + (long long)cb * ldj + ra, val);
         }
       }
+    }
+  }
+  if (A.det) {
+    __threadfence();                                   // this warp's adds are performed before it reports
+    __syncwarp();
+    if (lane == 0 && atomicAdd(&s_warps_done, 1u) == (unsigned)nlive - 1u) {
+      __threadfence();                                 // cumulativity: the other warps' adds were fenced before their count
+      atomicAdd(A.done, 1u);
     }
   }
 }

@@ -25,6 +25,9 @@ FULL = {
     "cfg2_full_lda": (2, {}, False, 24),
     "cfg3_full_gga": (3, {}, True, 24),
     "cfg4_full_b64": (4, dict(max_batch=64), True, 48),
+    "cfg4_full_b100": (4, dict(max_batch=100), True, 32),
+    "cfg4_full_b200": (4, dict(max_batch=200), True, 16),
+    "cfg4_full_b300": (4, dict(max_batch=300), True, 12),
     "cfg4_full_b500": (4, dict(max_batch=500), True, 10),
     "cfg5_full_gga": (5, {}, True, 24),
 }
@@ -89,6 +92,44 @@ def test_full_size_hamiltonian_on_sampled_batches(full):
     ctx.synchronize()
     ref = orc.integrate_hamiltonian(bun.v, g, batches=sel)
     assert _rel_fro(H.cpu().numpy(), ref) <= TOL_H
+
+
+def test_whole_grid_hamiltonian_and_density_against_the_full_oracle(full):
+    """Configs 2 (LDA) and 3 (GGA) in FULL: the whole-grid, default-workspace calls bench.py times, every stored value of H
+    and every point of n, grad n against a complete oracle run (about a minute on the box's host cores), plus the same H
+    through a workspace small enough to force several chunks and through the ordered (deterministic) scatter."""
+    import torch
+    import paper_1912_06636_b200 as aims
+    name, bun, orc, ctx, gga, sel = full
+    if name not in ("cfg2_full_lda", "cfg3_full_gga"):
+        pytest.skip("the oracle finishes a full run only for the 64-atom configurations")
+    g = bun.g if gga else None
+    ref = orc.integrate_hamiltonian(bun.v, g)
+    H = ctx.integrate_hamiltonian(bun.v, g)
+    n, gn = ctx.update_density(bun.D_values, want_grad=gga)
+    ctx.synchronize()
+    assert _rel_fro(H.cpu().numpy(), ref) <= TOL_H
+    n_ref, gn_ref = orc.update_density(bun.D_values, want_grad=gga)
+    assert _rel_max(n.cpu().numpy(), n_ref) <= TOL_N
+    if gga:
+        assert _rel_max(gn.cpu().numpy(), gn_ref) <= TOL_N
+    # strict pointwise figure, for information (SURVEY P14): floor 1e-6 max|ref|
+    floor = 1e-6 * np.abs(n_ref).max()
+    print("%s: strict pointwise relative error of n (floor 1e-6 max|n|): %.2e"
+          % (name, float((np.abs(n.cpu().numpy() - n_ref) / np.maximum(np.abs(n_ref), floor)).max())))
+    small = aims.aims_gpu_create(bun, device=0, workspace_bytes=256 << 20)     # 256 MiB: several chunks per call
+    n0 = small.launch_count()
+    Hs = small.integrate_hamiltonian(bun.v, g)
+    small.synchronize()
+    assert small.launch_count() - n0 >= 1 + 2 * 3
+    assert _rel_fro(Hs.cpu().numpy(), ref) <= TOL_H
+    small.set_deterministic(True)
+    Hd1 = small.integrate_hamiltonian(bun.v, g)
+    Hd2 = small.integrate_hamiltonian(bun.v, g)
+    small.synchronize()
+    assert torch.equal(Hd1, Hd2)
+    assert _rel_fro(Hd1.cpu().numpy(), ref) <= TOL_H
+    small.close()
 
 
 def test_full_size_properties_of_whole_grid_outputs(full):
