@@ -996,3 +996,161 @@ void orc_partition_weights(const orc_system *S, int64_t n, const double *xyz, co
     out[p] = sum > 0.0 ? pown / sum : 0.0;
   }
 }
+
+/* ====================================================================================================================
+ * O9  Pulay part of the stress tensor (Eq. 20: sigma_lm = (1/V) dE_tot/d eps_lm;
+ * L299-308: force AND stress components are the same per-batch dense products; L405: the Pulay contribution to F_at and
+ * sigma_lm is evaluated alongside the density update; L413-415 / Table 2: "SCF+F+sigma" is the paper's largest case).
+ * The paper defers the individual terms to its Ref. [83] (L158); what it does fix is the handle, Eq. 20, and that is what is
+ * written out here -- exactly as the forces above follow from Eq. 14 (reading P22).  Under a homogeneous strain
+ * r -> (1 + eps) r of atoms AND grid points, a basis function seen from a grid point becomes phi_i((1 + eps)(r - R_at)), so
+ *   d phi_i / d eps_lm = (d_l phi_i) (r - R_at)_m ,     d (d_c phi_i) / d eps_lm = (d_l d_c phi_i) (r - R_at)_m ,
+ * and the Pulay part of Eq. 20 is the derivative of  Tr(n h(eps)) - Tr(q s(eps))  at fixed n_ij, q_ij (Eq. 17) and fixed
+ * point values v_p, g_p, w_p (the strain dependence of the integration weights and of the fields belongs to the other terms
+ * of the stress, which like the Hellmann-Feynman and multipole forces are not on this path):
+ *   V sigma_lm = 2 sum_p w_p sum_i (r_p - R_at(i))_m { d_l phi_i [ sum_j n_ij (v_p phi_j + g_p.grad phi_j [- 1/2 lap phi_j]) - q_ij phi_j ]
+ *                                                      + (Hess phi_i g_p)_l sum_j n_ij phi_j } ,
+ * i.e. the force integrand of O5 weighted with the distance vector to the function's own atom.  With point-attached fields
+ * that do not co-rotate, sigma need not be symmetric; all nine components are returned, sigma[l][m].
+ * Pins (tests/test_oracle_stress_pins.py): central differences of the already pinned H and S on a strained copy of the
+ * inputs; the term-by-term brute force below (no batches, no culling, both index orders written out); sum rule with the
+ * forces for an s-only basis; invariance under translation of the whole system and under re-batching; linear in (n, q).
+ * ==================================================================================================================== */
+void orc_pulay_stress(const orc_system *S, int n_sel, const int32_t *batches, const double *v, const double *g,
+                      const double *D_values, const double *Q_values, int kinetic, double volume, double *sigma) {
+  int64_t *afp = (int64_t *)malloc(sizeof(int64_t) * (S->n_atoms + 1));
+  orc_atom_fn_ptr(S, afp);
+  int nf_tot = (int)afp[S->n_atoms];
+  int32_t *idx = (int32_t *)malloc(sizeof(int32_t) * 4 * (size_t)nf_tot);
+  int32_t *fa = idx + nf_tot, *fs = fa + nf_tot, *fm = fs + nf_tot;
+  static const int hx[3][3] = {{0, 3, 4}, {3, 1, 5}, {4, 5, 2}};   /* index of (c,e) in (xx,yy,zz,xy,xz,yz) */
+  for (int q = 0; q < n_sel; q++) {
+    int b = batches[q];
+    int64_t p0 = S->batch_ptr[b];
+    int np = (int)(S->batch_ptr[b + 1] - p0);
+    int nnz = orc_batch_nnz(S, b, idx, fa, fs, fm);
+    if (nnz == 0 || np == 0) continue;
+    size_t sz = (size_t)nnz * np;
+    double *phi = (double *)malloc(sizeof(double) * sz * 10);     /* phi, dphi[3], hess[6] */
+    double *dphi = phi + sz, *hes = phi + 4 * sz;
+    for (int i = 0; i < nnz;) {
+      int l = S->shell_l[fs[i]];
+      for (int p = 0; p < np; p++) {
+        double val[7], gr[7][3], hh[7][6];
+        orc_shell_hess_at_point(S, fa[i], fs[i], S->xyz + 3 * (p0 + p), val, gr, hh);
+        for (int m = 0; m < 2 * l + 1; m++) {
+          phi[(size_t)(i + m) * np + p] = val[m];
+          for (int c = 0; c < 3; c++) dphi[((size_t)c * nnz + i + m) * np + p] = gr[m][c];
+          for (int k = 0; k < 6; k++) hes[((size_t)k * nnz + i + m) * np + p] = hh[m][k];
+        }
+      }
+      i += 2 * l + 1;
+    }
+    double *Db = (double *)malloc(sizeof(double) * (size_t)nnz * nnz);
+    double *Qb = Q_values ? (double *)malloc(sizeof(double) * (size_t)nnz * nnz) : NULL;
+    restrict_matrix(S, afp, nnz, idx, fa, D_values, Db);
+    if (Qb) restrict_matrix(S, afp, nnz, idx, fa, Q_values, Qb);
+    double *Srow = (double *)calloc((size_t)nnz * 9, sizeof(double));     /* per-function contribution, summed below */
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int i = 0; i < nnz; i++) {
+      double s9[3][3] = {{0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}, {0.0, 0.0, 0.0}};
+      const double *Ra = S->atom_xyz + 3 * fa[i];
+      for (int p = 0; p < np; p++) {
+        double gp[3] = {0.0, 0.0, 0.0};
+        if (g) for (int c = 0; c < 3; c++) gp[c] = g[(size_t)c * S->n_points + p0 + p];
+        double tn = 0.0, tg = 0.0, tq = 0.0, tk = 0.0;
+        for (int j = 0; j < nnz; j++) {
+          double dij = Db[(size_t)i * nnz + j];
+          tn += dij * phi[(size_t)j * np + p];
+          if (kinetic) {
+            double lap = (hes[((size_t)0 * nnz + j) * np + p] + hes[((size_t)1 * nnz + j) * np + p]) + hes[((size_t)2 * nnz + j) * np + p];
+            tk += dij * (-0.5 * lap);
+          }
+          if (g) {
+            double Gj = 0.0;
+            for (int c = 0; c < 3; c++) Gj += gp[c] * dphi[((size_t)c * nnz + j) * np + p];
+            tg += dij * Gj;
+          }
+          if (Qb) tq += Qb[(size_t)i * nnz + j] * phi[(size_t)j * np + p];
+        }
+        double wp = S->w[p0 + p];
+        double x = v[p0 + p] * tn + tg - tq + tk;
+        for (int l = 0; l < 3; l++) {
+          double t = dphi[((size_t)l * nnz + i) * np + p] * x;
+          if (g) {
+            double hg = 0.0;
+            for (int e = 0; e < 3; e++) hg += hes[((size_t)hx[l][e] * nnz + i) * np + p] * gp[e];
+            t += hg * tn;
+          }
+          for (int m = 0; m < 3; m++) s9[l][m] += 2.0 * wp * t * (S->xyz[3 * (p0 + p) + m] - Ra[m]);
+        }
+      }
+      for (int l = 0; l < 3; l++)
+        for (int m = 0; m < 3; m++) Srow[(size_t)i * 9 + 3 * l + m] = s9[l][m];
+    }
+    for (int i = 0; i < nnz; i++)
+      for (int k = 0; k < 9; k++) sigma[k] += Srow[(size_t)i * 9 + k] / volume;
+    free(Srow);
+    free(Qb);
+    free(Db);
+    free(phi);
+  }
+  free(idx);
+  free(afp);
+}
+
+/* brute-force Pulay stress (tiny inputs only): no batches, no culling, dense Dd, Qd (Qd may be NULL).  d/d eps_lm of
+ *   sum_ab n_ab int [ phi_a v phi_b + g.(grad phi_a phi_b + phi_a grad phi_b) (+ 1/2 (phi_a t phi_b + t phi_a phi_b)) ] - sum_ab q_ab int phi_a phi_b
+ * with every strained factor differentiated separately (both index orders written out, nothing symmetrised by hand). */
+void orc_brute_stress(const orc_system *S, const double *v, const double *g, const double *Dd, const double *Qd, double volume,
+                      double *sigma) {
+  int64_t *afp = (int64_t *)malloc(sizeof(int64_t) * (S->n_atoms + 1));
+  orc_atom_fn_ptr(S, afp);
+  int nb = (int)afp[S->n_atoms];
+  double *phi = (double *)malloc(sizeof(double) * (size_t)nb * 10);
+  double *dph = phi + nb, *hes = phi + 4 * (size_t)nb;        /* dph[c*nb+i], hes[k*nb+i] */
+  int *at_of = (int *)malloc(sizeof(int) * (size_t)nb);
+  static const int hx[3][3] = {{0, 3, 4}, {3, 1, 5}, {4, 5, 2}};
+  for (int64_t p = 0; p < S->n_points; p++) {
+    int i = 0;
+    for (int a = 0; a < S->n_atoms; a++) {
+      int sp = S->atom_species[a];
+      for (int s = S->species_shell_ptr[sp]; s < S->species_shell_ptr[sp + 1]; s++) {
+        int l = S->shell_l[s];
+        double val[7], gr[7][3], hh[7][6];
+        orc_shell_hess_at_point(S, a, s, S->xyz + 3 * p, val, gr, hh);
+        for (int m = 0; m < 2 * l + 1; m++, i++) {
+          phi[i] = val[m]; at_of[i] = a;
+          for (int c = 0; c < 3; c++) dph[c * nb + i] = gr[m][c];
+          for (int k = 0; k < 6; k++) hes[k * nb + i] = hh[m][k];
+        }
+      }
+    }
+    double wp = S->w[p];
+    for (int a = 0; a < nb; a++)
+      for (int b = 0; b < nb; b++) {
+        double nab = Dd[(size_t)a * nb + b], qab = Qd ? Qd[(size_t)a * nb + b] : 0.0;
+        if (nab == 0.0 && qab == 0.0) continue;
+        const double *Ra = S->atom_xyz + 3 * at_of[a], *Rb = S->atom_xyz + 3 * at_of[b];
+        for (int l = 0; l < 3; l++)
+          for (int m = 0; m < 3; m++) {
+            double da = S->xyz[3 * p + m] - Ra[m], db = S->xyz[3 * p + m] - Rb[m];
+            double dphi_a = dph[l * nb + a] * da, dphi_b = dph[l * nb + b] * db;     /* d phi / d eps_lm */
+            double t = (nab * v[p] - qab) * (dphi_a * phi[b] + phi[a] * dphi_b);
+            if (g) {
+              double Ga = 0.0, Gb = 0.0, dGa = 0.0, dGb = 0.0;                        /* g.grad phi and its strain derivative */
+              for (int c = 0; c < 3; c++) {
+                double gc = g[(size_t)c * S->n_points + p];
+                Ga += gc * dph[c * nb + a]; Gb += gc * dph[c * nb + b];
+                dGa += gc * hes[hx[l][c] * nb + a] * da; dGb += gc * hes[hx[l][c] * nb + b] * db;
+              }
+              t += nab * (dGa * phi[b] + Ga * dphi_b + dphi_a * Gb + phi[a] * dGb);
+            }
+            sigma[3 * l + m] += wp * t / volume;
+          }
+      }
+  }
+  free(at_of);
+  free(phi);
+  free(afp);
+}

@@ -61,6 +61,8 @@ def _load():
         L.orc_shell_hess_at_point.argtypes = [sp, ctypes.c_int, ctypes.c_int, _dp, _dp, _dp, _dp]
         L.orc_pulay_forces.argtypes = [sp, ctypes.c_int, _ip, _dp, _dp, _dp, _dp, ctypes.c_int, _dp]
         L.orc_brute_forces.argtypes = [sp, _dp, _dp, _dp, _dp, ctypes.c_int, _dp]
+        L.orc_pulay_stress.argtypes = [sp, ctypes.c_int, _ip, _dp, _dp, _dp, _dp, ctypes.c_int, ctypes.c_double, _dp]
+        L.orc_brute_stress.argtypes = [sp, _dp, _dp, _dp, _dp, ctypes.c_double, _dp]
         L.orc_integrate_hamiltonian_ks.argtypes = [sp, ctypes.c_int, _ip, _dp, _dp, ctypes.c_int, _dp]
         L.orc_brute_kinetic.argtypes = [sp, _dp, _dp]
         L.orc_density_hessian.argtypes = [sp, ctypes.c_int, _ip, _dp, _dp]
@@ -294,3 +296,24 @@ class Oracle:
         F = np.zeros((self.sys.n_atoms, 3))
         self.L.orc_brute_forces(ctypes.byref(self.sys), _d(v), _d(g), _d(Dd), _d(Qd), int(bool(kinetic)), _d(F))
         return F
+
+    def pulay_stress(self, v, D_values, g=None, Q_values=None, batches=None, kinetic=False, volume=1.0):
+        """sigma[3][3] (O9): Pulay part of Eq. 20 summed over the listed batches; volume = 1 gives dE/d eps."""
+        sel = self._sel(batches)
+        v = np.ascontiguousarray(v, dtype=np.float64)
+        g = None if g is None else np.ascontiguousarray(g, dtype=np.float64)
+        D = np.ascontiguousarray(D_values, dtype=np.float64)
+        Q = None if Q_values is None else np.ascontiguousarray(Q_values, dtype=np.float64)
+        sig = np.zeros((3, 3))
+        self.L.orc_pulay_stress(ctypes.byref(self.sys), len(sel), _i(sel), _d(v), _d(g), _d(D), _d(Q), int(bool(kinetic)),
+                                float(volume), _d(sig))
+        return sig
+
+    def brute_stress(self, v, D_dense, g=None, Q_dense=None, volume=1.0):
+        v = np.ascontiguousarray(v, dtype=np.float64)
+        g = None if g is None else np.ascontiguousarray(g, dtype=np.float64)
+        Dd = np.ascontiguousarray(D_dense, dtype=np.float64)
+        Qd = None if Q_dense is None else np.ascontiguousarray(Q_dense, dtype=np.float64)
+        sig = np.zeros((3, 3))
+        self.L.orc_brute_stress(ctypes.byref(self.sys), _d(v), _d(g), _d(Dd), _d(Qd), float(volume), _d(sig))
+        return sig
