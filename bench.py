@@ -57,7 +57,7 @@ def parse():
     ap.add_argument("--cpu-sample-batches", type=int, default=96)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--path", default="scf", choices=["scf", "forces", "hessian"])
+    ap.add_argument("--path", default="scf", choices=["scf", "forces", "stress", "hessian"])
     ap.add_argument("--kinetic", action="store_true",
                     help="scf path with the full h_KS phi (kinetic term, row f2): a separate line, not the headline metric")
     return ap.parse_args()
@@ -127,7 +127,7 @@ def sample_batches(n_batches, k, seed=20191206):
     return np.sort(rng.choice(n_batches, size=min(k, n_batches), replace=False)).astype(np.int32)
 
 
-def time_oracle(bun, batches, gga, repeats=1, forces_q=None, kinetic=False, hessian=False):
+def time_oracle(bun, batches, gga, repeats=1, forces_q=None, kinetic=False, hessian=False, stress=False):
     """Oracle as it stands on the host cores: H integration + density update (or, with forces_q, the Pulay forces) on
     the listed batches."""
     from oracle import oracle as orc
@@ -140,6 +140,8 @@ def time_oracle(bun, batches, gga, repeats=1, forces_q=None, kinetic=False, hess
             o.density_hessian(bun.D_values, batches=batches)
         elif forces_q is not None:
             o.pulay_forces(bun.v, bun.D_values, g=bun.g if gga else None, Q_values=forces_q, batches=batches)
+            if stress:
+                o.pulay_stress(bun.v, bun.D_values, g=bun.g if gga else None, Q_values=forces_q, batches=batches)
         else:
             if kinetic:
                 o.integrate_hamiltonian_ks(bun.v, bun.g if gga else None, kinetic=True, batches=batches)
@@ -151,13 +153,13 @@ def time_oracle(bun, batches, gga, repeats=1, forces_q=None, kinetic=False, hess
     return pts, best, orc.num_threads()
 
 
-def run_reference(args, bun, gga, workload, metric, forces_q=None, hessian=False):
+def run_reference(args, bun, gga, workload, metric, forces_q=None, hessian=False, stress=False):
     """--impl reference: the CPU oracle, rank 0 only, a bounded sample per step."""
     per_step = max(4, args.cpu_sample_batches // 4)
     times, pts_step = [], 0
     for s in range(args.warmup + args.steps):
         sel = sample_batches(bun.n_batches, per_step, seed=1000 + s)
-        pts, dt, cores = time_oracle(bun, sel, gga, forces_q=forces_q, kinetic=args.kinetic and forces_q is None, hessian=hessian)
+        pts, dt, cores = time_oracle(bun, sel, gga, forces_q=forces_q, kinetic=args.kinetic and forces_q is None, hessian=hessian, stress=stress)
         if s >= args.warmup:
             times.append(dt)
             pts_step += pts
@@ -186,9 +188,12 @@ def main():
     if args.n_rad or args.n_ang:
         workload += " [DEBUG GRID n_rad=%s n_ang=%s: not the benchmark workload]" % (args.n_rad, args.n_ang)
 
-    forces = args.path == "forces"
+    stress = args.path == "stress"                       # Pulay forces AND stress in one pass (row f1, "SCF+F+sigma")
+    forces = args.path == "forces" or stress
     hessian = args.path == "hessian"
     metric = METRIC if not forces else "grid points/s for the Pulay-force pass (FP64); % of FP64 peak"
+    if stress:
+        metric = "grid points/s for the Pulay force + stress pass (FP64); % of FP64 peak"
     if hessian:
         metric = "grid points/s for the density-Hessian pass (FP64); % of FP64 peak"
     if args.kinetic and not forces and not hessian:
@@ -203,7 +208,7 @@ def main():
         if hessian:
             args.cpu_sample_batches = min(args.cpu_sample_batches, 32)
         run_reference(args, bun, gga, workload, metric, forces_q=aims_synth.make_q_values(bun) if forces else None,
-                      hessian=hessian)
+                      hessian=hessian, stress=stress)
         return 0
 
     import torch
@@ -245,6 +250,7 @@ def main():
         gn = torch.zeros((3, bun.n_points), dtype=torch.float64, device="cuda") if gga else None
         Q = torch.as_tensor(Qh).to("cuda") if forces else None
         F = torch.zeros((bun.n_atoms, 3), dtype=torch.float64, device="cuda")
+        SG = torch.zeros((3, 3), dtype=torch.float64, device="cuda")
         Hn = torch.zeros((6, bun.n_points), dtype=torch.float64, device="cuda") if hessian else None
     stream.synchronize()
 
@@ -254,9 +260,14 @@ def main():
                 ctx.density_hessian(D, hess_n=Hn, b0=b0, b1=b1)
                 return
             if forces:
-                ctx.pulay_forces(v, D, g=g, Q=Q, F=F, b0=b0, b1=b1, accumulate=False)
+                if stress:
+                    ctx.pulay_forces_stress(v, D, g=g, Q=Q, volume=1.0, F=F, sigma=SG, b0=b0, b1=b1, accumulate=False)
+                else:
+                    ctx.pulay_forces(v, D, g=g, Q=Q, F=F, b0=b0, b1=b1, accumulate=False)
                 if world > 1:
                     dist.all_reduce(F)
+                    if stress:
+                        dist.all_reduce(SG)
                 return
             ctx.integrate_hamiltonian(v, g, H=H, b0=b0, b1=b1, accumulate=False, kinetic=kin)
             if world > 1:
@@ -318,6 +329,8 @@ def main():
             hb["Q"].copy_(torch.as_tensor(Qh))
             hb["F"] = torch.empty((bun.n_atoms, 3), dtype=torch.float64, pin_memory=True)
             dv["Q"], dv["F"] = torch.empty_like(Q), torch.empty_like(F)
+            hb["SG"] = torch.empty((3, 3), dtype=torch.float64, pin_memory=True)
+            dv["SG"] = torch.empty_like(SG)
 
         if hessian:
             hb["Hn"] = torch.empty((6, bun.n_points), dtype=torch.float64, pin_memory=True)
@@ -337,10 +350,18 @@ def main():
                     dv["g"].copy_(hb["g"], non_blocking=True)
                 if forces:
                     dv["Q"].copy_(hb["Q"], non_blocking=True)
-                    ctx.pulay_forces(dv["v"], dv["D"], g=dv["g"] if gga else None, Q=dv["Q"], F=dv["F"], b0=b0, b1=b1)
+                    if stress:
+                        ctx.pulay_forces_stress(dv["v"], dv["D"], g=dv["g"] if gga else None, Q=dv["Q"], volume=1.0,
+                                                F=dv["F"], sigma=dv["SG"], b0=b0, b1=b1)
+                    else:
+                        ctx.pulay_forces(dv["v"], dv["D"], g=dv["g"] if gga else None, Q=dv["Q"], F=dv["F"], b0=b0, b1=b1)
                     if world > 1:
                         dist.all_reduce(dv["F"])
+                        if stress:
+                            dist.all_reduce(dv["SG"])
                     hb["F"].copy_(dv["F"], non_blocking=True)
+                    if stress:
+                        hb["SG"].copy_(dv["SG"], non_blocking=True)
                     return
                 ctx.integrate_hamiltonian(dv["v"], dv["g"] if gga else None, H=dv["H"], b0=b0, b1=b1, accumulate=False,
                                           kinetic=kin)
@@ -369,7 +390,7 @@ def main():
         h2d = 8 * (bun.n_points + bun.n_values + (3 * bun.n_points if gga else 0))
         d2h = 8 * (bun.n_values + my_points * (4 if gga else 1))
         if forces:
-            h2d, d2h = h2d + 8 * bun.n_values, 8 * 3 * bun.n_atoms
+            h2d, d2h = h2d + 8 * bun.n_values, 8 * (3 * bun.n_atoms + (9 if stress else 0))
         if hessian:
             h2d, d2h = 8 * bun.n_values, 8 * 6 * my_points
         e2e = {"value": bun.n_points / (ms_e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
@@ -452,7 +473,7 @@ def main():
         sel = sample_batches(bun.n_batches, args.cpu_sample_batches)
         if hessian:
             sel = sel[:32]
-        pts, dt, cores = time_oracle(bun, sel, gga, forces_q=Qh, kinetic=kin and not forces and not hessian, hessian=hessian)
+        pts, dt, cores = time_oracle(bun, sel, gga, forces_q=Qh, kinetic=kin and not forces and not hessian, hessian=hessian, stress=stress)
         out["cpu_baseline"] = {"value": pts / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
                                "sample": "%d seeded batches (%d points) of the same workload, %.1f s" % (len(sel), pts, dt)}
     else:

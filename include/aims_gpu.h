@@ -179,6 +179,22 @@ int aims_gpu_pulay_forces(aims_gpu_ctx *ctx, int32_t b0, int32_t b1, const doubl
 int aims_gpu_pulay_forces_ks(aims_gpu_ctx *ctx, int32_t b0, int32_t b1, const double *v, const double *g, int kinetic,
                              const double *D_values, const double *Q_values, double *F, int accumulate);
 
+/* Row f1 of SURVEY.md 8(f), stress: the Pulay contribution to the stress tensor, evaluated in the same pass as the Pulay
+ * forces (Eq. 20: sigma_lm = (1/V) dE_tot/d eps_lm; L299-308; L405 "the Pulay contribution to F_at and
+ * sigma_lm"; Table 2 "SCF+F+sigma").  The paper defers the terms to its Ref. [83]; reading P22 takes Eq. 20 itself:
+ * under a homogeneous strain r -> (1 + eps) r of atoms and grid points, at fixed n_ij, q_ij and fixed point values v_p, g_p, w_p,
+ *   sigma[l][m] (+)= (2 / volume) sum_{p in batches [b0,b1)} w_p sum_i (r_p - R_at(i))_m
+ *        { d_l phi_i [ sum_j n_ij (h_KS phi_j) - q_ij phi_j ]  +  (Hess phi_i g_p)_l sum_j n_ij phi_j }   (at r_p),
+ * = (1/volume) d/d eps_lm [ Tr(n h(eps)) - Tr(q s(eps)) ], i.e. the force integrand weighted with the distance vector to the
+ * function's own atom; (h_KS phi_j) = v phi_j + g.grad phi_j (- 1/2 lap phi_j if kinetic != 0) as in aims_gpu_pulay_forces_ks.
+ * Point-attached fields do not co-rotate, so sigma need not be symmetric: all nine components are returned.
+ * volume: the cell volume V (> 0; pass 1 for a cluster to obtain dE/d eps).  DEVICE pointers as in aims_gpu_pulay_forces_ks,
+ * plus sigma [3][3]; F may be NULL (stress only).  accumulate == 0: F and sigma are zeroed first.  Accumulated with
+ * floating-point atomics (reruns agree to rounding). */
+int aims_gpu_pulay_forces_stress(aims_gpu_ctx *ctx, int32_t b0, int32_t b1, const double *v, const double *g, int kinetic,
+                                 const double *D_values, const double *Q_values, double volume, double *F, double *sigma,
+                                 int accumulate);
+
 /* Row f4 of SURVEY.md 8(f): the partition-of-unity factor of the integration weights w(r) (Eq. 21-22; the
  * paper cites "a modified version of the partition function proposed by Stratmann et al." without writing it out; DESIGN.md
  * reading P5 takes the textbook Stratmann-Scuseria-Frisch cell function with a = 0.64, restricted to the atoms within r_part

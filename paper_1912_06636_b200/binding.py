@@ -93,6 +93,9 @@ def load_library():
     L.aims_gpu_pulay_forces.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp, _vp, _vp, _vp, ctypes.c_int]
     L.aims_gpu_pulay_forces_ks.restype = ctypes.c_int
     L.aims_gpu_pulay_forces_ks.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp, ctypes.c_int, _vp, _vp, _vp, ctypes.c_int]
+    L.aims_gpu_pulay_forces_stress.restype = ctypes.c_int
+    L.aims_gpu_pulay_forces_stress.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp, ctypes.c_int, _vp, _vp,
+                                               ctypes.c_double, _vp, _vp, ctypes.c_int]
     L.aims_gpu_synchronize.restype = ctypes.c_int
     L.aims_gpu_synchronize.argtypes = [cp]
     L.aims_gpu_set_deterministic.restype = ctypes.c_int
@@ -384,6 +387,34 @@ class Context:
                                                  int(bool(accumulate))), "aims_gpu_pulay_forces")
         return F
 
+    def pulay_forces_stress(self, v, D, g=None, Q=None, volume=1.0, F=None, sigma=None, b0=0, b1=None, accumulate=False,
+                            kinetic=False, want_forces=True):
+        """(F[n_atoms][3] | None, sigma[3][3]) device tensors (include/aims_gpu.h: aims_gpu_pulay_forces_stress)."""
+        torch = self.torch
+        b0, b1 = self._range(b0, b1)
+        v = self._dev(v, torch.float64)
+        D = self._dev(D, torch.float64)
+        g = None if g is None else self._dev(g, torch.float64)
+        Q = None if Q is None else self._dev(Q, torch.float64)
+        if v.numel() != self.n_points or (g is not None and g.numel() != 3 * self.n_points):
+            raise AimsError("v must have n_points entries and g 3*n_points")
+        if D.numel() != self.n_values or (Q is not None and Q.numel() != self.n_values):
+            raise AimsError("D and Q must have n_values entries")
+        with torch.cuda.stream(self.stream):
+            if sigma is None:
+                sigma = torch.zeros((3, 3), dtype=torch.float64, device=self.device)
+                fresh = True
+            else:
+                fresh = False
+            if F is None and want_forces:
+                F = torch.zeros((self.n_atoms, 3), dtype=torch.float64, device=self.device)
+            elif fresh and not accumulate and F is not None:
+                pass
+        self._check(self.L.aims_gpu_pulay_forces_stress(self.h, b0, b1, _ptr(v), _ptr(g), int(bool(kinetic)), _ptr(D), _ptr(Q),
+                                                        float(volume), _ptr(F), _ptr(sigma), int(bool(accumulate))),
+                    "aims_gpu_pulay_forces_stress")
+        return F, sigma
+
     # ---- end-to-end with HOST buffers (pinned): H2D of v, g, D; the two calls; D2H of H, n, grad n
     def make_host_buffers(self, want_grad):
         torch = self.torch
@@ -459,6 +490,11 @@ def aims_gpu_density_hessian(ctx, D, hess_n=None, b0=0, b1=None):
 
 def aims_gpu_pulay_forces(ctx, v, D, g=None, Q=None, F=None, b0=0, b1=None, accumulate=False):
     return ctx.pulay_forces(v, D, g, Q, F, b0, b1, accumulate)
+
+
+def aims_gpu_pulay_forces_stress(ctx, v, D, g=None, kinetic=False, Q=None, volume=1.0, F=None, sigma=None, b0=0, b1=None,
+                                 accumulate=False):
+    return ctx.pulay_forces_stress(v, D, g, Q, volume, F, sigma, b0, b1, accumulate, kinetic)
 
 
 def aims_gpu_pulay_forces_ks(ctx, v, D, g=None, kinetic=True, Q=None, F=None, b0=0, b1=None, accumulate=False):

@@ -248,7 +248,8 @@ cudaError_t smem_optin_all(int device, size_t optin) {
   AIMS_OPTIN(k_hamiltonian<false>) AIMS_OPTIN(k_hamiltonian<true>)
   AIMS_OPTIN(k_density<false>) AIMS_OPTIN(k_density<true>)
   AIMS_OPTIN(k_density_hessian)
-  AIMS_OPTIN(k_forces<false>) AIMS_OPTIN(k_forces<true>)
+  AIMS_OPTIN((k_forces<false, false>)) AIMS_OPTIN((k_forces<true, false>))
+  AIMS_OPTIN((k_forces<false, true>)) AIMS_OPTIN((k_forces<true, true>))
 #define AIMS_OPTIN_EV(M, LY) AIMS_OPTIN((k_eval<M, LY>))
   AIMS_OPTIN_EV(kEvalPhi, kLayApi) AIMS_OPTIN_EV(kEvalPhiGrad, kLayApi) AIMS_OPTIN_EV(kEvalHLda, kLayH)
   AIMS_OPTIN_EV(kEvalHGga, kLayH) AIMS_OPTIN_EV(kEvalHKinLda, kLayH) AIMS_OPTIN_EV(kEvalHKinGga, kLayH)
@@ -751,11 +752,14 @@ static int impl_update_density(aims_gpu_ctx *c, int32_t b0, int32_t b1, const do
 }
 
 static int run_forces(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, const double *g, int kinetic,
-                      const double *D_values, const double *Q_values, double *F, int accumulate) {
+                      const double *D_values, const double *Q_values, double *F, int accumulate, double *sigma = nullptr,
+                      double volume = 1.0) {
   if (!range_ok(c, b0, b1)) return fail(c, AIMS_ERR_INVALID_ARG, "batch range outside [0, n_batches]");
-  if ((!v && c->n_points) || !D_values || !F) return fail(c, AIMS_ERR_INVALID_ARG, "NULL v, D_values or F");
+  if ((!v && c->n_points) || !D_values || (!F && !sigma)) return fail(c, AIMS_ERR_INVALID_ARG, "NULL v, D_values or F");
+  if (sigma && !(volume > 0.0)) return fail(c, AIMS_ERR_INVALID_ARG, "volume must be positive");
   CU_TRY(c, cudaSetDevice(c->device));
-  if (!accumulate) CU_TRY(c, cudaMemsetAsync(F, 0, (size_t)c->S.n_atoms * 3 * sizeof(double), c->stream));
+  if (!accumulate && F) CU_TRY(c, cudaMemsetAsync(F, 0, (size_t)c->S.n_atoms * 3 * sizeof(double), c->stream));
+  if (!accumulate && sigma) CU_TRY(c, cudaMemsetAsync(sigma, 0, 9 * sizeof(double), c->stream));
   int rc = run_cull(c, b0, b1);
   if (rc) return rc;
   const int npl = g ? 8 : 5;
@@ -779,9 +783,16 @@ static int run_forces(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, 
       A.pad_off = c->d_dpad_off; A.pad_base = c->dpad_off[bs];
       A.D = D_values; A.Q = Q_values; A.F = F; A.max_nnz_pad = c->max_nnz;
       A.ptab_in_smem = c->f_ptab_in_smem ? 1 : 0;
+      A.sigma = sigma; A.inv_volume = 1.0 / volume;
       TimedLaunch t(c, kKindForce);
-      if (g) k_forces<true><<<(unsigned)ni, kDThreads, fsm, c->stream>>>(c->S, c->L, A, std::max(c->max_act, 1));
-      else k_forces<false><<<(unsigned)ni, kDThreads, fsm, c->stream>>>(c->S, c->L, A, std::max(c->max_act, 1));
+      const int mact = std::max(c->max_act, 1);
+      if (sigma) {
+        if (g) k_forces<true, true><<<(unsigned)ni, kDThreads, fsm, c->stream>>>(c->S, c->L, A, mact);
+        else k_forces<false, true><<<(unsigned)ni, kDThreads, fsm, c->stream>>>(c->S, c->L, A, mact);
+      } else {
+        if (g) k_forces<true, false><<<(unsigned)ni, kDThreads, fsm, c->stream>>>(c->S, c->L, A, mact);
+        else k_forces<false, false><<<(unsigned)ni, kDThreads, fsm, c->stream>>>(c->S, c->L, A, mact);
+      }
     }
     if ((rc = check_async(c))) return rc;
     bs = be;
@@ -896,6 +907,13 @@ static int impl_set_deterministic(aims_gpu_ctx *c, int enable) {
   if (!c) return AIMS_ERR_INVALID_ARG;
   c->deterministic = enable != 0;
   return AIMS_OK;
+}
+
+static int impl_pulay_forces_stress(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, const double *g, int kinetic,
+                                    const double *D_values, const double *Q_values, double volume, double *F, double *sigma,
+                                    int accumulate) {
+  if (!sigma) return fail(c, AIMS_ERR_INVALID_ARG, "NULL sigma");
+  return run_forces(c, b0, b1, v, g, kinetic, D_values, Q_values, F, accumulate, sigma, volume);
 }
 
 static int impl_timing_enable(aims_gpu_ctx *c, int enable) {
@@ -1054,6 +1072,10 @@ int aims_gpu_pulay_forces(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double 
 
 int aims_gpu_pulay_forces_ks(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, const double *g, int kinetic, const double *D_values, const double *Q_values, double *F, int accumulate) {
   return guarded(c, [&] { return impl_pulay_forces_ks(c, b0, b1, v, g, kinetic, D_values, Q_values, F, accumulate); });
+}
+
+int aims_gpu_pulay_forces_stress(aims_gpu_ctx *c, int32_t b0, int32_t b1, const double *v, const double *g, int kinetic, const double *D_values, const double *Q_values, double volume, double *F, double *sigma, int accumulate) {
+  return guarded(c, [&] { return impl_pulay_forces_stress(c, b0, b1, v, g, kinetic, D_values, Q_values, volume, F, sigma, accumulate); });
 }
 
 int aims_gpu_set_deterministic(aims_gpu_ctx *c, int enable) {

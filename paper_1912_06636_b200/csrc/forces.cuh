@@ -30,23 +30,32 @@ struct FArgs {
   double *F;                        // [n_atoms][3]
   int max_nnz_pad;                  // capacity of the fn_info smem array
   int ptab_in_smem;
+  double *sigma;                    // STRESS only: [3][3], sigma[l][m] += (1/V) dE/d eps_lm of the launch's batches
+  double inv_volume;
 };
 
 inline size_t f_smem_bytes(int max_nnz, int max_act, bool ptab_in_smem) {
   size_t s = (size_t)kDStages * kDStage * sizeof(double);
-  s += (size_t)kMaxActive * 3 * sizeof(double);               // per-CTA force table [slot][3]
+  s += (size_t)(kMaxActive * 3 + 16) * sizeof(double);        // per-CTA force table [slot][3] + stress sums [3][3]
   s += 2 * kDStages * sizeof(unsigned long long);             // full / empty barriers
   if (ptab_in_smem) s += (size_t)max_act * max_act * sizeof(long long);
   s += (size_t)pad8(max_nnz) * sizeof(int) + (size_t)kMaxActive * sizeof(int);
   return s;
 }
 
-template <bool GGA>
+// STRESS: additionally the Pulay part of the stress tensor (Eq. 20; L299-308; L405 "the Pulay contribution
+// to F_at and sigma_lm"): the same integrand weighted with the distance vector to the function's own atom (DESIGN.md reading
+// P22),  V sigma_lm = 2 sum_p sum_i (r_p - R_at(i))_m [ ... ]_l .  Written relative to a reference point c of the batch,
+//   sum_i sum_p (r_p - c)_m [...]_l  -  sum_slots (R_slot - c)_m sF[slot][l] ,
+// the first sum needs no per-atom separation (nine more accumulators per lane, weighted with the lane's two points) and the
+// second comes from the CTA's force table; both terms are of the size of the batch, so nothing cancels.
+template <bool GGA, bool STRESS>
 __global__ void __launch_bounds__(kDThreads, 1) k_forces(DevSys S, BatchLists L, FArgs A, int max_act) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   double *sA = reinterpret_cast<double *>(smem_raw);                     // stage s: [k4][tm][4] at sA + s * kDStage
   double *sF = sA + (size_t)kDStages * kDStage;                          // [slot][3]
-  unsigned long long *s_bar = reinterpret_cast<unsigned long long *>(sF + kMaxActive * 3);
+  double *sG = sF + kMaxActive * 3;                                      // [3][3] (STRESS)
+  unsigned long long *s_bar = reinterpret_cast<unsigned long long *>(sG + 16);
   int *sInfo = reinterpret_cast<int *>(s_bar + 2 * kDStages);           // 16-byte aligned; [pad8(max nnz)]
   int *sLd = sInfo + pad8(A.max_nnz_pad);
   long long *sPtab = reinterpret_cast<long long *>(sLd + kMaxActive);
@@ -75,7 +84,10 @@ __global__ void __launch_bounds__(kDThreads, 1) k_forces(DevSys S, BatchLists L,
   for (int i = tid; i < nact; i += kDThreads) sLd[i] = L.act_ld[ao + i];
   if (A.ptab_in_smem)
     for (int i = tid; i < nact * nact; i += kDThreads) sPtab[i] = gptab[i];
-  for (int i = tid; i < kMaxActive * 3; i += kDThreads) sF[i] = 0.0;
+  for (int i = tid; i < kMaxActive * 3 + 16; i += kDThreads) sF[i] = 0.0;
+  const long long pbase = S.batch_ptr[b];
+  double cref[3] = {0.0, 0.0, 0.0};                      // reference point of the batch (STRESS): its first point
+  if (STRESS && np > 0) { cref[0] = S.px[pbase]; cref[1] = S.py[pbase]; cref[2] = S.pz[pbase]; }
   const unsigned bar_full = smem_u32(s_bar), bar_empty = bar_full + 8 * kDStages;
   __shared__ int s_map[kDMmaWarps];
   if (tid == 0) {
@@ -144,6 +156,11 @@ __global__ void __launch_bounds__(kDThreads, 1) k_forces(DevSys S, BatchLists L,
     for (int a = 0; a < 4; a++)
 #pragma unroll
       for (int c = 0; c < 4; c++) { acc[a][c][0] = 0.0; acc[a][c][1] = 0.0; }
+    double G[STRESS ? 3 : 1][3];                         // sum over rows and points of (r_p - c)_m [...]_l
+#pragma unroll
+    for (int l = 0; l < (STRESS ? 3 : 1); l++)
+#pragma unroll
+      for (int m = 0; m < 3; m++) G[l][m] = 0.0;
 
     int step = 0;
 #pragma unroll 1
@@ -183,6 +200,15 @@ __global__ void __launch_bounds__(kDThreads, 1) k_forces(DevSys S, BatchLists L,
               for (int c = 0; c < 4; c++) {
                 if (c < wb) {
                   const int p = p0 + ps0 + c * 8 + 2 * fk;           // within the batch (even)
+                  double rp[STRESS ? 2 : 1][3];                       // the lane's two points relative to the reference
+                  if (STRESS) {
+#pragma unroll
+                    for (int e = 0; e < 2; e++) {
+                      const long long pg = pbase + min(p + e, np - 1);   // padding points: planes are zero there
+                      rp[STRESS ? e : 0][0] = S.px[pg] - cref[0]; rp[STRESS ? e : 0][1] = S.py[pg] - cref[1];
+                      rp[STRESS ? e : 0][2] = S.pz[pg] - cref[2];
+                    }
+                  }
                   double2 ev[2][3];
 #pragma unroll
                   for (int da = 0; da < 2; da++) {
@@ -194,8 +220,18 @@ __global__ void __launch_bounds__(kDThreads, 1) k_forces(DevSys S, BatchLists L,
 #pragma unroll
                   for (int da = 0; da < 2; da++)
 #pragma unroll
-                    for (int q = 0; q < 3; q++)
-                      f[da][q] += ev[da][q].x * acc[min(a0 + da, 3)][c][0] + ev[da][q].y * acc[min(a0 + da, 3)][c][1];
+                    for (int q = 0; q < 3; q++) {
+                      if (!STRESS) {
+                        f[da][q] += ev[da][q].x * acc[min(a0 + da, 3)][c][0] + ev[da][q].y * acc[min(a0 + da, 3)][c][1];
+                      } else {
+                        const double t0 = ev[da][q].x * acc[min(a0 + da, 3)][c][0], t1 = ev[da][q].y * acc[min(a0 + da, 3)][c][1];
+                        f[da][q] += t0 + t1;
+                        if (a0 + da < wa) {                            // the clamped duplicate row must not count twice
+#pragma unroll
+                          for (int m = 0; m < 3; m++) G[STRESS ? q : 0][m] += t0 * rp[0][m] + t1 * rp[STRESS ? 1 : 0][m];
+                        }
+                      }
+                    }
                 }
               }
 #pragma unroll
@@ -218,13 +254,31 @@ __global__ void __launch_bounds__(kDThreads, 1) k_forces(DevSys S, BatchLists L,
           for (int c = 0; c < 4; c++) { acc[a][c][0] = 0.0; acc[a][c][1] = 0.0; }
       }
     }
+    if (STRESS) {
+#pragma unroll
+      for (int l = 0; l < 3; l++)
+#pragma unroll
+        for (int m = 0; m < 3; m++) {
+          double u = G[STRESS ? l : 0][m];
+#pragma unroll
+          for (int o = 16; o > 0; o >>= 1) u += __shfl_xor_sync(0xffffffffu, u, o);
+          if (lane == 0) atomicAdd(sG + 3 * l + m, u);
+        }
+    }
   }
   __syncthreads();
 
   // ---- the CTA's contribution to F: nact x 3 numbers (factor 2 of Eq. 16/18: both index orders of the symmetric sums)
-  for (int i = tid; i < nact * 3; i += kDThreads) {
-    const int s = i / 3, q = i - 3 * s;
-    red_add_f64(A.F + (long long)L.act_atom[ao + s] * 3 + q, 2.0 * sF[i]);
+  if (A.F)
+    for (int i = tid; i < nact * 3; i += kDThreads) {
+      const int s = i / 3, q = i - 3 * s;
+      red_add_f64(A.F + (long long)L.act_atom[ao + s] * 3 + q, 2.0 * sF[i]);
+    }
+  if (STRESS && tid < 9) {
+    const int l = tid / 3, m = tid - 3 * l;
+    double u = sG[tid];
+    for (int s = 0; s < nact; s++) u -= (S.atom_xyz[3 * L.act_atom[ao + s] + m] - cref[m]) * sF[3 * s + l];
+    red_add_f64(A.sigma + tid, 2.0 * u * A.inv_volume);
   }
 }
 

@@ -130,3 +130,55 @@ def test_gpu_forces_are_the_energy_gradient_of_gpu_H_and_S():
         bm.atom_xyz[at, c] -= h
         fd = -(energy(bp) - energy(bm)) / (2 * h)
         assert abs(fd - F[at, c]) <= 2e-6 * scale, (at, c, fd, F[at, c])
+
+
+# ---------------------------------------------------------------------------------------------------------------------
+# Pulay stress (row f1, second half; Eq. 20): aims_gpu_pulay_forces_stress
+# ---------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("mode", ["lda", "lda_q", "gga", "gga_q", "gga_q_kin"])
+def test_stress_and_forces_match_oracle(case, mode):
+    name, bun, orc, ctx, Q = case
+    g = bun.g if mode.startswith("gga") else None
+    q = Q if "_q" in mode else None
+    kin = mode.endswith("_kin")
+    vol = 37.5
+    F, sig = ctx.pulay_forces_stress(bun.v, bun.D_values, g=g, Q=q, volume=vol, kinetic=kin)
+    ctx.synchronize()
+    ref = orc.pulay_stress(bun.v, bun.D_values, g=g, Q_values=q, kinetic=kin, volume=vol)
+    assert sig.shape == (3, 3)
+    assert _rel_max(sig.cpu().numpy(), ref) <= TOL_F
+    assert _rel_max(F.cpu().numpy(), orc.pulay_forces(bun.v, bun.D_values, g=g, Q_values=q, kinetic=kin)) <= TOL_F
+
+
+def test_stress_only_subranges_and_accumulation(case):
+    import torch
+    name, bun, orc, ctx, Q = case
+    mid = bun.n_batches // 2
+    sig = torch.zeros((3, 3), dtype=torch.float64, device="cuda")
+    F = torch.zeros((bun.n_atoms, 3), dtype=torch.float64, device="cuda")
+    ctx.pulay_forces_stress(bun.v, bun.D_values, g=bun.g, Q=Q, F=F, sigma=sig, b0=0, b1=mid, accumulate=True)
+    ctx.pulay_forces_stress(bun.v, bun.D_values, g=bun.g, Q=Q, F=None, sigma=sig, b0=mid, b1=None, accumulate=True,
+                            want_forces=False)                                    # stress only: F = NULL
+    ctx.synchronize()
+    assert _rel_max(sig.cpu().numpy(), orc.pulay_stress(bun.v, bun.D_values, g=bun.g, Q_values=Q)) <= TOL_F
+    assert _rel_max(F.cpu().numpy(), orc.pulay_forces(bun.v, bun.D_values, g=bun.g, Q_values=Q, batches=np.arange(0, mid))) <= TOL_F
+    import paper_1912_06636_b200 as aims
+    with pytest.raises(aims.AimsError):
+        ctx.pulay_forces_stress(bun.v, bun.D_values, volume=0.0)
+
+
+def test_stress_far_from_the_origin_loses_nothing():
+    """The kernel sums (r_p - c) and (R_at - c) relative to a point of the batch: translating the whole system by 1000 A must
+    not cost digits beyond the rounding of the translated coordinates themselves."""
+    bun = aims_synth.make_config(5, n_rad=8, n_ang=26, keep_atoms=12)
+    Q = make_q_values(bun)
+    t = np.array([1024.0, -2048.0, 512.0])                     # exactly representable shifts
+    far = copy.copy(bun)
+    far.atom_xyz = np.ascontiguousarray(bun.atom_xyz + t)
+    far.xyz = np.ascontiguousarray(bun.xyz + t)
+    ctx = _ctx(far)
+    _, sig = ctx.pulay_forces_stress(far.v, far.D_values, g=far.g, Q=Q)
+    ctx.synchronize()
+    ref = Oracle(far).pulay_stress(far.v, far.D_values, g=far.g, Q_values=Q)
+    assert _rel_max(sig.cpu().numpy(), ref) <= TOL_F
+    ctx.close()
