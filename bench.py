@@ -58,6 +58,8 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--path", default="scf", choices=["scf", "forces", "stress", "hessian"])
+    ap.add_argument("--deterministic", action="store_true",
+                    help="ordered (bitwise reproducible) scatter into H: aims_gpu_set_deterministic")
     ap.add_argument("--kinetic", action="store_true",
                     help="scf path with the full h_KS phi (kinetic term, row f2): a separate line, not the headline metric")
     return ap.parse_args()
@@ -153,6 +155,51 @@ def time_oracle(bun, batches, gga, repeats=1, forces_q=None, kinetic=False, hess
     return pts, best, orc.num_threads()
 
 
+def time_blas_baseline(bun, batches, gga):
+    """Paper-style CPU path (Fig. 6 CPU column, PAPER.md L319-329 / L353-363): per-batch DSYR2K / DSYMM-shaped products
+    through numpy's BLAS on the host cores (oracle/blas_baseline.py), same batches as the oracle sample."""
+    from oracle.blas_baseline import BlasBaseline
+    bl = BlasBaseline(bun)
+    Dd = bl.dense(bun.D_values)                              # set-up (the paper's loops start from the sparse n_ij too)
+    Hd = np.zeros((bl.nb, bl.nb))
+    pts = int(sum(bun.batch_ptr[b + 1] - bun.batch_ptr[b] for b in batches))
+    t0 = time.perf_counter()
+    bl.hamiltonian_dense(bun.v, bun.g if gga else None, batches=batches, out=Hd)
+    bl.density(Dd, want_grad=gga, batches=batches)
+    return pts, time.perf_counter() - t0
+
+
+def kernel_sources_sha():
+    """sha256 over the CUDA sources: profiles/*_traffic.txt records the hash its ncu capture was taken at."""
+    import hashlib
+    d = os.path.join(ROOT, "paper_1912_06636_b200", "csrc")
+    h = hashlib.sha256()
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh")):
+            with open(os.path.join(d, f), "rb") as fh:
+                h.update(f.encode() + b"\0" + fh.read())
+    return h.hexdigest()[:16]
+
+
+def committed_traffic(kernel, workload_key):
+    """DRAM bytes per launch of `kernel` from the committed `ncu --set full` summary (profiles/r02_traffic.txt, one JSON
+    object), or (None, why) when the capture was taken from other kernel sources than the ones this run loaded."""
+    path = os.path.join(ROOT, "profiles", "r02_traffic.txt")
+    try:
+        with open(path) as f:
+            rec = json.load(f)
+    except Exception:
+        return None, "no committed ncu capture (profiles/r02_traffic.txt)"
+    if rec.get("kernel_sources_sha") != kernel_sources_sha():
+        return None, "committed ncu capture was taken at kernel sources %s, this run has %s" % (
+            rec.get("kernel_sources_sha"), kernel_sources_sha())
+    val = rec.get("traffic", {}).get(workload_key, {}).get(kernel)
+    if val is None:
+        return None, "no capture of %s for %s in profiles/r02_traffic.txt" % (kernel, workload_key)
+    return float(val), "dram__bytes_read.sum + dram__bytes_write.sum of one launch, %s (commit %s)" % (
+        rec.get("source", "profiles/r02_traffic.txt"), rec.get("commit"))
+
+
 def run_reference(args, bun, gga, workload, metric, forces_q=None, hessian=False, stress=False):
     """--impl reference: the CPU oracle, rank 0 only, a bounded sample per step."""
     per_step = max(4, args.cpu_sample_batches // 4)
@@ -227,6 +274,8 @@ def main():
     t_create = time.time()
     ctx = aims.aims_gpu_create(bun, device=local_rank, stream=stream)
     t_create = time.time() - t_create
+    if args.deterministic:
+        ctx.set_deterministic(True)
     st = ctx.stats()
     nnz = ctx.batch_nnz().astype(np.float64)
     npb = np.diff(bun.batch_ptr).astype(np.float64)
@@ -429,11 +478,13 @@ def main():
                 "avg_launch_ms": dom_ms / max(dom_ln, 1), "algorithmic_flops_per_step": kflops[dom],
                 "share_of_step": dom_ms / ms_total}
     total_tflops = (flops_x if hessian else flops_f if forces else flops_h + flops_n) / (ms_step * 1e-3) / 1e12
-    # DRAM traffic per launch of the dominant kernel from the committed `ncu --set full` capture (config 5 only)
-    if args.config == 5 and not (args.max_batch or args.n_rad or args.n_ang) and world == 1:
-        roofline["traffic"] = {"k_density": 125.75e9, "k_hamiltonian": 28.46e9, "k_forces": 152.29e9}.get(dom)
-        roofline["traffic_note"] = ("dram__bytes_read.sum + dram__bytes_write.sum of one launch (bytes), "
-                                    "profiles/r01_ncu_full_config5.md; Phi-plane bytes consumed per launch: 25.8e9")
+    # DRAM traffic per launch of the dominant kernel: read from the committed `ncu --set full` summary, and only if that
+    # capture was taken from the kernel sources this run loaded (otherwise null, with the reason)
+    wkey = "config%d%s" % (args.config, "" if not (args.max_batch or args.n_rad or args.n_ang) else "_variant")
+    if world == 1:
+        roofline["traffic"], roofline["traffic_note"] = committed_traffic(dom, wkey)
+    roofline["algorithmic_bytes_note"] = ("compulsory HBM bytes of the dominant contraction are ~1 GB per step (points, v, g, D, H, "
+                                          "n, grad n); it is bound by the FP64 tensor pipe, so `achieved` is in flops")
     # second roofline: the HBM-bound evaluation kernel (algorithmic bytes = 8 B x planes x padded rows x padded points)
     pad = lambda a, m: np.ceil(a / m) * m                                   # noqa: E731
     pl_h, pl_d = 2.0, (4.0 if gga else 1.0)
@@ -461,6 +512,11 @@ def main():
            "data": "synthetic",
            "config": {"workload": workload, "n_points": bun.n_points, "n_batches": bun.n_batches, "n_basis": bun.n_basis,
                       "mean_nnz": float(nnz.mean()) if len(nnz) else 0.0, "max_nnz": st["max_nnz"],
+                      # workload metric of the paper, Eq. 31: #B x <|B|> x <nnz>^2, and the exact sum it models
+                      "eq31_ops": float(len(nnz) * npb.mean() * nnz.mean() ** 2) if len(nnz) else 0.0,
+                      "sum_np_nnz2": float((npb * nnz * nnz).sum()),
+                      "ms_per_eq31_gops": (ms_step / (len(nnz) * npb.mean() * nnz.mean() ** 2 * 1e-9)) if len(nnz) else None,
+                      "deterministic_H": bool(args.deterministic),
                       "max_active_atoms": st["max_active_atoms"], "parallelism": "batch-range x%d" % world,
                       "l2": "inputs larger than L2: each step streams %.1f GB of Phi planes plus a %.2f GB H and D"
                             % (1e-9 * eval_bytes, 8e-9 * bun.n_values)},
@@ -476,6 +532,11 @@ def main():
         pts, dt, cores = time_oracle(bun, sel, gga, forces_q=Qh, kinetic=kin and not forces and not hessian, hessian=hessian, stress=stress)
         out["cpu_baseline"] = {"value": pts / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
                                "sample": "%d seeded batches (%d points) of the same workload, %.1f s" % (len(sel), pts, dt)}
+        if not forces and not hessian and not kin:
+            # second, fairer CPU number: the paper's own CPU path, per-batch BLAS through numpy
+            pts2, dt2 = time_blas_baseline(bun, sel, gga)
+            out["cpu_baseline_blas"] = {"value": pts2 / dt2, "unit": UNIT, "cores": cores, "kind": "per-batch BLAS (numpy dgemm), Fig. 6 CPU column",
+                                        "sample": "%d seeded batches (%d points) of the same workload, %.1f s" % (len(sel), pts2, dt2)}
     else:
         out["cpu_baseline"] = None
     if rank == 0:
