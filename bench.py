@@ -65,16 +65,7 @@ def parse():
     return ap.parse_args()
 
 
-def partition_batches(cost, n_parts):
-    """Contiguous ranges [lo, hi) of (almost) equal total cost; cost[b] >= 0.  Pure host logic (tested on CPU)."""
-    nb = len(cost)
-    csum = np.concatenate([[0.0], np.cumsum(np.asarray(cost, dtype=np.float64))])
-    bounds = [0]
-    for r in range(1, n_parts):
-        target = csum[-1] * r / n_parts
-        bounds.append(int(np.clip(np.searchsorted(csum, target, side="left"), bounds[-1], nb)))
-    bounds.append(nb)
-    return [(bounds[r], bounds[r + 1]) for r in range(n_parts)]
+from paper_1912_06636_b200.sharding import first_phase_range, partition_batches, slice_bundle  # noqa: E402
 
 
 class ClockSampler:
@@ -268,20 +259,41 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
     t_gen = time.time()
-    bun = aims_synth.make_config(args.config, n_rad=args.n_rad, n_ang=args.n_ang, max_batch=args.max_batch)
+    # synthetic input generation (not the product): every rank generates the system, then keeps only its own batches
+    full = aims_synth.make_config(args.config, n_rad=args.n_rad, n_ang=args.n_ang, max_batch=args.max_batch)
     t_gen = time.time() - t_gen
+    n_points_total, n_batches_total = full.n_points, full.n_batches
     stream = torch.cuda.Stream(device=local_rank)
     t_create = time.time()
-    ctx = aims.aims_gpu_create(bun, device=local_rank, stream=stream)
+    npb_all = np.diff(full.batch_ptr).astype(np.float64)
+    if world == 1:
+        bun = full
+        ctx = aims.aims_gpu_create(bun, device=local_rank, stream=stream)
+        nnz_all = ctx.batch_nnz().astype(np.float64)
+        g0, g1 = 0, full.n_batches
+    else:
+        # "at no time does any process know the full grid" -- a rank's context holds its own batches only.
+        # 1. cost probe on an equal-count slice  2. one tiny all-reduce of |nnz(B)|  3. balanced contiguous ranges
+        p0, p1 = first_phase_range(full.n_batches, rank, world)
+        probe_bun, _, _ = slice_bundle(full, p0, p1)
+        probe = aims.aims_gpu_create(probe_bun, device=local_rank, stream=stream, workspace_bytes=1)
+        nnz_t = torch.zeros(full.n_batches, dtype=torch.int32, device="cuda")
+        nnz_t[p0:p1] = torch.as_tensor(probe.batch_nnz()).cuda()
+        probe.close()
+        dist.all_reduce(nnz_t)
+        nnz_all = nnz_t.cpu().numpy().astype(np.float64)
+        g0, g1 = partition_batches(npb_all * nnz_all * nnz_all, world)[rank]
+        bun, _, _ = slice_bundle(full, g0, g1)
+        ctx = aims.aims_gpu_create(bun, device=local_rank, stream=stream)
+    del full
     t_create = time.time() - t_create
     if args.deterministic:
         ctx.set_deterministic(True)
     st = ctx.stats()
-    nnz = ctx.batch_nnz().astype(np.float64)
-    npb = np.diff(bun.batch_ptr).astype(np.float64)
-    cost = npb * nnz * nnz
-    b0, b1 = partition_batches(cost, world)[rank]
-    my_points = int(bun.batch_ptr[b1] - bun.batch_ptr[b0])
+    nnz = nnz_all[g0:g1]                           # this rank's batches; b0, b1 index the rank's own context
+    npb = npb_all[g0:g1]
+    b0, b1 = 0, bun.n_batches
+    my_points = int(bun.n_points)
     syr2k = gga or bool(args.kinetic)            # Q not proportional to P: one full product, symmetrised
     flops_h = float(((2.0 if syr2k else 1.0) * npb * nnz * (nnz + (0.0 if syr2k else 1.0)))[b0:b1].sum())
     flops_n = float((2.0 * npb * nnz * nnz)[b0:b1].sum())
@@ -363,7 +375,7 @@ def main():
         dist.all_reduce(lt)
         launches = int(lt.item())
     ms_step = ms_total / args.steps
-    value = bun.n_points / (ms_step * 1e-3)
+    value = n_points_total / (ms_step * 1e-3)
 
     # ---- e2e: same step through the binding with pinned HOST buffers, copies inside the timed region
     e2e = None
@@ -442,7 +454,7 @@ def main():
             h2d, d2h = h2d + 8 * bun.n_values, 8 * (3 * bun.n_atoms + (9 if stress else 0))
         if hessian:
             h2d, d2h = 8 * bun.n_values, 8 * 6 * my_points
-        e2e = {"value": bun.n_points / (ms_e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+        e2e = {"value": n_points_total / (ms_e * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                "d2h_bytes_per_step": int(d2h), "ms_per_step": ms_e}
         # the end-to-end outputs are the same numbers as the device-resident ones
         if hessian:
@@ -510,12 +522,14 @@ def main():
     out = {"metric": metric, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
            "data": "synthetic",
-           "config": {"workload": workload, "n_points": bun.n_points, "n_batches": bun.n_batches, "n_basis": bun.n_basis,
-                      "mean_nnz": float(nnz.mean()) if len(nnz) else 0.0, "max_nnz": st["max_nnz"],
+           "config": {"workload": workload, "n_points": n_points_total, "n_batches": n_batches_total, "n_basis": bun.n_basis,
+                      "mean_nnz": float(nnz_all.mean()) if len(nnz_all) else 0.0, "max_nnz": int(nnz_all.max(initial=0)),
                       # workload metric of the paper, Eq. 31: #B x <|B|> x <nnz>^2, and the exact sum it models
-                      "eq31_ops": float(len(nnz) * npb.mean() * nnz.mean() ** 2) if len(nnz) else 0.0,
-                      "sum_np_nnz2": float((npb * nnz * nnz).sum()),
-                      "ms_per_eq31_gops": (ms_step / (len(nnz) * npb.mean() * nnz.mean() ** 2 * 1e-9)) if len(nnz) else None,
+                      "eq31_ops": float(len(nnz_all) * npb_all.mean() * nnz_all.mean() ** 2) if len(nnz_all) else 0.0,
+                      "sum_np_nnz2": float((npb_all * nnz_all * nnz_all).sum()),
+                      "ms_per_eq31_gops": (ms_step / (len(nnz_all) * npb_all.mean() * nnz_all.mean() ** 2 * 1e-9)) if len(nnz_all) else None,
+                      "sharding": ("none" if world == 1 else "each rank's context holds only its own contiguous batch range "
+                                   "(balanced by n_p*nnz^2); one NCCL all-reduce of H per step, none for n"),
                       "deterministic_H": bool(args.deterministic),
                       "max_active_atoms": st["max_active_atoms"], "parallelism": "batch-range x%d" % world,
                       "l2": "inputs larger than L2: each step streams %.1f GB of Phi planes plus a %.2f GB H and D"

@@ -85,9 +85,26 @@ def test_product_does_not_import_oracle():
 
 # ------------------------------------------------------------------------------------------- sharding host logic
 def _partition():
-    sys.path.insert(0, ROOT)
-    import bench
-    return bench.partition_batches
+    from paper_1912_06636_b200.sharding import partition_batches
+    return partition_batches
+
+
+def test_slice_bundle_keeps_exactly_the_ranks_own_batches():
+    import aims_synth
+    from paper_1912_06636_b200.sharding import first_phase_range, slice_bundle
+    bun = aims_synth.make_config(1, n_rad=12, n_ang=26, max_batch=40)
+    nb = bun.n_batches
+    covered = 0
+    for r in range(3):
+        b0, b1 = first_phase_range(nb, r, 3)
+        s, lo, hi = slice_bundle(bun, b0, b1)
+        assert s.batch_ptr[0] == 0 and s.batch_ptr[-1] == s.n_points == hi - lo and s.n_batches == b1 - b0
+        assert np.array_equal(s.xyz, bun.xyz[lo:hi]) and np.array_equal(s.w, bun.w[lo:hi])
+        assert np.array_equal(s.v, bun.v[lo:hi]) and np.array_equal(s.g, bun.g[:, lo:hi])
+        assert np.array_equal(np.diff(s.batch_ptr), np.diff(bun.batch_ptr[b0:b1 + 1]))
+        assert s.D_values is bun.D_values and s.n_values == bun.n_values           # global objects are shared, not cut
+        covered += s.n_points
+    assert covered == bun.n_points
 
 
 def test_partition_batches_is_a_contiguous_cover_and_balanced():
@@ -118,41 +135,51 @@ import os, sys
 import numpy as np
 import torch, torch.distributed as dist
 sys.path.insert(0, %(root)r)
-import aims_synth, bench
+import aims_synth
+from paper_1912_06636_b200.sharding import first_phase_range, partition_batches, slice_bundle
 from oracle.oracle import Oracle
 rank, world = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
 dist.init_process_group("gloo", rank=rank, world_size=world)
-bun = aims_synth.make_config(1, n_rad=12, n_ang=26, max_batch=40)
-orc = Oracle(bun)
-nnz = np.array([len(orc.batch_nnz(b)[0]) for b in range(bun.n_batches)], dtype=np.float64)
-cost = np.diff(bun.batch_ptr) * nnz * nnz
-b0, b1 = bench.partition_batches(cost, world)[rank]
-mine = np.arange(b0, b1)
-H = torch.from_numpy(orc.integrate_hamiltonian(bun.v, bun.g, batches=mine))     # Eq. 28: this rank's partial sum
+full = aims_synth.make_config(1, n_rad=12, n_ang=26, max_batch=40)
+# 1. cost probe on an equal-count slice (the per-rank "library" in this CPU test is the oracle; on a GPU it is aims_gpu_batch_nnz)
+p0, p1 = first_phase_range(full.n_batches, rank, world)
+probe, _, _ = slice_bundle(full, p0, p1)
+op = Oracle(probe)
+nnz = torch.zeros(full.n_batches, dtype=torch.int32)
+nnz[p0:p1] = torch.tensor([len(op.batch_nnz(b)[0]) for b in range(probe.n_batches)], dtype=torch.int32)
+dist.all_reduce(nnz)                                                             # 2. one tiny all-reduce
+cost = np.diff(full.batch_ptr) * nnz.numpy().astype(np.float64) ** 2
+b0, b1 = partition_batches(cost, world)[rank]                                    # 3. balanced contiguous ranges
+mine, lo, hi = slice_bundle(full, b0, b1)                                        # this rank knows only its own batches
+assert mine.n_points == hi - lo < full.n_points
+orc = Oracle(mine)
+H = torch.from_numpy(orc.integrate_hamiltonian(mine.v, mine.g))                  # Eq. 28: this rank's partial sum
 dist.all_reduce(H)                                                               # Eq. 29: the only communication step
-n, gn = orc.update_density(bun.D_values, want_grad=True, batches=mine)           # L312: no synchronisation needed
-lo, hi = int(bun.batch_ptr[b0]), int(bun.batch_ptr[b1])
-assert np.all(n[:lo] == 0) and np.all(n[hi:] == 0)
-parts = [torch.zeros(bun.n_points, dtype=torch.float64) for _ in range(world)]
-dist.all_gather(parts, torch.from_numpy(n))
-n_all = sum(parts).numpy()
-# widened rows: forces are partial sums like H (one all-reduce of 3 n_atoms numbers); the density Hessian shards like n
-Q = aims_synth.make_q_values(bun)
-F = torch.from_numpy(orc.pulay_forces(bun.v, bun.D_values, g=bun.g, Q_values=Q, batches=mine, kinetic=True))
+n, gn = orc.update_density(mine.D_values, want_grad=True)                        # L312: no synchronisation needed
+n_all = torch.zeros(full.n_points, dtype=torch.float64)
+n_all[lo:hi] = torch.from_numpy(n)
+dist.all_reduce(n_all)                                                           # (only to compare; a rank keeps its own points)
+# widened rows: forces and stress are partial sums like H; the density Hessian shards like n
+Q = aims_synth.make_q_values(mine)
+F = torch.from_numpy(orc.pulay_forces(mine.v, mine.D_values, g=mine.g, Q_values=Q, kinetic=True))
+sg = torch.from_numpy(orc.pulay_stress(mine.v, mine.D_values, g=mine.g, Q_values=Q))
 dist.all_reduce(F)
-hn = orc.density_hessian(bun.D_values, batches=mine)
-assert np.all(hn[:, :lo] == 0) and np.all(hn[:, hi:] == 0)
-hparts = [torch.zeros((6, bun.n_points), dtype=torch.float64) for _ in range(world)]
-dist.all_gather(hparts, torch.from_numpy(hn))
+dist.all_reduce(sg)
+hn_all = torch.zeros((6, full.n_points), dtype=torch.float64)
+hn_all[:, lo:hi] = torch.from_numpy(orc.density_hessian(mine.D_values))
+dist.all_reduce(hn_all)
 if rank == 0:
-    F_ref = orc.pulay_forces(bun.v, bun.D_values, g=bun.g, Q_values=Q, kinetic=True)
+    of = Oracle(full)
+    F_ref = of.pulay_forces(full.v, full.D_values, g=full.g, Q_values=Q, kinetic=True)
     assert np.abs(F.numpy() - F_ref).max() <= 1e-13 * np.abs(F_ref).max()
-    assert np.array_equal(sum(hparts).numpy(), orc.density_hessian(bun.D_values))
-    H_ref = orc.integrate_hamiltonian(bun.v, bun.g)
-    n_ref, _ = orc.update_density(bun.D_values, want_grad=True)
+    s_ref = of.pulay_stress(full.v, full.D_values, g=full.g, Q_values=Q)
+    assert np.abs(sg.numpy() - s_ref).max() <= 1e-13 * np.abs(s_ref).max()
+    assert np.array_equal(hn_all.numpy(), of.density_hessian(full.D_values))
+    H_ref = of.integrate_hamiltonian(full.v, full.g)
+    n_ref, _ = of.update_density(full.D_values, want_grad=True)
     eH = np.linalg.norm(H.numpy() - H_ref) / np.linalg.norm(H_ref)
     assert eH < 1e-13, eH
-    assert np.array_equal(n_all, n_ref)           # disjoint point ranges: bitwise the single-rank result
+    assert np.array_equal(n_all.numpy(), n_ref)   # disjoint point ranges: bitwise the single-rank result
     print("OK", b0, b1, eH)
 dist.destroy_process_group()
 """
