@@ -219,6 +219,18 @@ int aims_gpu_partition_weights(aims_gpu_ctx *ctx, int64_t n, const double *xyz, 
 int aims_gpu_bloch_fold(aims_gpu_ctx *ctx, const double *H_values, const int32_t *atom_home, const double *atom_T,
                         int32_t n_home, const double *kpt, double *out_re, double *out_im, int accumulate);
 
+/* Row f4 of SURVEY.md 8(f): the grid-adapted cut-plane batching of PAPER.md L210-218 on the GPU.  The paper cites "Algorithm 3 of
+ * [37]" without stating it; reading P12 fixes a deterministic recursive bisection: a set of n points is a batch if
+ * n <= max_batch_points; otherwise, with nb = ceil(n / max_batch_points), the n_left = round(floor(nb/2) n / nb) points smallest in
+ * (coordinate along the axis of largest extent -- ties to x, then y --, original index) form the left child and the rest the
+ * right child; batches are emitted depth-first and keep the order of their parent's sort.  Exactly one result is correct.
+ * No context is needed (batching precedes aims_gpu_create).  xyz: DEVICE [n_points][3]; order: DEVICE output [n_points],
+ * order[k] = original index of the point at position k of the batched grid; batch_ptr: HOST output, n_batches + 1 entries
+ * (capacity batch_ptr_capacity >= 2 ceil(n_points / max_batch_points) + 2 always suffices); n_batches: HOST output.
+ * Runs on `cuda_stream` of `device` and synchronises it before returning.  n_points < 2^31. */
+int aims_gpu_batch_points(int device, void *cuda_stream, int64_t n_points, const double *xyz, int32_t max_batch_points,
+                          int64_t *order, int64_t *batch_ptr, int64_t batch_ptr_capacity, int32_t *n_batches);
+
 /* Bitwise-reproducible H (PAPER.md L231 leaves the order of the batch sums free, it does not forbid a
  * fixed one).  enable != 0: aims_gpu_integrate_hamiltonian[_ks] and aims_gpu_add_tau_matrix add every batch's contribution
  * to H in ascending batch order ("ordered scatter": a tile of batch b waits until all tiles of the batches before b have

@@ -98,6 +98,8 @@ def load_library():
                                                ctypes.c_double, _vp, _vp, ctypes.c_int]
     L.aims_gpu_synchronize.restype = ctypes.c_int
     L.aims_gpu_synchronize.argtypes = [cp]
+    L.aims_gpu_batch_points.restype = ctypes.c_int
+    L.aims_gpu_batch_points.argtypes = [ctypes.c_int, _vp, ctypes.c_int64, _vp, ctypes.c_int32, _vp, _lp, ctypes.c_int64, _ip]
     L.aims_gpu_set_deterministic.restype = ctypes.c_int
     L.aims_gpu_set_deterministic.argtypes = [cp, ctypes.c_int]
     L.aims_gpu_batch_nnz.restype = ctypes.c_int
@@ -441,6 +443,30 @@ class Context:
             hb["n"].copy_(dv["n"], non_blocking=True)
             if want_grad:
                 hb["grad_n"].copy_(dv["grad_n"], non_blocking=True)
+
+
+def aims_gpu_batch_points(xyz, max_batch_points, device=0, stream=None):
+    """(order, batch_ptr): device int64 tensor [n] (position in the batched grid -> original point index) and a numpy
+    int64 array [n_batches + 1] (include/aims_gpu.h: aims_gpu_batch_points).  xyz: [n][3] array or tensor."""
+    import torch
+    L = load_library()
+    if not torch.cuda.is_available():
+        raise AimsError("no CUDA device: this path has no CPU fallback")
+    dev = torch.device("cuda", device)
+    st = stream if stream is not None else torch.cuda.current_stream(dev)
+    with torch.cuda.stream(st):
+        x = xyz if isinstance(xyz, torch.Tensor) else torch.as_tensor(np.ascontiguousarray(xyz, dtype=np.float64))
+        x = x.to(dev, torch.float64).reshape(-1, 3).contiguous()
+        n = int(x.shape[0])
+        order = torch.empty(max(n, 1), dtype=torch.int64, device=dev)
+    cap = 2 * ((n + int(max_batch_points) - 1) // max(int(max_batch_points), 1)) + 2
+    ptr = np.zeros(cap, dtype=np.int64)
+    nb = ctypes.c_int32()
+    rc = L.aims_gpu_batch_points(int(device), ctypes.c_void_p(st.cuda_stream), n, _ptr(x), int(max_batch_points), _ptr(order),
+                                 ptr.ctypes.data_as(_lp), cap, ctypes.byref(nb))
+    if rc != 0:
+        raise AimsError("aims_gpu_batch_points failed (%d)" % rc)
+    return order[:n], ptr[: nb.value + 1].copy()
 
 
 # ---- module-level functions with the names of the C ABI

@@ -4,9 +4,9 @@ import subprocess
 import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SRC = os.path.join(HERE, "csrc", "aims_gpu.cu")
+SRC = [os.path.join(HERE, "csrc", "aims_gpu.cu"), os.path.join(HERE, "csrc", "batching.cu")]
 LIB = os.path.join(HERE, "libaims_gpu.so")
-DEPS = [os.path.join(HERE, "csrc", f) for f in ("aims_gpu.cu", "common.cuh", "basis.cuh", "hamiltonian.cuh", "density.cuh", "forces.cuh", "hessian.cuh", "bloch.cuh", "partition.cuh")]
+DEPS = [os.path.join(HERE, "csrc", f) for f in ("aims_gpu.cu", "batching.cu", "common.cuh", "basis.cuh", "hamiltonian.cuh", "density.cuh", "forces.cuh", "hessian.cuh", "bloch.cuh", "partition.cuh")]
 DEPS.append(os.path.join(os.path.dirname(HERE), "include", "aims_gpu.h"))
 
 
@@ -22,7 +22,7 @@ def build(force=False, verbose=False):
         return LIB
     tmp = LIB + ".%d.tmp" % os.getpid()
     cmd = [nvcc_path(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-shared",
-           "-Xcompiler", "-fPIC", "-o", tmp, SRC]
+           "-Xcompiler", "-fPIC", "--threads", "2", "-o", tmp] + SRC
     if verbose:
         cmd[1:1] = ["-Xptxas", "-v"]
     subprocess.check_call(cmd)

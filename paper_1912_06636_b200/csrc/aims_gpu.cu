@@ -42,6 +42,9 @@ struct aims_gpu_ctx {
   // host copies of the static structure (dry run)
   std::vector<long long> batch_ptr, fn_off, act_off, ptab_off, pad_off, pad16_off, dpad_off, api_off, tile_off, item_off;
   std::vector<int> nnz, n_act;
+  std::vector<double> h_atom_xyz;                                // host copy of the atom positions (cell lists)
+  int *d_part = nullptr;                                         // cell list of aims_gpu_partition_weights (grows on demand)
+  size_t part_cap = 0;
   std::vector<int> h_atom_fn_ptr, h_col_atom, h_blk_ld;          // host copies of the pattern (Bloch sums)
   std::vector<long long> h_row_ptr, h_blk_off;
   int max_nnz = 0, max_act = 0, max_np = 0;
@@ -337,6 +340,7 @@ static int impl_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_
     }
   }
   c->h_atom_fn_ptr = atom_fn_ptr;
+  c->h_atom_xyz.assign(B->atom_xyz, B->atom_xyz + 3 * (size_t)na);
   c->h_row_ptr.assign(P->row_ptr, P->row_ptr + na + 1);
   c->h_col_atom.assign(P->col_atom, P->col_atom + n_blocks);
   c->h_blk_off.assign(P->blk_off, P->blk_off + n_blocks);
@@ -804,10 +808,55 @@ static int impl_partition_weights(aims_gpu_ctx *c, int64_t n, const double *xyz,
                                double *w_part) {
   if (!c || n < 0 || (n && (!xyz || !owner || !w_part)) || !(r_part > 0)) return fail(c, AIMS_ERR_INVALID_ARG, "NULL array, n < 0 or r_part <= 0");
   CU_TRY(c, cudaSetDevice(c->device));
-  if (n) {
+  if (!n) return AIMS_OK;
+  // cell list of the atoms, cell edge r_part (a hair more, so that rounding of a cell index never hides a neighbour):
+  // every atom within r_part of a point lies in the 27 cells around the point's cell -> O(N) overall
+  const int na = c->S.n_atoms;
+  const std::vector<double> &R = c->h_atom_xyz;
+  double lo[3] = {0, 0, 0}, hi[3] = {0, 0, 0};
+  for (int a = 0; a < na; a++)
+    for (int d = 0; d < 3; d++) {
+      if (a == 0 || R[3 * a + d] < lo[d]) lo[d] = R[3 * a + d];
+      if (a == 0 || R[3 * a + d] > hi[d]) hi[d] = R[3 * a + d];
+    }
+  const double edge = r_part * (1.0 + 1e-9);
+  int dim[3];
+  for (int d = 0; d < 3; d++) {
+    const double cells = std::floor((hi[d] - lo[d]) / edge) + 1.0;
+    if (!(cells < 2048.0)) return fail(c, AIMS_ERR_UNSUPPORTED, "atoms span more than 2048 cells of edge r_part");
+    dim[d] = (int)cells;
+  }
+  const long long ncell = (long long)dim[0] * dim[1] * dim[2];
+  if (ncell > (1ll << 26)) return fail(c, AIMS_ERR_UNSUPPORTED, "cell list of the atoms too large");
+  std::vector<int> start((size_t)ncell + 1, 0), order((size_t)std::max(na, 1)), cell_of((size_t)std::max(na, 1));
+  for (int a = 0; a < na; a++) {
+    int ic[3];
+    for (int d = 0; d < 3; d++) ic[d] = std::min(dim[d] - 1, std::max(0, (int)std::floor((R[3 * a + d] - lo[d]) / edge)));
+    cell_of[a] = (ic[2] * dim[1] + ic[1]) * dim[0] + ic[0];
+    start[(size_t)cell_of[a] + 1]++;
+  }
+  for (long long q = 0; q < ncell; q++) start[(size_t)q + 1] += start[(size_t)q];
+  {
+    std::vector<int> fill(start.begin(), start.end() - 1);
+    for (int a = 0; a < na; a++) order[(size_t)fill[(size_t)cell_of[a]]++] = a;      // ascending atom index inside a cell
+  }
+  // device copies live in a context-owned buffer that only grows
+  const size_t need = start.size() + order.size();
+  if (need > c->part_cap) {
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+    if (c->d_part) { c->owned.erase(std::remove(c->owned.begin(), c->owned.end(), (void *)c->d_part), c->owned.end()); cudaFree(c->d_part); c->d_part = nullptr; }
+    int rc = dev_alloc(c, &c->d_part, need);
+    if (rc) return rc;
+    c->part_cap = need;
+  }
+  CU_TRY(c, cudaMemcpyAsync(c->d_part, start.data(), start.size() * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+  CU_TRY(c, cudaMemcpyAsync(c->d_part + start.size(), order.data(), order.size() * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+  CU_TRY(c, cudaStreamSynchronize(c->stream));          // start / order are host temporaries
+  PartCells PC{lo[0], lo[1], lo[2], 1.0 / edge, dim[0], dim[1], dim[2], c->d_part, c->d_part + start.size()};
+  {
     TimedLaunch t(c, kKindOther);
-    k_partition_weights<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(c->S.n_atoms, c->S.atom_xyz, (long long)n, xyz, owner,
-                                                                          r_part, w_part);
+    k_partition_weights<<<(unsigned)((n + kPartWarps - 1) / kPartWarps), kPartWarps * 32, 0, c->stream>>>(
+        PC, c->S.atom_xyz, (long long)n, xyz, owner, r_part, w_part, c->L.error_flag);
   }
   return check_async(c);
 }
