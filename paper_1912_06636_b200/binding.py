@@ -10,7 +10,8 @@ import re
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libaims_gpu.so")
+# AIMS_GPU_LIB: a probe build of the same sources (build.py --define ... --tag ...) for the measurements under profiles/
+LIB_PATH = os.environ.get("AIMS_GPU_LIB") or os.path.join(_HERE, "libaims_gpu.so")
 HEADER_PATH = os.path.join(os.path.dirname(_HERE), "include", "aims_gpu.h")
 
 _dp = ctypes.POINTER(ctypes.c_double)

@@ -6,7 +6,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = [os.path.join(HERE, "csrc", "aims_gpu.cu"), os.path.join(HERE, "csrc", "batching.cu")]
 LIB = os.path.join(HERE, "libaims_gpu.so")
-DEPS = [os.path.join(HERE, "csrc", f) for f in ("aims_gpu.cu", "batching.cu", "common.cuh", "basis.cuh", "hamiltonian.cuh", "density.cuh", "forces.cuh", "hessian.cuh", "bloch.cuh", "partition.cuh")]
+DEPS = [os.path.join(HERE, "csrc", f) for f in sorted(os.listdir(os.path.join(HERE, "csrc"))) if f.endswith((".cu", ".cuh"))]
 DEPS.append(os.path.join(os.path.dirname(HERE), "include", "aims_gpu.h"))
 
 
@@ -17,18 +17,26 @@ def nvcc_path():
     return "nvcc"
 
 
-def build(force=False, verbose=False):
-    if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in DEPS):
-        return LIB
-    tmp = LIB + ".%d.tmp" % os.getpid()
+def build(force=False, verbose=False, defines=(), tag=None):
+    """defines / tag: a PROBE build for the profiles (e.g. `--define AIMS_PROBE_NO_H_EPILOGUE=1 --tag noepi` writes
+    libaims_gpu_noepi.so; load it with AIMS_GPU_LIB=<path>).  The product library is the untagged one."""
+    lib = LIB if not tag else os.path.join(HERE, "libaims_gpu_%s.so" % tag)
+    if not force and not defines and os.path.exists(lib) and all(os.path.getmtime(lib) >= os.path.getmtime(d) for d in DEPS):
+        return lib
+    tmp = lib + ".%d.tmp" % os.getpid()
     cmd = [nvcc_path(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-shared",
-           "-Xcompiler", "-fPIC", "--threads", "2", "-o", tmp] + SRC
+           "-Xcompiler", "-fPIC", "--threads", "2", "-o", tmp] + ["-D" + d for d in defines] + SRC
     if verbose:
         cmd[1:1] = ["-Xptxas", "-v"]
     subprocess.check_call(cmd)
-    os.replace(tmp, LIB)
-    return LIB
+    os.replace(tmp, lib)
+    return lib
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    argv = sys.argv[1:]
+    defs = [argv[i + 1] for i, a in enumerate(argv) if a == "--define"]
+    tag = next((argv[i + 1] for i, a in enumerate(argv) if a == "--tag"), None)
+    if defs and not tag:
+        raise SystemExit("--define needs --tag (the product library is never built with probe switches)")
+    print(build(force="--force" in argv, verbose="-v" in argv, defines=defs, tag=tag))

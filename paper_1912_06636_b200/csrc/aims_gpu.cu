@@ -16,6 +16,7 @@
 #include "bloch.cuh"
 #include "common.cuh"
 #include "density.cuh"
+#include "density2.cuh"
 #include "forces.cuh"
 #include "hessian.cuh"
 #include "partition.cuh"
@@ -55,6 +56,19 @@ struct aims_gpu_ctx {
   bool ptab_in_smem = true, f_ptab_in_smem = true, x_ptab_in_smem = true;
   std::vector<DItem> h_items;                                  // host copy of the density work items
   std::map<std::pair<int, int>, int *> item_order;             // (bs, be) -> device permutation, heaviest item first
+  // density2.cuh (bulk-copy pipeline): used when no atom of any batch is partially culled
+  bool fast_density = false, d2_pblk_in_smem = true;
+  std::vector<int> kq;                                         // K'' rows per batch
+  int max_kq = 0;
+  std::vector<long long> dq_off, item2_off;
+  long long *d_dq_off = nullptr;
+  DItem *d_items2 = nullptr;
+  std::vector<DItem> h_items2;
+  std::map<std::pair<int, int>, int *> item2_order;
+  long long *d_offU = nullptr, *d_offL = nullptr;              // full-storage offsets of every pattern block
+  int *d_blk_row = nullptr;
+  long long full_doubles = 0, n_blocks = 0;
+  double *Dfull = nullptr;                                     // full-storage copy of the density matrix (per call)
 
   double *ws = nullptr;      // Phi-plane workspace
   double *probe_out = nullptr;
@@ -250,6 +264,7 @@ cudaError_t smem_optin_all(int device, size_t optin) {
 #define AIMS_OPTIN(k) if ((e = smem_optin_max(k, optin)) != cudaSuccess) return e;
   AIMS_OPTIN(k_hamiltonian<false>) AIMS_OPTIN(k_hamiltonian<true>)
   AIMS_OPTIN(k_density<false>) AIMS_OPTIN(k_density<true>)
+  AIMS_OPTIN(k_density2<false>) AIMS_OPTIN(k_density2<true>)
   AIMS_OPTIN(k_density_hessian)
   AIMS_OPTIN((k_forces<false, false>)) AIMS_OPTIN((k_forces<true, false>))
   AIMS_OPTIN((k_forces<false, true>)) AIMS_OPTIN((k_forces<true, true>))
@@ -258,6 +273,7 @@ cudaError_t smem_optin_all(int device, size_t optin) {
   AIMS_OPTIN_EV(kEvalHGga, kLayH) AIMS_OPTIN_EV(kEvalHKinLda, kLayH) AIMS_OPTIN_EV(kEvalHKinGga, kLayH)
   AIMS_OPTIN_EV(kEvalTau, kLayH) AIMS_OPTIN_EV(kEvalHess, kLayD) AIMS_OPTIN_EV(kEvalPhi, kLayD)
   AIMS_OPTIN_EV(kEvalPhiGrad, kLayD) AIMS_OPTIN_EV(kEvalForceLda, kLayD) AIMS_OPTIN_EV(kEvalForceGga, kLayD)
+  AIMS_OPTIN_EV(kEvalPhi, kLayD2) AIMS_OPTIN_EV(kEvalPhiGrad, kLayD2)
 #undef AIMS_OPTIN_EV
 #undef AIMS_OPTIN
   if (device >= 0 && device < 64) done[device] = true;
@@ -399,14 +415,19 @@ static int impl_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_
   BatchLists &L = c->L;
   if ((rc = dev_alloc(c, &L.nnz, nb))) return rc;
   if ((rc = dev_alloc(c, &L.n_act, nb))) return rc;
+  if ((rc = dev_alloc(c, &L.kq, nb))) return rc;
+  if ((rc = dev_alloc(c, &L.nfull, nb))) return rc;
   if ((rc = dev_alloc(c, &L.error_flag, 1))) return rc;
   CU_TRY(c, cudaMemsetAsync(L.error_flag, 0, sizeof(int), c->stream));
   if (nb) {
     { TimedLaunch t(c, kKindCull); k_cull<<<nb, 256, 0, c->stream>>>(S, L, 0, 1); }
     if ((rc = check_async(c))) return rc;
   }
-  c->nnz.resize(nb); c->n_act.resize(nb);
+  c->nnz.resize(nb); c->n_act.resize(nb); c->kq.resize(nb);
+  std::vector<int> nfull(nb);
   int flag = 0;
+  CU_TRY(c, cudaMemcpyAsync(c->kq.data(), L.kq, nb * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+  CU_TRY(c, cudaMemcpyAsync(nfull.data(), L.nfull, nb * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
   CU_TRY(c, cudaMemcpyAsync(c->nnz.data(), L.nnz, nb * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
   CU_TRY(c, cudaMemcpyAsync(c->n_act.data(), L.n_act, nb * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
   CU_TRY(c, cudaMemcpyAsync(&flag, L.error_flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
@@ -417,8 +438,28 @@ static int impl_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_
   c->fn_off.assign(nb + 1, 0); c->act_off.assign(nb + 1, 0); c->ptab_off.assign(nb + 1, 0);
   c->pad_off.assign(nb + 1, 0); c->pad16_off.assign(nb + 1, 0); c->dpad_off.assign(nb + 1, 0); c->api_off.assign(nb + 1, 0); c->tile_off.assign(nb + 1, 0); c->item_off.assign(nb + 1, 0);
   std::vector<HTile> tiles;
-  std::vector<DItem> items;
+  std::vector<DItem> items, items2;
+  c->dq_off.assign(nb + 1, 0); c->item2_off.assign(nb + 1, 0);
+#ifdef AIMS_PROBE_DENSITY2
+  c->fast_density = true;            // probe build only: the bulk-copy / two-CTA density pipeline (profiles/r02_density2_history.md)
+#else
+  c->fast_density = false;
+#endif
   for (int b = 0; b < nb; b++) {
+    if (nfull[b] != c->nnz[b]) c->fast_density = false;          // an atom lost some of its shells: density.cuh handles that
+    c->max_kq = std::max(c->max_kq, c->kq[b]);
+    {
+      const int np_ = (int)(c->batch_ptr[b + 1] - c->batch_ptr[b]), np8_ = pad8(np_);
+      c->dq_off[b + 1] = c->dq_off[b] + (long long)round_up(c->kq[b], 16) * np8_;
+      if (c->nnz[b] > 0 && np_ > 0) {
+        const int nsub = np8_ >> 3, nit = (np8_ + kD2MaxPts - 1) / kD2MaxPts;
+        for (int q = 0; q < nit; q++) {
+          const int s0 = (int)((long long)q * nsub / nit), s1 = (int)((long long)(q + 1) * nsub / nit);
+          if (s1 > s0) items2.push_back(DItem{b, s0 * 8, (s1 - s0) * 8, 0});
+        }
+      }
+      c->item2_off[b + 1] = (long long)items2.size();
+    }
     const int nz = c->nnz[b], nact = c->n_act[b];
     const int np = (int)(c->batch_ptr[b + 1] - c->batch_ptr[b]);
     const int nz8 = pad8(nz), np8 = pad8(np);
@@ -474,6 +515,28 @@ static int impl_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_
   if ((rc = dev_upload<HTile>(c, &c->d_tiles, tiles.data(), tiles.size()))) return rc;
   if ((rc = dev_upload<DItem>(c, &c->d_items, items.data(), items.size()))) return rc;
   c->h_items = items;
+  if ((rc = dev_upload<DItem>(c, &c->d_items2, items2.data(), items2.size()))) return rc;
+  c->h_items2 = items2;
+  if ((rc = dev_upload<long long>(c, &c->d_dq_off, c->dq_off.data(), c->dq_off.size()))) return rc;
+  {
+    // full-storage layout of a pattern matrix (density2.cuh: k_expand_matrix): U part of block (A,B), L part = block (B,A)
+    std::vector<long long> offU((size_t)n_blocks), offL((size_t)n_blocks);
+    std::vector<int> blk_row((size_t)n_blocks);
+    long long off = 512;                                         // [0, 512): the zero page
+    for (int a = 0; a < na; a++)
+      for (long long q = P->row_ptr[a]; q < P->row_ptr[a + 1]; q++) {
+        const int bb = P->col_atom[q];
+        const long long nA = atom_fn_ptr[a + 1] - atom_fn_ptr[a], nB = atom_fn_ptr[bb + 1] - atom_fn_ptr[bb];
+        blk_row[(size_t)q] = a;
+        offU[(size_t)q] = off; off += nA * ((nB + 1) & ~1ll);
+        offL[(size_t)q] = off; if (bb != a) off += nB * ((nA + 1) & ~1ll);
+      }
+    c->full_doubles = off; c->n_blocks = n_blocks;
+    if ((rc = dev_upload<long long>(c, &c->d_offU, offU.data(), offU.size()))) return rc;
+    if ((rc = dev_upload<long long>(c, &c->d_offL, offL.data(), offL.size()))) return rc;
+    if ((rc = dev_upload<int>(c, &c->d_blk_row, blk_row.data(), blk_row.size()))) return rc;
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+  }
   CU_TRY(c, cudaStreamSynchronize(c->stream));
   if ((rc = dev_alloc(c, &L.fn_index, (size_t)c->fn_off[nb]))) return rc;
   if ((rc = dev_alloc(c, &L.fn_info, (size_t)c->fn_off[nb]))) return rc;
@@ -482,6 +545,7 @@ static int impl_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_
   if ((rc = dev_alloc(c, &L.act_row0, (size_t)c->act_off[nb]))) return rc;
   if ((rc = dev_alloc(c, &L.act_ld, (size_t)c->act_off[nb]))) return rc;
   if ((rc = dev_alloc(c, &L.ptab, (size_t)c->ptab_off[nb]))) return rc;
+  if ((rc = dev_alloc(c, &L.pblk, (size_t)c->ptab_off[nb]))) return rc;
 
   // ---- Phi-plane workspace: at least the largest single batch in EVERY plane layout used by a call (10 planes of the
   // density layout for the Hessian, 6 x the 16-point-padded H layout for the tau matrix), at most the requested budget
@@ -492,8 +556,8 @@ static int impl_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_
   long long need_min = 0;
   for (int b = 0; b < nb; b++)
     need_min = std::max({need_min, 10 * (c->dpad_off[b + 1] - c->dpad_off[b]), 6 * (c->pad16_off[b + 1] - c->pad16_off[b]),
-                         2 * (c->pad_off[b + 1] - c->pad_off[b])});
-  const long long need_all = std::max({10 * c->dpad_off[nb], 6 * c->pad16_off[nb], 2 * c->pad_off[nb]});
+                         2 * (c->pad_off[b + 1] - c->pad_off[b]), 4 * (c->dq_off[b + 1] - c->dq_off[b])});
+  const long long need_all = std::max({10 * c->dpad_off[nb], 6 * c->pad16_off[nb], 2 * c->pad_off[nb], 4 * c->dq_off[nb]});
   long long wsd = std::min(need_all, std::max(want / 8, need_min)) + 10 * 64;
   if (wsd * 8 > (long long)free_b) return fail(c, AIMS_ERR_NOMEM, "not enough device memory for one batch of Phi planes");
   if ((rc = dev_alloc(c, &c->ws, (size_t)wsd))) return rc;
@@ -515,6 +579,10 @@ static int impl_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_
     return fail(c, AIMS_ERR_UNSUPPORTED, "nnz(B) too large for the force kernel's shared memory");
   if (eval_smem_bytes(c->max_nnz) > lim)
     return fail(c, AIMS_ERR_UNSUPPORTED, "nnz(B) too large for the evaluation kernel's shared memory");
+  c->d2_pblk_in_smem = d2_smem_bytes(c->max_nnz, c->max_kq, mact, true) <= lim / 2;      // two CTAs per SM
+  if (d2_smem_bytes(c->max_nnz, c->max_kq, mact, c->d2_pblk_in_smem) > lim) c->fast_density = false;
+  if (c->fast_density && (rc = dev_alloc(c, &c->Dfull, (size_t)c->full_doubles))) return rc;
+  if (c->fast_density) CU_TRY(c, cudaMemsetAsync(c->Dfull, 0, 512 * sizeof(double), c->stream));
   CU_TRY(c, cudaStreamSynchronize(c->stream));
   return AIMS_OK;
 }
@@ -572,25 +640,29 @@ int chunk_end(const aims_gpu_ctx *c, const std::vector<long long> &off, int bs, 
 
 // Launch order of the density items of batches [bs, be): heaviest (largest nnz) first, so that the last CTAs of a launch
 // are the cheapest ones (a CTA's cost varies by 50x over a slab).  Built once per distinct range and kept on the device.
-int density_order(aims_gpu_ctx *c, int bs, int be, const int **out) {
-  const long long i0 = c->item_off[bs], i1 = c->item_off[be];
+int density_order(aims_gpu_ctx *c, int bs, int be, const int **out, bool v2 = false) {
+  const std::vector<long long> &ioff = v2 ? c->item2_off : c->item_off;
+  const std::vector<DItem> &hitems = v2 ? c->h_items2 : c->h_items;
+  std::map<std::pair<int, int>, int *> &cache = v2 ? c->item2_order : c->item_order;
+  const long long i0 = ioff[bs], i1 = ioff[be];
   if (i1 - i0 <= 2ll * c->sm_count) { *out = nullptr; return AIMS_OK; }   // fewer items than two waves: any order
   auto key = std::make_pair(bs, be);
-  auto it = c->item_order.find(key);
-  if (it != c->item_order.end()) { *out = it->second; return AIMS_OK; }
-  if (c->item_order.size() >= 64) {
+  auto it = cache.find(key);
+  if (it != cache.end()) { *out = it->second; return AIMS_OK; }
+  if (cache.size() >= 64) {
     // a caller walking over many distinct ranges: do not let the cache grow without bound
     CU_TRY(c, cudaStreamSynchronize(c->stream));
-    for (auto &kv : c->item_order) {
+    for (auto &kv : cache) {
       c->owned.erase(std::remove(c->owned.begin(), c->owned.end(), (void *)kv.second), c->owned.end());
       cudaFree(kv.second);
     }
-    c->item_order.clear();
+    cache.clear();
   }
   std::vector<int> ord((size_t)(i1 - i0));
   for (long long i = i0; i < i1; i++) ord[(size_t)(i - i0)] = (int)(i - i0);
   std::stable_sort(ord.begin(), ord.end(), [&](int a, int b) {
-    const DItem &x = c->h_items[(size_t)(i0 + a)], &y = c->h_items[(size_t)(i0 + b)];
+    const DItem &x = hitems[(size_t)(i0 + a)], &y = hitems[(size_t)(i0 + b)];
+    if (v2) return c->nnz[x.b] > c->nnz[y.b];       // the items of one batch stay neighbours: they read the same D_b pieces (L2)
     const long long cx = (long long)c->nnz[x.b] * c->nnz[x.b] * x.npt, cy = (long long)c->nnz[y.b] * c->nnz[y.b] * y.npt;
     return cx > cy;
   });
@@ -598,7 +670,7 @@ int density_order(aims_gpu_ctx *c, int bs, int be, const int **out) {
   int rc = dev_upload<int>(c, &d, ord.data(), ord.size());
   if (rc) return rc;
   CU_TRY(c, cudaStreamSynchronize(c->stream));   // ord is a temporary
-  c->item_order[key] = d;
+  cache[key] = d;
   *out = d;
   return AIMS_OK;
 }
@@ -724,6 +796,45 @@ static int impl_update_density(aims_gpu_ctx *c, int32_t b0, int32_t b1, const do
   int rc = run_cull(c, b0, b1);
   if (rc) return rc;
   const int npl = grad_n ? 4 : 1;
+  if (c->fast_density && b1 > b0) {
+    // density2.cuh: D written out in full storage once, then per chunk k_eval<., kLayD2> + k_density2
+    ExpandArgs X{D_values, c->Dfull, c->d_offU, c->d_offL, c->d_blk_row, 512};
+    if (c->n_blocks > 0) {
+      TimedLaunch t(c, kKindOther);
+      k_expand_matrix<<<(unsigned)c->n_blocks, 256, 0, c->stream>>>(c->S, X, c->n_blocks);
+    }
+    const int mact = std::max(c->max_act, 1);
+    const size_t dsm2 = d2_smem_bytes(c->max_nnz, c->max_kq, mact, c->d2_pblk_in_smem);
+    for (int bs = b0; bs < b1;) {
+      const int be = chunk_end(c, c->dq_off, bs, b1, npl);
+      if (be < 0) return fail(c, AIMS_ERR_NOMEM, "workspace too small for one batch of Phi planes");
+      const long long plane = (c->ws_doubles / npl) & ~63ll;
+      EvalArgs E{};
+      for (int q = 0; q < npl; q++) E.plane[q] = c->ws + q * plane;
+      if (!grad_n) E.plane[1] = c->ws;
+      E.pad_off = c->d_dq_off; E.pad_base = c->dq_off[bs];
+      E.n_points = c->n_points;
+      if (grad_n) launch_eval<kEvalPhiGrad, kLayD2>(c, E, bs, be); else launch_eval<kEvalPhi, kLayD2>(c, E, bs, be);
+      const long long ni = c->item2_off[be] - c->item2_off[bs];
+      if (ni > 0) {
+        D2Args A{};
+        if ((rc = density_order(c, bs, be, &A.order, true))) return rc;
+        A.items = c->d_items2 + c->item2_off[bs];
+        A.P = E.plane[0];
+        for (int q = 0; q < 3; q++) A.G[q] = grad_n ? E.plane[q + 1] : nullptr;
+        A.pad_off = c->d_dq_off; A.pad_base = c->dq_off[bs];
+        A.F = c->Dfull; A.offU = c->d_offU; A.offL = c->d_offL;
+        A.n = n; A.gn = grad_n; A.n_points = c->n_points; A.max_nnz_pad = c->max_nnz; A.max_kq_pad = c->max_kq;
+        A.pblk_in_smem = c->d2_pblk_in_smem ? 1 : 0;
+        TimedLaunch t(c, kKindDen);
+        if (grad_n) k_density2<true><<<(unsigned)ni, kD2Threads, dsm2, c->stream>>>(c->S, c->L, A, mact);
+        else k_density2<false><<<(unsigned)ni, kD2Threads, dsm2, c->stream>>>(c->S, c->L, A, mact);
+      }
+      if ((rc = check_async(c))) return rc;
+      bs = be;
+    }
+    return AIMS_OK;
+  }
   const size_t dsm = d_smem_bytes(c->max_nnz, std::max(c->max_act, 1), c->ptab_in_smem);
   for (int bs = b0; bs < b1;) {
     const int be = chunk_end(c, c->dpad_off, bs, b1, npl);

@@ -116,16 +116,19 @@ __global__ void __launch_bounds__(256) k_cull(DevSys S, BatchLists L, int b_firs
     }
   __syncthreads();
   if (tid == 0) {
-    int row = 0;
+    int row = 0, kq = 0, nfull = 0;
     for (int s = 0; s < nact; s++) {
       s_act_row0[s] = row;
-      const int sp = S.atom_species[s_act_atom[s]];
+      const int a = s_act_atom[s];
+      const int sp = S.atom_species[a];
       const int s0 = S.sp_shell_ptr[sp], s1 = S.sp_shell_ptr[sp + 1];
       for (int sh = s0; sh < s1; sh++)
         if (s_act_mask[s] >> (sh - s0) & 1u) row += 2 * S.shell_l[sh] + 1;
+      kq += (row - s_act_row0[s] + 1) & ~1;
+      nfull += S.atom_fn_ptr[a + 1] - S.atom_fn_ptr[a];
     }
     s_nnz = row;
-    if (dry) { L.nnz[b] = row; L.n_act[b] = nact; }
+    if (dry) { L.nnz[b] = row; L.n_act[b] = nact; L.kq[b] = kq; L.nfull[b] = nfull; }
   }
   __syncthreads();
   if (dry) return;
@@ -159,14 +162,15 @@ __global__ void __launch_bounds__(256) k_cull(DevSys S, BatchLists L, int b_firs
   for (int q = tid; q < nact * nact; q += 256) {
     const int sa = q / nact, sb = q - sa * nact;
     const int A = s_act_atom[min(sa, sb)], B = s_act_atom[max(sa, sb)];
-    long long lo2 = S.row_ptr[A], hi2 = S.row_ptr[A + 1] - 1, found = -1;
+    long long lo2 = S.row_ptr[A], hi2 = S.row_ptr[A + 1] - 1, found = -1, fidx = -1;
     while (lo2 <= hi2) {
       long long mid = (lo2 + hi2) >> 1;
       int cb = S.col_atom[mid];
-      if (cb == B) { found = S.blk_off[mid]; break; }
+      if (cb == B) { found = S.blk_off[mid]; fidx = mid; break; }
       if (cb < B) lo2 = mid + 1; else hi2 = mid - 1;
     }
     L.ptab[po + q] = found;
+    L.pblk[po + q] = (int)fidx;
   }
 }
 
@@ -313,7 +317,9 @@ __device__ __forceinline__ void solid_hessian_dot(int l, double x, double y, dou
 // of 16 rows of density.cuh / forces.cuh).  In the k4 layouts the four threads of a 4-point group write one full 32-byte
 // sector per row; in the API layout stores are coalesced along the point index.
 // ---------------------------------------------------------------------------------------------------------------
-enum EvalLayout { kLayApi = 0, kLayH = 1, kLayD = 2 };
+// kLayD2 (density2.cuh): kLayD with the rows in "K'' order" -- every active atom's rows start at an even row, i.e. one zero
+// row follows an atom with an odd number of rows -- so that a pair of consecutive rows never straddles two atoms.
+enum EvalLayout { kLayApi = 0, kLayH = 1, kLayD = 2, kLayD2 = 3 };
 
 #ifndef AIMS_EVAL_CTAS_PER_SM
 #define AIMS_EVAL_CTAS_PER_SM 2
@@ -352,6 +358,9 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
   int2 *s_ent = reinterpret_cast<int2 *>(s_rc2 + max_ent);                // [n_ent] x = slot | l << 8 | row << 12, y = spline row
   __shared__ double s_ax[kMaxActive], s_ay[kMaxActive], s_az[kMaxActive];
   __shared__ int s_e0[kMaxActive + 1];
+  __shared__ int s_shift[LAYOUT == kLayD2 ? kMaxActive : 1];      // kLayD2: zero rows inserted before the slot
+  __shared__ int s_zrow[LAYOUT == kLayD2 ? kMaxActive : 1];       // kLayD2: the inserted zero rows (K'' numbering)
+  __shared__ int s_nz;
   const int nk1 = S.n_knots - 1;
   for (int s = tid; s < nact; s += 256) {
     const int a = L.act_atom[ao + s];
@@ -364,6 +373,15 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
     s_e0[0] = 0;
     for (int s = 0; s < nact; s++) { const int c = s_e0[s + 1]; s_e0[s] = e; e += c; }
     s_e0[nact] = e;
+    if (LAYOUT == kLayD2) {
+      int shift = 0, nz = 0;
+      for (int s = 0; s < nact; s++) {
+        const int r0 = L.act_row0[ao + s], r1 = s + 1 < nact ? L.act_row0[ao + s + 1] : nnz;
+        s_shift[s] = shift;
+        if ((r1 - r0) & 1) { s_zrow[nz++] = r1 + shift; shift++; }
+      }
+      s_nz = nz;
+    }
   }
   __syncthreads();
   const int n_ent = s_e0[nact];
@@ -373,7 +391,7 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
     const int sp = S.atom_species[a];
     const int s0 = S.sp_shell_ptr[sp], s1 = S.sp_shell_ptr[sp + 1];
     const unsigned mask = L.act_mask[ao + s];
-    int row = L.act_row0[ao + s], e = s_e0[s];
+    int row = L.act_row0[ao + s] + (LAYOUT == kLayD2 ? s_shift[s] : 0), e = s_e0[s];
     for (int sh = s0; sh < s1; sh++) {
       if (!(mask >> (sh - s0) & 1u)) continue;
       const int l = S.shell_l[sh];
@@ -388,7 +406,8 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
   const int nnz8 = pad8(nnz), np8 = pad8(np);
   // points this CTA writes (k4 layouts: zero columns up to the padded point count)
   const int npx = LAYOUT == kLayApi ? np : (LAYOUT == kLayH && E.point_pad > 8 ? round_up(np, E.point_pad) : np8);
-  const int nrows = LAYOUT == kLayApi ? nnz : (LAYOUT == kLayD ? round_up(nnz, 16) : nnz8);   // rows this CTA writes
+  const int nkq = LAYOUT == kLayD2 ? nnz + s_nz : nnz;                                       // kLayD2: rows incl. the inserted ones
+  const int nrows = LAYOUT == kLayApi ? nnz : (LAYOUT == kLayD || LAYOUT == kLayD2 ? round_up(nkq, 16) : nnz8);   // rows this CTA writes
   double *o[NPL];
   if (LAYOUT == kLayApi) {
     const long long off = E.api_off[b] - E.api_base;
@@ -405,7 +424,7 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
 
   for (int p = tid; p < npx; p += 256) {
     // the thread's point base inside the batch's plane; element (row, p) at pbase + eval_row_off(row)
-    const int pbase = LAYOUT == kLayApi ? p : (LAYOUT == kLayH ? (p >> 2) * nnz8 * 4 + (p & 3) : (p >> 2) * 64 + (p & 3));
+    const int pbase = LAYOUT == kLayApi ? p : (LAYOUT == kLayH ? (p >> 2) * nnz8 * 4 + (p & 3) : (p >> 2) * 64 + (p & 3));   // kLayD, kLayD2
     double *op[NPL];
 #pragma unroll
     for (int q = 0; q < NPL; q++) op[q] = o[q] + pbase;
@@ -421,7 +440,9 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
       for (int r = 0; r < nrows; r++) AIMS_EZERO(eval_row_off<LAYOUT>(r, np, np8))
       continue;
     }
-    for (int r = nnz; r < nrows; r++) AIMS_EZERO(eval_row_off<LAYOUT>(r, np, np8))   // zero padding rows
+    for (int r = nkq; r < nrows; r++) AIMS_EZERO(eval_row_off<LAYOUT>(r, np, np8))   // zero padding rows
+    if (LAYOUT == kLayD2)
+      for (int q = 0; q < s_nz; q++) AIMS_EZERO(eval_row_off<LAYOUT>(s_zrow[LAYOUT == kLayD2 ? q : 0], np, np8))
     const double x = S.px[p0 + p], y = S.py[p0 + p], z = S.pz[p0 + p];
     double wv = 0.0, wgx = 0.0, wgy = 0.0, wgz = 0.0, w = 0.0;
     if (MODE == kEvalHLda) wv = S.w[p0 + p] * E.v[p0 + p];
@@ -465,8 +486,8 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
       const int ro = eval_row_off<LAYOUT>(row, np, np8);
       // offset of row + m: rows of one shell may straddle a 16-row chunk boundary in the D layout
       const int mstep = LAYOUT == kLayApi ? np : 4;
-      const int wrap = LAYOUT == kLayD ? 16 - (row & 15) : 8;          // first m that lies in the next chunk
-      const int jump = LAYOUT == kLayD ? np8 * 16 - 64 : 0;
+      const int wrap = (LAYOUT == kLayD || LAYOUT == kLayD2) ? 16 - (row & 15) : 8;          // first m that lies in the next chunk
+      const int jump = (LAYOUT == kLayD || LAYOUT == kLayD2) ? np8 * 16 - 64 : 0;
       if (d2 < s_rc2[e]) {
         if (l != lcur) {
           solid_harmonics<GRAD>(l, ux, uy, uz, Y, gx, gy, gz);

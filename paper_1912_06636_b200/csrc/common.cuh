@@ -44,6 +44,9 @@ struct BatchLists {
   int *act_row0;                 // [sum n_act]   first row of the slot in the batch's function list
   int *act_ld;                   // [sum n_act]   leading dimension of blocks whose column atom is this slot
   long long *ptab;               // [sum n_act^2] value offset of block (min,max) of the two slots, -1 if absent
+  int *pblk;                     // [sum n_act^2] index of that block in the pattern (col_atom / blk_off numbering), -1 if absent
+  int *kq;                       // [n_batches]   sum over the active atoms of their row count rounded up to even ("K'' rows")
+  int *nfull;                    // [n_batches]   sum over the active atoms of ALL their functions (== nnz iff no shell is culled)
   int *error_flag;               // [1] set if a capacity was exceeded
 };
 
