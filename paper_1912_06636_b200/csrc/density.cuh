@@ -24,8 +24,13 @@ constexpr int kDKC = 16;            // K (functions j) per stage
 constexpr int kDNP = 224;           // max points per CTA (7 blocks of 32)
 constexpr int kDStages = 4;
 constexpr int kDThreads = 512;
-constexpr int kDMmaWarps = 14;
-constexpr int kDProdLanes = 64;
+constexpr int kDMmaWarps = 14;             // MMA warps of a CTA with 5..7 point blocks (129..224 points)
+constexpr int kDProdLanes = 64;            // ... and its producer lanes (2 warps)
+// CTAs with <= 4 point blocks (<= 128 points) run 12 MMA warps and FOUR producer warps: the D_b tile of a stage has the
+// same number of rows per DMMA whatever the point count, so a short batch needs 2-3x more gather per flop, and round 1
+// measured its two producer warps as the limiter (17.6 TFLOP/s at 64-point batches); 12 warps, three per SM
+// sub-partition, still saturate the FP64 pipe (profiles/r01_dmma_probe.md: 8 warps reach 99.7 %).
+__host__ __device__ inline int d_mma_warps(int PB) { return PB <= 4 ? 12 : 14; }
 // One pipeline stage holds the D tile (M-tile rows x 16) followed by the Phi tile (CTA points x 16).  With PB point
 // blocks and IB = min(4, 14 / PB) row blocks per M-tile, rows + points never exceed 64 + 224 (PB = 7, IB = 2).
 constexpr int kDStageRows = 64 + kDNP;             // rows of D plus points of Phi per stage
@@ -159,12 +164,12 @@ __device__ __forceinline__ void d_mma_kloop(int variant, double (&acc)[4][4][2],
 // Producer side of one K stage: the tile D_b[i0 + r][k0 .. k0+15], r < tm, of the symmetric block-sparse matrix M restricted
 // to nnz(B) ("calculate_density_mat"), written as [4-function group][row][4] into dA.  pl = 0..63.
 __device__ __forceinline__ void d_gather_tile(double *dA, const double *M, int i0, int tm, int k0, int nnz, int nnz8, int nact,
-                                              const int *sInfo, const int *sLd, const long long *ptab, int pl) {
+                                              const int *sInfo, const int *sLd, const long long *ptab, int pl, int nprod) {
   // D_b[i0 + r][k0 + 4t .. +3]: one (row, 4-function group) per lane and pass; gathered from the block pattern
   // (stored block (si,sj) for si <= sj, transposed read of block (sj,si) below the diagonal)
   const int ng = min(kDKC, nnz8 - k0) >> 2;          // 4-function groups with at least one real function
   for (int t = 0; t < ng; t++)
-  for (int r = pl; r < tm; r += kDProdLanes) {       // consecutive lanes -> consecutive rows (transposed reads coalesce)
+  for (int r = pl; r < tm; r += nprod) {             // consecutive lanes -> consecutive rows (transposed reads coalesce)
     const int i = i0 + r, j = k0 + 4 * t;
     const unsigned dst = smem_u32(dA + (t * tm + r) * 4);
     if (i >= nnz) {
@@ -213,11 +218,11 @@ __device__ __forceinline__ void d_gather_tile(double *dA, const double *M, int i
 // DMMA load: sub-partition q hosts MMA warps q, q+4, q+8(, q+12) -- 2 and 3 have only three because the producers
 // sit there.  Blocks in descending size go to the sub-partition whose remaining slots need the largest average.
 // s_map[warp] = pb | ib << 8, -1 = idle.  One thread.
-__device__ __forceinline__ void d_deal_blocks(int *s_map, int PB, int IB, int psub) {
+__device__ __forceinline__ void d_deal_blocks(int *s_map, int PB, int IB, int psub, int nmma = kDMmaWarps) {
   const int nb = PB * IB;
   int cnt[4], load[4] = {0, 0, 0, 0}, used[4] = {0, 0, 0, 0}, total = 0;
   for (int q = 0; q < 4; q++) cnt[q] = nb / 4 + (q < (nb & 3) ? 1 : 0);
-  for (int w = 0; w < kDMmaWarps; w++) s_map[w] = -1;
+  for (int w = 0; w < nmma; w++) s_map[w] = -1;
   for (int pb2 = 0; pb2 < PB; pb2++) total += IB * ((blk_start(pb2 + 1, psub, PB) - blk_start(pb2, psub, PB)) >> 3);
   for (int sz = 4; sz >= 1; sz--)
     for (int pb2 = 0; pb2 < PB; pb2++) {
@@ -234,8 +239,9 @@ __device__ __forceinline__ void d_deal_blocks(int *s_map, int PB, int IB, int ps
     }
 }
 
-template <bool GRAD>
-__global__ void __launch_bounds__(kDThreads, 1) k_density(DevSys S, BatchLists L, DArgs A, int max_act) {
+// NMMA: 14 or 12 MMA warps (d_mma_warps); a compile-time constant inside the body, selected per CTA by the kernel below.
+template <bool GRAD, int NMMA>
+__device__ __forceinline__ void d_density_body(const DevSys &S, const BatchLists &L, const DArgs &A, int max_act, const DItem it) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   double *sA = reinterpret_cast<double *>(smem_raw);                     // stage s: [k4][tm][4] at sA + s * kDStage
   double *sPart = sA + (size_t)kDStages * kDStage;                       // [ib][q][col]
@@ -244,7 +250,6 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density(DevSys S, BatchLists L
   int *sLd = sInfo + pad8(A.max_nnz_pad);
   long long *sPtab = reinterpret_cast<long long *>(sLd + kMaxActive);
 
-  const DItem it = A.items[A.order ? A.order[blockIdx.x] : blockIdx.x];
   const int b = it.b;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int nnz = L.nnz[b], nact = L.n_act[b];
@@ -254,7 +259,8 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density(DevSys S, BatchLists L
   const long long boff = A.pad_off[b] - A.pad_base;
   const int p0 = it.p0, npt = it.npt;                    // this CTA's points [p0, p0+npt) of the batch (multiples of 8)
   const int psub = npt >> 3, PB = blk_count(psub);       // point sub-tiles and blocks
-  const int IB = min(8, kDMmaWarps / PB);                // row blocks per M-tile: 2,2,2,3,4,7,8 for PB = 7..1
+  constexpr int nmma = NMMA, nprod = (16 - NMMA) * 32;         // MMA warps and producer lanes of this CTA
+  const int IB = min(8, nmma / PB);                // row blocks per M-tile: 2,2,2,3,4,7,8 for PB = 7..1
   const int n_mt = (nblk + IB - 1) / IB;                 // M-tiles
   const double *sB = sA + IB * 32 * kDKC;                // stage s: [point group][16][4] at sB + s * kDStage
   const int nkc = (nnz8 + kDKC - 1) / kDKC;              // K stages per M-tile
@@ -271,19 +277,19 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density(DevSys S, BatchLists L
   if (tid == 0) {
 #pragma unroll
     for (int s = 0; s < kDStages; s++) {
-      mbar_init(bar_full + 8 * s, kDProdLanes + 1);      // 64 cp.async completions + the expect_tx arrival
-      mbar_init(bar_empty + 8 * s, kDMmaWarps);
+      mbar_init(bar_full + 8 * s, (unsigned)nprod + 1u);  // the producers' cp.async completions + the expect_tx arrival
+      mbar_init(bar_empty + 8 * s, (unsigned)nmma);
     }
     mbar_fence_init();
-    d_deal_blocks(s_map, PB, IB, psub);
+    d_deal_blocks(s_map, PB, IB, psub, nmma);
   }
   __syncthreads();
   const long long *ptab = A.ptab_in_smem ? sPtab : gptab;
   const double *gP = A.P + boff;
 
-  if (warp >= kDMmaWarps) {
+  if (warp >= nmma) {
     // =========================================================================== producers
-    const int pl = tid - kDMmaWarps * 32;                // 0..63
+    const int pl = tid - nmma * 32;                // 0..63
     const int np8 = pad8(np);
     int step = 0;
 #pragma unroll 1
@@ -299,19 +305,19 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density(DevSys S, BatchLists L
         // operands of this M-tile's epilogue (rows [i0, i0+tm) of Phi and grad Phi at the CTA's points): whole 16-row
         // chunks are contiguous in the density layout -> one bulk L2 prefetch per chunk and plane
         const int c0 = i0 >> 4, nch = ((i0 + tm - 1) >> 4) - c0 + 1;
-        for (int idx = pl; idx < nch * (GRAD ? 4 : 1); idx += kDProdLanes) {
+        for (int idx = pl; idx < nch * (GRAD ? 4 : 1); idx += nprod) {
           const int c = c0 + (GRAD ? (idx >> 2) : idx), q = GRAD ? (idx & 3) : 0;
           const double *base = (q == 0) ? gP : A.G[q - 1] + boff;
           bulk_prefetch_l2(base + ((long long)c * (np8 >> 2) + (p0 >> 2)) * 64, (unsigned)npt * 128u);
         }
       }
-      if (pl == kDProdLanes - 1) {
+      if (pl == nprod - 1) {
         // Phi rows [k0, k0+16) of every point of the CTA: ONE contiguous segment in the density layout
         mbar_expect_tx(bar_full + 8 * s, (unsigned)npt * 128u);
         bulk_g2s(smem_u32(sB + (size_t)s * kDStage), gP + ((long long)kc * (np8 >> 2) + (p0 >> 2)) * 64, (unsigned)npt * 128u,
                  bar_full + 8 * s);
       }
-      d_gather_tile(sA + (size_t)s * kDStage, A.D, i0, tm, k0, nnz, nnz8, nact, sInfo, sLd, ptab, pl);
+      d_gather_tile(sA + (size_t)s * kDStage, A.D, i0, tm, k0, nnz, nnz8, nact, sInfo, sLd, ptab, pl, nprod);
       cp_async_mbar_arrive_noinc(bar_full + 8 * s);
       }
     }
@@ -429,6 +435,13 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density(DevSys S, BatchLists L
         A.gn[(long long)q * A.n_points + pbase + p] = 2.0 * u;
       }
   }
+}
+
+template <bool GRAD>
+__global__ void __launch_bounds__(kDThreads, 1) k_density(DevSys S, BatchLists L, DArgs A, int max_act) {
+  const DItem it = A.items[A.order ? A.order[blockIdx.x] : blockIdx.x];
+  if (d_mma_warps(blk_count(it.npt >> 3)) == 12) d_density_body<GRAD, 12>(S, L, A, max_act, it);
+  else d_density_body<GRAD, 14>(S, L, A, max_act, it);
 }
 
 }  // namespace aims

@@ -49,8 +49,8 @@ inline size_t f_smem_bytes(int max_nnz, int max_act, bool ptab_in_smem) {
 //   sum_i sum_p (r_p - c)_m [...]_l  -  sum_slots (R_slot - c)_m sF[slot][l] ,
 // the first sum needs no per-atom separation (nine more accumulators per lane, weighted with the lane's two points) and the
 // second comes from the CTA's force table; both terms are of the size of the batch, so nothing cancels.
-template <bool GGA, bool STRESS>
-__global__ void __launch_bounds__(kDThreads, 1) k_forces(DevSys S, BatchLists L, FArgs A, int max_act) {
+template <bool GGA, bool STRESS, int NMMA>
+__device__ __forceinline__ void d_forces_body(const DevSys &S, const BatchLists &L, const FArgs &A, int max_act, const DItem it) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   double *sA = reinterpret_cast<double *>(smem_raw);                     // stage s: [k4][tm][4] at sA + s * kDStage
   double *sF = sA + (size_t)kDStages * kDStage;                          // [slot][3]
@@ -60,7 +60,6 @@ __global__ void __launch_bounds__(kDThreads, 1) k_forces(DevSys S, BatchLists L,
   int *sLd = sInfo + pad8(A.max_nnz_pad);
   long long *sPtab = reinterpret_cast<long long *>(sLd + kMaxActive);
 
-  const DItem it = A.items[A.order ? A.order[blockIdx.x] : blockIdx.x];
   const int b = it.b;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int nnz = L.nnz[b], nact = L.n_act[b];
@@ -70,7 +69,8 @@ __global__ void __launch_bounds__(kDThreads, 1) k_forces(DevSys S, BatchLists L,
   const long long boff = A.pad_off[b] - A.pad_base;
   const int p0 = it.p0, npt = it.npt;                    // this CTA's points [p0, p0+npt) of the batch (multiples of 8)
   const int psub = npt >> 3, PB = blk_count(psub);
-  const int IB = min(8, kDMmaWarps / PB);
+  constexpr int nmma = NMMA, nprod = (16 - NMMA) * 32;         // MMA warps and producer lanes of this CTA
+  const int IB = min(8, nmma / PB);
   const int n_mt = (nblk + IB - 1) / IB;
   const double *sB = sA + IB * 32 * kDKC;
   const int nkc = (nnz8 + kDKC - 1) / kDKC;
@@ -93,18 +93,18 @@ __global__ void __launch_bounds__(kDThreads, 1) k_forces(DevSys S, BatchLists L,
   if (tid == 0) {
 #pragma unroll
     for (int s = 0; s < kDStages; s++) {
-      mbar_init(bar_full + 8 * s, kDProdLanes + 1);
-      mbar_init(bar_empty + 8 * s, kDMmaWarps);
+      mbar_init(bar_full + 8 * s, (unsigned)nprod + 1u);
+      mbar_init(bar_empty + 8 * s, (unsigned)nmma);
     }
     mbar_fence_init();
-    d_deal_blocks(s_map, PB, IB, psub);
+    d_deal_blocks(s_map, PB, IB, psub, nmma);
   }
   __syncthreads();
   const long long *ptab = A.ptab_in_smem ? sPtab : gptab;
 
-  if (warp >= kDMmaWarps) {
+  if (warp >= nmma) {
     // =========================================================================== producers
-    const int pl = tid - kDMmaWarps * 32;
+    const int pl = tid - nmma * 32;
     int step = 0;
 #pragma unroll 1
     for (int mt = 0; mt < n_mt; mt++) {
@@ -126,17 +126,17 @@ __global__ void __launch_bounds__(kDThreads, 1) k_forces(DevSys S, BatchLists L,
             if (seg == nseg - 1 && kc == max(nkc - kDPrefetchLead, 0)) {
               // operands of this pass's epilogue (rows [i0, i0+tm) of three derivative planes at the CTA's points)
               const int c0 = i0 >> 4, nch = ((i0 + tm - 1) >> 4) - c0 + 1;
-              for (int idx = pl; idx < nch * 3; idx += kDProdLanes) {
+              for (int idx = pl; idx < nch * 3; idx += nprod) {
                 const int c = c0 + idx / 3, q = idx % 3;
                 bulk_prefetch_l2(A.E[3 * pass + q] + boff + ((long long)c * (np8 >> 2) + (p0 >> 2)) * 64, (unsigned)npt * 128u);
               }
             }
-            if (pl == kDProdLanes - 1) {
+            if (pl == nprod - 1) {
               mbar_expect_tx(bar_full + 8 * s, (unsigned)npt * 128u);
               bulk_g2s(smem_u32(sB + (size_t)s * kDStage), gB + ((long long)kc * (np8 >> 2) + (p0 >> 2)) * 64, (unsigned)npt * 128u,
                        bar_full + 8 * s);
             }
-            d_gather_tile(sA + (size_t)s * kDStage, M, i0, tm, k0, nnz, nnz8, nact, sInfo, sLd, ptab, pl);
+            d_gather_tile(sA + (size_t)s * kDStage, M, i0, tm, k0, nnz, nnz8, nact, sInfo, sLd, ptab, pl, nprod);
             cp_async_mbar_arrive_noinc(bar_full + 8 * s);
           }
         }
@@ -280,6 +280,13 @@ __global__ void __launch_bounds__(kDThreads, 1) k_forces(DevSys S, BatchLists L,
     for (int s = 0; s < nact; s++) u -= (S.atom_xyz[3 * L.act_atom[ao + s] + m] - cref[m]) * sF[3 * s + l];
     red_add_f64(A.sigma + tid, 2.0 * u * A.inv_volume);
   }
+}
+
+template <bool GGA, bool STRESS>
+__global__ void __launch_bounds__(kDThreads, 1) k_forces(DevSys S, BatchLists L, FArgs A, int max_act) {
+  const DItem it = A.items[A.order ? A.order[blockIdx.x] : blockIdx.x];
+  if (d_mma_warps(blk_count(it.npt >> 3)) == 12) d_forces_body<GGA, STRESS, 12>(S, L, A, max_act, it);
+  else d_forces_body<GGA, STRESS, 14>(S, L, A, max_act, it);
 }
 
 }  // namespace aims

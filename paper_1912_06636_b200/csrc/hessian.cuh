@@ -84,7 +84,8 @@ __device__ __forceinline__ void x_epilogue(const double (&acc)[4][4][2], const X
   }
 }
 
-__global__ void __launch_bounds__(kDThreads, 1) k_density_hessian(DevSys S, BatchLists L, XArgs A, int max_act) {
+template <int NMMA>
+__device__ __forceinline__ void d_hessian_body(const DevSys &S, const BatchLists &L, const XArgs &A, int max_act, const DItem it) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   double *sA = reinterpret_cast<double *>(smem_raw);                     // stage s: [k4][tm][4] at sA + s * kDStage
   double *sPart = sA + (size_t)kDStages * kDStage;                       // [ib][component][col]
@@ -93,7 +94,6 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density_hessian(DevSys S, Batc
   int *sLd = sInfo + pad8(A.max_nnz_pad);
   long long *sPtab = reinterpret_cast<long long *>(sLd + kMaxActive);
 
-  const DItem it = A.items[A.order ? A.order[blockIdx.x] : blockIdx.x];
   const int b = it.b;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int nnz = L.nnz[b], nact = L.n_act[b];
@@ -104,7 +104,8 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density_hessian(DevSys S, Batc
   const long long boff = A.pad_off[b] - A.pad_base;
   const int p0 = it.p0, npt = it.npt;
   const int psub = npt >> 3, PB = blk_count(psub);
-  const int IB = min(8, kDMmaWarps / PB);
+  constexpr int nmma = NMMA, nprod = (16 - NMMA) * 32;         // MMA warps and producer lanes of this CTA
+  const int IB = min(8, nmma / PB);
   const int n_mt = (nblk + IB - 1) / IB;
   const double *sB = sA + IB * 32 * kDKC;
   const int nkc = (nnz8 + kDKC - 1) / kDKC;
@@ -121,18 +122,18 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density_hessian(DevSys S, Batc
   if (tid == 0) {
 #pragma unroll
     for (int s = 0; s < kDStages; s++) {
-      mbar_init(bar_full + 8 * s, kDProdLanes + 1);
-      mbar_init(bar_empty + 8 * s, kDMmaWarps);
+      mbar_init(bar_full + 8 * s, (unsigned)nprod + 1u);
+      mbar_init(bar_empty + 8 * s, (unsigned)nmma);
     }
     mbar_fence_init();
-    d_deal_blocks(s_map, PB, IB, psub);
+    d_deal_blocks(s_map, PB, IB, psub, nmma);
   }
   __syncthreads();
   const long long *ptab = A.ptab_in_smem ? sPtab : gptab;
 
-  if (warp >= kDMmaWarps) {
+  if (warp >= nmma) {
     // =========================================================================== producers
-    const int pl = tid - kDMmaWarps * 32;
+    const int pl = tid - nmma * 32;
     int step = 0;
 #pragma unroll 1
     for (int mt = 0; mt < n_mt; mt++) {
@@ -150,17 +151,17 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density_hessian(DevSys S, Batc
             // operands of this pass's epilogue: rows [i0, i0+tm) of the six Hessian planes (pass 0) or of d_x..d_e Phi
             const int c0 = i0 >> 4, nch = ((i0 + tm - 1) >> 4) - c0 + 1;
             const int npl = pass == 0 ? 6 : pass, pl0 = pass == 0 ? 4 : 1;
-            for (int idx = pl; idx < nch * npl; idx += kDProdLanes) {
+            for (int idx = pl; idx < nch * npl; idx += nprod) {
               const int c = c0 + idx / npl, q = idx % npl;
               bulk_prefetch_l2(A.PL[pl0 + q] + boff + ((long long)c * (np8 >> 2) + (p0 >> 2)) * 64, (unsigned)npt * 128u);
             }
           }
-          if (pl == kDProdLanes - 1) {
+          if (pl == nprod - 1) {
             mbar_expect_tx(bar_full + 8 * s, (unsigned)npt * 128u);
             bulk_g2s(smem_u32(sB + (size_t)s * kDStage), gB + ((long long)kc * (np8 >> 2) + (p0 >> 2)) * 64, (unsigned)npt * 128u,
                      bar_full + 8 * s);
           }
-          d_gather_tile(sA + (size_t)s * kDStage, A.D, i0, tm, k0, nnz, nnz8, nact, sInfo, sLd, ptab, pl);
+          d_gather_tile(sA + (size_t)s * kDStage, A.D, i0, tm, k0, nnz, nnz8, nact, sInfo, sLd, ptab, pl, nprod);
           cp_async_mbar_arrive_noinc(bar_full + 8 * s);
         }
       }
@@ -230,6 +231,12 @@ __global__ void __launch_bounds__(kDThreads, 1) k_density_hessian(DevSys S, Batc
       A.hn[(long long)k * A.n_points + pbase + p] = 2.0 * u;
     }
   }
+}
+
+__global__ void __launch_bounds__(kDThreads, 1) k_density_hessian(DevSys S, BatchLists L, XArgs A, int max_act) {
+  const DItem it = A.items[A.order ? A.order[blockIdx.x] : blockIdx.x];
+  if (d_mma_warps(blk_count(it.npt >> 3)) == 12) d_hessian_body<12>(S, L, A, max_act, it);
+  else d_hessian_body<14>(S, L, A, max_act, it);
 }
 
 }  // namespace aims
