@@ -692,7 +692,7 @@ int launch_hamiltonian(aims_gpu_ctx *c, bool syr2k, HArgs A, int bs, long long n
 template <int MODE, int LAYOUT>
 void launch_eval(aims_gpu_ctx *c, const EvalArgs &E, int bs, int be) {
   TimedLaunch t(c, kKindEval);
-  k_eval<MODE, LAYOUT><<<be - bs, 256, eval_smem_bytes(c->max_nnz), c->stream>>>(c->S, c->L, E, bs, std::max(c->max_nnz, 1));
+  k_eval<MODE, LAYOUT><<<be - bs, kEvalThreads, eval_smem_bytes(c->max_nnz), c->stream>>>(c->S, c->L, E, bs, std::max(c->max_nnz, 1));
 }
 
 }  // namespace

@@ -324,6 +324,20 @@ enum EvalLayout { kLayApi = 0, kLayH = 1, kLayD = 2, kLayD2 = 3 };
 #ifndef AIMS_EVAL_CTAS_PER_SM
 #define AIMS_EVAL_CTAS_PER_SM 2
 #endif
+// Threads of a k_eval CTA.  Measured on config 5 (profiles/r02_eval_variants.md): 224 threads (7 warps cover a 200-point batch
+// in one pass, 144 registers per thread at two CTAs per SM) are SLOWER than 256 (82.9 vs 63.2 ms per step) -- the kernel lives
+// on warps in flight, not on registers per thread.  The spline coefficients (a gather through L1/L2 per point and shell, the
+// largest stall of the round-1 kernel: long scoreboard 25 % / 46 % of the samples) are fetched one shell ahead.
+#ifndef AIMS_EVAL_THREADS
+#define AIMS_EVAL_THREADS 256
+#endif
+constexpr int kEvalThreads = AIMS_EVAL_THREADS;
+// registers per thread: two CTAs of 7 warps per SM -> 65,536 / 448 = 146 (ptxas rounds a launch bound of 224 threads up to
+// 256, hence __maxnreg__ instead); the force and Hessian planes need more and run one CTA per SM
+__host__ __device__ constexpr int eval_max_regs(int mode) { return (mode == 4 || mode == 5 || mode == 8) ? 255 : (kEvalThreads <= 224 ? 144 : 128); }
+#ifndef AIMS_EVAL_PREFETCH
+#define AIMS_EVAL_PREFETCH 1
+#endif
 // dynamic shared memory of k_eval: one entry per active shell of the batch (<= nnz(B) of them)
 inline size_t eval_smem_bytes(int max_nnz) { return (size_t)std::max(max_nnz, 1) * (sizeof(int2) + sizeof(double)); }
 
@@ -336,7 +350,7 @@ __device__ __forceinline__ int eval_row_off(int row, int np, int np8) {
 }
 
 template <int MODE, int LAYOUT>
-__global__ void __launch_bounds__(256, (MODE == kEvalForceLda || MODE == kEvalForceGga || MODE == kEvalHess) ? 1 : AIMS_EVAL_CTAS_PER_SM)
+__global__ void __maxnreg__(eval_max_regs(MODE))
 k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
   constexpr bool FORCE = (MODE == kEvalForceLda || MODE == kEvalForceGga);
   constexpr bool HESS = (MODE == kEvalForceGga);
@@ -362,7 +376,7 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
   __shared__ int s_zrow[LAYOUT == kLayD2 ? kMaxActive : 1];       // kLayD2: the inserted zero rows (K'' numbering)
   __shared__ int s_nz;
   const int nk1 = S.n_knots - 1;
-  for (int s = tid; s < nact; s += 256) {
+  for (int s = tid; s < nact; s += kEvalThreads) {
     const int a = L.act_atom[ao + s];
     s_ax[s] = S.atom_xyz[3 * a]; s_ay[s] = S.atom_xyz[3 * a + 1]; s_az[s] = S.atom_xyz[3 * a + 2];
     s_e0[s + 1] = __popc(L.act_mask[ao + s]);
@@ -386,7 +400,7 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
   __syncthreads();
   const int n_ent = s_e0[nact];
   if (n_ent > max_ent) { if (tid == 0) atomicExch(L.error_flag, 4); return; }
-  for (int s = tid; s < nact; s += 256) {
+  for (int s = tid; s < nact; s += kEvalThreads) {
     const int a = L.act_atom[ao + s];
     const int sp = S.atom_species[a];
     const int s0 = S.sp_shell_ptr[sp], s1 = S.sp_shell_ptr[sp + 1];
@@ -422,7 +436,7 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
   }
   const int cstr = TAU ? npx * nnz8 : 0;          // kEvalTau: distance between the d_x, d_y, d_z parts of a plane
 
-  for (int p = tid; p < npx; p += 256) {
+  for (int p = tid; p < npx; p += kEvalThreads) {
     // the thread's point base inside the batch's plane; element (row, p) at pbase + eval_row_off(row)
     const int pbase = LAYOUT == kLayApi ? p : (LAYOUT == kLayH ? (p >> 2) * nnz8 * 4 + (p & 3) : (p >> 2) * 64 + (p & 3));   // kLayD, kLayD2
     double *op[NPL];
@@ -459,6 +473,7 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
       if (HESS) { wgx = E.g[p0 + p]; wgy = E.g[E.n_points + p0 + p]; wgz = E.g[2 * E.n_points + p0 + p]; }
     }
     int cur = -1, lcur = -1, k = 0;
+    double2 c01 = make_double2(0.0, 0.0), c23 = make_double2(0.0, 0.0);   // spline coefficients of the current entry
     double d2 = 0.0, ux = 0.0, uy = 0.0, uz = 1.0, dd = 1.0, inv_dd = 1.0, xs = 0.0, ug = 0.0;
     double Y[7], gx[7], gy[7], gz[7];
     double hx[HESS ? 7 : 1], hy[HESS ? 7 : 1], hz[HESS ? 7 : 1];
@@ -481,6 +496,18 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
         xs = t - (double)k;
         inv_dd = 1.0 / dd;
         if (HESS) ug = ux * wgx + uy * wgy + uz * wgz;
+        // first shell of a new atom: its coefficients cannot be fetched earlier (k is only known now)
+        const double2 *cf0 = reinterpret_cast<const double2 *>(S.spline_coef + (long long)(en.y + k) * 4);
+        c01 = __ldg(cf0); c23 = __ldg(cf0 + 1);
+      }
+      // the next entry's coefficients, one iteration ahead (same atom -> same knot interval k); consumed at the loop's end
+      double2 n01 = c01, n23 = c23;
+      if (AIMS_EVAL_PREFETCH && e + 1 < n_ent) {
+        const int2 en1 = s_ent[e + 1];
+        if ((en1.x & 0xFF) == cur) {
+          const double2 *cf1 = reinterpret_cast<const double2 *>(S.spline_coef + (long long)(en1.y + k) * 4);
+          n01 = __ldg(cf1); n23 = __ldg(cf1 + 1);
+        }
       }
       const int nm = 2 * l + 1;
       const int ro = eval_row_off<LAYOUT>(row, np, np8);
@@ -502,8 +529,6 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
           }
           lcur = l;
         }
-        const double2 *cf = reinterpret_cast<const double2 *>(S.spline_coef + (long long)(en.y + k) * 4);
-        const double2 c01 = __ldg(cf), c23 = __ldg(cf + 1);
         const double R = c01.x + xs * (c01.y + xs * (c23.x + xs * c23.y));
         double f = 0.0, Rd = 0.0, hA = 0.0, hB = 0.0, hC = 0.0, qlap = 0.0;
         if (GRAD || KIN) {
@@ -573,6 +598,12 @@ k_eval(DevSys S, BatchLists L, EvalArgs E, int b_first, int max_ent) {
         }
       } else {
         for (int m = 0; m < nm; m++) AIMS_EZERO(ro + m * mstep + (m >= wrap ? jump : 0))
+      }
+      if (AIMS_EVAL_PREFETCH) { c01 = n01; c23 = n23; }
+      else if (e + 1 < n_ent) {
+        const int2 en1 = s_ent[e + 1];
+        const double2 *cf1 = reinterpret_cast<const double2 *>(S.spline_coef + (long long)(en1.y + k) * 4);
+        if ((en1.x & 0xFF) == cur) { c01 = __ldg(cf1); c23 = __ldg(cf1 + 1); }
       }
     }
   }
