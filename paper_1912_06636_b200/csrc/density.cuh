@@ -20,9 +20,15 @@
 
 namespace aims {
 
+#ifndef AIMS_D_NP
+#define AIMS_D_NP 224
+#endif
+#ifndef AIMS_D_STAGES
+#define AIMS_D_STAGES 4
+#endif
 constexpr int kDKC = 16;            // K (functions j) per stage
-constexpr int kDNP = 224;           // max points per CTA (7 blocks of 32)
-constexpr int kDStages = 4;
+constexpr int kDNP = AIMS_D_NP;     // max points per CTA (7 blocks of 32)
+constexpr int kDStages = AIMS_D_STAGES;
 constexpr int kDThreads = 512;
 constexpr int kDMmaWarps = 14;             // MMA warps of a CTA with 5..7 point blocks (129..224 points)
 constexpr int kDProdLanes = 64;            // ... and its producer lanes (2 warps)
@@ -37,6 +43,15 @@ constexpr int kDStageRows = 64 + kDNP;             // rows of D plus points of P
 constexpr int kDStage = kDStageRows * kDKC;        // doubles per stage
 constexpr int kDPartCols = 448;                    // max of (row blocks per M-tile) x (points of the CTA): 7 x 64
 constexpr int kDPrefetchLead = 6;                  // stages before the M-tile epilogue at which its operands are prefetched to L2
+
+// AIMS_PROBE_WARP_CYCLES (probe builds only): per-warp cycle counters -- [0] waiting for a stage (MMA warps: full barrier,
+// producers: empty barrier), [1] M-tile epilogues (MMA warps) / gather + copy issue (producers); a few CTAs print theirs.
+#ifdef AIMS_PROBE_WARP_CYCLES
+__device__ __forceinline__ long long *probe_wc() { __shared__ long long s[16][4]; return s[threadIdx.x >> 5]; }
+#define AIMS_TIMED(idx, ...) { const long long t0_ = clock64(); __VA_ARGS__; if ((threadIdx.x & 31) == 0) probe_wc()[idx] += clock64() - t0_; }
+#else
+#define AIMS_TIMED(idx, ...) { __VA_ARGS__; }
+#endif
 
 struct DItem { int b, p0, npt, pad; };     // points [p0, p0+npt) of batch b; p0 and npt multiples of 8
 
@@ -78,7 +93,7 @@ template <int WA, int WB>
 __device__ __forceinline__ void d_mma_kloop_t(double (&acc)[4][4][2], const double *sAl, const double *sBl, int tm, int nkc,
                                               int nnz8, int &step, unsigned bar_full, unsigned bar_empty, int lane) {
   int s = step % kDStages;
-  mbar_wait(bar_full + 8 * s, (unsigned)(step / kDStages) & 1u);
+  AIMS_TIMED(0, mbar_wait(bar_full + 8 * s, (unsigned)(step / kDStages) & 1u))
   const double *tA = sAl + (size_t)s * kDStage, *tB = sBl + (size_t)s * kDStage;
   double fa[WA], fb[WB];
 #pragma unroll
@@ -99,7 +114,7 @@ __device__ __forceinline__ void d_mma_kloop_t(double (&acc)[4][4][2], const doub
       if (last) {
         if (more_stages) {
           const int s1 = (step + 1) % kDStages;
-          mbar_wait(bar_full + 8 * s1, (unsigned)((step + 1) / kDStages) & 1u);
+          AIMS_TIMED(0, mbar_wait(bar_full + 8 * s1, (unsigned)((step + 1) / kDStages) & 1u))
           a1 = sAl + (size_t)s1 * kDStage; b1 = sBl + (size_t)s1 * kDStage;
         } else {
           a1 = tA; b1 = tB;                      // nothing follows: harmless reload of this stage's first step
@@ -165,50 +180,72 @@ __device__ __forceinline__ void d_mma_kloop(int variant, double (&acc)[4][4][2],
 // to nnz(B) ("calculate_density_mat"), written as [4-function group][row][4] into dA.  pl = 0..63.
 __device__ __forceinline__ void d_gather_tile(double *dA, const double *M, int i0, int tm, int k0, int nnz, int nnz8, int nact,
                                               const int *sInfo, const int *sLd, const long long *ptab, int pl, int nprod) {
-  // D_b[i0 + r][k0 + 4t .. +3]: one (row, 4-function group) per lane and pass; gathered from the block pattern
-  // (stored block (si,sj) for si <= sj, transposed read of block (sj,si) below the diagonal)
+  // D_b[i0 + r][k0 + 4t .. +3]: one (row, 4-function group) unit = four 8-byte copies, gathered from the block pattern
+  // (stored block (si,sj) for si <= sj, transposed read of block (sj,si) below the diagonal).  The column side of a stage is
+  // the same for every row, so it is decoded once per lane (registers); a row is decoded once per stage; what is left per
+  // unit is one table look-up (block offset of the atom pair) and the address -- four independent units per row.
   const int ng = min(kDKC, nnz8 - k0) >> 2;          // 4-function groups with at least one real function
-  for (int t = 0; t < ng; t++)
+  int sjt[4], cjt[4], ldjt[4];                       // atom slot / first column / ld of group t; sjt < 0: not 4 functions of one atom
+#pragma unroll
+  for (int t = 0; t < 4; t++) {
+    sjt[t] = -1; cjt[t] = 0; ldjt[t] = 0;
+    if (t < ng) {
+      const int4 fj4 = *reinterpret_cast<const int4 *>(sInfo + k0 + 4 * t);   // sInfo is padded with -1 up to nnz8
+      if (fj4.w >= 0 && (fj4.x >> 16) == (fj4.w >> 16) && (fj4.w - fj4.x) == 3) {
+        sjt[t] = fj4.x >> 16; cjt[t] = fj4.x & 0xFFFF; ldjt[t] = sLd[sjt[t]];
+      }
+    }
+  }
   for (int r = pl; r < tm; r += nprod) {             // consecutive lanes -> consecutive rows (transposed reads coalesce)
-    const int i = i0 + r, j = k0 + 4 * t;
-    const unsigned dst = smem_u32(dA + (t * tm + r) * 4);
+    const int i = i0 + r;
     if (i >= nnz) {
 #pragma unroll
-      for (int q = 0; q < 4; q++) cp_async8(dst + 8u * q, M, 0);
+      for (int t = 0; t < 4; t++)
+        if (t < ng) {
+          const unsigned dst = smem_u32(dA + (t * tm + r) * 4);
+#pragma unroll
+          for (int q = 0; q < 4; q++) cp_async8(dst + 8u * q, M, 0);
+        }
       continue;
     }
     const int fi = sInfo[i];
     const int si = fi >> 16, ri = fi & 0xFFFF;
-    const int4 fj4 = *reinterpret_cast<const int4 *>(sInfo + j);   // sInfo is padded with -1 up to nnz8
-    const int fjq[4] = {fj4.x, fj4.y, fj4.z, fj4.w};
-    if (fj4.w >= 0 && (fj4.x >> 16) == (fj4.w >> 16) && (fj4.w - fj4.x) == 3) {
-      // fast path: four consecutive functions of one atom
-      const int sj = fj4.x >> 16, cj = fj4.x & 0xFFFF;
-      const long long base = ptab[si * nact + sj];
-      const double *src = M;
-      long long stride = 0;
-      int bytes = 0;
-      if (base >= 0) {
-        bytes = 8;
-        if (si <= sj) { src = M + base + (long long)ri * sLd[sj] + cj; stride = 1; }
-        else { src = M + base + (long long)cj * sLd[si] + ri; stride = sLd[si]; }
-      }
+    const long long *prow = ptab + si * nact;
+    const int ldi = sLd[si];
 #pragma unroll
-      for (int q = 0; q < 4; q++) cp_async8(dst + 8u * q, src + q * stride, bytes);
-    } else {
-#pragma unroll
-      for (int q = 0; q < 4; q++) {
+    for (int t = 0; t < 4; t++) {
+      if (t >= ng) continue;
+      const unsigned dst = smem_u32(dA + (t * tm + r) * 4);
+      if (sjt[t] >= 0) {
+        // fast path: four consecutive functions of one atom
+        const int sj = sjt[t];
+        const long long base = prow[sj];
         const double *src = M;
+        long long stride = 0;
         int bytes = 0;
-        if (fjq[q] >= 0) {
-          const int sj = fjq[q] >> 16, cj = fjq[q] & 0xFFFF;
-          const long long base = ptab[si * nact + sj];
-          if (base >= 0) {
-            src = (si <= sj) ? M + base + (long long)ri * sLd[sj] + cj : M + base + (long long)cj * sLd[si] + ri;
-            bytes = 8;
-          }
+        if (base >= 0) {
+          bytes = 8;
+          if (si <= sj) { src = M + base + (long long)ri * ldjt[t] + cjt[t]; stride = 1; }
+          else { src = M + base + (long long)cjt[t] * ldi + ri; stride = ldi; }
         }
-        cp_async8(dst + 8u * q, src, bytes);
+#pragma unroll
+        for (int q = 0; q < 4; q++) cp_async8(dst + 8u * q, src + q * stride, bytes);
+      } else {
+#pragma unroll
+        for (int q = 0; q < 4; q++) {
+          const int fj = sInfo[k0 + 4 * t + q];
+          const double *src = M;
+          int bytes = 0;
+          if (fj >= 0) {
+            const int sj = fj >> 16, cj = fj & 0xFFFF;
+            const long long base = prow[sj];
+            if (base >= 0) {
+              src = (si <= sj) ? M + base + (long long)ri * sLd[sj] + cj : M + base + (long long)cj * ldi + ri;
+              bytes = 8;
+            }
+          }
+          cp_async8(dst + 8u * q, src, bytes);
+        }
       }
     }
   }
@@ -284,6 +321,10 @@ __device__ __forceinline__ void d_density_body(const DevSys &S, const BatchLists
     d_deal_blocks(s_map, PB, IB, psub, nmma);
   }
   __syncthreads();
+#ifdef AIMS_PROBE_WARP_CYCLES
+  if (lane == 0) { long long *w = probe_wc(); w[0] = 0; w[1] = 0; w[2] = clock64(); }
+  __syncwarp();
+#endif
   const long long *ptab = A.ptab_in_smem ? sPtab : gptab;
   const double *gP = A.P + boff;
 
@@ -299,8 +340,11 @@ __device__ __forceinline__ void d_density_body(const DevSys &S, const BatchLists
 #pragma unroll 1
       for (int kc = 0; kc < nkc; kc++, step++) {
       const int s = step % kDStages;
-      if (step >= kDStages) mbar_wait(bar_empty + 8 * s, (unsigned)(step / kDStages - 1) & 1u);
+      if (step >= kDStages) AIMS_TIMED(0, mbar_wait(bar_empty + 8 * s, (unsigned)(step / kDStages - 1) & 1u))
       const int k0 = kc * kDKC;
+#ifdef AIMS_PROBE_WARP_CYCLES
+      const long long tg0 = clock64();
+#endif
       if (kc == max(nkc - kDPrefetchLead, 0)) {
         // operands of this M-tile's epilogue (rows [i0, i0+tm) of Phi and grad Phi at the CTA's points): whole 16-row
         // chunks are contiguous in the density layout -> one bulk L2 prefetch per chunk and plane
@@ -319,6 +363,9 @@ __device__ __forceinline__ void d_density_body(const DevSys &S, const BatchLists
       }
       d_gather_tile(sA + (size_t)s * kDStage, A.D, i0, tm, k0, nnz, nnz8, nact, sInfo, sLd, ptab, pl, nprod);
       cp_async_mbar_arrive_noinc(bar_full + 8 * s);
+#ifdef AIMS_PROBE_WARP_CYCLES
+      if (lane == 0) probe_wc()[1] += clock64() - tg0;
+#endif
       }
     }
   } else {
@@ -350,7 +397,24 @@ __device__ __forceinline__ void d_density_body(const DevSys &S, const BatchLists
       const int aoffl = (ri0 - i0) * 4 + lane;
       d_mma_kloop(blive ? variant : 0, acc, sA + aoffl, sB + boffl, tm, nkc, nnz8, step, bar_full, bar_empty, lane);
 
+#ifdef AIMS_PROBE_WARP_CYCLES
+      const long long te0 = clock64();
+#endif
+      // AIMS_PROBE_NO_D_EPILOGUE (probe builds only; results are NOT n): the bound of the K loops alone; the accumulators stay
+      // live through a store that never happens (ptxas removes DMMAs whose results are dead)
+#ifdef AIMS_PROBE_NO_D_EPILOGUE
       if (blive) {
+        double sum = 0.0;
+#pragma unroll
+        for (int a = 0; a < 4; a++)
+#pragma unroll
+          for (int c = 0; c < 4; c++) sum += acc[a][c][0] + acc[a][c][1];
+        if (sum == 12345.678) sPart[lane] = sum;
+      }
+      if (false) {
+#else
+      if (blive) {
+#endif
         // ---- M-tile epilogue: n_p += sum_i Phi_ip temp_ip (and gradient), rows reduced by shuffles
 #pragma unroll
         for (int c = 0; c < 4; c++) {
@@ -416,9 +480,19 @@ __device__ __forceinline__ void d_density_body(const DevSys &S, const BatchLists
 #pragma unroll
           for (int c = 0; c < 4; c++) { acc[a][c][0] = 0.0; acc[a][c][1] = 0.0; }
       }
+#ifdef AIMS_PROBE_WARP_CYCLES
+      if (lane == 0) probe_wc()[1] += clock64() - te0;
+#endif
     }
   }
   __syncthreads();
+#ifdef AIMS_PROBE_WARP_CYCLES
+  if ((blockIdx.x & 1023) == 517 && lane == 0) {
+    const long long *w = probe_wc();
+    printf("WC cta %d b %d nnz %d npt %d warp %2d %s map %d total %lld wait %lld %s %lld\n", (int)blockIdx.x, b, nnz, npt, warp,
+           warp >= nmma ? "prod" : "mma ", warp < nmma ? s_map[warp] : -1, clock64() - w[2], w[0], warp >= nmma ? "gather" : "epilogue", w[1]);
+  }
+#endif
 
   // ---- S3d: store (mapping to the global point array is the identity on the batch's contiguous range)
   for (int col = tid; col < npt; col += kDThreads) {

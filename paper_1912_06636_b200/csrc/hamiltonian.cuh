@@ -290,6 +290,19 @@ __global__ void __launch_bounds__(kHThreads, 2) k_hamiltonian(DevSys S, BatchLis
     }
     __syncwarp();
   }
+  // AIMS_PROBE_H_EPILOGUE (probe builds only, build.py --define/--tag; results are NOT H): 0 = no scatter at all (the bound of
+  // the main loop), 1 = plain stores instead of REDs (what the atomic unit costs beyond the store traffic); profiles/r02_scatter.md
+#if defined(AIMS_PROBE_H_EPILOGUE) && AIMS_PROBE_H_EPILOGUE == 0
+  {   // keep the accumulators live through a store that never happens (ptxas removes DMMAs whose results are dead)
+    double sum = 0.0;
+#pragma unroll
+    for (int a = 0; a < 4; a++)
+#pragma unroll
+      for (int c = 0; c < 4; c++) sum += acc[a][c][0] + acc[a][c][1];
+    if (sum == 12345.678) s_strip[lane] = sum;
+  }
+#endif
+#if !defined(AIMS_PROBE_H_EPILOGUE) || AIMS_PROBE_H_EPILOGUE != 0
   double *strip = s_strip + warp * (8 * kHStripLd);
   const int fr = lane >> 2, fk = lane & 3;
   const long long *ptab = L.ptab + L.ptab_off[b];
@@ -318,13 +331,19 @@ __global__ void __launch_bounds__(kHThreads, 2) k_hamiltonian(DevSys S, BatchLis
           if (si != cur_si) { cur_si = si; base = __ldg(ptab + si * nact + sj); }   // rows of one atom share the block
           if (base < 0) continue;                             // atom pair outside the pattern: exact zero
           const double val = strip[r * kHStripLd + lane];
+#if defined(AIMS_PROBE_H_EPILOGUE) && AIMS_PROBE_H_EPILOGUE == 1
+          A.H[base + (long long)ra * ldj + cb] = val;
+          if (si == sj && !(diag && csub == a)) A.H[base + (long long)cb * ldj + ra] = val;
+#else
           red_add_f64(A.H + base + (long long)ra * ldj + cb, val);
           // diagonal atom block holds the full square: mirror unless (col,row) is itself computed (same diagonal sub-tile)
           if (si == sj && !(diag && csub == a)) red_add_f64(A.H + base + (long long)cb * ldj + ra, val);
+#endif
         }
       }
     }
   }
+#endif
   if (A.det) {
     __threadfence();                                   // this warp's adds are performed before it reports
     __syncwarp();
