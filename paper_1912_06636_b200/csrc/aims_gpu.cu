@@ -17,6 +17,7 @@
 #include "common.cuh"
 #include "density.cuh"
 #include "density2.cuh"
+#include "density_b.cuh"
 #include "forces.cuh"
 #include "hessian.cuh"
 #include "partition.cuh"
@@ -53,9 +54,15 @@ struct aims_gpu_ctx {
   HTile *d_tiles = nullptr;
   DItem *d_items = nullptr;
   double flops_h_lda = 0, flops_h_gga = 0, flops_den = 0;
-  bool ptab_in_smem = true, f_ptab_in_smem = true, x_ptab_in_smem = true;
+  bool ptab_in_smem = true, f_ptab_in_smem = true, x_ptab_in_smem = true, b_ptab_in_smem = true;
   std::vector<DItem> h_items;                                  // host copy of the density work items
   std::map<std::pair<int, int>, int *> item_order;             // (bs, be) -> device permutation, heaviest item first
+  // density_b.cuh: items of 192..224 points (update_density only; forces / Hessian keep every item in `items`)
+  bool balanced_density = true;
+  std::vector<long long> itemb_off, itemg_off;                 // per batch: balanced items / the other ("generic") items
+  DItem *d_itemsb = nullptr, *d_itemsg = nullptr;
+  std::vector<DItem> h_itemsb, h_itemsg;
+  std::map<std::pair<int, int>, int *> itemb_order, itemg_order;
   // density2.cuh (bulk-copy pipeline): used when no atom of any batch is partially culled
   bool fast_density = false, d2_pblk_in_smem = true;
   std::vector<int> kq;                                         // K'' rows per batch
@@ -226,6 +233,73 @@ __global__ void __launch_bounds__(512, 1) k_dmma_probe(double *out, int iters, d
   if (s == 12345.678) out[0] = s;
 }
 
+// Second operand-pattern probe: a (WA x WB) accumulator block per warp, WA*WB DMMAs per step.
+//   INPLACE = true : the K-step body of d_mma_kloop_t / b_mma_kloop_t -- a fragment is reloaded in place (same register) as soon
+//                    as the row of DMMAs that used it has been issued;
+//   INPLACE = false: the fragments of step t+1 are loaded into a second register set before the DMMAs of step t.
+template <int WA, int WB, bool INPLACE>
+__global__ void __launch_bounds__(640) k_dmma_probe2(double *out, int iters, double a0) {
+  __shared__ double sm[4096];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int i = threadIdx.x; i < 4096; i += blockDim.x) sm[i] = 1e-9 * i + a0;
+  __syncthreads();
+  double acc[WA][WB][2];
+#pragma unroll
+  for (int a = 0; a < WA; a++)
+#pragma unroll
+    for (int c = 0; c < WB; c++) { acc[a][c][0] = a + lane; acc[a][c][1] = c; }
+  const double *tA = sm + lane + (warp & 1) * 1024, *tB = sm + 2048 + lane + (warp & 1) * 1024;
+  double fa[WA], fb[WB];
+#pragma unroll
+  for (int a = 0; a < WA; a++) fa[a] = tA[a * 32];
+#pragma unroll
+  for (int c = 0; c < WB; c++) fb[c] = tB[c * 32];
+  if (INPLACE) {
+#pragma unroll 1
+    for (int it = 0; it < iters; it++) {
+      const double *a1 = tA + ((it + 1) & 3) * 256, *b1 = tB + ((it + 1) & 3) * 256;
+#pragma unroll
+      for (int a = 0; a < WA; a++) {
+#pragma unroll
+        for (int c = 0; c < WB; c++) {
+          dmma8x8x4(acc[a][c][0], acc[a][c][1], fa[a], fb[c]);
+          if (a == WA - 1) fb[c] = b1[c * 32];
+        }
+        fa[a] = a1[a * 32];
+      }
+    }
+  } else {
+    double na[WA], nb[WB];
+#pragma unroll 1
+    for (int it = 0; it < iters; it += 2) {
+      const double *a1 = tA + ((it + 1) & 3) * 256, *b1 = tB + ((it + 1) & 3) * 256;
+      const double *a2 = tA + ((it + 2) & 3) * 256, *b2 = tB + ((it + 2) & 3) * 256;
+#pragma unroll
+      for (int a = 0; a < WA; a++) na[a] = a1[a * 32];
+#pragma unroll
+      for (int c = 0; c < WB; c++) nb[c] = b1[c * 32];
+#pragma unroll
+      for (int a = 0; a < WA; a++)
+#pragma unroll
+        for (int c = 0; c < WB; c++) dmma8x8x4(acc[a][c][0], acc[a][c][1], fa[a], fb[c]);
+#pragma unroll
+      for (int a = 0; a < WA; a++) fa[a] = a2[a * 32];
+#pragma unroll
+      for (int c = 0; c < WB; c++) fb[c] = b2[c * 32];
+#pragma unroll
+      for (int a = 0; a < WA; a++)
+#pragma unroll
+        for (int c = 0; c < WB; c++) dmma8x8x4(acc[a][c][0], acc[a][c][1], na[a], nb[c]);
+    }
+  }
+  double s = 0;
+#pragma unroll
+  for (int a = 0; a < WA; a++)
+#pragma unroll
+    for (int c = 0; c < WB; c++) s += acc[a][c][0] + acc[a][c][1];
+  if (s == 12345.678) out[0] = s;
+}
+
 bool range_ok(const aims_gpu_ctx *c, int b0, int b1) { return c && b0 >= 0 && b1 >= b0 && b1 <= c->n_batches; }
 
 // Every extern "C" entry runs its body through this: no C++ exception (std::bad_alloc of the host-side tables and
@@ -265,6 +339,7 @@ cudaError_t smem_optin_all(int device, size_t optin) {
   AIMS_OPTIN(k_hamiltonian<false>) AIMS_OPTIN(k_hamiltonian<true>)
   AIMS_OPTIN(k_density<false>) AIMS_OPTIN(k_density<true>)
   AIMS_OPTIN(k_density2<false>) AIMS_OPTIN(k_density2<true>)
+  AIMS_OPTIN(k_density_b<false>) AIMS_OPTIN(k_density_b<true>)
   AIMS_OPTIN(k_density_hessian)
   AIMS_OPTIN((k_forces<false, false>)) AIMS_OPTIN((k_forces<true, false>))
   AIMS_OPTIN((k_forces<false, true>)) AIMS_OPTIN((k_forces<true, true>))
@@ -438,10 +513,14 @@ static int impl_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_
   c->fn_off.assign(nb + 1, 0); c->act_off.assign(nb + 1, 0); c->ptab_off.assign(nb + 1, 0);
   c->pad_off.assign(nb + 1, 0); c->pad16_off.assign(nb + 1, 0); c->dpad_off.assign(nb + 1, 0); c->api_off.assign(nb + 1, 0); c->tile_off.assign(nb + 1, 0); c->item_off.assign(nb + 1, 0);
   std::vector<HTile> tiles;
-  std::vector<DItem> items, items2;
+  std::vector<DItem> items, items2, itemsb, itemsg;
   c->dq_off.assign(nb + 1, 0); c->item2_off.assign(nb + 1, 0);
+  c->itemb_off.assign(nb + 1, 0); c->itemg_off.assign(nb + 1, 0);
+#ifndef AIMS_PROBE_BALANCED_DENSITY
+  c->balanced_density = false;       // density_b.cuh is a measured-and-rejected variant (profiles/r02_kernel_experiments.md): probe builds only
+#endif
 #ifdef AIMS_PROBE_DENSITY2
-  c->fast_density = true;            // probe build only: the bulk-copy / two-CTA density pipeline (profiles/r02_density2_history.md)
+  c->fast_density = true;            // probe build only: the bulk-copy / two-CTA density pipeline (profiles/r02_kernel_experiments.md)
 #else
   c->fast_density = false;
 #endif
@@ -499,7 +578,11 @@ static int impl_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_
         }
       }
     }
+    for (size_t q = (size_t)c->item_off[b]; q < items.size(); q++)
+      (c->balanced_density && b_item_ok(items[q].npt) ? itemsb : itemsg).push_back(items[q]);
     c->item_off[b + 1] = (long long)items.size();
+    c->itemb_off[b + 1] = (long long)itemsb.size();
+    c->itemg_off[b + 1] = (long long)itemsg.size();
     c->flops_h_lda += (double)np * nz * (nz + 1.0);
     c->flops_h_gga += 2.0 * np * (double)nz * nz;
     c->flops_den += 2.0 * np * (double)nz * nz;
@@ -515,6 +598,9 @@ static int impl_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_
   if ((rc = dev_upload<HTile>(c, &c->d_tiles, tiles.data(), tiles.size()))) return rc;
   if ((rc = dev_upload<DItem>(c, &c->d_items, items.data(), items.size()))) return rc;
   c->h_items = items;
+  if ((rc = dev_upload<DItem>(c, &c->d_itemsb, itemsb.data(), itemsb.size()))) return rc;
+  if ((rc = dev_upload<DItem>(c, &c->d_itemsg, itemsg.data(), itemsg.size()))) return rc;
+  c->h_itemsb = itemsb; c->h_itemsg = itemsg;
   if ((rc = dev_upload<DItem>(c, &c->d_items2, items2.data(), items2.size()))) return rc;
   c->h_items2 = items2;
   if ((rc = dev_upload<long long>(c, &c->d_dq_off, c->dq_off.data(), c->dq_off.size()))) return rc;
@@ -572,6 +658,9 @@ static int impl_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_
   const int mact = std::max(c->max_act, 1);
   c->ptab_in_smem = d_smem_bytes(c->max_nnz, mact, true) <= lim;
   if (d_smem_bytes(c->max_nnz, mact, c->ptab_in_smem) > lim)
+    return fail(c, AIMS_ERR_UNSUPPORTED, "nnz(B) too large for the density kernel's shared memory");
+  c->b_ptab_in_smem = b_smem_bytes(c->max_nnz, mact, true) <= lim;
+  if (b_smem_bytes(c->max_nnz, mact, c->b_ptab_in_smem) > lim)
     return fail(c, AIMS_ERR_UNSUPPORTED, "nnz(B) too large for the density kernel's shared memory");
   c->x_ptab_in_smem = x_smem_bytes(c->max_nnz, mact, true) <= lim;
   c->f_ptab_in_smem = f_smem_bytes(c->max_nnz, mact, true) <= lim;
@@ -640,10 +729,15 @@ int chunk_end(const aims_gpu_ctx *c, const std::vector<long long> &off, int bs, 
 
 // Launch order of the density items of batches [bs, be): heaviest (largest nnz) first, so that the last CTAs of a launch
 // are the cheapest ones (a CTA's cost varies by 50x over a slab).  Built once per distinct range and kept on the device.
-int density_order(aims_gpu_ctx *c, int bs, int be, const int **out, bool v2 = false) {
-  const std::vector<long long> &ioff = v2 ? c->item2_off : c->item_off;
-  const std::vector<DItem> &hitems = v2 ? c->h_items2 : c->h_items;
-  std::map<std::pair<int, int>, int *> &cache = v2 ? c->item2_order : c->item_order;
+enum { kItemsAll = 0, kItemsV2 = 1, kItemsBalanced = 2, kItemsGeneric = 3 };
+int density_order(aims_gpu_ctx *c, int bs, int be, const int **out, int which = kItemsAll) {
+  const bool v2 = which == kItemsV2;
+  const std::vector<long long> &ioff = which == kItemsV2 ? c->item2_off : which == kItemsBalanced ? c->itemb_off
+                                       : which == kItemsGeneric ? c->itemg_off : c->item_off;
+  const std::vector<DItem> &hitems = which == kItemsV2 ? c->h_items2 : which == kItemsBalanced ? c->h_itemsb
+                                     : which == kItemsGeneric ? c->h_itemsg : c->h_items;
+  std::map<std::pair<int, int>, int *> &cache = which == kItemsV2 ? c->item2_order : which == kItemsBalanced ? c->itemb_order
+                                                : which == kItemsGeneric ? c->itemg_order : c->item_order;
   const long long i0 = ioff[bs], i1 = ioff[be];
   if (i1 - i0 <= 2ll * c->sm_count) { *out = nullptr; return AIMS_OK; }   // fewer items than two waves: any order
   auto key = std::make_pair(bs, be);
@@ -818,7 +912,7 @@ static int impl_update_density(aims_gpu_ctx *c, int32_t b0, int32_t b1, const do
       const long long ni = c->item2_off[be] - c->item2_off[bs];
       if (ni > 0) {
         D2Args A{};
-        if ((rc = density_order(c, bs, be, &A.order, true))) return rc;
+        if ((rc = density_order(c, bs, be, &A.order, kItemsV2))) return rc;
         A.items = c->d_items2 + c->item2_off[bs];
         A.P = E.plane[0];
         for (int q = 0; q < 3; q++) A.G[q] = grad_n ? E.plane[q + 1] : nullptr;
@@ -846,19 +940,29 @@ static int impl_update_density(aims_gpu_ctx *c, int32_t b0, int32_t b1, const do
     E.pad_off = c->d_dpad_off; E.pad_base = c->dpad_off[bs];
     E.n_points = c->n_points;
     if (grad_n) launch_eval<kEvalPhiGrad, kLayD>(c, E, bs, be); else launch_eval<kEvalPhi, kLayD>(c, E, bs, be);
-    const long long ni = c->item_off[be] - c->item_off[bs];
-    if (ni > 0) {
-      DArgs A{};
-      if ((rc = density_order(c, bs, be, &A.order))) return rc;
-      A.items = c->d_items + c->item_off[bs];
-      A.P = E.plane[0];
-      for (int q = 0; q < 3; q++) A.G[q] = grad_n ? E.plane[q + 1] : nullptr;
-      A.pad_off = c->d_dpad_off; A.pad_base = c->dpad_off[bs];
-      A.D = D_values; A.n = n; A.gn = grad_n; A.n_points = c->n_points; A.max_nnz_pad = c->max_nnz;
+    // items of 192..224 points (all of a 200-point configuration) -> k_density_b, the others -> k_density
+    const long long nib = c->itemb_off[be] - c->itemb_off[bs], nig = c->itemg_off[be] - c->itemg_off[bs];
+    DArgs A{};
+    A.P = E.plane[0];
+    for (int q = 0; q < 3; q++) A.G[q] = grad_n ? E.plane[q + 1] : nullptr;
+    A.pad_off = c->d_dpad_off; A.pad_base = c->dpad_off[bs];
+    A.D = D_values; A.n = n; A.gn = grad_n; A.n_points = c->n_points; A.max_nnz_pad = c->max_nnz;
+    if (nib > 0) {
+      if ((rc = density_order(c, bs, be, &A.order, kItemsBalanced))) return rc;
+      A.items = c->d_itemsb + c->itemb_off[bs];
+      A.ptab_in_smem = c->b_ptab_in_smem ? 1 : 0;
+      const size_t bsm = b_smem_bytes(c->max_nnz, std::max(c->max_act, 1), c->b_ptab_in_smem);
+      TimedLaunch t(c, kKindDen);
+      if (grad_n) k_density_b<true><<<(unsigned)nib, kBThreads, bsm, c->stream>>>(c->S, c->L, A, std::max(c->max_act, 1));
+      else k_density_b<false><<<(unsigned)nib, kBThreads, bsm, c->stream>>>(c->S, c->L, A, std::max(c->max_act, 1));
+    }
+    if (nig > 0) {
+      if ((rc = density_order(c, bs, be, &A.order, kItemsGeneric))) return rc;
+      A.items = c->d_itemsg + c->itemg_off[bs];
       A.ptab_in_smem = c->ptab_in_smem ? 1 : 0;
       TimedLaunch t(c, kKindDen);
-      if (grad_n) k_density<true><<<(unsigned)ni, kDThreads, dsm, c->stream>>>(c->S, c->L, A, std::max(c->max_act, 1));
-      else k_density<false><<<(unsigned)ni, kDThreads, dsm, c->stream>>>(c->S, c->L, A, std::max(c->max_act, 1));
+      if (grad_n) k_density<true><<<(unsigned)nig, kDThreads, dsm, c->stream>>>(c->S, c->L, A, std::max(c->max_act, 1));
+      else k_density<false><<<(unsigned)nig, kDThreads, dsm, c->stream>>>(c->S, c->L, A, std::max(c->max_act, 1));
     }
     if ((rc = check_async(c))) return rc;
     bs = be;
@@ -1121,7 +1225,8 @@ static int impl_synchronize(aims_gpu_ctx *c) {
 }
 
 static int impl_dmma_probe(aims_gpu_ctx *c, int variant, int warps_per_sm, double *tflops) {
-  if (!c || !tflops || variant < 1 || variant > 3 || warps_per_sm < 1 || warps_per_sm > 16) return fail(c, AIMS_ERR_INVALID_ARG, "variant 1..3, warps_per_sm 1..16");
+  if (!c || !tflops || variant < 1 || variant > 9 || warps_per_sm < 1 || warps_per_sm > (variant <= 3 ? 16 : 20))
+    return fail(c, AIMS_ERR_INVALID_ARG, "variant 1..9, warps_per_sm 1..16 (variants 4..9: 1..20)");
   CU_TRY(c, cudaSetDevice(c->device));
   if (!c->probe_out) { int rc = dev_alloc(c, &c->probe_out, 16); if (rc) return rc; }   // scratch of the probes, allocated once
   double *out = c->probe_out;
@@ -1133,7 +1238,13 @@ static int impl_dmma_probe(aims_gpu_ctx *c, int variant, int warps_per_sm, doubl
     if (rep == 1) CU_TRY(c, cudaEventRecord(e0, c->stream));
     if (variant == 1) k_dmma_probe<1><<<c->sm_count, threads, 0, c->stream>>>(out, iters, 1.0000001, 1e-9);
     else if (variant == 2) k_dmma_probe<2><<<c->sm_count, threads, 0, c->stream>>>(out, iters, 1.0000001, 1e-9);
-    else k_dmma_probe<3><<<c->sm_count, threads, 0, c->stream>>>(out, iters, 1.0000001, 1e-9);
+    else if (variant == 3) k_dmma_probe<3><<<c->sm_count, threads, 0, c->stream>>>(out, iters, 1.0000001, 1e-9);
+    else if (variant == 4) k_dmma_probe2<4, 4, true><<<c->sm_count, threads, 0, c->stream>>>(out, iters, 1e-9);
+    else if (variant == 5) k_dmma_probe2<4, 3, true><<<c->sm_count, threads, 0, c->stream>>>(out, iters, 1e-9);
+    else if (variant == 6) k_dmma_probe2<3, 3, true><<<c->sm_count, threads, 0, c->stream>>>(out, iters, 1e-9);
+    else if (variant == 7) k_dmma_probe2<4, 4, false><<<c->sm_count, threads, 0, c->stream>>>(out, iters, 1e-9);
+    else if (variant == 8) k_dmma_probe2<4, 3, false><<<c->sm_count, threads, 0, c->stream>>>(out, iters, 1e-9);
+    else k_dmma_probe2<2, 2, true><<<c->sm_count, threads, 0, c->stream>>>(out, iters, 1e-9);
     c->launches++;
   }
   CU_TRY(c, cudaEventRecord(e1, c->stream));
@@ -1141,7 +1252,8 @@ static int impl_dmma_probe(aims_gpu_ctx *c, int variant, int warps_per_sm, doubl
   float ms = 0;
   CU_TRY(c, cudaEventElapsedTime(&ms, e0, e1));
   cudaEventDestroy(e0); cudaEventDestroy(e1);
-  *tflops = 2.0 * 256 * 16 * (double)iters * c->sm_count * warps_per_sm / (ms * 1e-3) * 1e-12;
+  const int per_step[10] = {0, 16, 16, 16, 16, 12, 9, 16, 12, 4};        // DMMAs per step and warp
+  *tflops = 2.0 * 256 * per_step[variant] * (double)iters * c->sm_count * warps_per_sm / (ms * 1e-3) * 1e-12;
   return check_async(c);
 }
 

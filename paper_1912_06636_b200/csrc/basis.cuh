@@ -324,7 +324,7 @@ enum EvalLayout { kLayApi = 0, kLayH = 1, kLayD = 2, kLayD2 = 3 };
 #ifndef AIMS_EVAL_CTAS_PER_SM
 #define AIMS_EVAL_CTAS_PER_SM 2
 #endif
-// Threads of a k_eval CTA.  Measured on config 5 (profiles/r02_eval_variants.md): 224 threads (7 warps cover a 200-point batch
+// Threads of a k_eval CTA.  Measured on config 5 (profiles/r02_kernel_experiments.md): 224 threads (7 warps cover a 200-point batch
 // in one pass, 144 registers per thread at two CTAs per SM) are SLOWER than 256 (82.9 vs 63.2 ms per step) -- the kernel lives
 // on warps in flight, not on registers per thread.  The spline coefficients (a gather through L1/L2 per point and shell, the
 // largest stall of the round-1 kernel: long scoreboard 25 % / 46 % of the samples) are fetched one shell ahead.

@@ -47,10 +47,16 @@ constexpr int kDPrefetchLead = 6;                  // stages before the M-tile e
 // AIMS_PROBE_WARP_CYCLES (probe builds only): per-warp cycle counters -- [0] waiting for a stage (MMA warps: full barrier,
 // producers: empty barrier), [1] M-tile epilogues (MMA warps) / gather + copy issue (producers); a few CTAs print theirs.
 #ifdef AIMS_PROBE_WARP_CYCLES
-__device__ __forceinline__ long long *probe_wc() { __shared__ long long s[16][4]; return s[threadIdx.x >> 5]; }
+__device__ __forceinline__ long long *probe_wc() { __shared__ long long s[20][4]; return s[threadIdx.x >> 5]; }
 #define AIMS_TIMED(idx, ...) { const long long t0_ = clock64(); __VA_ARGS__; if ((threadIdx.x & 31) == 0) probe_wc()[idx] += clock64() - t0_; }
 #else
 #define AIMS_TIMED(idx, ...) { __VA_ARGS__; }
+#endif
+
+#ifdef AIMS_PROBE_D_NO_HANDSHAKE
+#define AIMS_HS(...)
+#else
+#define AIMS_HS(...) __VA_ARGS__
 #endif
 
 struct DItem { int b, p0, npt, pad; };     // points [p0, p0+npt) of batch b; p0 and npt multiples of 8
@@ -93,7 +99,7 @@ template <int WA, int WB>
 __device__ __forceinline__ void d_mma_kloop_t(double (&acc)[4][4][2], const double *sAl, const double *sBl, int tm, int nkc,
                                               int nnz8, int &step, unsigned bar_full, unsigned bar_empty, int lane) {
   int s = step % kDStages;
-  AIMS_TIMED(0, mbar_wait(bar_full + 8 * s, (unsigned)(step / kDStages) & 1u))
+  AIMS_HS(AIMS_TIMED(0, mbar_wait(bar_full + 8 * s, (unsigned)(step / kDStages) & 1u)))
   const double *tA = sAl + (size_t)s * kDStage, *tB = sBl + (size_t)s * kDStage;
   double fa[WA], fb[WB];
 #pragma unroll
@@ -114,7 +120,7 @@ __device__ __forceinline__ void d_mma_kloop_t(double (&acc)[4][4][2], const doub
       if (last) {
         if (more_stages) {
           const int s1 = (step + 1) % kDStages;
-          AIMS_TIMED(0, mbar_wait(bar_full + 8 * s1, (unsigned)((step + 1) / kDStages) & 1u))
+          AIMS_HS(AIMS_TIMED(0, mbar_wait(bar_full + 8 * s1, (unsigned)((step + 1) / kDStages) & 1u)))
           a1 = sAl + (size_t)s1 * kDStage; b1 = sBl + (size_t)s1 * kDStage;
         } else {
           a1 = tA; b1 = tB;                      // nothing follows: harmless reload of this stage's first step
@@ -143,7 +149,7 @@ __device__ __forceinline__ void d_mma_kloop_t(double (&acc)[4][4][2], const doub
     }
     // every fragment of stage s is in registers (the reloads above already read the next stage): release it
     __syncwarp();
-    if (lane == 0) mbar_arrive(bar_empty + 8 * s);
+    AIMS_HS(if (lane == 0) mbar_arrive(bar_empty + 8 * s);)
     step++;
     s = step % kDStages;
   }
@@ -154,9 +160,9 @@ __device__ __forceinline__ void d_idle_kloop(int nkc, int &step, unsigned bar_fu
 #pragma unroll 1
   for (int kc = 0; kc < nkc; kc++, step++) {
     const int s = step % kDStages;
-    mbar_wait(bar_full + 8 * s, (unsigned)(step / kDStages) & 1u);
+    AIMS_HS(mbar_wait(bar_full + 8 * s, (unsigned)(step / kDStages) & 1u);)
     __syncwarp();
-    if (lane == 0) mbar_arrive(bar_empty + 8 * s);
+    AIMS_HS(if (lane == 0) mbar_arrive(bar_empty + 8 * s);)
   }
 }
 
@@ -330,6 +336,9 @@ __device__ __forceinline__ void d_density_body(const DevSys &S, const BatchLists
 
   if (warp >= nmma) {
     // =========================================================================== producers
+#ifdef AIMS_PROBE_D_NO_HANDSHAKE
+    if (warp >= nmma) return;
+#endif
     const int pl = tid - nmma * 32;                // 0..63
     const int np8 = pad8(np);
     int step = 0;
@@ -355,13 +364,21 @@ __device__ __forceinline__ void d_density_body(const DevSys &S, const BatchLists
           bulk_prefetch_l2(base + ((long long)c * (np8 >> 2) + (p0 >> 2)) * 64, (unsigned)npt * 128u);
         }
       }
+      // AIMS_PROBE_D_NO_BULK / _NO_GATHER / _NO_HANDSHAKE (probe builds only; results are NOT n): what each part of the
+      // producer -> MMA hand-over costs, profiles/r02_kernel_experiments.md
       if (pl == nprod - 1) {
         // Phi rows [k0, k0+16) of every point of the CTA: ONE contiguous segment in the density layout
+#ifdef AIMS_PROBE_D_NO_BULK
+        mbar_arrive(bar_full + 8 * s);
+#else
         mbar_expect_tx(bar_full + 8 * s, (unsigned)npt * 128u);
         bulk_g2s(smem_u32(sB + (size_t)s * kDStage), gP + ((long long)kc * (np8 >> 2) + (p0 >> 2)) * 64, (unsigned)npt * 128u,
                  bar_full + 8 * s);
+#endif
       }
+#ifndef AIMS_PROBE_D_NO_GATHER
       d_gather_tile(sA + (size_t)s * kDStage, A.D, i0, tm, k0, nnz, nnz8, nact, sInfo, sLd, ptab, pl, nprod);
+#endif
       cp_async_mbar_arrive_noinc(bar_full + 8 * s);
 #ifdef AIMS_PROBE_WARP_CYCLES
       if (lane == 0) probe_wc()[1] += clock64() - tg0;

@@ -12,7 +12,7 @@
 //     set of 16-byte pieces with ONE table look-up each: every MMA warp copies its share of the next tile (two to four
 //     cp.async of 16 bytes per lane and stage) -- no 8-byte gathers, no transposed reads, no branches, no producer warps.
 //     (Issuing the runs as bulk copies, UBLKCP, from the lanes of one warp was measured first: per-lane operands of a
-//     uniform-datapath instruction are serialised, ~1,500 cycles per stage: profiles/r02_density2_history.md.)
+//     uniform-datapath instruction are serialised, ~1,500 cycles per stage: profiles/r02_kernel_experiments.md.)
 //   * A CTA is 8 MMA warps on a (batch, <= 128 points) item and two CTAs share an SM: one CTA's M-tile epilogue and set-up
 //     overlap the other's DMMAs, and the ragged sub-partition loads of the two CTAs (rotated by the CTA index) average out.
 // Only for batches whose active atoms keep ALL their shells (true whenever the shells of a species share one cutoff, as in
@@ -33,7 +33,7 @@ constexpr int kD2MaxPts = 104;            // points per CTA (4 blocks of <= 32; 
 //   1-2 point blocks (<= 64 points): tm = 128 -> 2112 + 1024 = 3136 doubles, THREE stages in the same 88 KB.
 // The refill of a stage is issued one stage after its release (so that the issuing warp never waits for the slowest
 // one), which leaves N - 2 stages of flight time for the copies: with three stages of 16 functions the 100-point items of
-// the first version waited on the "full" barriers for 19 % of their time (ncu, profiles/r02_density2_history.md).
+// the first version waited on the "full" barriers for 19 % of their time (ncu, profiles/r02_kernel_experiments.md).
 constexpr int kD2StageDoubles4 = 2752, kD2StageDoubles3 = 3136;
 constexpr int kD2SmemStageDoubles = 4 * kD2StageDoubles4;      // 11008 >= 3 * 3136
 constexpr int kD2PrefetchLead = 6;

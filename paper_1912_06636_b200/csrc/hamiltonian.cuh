@@ -24,11 +24,16 @@
 
 namespace aims {
 
-constexpr int kHI = 128;          // max rows of the I panel (4 blocks)
-constexpr int kHJ = 64;           // max rows of the J panel (2 blocks)
-constexpr int kHIB = 4, kHJB = 2; // blocks per panel
+#ifndef AIMS_H_IB
+#define AIMS_H_IB 4               // blocks of the I panel: 4 (8 warps, 2 CTAs per SM) or 2 (4 warps, 4 CTAs per SM; profiles/r02_kernel_experiments.md)
+#endif
+constexpr int kHIB = AIMS_H_IB, kHJB = 2; // blocks per panel
+constexpr int kHI = 32 * kHIB;    // max rows of the I panel
+constexpr int kHJ = 32 * kHJB;    // max rows of the J panel
+constexpr int kHWarps = kHIB * kHJB;      // one warp per block of a full tile
 constexpr int kHStages = 3;
-constexpr int kHThreads = 256;
+constexpr int kHThreads = 32 * kHWarps;
+constexpr int kHCtasPerSm = 16 / kHWarps;
 constexpr int kHStripLd = 40;     // row stride of a warp's 8-row staging strip (conflict-free 16-byte stores)
 
 struct HTile { int b; short ti, tj; };
@@ -60,7 +65,7 @@ template <bool GGA>
 __host__ __device__ constexpr int h_stage_doubles() { return h_stage_groups<GGA>() * h_group_doubles<GGA>(); }
 template <bool GGA>
 constexpr size_t h_smem_bytes() {
-  return (size_t)kHStages * h_stage_doubles<GGA>() * sizeof(double) + (size_t)8 * 8 * kHStripLd * sizeof(double) +
+  return (size_t)kHStages * h_stage_doubles<GGA>() * sizeof(double) + (size_t)kHWarps * 8 * kHStripLd * sizeof(double) +
          2 * kHStages * sizeof(unsigned long long) + (kHI + kHJ + kMaxActive) * sizeof(int);
 }
 
@@ -163,13 +168,13 @@ __device__ __forceinline__ void h_mma_loop(int variant, double (&acc)[4][4][2], 
 }
 
 template <bool GGA>
-__global__ void __launch_bounds__(kHThreads, 2) k_hamiltonian(DevSys S, BatchLists L, HArgs A) {
+__global__ void __launch_bounds__(kHThreads, kHCtasPerSm) k_hamiltonian(DevSys S, BatchLists L, HArgs A) {
   constexpr int NST = kHStages;
   constexpr int GW = h_group_doubles<GGA>(), SW = h_stage_doubles<GGA>();
   extern __shared__ __align__(128) unsigned char smem_raw[];
   double *sm = reinterpret_cast<double *>(smem_raw);
-  double *s_strip = sm + (size_t)NST * SW;                                  // [8 warps][8][kHStripLd]
-  unsigned long long *s_bar = reinterpret_cast<unsigned long long *>(s_strip + 8 * 8 * kHStripLd);   // full[NST], empty[NST]
+  double *s_strip = sm + (size_t)NST * SW;                                  // [warps][8][kHStripLd]
+  unsigned long long *s_bar = reinterpret_cast<unsigned long long *>(s_strip + kHWarps * 8 * kHStripLd);   // full[NST], empty[NST]
   int *s_rowinfo = reinterpret_cast<int *>(s_bar + 2 * NST);
   int *s_colinfo = s_rowinfo + kHI;
   int *s_ld = s_colinfo + kHJ;
@@ -205,7 +210,7 @@ __global__ void __launch_bounds__(kHThreads, 2) k_hamiltonian(DevSys S, BatchLis
   // the tile index so that the partly filled tiles along the diagonal load the four SM sub-partitions evenly.
   const int nI = bI1 - bI0, nJ = bJ1 - bJ0;
   int nlive = 0, my_bi = -1, my_bj = -1;
-  const int slot = (warp + (int)(blockIdx.x & 7)) & 7;
+  const int slot = (warp + (int)(blockIdx.x & (kHWarps - 1))) & (kHWarps - 1);
   for (int cj = 0; cj < nJ; cj++) {
     const int cnt = min(nI, bJ0 + cj - bI0 + 1);                  // blocks bi = bI0 .. bI0+cnt-1 are on or above the diagonal
     if (cnt > 0) {
@@ -291,7 +296,7 @@ __global__ void __launch_bounds__(kHThreads, 2) k_hamiltonian(DevSys S, BatchLis
     __syncwarp();
   }
   // AIMS_PROBE_H_EPILOGUE (probe builds only, build.py --define/--tag; results are NOT H): 0 = no scatter at all (the bound of
-  // the main loop), 1 = plain stores instead of REDs (what the atomic unit costs beyond the store traffic); profiles/r02_scatter.md
+  // the main loop), 1 = plain stores instead of REDs (what the atomic unit costs beyond the store traffic); profiles/r02_kernel_experiments.md
 #if defined(AIMS_PROBE_H_EPILOGUE) && AIMS_PROBE_H_EPILOGUE == 0
   {   // keep the accumulators live through a store that never happens (ptxas removes DMMAs whose results are dead)
     double sum = 0.0;
