@@ -7,7 +7,7 @@ computed using the exact same real-space integration code" (L113) -- plus atom_h
 import numpy as np
 
 from .bundle import bsr_pad_mask, build_bsr
-from .configs import (BASE_SEED, N_KNOTS, R0_KNOT, Bundle, _radial_norm, bisect_batches, build_splines, fibonacci_sphere,
+from .configs import (BASE_SEED, N_KNOTS, R0_KNOT, SPECIES, Bundle, _radial_norm, bisect_batches, build_splines, fibonacci_sphere,
                       partition_weights, radial_analytic, radial_grid, smooth_fields)
 
 LATTICE = np.array([[4.2, 0.0, 0.0], [0.6, 4.6, 0.0], [0.3, 0.5, 5.0]])      # rows a1, a2, a3 (Angstrom)
@@ -35,12 +35,36 @@ def _images(lat, frac_atoms, reach):
 
 
 def make_periodic(n_rad=24, n_ang=50, max_batch=100, rcut=4.0, seed=None, gaussian_s_only=None):
-    """Bundle of the periodic toy crystal, with three extra attributes: lattice [3][3], atom_home [n_atoms] (index of the
-    cell atom an atom is an image of) and atom_T [n_atoms][3] (its lattice translation, Angstrom).  Atoms 0..1 are the cell's."""
+    """Bundle of the periodic toy crystal, with extra attributes: lattice [3][3], frac [n_home][3], atom_home [n_atoms] (index of
+    the cell atom an atom is an image of), atom_T [n_atoms][3] (its lattice translation, Angstrom), xyz_unwrapped (the grid
+    points before they are mapped into the cell, in the batched order).  Atoms 0..n_home-1 are the cell's."""
     seed = BASE_SEED + 77 if seed is None else seed
     rng = np.random.default_rng(seed)
     lat = LATTICE.copy()
     frac = FRAC + rng.uniform(-0.02, 0.02, FRAC.shape)
+    return _make(lat, frac, SHELLS, rcut, n_rad, n_ang, max_batch, seed, rng, gaussian_s_only, "periodic")
+
+
+def make_periodic_si(n_cells=3, n_rad=60, n_ang=302, max_batch=200, seed=None, jitter=0.05):
+    """Periodic workload shaped like the paper's main benchmark (a diamond-Si supercell of 54 atoms): n_cells^3
+    primitive fcc cells of the diamond structure (a = 5.43 Angstrom, two atoms per primitive cell: 54 atoms for n_cells = 3),
+    positions jittered by +-jitter Angstrom from the seed, the basis and grid of BASELINE.json's config 2/3 (13 functions per atom:
+    s, s, p, p, d; cutoff 6 Angstrom; 60 x 302 points per atom; batches of <= 200 points), GGA fields.  Stands in for the paper's
+    FHI-aims "tight" silicon run, which is not in this container."""
+    seed = BASE_SEED + 54 if seed is None else seed
+    rng = np.random.default_rng(seed)
+    a = 5.43
+    prim = 0.5 * a * np.array([[0.0, 1.0, 1.0], [1.0, 0.0, 1.0], [1.0, 1.0, 0.0]])
+    lat = n_cells * prim
+    cells = np.array([[i, j, k] for i in range(n_cells) for j in range(n_cells) for k in range(n_cells)], dtype=np.float64)
+    frac = np.concatenate([(cells + f) / n_cells for f in (np.zeros(3), np.full(3, 0.25))])
+    frac = frac + (rng.uniform(-jitter, jitter, frac.shape) @ np.linalg.inv(lat))
+    frac = frac - np.floor(frac)
+    ls, rcut = SPECIES["Si"]
+    return _make(lat, frac, list(ls), rcut, n_rad, n_ang, max_batch, seed, rng, None, "periodic_si%d" % len(frac))
+
+
+def _make(lat, frac, shells, rcut, n_rad, n_ang, max_batch, seed, rng, gaussian_s_only, name):
     n_home = len(frac)
     img = _images(lat, frac, rcut)
     atom_home = np.array([t[0] for t in img], dtype=np.int32)
@@ -50,7 +74,7 @@ def make_periodic(n_rad=24, n_ang=50, max_batch=100, rcut=4.0, seed=None, gaussi
     na = len(atom_xyz)
     assert np.all(atom_n[:n_home] == 0) and np.array_equal(atom_home[:n_home], np.arange(n_home))
 
-    ls = [0] if gaussian_s_only is not None else SHELLS
+    ls = [0] if gaussian_s_only is not None else shells
     shell_l = np.array(ls, dtype=np.int32)
     n_shells = len(ls)
     shell_rcut = np.full(n_shells, rcut)
@@ -85,12 +109,14 @@ def make_periodic(n_rad=24, n_ang=50, max_batch=100, rcut=4.0, seed=None, gaussi
         own.append(np.full(n_rad * n_ang, part_home_idx[a], dtype=np.int32))
     xyz = np.concatenate(pts)
     w = np.concatenate(wts) * partition_weights(part_xyz, xyz, np.concatenate(own), r_part)
+    xyz_unwrapped = xyz
     fr = xyz @ np.linalg.inv(lat)
     xyz = np.ascontiguousarray((fr - np.floor(fr)) @ lat)                     # L113-115: back into the cell at T = 0
     owner = np.concatenate([np.full(n_rad * n_ang, a, dtype=np.int32) for a in range(n_home)])
 
     order, batch_ptr = bisect_batches(xyz, max_batch)
     xyz, w, owner = np.ascontiguousarray(xyz[order]), np.ascontiguousarray(w[order]), np.ascontiguousarray(owner[order])
+    xyz_unwrapped = np.ascontiguousarray(xyz_unwrapped[order])
 
     row_ptr, col_atom, blk_off, blk_ld, n_values = build_bsr(atom_xyz, atom_rc, atom_nfn)
     # periodic smooth fields: the same Gaussians on every image of a cell atom
@@ -100,7 +126,7 @@ def make_periodic(n_rad=24, n_ang=50, max_batch=100, rcut=4.0, seed=None, gaussi
     beta = rng.uniform(0.5, 2.0, n_home)[[t[0] for t in part]]
     v, g = smooth_fields(part_xyz, xyz, c, alpha, bb, beta, want_g=True)
 
-    bun = Bundle(name="periodic", seed=int(seed), atom_xyz=atom_xyz, atom_species=np.zeros(na, dtype=np.int32),
+    bun = Bundle(name=name, seed=int(seed), atom_xyz=atom_xyz, atom_species=np.zeros(na, dtype=np.int32),
                  species_names=["P"], species_shell_ptr=np.array([0, n_shells], dtype=np.int32), shell_l=shell_l,
                  shell_rcut=shell_rcut, shell_spline=np.arange(n_shells, dtype=np.int32), r0=R0_KNOT, log_inc=float(log_inc),
                  n_knots=N_KNOTS, spline_coef=spline_coef, shell_zeta=shell_zeta, shell_norm=np.array(shell_norm),
@@ -118,4 +144,5 @@ def make_periodic(n_rad=24, n_ang=50, max_batch=100, rcut=4.0, seed=None, gaussi
         blk[:, :nfn] = 0.5 * (blk[:, :nfn] + blk[:, :nfn].T)
     bun.D_values = vals
     bun.lattice, bun.atom_home, bun.atom_T, bun.n_home = lat, atom_home, atom_T, n_home
+    bun.frac, bun.atom_n, bun.xyz_unwrapped, bun.rcut = frac, atom_n.astype(np.int32), xyz_unwrapped, float(rcut)
     return bun

@@ -219,6 +219,28 @@ int aims_gpu_partition_weights(aims_gpu_ctx *ctx, int64_t n, const double *xyz, 
 int aims_gpu_bloch_fold(aims_gpu_ctx *ctx, const double *H_values, const int32_t *atom_home, const double *atom_T,
                         int32_t n_home, const double *kpt, double *out_re, double *out_im, int accumulate);
 
+/* Row f3, geometry.  The paper says which functions enter h^uc of Eq. 12 ("all N_rs basis functions that are
+ * non-zero on the unit cell", centred in the cell or in its periodic images, L109-113) and that "each integration point r is mapped
+ * back to its periodic image within the unit cell at T = (0,0,0)" (L113-115), but states neither rule; reading P23:
+ *
+ * aims_gpu_periodic_images.  lattice: HOST [3][3], rows a_1, a_2, a_3; frac: HOST [n_home][3] fractional coordinates of the cell
+ * atoms.  With h_i = V / |a_j x a_k| (height of the cell along the i-th reciprocal direction) and delta_i = reach / h_i, the
+ * periodic atom (a, n) = cell atom a translated by the integer vector n is kept iff -delta_i < frac[a][i] + n_i < 1 + delta_i for
+ * i = 1, 2, 3 -- a parallelepiped containing every point within `reach` of the cell, i.e. a superset of the atoms whose functions
+ * (cutoff <= reach) are non-zero somewhere in the cell; the per-batch culling of aims_gpu_eval_basis drops the rest.  Order: the
+ * cell's own atoms first (n = 0, ascending a), then ascending (n_1, n_2, n_3, a).  HOST outputs: atom_home [capacity],
+ * atom_n [capacity][3], *n_atoms = number of periodic atoms.  capacity == 0 is a size query (returns AIMS_OK); 0 < capacity <
+ * *n_atoms returns AIMS_ERR_INVALID_ARG with *n_atoms set.  Runs on the host (a few thousand atoms); no context, no device.
+ * The caller forms atom_xyz = (frac[home] + n) . lattice and atom_T = n . lattice for aims_gpu_create / aims_gpu_bloch_fold. */
+int aims_gpu_periodic_images(const double *lattice, int32_t n_home, const double *frac, double reach, int32_t *atom_home,
+                             int32_t *atom_n, int64_t capacity, int64_t *n_atoms);
+
+/* aims_gpu_wrap_points.  xyz: DEVICE [n_points][3], in place: f = r A^-1 (A = lattice rows; A^-1 by the cofactor formula,
+ * determinant along the first row, computed on the host), f <- f - floor(f), r <- f A; every product and sum separately rounded
+ * (IEEE RN, no FMA), sums left to right, so that exactly one result is correct.  lattice: HOST [3][3].  Enqueued on `cuda_stream` of
+ * `device`; asynchronous.  A singular lattice returns AIMS_ERR_INVALID_ARG. */
+int aims_gpu_wrap_points(int device, void *cuda_stream, const double *lattice, int64_t n_points, double *xyz);
+
 /* Row f4 of SURVEY.md 8(f): the grid-adapted cut-plane batching of PAPER.md L210-218 on the GPU.  The paper cites "Algorithm 3 of
  * [37]" without stating it; reading P12 fixes a deterministic recursive bisection: a set of n points is a batch if
  * n <= max_batch_points; otherwise, with nb = ceil(n / max_batch_points), the n_left = round(floor(nb/2) n / nb) points smallest in

@@ -101,6 +101,10 @@ def load_library():
     L.aims_gpu_synchronize.argtypes = [cp]
     L.aims_gpu_batch_points.restype = ctypes.c_int
     L.aims_gpu_batch_points.argtypes = [ctypes.c_int, _vp, ctypes.c_int64, _vp, ctypes.c_int32, _vp, _lp, ctypes.c_int64, _ip]
+    L.aims_gpu_periodic_images.restype = ctypes.c_int
+    L.aims_gpu_periodic_images.argtypes = [_vp, ctypes.c_int32, _vp, ctypes.c_double, _vp, _vp, ctypes.c_int64, _lp]
+    L.aims_gpu_wrap_points.restype = ctypes.c_int
+    L.aims_gpu_wrap_points.argtypes = [ctypes.c_int, _vp, _vp, ctypes.c_int64, _vp]
     L.aims_gpu_set_deterministic.restype = ctypes.c_int
     L.aims_gpu_set_deterministic.argtypes = [cp, ctypes.c_int]
     L.aims_gpu_batch_nnz.restype = ctypes.c_int
@@ -468,6 +472,43 @@ def aims_gpu_batch_points(xyz, max_batch_points, device=0, stream=None):
     if rc != 0:
         raise AimsError("aims_gpu_batch_points failed (%d)" % rc)
     return order[:n], ptr[: nb.value + 1].copy()
+
+
+def aims_gpu_periodic_images(lattice, frac, reach):
+    """(atom_home int32 [n], atom_n int32 [n][3]) of include/aims_gpu.h: aims_gpu_periodic_images (host arrays in, host arrays out)."""
+    L = load_library()
+    lat = np.ascontiguousarray(lattice, dtype=np.float64).reshape(3, 3)
+    fr = np.ascontiguousarray(frac, dtype=np.float64).reshape(-1, 3)
+    n = ctypes.c_int64()
+    rc = L.aims_gpu_periodic_images(lat.ctypes.data_as(_vp), len(fr), fr.ctypes.data_as(_vp), float(reach), None, None, 0, ctypes.byref(n))
+    if rc != 0:
+        raise AimsError("aims_gpu_periodic_images failed (%d)" % rc)
+    home = np.zeros(max(n.value, 1), dtype=np.int32)
+    nn = np.zeros((max(n.value, 1), 3), dtype=np.int32)
+    rc = L.aims_gpu_periodic_images(lat.ctypes.data_as(_vp), len(fr), fr.ctypes.data_as(_vp), float(reach), home.ctypes.data_as(_vp),
+                                    nn.ctypes.data_as(_vp), n.value, ctypes.byref(n))
+    if rc != 0:
+        raise AimsError("aims_gpu_periodic_images failed (%d)" % rc)
+    return home[: n.value], nn[: n.value]
+
+
+def aims_gpu_wrap_points(lattice, xyz, device=0, stream=None):
+    """Device tensor [n][3] of the points mapped into the cell at T = 0 (include/aims_gpu.h: aims_gpu_wrap_points).  A tensor
+    argument on the device is wrapped in place and returned."""
+    import torch
+    L = load_library()
+    if not torch.cuda.is_available():
+        raise AimsError("no CUDA device: this path has no CPU fallback")
+    dev = torch.device("cuda", device)
+    st = stream if stream is not None else torch.cuda.current_stream(dev)
+    lat = np.ascontiguousarray(lattice, dtype=np.float64).reshape(3, 3)
+    with torch.cuda.stream(st):
+        x = xyz if isinstance(xyz, torch.Tensor) else torch.as_tensor(np.ascontiguousarray(xyz, dtype=np.float64))
+        x = x.to(dev, torch.float64).reshape(-1, 3).contiguous()
+    rc = L.aims_gpu_wrap_points(int(device), ctypes.c_void_p(st.cuda_stream), lat.ctypes.data_as(_vp), int(x.shape[0]), _ptr(x))
+    if rc != 0:
+        raise AimsError("aims_gpu_wrap_points failed (%d)" % rc)
+    return x
 
 
 # ---- module-level functions with the names of the C ABI

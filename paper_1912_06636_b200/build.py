@@ -4,7 +4,7 @@ import subprocess
 import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SRC = [os.path.join(HERE, "csrc", "aims_gpu.cu"), os.path.join(HERE, "csrc", "batching.cu")]
+SRC = [os.path.join(HERE, "csrc", f) for f in ("aims_gpu.cu", "batching.cu", "periodic.cu")]
 LIB = os.path.join(HERE, "libaims_gpu.so")
 DEPS = [os.path.join(HERE, "csrc", f) for f in sorted(os.listdir(os.path.join(HERE, "csrc"))) if f.endswith((".cu", ".cuh"))]
 DEPS.append(os.path.join(os.path.dirname(HERE), "include", "aims_gpu.h"))

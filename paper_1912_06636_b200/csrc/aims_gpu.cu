@@ -77,6 +77,14 @@ struct aims_gpu_ctx {
   long long full_doubles = 0, n_blocks = 0;
   double *Dfull = nullptr;                                     // full-storage copy of the density matrix (per call)
 
+  // aims_gpu_bloch_fold: contribution lists per (cell atom, cell atom) tile, cached for the last atom_home seen
+  std::vector<int> bloch_home;
+  std::vector<double> bloch_T_host;
+  int bloch_n_home = 0;
+  BlochContrib *d_bloch_contrib = nullptr;
+  int *d_bloch_tile_ptr = nullptr;
+  double *d_bloch_T = nullptr;
+
   double *ws = nullptr;      // Phi-plane workspace
   double *probe_out = nullptr;
   bool deterministic = false;                                   // aims_gpu_set_deterministic: ordered scatter into H
@@ -1088,35 +1096,48 @@ static int impl_bloch_fold(aims_gpu_ctx *c, const double *H_values, const int32_
   }
   CU_TRY(c, cudaSetDevice(c->device));
   const int nhb = c->h_atom_fn_ptr[n_home];
-  if (!accumulate) {
-    CU_TRY(c, cudaMemsetAsync(out_re, 0, (size_t)nhb * nhb * sizeof(double), c->stream));
-    CU_TRY(c, cudaMemsetAsync(out_im, 0, (size_t)nhb * nhb * sizeof(double), c->stream));
+  // the contribution lists depend on atom_home alone: built once and kept (rebuilt when the caller passes another mapping)
+  if (c->bloch_n_home != n_home || c->bloch_home.size() != (size_t)na || !std::equal(c->bloch_home.begin(), c->bloch_home.end(), atom_home)) {
+    std::vector<int> cnt((size_t)n_home * n_home + 1, 0);
+    for (int A = 0; A < na; A++)
+      for (long long q = c->h_row_ptr[A]; q < c->h_row_ptr[A + 1]; q++) {
+        const int B = c->h_col_atom[(size_t)q];
+        cnt[(size_t)atom_home[A] * n_home + atom_home[B] + 1]++;
+        if (A != B) cnt[(size_t)atom_home[B] * n_home + atom_home[A] + 1]++;
+      }
+    for (size_t t = 0; t + 1 < cnt.size(); t++) cnt[t + 1] += cnt[t];
+    std::vector<int> pos(cnt.begin(), cnt.end() - 1);
+    std::vector<BlochContrib> contrib((size_t)cnt.back());
+    for (int A = 0; A < na; A++)                                   // ascending block index inside every tile: a fixed order
+      for (long long q = c->h_row_ptr[A]; q < c->h_row_ptr[A + 1]; q++) {
+        const int B = c->h_col_atom[(size_t)q];
+        BlochContrib bc{c->h_blk_off[(size_t)q], c->h_blk_ld[(size_t)q], A, B, 0};
+        contrib[(size_t)pos[(size_t)atom_home[A] * n_home + atom_home[B]]++] = bc;
+        if (A != B) { bc.transposed = 1; contrib[(size_t)pos[(size_t)atom_home[B] * n_home + atom_home[A]]++] = bc; }
+      }
+    CU_TRY(c, cudaStreamSynchronize(c->stream));                   // nothing in flight may still read the old lists
+    for (void *p : {(void *)c->d_bloch_contrib, (void *)c->d_bloch_tile_ptr, (void *)c->d_bloch_T})
+      if (p) { c->owned.erase(std::remove(c->owned.begin(), c->owned.end(), p), c->owned.end()); cudaFree(p); }
+    c->d_bloch_contrib = nullptr; c->d_bloch_tile_ptr = nullptr; c->d_bloch_T = nullptr; c->bloch_n_home = 0;
+    int rc;
+    if ((rc = dev_upload<BlochContrib>(c, &c->d_bloch_contrib, contrib.data(), contrib.size()))) return rc;
+    if ((rc = dev_upload<int>(c, &c->d_bloch_tile_ptr, cnt.data(), cnt.size()))) return rc;
+    if ((rc = dev_alloc(c, &c->d_bloch_T, (size_t)3 * na))) return rc;
+    CU_TRY(c, cudaStreamSynchronize(c->stream));                   // contrib / cnt are host temporaries
+    c->bloch_home.assign(atom_home, atom_home + na);
+    c->bloch_n_home = n_home;
   }
-  std::vector<BlochBlock> blocks;
-  blocks.reserve(c->h_col_atom.size());
-  for (int A = 0; A < na; A++)
-    for (long long q = c->h_row_ptr[A]; q < c->h_row_ptr[A + 1]; q++) {
-      const int B = c->h_col_atom[(size_t)q];
-      double th = 0.0;
-      for (int d = 0; d < 3; d++) th += kpt[d] * (atom_T[3 * B + d] - atom_T[3 * A + d]);
-      BlochBlock bb;
-      bb.off = c->h_blk_off[(size_t)q]; bb.ld = c->h_blk_ld[(size_t)q];
-      bb.nA = c->h_atom_fn_ptr[A + 1] - c->h_atom_fn_ptr[A]; bb.nB = c->h_atom_fn_ptr[B + 1] - c->h_atom_fn_ptr[B];
-      bb.i0 = c->h_atom_fn_ptr[atom_home[A]]; bb.j0 = c->h_atom_fn_ptr[atom_home[B]];
-      bb.diag = (A == B) ? 1 : 0;
-      bb.cs = cos(th); bb.sn = sin(th);
-      blocks.push_back(bb);
-    }
-  if (blocks.empty()) return AIMS_OK;
-  BlochBlock *d_blocks = nullptr;
-  CU_TRY(c, cudaMalloc(&d_blocks, blocks.size() * sizeof(BlochBlock)));
-  cudaError_t e = cudaMemcpyAsync(d_blocks, blocks.data(), blocks.size() * sizeof(BlochBlock), cudaMemcpyHostToDevice, c->stream);
-  if (e == cudaSuccess) {
+  // atom_T is a HOST array the caller may free after the call: staged through a context-owned copy, then the stream
+  // is synchronised (as the header states)
+  c->bloch_T_host.assign(atom_T, atom_T + 3 * (size_t)na);
+  CU_TRY(c, cudaMemcpyAsync(c->d_bloch_T, c->bloch_T_host.data(), 3 * (size_t)na * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+  {
     TimedLaunch t(c, kKindOther);
-    k_bloch_fold<<<(unsigned)blocks.size(), 128, 0, c->stream>>>(d_blocks, H_values, nhb, out_re, out_im);
+    k_bloch_fold<<<(unsigned)(n_home * n_home), 128, 0, c->stream>>>(c->d_bloch_contrib, c->d_bloch_tile_ptr, c->S.atom_fn_ptr, c->d_bloch_T,
+                                                                  kpt[0], kpt[1], kpt[2], H_values, n_home, nhb, out_re, out_im,
+                                                                  accumulate ? 1 : 0);
   }
-  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);   // blocks is a host temporary; the table is freed below
-  cudaFree(d_blocks);
+  cudaError_t e = cudaStreamSynchronize(c->stream);
   if (e != cudaSuccess) { c->err = std::string("aims_gpu_bloch_fold: ") + cudaGetErrorString(e); return AIMS_ERR_CUDA; }
   return check_async(c);
 }

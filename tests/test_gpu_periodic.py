@@ -69,3 +69,75 @@ def test_bloch_fold_bad_arguments(per):
         ctx.bloch_fold(H, bad_home, bun.atom_T, bun.n_home, KPTS[1], nhb)
     with pytest.raises(aims.AimsError):
         ctx.bloch_fold(H, bun.atom_home, bun.atom_T, 0, KPTS[1], nhb)
+
+
+# ---- geometry of reading P23 behind the boundary: image enumeration and the point map
+@pytest.mark.parametrize("case", ["toy", "si54"])
+def test_periodic_images_and_point_wrap_are_bit_exact(case):
+    import paper_1912_06636_b200 as aims
+    from oracle.periodic import periodic_images, wrap_points
+    bun = aims_synth.make_periodic(n_rad=12, n_ang=26) if case == "toy" else aims_synth.make_periodic_si(n_rad=16, n_ang=38, max_batch=16)
+    for reach in (bun.rcut, 0.0, 2.5 * bun.rcut):
+        home, n = aims.aims_gpu_periodic_images(bun.lattice, bun.frac, reach)
+        home_ref, n_ref = periodic_images(bun.lattice, bun.frac, reach)
+        assert np.array_equal(home, home_ref) and np.array_equal(n, n_ref)
+    w = aims.aims_gpu_wrap_points(bun.lattice, bun.xyz_unwrapped).cpu().numpy()
+    assert np.array_equal(w, wrap_points(bun.lattice, bun.xyz_unwrapped))            # separately rounded operations: one result
+    # degenerate inputs
+    assert aims.aims_gpu_wrap_points(bun.lattice, np.zeros((0, 3))).shape[0] == 0
+    with pytest.raises(aims.AimsError):
+        aims.aims_gpu_wrap_points(np.array([[1.0, 0, 0], [2.0, 0, 0], [0, 0, 1.0]]), bun.xyz_unwrapped[:4])   # singular lattice
+    # the library consumes what it produced: a context over (images, wrapped points) has the oracle's lists
+    import copy
+    b2 = copy.copy(bun)
+    home, n = aims.aims_gpu_periodic_images(bun.lattice, bun.frac, bun.rcut)
+    b2.atom_xyz = np.ascontiguousarray((bun.frac[home] + n) @ bun.lattice)
+    b2.xyz = np.ascontiguousarray(w)
+    assert np.abs(b2.atom_xyz - bun.atom_xyz).max() < 1e-12
+    ctx = aims.aims_gpu_create(b2, device=0)
+    orc = Oracle(b2)
+    nnz = ctx.batch_nnz()
+    for b in range(0, b2.n_batches, max(1, b2.n_batches // 12)):
+        assert nnz[b] == len(orc.batch_nnz(b)[0])
+    ctx.close()
+
+
+def test_si54_supercell_at_full_size_on_sampled_batches():
+    """The periodic workload shaped like the paper's main benchmark (54-atom diamond-Si supercell, config-2 basis,
+    60 x 302 points per atom, batches of <= 200): whole-grid calls as bench.py --config 6 launches them; lists, n / grad n and
+    H^uc restricted to a seeded sample of batches against the oracle; Bloch sums at Gamma and one general k."""
+    import torch
+    import paper_1912_06636_b200 as aims
+    bun = aims_synth.make_periodic_si()
+    assert bun.n_home == 54 and bun.n_points == 54 * 60 * 302
+    ctx = aims.aims_gpu_create(bun, device=0)
+    orc = Oracle(bun)
+    nnz = ctx.batch_nnz()
+    rng = np.random.default_rng(54)
+    sel = np.unique(np.concatenate([[0, bun.n_batches - 1, int(np.argmax(nnz)), int(np.argmin(nnz))],
+                                    rng.integers(0, bun.n_batches, 12)])).astype(np.int32)
+    for b in sel:
+        _, fn_index, _, _, _ = ctx.eval_basis(int(b), int(b) + 1, want_grad=False)
+        assert np.array_equal(fn_index.cpu().numpy(), orc.batch_nnz(int(b))[0])
+    n, gn = ctx.update_density(bun.D_values, want_grad=True)                       # whole grid
+    vd, gd = torch.as_tensor(bun.v).cuda(), torch.as_tensor(bun.g).cuda()
+    H = torch.zeros(bun.n_values, dtype=torch.float64, device="cuda")
+    for b in sel:
+        ctx.integrate_hamiltonian(vd, gd, H=H, b0=int(b), b1=int(b) + 1, accumulate=True)
+    ctx.synchronize()
+    n_ref, gn_ref = orc.update_density(bun.D_values, want_grad=True, batches=sel)
+    idx = np.concatenate([np.arange(bun.batch_ptr[b], bun.batch_ptr[b + 1]) for b in sel])
+    assert np.abs(n.cpu().numpy()[idx] - n_ref[idx]).max() <= 1e-11 * np.abs(n_ref[idx]).max()
+    assert np.abs(gn.cpu().numpy()[:, idx] - gn_ref[:, idx]).max() <= 1e-11 * np.abs(gn_ref[:, idx]).max()
+    H_ref = orc.integrate_hamiltonian(bun.v, bun.g, batches=sel)
+    assert _rel_fro(H.cpu().numpy(), H_ref) <= 1e-11
+    nhb = int(bun.atom_fn_ptr[bun.n_home])
+    for k in (np.zeros(3), np.array([0.11, -0.07, 0.05])):
+        Hk = ctx.bloch_fold(H, bun.atom_home, bun.atom_T, bun.n_home, k, nhb).cpu().numpy()
+        assert _rel_fro(Hk, orc.bloch_fold(H_ref, bun.atom_home, bun.atom_T, bun.n_home, k)) <= 1e-11
+        assert np.abs(Hk - Hk.conj().T).max() <= 1e-12 * np.abs(Hk).max()
+    # whole-grid overlap folded at Gamma: Hermitian and positive definite (a property of the GPU outputs alone)
+    S = ctx.integrate_hamiltonian(np.ones(bun.n_points))
+    Sk = ctx.bloch_fold(S, bun.atom_home, bun.atom_T, bun.n_home, np.zeros(3), nhb).cpu().numpy()
+    assert np.linalg.eigvalsh(0.5 * (Sk + Sk.conj().T)).min() > 0.0
+    ctx.close()

@@ -85,3 +85,62 @@ def test_folded_matrices_are_hermitian_and_overlap_is_positive_definite(per):
             assert np.abs(S.imag).max() == 0.0 and np.abs(H.imag).max() == 0.0
         else:
             assert np.abs(S.imag).max() > 1e-6
+
+
+# ---- geometry of reading P23 (oracle/periodic.py): image enumeration and the point map
+def _cell_samples(lat, m=7):
+    g = (np.arange(m) + 0.5) / m
+    f = np.array([[a, b, c] for a in g for b in g for c in g])
+    corners = np.array([[a, b, c] for a in (0.0, 1.0) for b in (0.0, 1.0) for c in (0.0, 1.0)])
+    return np.concatenate([f, corners]) @ lat
+
+
+@pytest.mark.parametrize("case", ["toy", "si"])
+def test_image_list_is_a_superset_of_every_atom_within_reach_and_is_ordered(case):
+    from oracle.periodic import periodic_images
+    b = aims_synth.make_periodic(n_rad=6, n_ang=10) if case == "toy" else aims_synth.make_periodic_si(n_cells=2, n_rad=4, n_ang=6)
+    reach = b.rcut
+    home, n = periodic_images(b.lattice, b.frac, reach)
+    keys = set((int(h), int(a), int(bb), int(c)) for h, (a, bb, c) in zip(home, n))
+    assert len(keys) == len(home)                                            # no atom twice
+    assert np.all(n[: b.n_home] == 0) and np.array_equal(home[: b.n_home], np.arange(b.n_home))   # the cell's own atoms first
+    rest = [(int(a), int(bb), int(c), int(h)) for h, (a, bb, c) in zip(home[b.n_home:], n[b.n_home:])]
+    assert rest == sorted(rest)
+    # brute force over a large integer box: every periodic atom closer than `reach` to a sample point of the cell is listed
+    samples = _cell_samples(b.lattice)
+    R = 4
+    for a in range(b.n_home):
+        for n1 in range(-R, R + 1):
+            for n2 in range(-R, R + 1):
+                for n3 in range(-R, R + 1):
+                    pos = (b.frac[a] + np.array([n1, n2, n3])) @ b.lattice
+                    if np.linalg.norm(samples - pos, axis=1).min() < reach:
+                        assert (a, n1, n2, n3) in keys
+    # ... and the list is not wildly larger than needed: every listed atom is within reach + cell diagonal of the cell centre
+    centre = np.array([0.5, 0.5, 0.5]) @ b.lattice
+    diag = np.linalg.norm(b.lattice.sum(axis=0)) + np.linalg.norm(b.lattice[0] - b.lattice[1]) + np.linalg.norm(b.lattice[2])
+    pos = (b.frac[home] + n) @ b.lattice
+    assert np.linalg.norm(pos - centre, axis=1).max() < 2.0 * reach + diag
+    # the seeded periodic bundle (whose Bloch sums are pinned by the Gaussian lattice sums above) uses exactly this list
+    assert np.array_equal(home, b.atom_home) and np.allclose(n @ b.lattice, b.atom_T, rtol=0, atol=1e-12)
+
+
+def test_wrapped_points_differ_by_a_lattice_vector_and_lie_in_the_cell():
+    from oracle.periodic import inverse_lattice, wrap_points
+    b = aims_synth.make_periodic(n_rad=10, n_ang=14)
+    lat = b.lattice
+    assert np.abs(inverse_lattice(lat) @ lat - np.eye(3)).max() < 1e-14
+    assert np.abs(inverse_lattice(lat) - np.linalg.inv(lat)).max() < 1e-15
+    r = b.xyz_unwrapped
+    w = wrap_points(lat, r)
+    shift = (r - w) @ np.linalg.inv(lat)
+    assert np.abs(shift - np.rint(shift)).max() < 1e-11                      # an integer combination of a_1, a_2, a_3
+    assert np.abs(np.rint(shift)).max() >= 1                                 # some points really were outside
+    f = w @ np.linalg.inv(lat)
+    assert f.min() > -1e-12 and f.max() < 1.0 + 1e-12
+    assert np.abs(wrap_points(lat, w) - w).max() < 1e-12                     # idempotent
+    assert np.abs(w - b.xyz).max() < 1e-12                                   # the bundle's (pinned) points
+    # a point on a lattice translate of r0 maps onto the image of r0
+    r0 = np.array([[0.3, 0.2, 0.1]]) @ lat
+    for nvec in ([1, 0, 0], [-2, 3, 1], [0, -1, 4]):
+        assert np.abs(wrap_points(lat, r0 + np.array(nvec) @ lat) - r0).max() < 1e-12
