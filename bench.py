@@ -514,6 +514,7 @@ def main():
     wkey = "config%d%s" % (args.config, "" if not (args.max_batch or args.n_rad or args.n_ang) else "_variant")
     if world == 1:
         roofline["traffic"], roofline["traffic_note"] = committed_traffic(dom, wkey)
+        roofline_eval_traffic = committed_traffic("k_eval", wkey)
     roofline["algorithmic_bytes_note"] = ("compulsory HBM bytes of the dominant contraction are ~1 GB per step (points, v, g, D, H, "
                                           "n, grad n); it is bound by the FP64 tensor pipe, so `achieved` is in flops")
     # second roofline: the HBM-bound evaluation kernel (algorithmic bytes = 8 B x planes x padded rows x padded points)
@@ -533,10 +534,12 @@ def main():
         pass
     ev_ms, ev_ln = kern["k_eval"]
     ev_gbs = eval_bytes * args.steps / (ev_ms * 1e-3) / 1e9 if ev_ms > 0 else 0.0
+    if world != 1:
+        roofline_eval_traffic = (None, "single-GPU capture only")
     roofline_eval = {"bound": "hbm", "kernel": "k_eval", "achieved": ev_gbs, "peak": hbm_peak, "unit": "GB/s",
                      "frac": ev_gbs / hbm_peak, "peak_source": hbm_src, "algorithmic_bytes_per_step": eval_bytes,
                      "avg_launch_ms": ev_ms / max(ev_ln, 1), "share_of_step": ev_ms / ms_total,
-                     "traffic": None}
+                     "traffic": roofline_eval_traffic[0], "traffic_note": roofline_eval_traffic[1]}
 
     out = {"metric": metric, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
