@@ -298,7 +298,9 @@ int aims_gpu_fp64_peak(aims_gpu_ctx *ctx, double ms_target, double *tflops);
  *   variant 1: operands in registers;  2: the step's 8 fragments loaded from shared memory, then its DMMAs;
  *   variant 3: the loads of the next step issued before the DMMAs of the current one;
  * variants 4..9 (warps_per_sm 1..20) run the K-step body of the kernels on a (WA x WB) block of 8x8 accumulator tiles:
- *   4, 5, 6, 9: fragments reloaded in place, blocks 4x4, 4x3, 3x3, 2x2;  7, 8: second fragment register set, blocks 4x4, 4x3.
+ *   4, 5, 6, 9: fragments reloaded in place, blocks 4x4, 4x3, 3x3, 2x2;  7, 8: second fragment register set, blocks 4x4, 4x3;
+ *   10, 11: the in-place 4x3 step inside the kernels' control flow (trip counts from global memory, stage loop around a step loop);
+ *   11 with the four steps of a stage unrolled into one block.
  * Returns the achieved TFLOP/s in *tflops (HOST output).  Diagnostic only. */
 int aims_gpu_dmma_probe(aims_gpu_ctx *ctx, int variant, int warps_per_sm, double *tflops);
 

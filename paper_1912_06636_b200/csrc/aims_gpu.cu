@@ -308,6 +308,72 @@ __global__ void __launch_bounds__(640) k_dmma_probe2(double *out, int iters, dou
   if (s == 12345.678) out[0] = s;
 }
 
+// Third probe: the (4 x 3) in-place K step inside the CONTROL FLOW of the kernels -- trip counts that come from global memory (so the
+// compiler cannot prove them warp-uniform: vector-register loop counters, predicated branches, WARPSYNC before the DMMAs of every
+// basic block), a stage loop around a step loop, and the "last step of a stage" branch that redirects the reload pointers.
+//   UNROLL = false: one step per iteration of the inner loop, as d_mma_kloop_t;  true: the four steps of a stage as one block.
+template <bool UNROLL>
+__global__ void __launch_bounds__(640) k_dmma_probe3(double *out, const int *cnt, double a0) {
+  __shared__ double sm[4096];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int i = threadIdx.x; i < 4096; i += blockDim.x) sm[i] = 1e-9 * i + a0;
+  __syncthreads();
+  const int nkc = cnt[0], nnz8 = cnt[1];                 // run-time values from global memory, like L.nnz[b]
+  double acc[4][3][2];
+#pragma unroll
+  for (int a = 0; a < 4; a++)
+#pragma unroll
+    for (int c = 0; c < 3; c++) { acc[a][c][0] = a + lane; acc[a][c][1] = c; }
+  const double *sAl = sm + lane + (warp & 1) * 1024, *sBl = sm + 2048 + lane + (warp & 1) * 1024;
+  const double *tA = sAl, *tB = sBl;
+  double fa[4], fb[3];
+#pragma unroll
+  for (int a = 0; a < 4; a++) fa[a] = tA[a * 32];
+#pragma unroll
+  for (int c = 0; c < 3; c++) fb[c] = tB[c * 32];
+  int step = 0;
+  auto one_step = [&](const double *a1, const double *b1) {
+#pragma unroll
+    for (int a = 0; a < 4; a++) {
+#pragma unroll
+      for (int c = 0; c < 3; c++) {
+        dmma8x8x4(acc[a][c][0], acc[a][c][1], fa[a], fb[c]);
+        if (a == 3) fb[c] = b1[c * 32];
+      }
+      fa[a] = a1[a * 32];
+    }
+  };
+#pragma unroll 1
+  for (int kc = 0; kc < nkc; kc++) {
+    const int nk4 = min(16, nnz8 - kc * 16) >> 2;
+    const bool more = kc + 1 < nkc;
+    if (UNROLL && nk4 == 4) {
+      one_step(tA + 128, tB + 128);
+      one_step(tA + 256, tB + 256);
+      one_step(tA + 384, tB + 384);
+      const double *a1 = more ? sAl + ((step + 1) & 1) * 512 : tA, *b1 = more ? sBl + ((step + 1) & 1) * 512 : tB;
+      one_step(a1, b1);
+      tA = a1; tB = b1;
+    } else {
+#pragma unroll 1
+      for (int t = 0; t < nk4; t++) {
+        const bool last = t + 1 == nk4;
+        const double *a1 = tA + (t + 1) * 128, *b1 = tB + (t + 1) * 128;
+        if (last) { a1 = more ? sAl + ((step + 1) & 1) * 512 : tA; b1 = more ? sBl + ((step + 1) & 1) * 512 : tB; }
+        one_step(a1, b1);
+        if (last) { tA = a1; tB = b1; }
+      }
+    }
+    step++;
+  }
+  double s = 0;
+#pragma unroll
+  for (int a = 0; a < 4; a++)
+#pragma unroll
+    for (int c = 0; c < 3; c++) s += acc[a][c][0] + acc[a][c][1];
+  if (s == 12345.678) out[0] = s;
+}
+
 bool range_ok(const aims_gpu_ctx *c, int b0, int b1) { return c && b0 >= 0 && b1 >= b0 && b1 <= c->n_batches; }
 
 // Every extern "C" entry runs its body through this: no C++ exception (std::bad_alloc of the host-side tables and
@@ -1246,12 +1312,17 @@ static int impl_synchronize(aims_gpu_ctx *c) {
 }
 
 static int impl_dmma_probe(aims_gpu_ctx *c, int variant, int warps_per_sm, double *tflops) {
-  if (!c || !tflops || variant < 1 || variant > 9 || warps_per_sm < 1 || warps_per_sm > (variant <= 3 ? 16 : 20))
-    return fail(c, AIMS_ERR_INVALID_ARG, "variant 1..9, warps_per_sm 1..16 (variants 4..9: 1..20)");
+  if (!c || !tflops || variant < 1 || variant > 11 || warps_per_sm < 1 || warps_per_sm > (variant <= 3 ? 16 : 20))
+    return fail(c, AIMS_ERR_INVALID_ARG, "variant 1..11, warps_per_sm 1..16 (variants 4..11: 1..20)");
   CU_TRY(c, cudaSetDevice(c->device));
   if (!c->probe_out) { int rc = dev_alloc(c, &c->probe_out, 16); if (rc) return rc; }   // scratch of the probes, allocated once
   double *out = c->probe_out;
   const int iters = 40000, threads = 32 * warps_per_sm;
+  if (variant >= 10) {   // trip counts of k_dmma_probe3 live in global memory: 10,000 stages of 4 steps
+    const int cnt[2] = {iters / 4, (iters / 4) * 16};
+    CU_TRY(c, cudaMemcpyAsync(out + 8, cnt, sizeof(cnt), cudaMemcpyHostToDevice, c->stream));
+    CU_TRY(c, cudaStreamSynchronize(c->stream));
+  }
   cudaEvent_t e0, e1;
   CU_TRY(c, cudaEventCreate(&e0));
   CU_TRY(c, cudaEventCreate(&e1));
@@ -1265,7 +1336,9 @@ static int impl_dmma_probe(aims_gpu_ctx *c, int variant, int warps_per_sm, doubl
     else if (variant == 6) k_dmma_probe2<3, 3, true><<<c->sm_count, threads, 0, c->stream>>>(out, iters, 1e-9);
     else if (variant == 7) k_dmma_probe2<4, 4, false><<<c->sm_count, threads, 0, c->stream>>>(out, iters, 1e-9);
     else if (variant == 8) k_dmma_probe2<4, 3, false><<<c->sm_count, threads, 0, c->stream>>>(out, iters, 1e-9);
-    else k_dmma_probe2<2, 2, true><<<c->sm_count, threads, 0, c->stream>>>(out, iters, 1e-9);
+    else if (variant == 9) k_dmma_probe2<2, 2, true><<<c->sm_count, threads, 0, c->stream>>>(out, iters, 1e-9);
+    else if (variant == 10) k_dmma_probe3<false><<<c->sm_count, threads, 0, c->stream>>>(out, reinterpret_cast<const int *>(out + 8), 1e-9);
+    else k_dmma_probe3<true><<<c->sm_count, threads, 0, c->stream>>>(out, reinterpret_cast<const int *>(out + 8), 1e-9);
     c->launches++;
   }
   CU_TRY(c, cudaEventRecord(e1, c->stream));
@@ -1273,7 +1346,7 @@ static int impl_dmma_probe(aims_gpu_ctx *c, int variant, int warps_per_sm, doubl
   float ms = 0;
   CU_TRY(c, cudaEventElapsedTime(&ms, e0, e1));
   cudaEventDestroy(e0); cudaEventDestroy(e1);
-  const int per_step[10] = {0, 16, 16, 16, 16, 12, 9, 16, 12, 4};        // DMMAs per step and warp
+  const int per_step[12] = {0, 16, 16, 16, 16, 12, 9, 16, 12, 4, 12, 12};        // DMMAs per step and warp
   *tflops = 2.0 * 256 * per_step[variant] * (double)iters * c->sm_count * warps_per_sm / (ms * 1e-3) * 1e-12;
   return check_async(c);
 }

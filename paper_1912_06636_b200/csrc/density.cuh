@@ -95,6 +95,94 @@ inline size_t d_smem_bytes(int max_nnz, int max_act, bool ptab_in_smem) {
 // Micro-benchmark on the B200 (8 LDS.64 + 16 DMMA per step): one warp per sub-partition reaches 79 % of the pipe peak
 // with load-then-compute steps and 92 % with overlapped loads; four warps 94 % -> 99.6 %.
 // step: running stage counter of the CTA (stage = step % kDStages, parity from step / kDStages), advanced by nkc.
+// --define AIMS_D_UNROLL_STAGE=1 (probe builds): the K loop below with the four steps of a full stage as ONE straight-line block.
+#ifndef AIMS_D_UNROLL_STAGE
+#define AIMS_D_UNROLL_STAGE 0
+#endif
+#if AIMS_D_UNROLL_STAGE
+// One K step of a (WA x WB) block: DMMAs row by row, every fragment reloaded in place from (a1, b1) as soon as it is dead.
+// LAST (compile time): the last step of a stage -- after the first row of DMMAs is in the pipe, make sure the next stage has
+// landed and redirect the reloads to it.
+template <int WA, int WB, bool LAST>
+__device__ __forceinline__ void d_step(double (&acc)[4][4][2], double (&fa)[WA], double (&fb)[WB], const double *a1, const double *b1,
+                                       const double *&tA, const double *&tB, const double *sAl, const double *sBl, bool more_stages,
+                                       int step, unsigned bar_full) {
+#pragma unroll
+  for (int c = 0; c < WB; c++) dmma8x8x4(acc[0][c][0], acc[0][c][1], fa[0], fb[c]);
+  if (LAST) {
+    if (more_stages) {
+      const int s1 = (step + 1) % kDStages;
+      AIMS_HS(AIMS_TIMED(0, mbar_wait(bar_full + 8 * s1, (unsigned)((step + 1) / kDStages) & 1u)))
+      a1 = sAl + (size_t)s1 * kDStage; b1 = sBl + (size_t)s1 * kDStage;
+    } else {
+      a1 = tA; b1 = tB;                      // nothing follows: harmless reload of this stage's first step
+    }
+  }
+  if (WA > 1) {
+    fa[0] = a1[0];
+#pragma unroll
+    for (int a = 1; a < WA - 1; a++) {
+#pragma unroll
+      for (int c = 0; c < WB; c++) dmma8x8x4(acc[a][c][0], acc[a][c][1], fa[a], fb[c]);
+      fa[a] = a1[a * 32];
+    }
+#pragma unroll
+    for (int c = 0; c < WB; c++) {
+      dmma8x8x4(acc[WA - 1][c][0], acc[WA - 1][c][1], fa[WA - 1], fb[c]);
+      fb[c] = b1[c * (2 * kDKC * 4)];
+    }
+    fa[WA - 1] = a1[(WA - 1) * 32];
+  } else {
+    fa[0] = a1[0];
+#pragma unroll
+    for (int c = 0; c < WB; c++) fb[c] = b1[c * (2 * kDKC * 4)];
+  }
+  if (LAST) { tA = a1; tB = b1; }
+}
+
+// nnz(B) and the stage count come from global memory, so the compiler cannot prove the loop counters warp-uniform and guards
+// the DMMAs of every basic block with a WARPSYNC after a predicated branch.  aims_gpu_dmma_probe variants 5 / 10 / 11
+// (profiles/r02_dmma_probe.md): the same K step reaches 99.7 % of the pipe in a uniform loop, 96.2 % inside this control flow
+// with one step per iteration, 98.5 % with the four steps of a stage unrolled (four warps per pipe; 98 / 90 / 95.5 % with two).
+// In the kernels the unrolled form (--define AIMS_D_UNROLL_STAGE=1) is a wash: k_density 388.2 instead of 392.2 ms on config 5,
+// but 117.6 instead of 115.1 ms on 64-point batches and 10.50 instead of 10.40 ms on config 3 (profiles/r02_kernel_experiments.md).
+template <int WA, int WB>
+__device__ __forceinline__ void d_mma_kloop_t(double (&acc)[4][4][2], const double *sAl, const double *sBl, int tm, int nkc,
+                                              int nnz8, int &step, unsigned bar_full, unsigned bar_empty, int lane) {
+  int s = step % kDStages;
+  AIMS_HS(AIMS_TIMED(0, mbar_wait(bar_full + 8 * s, (unsigned)(step / kDStages) & 1u)))
+  const double *tA = sAl + (size_t)s * kDStage, *tB = sBl + (size_t)s * kDStage;
+  const int tm4 = tm * 4;
+  double fa[WA], fb[WB];
+#pragma unroll
+  for (int a = 0; a < WA; a++) fa[a] = tA[a * 32];
+#pragma unroll
+  for (int c = 0; c < WB; c++) fb[c] = tB[c * (2 * kDKC * 4)];
+#pragma unroll 1
+  for (int kc = 0; kc < nkc; kc++) {
+    const int nk4 = min(kDKC, nnz8 - kc * kDKC) >> 2;
+    const bool more_stages = kc + 1 < nkc;
+    if (nk4 == 4) {
+      d_step<WA, WB, false>(acc, fa, fb, tA + tm4, tB + 16, tA, tB, sAl, sBl, more_stages, step, bar_full);
+      d_step<WA, WB, false>(acc, fa, fb, tA + 2 * tm4, tB + 32, tA, tB, sAl, sBl, more_stages, step, bar_full);
+      d_step<WA, WB, false>(acc, fa, fb, tA + 3 * tm4, tB + 48, tA, tB, sAl, sBl, more_stages, step, bar_full);
+      d_step<WA, WB, true>(acc, fa, fb, tA, tB, tA, tB, sAl, sBl, more_stages, step, bar_full);
+    } else {
+#pragma unroll 1
+      for (int t = 0; t < nk4; t++) {
+        if (t + 1 == nk4) d_step<WA, WB, true>(acc, fa, fb, tA, tB, tA, tB, sAl, sBl, more_stages, step, bar_full);
+        else d_step<WA, WB, false>(acc, fa, fb, tA + (t + 1) * tm4, tB + (t + 1) * 16, tA, tB, sAl, sBl, more_stages, step, bar_full);
+      }
+    }
+    // every fragment of stage s is in registers (the reloads above already read the next stage): release it
+    __syncwarp();
+    AIMS_HS(if (lane == 0) mbar_arrive(bar_empty + 8 * s);)
+    step++;
+    s = step % kDStages;
+  }
+}
+
+#else
 template <int WA, int WB>
 __device__ __forceinline__ void d_mma_kloop_t(double (&acc)[4][4][2], const double *sAl, const double *sBl, int tm, int nkc,
                                               int nnz8, int &step, unsigned bar_full, unsigned bar_empty, int lane) {
@@ -154,6 +242,8 @@ __device__ __forceinline__ void d_mma_kloop_t(double (&acc)[4][4][2], const doub
     s = step % kDStages;
   }
 }
+
+#endif
 
 // K loop of a warp without a block in this M-tile: it only takes part in the stage hand-over
 __device__ __forceinline__ void d_idle_kloop(int nkc, int &step, unsigned bar_full, unsigned bar_empty, int lane) {

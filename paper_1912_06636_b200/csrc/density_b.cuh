@@ -57,7 +57,7 @@ __device__ __forceinline__ void b_step(double (&acc)[4][3][2], double (&ex)[2][2
     // the first row of DMMAs is in the pipe: make sure the next stage has landed before reloading from it
     if (more_stages) {
       s1 = (step + 1) % kDStages;
-      AIMS_TIMED(0, mbar_wait(bar_full + 8 * s1, (unsigned)((step + 1) / kDStages) & 1u))
+      AIMS_HS(AIMS_TIMED(0, mbar_wait(bar_full + 8 * s1, (unsigned)((step + 1) / kDStages) & 1u)))
       a1 = sAl + (size_t)s1 * kDStage; b1 = sBl + (size_t)s1 * kDStage;
     } else {
       a1 = tA; b1 = tB;                      // nothing follows: harmless reload of this stage's first step
@@ -87,7 +87,7 @@ __device__ __forceinline__ void b_mma_kloop_t(double (&acc)[4][3][2], double (&e
                                               unsigned bar_empty, int lane) {
   constexpr int BS = 2 * kDKC * 4;
   int s = step % kDStages;
-  AIMS_TIMED(0, mbar_wait(bar_full + 8 * s, (unsigned)(step / kDStages) & 1u))
+  AIMS_HS(AIMS_TIMED(0, mbar_wait(bar_full + 8 * s, (unsigned)(step / kDStages) & 1u)))
   const double *tA = sAl + (size_t)s * kDStage, *tB = sBl + (size_t)s * kDStage;
   double fa[WA], fb[3], fx = 0.0;
 #pragma unroll
@@ -113,7 +113,7 @@ __device__ __forceinline__ void b_mma_kloop_t(double (&acc)[4][3][2], double (&e
     }
     // every fragment of stage s is in registers (the reloads above already read the next stage): release it
     __syncwarp();
-    if (lane == 0) mbar_arrive(bar_empty + 8 * s);
+    AIMS_HS(if (lane == 0) mbar_arrive(bar_empty + 8 * s);)
     step++;
     s = step % kDStages;
   }
@@ -190,6 +190,9 @@ __global__ void __launch_bounds__(kBThreads, 1) k_density_b(DevSys S, BatchLists
 
   if (warp >= kBMma) {
     // =========================================================================== producers (as in density.cuh)
+#ifdef AIMS_PROBE_D_NO_HANDSHAKE
+    if (warp >= kBMma) return;
+#endif
     const int pl = tid - kBMma * 32;               // 0..63
     int step = 0;
 #pragma unroll 1
@@ -312,7 +315,19 @@ __global__ void __launch_bounds__(kBThreads, 1) k_density_b(DevSys S, BatchLists
             for (int q = 0; q < 3; q++) { pp[(q + 1) * pstride] += sg[q][0]; pp[(q + 1) * pstride + 1] += sg[q][1]; }
         }
       };
+#ifdef AIMS_PROBE_NO_D_EPILOGUE
+      if (wa > 0) {   // keep the accumulators live through a store that never happens
+        double sum = ex[0][0] + ex[0][1] + ex[1][0] + ex[1][1];
+#pragma unroll
+        for (int a = 0; a < 4; a++)
+#pragma unroll
+          for (int c = 0; c < 3; c++) sum += acc[a][c][0] + acc[a][c][1];
+        if (sum == 12345.678) sPart[lane] = sum;
+      }
+      if (false) {
+#else
       if (wa > 0) {
+#endif
 #pragma unroll
         for (int c = 0; c < 3; c++) {
           double av[4][2];

@@ -163,7 +163,7 @@ def test_diagnostic_probes_report_plausible_fp64_throughput():
     assert 0.8 * peak < t <= 1.02 * peak
     import paper_1912_06636_b200 as aims
     with pytest.raises(aims.AimsError):
-        ctx.dmma_probe(10, 16)
+        ctx.dmma_probe(12, 16)
     ctx.close()
 
 
