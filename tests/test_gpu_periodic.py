@@ -141,3 +141,27 @@ def test_si54_supercell_at_full_size_on_sampled_batches():
     Sk = ctx.bloch_fold(S, bun.atom_home, bun.atom_T, bun.n_home, np.zeros(3), nhb).cpu().numpy()
     assert np.linalg.eigvalsh(0.5 * (Sk + Sk.conj().T)).min() > 0.0
     ctx.close()
+
+
+def test_forces_stress_and_density_hessian_on_the_periodic_bundle(per):
+    """The widened rows run unchanged on a periodic bundle too ("the exact same real-space integration code"):
+    Pulay forces on all periodic atoms, the Pulay stress with the cell volume (Eq. 20: sigma = (1/V) dE/d eps), hess n."""
+    from aims_synth import make_q_values
+    bun, orc, ctx = per
+    Q = make_q_values(bun)
+    vol = abs(float(np.linalg.det(bun.lattice)))
+    F, sig = ctx.pulay_forces_stress(bun.v, bun.D_values, g=bun.g, Q=Q, volume=vol, kinetic=True)
+    Hn = ctx.density_hessian(bun.D_values)
+    ctx.synchronize()
+    F_ref = orc.pulay_forces(bun.v, bun.D_values, g=bun.g, Q_values=Q, kinetic=True)
+    sig_ref = orc.pulay_stress(bun.v, bun.D_values, g=bun.g, Q_values=Q, kinetic=True, volume=vol)
+    Hn_ref = orc.density_hessian(bun.D_values)
+    assert np.abs(F.cpu().numpy() - F_ref).max() <= 1e-11 * np.abs(F_ref).max()
+    assert np.abs(sig.cpu().numpy() - sig_ref).max() <= 1e-11 * np.abs(sig_ref).max()
+    assert np.abs(Hn.cpu().numpy() - Hn_ref).max() <= 1e-11 * np.abs(Hn_ref).max()
+    # forces of the images fold onto their cell atoms: sum over images of one cell atom is what a periodic code reports
+    F_home = np.zeros((bun.n_home, 3))
+    np.add.at(F_home, bun.atom_home, F.cpu().numpy())
+    F_home_ref = np.zeros((bun.n_home, 3))
+    np.add.at(F_home_ref, bun.atom_home, F_ref)
+    assert np.abs(F_home - F_home_ref).max() <= 1e-11 * np.abs(F_ref).max()
