@@ -67,7 +67,7 @@ def parse():
     ap.add_argument("--cpu-sample-batches", type=int, default=96)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--path", default="scf", choices=["scf", "forces", "stress", "hessian"])
+    ap.add_argument("--path", default="scf", choices=["scf", "forces", "stress", "hessian", "setup"])
     ap.add_argument("--deterministic", action="store_true",
                     help="ordered (bitwise reproducible) scatter into H: aims_gpu_set_deterministic")
     ap.add_argument("--kinetic", action="store_true",
@@ -199,6 +199,67 @@ def committed_traffic(kernel, workload_key):
         return None, "no capture of %s for %s in profiles/r02_traffic.txt" % (kernel, workload_key)
     return float(val), "dram__bytes_read.sum + dram__bytes_write.sum of one launch, %s (commit %s)" % (
         rec.get("source", "profiles/r02_traffic.txt"), rec.get("commit"))
+
+
+def run_setup_path(args, aims, torch, ctx, bun, stream, workload, n_points_total, world, rank):
+    """--path setup (row f4 of SURVEY.md 8(f)): one step = the partition-of-unity factor of every grid point
+    (aims_gpu_partition_weights, Eq. 21-22) + the cut-plane batching of the whole grid (aims_gpu_batch_points, L210-218),
+    inputs resident on the device.  Memory / latency-bound set-up work, outside the hot path: a separate line, no FP64 roofline."""
+    import torch.distributed as dist
+    r_part = float(bun.meta["r_part"])
+    max_batch = int(bun.meta["max_batch"])
+    with torch.cuda.stream(stream):
+        xyz = torch.as_tensor(bun.xyz).to("cuda")
+        owner = torch.as_tensor(bun.owner.astype(np.int32)).to("cuda")
+    stream.synchronize()
+
+    def step():
+        with torch.cuda.stream(stream):
+            w = ctx.partition_weights(xyz, owner, r_part)
+        order, ptr = aims.aims_gpu_batch_points(xyz, max_batch, device=stream.device.index, stream=stream)
+        return w, order, ptr
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    stream.synchronize()
+    sampler = ClockSampler(stream.device.index)
+    sampler.start()
+    time.sleep(0.3)
+    t_part = t_batch = 0.0
+    e = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+    tw0 = time.time()
+    for _ in range(args.steps):
+        e[0].record(stream)
+        with torch.cuda.stream(stream):
+            ctx.partition_weights(xyz, owner, r_part)
+        e[1].record(stream)
+        order, ptr = aims.aims_gpu_batch_points(xyz, max_batch, device=stream.device.index, stream=stream)
+        e[2].record(stream)
+        stream.synchronize()
+        t_part += e[0].elapsed_time(e[1])
+        t_batch += e[1].elapsed_time(e[2])
+    tw1 = time.time()
+    clocks = sampler.stop(tw0, tw1)
+    ms_step = (t_part + t_batch) / args.steps
+    if world > 1:
+        t = torch.tensor([ms_step], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_step = float(t.item())
+    out = {"metric": "grid points/s for the GPU-side grid set-up (partition weights + cut-plane batching)", "value": n_points_total / (ms_step * 1e-3),
+           "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_step,
+           "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": workload + "; set-up path", "n_points": n_points_total, "n_atoms": int(bun.n_atoms), "r_part": r_part,
+                      "max_batch": max_batch, "n_batches_found": int(len(ptr) - 1)},
+           "clocks": clocks, "gpu_launches": None,
+           "kernels": {"aims_gpu_partition_weights": {"ms_per_step": t_part / args.steps, "points_per_s": n_points_total / (t_part / args.steps * 1e-3)},
+                       "aims_gpu_batch_points": {"ms_per_step": t_batch / args.steps, "points_per_s": n_points_total / (t_batch / args.steps * 1e-3)}},
+           "e2e": None, "roofline": None, "cpu_baseline": None}
+    if rank == 0:
+        print(json.dumps(out))
+    ctx.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
 
 
 def run_reference(args, bun, gga, workload, metric, forces_q=None, hessian=False, stress=False):
@@ -360,6 +421,8 @@ def main():
         if world > 1:
             dist.barrier()
 
+    if args.path == "setup":
+        return run_setup_path(args, aims, torch, ctx, bun, stream, workload, n_points_total, world, rank)
     peak_measured = ctx.fp64_peak(200.0)
     for _ in range(max(args.warmup, 3)):
         step()

@@ -85,6 +85,18 @@ __device__ __forceinline__ int find_seg(const Seg *segs, int n_segs, long long p
   return lo;
 }
 
+// the same for a whole block of consecutive positions: one binary search for the block's first position, then every thread walks
+// forward from there (a segment that still splits has more than max_pts points, so a block of 256 positions spans a few segments;
+// per-thread binary searches over up to 40,000 segments were most of the time of a level on a 7.9 M point grid)
+__device__ __forceinline__ int find_seg_block(const Seg *segs, int n_segs, long long pos, long long n) {
+  __shared__ int s_first;
+  if (threadIdx.x == 0) s_first = find_seg(segs, n_segs, min((long long)blockIdx.x * blockDim.x, n - 1));
+  __syncthreads();
+  int s = s_first;
+  while (s + 1 < n_segs && segs[s + 1].start <= pos) s++;
+  return s;
+}
+
 __global__ void k_keys(const double *xyz, long long n, int c, double *key, int *idx) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
@@ -112,8 +124,8 @@ __global__ void k_axis(const Seg *segs, int n_segs, const double *xyz, const int
 __global__ void k_mark(const Seg *segs, int n_segs, const int *axis, const int *p0, const int *p1, const int *p2, long long n,
                        unsigned char *side) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const int s = find_seg_block(segs, n_segs, min(i, n - 1), n);
   if (i >= n) return;
-  const int s = find_seg(segs, n_segs, i);
   const Seg g = segs[s];
   if (!g.split) return;
   const int ax = axis[s];
@@ -130,8 +142,8 @@ __global__ void k_flags(const int *perm, const unsigned char *side, long long n,
 __global__ void k_partition(const Seg *segs, int n_segs, const int *perm, const unsigned char *side, const int *scan,
                             const int *block_sum, long long n, int *perm_out) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const int s = find_seg_block(segs, n_segs, min(i, n - 1), n);
   if (i >= n) return;
-  const int s = find_seg(segs, n_segs, i);
   const Seg g = segs[s];
   const int pt = perm[i];
   if (!g.split) { perm_out[i] = pt; return; }
@@ -144,8 +156,8 @@ __global__ void k_partition(const Seg *segs, int n_segs, const int *perm, const 
 // a finished level: leaves take their final order from perm_(parent's axis); tag[pos] = axis array to read at the end
 __global__ void k_tag_children(const Seg *segs, int n_segs, const int *axis, long long n, signed char *tag) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const int s = find_seg_block(segs, n_segs, min(i, n - 1), n);
   if (i >= n) return;
-  const int s = find_seg(segs, n_segs, i);
   if (segs[s].split) tag[i] = (signed char)axis[s];
 }
 
