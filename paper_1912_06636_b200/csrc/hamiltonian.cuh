@@ -31,7 +31,14 @@ constexpr int kHIB = AIMS_H_IB, kHJB = 2; // blocks per panel
 constexpr int kHI = 32 * kHIB;    // max rows of the I panel
 constexpr int kHJ = 32 * kHJB;    // max rows of the J panel
 constexpr int kHWarps = kHIB * kHJB;      // one warp per block of a full tile
-constexpr int kHStages = 3;
+#ifndef AIMS_H_STAGES
+#define AIMS_H_STAGES 3
+#endif
+#ifndef AIMS_H_STRIP_ROWS
+#define AIMS_H_STRIP_ROWS 8           // rows of a warp's staging strip: 8, or 4 (two passes per sub-tile row; frees shared memory for a 4th stage)
+#endif
+constexpr int kHStages = AIMS_H_STAGES;
+constexpr int kHStripRows = AIMS_H_STRIP_ROWS;
 constexpr int kHThreads = 32 * kHWarps;
 constexpr int kHCtasPerSm = 16 / kHWarps;
 constexpr int kHStripLd = 40;     // row stride of a warp's 8-row staging strip (conflict-free 16-byte stores)
@@ -65,7 +72,7 @@ template <bool GGA>
 __host__ __device__ constexpr int h_stage_doubles() { return h_stage_groups<GGA>() * h_group_doubles<GGA>(); }
 template <bool GGA>
 constexpr size_t h_smem_bytes() {
-  return (size_t)kHStages * h_stage_doubles<GGA>() * sizeof(double) + (size_t)kHWarps * 8 * kHStripLd * sizeof(double) +
+  return (size_t)kHStages * h_stage_doubles<GGA>() * sizeof(double) + (size_t)kHWarps * kHStripRows * kHStripLd * sizeof(double) +
          2 * kHStages * sizeof(unsigned long long) + (kHI + kHJ + kMaxActive) * sizeof(int);
 }
 
@@ -174,7 +181,7 @@ __global__ void __launch_bounds__(kHThreads, kHCtasPerSm) k_hamiltonian(DevSys S
   extern __shared__ __align__(128) unsigned char smem_raw[];
   double *sm = reinterpret_cast<double *>(smem_raw);
   double *s_strip = sm + (size_t)NST * SW;                                  // [warps][8][kHStripLd]
-  unsigned long long *s_bar = reinterpret_cast<unsigned long long *>(s_strip + kHWarps * 8 * kHStripLd);   // full[NST], empty[NST]
+  unsigned long long *s_bar = reinterpret_cast<unsigned long long *>(s_strip + kHWarps * kHStripRows * kHStripLd);   // full[NST], empty[NST]
   int *s_rowinfo = reinterpret_cast<int *>(s_bar + 2 * NST);
   int *s_colinfo = s_rowinfo + kHI;
   int *s_ld = s_colinfo + kHJ;
@@ -308,7 +315,7 @@ __global__ void __launch_bounds__(kHThreads, kHCtasPerSm) k_hamiltonian(DevSys S
   }
 #endif
 #if !defined(AIMS_PROBE_H_EPILOGUE) || AIMS_PROBE_H_EPILOGUE != 0
-  double *strip = s_strip + warp * (8 * kHStripLd);
+  double *strip = s_strip + warp * (kHStripRows * kHStripLd);
   const int fr = lane >> 2, fk = lane & 3;
   const long long *ptab = L.ptab + L.ptab_off[b];
   const int ci = (lane < wb * 8) ? s_colinfo[cj0 - rJ0 + lane] : -1;
@@ -320,16 +327,20 @@ __global__ void __launch_bounds__(kHThreads, kHCtasPerSm) k_hamiltonian(DevSys S
 #pragma unroll
   for (int a = 0; a < 4; a++) {
     if (a < wa) {
-      __syncwarp();
 #pragma unroll
-      for (int c = 0; c < 4; c++)
-        if (c < wb && (!diag || c >= a))
-          *reinterpret_cast<double2 *>(strip + fr * kHStripLd + c * 8 + 2 * fk) = make_double2(acc[a][c][0], acc[a][c][1]);
+      for (int h = 0; h < 8 / kHStripRows; h++) {
+      __syncwarp();
+      if (kHStripRows == 8 || (fr / kHStripRows) == h) {
+#pragma unroll
+        for (int c = 0; c < 4; c++)
+          if (c < wb && (!diag || c >= a))
+            *reinterpret_cast<double2 *>(strip + (fr % kHStripRows) * kHStripLd + c * 8 + 2 * fk) = make_double2(acc[a][c][0], acc[a][c][1]);
+      }
       __syncwarp();
       if (ci >= 0 && !(diag && csub < a)) {
 #pragma unroll
-        for (int r = 0; r < 8; r++) {
-          const int ri = s_rowinfo[ri0 - rI0 + a * 8 + r];
+        for (int r = 0; r < kHStripRows; r++) {
+          const int ri = s_rowinfo[ri0 - rI0 + a * 8 + h * kHStripRows + r];
           if (ri < 0) break;                                  // rows beyond nnz (zero padding) end the batch matrix
           const int si = ri >> 16, ra = ri & 0xFFFF;
           if (si > sj) continue;                              // lower atom block (only inside diagonal sub-tiles)
@@ -345,6 +356,7 @@ __global__ void __launch_bounds__(kHThreads, kHCtasPerSm) k_hamiltonian(DevSys S
           if (si == sj && !(diag && csub == a)) red_add_f64(A.H + base + (long long)cb * ldj + ra, val);
 #endif
         }
+      }
       }
     }
   }
