@@ -66,6 +66,7 @@ def parse():
     ap.add_argument("--n-ang", type=int, default=None)
     ap.add_argument("--cpu-sample-batches", type=int, default=96)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--workspace-gib", type=float, default=0.0, help="Phi-plane workspace of the context (0 = library default, 24 GiB)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--path", default="scf", choices=["scf", "forces", "stress", "hessian", "setup"])
     ap.add_argument("--deterministic", action="store_true",
@@ -342,7 +343,7 @@ def main():
     npb_all = np.diff(full.batch_ptr).astype(np.float64)
     if world == 1:
         bun = full
-        ctx = aims.aims_gpu_create(bun, device=local_rank, stream=stream)
+        ctx = aims.aims_gpu_create(bun, device=local_rank, stream=stream, workspace_bytes=int(args.workspace_gib * 2 ** 30))
         nnz_all = ctx.batch_nnz().astype(np.float64)
         g0, g1 = 0, full.n_batches
     else:
@@ -358,7 +359,7 @@ def main():
         nnz_all = nnz_t.cpu().numpy().astype(np.float64)
         g0, g1 = partition_batches(npb_all * nnz_all * nnz_all, world)[rank]
         bun, _, _ = slice_bundle(full, g0, g1)
-        ctx = aims.aims_gpu_create(bun, device=local_rank, stream=stream)
+        ctx = aims.aims_gpu_create(bun, device=local_rank, stream=stream, workspace_bytes=int(args.workspace_gib * 2 ** 30))
     del full
     t_create = time.time() - t_create
     if args.deterministic:
