@@ -206,6 +206,42 @@ int aims_gpu_pulay_forces_stress(aims_gpu_ctx *ctx, int32_t b0, int32_t b1, cons
 int aims_gpu_partition_weights(aims_gpu_ctx *ctx, int64_t n, const double *xyz, const int32_t *owner, double r_part,
                                double *w_part);
 
+/* The same weights for a caller that must not allocate device memory.  Who that is: a rank that shares its GPU with other
+ * MPI tasks through MPS (how the paper runs) under a per-client memory limit its own pools have already used
+ * up; a host program whose caching allocator (torch's, an MD driver's) holds all free HBM, so that a raw cudaMalloc fails
+ * although the program still has room; and a loop that cannot afford the device-wide stall of cudaMalloc / cudaFree.  For
+ * them every other call here is out of reach: aims_gpu_create allocates, and aims_gpu_partition_weights needs a context
+ * and grows a buffer.  The weights come before the context in any case (they go into aims_grid_desc.w), so this call
+ * takes no context: the atoms are passed directly and the caller still owns every input and output array.
+ *
+ * The scratch the kernel needs next to them -- the cell list of the atoms, the device copy of their positions, one flag
+ * word -- lives in a fixed array inside the library, AIMS_NOALLOC_SCRATCH_BYTES (about 1.5 MB) of device memory that EVERY
+ * GPU which loads the library holds until the process exits, whether this call is used or not.  That fixes the sizes:
+ *   n_atoms <= AIMS_NOALLOC_MAX_ATOMS, and the cells of edge r_part spanned by the atoms' bounding box <= AIMS_NOALLOC_MAX_CELLS;
+ * anything larger returns AIMS_ERR_UNSUPPORTED and says which limit in err_text; nothing has been enqueued then.  A point
+ * with more than 256 atoms within r_part also returns AIMS_ERR_UNSUPPORTED (found on the device; w_part of such points is 0,
+ * the others are valid).  The call makes no cudaMalloc / cudaFree and uses no library routine that allocates device memory;
+ * on the host it builds the cell list in ordinary heap vectors.
+ *
+ * Arguments.  HOST: atom_xyz [n_atoms][3] (NULL only if n_atoms == 0; read during the call); err_text NULL or a buffer of
+ * err_capacity bytes that receives a NUL-terminated message on failure ("" on success).  DEVICE, on `device`: xyz [n][3],
+ * owner [n], w_part [n] (output).  Same definition, same kernel and the same results as aims_gpu_partition_weights.
+ * Enqueued on `cuda_stream` of `device`; the call waits for that stream before it returns (it reads the flag word back).
+ *
+ * Sharing.  All calls on one device use the one array, and it keeps what the last call wrote: each call overwrites the
+ * part it reads and clears the flag word first, so calls one after another need no care.  Two calls that are in flight on
+ * the same GPU at once (two host threads, each on its own stream) overwrite each other's cell list -- a race the library
+ * does not guard against; keep such calls apart yourself.  Other devices, and other processes, have their own copy.
+ *
+ * First call on a device.  It looks up where the array lives on that device (once per device and process, with that device
+ * made current) and keeps the address.  Make this first call before you begin any stream capture on that device. */
+#define AIMS_NOALLOC_MAX_ATOMS 16384
+#define AIMS_NOALLOC_MAX_CELLS 262144
+#define AIMS_NOALLOC_SCRATCH_BYTES (4 * (AIMS_NOALLOC_MAX_CELLS + 64) + 4 * AIMS_NOALLOC_MAX_ATOMS + 24 * AIMS_NOALLOC_MAX_ATOMS + 256)
+int aims_gpu_partition_weights_noalloc(int device, void *cuda_stream, int32_t n_atoms, const double *atom_xyz, int64_t n,
+                                       const double *xyz, const int32_t *owner, double r_part, double *w_part,
+                                       char *err_text, int32_t err_capacity);
+
 /* Row f3 of SURVEY.md 8(f): periodic boundary conditions.  The real-space matrix h^uc of Eq. 12 runs over
  * the N_rs functions of the cell atoms AND their periodic images that reach into the cell; the caller passes all of them as
  * atoms (the cell's own atoms first) with the grid points mapped back into the cell at T = 0 (L113-115), and

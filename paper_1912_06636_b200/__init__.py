@@ -5,5 +5,5 @@ binding over it (argument marshalling only).  There is no CPU fallback: a missin
 """
 from .binding import (AimsError, Context, aims_gpu_add_tau_matrix, aims_gpu_batch_points, aims_gpu_bloch_fold, aims_gpu_create,  # noqa: F401
                       aims_gpu_density_hessian, aims_gpu_destroy, aims_gpu_eval_basis, aims_gpu_integrate_hamiltonian,
-                      aims_gpu_integrate_hamiltonian_ks, aims_gpu_partition_weights, aims_gpu_periodic_images, aims_gpu_pulay_forces,
+                      aims_gpu_integrate_hamiltonian_ks, aims_gpu_partition_weights, aims_gpu_partition_weights_noalloc, aims_gpu_periodic_images, aims_gpu_pulay_forces,
                       aims_gpu_pulay_forces_ks, aims_gpu_pulay_forces_stress, aims_gpu_set_deterministic, aims_gpu_update_density, aims_gpu_wrap_points, exported_symbols, load_library)

@@ -86,6 +86,9 @@ def load_library():
     L.aims_gpu_update_density.argtypes = [cp, ctypes.c_int32, ctypes.c_int32, _vp, _vp, _vp]
     L.aims_gpu_partition_weights.restype = ctypes.c_int
     L.aims_gpu_partition_weights.argtypes = [cp, ctypes.c_int64, _vp, _vp, ctypes.c_double, _vp]
+    L.aims_gpu_partition_weights_noalloc.restype = ctypes.c_int
+    L.aims_gpu_partition_weights_noalloc.argtypes = [ctypes.c_int, _vp, ctypes.c_int32, _vp, ctypes.c_int64, _vp, _vp, ctypes.c_double, _vp,
+                                                     ctypes.c_char_p, ctypes.c_int32]
     L.aims_gpu_bloch_fold.restype = ctypes.c_int
     L.aims_gpu_bloch_fold.argtypes = [cp, _vp, _ip, _dp, ctypes.c_int32, _dp, _vp, _vp, ctypes.c_int]
     L.aims_gpu_density_hessian.restype = ctypes.c_int
@@ -509,6 +512,43 @@ def aims_gpu_wrap_points(lattice, xyz, device=0, stream=None):
     if rc != 0:
         raise AimsError("aims_gpu_wrap_points failed (%d)" % rc)
     return x
+
+
+def aims_gpu_partition_weights_noalloc(atom_xyz, xyz, owner, r_part, w_part=None, device=0, stream=None):
+    """Device tensor [n] of partition-of-unity weights, computed without the library allocating any device memory
+    (include/aims_gpu.h: aims_gpu_partition_weights_noalloc).  For programs that cannot let a library call cudaMalloc: a rank
+    at its MPS memory limit, a host whose pool allocator already owns the HBM, a loop that must not stall in the allocator.
+    No context is needed; atom_xyz is a HOST array [n_atoms][3].  Pass xyz, owner and w_part as device tensors (float64
+    [n][3], int32 [n], float64 [n]) and the call touches no allocator at all; host arrays are copied to the device through
+    torch first and a missing w_part is made with torch, both for convenience only.  The library's built-in scratch array is
+    shared by every call on the device: do not run two of these calls concurrently on one GPU.  Waits for the stream.
+    Raises AimsError with the library's message when a size limit (AIMS_NOALLOC_MAX_ATOMS / _MAX_CELLS) is exceeded."""
+    import torch
+    L = load_library()
+    if not torch.cuda.is_available():
+        raise AimsError("no CUDA device: this path has no CPU fallback")
+    dev = torch.device("cuda", device)
+    st = stream if stream is not None else torch.cuda.current_stream(dev)
+    R = np.ascontiguousarray(atom_xyz, dtype=np.float64).reshape(-1, 3)
+    with torch.cuda.stream(st):
+        x = xyz if isinstance(xyz, torch.Tensor) else torch.as_tensor(np.ascontiguousarray(xyz, dtype=np.float64))
+        x = x.to(dev, torch.float64).reshape(-1, 3).contiguous()
+        o = owner if isinstance(owner, torch.Tensor) else torch.as_tensor(np.ascontiguousarray(owner, dtype=np.int32))
+        o = o.to(dev, torch.int32).contiguous()
+        n = int(x.shape[0])
+        if o.numel() != n:
+            raise AimsError("owner must have one entry per point")
+        if w_part is None:
+            w_part = torch.empty(n, dtype=torch.float64, device=dev)
+    if w_part.dtype != torch.float64 or w_part.device != dev or w_part.numel() != n or not w_part.is_contiguous():
+        raise AimsError("w_part must be a contiguous float64 tensor of n entries on the device")
+    msg = ctypes.create_string_buffer(512)
+    rc = L.aims_gpu_partition_weights_noalloc(int(device), ctypes.c_void_p(st.cuda_stream), int(R.shape[0]), R.ctypes.data_as(_vp), n,
+                                              _ptr(x) if n else None, _ptr(o) if n else None, float(r_part), _ptr(w_part) if n else None,
+                                              msg, len(msg))
+    if rc != 0:
+        raise AimsError("aims_gpu_partition_weights_noalloc failed (%d): %s" % (rc, msg.value.decode(errors="replace")))
+    return w_part
 
 
 # ---- module-level functions with the names of the C ABI

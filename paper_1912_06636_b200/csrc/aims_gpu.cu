@@ -4,6 +4,7 @@
 
 #include <algorithm>
 #include <cmath>
+#include <cstdarg>
 #include <cstdio>
 #include <cstring>
 #include <map>
@@ -1378,8 +1379,144 @@ static int impl_fp64_peak(aims_gpu_ctx *c, double ms_target, double *tflops) {
 
 }  // extern "C"
 
+// ---- aims_gpu_partition_weights_noalloc: k_partition_weights for callers that cannot allocate device memory (an MPS client at
+// its memory limit, a program whose pool allocator owns the HBM, a loop that must not stall in cudaMalloc).  What
+// impl_partition_weights keeps in a cudaMalloc'ed buffer of the context -- cell_start, cell_atom -- and what it borrows from
+// the context -- the device copy of the atom positions, the error flag -- sits here in ONE array that is part of the library
+// image: every device that loads the library carries these 1.5 MB until the process ends.  The sizes the array is cut for
+// are the limits in include/aims_gpu.h.
+//
+// `g_noalloc_scratch` names the array in DEVICE code.  In host code the same name is only the handle the runtime registered for
+// it -- not an address a kernel may dereference -- so the host asks the runtime, per device, where the array actually lives
+// (noalloc_scratch_on) and passes that pointer to the kernel.
+constexpr size_t kNaCellStartBytes = 4 * ((size_t)AIMS_NOALLOC_MAX_CELLS + 64);    // int [cells + 1], rounded up to 256 B
+constexpr size_t kNaCellAtomBytes = 4 * (size_t)AIMS_NOALLOC_MAX_ATOMS;            // int [atoms]
+constexpr size_t kNaAtomXyzBytes = 24 * (size_t)AIMS_NOALLOC_MAX_ATOMS;            // double [atoms][3]
+constexpr size_t kNaOffCellAtom = kNaCellStartBytes, kNaOffAtomXyz = kNaOffCellAtom + kNaCellAtomBytes,
+                 kNaOffFlag = kNaOffAtomXyz + kNaAtomXyzBytes, kNaBytes = kNaOffFlag + 256;
+static_assert(kNaBytes == AIMS_NOALLOC_SCRATCH_BYTES, "header states the size of the array");
+static_assert(kNaOffCellAtom % 256 == 0 && kNaOffAtomXyz % 256 == 0 && kNaOffFlag % 256 == 0, "sub-arrays keep the alignment");
+
+static __device__ __align__(256) unsigned char g_noalloc_scratch[kNaBytes];
+
+namespace {
+
+constexpr int kNaMaxDevices = 64;
+std::mutex g_noalloc_mu;
+unsigned char *g_noalloc_ptr[kNaMaxDevices] = {};   // device address of g_noalloc_scratch, per device ordinal (0 = not asked yet)
+
+// Set-up, once per device and process: `device` must be current.  The first use of a symbol of this module may make the
+// runtime load the module, which is why the header asks for the first call to come before any stream capture.
+cudaError_t noalloc_scratch_on(int device, unsigned char **out) {
+  std::lock_guard<std::mutex> lock(g_noalloc_mu);
+  if (!g_noalloc_ptr[device]) {
+    void *p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&p, g_noalloc_scratch);
+    if (e != cudaSuccess) return e;
+    g_noalloc_ptr[device] = static_cast<unsigned char *>(p);
+  }
+  *out = g_noalloc_ptr[device];
+  return cudaSuccess;
+}
+
+int na_fail(char *err_text, int cap, int code, const char *fmt, ...) {
+  if (err_text && cap > 0) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(err_text, (size_t)cap, fmt, ap);
+    va_end(ap);
+  }
+  return code;
+}
+
+#define NA_TRY(call)                                                                                            \
+  do {                                                                                                          \
+    const cudaError_t e_ = (call);                                                                              \
+    if (e_ != cudaSuccess) return na_fail(err_text, cap, AIMS_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
+  } while (0)
+
+int impl_partition_weights_noalloc(int device, cudaStream_t st, int na, const double *R, long long n, const double *xyz,
+                                   const int *owner, double r_part, double *w_part, char *err_text, int cap) {
+  if (err_text && cap > 0) err_text[0] = 0;
+  if (device < 0 || device >= kNaMaxDevices || na < 0 || n < 0 || (na && !R) || (n && (!xyz || !owner || !w_part)) || !(r_part > 0))
+    return na_fail(err_text, cap, AIMS_ERR_INVALID_ARG, "NULL array, negative size, r_part <= 0 or device outside [0, %d)", kNaMaxDevices);
+  if (na > AIMS_NOALLOC_MAX_ATOMS)
+    return na_fail(err_text, cap, AIMS_ERR_UNSUPPORTED, "n_atoms = %d is more than AIMS_NOALLOC_MAX_ATOMS = %d, the size the built-in scratch "
+                   "array is cut for; use aims_gpu_partition_weights (it allocates)", na, AIMS_NOALLOC_MAX_ATOMS);
+  if (!n) return AIMS_OK;
+  // cell list of the atoms on the host, as in impl_partition_weights: edge a hair above r_part, atoms ascending inside a cell
+  double lo[3] = {0, 0, 0}, hi[3] = {0, 0, 0};
+  for (int a = 0; a < na; a++)
+    for (int d = 0; d < 3; d++) {
+      if (!std::isfinite(R[3 * a + d])) return na_fail(err_text, cap, AIMS_ERR_INVALID_ARG, "atom_xyz[%d][%d] is not finite", a, d);
+      if (a == 0 || R[3 * a + d] < lo[d]) lo[d] = R[3 * a + d];
+      if (a == 0 || R[3 * a + d] > hi[d]) hi[d] = R[3 * a + d];
+    }
+  const double edge = r_part * (1.0 + 1e-9);
+  int dim[3];
+  double cells_total = 1.0;
+  for (int d = 0; d < 3; d++) {
+    const double cells = std::floor((hi[d] - lo[d]) / edge) + 1.0;
+    cells_total *= cells;
+    dim[d] = cells <= (double)AIMS_NOALLOC_MAX_CELLS ? (int)cells : 0;
+  }
+  if (!(cells_total <= (double)AIMS_NOALLOC_MAX_CELLS))
+    return na_fail(err_text, cap, AIMS_ERR_UNSUPPORTED, "the atoms span %.0f cells of edge r_part = %g, more than AIMS_NOALLOC_MAX_CELLS = %d, the "
+                   "size the built-in scratch array is cut for; use aims_gpu_partition_weights (it allocates)", cells_total, r_part,
+                   AIMS_NOALLOC_MAX_CELLS);
+  const int ncell = dim[0] * dim[1] * dim[2];
+  std::vector<int> start((size_t)ncell + 1, 0), order((size_t)std::max(na, 1)), cell_of((size_t)std::max(na, 1));
+  for (int a = 0; a < na; a++) {
+    int ic[3];
+    for (int d = 0; d < 3; d++) ic[d] = std::min(dim[d] - 1, std::max(0, (int)std::floor((R[3 * a + d] - lo[d]) / edge)));
+    cell_of[a] = (ic[2] * dim[1] + ic[1]) * dim[0] + ic[0];
+    start[(size_t)cell_of[a] + 1]++;
+  }
+  for (int q = 0; q < ncell; q++) start[(size_t)q + 1] += start[(size_t)q];
+  {
+    std::vector<int> fill(start.begin(), start.end() - 1);
+    for (int a = 0; a < na; a++) order[(size_t)fill[(size_t)cell_of[a]]++] = a;
+  }
+
+  NA_TRY(cudaSetDevice(device));
+  unsigned char *base = nullptr;
+  NA_TRY(noalloc_scratch_on(device, &base));
+  int *d_start = reinterpret_cast<int *>(base), *d_order = reinterpret_cast<int *>(base + kNaOffCellAtom),
+      *d_flag = reinterpret_cast<int *>(base + kNaOffFlag);
+  double *d_R = reinterpret_cast<double *>(base + kNaOffAtomXyz);
+  // the array still holds the previous call's cell list and flag: everything the kernel reads is overwritten here, and the
+  // flag -- which the kernel only ever raises -- is cleared
+  NA_TRY(cudaMemcpyAsync(d_start, start.data(), start.size() * sizeof(int), cudaMemcpyHostToDevice, st));
+  if (na) {
+    NA_TRY(cudaMemcpyAsync(d_order, order.data(), (size_t)na * sizeof(int), cudaMemcpyHostToDevice, st));
+    NA_TRY(cudaMemcpyAsync(d_R, R, (size_t)na * 3 * sizeof(double), cudaMemcpyHostToDevice, st));
+  }
+  NA_TRY(cudaMemsetAsync(d_flag, 0, sizeof(int), st));
+  const PartCells PC{lo[0], lo[1], lo[2], 1.0 / edge, dim[0], dim[1], dim[2], d_start, d_order};
+  k_partition_weights<<<(unsigned)((n + kPartWarps - 1) / kPartWarps), kPartWarps * 32, 0, st>>>(PC, d_R, n, xyz, owner, r_part, w_part, d_flag);
+  NA_TRY(cudaGetLastError());
+  int flag = 0;
+  NA_TRY(cudaMemcpyAsync(&flag, d_flag, sizeof(int), cudaMemcpyDeviceToHost, st));
+  NA_TRY(cudaStreamSynchronize(st));                     // start / order / R are the caller's or host temporaries; flag is read here
+  if (flag)
+    return na_fail(err_text, cap, AIMS_ERR_UNSUPPORTED, "a point has more than %d atoms within r_part = %g (its weight was set to 0)", kPartMaxCand, r_part);
+  return AIMS_OK;
+}
+
+}  // namespace
+
 // ---- the exported entry points: every body runs under `guarded` (no exception leaves the library)
 extern "C" {
+
+int aims_gpu_partition_weights_noalloc(int device, void *cuda_stream, int32_t n_atoms, const double *atom_xyz, int64_t n, const double *xyz,
+                                       const int32_t *owner, double r_part, double *w_part, char *err_text, int32_t err_capacity) {
+  const int rc = guarded(nullptr, [&] {
+    return impl_partition_weights_noalloc(device, static_cast<cudaStream_t>(cuda_stream), n_atoms, atom_xyz, (long long)n, xyz, owner, r_part,
+                                          w_part, err_text, err_capacity);
+  });
+  if (rc == AIMS_ERR_NOMEM && err_text && err_capacity > 0 && !err_text[0]) snprintf(err_text, (size_t)err_capacity, "out of host memory");
+  return rc;
+}
 
 int aims_gpu_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_grid_desc *G, const aims_bsr_desc *P, int device, void *cuda_stream, int64_t workspace_bytes) {
   // on failure *out is either NULL or a context that only aims_gpu_last_error and aims_gpu_destroy accept
