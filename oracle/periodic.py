@@ -11,8 +11,10 @@ T = (0,0,0)" (L113-115); it states neither how the images are enumerated nor how
            integer vector n -- is KEPT iff  -delta_i < f_a,i + n_i < 1 + delta_i  for i = 1, 2, 3  (a parallelepiped that contains
            every point within `reach` of the cell: a superset of the atoms whose functions reach into the cell; the culling of
            S1a drops the rest per batch).  Order: the cell's own atoms (n = 0) first, then ascending (n_1, n_2, n_3, a).
-  wrap     f = r A^-1 with A^-1 from the cofactor formula, f <- f - floor(f), r <- f A; every product and sum separately
-           rounded, sums left to right -- one result is correct to the last bit.
+  wrap     f = r A^-1 with A^-1 from the cofactor formula, f <- f - floor(f), and f <- 0 where that difference rounds to 1
+           (a tiny negative f: 1 - 1e-20 is not a double; the face f = 1 is the face f = 0 of the next cell, so the point is
+           put on f = 0 and the promised range [0, 1) holds), r <- f A; every product and sum separately rounded, sums left to
+           right -- one result is correct to the last bit.
 Pins (tests/test_oracle_periodic_pins.py): every atom within `reach` of a dense sample of cell points is in the list, no atom
 twice, brute force over a large integer box; wrapped points differ from the originals by an integer lattice vector, have
 fractional coordinates in [0, 1), wrapping is idempotent; and both reproduce the atoms / points of the seeded periodic bundle
@@ -69,6 +71,7 @@ def wrap_points(lat, xyz):
     for j in range(3):
         f[:, j] = (r[:, 0] * inv[0, j] + r[:, 1] * inv[1, j]) + r[:, 2] * inv[2, j]
     f = f - np.floor(f)
+    f[f >= 1.0] = 0.0                          # -tiny - floor(-tiny) rounds to 1.0: the same face as 0.0, and [0, 1) is the promise
     out = np.empty_like(r)
     for j in range(3):
         out[:, j] = (f[:, 0] * a[0, j] + f[:, 1] * a[1, j]) + f[:, 2] * a[2, j]

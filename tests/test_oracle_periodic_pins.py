@@ -144,3 +144,19 @@ def test_wrapped_points_differ_by_a_lattice_vector_and_lie_in_the_cell():
     r0 = np.array([[0.3, 0.2, 0.1]]) @ lat
     for nvec in ([1, 0, 0], [-2, 3, 1], [0, -1, 4]):
         assert np.abs(wrap_points(lat, r0 + np.array(nvec) @ lat) - r0).max() < 1e-12
+
+
+def test_wrap_of_a_point_a_hair_below_a_cell_face_stays_inside_the_half_open_cell():
+    """Reading P23 promises fractional coordinates in [0, 1).  For f = -1e-20 the difference f - floor(f) = 1 - 1e-20 rounds to
+    1.0, the excluded face; that face is the f = 0 face of the neighbouring cell, so the wrapped point must sit at f = 0
+    exactly (cubic cell of edge 4: coordinates 0, not 4).  Points well inside and exactly on faces keep their textbook images."""
+    from oracle.periodic import wrap_points
+    lat = 4.0 * np.eye(3)
+    tiny = 1e-20
+    r = np.array([[-tiny, 1.0, 2.0], [1.0, -tiny, -tiny], [4.0, 8.0, -4.0], [-1.0, 5.0, 3.5], [-4.0 * 2.0 ** -60, 0.5, 0.5]])
+    w = wrap_points(lat, r)
+    want = np.array([[0.0, 1.0, 2.0], [1.0, 0.0, 0.0], [0.0, 0.0, 0.0], [3.0, 1.0, 3.5], [0.0, 0.5, 0.5]])
+    assert np.array_equal(w, want)
+    f = w / 4.0
+    assert f.min() >= 0.0 and f.max() < 1.0
+    assert np.array_equal(wrap_points(lat, w), w)          # idempotent to the bit
