@@ -31,17 +31,30 @@ def first_phase_range(n_batches, rank, world):
     return (n_batches * rank) // world, (n_batches * (rank + 1)) // world
 
 
+# attributes that describe the whole system (atoms, basis, block pattern, matrices): every rank keeps them whole, also when one
+# of their dimensions happens to equal the number of grid points
+GLOBAL_FIELDS = frozenset((
+    "atom_xyz", "atom_species", "species_shell_ptr", "shell_l", "shell_rcut", "shell_spline", "spline_coef", "shell_zeta",
+    "shell_norm", "row_ptr", "col_atom", "blk_off", "blk_ld", "D_values", "atom_fn_ptr", "batch_ptr",
+    "lattice", "frac", "atom_home", "atom_n", "atom_T"))
+
+
 def slice_bundle(bun, b0, b1):
-    """The inputs of batches [b0, b1) only: grid arrays cut to the batches' point range, batch_ptr rebased to 0; atoms, basis,
-    block pattern, D (global objects every rank needs) unchanged.  Returns (sliced bundle, first point, last point)."""
+    """The inputs of batches [b0, b1) only.  batch_ptr is cut and rebased to 0; EVERY other array attribute that carries one
+    entry per grid point -- leading dimension n_points ([n], [n][k]: xyz, w, v, owner, xyz_unwrapped, ...) or, for two-dimensional
+    component-major fields, trailing dimension n_points ([k][n]: g) -- is cut to the batches' point range, whatever its name, so
+    that a per-point field added to the bundle later cannot stay full-size beside a shrunken grid.  GLOBAL_FIELDS (atoms, basis,
+    block pattern, D: objects every rank needs whole) and non-array attributes are shared unchanged.
+    Returns (sliced bundle, first point, last point)."""
+    n = int(bun.xyz.shape[0])
     lo, hi = int(bun.batch_ptr[b0]), int(bun.batch_ptr[b1])
     s = copy.copy(bun)
-    s.xyz = np.ascontiguousarray(bun.xyz[lo:hi])
-    s.w = np.ascontiguousarray(bun.w[lo:hi])
     s.batch_ptr = np.ascontiguousarray(bun.batch_ptr[b0:b1 + 1] - lo).astype(np.int64)
-    for name in ("v", "owner"):
-        if getattr(bun, name, None) is not None:
-            setattr(s, name, np.ascontiguousarray(getattr(bun, name)[lo:hi]))
-    if getattr(bun, "g", None) is not None:
-        s.g = np.ascontiguousarray(bun.g[:, lo:hi])
+    for name, val in vars(bun).items():
+        if name in GLOBAL_FIELDS or not isinstance(val, np.ndarray) or val.ndim == 0:
+            continue
+        if val.shape[0] == n:
+            setattr(s, name, np.ascontiguousarray(val[lo:hi]))
+        elif val.ndim == 2 and val.shape[1] == n:
+            setattr(s, name, np.ascontiguousarray(val[:, lo:hi]))
     return s, lo, hi
