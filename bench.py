@@ -68,6 +68,8 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--workspace-gib", type=float, default=0.0, help="Phi-plane workspace of the context (0 = library default, 24 GiB)")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--lib", default=None, help="measure with a probe build of the library (build.py --define ... --tag ...); its "
+                    "switches are recorded in the JSON line under build_flags, and such a line is not a bench value")
     ap.add_argument("--path", default="scf", choices=["scf", "forces", "stress", "hessian", "setup"])
     ap.add_argument("--deterministic", action="store_true",
                     help="ordered (bitwise reproducible) scatter into H: aims_gpu_set_deterministic")
@@ -326,6 +328,7 @@ def main():
     import paper_1912_06636_b200 as aims
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    build_flags = aims.load_library(args.lib, allow_probe=args.lib is not None)._aims_build_flags
     torch.cuda.set_device(local_rank)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
@@ -641,7 +644,7 @@ def main():
                             % (1e-9 * eval_bytes, 8e-9 * bun.n_values)},
            "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "roofline": roofline,
            "roofline_eval": roofline_eval, "fp64_tflops_step": total_tflops, "fp64_frac_of_peak_step": total_tflops / FP64_PEAK_NOMINAL_TFLOPS,
-           "kernels": kd, "setup_s": {"generate_inputs": t_gen, "create_ctx": t_create}}
+           "kernels": kd, "setup_s": {"generate_inputs": t_gen, "create_ctx": t_create}, "build_flags": build_flags}
 
     # ---- CPU baseline: the oracle on a bounded seeded sample, rank 0 at N=1 only
     if rank == 0 and world == 1 and not args.no_cpu_baseline:

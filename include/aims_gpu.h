@@ -202,7 +202,12 @@ int aims_gpu_pulay_forces_stress(aims_gpu_ctx *ctx, int32_t b0, int32_t b1, cons
  * mu_AB = (|r-R_A| - |r-R_B|) / |R_A-R_B|, cand(r) = atoms with sqrt((dx*dx + dy*dy) + dz*dz) <= r_part in separately rounded IEEE
  * operations (a discrete decision, as in reading P6); 0 if the owner is not a candidate.  The atoms are
  * the context's.  DEVICE pointers: xyz [n][3], owner [n] (atom index of the point's grid), w_part [n] (output).  The caller
- * multiplies with the radial and angular quadrature weights to obtain aims_grid_desc.w. */
+ * multiplies with the radial and angular quadrature weights to obtain aims_grid_desc.w.
+ * Limits (AIMS_ERR_UNSUPPORTED, text in aims_gpu_last_error): at most 256 atoms within r_part of any one point -- found on the
+ * device; w_part of such a point is 0, the other points are valid --; the atoms' bounding box may span at most 2048 cells of
+ * edge r_part along an axis and 2^26 cells in all.  The call waits for the context stream before it returns (it reads the
+ * device's flag back), so an error is reported by this call, not by a later aims_gpu_synchronize.  The cell list of the atoms
+ * is kept in the context for the last r_part used. */
 int aims_gpu_partition_weights(aims_gpu_ctx *ctx, int64_t n, const double *xyz, const int32_t *owner, double r_part,
                                double *w_part);
 
@@ -260,7 +265,7 @@ int aims_gpu_bloch_fold(aims_gpu_ctx *ctx, const double *H_values, const int32_t
  * back to its periodic image within the unit cell at T = (0,0,0)" (L113-115), but states neither rule; reading P23:
  *
  * aims_gpu_periodic_images.  lattice: HOST [3][3], rows a_1, a_2, a_3; frac: HOST [n_home][3] fractional coordinates of the cell
- * atoms.  With h_i = V / |a_j x a_k| (height of the cell along the i-th reciprocal direction) and delta_i = reach / h_i, the
+ * atoms, each in [0, 1) (anything else, NaN included, returns AIMS_ERR_INVALID_ARG: the enumeration box is sized for atoms inside the cell).  With h_i = V / |a_j x a_k| (height of the cell along the i-th reciprocal direction) and delta_i = reach / h_i, the
  * periodic atom (a, n) = cell atom a translated by the integer vector n is kept iff -delta_i < frac[a][i] + n_i < 1 + delta_i for
  * i = 1, 2, 3 -- a parallelepiped containing every point within `reach` of the cell, i.e. a superset of the atoms whose functions
  * (cutoff <= reach) are non-zero somewhere in the cell; the per-batch culling of aims_gpu_eval_basis drops the rest.  Order: the
@@ -272,7 +277,8 @@ int aims_gpu_periodic_images(const double *lattice, int32_t n_home, const double
                              int32_t *atom_n, int64_t capacity, int64_t *n_atoms);
 
 /* aims_gpu_wrap_points.  xyz: DEVICE [n_points][3], in place: f = r A^-1 (A = lattice rows; A^-1 by the cofactor formula,
- * determinant along the first row, computed on the host), f <- f - floor(f), r <- f A; every product and sum separately rounded
+ * determinant along the first row, computed on the host), f <- f - floor(f) (and f <- 0 where that difference rounds to 1.0, so
+ * that f lies in [0, 1) also for a point a hair below a cell face), r <- f A; every product and sum separately rounded
  * (IEEE RN, no FMA), sums left to right, so that exactly one result is correct.  lattice: HOST [3][3].  Enqueued on `cuda_stream` of
  * `device`; asynchronous.  A singular lattice returns AIMS_ERR_INVALID_ARG. */
 int aims_gpu_wrap_points(int device, void *cuda_stream, const double *lattice, int64_t n_points, double *xyz);
@@ -312,6 +318,12 @@ int aims_gpu_batch_nnz(aims_gpu_ctx *ctx, int32_t *nnz);
 
 /* ===================================================== diagnostics =====================================================
  * Nothing below is needed to compute anything; bench.py and the profiles use it. */
+
+/* Compile-time switches this library was built with: "" for the product build (the only one whose results are H, n, ...), else
+ * the -D list of a measurement ("probe") build of paper_1912_06636_b200/build.py --define ... --tag ..., some of which switch
+ * parts of the arithmetic off on purpose.  Static string.  The Python binding refuses a library that reports switches unless
+ * the caller asks for it by path and says so (load_library(path, allow_probe=True); bench.py --lib). */
+const char *aims_gpu_build_flags(void);
 
 /* Per-kernel device timing for bench.py's roofline: when enabled, every kernel launch of this context is bracketed by
  * CUDA events on the context stream.  aims_gpu_timing_enable synchronises, clears what was recorded and switches

@@ -10,8 +10,7 @@ import re
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-# AIMS_GPU_LIB: a probe build of the same sources (build.py --define ... --tag ...) for the measurements under profiles/
-LIB_PATH = os.environ.get("AIMS_GPU_LIB") or os.path.join(_HERE, "libaims_gpu.so")
+LIB_PATH = os.path.join(_HERE, "libaims_gpu.so")        # the product library; no environment variable changes this
 HEADER_PATH = os.path.join(os.path.dirname(_HERE), "include", "aims_gpu.h")
 
 _dp = ctypes.POINTER(ctypes.c_double)
@@ -52,18 +51,32 @@ def exported_symbols():
     return sorted(set(re.findall(r"\b(aims_gpu_[a-z0-9_]+)\s*\(", text)))
 
 
-def load_library():
-    """dlopen libaims_gpu.so; raises (never falls back) if it is missing or lacks a declared symbol."""
+def load_library(path=None, allow_probe=False):
+    """dlopen libaims_gpu.so; raises (never falls back) if it is missing or lacks a declared symbol.
+    path: another build of the same sources (build.py --define ... --tag ...), for the measurements under profiles/ only; it must
+    be given before the first use of the binding.  A library that reports compile-time switches (aims_gpu_build_flags() != "")
+    may compute something else than H and n on purpose and is refused unless allow_probe is set."""
     global _lib
+    want = os.path.abspath(path) if path else LIB_PATH
     if _lib is not None:
+        if want != _lib._aims_path:
+            raise AimsError("a different library is already loaded: %s" % _lib._aims_path)
         return _lib
-    if not os.path.exists(LIB_PATH):
-        raise AimsError("libaims_gpu.so is not built: run `python -m paper_1912_06636_b200.build` "
-                        "(nvcc, sm_100a). There is no CPU fallback.")
-    L = ctypes.CDLL(LIB_PATH)
+    if not os.path.exists(want):
+        raise AimsError("%s is not built: run `python -m paper_1912_06636_b200.build` "
+                        "(nvcc, sm_100a). There is no CPU fallback." % os.path.basename(want))
+    L = ctypes.CDLL(want)
     for name in exported_symbols():
         if not hasattr(L, name):
-            raise AimsError("libaims_gpu.so does not export %s" % name)
+            raise AimsError("%s does not export %s" % (os.path.basename(want), name))
+    L.aims_gpu_build_flags.restype = ctypes.c_char_p
+    L.aims_gpu_build_flags.argtypes = []
+    flags = L.aims_gpu_build_flags().decode()
+    if flags and not allow_probe:
+        raise AimsError("%s is a probe build (%s): its results are not the product's; pass allow_probe=True to measure with it"
+                        % (want, flags))
+    L._aims_path = want
+    L._aims_build_flags = flags
     cp = _vp
     L.aims_gpu_create.restype = ctypes.c_int
     L.aims_gpu_create.argtypes = [ctypes.POINTER(cp), ctypes.POINTER(_BasisDesc), ctypes.POINTER(_GridDesc),

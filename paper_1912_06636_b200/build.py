@@ -18,14 +18,17 @@ def nvcc_path():
 
 
 def build(force=False, verbose=False, defines=(), tag=None):
-    """defines / tag: a PROBE build for the profiles (e.g. `--define AIMS_PROBE_NO_H_EPILOGUE=1 --tag noepi` writes
-    libaims_gpu_noepi.so; load it with AIMS_GPU_LIB=<path>).  The product library is the untagged one."""
+    """defines / tag: a PROBE build for the profiles (e.g. `--define AIMS_PROBE_H_EPILOGUE=0 --tag noepi` writes
+    libaims_gpu_noepi.so, which reports its switches through aims_gpu_build_flags(); run it with `bench.py --lib <path>` or
+    binding.load_library(path, allow_probe=True)).  The product library is the untagged one and is built without switches."""
     lib = LIB if not tag else os.path.join(HERE, "libaims_gpu_%s.so" % tag)
     if not force and not defines and os.path.exists(lib) and all(os.path.getmtime(lib) >= os.path.getmtime(d) for d in DEPS):
         return lib
     tmp = lib + ".%d.tmp" % os.getpid()
     cmd = [nvcc_path(), "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-shared",
            "-Xcompiler", "-fPIC", "--threads", "2", "-o", tmp] + ["-D" + d for d in defines] + SRC
+    if defines:
+        cmd.insert(-len(SRC), '-DAIMS_BUILD_FLAGS="%s"' % " ".join(defines))
     if verbose:
         cmd[1:1] = ["-Xptxas", "-v"]
     subprocess.check_call(cmd)

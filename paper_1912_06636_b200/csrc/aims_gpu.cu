@@ -46,8 +46,10 @@ struct aims_gpu_ctx {
   std::vector<long long> batch_ptr, fn_off, act_off, ptab_off, pad_off, pad16_off, dpad_off, api_off, tile_off, item_off;
   std::vector<int> nnz, n_act;
   std::vector<double> h_atom_xyz;                                // host copy of the atom positions (cell lists)
-  int *d_part = nullptr;                                         // cell list of aims_gpu_partition_weights (grows on demand)
+  int *d_part = nullptr;                                         // flag word + cell list of aims_gpu_partition_weights (grows on demand)
   size_t part_cap = 0;
+  double part_r = -1.0;                                          // r_part the cached cell list was built for (< 0: none)
+  PartCells part_cells{};
   std::vector<int> h_atom_fn_ptr, h_col_atom, h_blk_ld;          // host copies of the pattern (Bloch sums)
   std::vector<long long> h_row_ptr, h_blk_off;
   int max_nnz = 0, max_act = 0, max_np = 0;
@@ -1100,55 +1102,71 @@ static int impl_partition_weights(aims_gpu_ctx *c, int64_t n, const double *xyz,
   CU_TRY(c, cudaSetDevice(c->device));
   if (!n) return AIMS_OK;
   // cell list of the atoms, cell edge r_part (a hair more, so that rounding of a cell index never hides a neighbour):
-  // every atom within r_part of a point lies in the 27 cells around the point's cell -> O(N) overall
-  const int na = c->S.n_atoms;
-  const std::vector<double> &R = c->h_atom_xyz;
-  double lo[3] = {0, 0, 0}, hi[3] = {0, 0, 0};
-  for (int a = 0; a < na; a++)
+  // every atom within r_part of a point lies in the 27 cells around the point's cell -> O(N) overall.
+  // The atoms of a context never change, so the list is kept for the last r_part seen (a grid is usually weighted in several
+  // calls with one radius); d_part = [flag word, 63 pad | cell_start | cell_atom].
+  if (!(c->part_r == r_part)) {
+    const int na = c->S.n_atoms;
+    const std::vector<double> &R = c->h_atom_xyz;
+    double lo[3] = {0, 0, 0}, hi[3] = {0, 0, 0};
+    for (int a = 0; a < na; a++)
+      for (int d = 0; d < 3; d++) {
+        if (a == 0 || R[3 * a + d] < lo[d]) lo[d] = R[3 * a + d];
+        if (a == 0 || R[3 * a + d] > hi[d]) hi[d] = R[3 * a + d];
+      }
+    const double edge = r_part * (1.0 + 1e-9);
+    int dim[3];
     for (int d = 0; d < 3; d++) {
-      if (a == 0 || R[3 * a + d] < lo[d]) lo[d] = R[3 * a + d];
-      if (a == 0 || R[3 * a + d] > hi[d]) hi[d] = R[3 * a + d];
+      const double cells = std::floor((hi[d] - lo[d]) / edge) + 1.0;
+      if (!(cells < 2048.0)) return fail(c, AIMS_ERR_UNSUPPORTED, "atoms span more than 2048 cells of edge r_part along one axis");
+      dim[d] = (int)cells;
     }
-  const double edge = r_part * (1.0 + 1e-9);
-  int dim[3];
-  for (int d = 0; d < 3; d++) {
-    const double cells = std::floor((hi[d] - lo[d]) / edge) + 1.0;
-    if (!(cells < 2048.0)) return fail(c, AIMS_ERR_UNSUPPORTED, "atoms span more than 2048 cells of edge r_part");
-    dim[d] = (int)cells;
+    const long long ncell = (long long)dim[0] * dim[1] * dim[2];
+    if (ncell > (1ll << 26)) return fail(c, AIMS_ERR_UNSUPPORTED, "cell list of the atoms too large (more than 2^26 cells of edge r_part)");
+    std::vector<int> start((size_t)ncell + 1, 0), order((size_t)std::max(na, 1)), cell_of((size_t)std::max(na, 1));
+    for (int a = 0; a < na; a++) {
+      int ic[3];
+      for (int d = 0; d < 3; d++) ic[d] = std::min(dim[d] - 1, std::max(0, (int)std::floor((R[3 * a + d] - lo[d]) / edge)));
+      cell_of[a] = (ic[2] * dim[1] + ic[1]) * dim[0] + ic[0];
+      start[(size_t)cell_of[a] + 1]++;
+    }
+    for (long long q = 0; q < ncell; q++) start[(size_t)q + 1] += start[(size_t)q];
+    {
+      std::vector<int> fill(start.begin(), start.end() - 1);
+      for (int a = 0; a < na; a++) order[(size_t)fill[(size_t)cell_of[a]]++] = a;      // ascending atom index inside a cell
+    }
+    // device copies live in a context-owned buffer that only grows
+    const size_t need = 64 + start.size() + order.size();
+    c->part_r = -1.0;                                     // nothing cached while the buffer is being replaced
+    if (need > c->part_cap) {
+      CU_TRY(c, cudaStreamSynchronize(c->stream));
+      if (c->d_part) { c->owned.erase(std::remove(c->owned.begin(), c->owned.end(), (void *)c->d_part), c->owned.end()); cudaFree(c->d_part); c->d_part = nullptr; }
+      c->part_cap = 0;
+      int rc = dev_alloc(c, &c->d_part, need);
+      if (rc) return rc;
+      c->part_cap = need;
+    }
+    CU_TRY(c, cudaMemcpyAsync(c->d_part + 64, start.data(), start.size() * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+    CU_TRY(c, cudaMemcpyAsync(c->d_part + 64 + start.size(), order.data(), order.size() * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+    CU_TRY(c, cudaStreamSynchronize(c->stream));          // start / order are host temporaries
+    c->part_cells = PartCells{lo[0], lo[1], lo[2], 1.0 / edge, dim[0], dim[1], dim[2], c->d_part + 64, c->d_part + 64 + start.size()};
+    c->part_r = r_part;
   }
-  const long long ncell = (long long)dim[0] * dim[1] * dim[2];
-  if (ncell > (1ll << 26)) return fail(c, AIMS_ERR_UNSUPPORTED, "cell list of the atoms too large");
-  std::vector<int> start((size_t)ncell + 1, 0), order((size_t)std::max(na, 1)), cell_of((size_t)std::max(na, 1));
-  for (int a = 0; a < na; a++) {
-    int ic[3];
-    for (int d = 0; d < 3; d++) ic[d] = std::min(dim[d] - 1, std::max(0, (int)std::floor((R[3 * a + d] - lo[d]) / edge)));
-    cell_of[a] = (ic[2] * dim[1] + ic[1]) * dim[0] + ic[0];
-    start[(size_t)cell_of[a] + 1]++;
-  }
-  for (long long q = 0; q < ncell; q++) start[(size_t)q + 1] += start[(size_t)q];
-  {
-    std::vector<int> fill(start.begin(), start.end() - 1);
-    for (int a = 0; a < na; a++) order[(size_t)fill[(size_t)cell_of[a]]++] = a;      // ascending atom index inside a cell
-  }
-  // device copies live in a context-owned buffer that only grows
-  const size_t need = start.size() + order.size();
-  if (need > c->part_cap) {
-    CU_TRY(c, cudaStreamSynchronize(c->stream));
-    if (c->d_part) { c->owned.erase(std::remove(c->owned.begin(), c->owned.end(), (void *)c->d_part), c->owned.end()); cudaFree(c->d_part); c->d_part = nullptr; }
-    int rc = dev_alloc(c, &c->d_part, need);
-    if (rc) return rc;
-    c->part_cap = need;
-  }
-  CU_TRY(c, cudaMemcpyAsync(c->d_part, start.data(), start.size() * sizeof(int), cudaMemcpyHostToDevice, c->stream));
-  CU_TRY(c, cudaMemcpyAsync(c->d_part + start.size(), order.data(), order.size() * sizeof(int), cudaMemcpyHostToDevice, c->stream));
-  CU_TRY(c, cudaStreamSynchronize(c->stream));          // start / order are host temporaries
-  PartCells PC{lo[0], lo[1], lo[2], 1.0 / edge, dim[0], dim[1], dim[2], c->d_part, c->d_part + start.size()};
+  // the kernel raises the flag word for a point with more than kPartMaxCand atoms within r_part (and writes 0 for it): read
+  // back here, so that the caller is told by THIS call and not by a later aims_gpu_synchronize
+  CU_TRY(c, cudaMemsetAsync(c->d_part, 0, sizeof(int), c->stream));
   {
     TimedLaunch t(c, kKindOther);
     k_partition_weights<<<(unsigned)((n + kPartWarps - 1) / kPartWarps), kPartWarps * 32, 0, c->stream>>>(
-        PC, c->S.atom_xyz, (long long)n, xyz, owner, r_part, w_part, c->L.error_flag);
+        c->part_cells, c->S.atom_xyz, (long long)n, xyz, owner, r_part, w_part, c->d_part);
   }
-  return check_async(c);
+  int rc = check_async(c);
+  if (rc) return rc;
+  int flag = 0;
+  CU_TRY(c, cudaMemcpyAsync(&flag, c->d_part, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+  CU_TRY(c, cudaStreamSynchronize(c->stream));
+  if (flag) return fail(c, AIMS_ERR_UNSUPPORTED, "a point has more than 256 atoms within r_part (its weight was set to 0)");
+  return AIMS_OK;
 }
 
 static int impl_bloch_fold(aims_gpu_ctx *c, const double *H_values, const int32_t *atom_home, const double *atom_T,
@@ -1381,8 +1399,8 @@ static int impl_fp64_peak(aims_gpu_ctx *c, double ms_target, double *tflops) {
 
 // ---- aims_gpu_partition_weights_noalloc: k_partition_weights for callers that cannot allocate device memory (an MPS client at
 // its memory limit, a program whose pool allocator owns the HBM, a loop that must not stall in cudaMalloc).  What
-// impl_partition_weights keeps in a cudaMalloc'ed buffer of the context -- cell_start, cell_atom -- and what it borrows from
-// the context -- the device copy of the atom positions, the error flag -- sits here in ONE array that is part of the library
+// impl_partition_weights keeps in a cudaMalloc'ed buffer of the context -- flag word, cell_start, cell_atom -- and what it
+// borrows from the context -- the device copy of the atom positions -- sits here in ONE array that is part of the library
 // image: every device that loads the library carries these 1.5 MB until the process ends.  The sizes the array is cut for
 // are the limits in include/aims_gpu.h.
 //
@@ -1596,6 +1614,11 @@ int aims_gpu_timing_read(aims_gpu_ctx *c, double *ms, int64_t *launches) {
 int aims_gpu_synchronize(aims_gpu_ctx *c) {
   return guarded(c, [&] { return impl_synchronize(c); });
 }
+
+#ifndef AIMS_BUILD_FLAGS
+#define AIMS_BUILD_FLAGS ""        // build.py sets it to the -D list of a probe build
+#endif
+const char *aims_gpu_build_flags(void) { return AIMS_BUILD_FLAGS; }
 
 int aims_gpu_dmma_probe(aims_gpu_ctx *c, int variant, int warps_per_sm, double *tflops) {
   return guarded(c, [&] { return impl_dmma_probe(c, variant, warps_per_sm, tflops); });

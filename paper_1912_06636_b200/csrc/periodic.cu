@@ -26,7 +26,8 @@ __global__ void __launch_bounds__(256) k_wrap_points(Inv3 M, long long n, double
 #pragma unroll
   for (int j = 0; j < 3; j++) {
     const double t = __dadd_rn(__dadd_rn(__dmul_rn(x, M.inv[j]), __dmul_rn(y, M.inv[3 + j])), __dmul_rn(z, M.inv[6 + j]));
-    f[j] = __dsub_rn(t, floor(t));
+    const double d = __dsub_rn(t, floor(t));
+    f[j] = d >= 1.0 ? 0.0 : d;              // t = -tiny: 1 - tiny rounds to 1.0, the excluded face; it is the f = 0 face of the next cell
   }
 #pragma unroll
   for (int j = 0; j < 3; j++)
@@ -69,6 +70,10 @@ int aims_gpu_periodic_images(const double *lattice, int32_t n_home, const double
     cross3(lattice + 3, lattice + 6, c12);
     vol = std::fabs(lattice[0] * c12[0] + lattice[1] * c12[1] + lattice[2] * c12[2]);
     if (!(vol > 0.0)) return AIMS_ERR_INVALID_ARG;
+    // the search box below (nmax) is sized for cell atoms inside the cell: unwrapped coordinates would silently lose images
+    for (int a = 0; a < n_home; a++)
+      for (int i = 0; i < 3; i++)
+        if (!(frac[3 * a + i] >= 0.0 && frac[3 * a + i] < 1.0)) return AIMS_ERR_INVALID_ARG;
     int nmax[3];
     for (int i = 0; i < 3; i++) {
       double w[3];

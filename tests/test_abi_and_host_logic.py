@@ -105,6 +105,18 @@ def test_slice_bundle_keeps_exactly_the_ranks_own_batches():
         assert s.D_values is bun.D_values and s.n_values == bun.n_values           # global objects are shared, not cut
         covered += s.n_points
     assert covered == bun.n_points
+    # per-point fields the slicer has never heard of are cut as well (by shape, not by name); global ones are not, even when a
+    # dimension coincides with the number of points
+    import copy
+    b2 = copy.copy(bun)
+    b2.xi = np.arange(bun.n_points, dtype=np.float64)                     # [n]
+    b2.hess = np.arange(6 * bun.n_points, dtype=np.float64).reshape(6, -1)  # [6][n]
+    b2.D_values = np.zeros(bun.n_points)                                  # global, size coincides
+    s, lo, hi = slice_bundle(b2, 1, nb - 1)
+    assert np.array_equal(s.xi, b2.xi[lo:hi]) and np.array_equal(s.hess, b2.hess[:, lo:hi]) and s.D_values is b2.D_values
+    per = aims_synth.make_periodic(n_rad=10, n_ang=14)
+    s, lo, hi = slice_bundle(per, 1, per.n_batches)
+    assert np.array_equal(s.xyz_unwrapped, per.xyz_unwrapped[lo:hi]) and s.atom_T is per.atom_T and s.frac is per.frac
 
 
 def test_partition_batches_is_a_contiguous_cover_and_balanced():
@@ -198,3 +210,34 @@ def test_two_rank_gloo_partial_sums_equal_single_rank(tmp_path):
     outs = [p.communicate(timeout=300)[0] for p in procs]
     assert all(p.returncode == 0 for p in procs), "\n".join(outs)
     assert "OK" in outs[0]
+
+
+def test_periodic_images_rejects_unwrapped_fractional_coordinates():
+    """aims_gpu_periodic_images runs on the host (no device needed).  Its enumeration box is sized for cell atoms inside the
+    cell, so fractional coordinates outside [0, 1) are refused instead of silently losing images (include/aims_gpu.h); the
+    same atom wrapped into the cell is accepted and gives the oracle's list."""
+    import numpy as np
+
+    import paper_1912_06636_b200 as aims
+    from oracle.periodic import periodic_images
+    lat = np.array([[4.0, 0.0, 0.0], [1.0, 5.0, 0.0], [0.0, 0.5, 6.0]])
+    for bad in ([1.0, 0.5, 0.5], [0.2, -1e-9, 0.5], [0.2, 0.5, 1.5], [np.nan, 0.5, 0.5]):
+        with pytest.raises(aims.AimsError):
+            aims.aims_gpu_periodic_images(lat, np.array([[0.1, 0.2, 0.3], bad]), 3.0)
+    frac = np.array([[0.1, 0.2, 0.3], [0.0, 0.999999, 0.5]])
+    home, n = aims.aims_gpu_periodic_images(lat, frac, 3.0)
+    home_ref, n_ref = periodic_images(lat, frac, 3.0)
+    assert np.array_equal(home, home_ref) and np.array_equal(n, n_ref)
+
+
+def test_product_library_reports_no_build_switches_and_ignores_the_environment(monkeypatch):
+    """The binding loads the product library only: AIMS_GPU_LIB (a round-2 override) no longer redirects it, the product build
+    reports "" from aims_gpu_build_flags(), and asking for another path once a library is loaded is an error, not a swap."""
+    import paper_1912_06636_b200 as aims
+    from paper_1912_06636_b200 import binding
+    monkeypatch.setenv("AIMS_GPU_LIB", "/nonexistent/libaims_gpu_probe.so")
+    L = aims.load_library()
+    assert L._aims_path == binding.LIB_PATH and L._aims_build_flags == ""
+    assert "AIMS_GPU_LIB" not in open(binding.__file__).read()
+    with pytest.raises(aims.AimsError):
+        aims.load_library("/nonexistent/libaims_gpu_probe.so", allow_probe=True)

@@ -30,3 +30,22 @@ def test_partition_weights_match_oracle(cfg, kw):
     with pytest.raises(aims.AimsError):
         ctx.partition_weights(bun.xyz[:5], bun.owner[:5], -1.0)
     ctx.close()
+
+
+def test_partition_weights_candidate_overflow_is_reported_by_the_call():
+    """More than 256 atoms within r_part of a point: the call itself returns AIMS_ERR_UNSUPPORTED (include/aims_gpu.h), and the
+    next call with a sane radius -- another cell list in the same context buffer -- is right again."""
+    import paper_1912_06636_b200 as aims
+    bun = aims_synth.make_config(5, n_rad=6, n_ang=14)
+    assert bun.n_atoms > 256
+    ctx = aims.aims_gpu_create(bun, device=0)
+    pts, own = bun.xyz[:200], bun.owner[:200]
+    with pytest.raises(aims.AimsError, match="more than 256 atoms"):
+        ctx.partition_weights(pts, own, 1.0e3)
+    ctx.synchronize()                                  # nothing left flagged for later
+    r_part = bun.meta["r_part"]
+    ref = Oracle(bun).partition_weights(pts, own, r_part)
+    for _ in range(2):                                 # second pass runs on the cached cell list
+        w = ctx.partition_weights(pts, own, r_part).cpu().numpy()
+        assert np.abs(w - ref).max() <= 1e-12
+    ctx.close()

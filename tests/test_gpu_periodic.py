@@ -83,6 +83,16 @@ def test_periodic_images_and_point_wrap_are_bit_exact(case):
         assert np.array_equal(home, home_ref) and np.array_equal(n, n_ref)
     w = aims.aims_gpu_wrap_points(bun.lattice, bun.xyz_unwrapped).cpu().numpy()
     assert np.array_equal(w, wrap_points(bun.lattice, bun.xyz_unwrapped))            # separately rounded operations: one result
+    # points a hair below a cell face, on faces and on lattice translates of the origin: f - floor(f) rounds to 1.0 for the first
+    # kind, and both sides put those on f = 0 (reading P23: [0, 1)); cubic cell, so the expected coordinates are exact
+    cube = 4.0 * np.eye(3)
+    edge_pts = np.array([[-1e-20, 1.0, 2.0], [1.0, -1e-20, -1e-20], [4.0, 8.0, -4.0], [-1.0, 5.0, 3.5], [-4.0 * 2.0 ** -60, 0.5, 0.5]])
+    we = aims.aims_gpu_wrap_points(cube, edge_pts).cpu().numpy()
+    assert np.array_equal(we, wrap_points(cube, edge_pts))
+    assert np.array_equal(we, np.array([[0.0, 1.0, 2.0], [1.0, 0.0, 0.0], [0.0, 0.0, 0.0], [3.0, 1.0, 3.5], [0.0, 0.5, 0.5]]))
+    hair = bun.xyz_unwrapped[:64] * 0.0 - 1e-18 * bun.lattice.sum(axis=0)              # a hair outside the corner of the real cell
+    wh = aims.aims_gpu_wrap_points(bun.lattice, hair).cpu().numpy()
+    assert np.array_equal(wh, wrap_points(bun.lattice, hair))
     # degenerate inputs
     assert aims.aims_gpu_wrap_points(bun.lattice, np.zeros((0, 3))).shape[0] == 0
     with pytest.raises(aims.AimsError):
