@@ -187,6 +187,8 @@ int aims_gpu_pulay_forces_ks(aims_gpu_ctx *ctx, int32_t b0, int32_t b1, const do
  *        { d_l phi_i [ sum_j n_ij (h_KS phi_j) - q_ij phi_j ]  +  (Hess phi_i g_p)_l sum_j n_ij phi_j }   (at r_p),
  * = (1/volume) d/d eps_lm [ Tr(n h(eps)) - Tr(q s(eps)) ], i.e. the force integrand weighted with the distance vector to the
  * function's own atom; (h_KS phi_j) = v phi_j + g.grad phi_j (- 1/2 lap phi_j if kinetic != 0) as in aims_gpu_pulay_forces_ks.
+ * For the kinetic part this is the PULAY term only (derivative of the basis-function factors); d/d eps_lm Tr(n t(eps)) has in
+ * addition sum_ij n_ij <phi_i| d_l d_m |phi_j> from the operator itself, which the caller adds with the other non-Pulay terms.
  * Point-attached fields do not co-rotate, so sigma need not be symmetric: all nine components are returned.
  * volume: the cell volume V (> 0; pass 1 for a cluster to obtain dE/d eps).  DEVICE pointers as in aims_gpu_pulay_forces_ks,
  * plus sigma [3][3]; F may be NULL (stress only).  accumulate == 0: F and sigma are zeroed first.  Accumulated with

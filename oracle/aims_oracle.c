@@ -1015,6 +1015,11 @@ void orc_partition_weights(const orc_system *S, int64_t n, const double *xyz, co
  * Pins (tests/test_oracle_stress_pins.py): central differences of the already pinned H and S on a strained copy of the
  * inputs; the term-by-term brute force below (no batches, no culling, both index orders written out); sum rule with the
  * forces for an s-only basis; invariance under translation of the whole system and under re-batching; linear in (n, q).
+ * kinetic != 0 (the -1/2 lap phi_j inside h_KS phi_j, as in O5/Eq. 16) is the PULAY part of the kinetic stress: the derivative
+ * of the basis-function factors only.  Its pins: orc_brute_stress_ks (radial-form Laplacian, both index orders), additivity
+ * sigma(v, kin) = sigma(v, off) + sigma(0, kin), and central differences of Tr(n t(eps)) of the pinned kinetic matrix, which
+ * equal sigma(0, kin) + sum_ij n_ij <phi_i| d_l d_m |phi_j> to grid accuracy (the commutator [t, x_m d_l] = -d_l d_m; that
+ * second term is the kinetic stress proper and, like the Hellmann-Feynman terms, not on this path).
  * ==================================================================================================================== */
 void orc_pulay_stress(const orc_system *S, int n_sel, const int32_t *batches, const double *v, const double *g,
                       const double *D_values, const double *Q_values, int kinetic, double volume, double *sigma) {
@@ -1147,6 +1152,75 @@ void orc_brute_stress(const orc_system *S, const double *v, const double *g, con
               t += nab * (dGa * phi[b] + Ga * dphi_b + dphi_a * Gb + phi[a] * dGb);
             }
             sigma[3 * l + m] += wp * t / volume;
+          }
+      }
+  }
+  free(at_of);
+  free(phi);
+  free(afp);
+}
+
+/* brute-force Pulay stress WITH the kinetic operator (tiny inputs only): orc_brute_stress plus the kinetic part of
+ * orc_pulay_stress written independently -- no batches, no culling, both index orders of the symmetrised product
+ * 1/2 (phi_a t phi_b + t phi_a phi_b) written out, and t phi taken in the RADIAL form
+ *   t (R(d) Y_lm) = -1/2 (R'' + 2 R'/d - l(l+1) R/d^2) Y_lm        (as orc_brute_kinetic does)
+ * instead of the trace of the Cartesian Hessian that orc_pulay_stress uses, so that the two pin each other.
+ * What is differentiated is the PULAY part ("the Pulay contribution to F_at and sigma_lm"): the strain derivative
+ * of the basis-function factor, d phi_a / d eps_lm = (d_l phi_a)(r - R_a)_m, with t phi_b held as the force expression of Eq. 16
+ * holds h_KS phi_j:
+ *   V sigma^kin_lm = sum_p w_p sum_ab n_ab [ (d phi_a / d eps_lm) (t phi_b) + (t phi_a) (d phi_b / d eps_lm) ] .
+ * The derivative of the operator's own factor, x_m d_l (t phi_b), is not a Pulay term; by [t, x_m d_l] = -d_l d_m it differs
+ * from the above by  sum_ab n_ab <phi_a| d_l d_m |phi_b>  (the kinetic stress proper), which tests/test_oracle_stress_pins.py
+ * adds when it compares with finite differences of Tr(n t(eps)). */
+void orc_brute_stress_ks(const orc_system *S, const double *v, const double *g, const double *Dd, const double *Qd, int kinetic,
+                         double volume, double *sigma) {
+  orc_brute_stress(S, v, g, Dd, Qd, volume, sigma);
+  if (!kinetic) return;
+  int64_t *afp = (int64_t *)malloc(sizeof(int64_t) * (S->n_atoms + 1));
+  orc_atom_fn_ptr(S, afp);
+  int nb = (int)afp[S->n_atoms];
+  double *phi = (double *)malloc(sizeof(double) * (size_t)nb * 5);
+  double *dph = phi + nb, *tph = phi + 4 * (size_t)nb;        /* dph[c*nb+i], tph[i] = (t phi_i)(r_p) */
+  int *at_of = (int *)malloc(sizeof(int) * (size_t)nb);
+  for (int64_t p = 0; p < S->n_points; p++) {
+    int i = 0;
+    for (int a = 0; a < S->n_atoms; a++) {
+      int sp = S->atom_species[a];
+      for (int s = S->species_shell_ptr[sp]; s < S->species_shell_ptr[sp + 1]; s++) {
+        int l = S->shell_l[s];
+        double val[7], gr[7][3], hh[7][6];
+        orc_shell_hess_at_point(S, a, s, S->xyz + 3 * p, val, gr, hh);     /* phi and grad phi (pinned by finite differences) */
+        double rc = S->shell_rcut[s], dv[3];
+        double d2 = dist2(S->xyz + 3 * p, S->atom_xyz + 3 * a, dv);
+        double Y[7];
+        double R = 0.0, dR = 0.0, d2R = 0.0, dd = 1.0;
+        int inside = d2 < rc * rc;
+        if (inside) {
+          double d = sqrt(d2);
+          double u[3] = {0.0, 0.0, 1.0};
+          if (d > 0.0) { u[0] = dv[0] / d; u[1] = dv[1] / d; u[2] = dv[2] / d; }
+          dd = d > S->r0 ? d : S->r0;
+          orc_radial2(S, S->shell_spline[s], d, &R, &dR, &d2R);
+          orc_solid_harmonics(l, u, Y, NULL);
+        }
+        for (int m = 0; m < 2 * l + 1; m++, i++) {
+          phi[i] = val[m]; at_of[i] = a;
+          for (int c = 0; c < 3; c++) dph[c * nb + i] = gr[m][c];
+          tph[i] = inside ? -0.5 * (d2R + 2.0 * dR / dd - (double)(l * (l + 1)) * R / (dd * dd)) * Y[m] : 0.0;
+        }
+      }
+    }
+    double wp = S->w[p];
+    for (int a = 0; a < nb; a++)
+      for (int b = 0; b < nb; b++) {
+        double nab = Dd[(size_t)a * nb + b];
+        if (nab == 0.0) continue;
+        const double *Ra = S->atom_xyz + 3 * at_of[a], *Rb = S->atom_xyz + 3 * at_of[b];
+        for (int l = 0; l < 3; l++)
+          for (int m = 0; m < 3; m++) {
+            double dphi_a = dph[l * nb + a] * (S->xyz[3 * p + m] - Ra[m]);     /* d phi_a / d eps_lm */
+            double dphi_b = dph[l * nb + b] * (S->xyz[3 * p + m] - Rb[m]);
+            sigma[3 * l + m] += wp * nab * (dphi_a * tph[b] + tph[a] * dphi_b) / volume;
           }
       }
   }

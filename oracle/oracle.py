@@ -63,6 +63,7 @@ def _load():
         L.orc_brute_forces.argtypes = [sp, _dp, _dp, _dp, _dp, ctypes.c_int, _dp]
         L.orc_pulay_stress.argtypes = [sp, ctypes.c_int, _ip, _dp, _dp, _dp, _dp, ctypes.c_int, ctypes.c_double, _dp]
         L.orc_brute_stress.argtypes = [sp, _dp, _dp, _dp, _dp, ctypes.c_double, _dp]
+        L.orc_brute_stress_ks.argtypes = [sp, _dp, _dp, _dp, _dp, ctypes.c_int, ctypes.c_double, _dp]
         L.orc_integrate_hamiltonian_ks.argtypes = [sp, ctypes.c_int, _ip, _dp, _dp, ctypes.c_int, _dp]
         L.orc_brute_kinetic.argtypes = [sp, _dp, _dp]
         L.orc_density_hessian.argtypes = [sp, ctypes.c_int, _ip, _dp, _dp]
@@ -309,11 +310,14 @@ class Oracle:
                                 float(volume), _d(sig))
         return sig
 
-    def brute_stress(self, v, D_dense, g=None, Q_dense=None, volume=1.0):
+    def brute_stress(self, v, D_dense, g=None, Q_dense=None, volume=1.0, kinetic=False):
         v = np.ascontiguousarray(v, dtype=np.float64)
         g = None if g is None else np.ascontiguousarray(g, dtype=np.float64)
         Dd = np.ascontiguousarray(D_dense, dtype=np.float64)
         Qd = None if Q_dense is None else np.ascontiguousarray(Q_dense, dtype=np.float64)
         sig = np.zeros((3, 3))
-        self.L.orc_brute_stress(ctypes.byref(self.sys), _d(v), _d(g), _d(Dd), _d(Qd), float(volume), _d(sig))
+        if kinetic:
+            self.L.orc_brute_stress_ks(ctypes.byref(self.sys), _d(v), _d(g), _d(Dd), _d(Qd), 1, float(volume), _d(sig))
+        else:
+            self.L.orc_brute_stress(ctypes.byref(self.sys), _d(v), _d(g), _d(Dd), _d(Qd), float(volume), _d(sig))
         return sig

@@ -6,7 +6,11 @@ fixed by mathematics -- never against the CUDA path:
   * batched-and-culled == the term-by-term brute force (every strained factor differentiated separately);
   * for a uniform translation of the whole system nothing changes; for an s-only basis without the GGA term sigma is
     symmetric (the integrand is d_l d_m R'(d)/d); the trace of V sigma equals the derivative under isotropic scaling;
-  * linear in (D, Q), 1/V scaling, invariant under re-batching.
+  * linear in (D, Q), 1/V scaling, invariant under re-batching;
+  * kinetic != 0 (the Pulay part of the kinetic stress): batched-and-culled with the Hessian-trace Laplacian == brute force with the
+    radial-form Laplacian and both index orders; additive in (v, kinetic); and, through the commutator [t, x_m d_l] = -d_l d_m,
+    sigma(0, kin) + sum_ij n_ij <phi_i| d_l d_m |phi_j> == central differences of Tr(n t(eps)) of the pinned kinetic matrix, to
+    grid accuracy (the bar tests/test_oracle_kinetic_pins.py uses for the kinetic forces).
 """
 import copy
 
@@ -120,3 +124,61 @@ def test_stress_invariant_under_rebatching():
     sa = Oracle(a).pulay_stress(a.v, a.D_values, g=a.g, Q_values=make_q_values(a))
     sc = Oracle(c).pulay_stress(c.v, c.D_values, g=c.g, Q_values=make_q_values(c))
     assert np.abs(sa - sc).max() <= 1e-12 * np.abs(sa).max()
+
+
+# --------------------------------------------------------------------------- kinetic branch (h_KS phi_j carries -1/2 lap phi_j)
+@pytest.mark.parametrize("use_g", [False, True])
+def test_kinetic_stress_batched_equals_brute_force_and_is_additive(toy5, cfg1, use_g):
+    for b in (cfg1, toy5[0]):
+        o = Oracle(b)
+        Qv = make_q_values(b)
+        g = b.g if use_g else None
+        Dd, Qd = bsr_to_dense(b, b.D_values), bsr_to_dense(b, Qv)
+        sig = o.pulay_stress(b.v, b.D_values, g=g, Q_values=Qv, kinetic=True, volume=3.5)
+        sb = o.brute_stress(b.v, Dd, g=g, Q_dense=Qd, kinetic=True, volume=3.5)      # radial-form Laplacian, no batches, no culling
+        assert np.abs(sig - sb).max() <= 1e-12 * np.abs(sb).max()
+        s_off = o.pulay_stress(b.v, b.D_values, g=g, Q_values=Qv, kinetic=False, volume=3.5)
+        s_kin = o.pulay_stress(np.zeros(b.n_points), b.D_values, kinetic=True, volume=3.5)
+        assert np.abs(s_kin).max() > 1e-3 * np.abs(sig).max()                         # the branch contributes
+        assert np.abs(sig - (s_off + s_kin)).max() <= 1e-12 * np.abs(sig).max()       # and is additive
+        sk_b = o.brute_stress(np.zeros(b.n_points), Dd, kinetic=True, volume=3.5)
+        assert np.abs(s_kin - sk_b).max() <= 1e-12 * np.abs(sk_b).max()
+
+
+def test_kinetic_stress_plus_commutator_term_is_the_strain_derivative_of_the_kinetic_energy():
+    """E(eps) = Tr(n t(eps)) on the strained grid = sum_p w_p sum_ij n_ij phi_i (t phi_j).  Its derivative has the Pulay part the
+    oracle returns, 2 sum w n_ij (d_l phi_i)(r - R_i)_m (t phi_j), and the derivative of the factor t phi_j, which by Hermiticity of
+    t and [t, x_m d_l] = -d_l d_m equals the Pulay part again plus C_lm = sum_ij n_ij <phi_i| d_l d_m |phi_j>.  C is evaluated here
+    from the oracle's finite-difference-pinned Hessian of the density: phi_i d_l d_m phi_j summed with n_ij is
+    hess_n[lm] / 2 - sum_ij n_ij d_l phi_i d_m phi_j.  Hermiticity holds on the grid to quadrature accuracy only, hence the loose
+    bar -- but a wrong sign or factor in the kinetic branch is an error of the order of the scale itself."""
+    b = aims_synth.make_config(1, n_rad=60, n_ang=302)
+    o = Oracle(b)
+    zero = np.zeros(b.n_points)
+    Dd = bsr_to_dense(b, b.D_values)
+    P = o.pulay_stress(zero, b.D_values, kinetic=True)
+    hess = o.density_hessian(b.D_values)                                   # [6][n]: xx, yy, zz, xy, xz, yz
+    hx = [[0, 3, 4], [3, 1, 5], [4, 5, 2]]
+    C = np.zeros((3, 3))
+    for bi in range(b.n_batches):
+        idx, phi, dphi = o.eval_basis(bi, want_grad=True)
+        sl = slice(b.batch_ptr[bi], b.batch_ptr[bi + 1])
+        Db = Dd[np.ix_(idx, idx)]
+        for l in range(3):
+            for m in range(3):
+                gg = np.einsum("ip,ij,jp->p", dphi[l], Db, dphi[m])
+                C[l, m] += (b.w[sl] * (0.5 * hess[hx[l][m]][sl] - gg)).sum()
+
+    def energy(eps):
+        b2 = _strained(b, eps)
+        return float((Dd * bsr_to_dense(b2, Oracle(b2).integrate_hamiltonian_ks(zero, kinetic=True))).sum())
+
+    h = 2e-4
+    scale = np.abs(P).max()
+    assert np.abs(C).max() > 0.3 * scale                                   # the commutator term is not a detail
+    for (l, m) in [(0, 0), (1, 1), (0, 1), (1, 0), (2, 1)]:
+        e = np.zeros((3, 3))
+        e[l, m] = h
+        fd = (energy(e) - energy(-e)) / (2 * h)
+        assert abs(fd - (P[l, m] + C[l, m])) <= 2e-2 * scale, (l, m, fd, P[l, m], C[l, m])
+        assert abs(fd - (-P[l, m] + C[l, m])) > 2e-2 * scale or abs(P[l, m]) < 2e-2 * scale     # a sign slip would be seen
