@@ -176,7 +176,7 @@ def test_full_size_properties_of_whole_grid_outputs(full):
 
 
 def test_full_size_widened_rows_on_sampled_batches(full):
-    """Kinetic term + tau matrix, Pulay forces and the density Hessian at full size: sampled batches against the oracle
+    """Kinetic term + tau matrix, Pulay forces, Pulay stress and the density Hessian at full size: sampled batches against the oracle
     (through [b, b+1) for the sums H and F, whole-grid call for the per-point Hessian).  Config 5 and config 3 only, and a
     subset of the sample, to bound the oracle's time."""
     import torch
@@ -190,16 +190,47 @@ def test_full_size_widened_rows_on_sampled_batches(full):
     Q = make_q_values(bun)
     H = torch.zeros(bun.n_values, dtype=torch.float64, device="cuda")
     F = torch.zeros((bun.n_atoms, 3), dtype=torch.float64, device="cuda")
+    sig = torch.zeros((3, 3), dtype=torch.float64, device="cuda")
+    F2 = torch.zeros((bun.n_atoms, 3), dtype=torch.float64, device="cuda")
     for b in sub:
         ctx.integrate_hamiltonian(vd, gd, H=H, b0=int(b), b1=int(b) + 1, accumulate=True, kinetic=True)
         ctx.add_tau_matrix(xi, H=H, b0=int(b), b1=int(b) + 1)
         ctx.pulay_forces(vd, bun.D_values, g=gd, Q=Q, F=F, b0=int(b), b1=int(b) + 1, accumulate=True, kinetic=True)
+        # forces and stress in one pass (aims_gpu_pulay_forces_stress, kinetic branch included)
+        ctx.pulay_forces_stress(vd, bun.D_values, g=gd, Q=Q, volume=2.5, F=F2, sigma=sig, b0=int(b), b1=int(b) + 1, accumulate=True,
+                                kinetic=True)
     Hn = ctx.density_hessian(bun.D_values)                          # whole grid, as bench.py --path hessian launches it
     ctx.synchronize()
     ref = orc.tau_matrix(xi, batches=sub, H_values=orc.integrate_hamiltonian_ks(bun.v, bun.g, kinetic=True, batches=sub))
     assert _rel_fro(H.cpu().numpy(), ref) <= TOL_H
     F_ref = orc.pulay_forces(bun.v, bun.D_values, g=bun.g, Q_values=Q, batches=sub, kinetic=True)
     assert _rel_max(F.cpu().numpy(), F_ref) <= TOL_N
+    sig_ref = orc.pulay_stress(bun.v, bun.D_values, g=bun.g, Q_values=Q, batches=sub, kinetic=True, volume=2.5)
+    assert _rel_max(sig.cpu().numpy(), sig_ref) <= TOL_N
+    assert _rel_max(F2.cpu().numpy(), F_ref) <= TOL_N
     Hn_ref = orc.density_hessian(bun.D_values, batches=sub[:3])
     idx = np.concatenate([np.arange(bun.batch_ptr[b], bun.batch_ptr[b + 1]) for b in sub[:3]])
     assert _rel_max(Hn.cpu().numpy()[:, idx], Hn_ref[:, idx]) <= TOL_N
+
+
+def test_full_size_hamiltonian_contiguous_range_around_the_heaviest_batch(full):
+    """H in the launch shape bench.py times, against the oracle element by element: ONE call over a contiguous range of 320
+    batches that contains the max-nnz batch -- a multi-tile launch in heaviest-first order in which neighbouring batches add into
+    the same atom-pair blocks -- compared with the oracle on the same list (Eq. 23-24: h = sum over batches).
+    Config 5 (the benchmark: two species, l = 3, nnz up to 1,779) and one config-4 sweep size; the oracle needs about 64,000 points."""
+    import torch
+    name, bun, orc, ctx, gga, sel = full
+    if name not in ("cfg5_full_gga", "cfg4_full_b200"):
+        pytest.skip("contiguous-range H parity runs on config 5 and on config 4 at 200 points per batch")
+    nnz = ctx.batch_nnz()
+    span = 320
+    b0 = int(min(max(int(np.argmax(nnz)) - span // 2, 0), bun.n_batches - span))
+    b1 = b0 + span
+    vd, gd = torch.as_tensor(bun.v).cuda(), torch.as_tensor(bun.g).cuda()
+    H = ctx.integrate_hamiltonian(vd, gd, b0=b0, b1=b1)
+    ctx.synchronize()
+    H = H.cpu().numpy()
+    ref = orc.integrate_hamiltonian(bun.v, bun.g, batches=np.arange(b0, b1, dtype=np.int32))
+    assert np.linalg.norm(ref) > 0
+    assert _rel_fro(H, ref) <= TOL_H
+    assert not H[bsr_pad_mask(bun)].any()
