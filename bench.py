@@ -9,7 +9,9 @@ aims_gpu_update_density (with grad n), each including its own culling and basis 
 --path forces times the widened row f1 instead: one step = one aims_gpu_pulay_forces (GGA term and the
 energy-weighted density matrix) over the whole grid; it is a separate line, not the headline metric.
 
-N > 1 (torchrun): contiguous batch ranges balanced by n_p*nnz^2 are sharded over the ranks; each rank adds its
+N > 1: under torchrun (the driver's form) the ranks come from the launcher; a bare `python bench.py --gpus N` starts the N ranks
+itself through torch.distributed.run on 127.0.0.1 and refuses if fewer than N devices are visible (--launch-dry-run checks that
+launch without GPUs).  Contiguous batch ranges balanced by n_p*nnz^2 are sharded over the ranks; each rank adds its
 partial H (Eq. 28) and the partial sums are combined by ONE NCCL all-reduce (Eq. 29, "the only communication
 step"); the density needs none (L312).  Total work is fixed -> "scaling": "strong".
 
@@ -68,6 +70,9 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--workspace-gib", type=float, default=0.0, help="Phi-plane workspace of the context (0 = library default, 24 GiB)")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--launch-dry-run", action="store_true",
+                    help="start the ranks exactly as a real run would, have each print its RANK / LOCAL_RANK / WORLD_SIZE and exit "
+                         "(no CUDA, no workload): the launch path can be checked on a machine without GPUs")
     ap.add_argument("--lib", default=None, help="measure with a probe build of the library (build.py --define ... --tag ...); its "
                     "switches are recorded in the JSON line under build_flags, and such a line is not a bench value")
     ap.add_argument("--path", default="scf", choices=["scf", "forces", "stress", "hessian", "setup"])
@@ -288,11 +293,38 @@ def run_reference(args, bun, gga, workload, metric, forces_q=None, hessian=False
     print(json.dumps(out))
 
 
+def self_launch(args):
+    """`python bench.py --gpus N` with N > 1 outside torchrun: start the N ranks here, one per GPU of this node, through the same
+    launcher the driver uses (torch.distributed.run, rendezvous on 127.0.0.1), and return its exit code.  Rank 0 of the children
+    prints the one JSON line.  Refuses when fewer than N devices are visible -- it never falls back to fewer ranks."""
+    import socket
+    import subprocess
+    if not args.launch_dry_run:
+        import torch
+        have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+        if have < args.gpus:
+            raise SystemExit("bench.py: --gpus %d but %d CUDA device(s) visible; refusing to run fewer ranks than asked for" % (args.gpus, have))
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus), "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
 def main():
     args = parse()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and (args.impl != "reference" or args.launch_dry_run):
+        return self_launch(args)
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != max(args.gpus, 1):
+        raise SystemExit("bench.py: --gpus %d but the launcher started WORLD_SIZE=%d ranks" % (args.gpus, world))
+    if args.launch_dry_run:
+        print(json.dumps({"launch_dry_run": True, "rank": rank, "local_rank": local_rank, "world_size": world, "pid": os.getpid(),
+                          "master": "%s:%s" % (os.environ.get("MASTER_ADDR"), os.environ.get("MASTER_PORT"))}), flush=True)
+        return 0
     gga = args.config != 2
     workload = WORKLOADS[args.config]
     if args.max_batch:
@@ -329,6 +361,8 @@ def main():
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
     build_flags = aims.load_library(args.lib, allow_probe=args.lib is not None)._aims_build_flags
+    if torch.cuda.device_count() <= local_rank:
+        raise SystemExit("bench.py: rank %d wants cuda:%d but %d device(s) are visible" % (rank, local_rank, torch.cuda.device_count()))
     torch.cuda.set_device(local_rank)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))

@@ -241,3 +241,33 @@ def test_product_library_reports_no_build_switches_and_ignores_the_environment(m
     assert "AIMS_GPU_LIB" not in open(binding.__file__).read()
     with pytest.raises(aims.AimsError):
         aims.load_library("/nonexistent/libaims_gpu_probe.so", allow_probe=True)
+
+
+def test_bench_gpus_2_starts_two_ranks_with_distinct_local_ranks():
+    """`python bench.py --gpus N` (the form the driver uses at N = 1) must be a real N-rank run for N > 1: outside torchrun it
+    starts the ranks itself through torch.distributed.run on 127.0.0.1.  --launch-dry-run goes through exactly that launch and has
+    every rank report who it is instead of touching CUDA, so the path is checked here without GPUs.  A launcher that started a
+    different number of ranks than --gpus says is refused, and without enough devices a real run refuses instead of shrinking."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--launch-dry-run"], env=env, cwd=root,
+                         capture_output=True, text=True, timeout=300)
+    assert out.returncode == 0, out.stderr[-2000:]
+    ranks = [json.loads(line) for line in out.stdout.splitlines() if line.startswith("{")]
+    assert len(ranks) == 2 and all(r["launch_dry_run"] and r["world_size"] == 2 for r in ranks)
+    assert sorted(r["local_rank"] for r in ranks) == [0, 1] and sorted(r["rank"] for r in ranks) == [0, 1]
+    assert len({r["pid"] for r in ranks}) == 2 and len({r["master"] for r in ranks}) == 1 and ranks[0]["master"].startswith("127.0.0.1:")
+    # WORLD_SIZE from a launcher that disagrees with --gpus
+    bad = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--launch-dry-run"],
+                         env=dict(env, WORLD_SIZE="1", RANK="0", LOCAL_RANK="0"), cwd=root, capture_output=True, text=True, timeout=300)
+    assert bad.returncode != 0 and "WORLD_SIZE=1" in bad.stderr
+    # a real 2-GPU run on a machine with fewer than two devices refuses loudly (this container has none)
+    import torch
+    if torch.cuda.device_count() < 2:
+        real = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--steps", "1"], env=env, cwd=root,
+                              capture_output=True, text=True, timeout=300)
+        assert real.returncode != 0 and "refusing" in real.stderr
