@@ -191,22 +191,22 @@ def kernel_sources_sha():
 
 
 def committed_traffic(kernel, workload_key):
-    """DRAM bytes per launch of `kernel` from the committed `ncu --set full` summary (profiles/r02_traffic.txt, one JSON
+    """DRAM bytes per launch of `kernel` from the committed `ncu --set full` summary (profiles/r03_traffic.txt, one JSON
     object), or (None, why) when the capture was taken from other kernel sources than the ones this run loaded."""
-    path = os.path.join(ROOT, "profiles", "r02_traffic.txt")
+    path = os.path.join(ROOT, "profiles", "r03_traffic.txt")
     try:
         with open(path) as f:
             rec = json.load(f)
     except Exception:
-        return None, "no committed ncu capture (profiles/r02_traffic.txt)"
+        return None, "no committed ncu capture (profiles/r03_traffic.txt)"
     if rec.get("kernel_sources_sha") != kernel_sources_sha():
         return None, "committed ncu capture was taken at kernel sources %s, this run has %s" % (
             rec.get("kernel_sources_sha"), kernel_sources_sha())
     val = rec.get("traffic", {}).get(workload_key, {}).get(kernel)
     if val is None:
-        return None, "no capture of %s for %s in profiles/r02_traffic.txt" % (kernel, workload_key)
+        return None, "no capture of %s for %s in profiles/r03_traffic.txt" % (kernel, workload_key)
     return float(val), "dram__bytes_read.sum + dram__bytes_write.sum of one launch, %s (commit %s)" % (
-        rec.get("source", "profiles/r02_traffic.txt"), rec.get("commit"))
+        rec.get("source", "profiles/r03_traffic.txt"), rec.get("commit"))
 
 
 def run_setup_path(args, aims, torch, ctx, bun, stream, workload, n_points_total, world, rank):

@@ -59,7 +59,9 @@ def load_library(path=None, allow_probe=False):
     global _lib
     want = os.path.abspath(path) if path else LIB_PATH
     if _lib is not None:
-        if want != _lib._aims_path:
+        # one library per process: whoever loads first decides (bench.py --lib does it before anything else); a later call
+        # without a path gets that library, a later call that names ANOTHER file is an error, never a silent swap
+        if path and want != _lib._aims_path:
             raise AimsError("a different library is already loaded: %s" % _lib._aims_path)
         return _lib
     if not os.path.exists(want):

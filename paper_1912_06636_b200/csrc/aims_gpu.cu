@@ -13,12 +13,21 @@
 #include <string>
 #include <vector>
 
+#if defined(AIMS_PROBE_DENSITY2) || defined(AIMS_PROBE_BALANCED_DENSITY)
+#define AIMS_WITH_VARIANTS 1        // see the note at density2.cuh below; defined before basis.cuh, whose k_cull serves the variants too
+#endif
 #include "basis.cuh"
 #include "bloch.cuh"
 #include "common.cuh"
 #include "density.cuh"
+// The product library contains the product only.  The two measured-and-rejected density variants (density2.cuh, density_b.cuh;
+// profiles/r02_kernel_experiments.md), every table, context field and launch branch that serves them, and the DMMA
+// operand-pattern probes are compiled ONLY into probe builds (build.py --define AIMS_PROBE_DENSITY2=1 / AIMS_PROBE_BALANCED_DENSITY=1 /
+// AIMS_PROBE_DMMA=1 --tag ...), which report their switches through aims_gpu_build_flags().
+#ifdef AIMS_WITH_VARIANTS
 #include "density2.cuh"
 #include "density_b.cuh"
+#endif
 #include "forces.cuh"
 #include "hessian.cuh"
 #include "partition.cuh"
@@ -57,9 +66,11 @@ struct aims_gpu_ctx {
   HTile *d_tiles = nullptr;
   DItem *d_items = nullptr;
   double flops_h_lda = 0, flops_h_gga = 0, flops_den = 0;
-  bool ptab_in_smem = true, f_ptab_in_smem = true, x_ptab_in_smem = true, b_ptab_in_smem = true;
+  bool ptab_in_smem = true, f_ptab_in_smem = true, x_ptab_in_smem = true;
   std::vector<DItem> h_items;                                  // host copy of the density work items
   std::map<std::pair<int, int>, int *> item_order;             // (bs, be) -> device permutation, heaviest item first
+#ifdef AIMS_WITH_VARIANTS
+  bool b_ptab_in_smem = true;
   // density_b.cuh: items of 192..224 points (update_density only; forces / Hessian keep every item in `items`)
   bool balanced_density = true;
   std::vector<long long> itemb_off, itemg_off;                 // per batch: balanced items / the other ("generic") items
@@ -79,6 +90,7 @@ struct aims_gpu_ctx {
   int *d_blk_row = nullptr;
   long long full_doubles = 0, n_blocks = 0;
   double *Dfull = nullptr;                                     // full-storage copy of the density matrix (per call)
+#endif
 
   // aims_gpu_bloch_fold: contribution lists per (cell atom, cell atom) tile, cached for the last atom_home seen
   std::vector<int> bloch_home;
@@ -177,6 +189,7 @@ __global__ void k_fp64_peak(double *out, int iters, double a, double b) {
   if (s == 12345.678) out[0] = s;
 }
 
+#ifdef AIMS_PROBE_DMMA
 // DMMA operand-pattern probe (aims_gpu_dmma_probe): one warp works on a 32x32 accumulator block, 16 DMMAs per step.
 //   V = 1: operands stay in registers (4x4 outer product);  V = 2: the 8 fragments of a step are loaded from shared memory,
 //   then its 16 DMMAs are issued ("load-then-compute");  V = 3: the loads of step t+1 are issued before the DMMAs of step t.
@@ -377,6 +390,8 @@ __global__ void __launch_bounds__(640) k_dmma_probe3(double *out, const int *cnt
   if (s == 12345.678) out[0] = s;
 }
 
+#endif  // AIMS_PROBE_DMMA
+
 bool range_ok(const aims_gpu_ctx *c, int b0, int b1) { return c && b0 >= 0 && b1 >= b0 && b1 <= c->n_batches; }
 
 // Every extern "C" entry runs its body through this: no C++ exception (std::bad_alloc of the host-side tables and
@@ -415,8 +430,11 @@ cudaError_t smem_optin_all(int device, size_t optin) {
 #define AIMS_OPTIN(k) if ((e = smem_optin_max(k, optin)) != cudaSuccess) return e;
   AIMS_OPTIN(k_hamiltonian<false>) AIMS_OPTIN(k_hamiltonian<true>)
   AIMS_OPTIN(k_density<false>) AIMS_OPTIN(k_density<true>)
+#ifdef AIMS_WITH_VARIANTS
   AIMS_OPTIN(k_density2<false>) AIMS_OPTIN(k_density2<true>)
   AIMS_OPTIN(k_density_b<false>) AIMS_OPTIN(k_density_b<true>)
+  AIMS_OPTIN((k_eval<kEvalPhi, kLayD2>)) AIMS_OPTIN((k_eval<kEvalPhiGrad, kLayD2>))
+#endif
   AIMS_OPTIN(k_density_hessian)
   AIMS_OPTIN((k_forces<false, false>)) AIMS_OPTIN((k_forces<true, false>))
   AIMS_OPTIN((k_forces<false, true>)) AIMS_OPTIN((k_forces<true, true>))
@@ -425,7 +443,6 @@ cudaError_t smem_optin_all(int device, size_t optin) {
   AIMS_OPTIN_EV(kEvalHGga, kLayH) AIMS_OPTIN_EV(kEvalHKinLda, kLayH) AIMS_OPTIN_EV(kEvalHKinGga, kLayH)
   AIMS_OPTIN_EV(kEvalTau, kLayH) AIMS_OPTIN_EV(kEvalHess, kLayD) AIMS_OPTIN_EV(kEvalPhi, kLayD)
   AIMS_OPTIN_EV(kEvalPhiGrad, kLayD) AIMS_OPTIN_EV(kEvalForceLda, kLayD) AIMS_OPTIN_EV(kEvalForceGga, kLayD)
-  AIMS_OPTIN_EV(kEvalPhi, kLayD2) AIMS_OPTIN_EV(kEvalPhiGrad, kLayD2)
 #undef AIMS_OPTIN_EV
 #undef AIMS_OPTIN
   if (device >= 0 && device < 64) done[device] = true;
@@ -567,19 +584,24 @@ static int impl_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_
   BatchLists &L = c->L;
   if ((rc = dev_alloc(c, &L.nnz, nb))) return rc;
   if ((rc = dev_alloc(c, &L.n_act, nb))) return rc;
+#ifdef AIMS_WITH_VARIANTS
   if ((rc = dev_alloc(c, &L.kq, nb))) return rc;
   if ((rc = dev_alloc(c, &L.nfull, nb))) return rc;
+#endif
   if ((rc = dev_alloc(c, &L.error_flag, 1))) return rc;
   CU_TRY(c, cudaMemsetAsync(L.error_flag, 0, sizeof(int), c->stream));
   if (nb) {
     { TimedLaunch t(c, kKindCull); k_cull<<<nb, 256, 0, c->stream>>>(S, L, 0, 1); }
     if ((rc = check_async(c))) return rc;
   }
-  c->nnz.resize(nb); c->n_act.resize(nb); c->kq.resize(nb);
-  std::vector<int> nfull(nb);
+  c->nnz.resize(nb); c->n_act.resize(nb);
   int flag = 0;
+#ifdef AIMS_WITH_VARIANTS
+  c->kq.resize(nb);
+  std::vector<int> nfull(nb);
   CU_TRY(c, cudaMemcpyAsync(c->kq.data(), L.kq, nb * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
   CU_TRY(c, cudaMemcpyAsync(nfull.data(), L.nfull, nb * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+#endif
   CU_TRY(c, cudaMemcpyAsync(c->nnz.data(), L.nnz, nb * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
   CU_TRY(c, cudaMemcpyAsync(c->n_act.data(), L.n_act, nb * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
   CU_TRY(c, cudaMemcpyAsync(&flag, L.error_flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
@@ -590,7 +612,9 @@ static int impl_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_
   c->fn_off.assign(nb + 1, 0); c->act_off.assign(nb + 1, 0); c->ptab_off.assign(nb + 1, 0);
   c->pad_off.assign(nb + 1, 0); c->pad16_off.assign(nb + 1, 0); c->dpad_off.assign(nb + 1, 0); c->api_off.assign(nb + 1, 0); c->tile_off.assign(nb + 1, 0); c->item_off.assign(nb + 1, 0);
   std::vector<HTile> tiles;
-  std::vector<DItem> items, items2, itemsb, itemsg;
+  std::vector<DItem> items;
+#ifdef AIMS_WITH_VARIANTS
+  std::vector<DItem> items2, itemsb, itemsg;
   c->dq_off.assign(nb + 1, 0); c->item2_off.assign(nb + 1, 0);
   c->itemb_off.assign(nb + 1, 0); c->itemg_off.assign(nb + 1, 0);
 #ifndef AIMS_PROBE_BALANCED_DENSITY
@@ -601,7 +625,9 @@ static int impl_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_
 #else
   c->fast_density = false;
 #endif
+#endif  // AIMS_WITH_VARIANTS
   for (int b = 0; b < nb; b++) {
+#ifdef AIMS_WITH_VARIANTS
     if (nfull[b] != c->nnz[b]) c->fast_density = false;          // an atom lost some of its shells: density.cuh handles that
     c->max_kq = std::max(c->max_kq, c->kq[b]);
     {
@@ -616,6 +642,7 @@ static int impl_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_
       }
       c->item2_off[b + 1] = (long long)items2.size();
     }
+#endif
     const int nz = c->nnz[b], nact = c->n_act[b];
     const int np = (int)(c->batch_ptr[b + 1] - c->batch_ptr[b]);
     const int nz8 = pad8(nz), np8 = pad8(np);
@@ -655,11 +682,13 @@ static int impl_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_
         }
       }
     }
+#ifdef AIMS_WITH_VARIANTS
     for (size_t q = (size_t)c->item_off[b]; q < items.size(); q++)
       (c->balanced_density && b_item_ok(items[q].npt) ? itemsb : itemsg).push_back(items[q]);
-    c->item_off[b + 1] = (long long)items.size();
     c->itemb_off[b + 1] = (long long)itemsb.size();
     c->itemg_off[b + 1] = (long long)itemsg.size();
+#endif
+    c->item_off[b + 1] = (long long)items.size();
     c->flops_h_lda += (double)np * nz * (nz + 1.0);
     c->flops_h_gga += 2.0 * np * (double)nz * nz;
     c->flops_den += 2.0 * np * (double)nz * nz;
@@ -675,6 +704,7 @@ static int impl_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_
   if ((rc = dev_upload<HTile>(c, &c->d_tiles, tiles.data(), tiles.size()))) return rc;
   if ((rc = dev_upload<DItem>(c, &c->d_items, items.data(), items.size()))) return rc;
   c->h_items = items;
+#ifdef AIMS_WITH_VARIANTS
   if ((rc = dev_upload<DItem>(c, &c->d_itemsb, itemsb.data(), itemsb.size()))) return rc;
   if ((rc = dev_upload<DItem>(c, &c->d_itemsg, itemsg.data(), itemsg.size()))) return rc;
   c->h_itemsb = itemsb; c->h_itemsg = itemsg;
@@ -700,6 +730,7 @@ static int impl_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_
     if ((rc = dev_upload<int>(c, &c->d_blk_row, blk_row.data(), blk_row.size()))) return rc;
     CU_TRY(c, cudaStreamSynchronize(c->stream));
   }
+#endif
   CU_TRY(c, cudaStreamSynchronize(c->stream));
   if ((rc = dev_alloc(c, &L.fn_index, (size_t)c->fn_off[nb]))) return rc;
   if ((rc = dev_alloc(c, &L.fn_info, (size_t)c->fn_off[nb]))) return rc;
@@ -708,7 +739,9 @@ static int impl_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_
   if ((rc = dev_alloc(c, &L.act_row0, (size_t)c->act_off[nb]))) return rc;
   if ((rc = dev_alloc(c, &L.act_ld, (size_t)c->act_off[nb]))) return rc;
   if ((rc = dev_alloc(c, &L.ptab, (size_t)c->ptab_off[nb]))) return rc;
+#ifdef AIMS_WITH_VARIANTS
   if ((rc = dev_alloc(c, &L.pblk, (size_t)c->ptab_off[nb]))) return rc;
+#endif
 
   // ---- Phi-plane workspace: at least the largest single batch in EVERY plane layout used by a call (10 planes of the
   // density layout for the Hessian, 6 x the 16-point-padded H layout for the tau matrix), at most the requested budget
@@ -719,8 +752,12 @@ static int impl_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_
   long long need_min = 0;
   for (int b = 0; b < nb; b++)
     need_min = std::max({need_min, 10 * (c->dpad_off[b + 1] - c->dpad_off[b]), 6 * (c->pad16_off[b + 1] - c->pad16_off[b]),
-                         2 * (c->pad_off[b + 1] - c->pad_off[b]), 4 * (c->dq_off[b + 1] - c->dq_off[b])});
-  const long long need_all = std::max({10 * c->dpad_off[nb], 6 * c->pad16_off[nb], 2 * c->pad_off[nb], 4 * c->dq_off[nb]});
+                         2 * (c->pad_off[b + 1] - c->pad_off[b])});
+  long long need_all = std::max({10 * c->dpad_off[nb], 6 * c->pad16_off[nb], 2 * c->pad_off[nb]});
+#ifdef AIMS_WITH_VARIANTS
+  for (int b = 0; b < nb; b++) need_min = std::max(need_min, 4 * (c->dq_off[b + 1] - c->dq_off[b]));
+  need_all = std::max(need_all, 4 * c->dq_off[nb]);
+#endif
   long long wsd = std::min(need_all, std::max(want / 8, need_min)) + 10 * 64;
   if (wsd * 8 > (long long)free_b) return fail(c, AIMS_ERR_NOMEM, "not enough device memory for one batch of Phi planes");
   if ((rc = dev_alloc(c, &c->ws, (size_t)wsd))) return rc;
@@ -736,19 +773,23 @@ static int impl_create(aims_gpu_ctx **out, const aims_basis_desc *B, const aims_
   c->ptab_in_smem = d_smem_bytes(c->max_nnz, mact, true) <= lim;
   if (d_smem_bytes(c->max_nnz, mact, c->ptab_in_smem) > lim)
     return fail(c, AIMS_ERR_UNSUPPORTED, "nnz(B) too large for the density kernel's shared memory");
+#ifdef AIMS_WITH_VARIANTS
   c->b_ptab_in_smem = b_smem_bytes(c->max_nnz, mact, true) <= lim;
   if (b_smem_bytes(c->max_nnz, mact, c->b_ptab_in_smem) > lim)
     return fail(c, AIMS_ERR_UNSUPPORTED, "nnz(B) too large for the density kernel's shared memory");
+#endif
   c->x_ptab_in_smem = x_smem_bytes(c->max_nnz, mact, true) <= lim;
   c->f_ptab_in_smem = f_smem_bytes(c->max_nnz, mact, true) <= lim;
   if (f_smem_bytes(c->max_nnz, mact, c->f_ptab_in_smem) > lim)
     return fail(c, AIMS_ERR_UNSUPPORTED, "nnz(B) too large for the force kernel's shared memory");
   if (eval_smem_bytes(c->max_nnz) > lim)
     return fail(c, AIMS_ERR_UNSUPPORTED, "nnz(B) too large for the evaluation kernel's shared memory");
+#ifdef AIMS_WITH_VARIANTS
   c->d2_pblk_in_smem = d2_smem_bytes(c->max_nnz, c->max_kq, mact, true) <= lim / 2;      // two CTAs per SM
   if (d2_smem_bytes(c->max_nnz, c->max_kq, mact, c->d2_pblk_in_smem) > lim) c->fast_density = false;
   if (c->fast_density && (rc = dev_alloc(c, &c->Dfull, (size_t)c->full_doubles))) return rc;
   if (c->fast_density) CU_TRY(c, cudaMemsetAsync(c->Dfull, 0, 512 * sizeof(double), c->stream));
+#endif
   CU_TRY(c, cudaStreamSynchronize(c->stream));
   return AIMS_OK;
 }
@@ -808,13 +849,19 @@ int chunk_end(const aims_gpu_ctx *c, const std::vector<long long> &off, int bs, 
 // are the cheapest ones (a CTA's cost varies by 50x over a slab).  Built once per distinct range and kept on the device.
 enum { kItemsAll = 0, kItemsV2 = 1, kItemsBalanced = 2, kItemsGeneric = 3 };
 int density_order(aims_gpu_ctx *c, int bs, int be, const int **out, int which = kItemsAll) {
-  const bool v2 = which == kItemsV2;
+#ifdef AIMS_WITH_VARIANTS
   const std::vector<long long> &ioff = which == kItemsV2 ? c->item2_off : which == kItemsBalanced ? c->itemb_off
                                        : which == kItemsGeneric ? c->itemg_off : c->item_off;
   const std::vector<DItem> &hitems = which == kItemsV2 ? c->h_items2 : which == kItemsBalanced ? c->h_itemsb
                                      : which == kItemsGeneric ? c->h_itemsg : c->h_items;
   std::map<std::pair<int, int>, int *> &cache = which == kItemsV2 ? c->item2_order : which == kItemsBalanced ? c->itemb_order
                                                 : which == kItemsGeneric ? c->itemg_order : c->item_order;
+#else
+  (void)which;
+  const std::vector<long long> &ioff = c->item_off;
+  const std::vector<DItem> &hitems = c->h_items;
+  std::map<std::pair<int, int>, int *> &cache = c->item_order;
+#endif
   const long long i0 = ioff[bs], i1 = ioff[be];
   if (i1 - i0 <= 2ll * c->sm_count) { *out = nullptr; return AIMS_OK; }   // fewer items than two waves: any order
   auto key = std::make_pair(bs, be);
@@ -833,7 +880,9 @@ int density_order(aims_gpu_ctx *c, int bs, int be, const int **out, int which = 
   for (long long i = i0; i < i1; i++) ord[(size_t)(i - i0)] = (int)(i - i0);
   std::stable_sort(ord.begin(), ord.end(), [&](int a, int b) {
     const DItem &x = hitems[(size_t)(i0 + a)], &y = hitems[(size_t)(i0 + b)];
-    if (v2) return c->nnz[x.b] > c->nnz[y.b];       // the items of one batch stay neighbours: they read the same D_b pieces (L2)
+#ifdef AIMS_WITH_VARIANTS
+    if (which == kItemsV2) return c->nnz[x.b] > c->nnz[y.b];       // the items of one batch stay neighbours: they read the same D_b pieces (L2)
+#endif
     const long long cx = (long long)c->nnz[x.b] * c->nnz[x.b] * x.npt, cy = (long long)c->nnz[y.b] * c->nnz[y.b] * y.npt;
     return cx > cy;
   });
@@ -967,6 +1016,7 @@ static int impl_update_density(aims_gpu_ctx *c, int32_t b0, int32_t b1, const do
   int rc = run_cull(c, b0, b1);
   if (rc) return rc;
   const int npl = grad_n ? 4 : 1;
+#ifdef AIMS_WITH_VARIANTS
   if (c->fast_density && b1 > b0) {
     // density2.cuh: D written out in full storage once, then per chunk k_eval<., kLayD2> + k_density2
     ExpandArgs X{D_values, c->Dfull, c->d_offU, c->d_offL, c->d_blk_row, 512};
@@ -1006,6 +1056,7 @@ static int impl_update_density(aims_gpu_ctx *c, int32_t b0, int32_t b1, const do
     }
     return AIMS_OK;
   }
+#endif
   const size_t dsm = d_smem_bytes(c->max_nnz, std::max(c->max_act, 1), c->ptab_in_smem);
   for (int bs = b0; bs < b1;) {
     const int be = chunk_end(c, c->dpad_off, bs, b1, npl);
@@ -1017,13 +1068,18 @@ static int impl_update_density(aims_gpu_ctx *c, int32_t b0, int32_t b1, const do
     E.pad_off = c->d_dpad_off; E.pad_base = c->dpad_off[bs];
     E.n_points = c->n_points;
     if (grad_n) launch_eval<kEvalPhiGrad, kLayD>(c, E, bs, be); else launch_eval<kEvalPhi, kLayD>(c, E, bs, be);
+#ifdef AIMS_WITH_VARIANTS
     // items of 192..224 points (all of a 200-point configuration) -> k_density_b, the others -> k_density
     const long long nib = c->itemb_off[be] - c->itemb_off[bs], nig = c->itemg_off[be] - c->itemg_off[bs];
+#else
+    const long long nig = c->item_off[be] - c->item_off[bs];
+#endif
     DArgs A{};
     A.P = E.plane[0];
     for (int q = 0; q < 3; q++) A.G[q] = grad_n ? E.plane[q + 1] : nullptr;
     A.pad_off = c->d_dpad_off; A.pad_base = c->dpad_off[bs];
     A.D = D_values; A.n = n; A.gn = grad_n; A.n_points = c->n_points; A.max_nnz_pad = c->max_nnz;
+#ifdef AIMS_WITH_VARIANTS
     if (nib > 0) {
       if ((rc = density_order(c, bs, be, &A.order, kItemsBalanced))) return rc;
       A.items = c->d_itemsb + c->itemb_off[bs];
@@ -1033,9 +1089,15 @@ static int impl_update_density(aims_gpu_ctx *c, int32_t b0, int32_t b1, const do
       if (grad_n) k_density_b<true><<<(unsigned)nib, kBThreads, bsm, c->stream>>>(c->S, c->L, A, std::max(c->max_act, 1));
       else k_density_b<false><<<(unsigned)nib, kBThreads, bsm, c->stream>>>(c->S, c->L, A, std::max(c->max_act, 1));
     }
+#endif
     if (nig > 0) {
+#ifdef AIMS_WITH_VARIANTS
       if ((rc = density_order(c, bs, be, &A.order, kItemsGeneric))) return rc;
       A.items = c->d_itemsg + c->itemg_off[bs];
+#else
+      if ((rc = density_order(c, bs, be, &A.order))) return rc;
+      A.items = c->d_items + c->item_off[bs];
+#endif
       A.ptab_in_smem = c->ptab_in_smem ? 1 : 0;
       TimedLaunch t(c, kKindDen);
       if (grad_n) k_density<true><<<(unsigned)nig, kDThreads, dsm, c->stream>>>(c->S, c->L, A, std::max(c->max_act, 1));
@@ -1330,6 +1392,7 @@ static int impl_synchronize(aims_gpu_ctx *c) {
   return AIMS_OK;
 }
 
+#ifdef AIMS_PROBE_DMMA
 static int impl_dmma_probe(aims_gpu_ctx *c, int variant, int warps_per_sm, double *tflops) {
   if (!c || !tflops || variant < 1 || variant > 11 || warps_per_sm < 1 || warps_per_sm > (variant <= 3 ? 16 : 20))
     return fail(c, AIMS_ERR_INVALID_ARG, "variant 1..11, warps_per_sm 1..16 (variants 4..11: 1..20)");
@@ -1369,6 +1432,12 @@ static int impl_dmma_probe(aims_gpu_ctx *c, int variant, int warps_per_sm, doubl
   *tflops = 2.0 * 256 * per_step[variant] * (double)iters * c->sm_count * warps_per_sm / (ms * 1e-3) * 1e-12;
   return check_async(c);
 }
+#else
+static int impl_dmma_probe(aims_gpu_ctx *c, int, int, double *) {
+  return fail(c, AIMS_ERR_UNSUPPORTED, "aims_gpu_dmma_probe: the operand-pattern probes are compiled into probe builds only "
+                                       "(python -m paper_1912_06636_b200.build --define AIMS_PROBE_DMMA=1 --tag dmma)");
+}
+#endif
 
 static int impl_fp64_peak(aims_gpu_ctx *c, double ms_target, double *tflops) {
   if (!c || !tflops) return AIMS_ERR_INVALID_ARG;

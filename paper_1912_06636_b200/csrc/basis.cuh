@@ -128,7 +128,14 @@ __global__ void __launch_bounds__(256) k_cull(DevSys S, BatchLists L, int b_firs
       nfull += S.atom_fn_ptr[a + 1] - S.atom_fn_ptr[a];
     }
     s_nnz = row;
-    if (dry) { L.nnz[b] = row; L.n_act[b] = nact; L.kq[b] = kq; L.nfull[b] = nfull; }
+    if (dry) {
+      L.nnz[b] = row; L.n_act[b] = nact;
+#ifdef AIMS_WITH_VARIANTS
+      L.kq[b] = kq; L.nfull[b] = nfull;                 // density2.cuh only (probe builds)
+#else
+      (void)kq; (void)nfull;
+#endif
+    }
   }
   __syncthreads();
   if (dry) return;
@@ -170,7 +177,9 @@ __global__ void __launch_bounds__(256) k_cull(DevSys S, BatchLists L, int b_firs
       if (cb < B) lo2 = mid + 1; else hi2 = mid - 1;
     }
     L.ptab[po + q] = found;
-    L.pblk[po + q] = (int)fidx;
+#ifdef AIMS_WITH_VARIANTS
+    L.pblk[po + q] = (int)fidx;                         // density2.cuh only (probe builds)
+#endif
   }
 }
 

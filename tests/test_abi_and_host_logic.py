@@ -271,3 +271,14 @@ def test_bench_gpus_2_starts_two_ranks_with_distinct_local_ranks():
         real = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--steps", "1"], env=env, cwd=root,
                               capture_output=True, text=True, timeout=300)
         assert real.returncode != 0 and "refusing" in real.stderr
+
+
+def test_product_library_holds_no_experiment_kernels(lib_path):
+    """The shipped library contains the product only: the measured-and-rejected density variants, the matrix expansion that
+    served one of them and the DMMA operand-pattern probes exist in probe builds (build.py --define ... --tag ...) and nowhere else."""
+    import subprocess
+    out = subprocess.run(["cuobjdump", "-sass", lib_path], capture_output=True, text=True, timeout=600).stdout
+    funcs = [line for line in out.splitlines() if "Function :" in line]
+    assert any("k_density" in f for f in funcs) and any("k_hamiltonian" in f for f in funcs)
+    for name in ("k_density2", "k_density_b", "k_expand_matrix", "k_dmma_probe"):
+        assert not any(name in f for f in funcs), name
